@@ -1,0 +1,378 @@
+"""CPU ORACLE for the k-point ph-AFQMC per-walker step  --  TEST INFRASTRUCTURE ONLY.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` leg may import this file.  It shares no code with the CUDA library
+(`paper_2003_09468_b200/csrc`): no kernels, headers, helpers, tables or pre/post-processing.
+It imports nothing from the product package.
+
+Everything is complex128 (numpy), written for readability against the paper
+(`/root/reference/PAPER.md`, arxiv 2003.09468), not for speed.  Library primitives used as
+steps: ``numpy.matmul`` / ``einsum`` (a matrix product) and ``numpy.linalg.eigh`` (only in the
+exact-exponential reference of level D).  There is no blocking, fusion or reordering beyond
+what the cited definition or algorithm states.
+
+Two levels:
+
+* **Level D (definition)** -- dense supercell objects and explicit 4-index sums:
+  Eq. 20, Eq. 26-30 (:135-146), Eq. 25/37 (:131,:178), Eq. 36 (:171),
+  Eq. 33 (:158) and the Taylor series of :160.  Tiny sizes only.
+* **Level P (production)** -- the k-blocked algorithm the GPU implements and is compared
+  with: Eq. 47 (:220), Eq. 48 (:224), Eq. 49 (:230-236) evaluated by the paper's
+  steps 1-3 (:306-319) literally (both T^1 and T^2 for every (Q,k,k')).
+
+Pins (tests/test_oracle_pins.py): level P == level D on tiny meshes; level D against
+closed forms and invariants (O = 1 and Theta = A^T at Phi = Psi_T; G^2 = G, Tr G = N;
+brute-force cofactor determinant; numpy.linalg.slogdet; exact exponential as dtau -> 0 with
+slope 7/2; anti-Hermitian vHS without force bias; momentum conservation; gauge invariance
+Phi -> Phi R).  No function here is "parity unpinned"; the field-assembly rule
+(`assemble_fields`, reading R7) and the Taylor order (R8) are conventions pinned
+only by level D of this file, as DESIGN.md states.
+
+Layouts (row-major, last index fastest):
+  L[Q][k][gamma][p][r]   p at k-point k, r at k-Q
+  psi_t[k][p][a]         trial, block diagonal in k
+  h1[k][p][q]            one-body Hamiltonian, block diagonal     (Eq. 45)
+  phi[w][M][N]           dense walker, row (k,p), column (k,a)
+  theta[w][N][M]         half-rotated Green's function, Eq. 30
+  vbias[w][Q][gamma], x[w][Q][gamma] (real), vhs[w][M][M], energy[w][3] = (E1, EC, EX)
+"""
+from __future__ import annotations
+
+import numpy as np
+
+C128 = np.complex128
+
+
+# --------------------------------------------------------------------------------------
+# k-point index arithmetic (Gamma-centred regular mesh; index (i1*g2+i2)*g3+i3)
+# --------------------------------------------------------------------------------------
+def k_coords(mesh):
+    g1, g2, g3 = mesh
+    return [(i1, i2, i3) for i1 in range(g1) for i2 in range(g2) for i3 in range(g3)]
+
+
+def k_index(mesh, c):
+    g1, g2, g3 = mesh
+    return ((c[0] % g1) * g2 + (c[1] % g2)) * g3 + (c[2] % g3)
+
+
+def k_sub(mesh, k, Q):
+    """Index of k - Q (k_r = k_p - Q)."""
+    ck, cq = k_coords(mesh)[k], k_coords(mesh)[Q]
+    return k_index(mesh, (ck[0] - cq[0], ck[1] - cq[1], ck[2] - cq[2]))
+
+
+def k_neg(mesh, Q):
+    cq = k_coords(mesh)[Q]
+    return k_index(mesh, (-cq[0], -cq[1], -cq[2]))
+
+
+def k_tables(mesh):
+    nk = mesh[0] * mesh[1] * mesh[2]
+    kminus = np.array([[k_sub(mesh, k, Q) for Q in range(nk)] for k in range(nk)])
+    neg = np.array([k_neg(mesh, Q) for Q in range(nk)])
+    return kminus, neg
+
+
+# --------------------------------------------------------------------------------------
+# LEVEL D : dense supercell definitions
+# --------------------------------------------------------------------------------------
+def supercell_trial(psi_t):
+    """A (M x N), block diagonal in k."""
+    nk, m, n = psi_t.shape
+    A = np.zeros((nk * m, nk * n), dtype=C128)
+    for k in range(nk):
+        A[k * m:(k + 1) * m, k * n:(k + 1) * n] = psi_t[k]
+    return A
+
+
+def supercell_h1(h1):
+    """h (M x M), block diagonal in k (Eq. 45)."""
+    nk, m, _ = h1.shape
+    H = np.zeros((nk * m, nk * m), dtype=C128)
+    for k in range(nk):
+        H[k * m:(k + 1) * m, k * m:(k + 1) * m] = h1[k]
+    return H
+
+
+def supercell_L(mesh, L):
+    """L_sc[P][R][Gamma], Gamma = (Q,gamma); zero unless k_R = k_P - Q."""
+    nk, _, nchol, m, _ = L.shape
+    Lsc = np.zeros((nk * m, nk * m, nk * nchol), dtype=C128)
+    for Q in range(nk):
+        for k in range(nk):
+            kq = k_sub(mesh, k, Q)
+            # L[Q,k] is [gamma][p][r] -> [p][r][gamma]
+            Lsc[k * m:(k + 1) * m, kq * m:(kq + 1) * m, Q * nchol:(Q + 1) * nchol] = \
+                np.transpose(L[Q, k], (1, 2, 0))
+    return Lsc
+
+
+def eri_from_L(Lsc):
+    """v_pqrs = sum_Gamma L_{pr,Gamma} conj(L_{sq,Gamma})   (Eq. 20)."""
+    return np.einsum('prg,sqg->pqrs', Lsc, np.conj(Lsc))
+
+
+def dense_overlap(A, phi):
+    """O = A^dagger Phi  (the matrix inverted in Eq. 27)."""
+    return np.conj(A.T) @ phi
+
+
+def dense_theta(A, phi):
+    """Eq. 30: Theta = (Phi^T A^*)^{-1} Phi^T, via numpy's inverse (level D only)."""
+    return np.linalg.inv(phi.T @ np.conj(A)) @ phi.T
+
+
+def dense_green(A, phi):
+    """Eq. 28-29: G_pr = [A^* Theta]_pr = <c_p^dag c_r>."""
+    return np.conj(A) @ dense_theta(A, phi)
+
+
+def dense_vbias(Lsc, G):
+    """v_Gamma = 2 sum_pr L_{pr,Gamma} G_pr (Eq. 25/37 without the -sqrt(dtau) c_pm prefactor;
+    the 2 is the closed-shell spin sum)."""
+    return 2.0 * np.einsum('prg,pr->g', Lsc, G)
+
+
+def dense_energy(H, V, G):
+    """Eq. 36 for a closed shell (both spins share G):
+    E1 = 2 sum h_pq G_pq;  EC = (1/2) 4 sum v_pqrs G_pr G_qs;  EX = -(1/2) 2 sum v_pqrs G_ps G_qr."""
+    e1 = 2.0 * np.einsum('pq,pq->', H, G)
+    ec = 0.5 * 4.0 * np.einsum('pqrs,pr,qs->', V, G, G)
+    ex = -0.5 * 2.0 * np.einsum('pqrs,ps,qr->', V, G, G)
+    return np.array([e1, ec, ex], dtype=C128)
+
+
+def dense_vhs(Lsc, xi):
+    """vHS_pr = sum_Gamma xi_Gamma L_{pr,Gamma} (the contraction of Eq. 33/48)."""
+    return np.einsum('prg,g->pr', Lsc, xi)
+
+
+def taylor_apply(vhs, phi, dtau, order):
+    """Phi' = sum_{j=0..order} (s V)^j / j!  Phi with s = -sqrt(dtau), by repeated
+    multiplication T_j = (s/j) V T_{j-1} (R7(v), R8)."""
+    s = -np.sqrt(dtau)
+    term = phi.astype(C128).copy()
+    out = term.copy()
+    for j in range(1, order + 1):
+        term = (s / j) * (vhs @ term)
+        out = out + term
+    return out
+
+
+def exact_exp_apply(herm, phi, scale):
+    """exp(scale * herm) Phi for a HERMITIAN matrix `herm` by eigendecomposition."""
+    w, U = np.linalg.eigh(herm)
+    return (U * np.exp(scale * w)) @ (np.conj(U.T) @ phi)
+
+
+# --------------------------------------------------------------------------------------
+# LEVEL P : the k-blocked production algorithm
+# --------------------------------------------------------------------------------------
+def half_rotate(L, psi_t, h1):
+    """a0.  Lh[Q][k][a][gamma][r] = sum_p conj(A_k[p,a]) L[Q][k][gamma][p][r],
+    stored 'transposed' as (a gamma, r) like steps 2(a)/(b) use it;
+    ht[k][a][q] = sum_p conj(A_k[p,a]) h_k[p,q]  (first line of Eq. 49)."""
+    nk, _, nchol, m, _ = L.shape
+    n = psi_t.shape[2]
+    Lh = np.empty((nk, nk, n, nchol, m), dtype=C128)
+    for Q in range(nk):
+        for k in range(nk):
+            Ak = np.conj(psi_t[k])          # [p][a]
+            for g in range(nchol):
+                Lh[Q, k, :, g, :] = Ak.T @ L[Q, k, g]     # [a][r]
+    ht = np.empty((nk, n, m), dtype=C128)
+    for k in range(nk):
+        ht[k] = np.conj(psi_t[k]).T @ h1[k]
+    return Lh, ht
+
+
+def overlap(psi_t, phi_w):
+    """a1.  O = A^dagger Phi assembled as Nk row blocks A_k^dagger Phi[k rows, :]."""
+    nk, m, n = psi_t.shape
+    N = nk * n
+    O = np.empty((N, N), dtype=C128)
+    for k in range(nk):
+        O[k * n:(k + 1) * n, :] = np.conj(psi_t[k]).T @ phi_w[k * m:(k + 1) * m, :]
+    return O
+
+
+def lu_factor(O):
+    """a2.  LU with partial (row) pivoting, column by column (Doolittle, unblocked).
+    Returns (LU packed, perm, sign, info); info = j+1 of the first exactly-zero pivot, else 0."""
+    a = O.astype(C128).copy()
+    nn = a.shape[0]
+    perm = np.arange(nn)
+    sign = 1.0
+    info = 0
+    for j in range(nn):
+        p = j + int(np.argmax(np.abs(a[j:, j])))
+        if a[p, j] == 0:
+            if info == 0:
+                info = j + 1
+            continue
+        if p != j:
+            a[[j, p], :] = a[[p, j], :]
+            perm[[j, p]] = perm[[p, j]]
+            sign = -sign
+        a[j + 1:, j] /= a[j, j]
+        a[j + 1:, j + 1:] -= np.outer(a[j + 1:, j], a[j, j + 1:])
+    return a, perm, sign, info
+
+
+def lu_logdet(lu, sign):
+    """log det O = sum_j log(u_jj) (+ i pi if the permutation is odd): log|det| + i arg det."""
+    d = np.diag(lu)
+    logabs = np.sum(np.log(np.abs(d)))
+    phase = np.sum(np.angle(d)) + (np.pi if sign < 0 else 0.0)
+    phase = (phase + np.pi) % (2 * np.pi) - np.pi
+    return complex(logabs, phase)
+
+
+def lu_inverse(lu, perm):
+    """O^{-1} from the factors: solve L U X = P I by forward then back substitution."""
+    nn = lu.shape[0]
+    X = np.eye(nn, dtype=C128)[perm, :]
+    for j in range(nn):                     # L y = P I   (unit lower)
+        X[j + 1:, :] -= np.outer(lu[j + 1:, j], X[j, :])
+    for j in range(nn - 1, -1, -1):         # U x = y
+        X[j, :] /= lu[j, j]
+        X[:j, :] -= np.outer(lu[:j, j], X[j, :])
+    return X
+
+
+def green(psi_t, phi_w):
+    """a1-a3 for one walker: returns (Theta [N][M], logdet, info).
+    Theta = (Phi^T A^*)^{-1} Phi^T = (Phi O^{-1})^T, Eq. 30."""
+    O = overlap(psi_t, phi_w)
+    lu, perm, sign, info = lu_factor(O)
+    if info != 0:
+        return np.full((O.shape[0], phi_w.shape[0]), np.nan, dtype=C128), complex(np.nan, np.nan), info
+    Oinv = lu_inverse(lu, perm)
+    theta = (phi_w @ Oinv).T
+    return np.ascontiguousarray(theta), lu_logdet(lu, sign), 0
+
+
+def force_bias(mesh, Lh, theta_w):
+    """a4.  vbias[Q][gamma] = 2 sum_k sum_{a,r} Lh[Q][k][a][gamma][r] Theta[(k,a),(k-Q,r)]
+    (the half-rotated contraction at the core of Eq. 47, = 2 X_gamma of Eq. 37)."""
+    nk, _, n, nchol, m = Lh.shape
+    vb = np.zeros((nk, nchol), dtype=C128)
+    for Q in range(nk):
+        for k in range(nk):
+            kq = k_sub(mesh, k, Q)
+            blk = theta_w[k * n:(k + 1) * n, kq * m:(kq + 1) * m]     # [a][r]
+            vb[Q] += 2.0 * np.einsum('agr,ar->g', Lh[Q, k], blk)
+    return vb
+
+
+def assemble_fields(mesh, x_w, vbias_w, dtau):
+    """Field assembly, reading R7 (the paper's Eq. 8/17/24/47/48 are mutually
+    inconsistent in signs and factors of i):
+      (i)   one real field x[Q][gamma] per (Q,gamma);
+      (ii)  z_Q = x_Q if -Q == Q; for idx(Q) < idx(-Q): z_Q = (x_Q + i x_{-Q})/sqrt2,
+            z_{-Q} = conj(z_Q);
+      (iii) zbar_{Q,gamma} = -i sqrt(dtau) vbias_{-Q,gamma}   (Eq. 17 in this basis; 0 if no vbias);
+      (iv)  xi = -i (z - zbar).
+    """
+    nk = x_w.shape[0]
+    z = np.zeros(x_w.shape, dtype=C128)
+    for Q in range(nk):
+        mq = k_neg(mesh, Q)
+        if mq == Q:
+            z[Q] = x_w[Q]
+        elif Q < mq:
+            z[Q] = (x_w[Q] + 1j * x_w[mq]) / np.sqrt(2.0)
+            z[mq] = np.conj(z[Q])
+    zbar = np.zeros_like(z)
+    if vbias_w is not None:
+        for Q in range(nk):
+            zbar[Q] = -1j * np.sqrt(dtau) * vbias_w[k_neg(mesh, Q)]
+    return -1j * (z - zbar)
+
+
+def vhs(mesh, L, xi_w):
+    """a5.  V[(k,p),(k-Q,r)] = sum_gamma L[Q][k][gamma][p][r] xi[Q][gamma]   (Eq. 48);
+    each (k,k') block of the M x M matrix receives exactly one Q = k - k'."""
+    nk, _, nchol, m, _ = L.shape
+    V = np.zeros((nk * m, nk * m), dtype=C128)
+    for Q in range(nk):
+        for k in range(nk):
+            kq = k_sub(mesh, k, Q)
+            V[k * m:(k + 1) * m, kq * m:(kq + 1) * m] += np.einsum('gpr,g->pr', L[Q, k], xi_w[Q])
+    return V
+
+
+def propagate(vhs_w, phi_w, dtau, order):
+    """a6.  Same recurrence as level D."""
+    return taylor_apply(vhs_w, phi_w, dtau, order)
+
+
+def reshape_theta(theta_w, nk, n, m):
+    """Step 1: G[(k1 a),(k2 q)] -> G[k1][k2][a][q]."""
+    return np.ascontiguousarray(theta_w.reshape(nk, n, nk, m).transpose(0, 2, 1, 3))
+
+
+def local_energy(mesh, Lh, ht, theta_w):
+    """a7-a9 for one walker, by the paper's steps 1-3, closed shell.
+
+    Returns (E1, EC, EX).  Spin factors: E1 x2; the traces v_j carry x2 each so EC = (1/2) v1 v2
+    has x4 (sigma, sigma' independent); EX x2 (delta_{sigma sigma'} in Eq. 49)."""
+    nk, _, n, nchol, m = Lh.shape
+    G = reshape_theta(theta_w, nk, n, m)                    # step 1
+    e1 = 0.0 + 0.0j
+    for k in range(nk):                                     # Eq. 49 line 1
+        e1 += 2.0 * np.sum(ht[k] * G[k, k])
+    ex = 0.0 + 0.0j
+    ec = 0.0 + 0.0j
+    for Q in range(nk):
+        mQ = k_neg(mesh, Q)
+        v1 = np.zeros(nchol, dtype=C128)
+        v2 = np.zeros(nchol, dtype=C128)
+        for k in range(nk):
+            kq = k_sub(mesh, k, Q)
+            for kp in range(nk):
+                kpq = k_sub(mesh, kp, Q)
+                # 2(a): T1[b,a,g] = sum_r Lh[Q,k][a,g,r] G[k'-Q, k-Q][b,r]
+                T1 = np.einsum('agr,br->bag', Lh[Q, k], G[kpq, kq])
+                # 2(b): T2[a,b,g] = sum_s Lh[-Q,k'-Q][b,g,s] G[k, k'][a,s]
+                T2 = np.einsum('bgs,as->abg', Lh[mQ, kpq], G[k, kp])
+                # 2(c)
+                ex += -0.5 * 2.0 * np.einsum('bag,abg->', T1, T2)
+                # 2(d): the trace is a density only when k'-Q == k
+                if kpq == k:
+                    v1 += 2.0 * np.einsum('aag->g', T1)
+                    v2 += 2.0 * np.einsum('aag->g', T2)
+        ec += 0.5 * np.sum(v1 * v2)                         # step 3, summed over Q
+    return np.array([e1, ec, ex], dtype=C128)
+
+
+def coulomb_from_vbias(mesh, vbias_w):
+    """EC = (1/2) sum_Q sum_gamma vbias[Q] vbias[-Q]  (bilinear; Eq. 41)."""
+    nk = vbias_w.shape[0]
+    ec = 0.0 + 0.0j
+    for Q in range(nk):
+        ec += 0.5 * np.sum(vbias_w[Q] * vbias_w[k_neg(mesh, Q)])
+    return ec
+
+
+# --------------------------------------------------------------------------------------
+# One full step for a batch (the composition bench.py times)
+# --------------------------------------------------------------------------------------
+def step(mesh, L, Lh, ht, psi_t, phi, x, dtau, order):
+    """overlap+green, force bias, vHS, propagate on Phi; then overlap+green+local energy on Phi'.
+    Returns (phi_new [nw][M][N], energy [nw][3], logdet_new [nw])."""
+    nw = phi.shape[0]
+    phi_new = np.empty_like(phi)
+    energy = np.empty((nw, 3), dtype=C128)
+    logdet = np.empty(nw, dtype=C128)
+    for w in range(nw):
+        th, _, _ = green(psi_t, phi[w])
+        vb = force_bias(mesh, Lh, th)
+        xi = assemble_fields(mesh, x[w], vb, dtau)
+        V = vhs(mesh, L, xi)
+        phi_new[w] = propagate(V, phi[w], dtau, order)
+        th2, ld, _ = green(psi_t, phi_new[w])
+        energy[w] = local_energy(mesh, Lh, ht, th2)
+        logdet[w] = ld
+    return phi_new, energy, logdet
