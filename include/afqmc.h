@@ -1,0 +1,173 @@
+/*
+ * afqmc.h -- C ABI of libafqmc: the batched per-walker step of k-point phaseless AFQMC
+ * (Malone, Zhang, Morales, arxiv 2003.09468; citations are /root/reference/PAPER.md:<line>).
+ *
+ * All step calls work on a batch of `nw` walkers at once ("all walkers should be operated on
+ * simultaneously") and are ASYNCHRONOUS on the cudaStream_t passed as `stream`.
+ *
+ * Conventions
+ *   Nk = g[0]*g[1]*g[2] k-points = number of Q vectors; k-point linear index
+ *   (i1*g[1] + i2)*g[2] + i3 on a Gamma-centred regular mesh; k-Q and -Q are
+ *   taken componentwise modulo the mesh.  M = Nk*m basis functions, N = Nk*n electrons per
+ *   spin.  Closed shell: one walker matrix serves both spins.
+ *
+ *   Every array is row-major (last index fastest), complex numbers interleaved (re, im),
+ *   double precision (complex128).  "device" = device memory owned by the caller (e.g. a
+ *   torch tensor); the library borrows the pointer for the duration of the enqueued work and
+ *   never frees it.  Workspace is owned by the context and sized from max_walkers at create.
+ *
+ *   phi   [nw][M][N]      walker U, DENSE; row (k,p) = k*m+p, column (k,a) = k*n+a
+ *   theta [nw][N][M]      half-rotated Green's function, Eq. 30 = the paper's
+ *                         G[n,k1,a,k2,q] of PAPER.md:306-312
+ *   vbias [nw][Nk][nchol] complex; x [nw][Nk][nchol] real; vhs [nw][M][M];
+ *   energy[nw][3]         complex (E1, EC, EX);  logdet[nw] complex = log|det O| + i arg det O of
+ *                         ONE spin channel, arg in (-pi, pi];  info[nw] int32.
+ *
+ * Errors: every call returns an int; 0 = AFQMC_OK.  No exceptions cross the ABI, there is no
+ * global state.  A singular overlap cannot be a return code of an asynchronous call: it is
+ * reported LAPACK-style in the device array info[w] (0 ok, j>0 = exactly-zero pivot at
+ * elimination step j); theta/logdet of such a walker are undefined.
+ * One context must not be used from two streams at the same time (it owns workspace).
+ */
+#ifndef AFQMC_H
+#define AFQMC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct afqmc_ctx afqmc_ctx; /* opaque, library-owned */
+
+typedef struct {
+    int g[3];         /* k-point mesh                                              */
+    int m;            /* bands per k-point                                          */
+    int n;            /* occupied orbitals per k-point per spin                      */
+    int nchol;        /* Cholesky vectors per Q             */
+    int closed_shell; /* must be 1 (else AFQMC_UNSUPPORTED)                          */
+    int precision;    /* 0 = complex128 (only value supported so far)               */
+    int max_walkers;  /* workspace is sized for this many walkers                    */
+} afqmc_dims;
+
+enum {
+    AFQMC_OK = 0,
+    AFQMC_INVALID_ARGUMENT = 1, /* null pointer, nw < 0 or > max_walkers, bad dims, bad order */
+    AFQMC_UNSUPPORTED = 2,      /* open shell, precision != 0                                 */
+    AFQMC_CUDA_ERROR = 3,       /* a CUDA runtime call or launch failed                       */
+    AFQMC_OUT_OF_MEMORY = 4     /* device allocation failed                                   */
+};
+
+/* Text for an error code (static storage, never NULL). */
+const char* afqmc_strerror(int code);
+
+/*
+ * a0 (setup, once per simulation).  Validates dims, copies the trial,
+ * half-rotates  Lh[Q][k][a][g][r] = sum_p conj(psi_t[k][p][a]) L[Q][k][g][p][r]  and
+ * ht[k][a][q] = sum_p conj(psi_t[k][p][a]) h1[k][p][q], repacks L and Lh into the library's
+ * internal tensor-core fragment layouts and allocates workspace.  Synchronises `stream` before
+ * returning, so the caller may free h1, L and psi_t afterwards.
+ *   h1    [Nk][m][m]            device, complex128, Hermitian blocks (Eq. 45)
+ *   L     [Nk][Nk][nchol][m][m] device, complex128: L[Q][k][g][p][r], p at k, r at k-Q.
+ *         The (Q,-Q) identity L[-Q][k-Q][g][r][p] = conj(L[Q][k][g][p][r]) is ASSUMED
+ *         by afqmc_local_energy (it is what lets Lbar of Eq. 40 be read from Lh); it is not checked.
+ *   psi_t [Nk][m][n]            device, complex128 (trial block-diagonal in k)
+ */
+int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* h1, const void* L,
+                 const void* psi_t, void* stream);
+
+/* Frees everything the context owns.  NULL is allowed. */
+void afqmc_destroy(afqmc_ctx* ctx);
+
+/*
+ * a1+a2.  O_w = A^dagger Phi_w (N x N, assembled as Nk row blocks because the trial is block
+ * diagonal, PAPER.md:142 Eq. 27-28, :226) and its elimination with partial pivoting:
+ * logdet[w] = log det O_w, info[w].   phi, logdet, info: device.
+ */
+int afqmc_overlap(afqmc_ctx* ctx, const void* phi, int nw, void* logdet, int* info, void* stream);
+
+/*
+ * a1+a2+a3.  Additionally theta_w = (Phi_w^T A^*)^{-1} Phi_w^T = (Phi_w O_w^{-1})^T, Eq. 30
+ * (PAPER.md:146).  logdet and info may be NULL.   phi, theta, logdet, info: device.
+ */
+int afqmc_green(afqmc_ctx* ctx, const void* phi, int nw, void* theta, void* logdet, int* info,
+                void* stream);
+
+/*
+ * a4.  vbias[w][Q][g] = 2 sum_k sum_{a,r} Lh[Q][k][a][g][r] theta_w[(k,a),(k-Q,r)]
+ * = <Psi_T| rho_{Q g} |phi_w> / <Psi_T|phi_w> summed over both spins: the half-rotated contraction
+ * of Eq. 47 = 2 X_g of Eq. 37, WITHOUT the -sqrt(dtau) c_pm prefactor
+ * of Eq. 25 (that belongs to the field assembly in afqmc_vhs).   theta, vbias: device.
+ */
+int afqmc_force_bias(afqmc_ctx* ctx, const void* theta, int nw, void* vbias, void* stream);
+
+/*
+ * a5.  Field assembly then the contraction of Eq. 48 (PAPER.md:224; Eq. 33, :158):
+ *   z_Q = x_Q if -Q == Q, else z_Q = (x_Q + i x_{-Q})/sqrt2 for idx(Q) < idx(-Q), z_{-Q} = conj(z_Q);
+ *   zbar_{Q g} = -i sqrt(dtau) vbias[w][-Q][g]   (Eq. 17; zero if vbias == NULL);
+ *   xi = -i (z - zbar);   vhs_w[(k,p),(k-Q,r)] = sum_g L[Q][k][g][p][r] xi_{Q g}.
+ * Every (k,k') block of vhs_w is written exactly once (Q = k - k').  The propagator applied by
+ * afqmc_propagate is then exp(-sqrt(dtau) vhs) = exp(i sqrt(dtau) sum z rho - dtau sum vbias_{-Q} rho_Q)
+ * (reading R7).    x: device double [nw][Nk][nchol]; vbias: device or NULL; vhs: device.
+ */
+int afqmc_vhs(afqmc_ctx* ctx, const double* x, const void* vbias, double dtau, int nw, void* vhs,
+              void* stream);
+
+/*
+ * a6.  phi_w <- sum_{j=0..order} (s vhs_w)^j / j!  phi_w,  s = -sqrt(dtau), by the recurrence
+ * T_0 = phi, T_j = (s/j) vhs T_{j-1} (truncated Taylor series of PAPER.md:160).  In place.
+ * 0 <= order <= 32.    vhs, phi: device.
+ */
+int afqmc_propagate(afqmc_ctx* ctx, const void* vhs, double dtau, int order, void* phi, int nw,
+                    void* stream);
+
+/*
+ * a7+a8+a9.  Local energy of Eq. 49 by the recipe of PAPER.md:306-319:
+ *   energy[w][0] = E1 = 2 sum_k sum_{a,q} ht[k][a][q] theta_w[(k,a),(k,q)]
+ *   energy[w][1] = EC = 1/2 sum_Q sum_g v_{Q g} v_{-Q g},  v = the force bias of theta_w (steps 2d, 3)
+ *   energy[w][2] = EX = - sum_{Q,k,k'} sum_{a,b,g} T1[b,a,g] T2[a,b,g]                (steps 2a-2c)
+ *       T1[b,a,g] = sum_r Lh[Q][k][a][g][r]     theta_w[(k'-Q,b),(k-Q,r)]
+ *       T2[a,b,g] = sum_s Lh[-Q][k'-Q][b][g][s] theta_w[(k,a),(k',s)]
+ * Closed-shell spin factors (2, 4, 2) are included.   theta, energy: device.
+ */
+int afqmc_local_energy(afqmc_ctx* ctx, const void* theta, int nw, void* energy, void* stream);
+
+/*
+ * One whole step on DEVICE buffers, the composition bench.py times:
+ * green(phi) -> force_bias -> vhs(x, vbias, dtau) -> propagate(order) [phi updated in place]
+ * -> green(phi') -> local_energy.  energy [nw][3], logdet [nw] (of phi'), info [nw]: device;
+ * logdet/info may be NULL.
+ */
+int afqmc_step(afqmc_ctx* ctx, void* phi, const double* x, double dtau, int order, int nw,
+               void* energy, void* logdet, int* info, void* stream);
+
+/*
+ * The same step on HOST buffers: copies phi and x to the device, runs afqmc_step, copies phi',
+ * energy (and logdet, info if not NULL) back and synchronises `stream` before returning.
+ * Host buffers should be pinned for full copy bandwidth; pageable memory also works.
+ */
+int afqmc_step_host(afqmc_ctx* ctx, void* phi_host, const double* x_host, double dtau, int order,
+                    int nw, void* energy_host, void* logdet_host, int* info_host, void* stream);
+
+/* Number of kernels the context has launched so far (for bench.py's gpu_launches). */
+long long afqmc_launch_count(const afqmc_ctx* ctx);
+
+/* Executed real flops of the exchange contraction (a9) of ONE afqmc_local_energy call on nw
+ * walkers, as the kernel executes it (pairs (Q,k,k') ~ (-Q,k'-Q,k-Q) computed once). */
+double afqmc_exchange_flops(const afqmc_ctx* ctx, int nw);
+
+/* Selects the exchange-kernel variant: 0 = default (best), 1 = simple direct-load variant. */
+int afqmc_set_option(afqmc_ctx* ctx, const char* name, int value);
+
+/*
+ * FP64 peak probes (measurement aid, no AFQMC arithmetic): runs a register-resident loop of
+ * kind 0 = DFMA (fma.rn.f64), 1 = DMMA (mma.sync.m8n8k4.f64) on every SM for `iters` iterations and
+ * returns the achieved TFLOP/s in *tflops (host).  Synchronous.
+ */
+int afqmc_probe_fp64(int kind, int iters, double* tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AFQMC_H */

@@ -1,0 +1,224 @@
+"""Thin ctypes binding of libafqmc (include/afqmc.h): argument marshalling only.
+
+Every step of the path runs inside the library's CUDA kernels; PyTorch is used for device
+memory (torch tensors own every buffer) and for the current CUDA stream.  There is no CPU
+fallback: if the library is missing or a call fails, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libafqmc.so")
+_lib = None
+
+ERRORS = {0: "ok", 1: "invalid argument", 2: "unsupported configuration", 3: "CUDA error", 4: "out of device memory"}
+
+
+class AfqmcError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        super().__init__("%s failed: %s (code %d)" % (where, ERRORS.get(code, "?"), code))
+
+
+class Dims(ctypes.Structure):
+    _fields_ = [("g", ctypes.c_int * 3), ("m", ctypes.c_int), ("n", ctypes.c_int), ("nchol", ctypes.c_int),
+                ("closed_shell", ctypes.c_int), ("precision", ctypes.c_int), ("max_walkers", ctypes.c_int)]
+
+
+EXPORTS = ["afqmc_strerror", "afqmc_create", "afqmc_destroy", "afqmc_overlap", "afqmc_green", "afqmc_force_bias",
+           "afqmc_vhs", "afqmc_propagate", "afqmc_local_energy", "afqmc_step", "afqmc_step_host",
+           "afqmc_launch_count", "afqmc_exchange_flops", "afqmc_set_option", "afqmc_probe_fp64"]
+
+
+def lib():
+    """Loads libafqmc.so (built in-tree by `paper_2003_09468_b200.build`); raises if it is absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError("libafqmc.so not found at %s: run `python -m paper_2003_09468_b200.build` "
+                           "(there is no CPU fallback)" % LIB_PATH)
+    L = ctypes.CDLL(LIB_PATH)
+    vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+    L.afqmc_strerror.restype = ctypes.c_char_p
+    L.afqmc_strerror.argtypes = [ci]
+    L.afqmc_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(Dims), vp, vp, vp, vp]
+    L.afqmc_destroy.argtypes = [vp]
+    L.afqmc_destroy.restype = None
+    L.afqmc_overlap.argtypes = [vp, vp, ci, vp, vp, vp]
+    L.afqmc_green.argtypes = [vp, vp, ci, vp, vp, vp, vp]
+    L.afqmc_force_bias.argtypes = [vp, vp, ci, vp, vp]
+    L.afqmc_vhs.argtypes = [vp, vp, vp, cd, ci, vp, vp]
+    L.afqmc_propagate.argtypes = [vp, vp, cd, ci, vp, ci, vp]
+    L.afqmc_local_energy.argtypes = [vp, vp, ci, vp, vp]
+    L.afqmc_step.argtypes = [vp, vp, vp, cd, ci, ci, vp, vp, vp, vp]
+    L.afqmc_step_host.argtypes = [vp, vp, vp, cd, ci, ci, vp, vp, vp, vp]
+    L.afqmc_launch_count.argtypes = [vp]
+    L.afqmc_launch_count.restype = ctypes.c_longlong
+    L.afqmc_exchange_flops.argtypes = [vp, ci]
+    L.afqmc_exchange_flops.restype = cd
+    L.afqmc_set_option.argtypes = [vp, ctypes.c_char_p, ci]
+    L.afqmc_probe_fp64.argtypes = [ci, ci, ctypes.POINTER(cd)]
+    for name in EXPORTS:
+        if name not in ("afqmc_strerror", "afqmc_destroy", "afqmc_launch_count", "afqmc_exchange_flops"):
+            getattr(L, name).restype = ci
+    _lib = L
+    return L
+
+
+def _stream():
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t, dtype=None, optional=False):
+    if t is None:
+        if optional:
+            return ctypes.c_void_p(0)
+        raise ValueError("required tensor is None")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError("expected %s, got %s" % (dtype, t.dtype))
+    if not t.is_contiguous():
+        raise ValueError("tensor must be contiguous")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _check(code, where):
+    if code != 0:
+        raise AfqmcError(code, where)
+
+
+def probe_fp64(kind: int, iters: int = 20000) -> float:
+    out = ctypes.c_double(0.0)
+    _check(lib().afqmc_probe_fp64(kind, iters, ctypes.byref(out)), "afqmc_probe_fp64")
+    return out.value
+
+
+class Afqmc:
+    """Context of one Hamiltonian + trial on the current CUDA device (afqmc_create / afqmc_destroy)."""
+
+    def __init__(self, mesh, m, n, nchol, h1, L, psi_t, max_walkers, closed_shell=1, precision=0):
+        self._h = ctypes.c_void_p(0)
+        self.mesh = tuple(int(v) for v in mesh)
+        self.nk = self.mesh[0] * self.mesh[1] * self.mesh[2]
+        self.m, self.n, self.nchol = int(m), int(n), int(nchol)
+        self.M, self.N = self.nk * self.m, self.nk * self.n
+        self.max_walkers = int(max_walkers)
+        d = Dims((ctypes.c_int * 3)(*self.mesh), self.m, self.n, self.nchol, closed_shell, precision, self.max_walkers)
+        for name, t, shape in (("h1", h1, (self.nk, self.m, self.m)),
+                               ("L", L, (self.nk, self.nk, self.nchol, self.m, self.m)),
+                               ("psi_t", psi_t, (self.nk, self.m, self.n))):
+            if not t.is_cuda or tuple(t.shape) != shape:
+                raise ValueError("%s must be a CUDA tensor of shape %s" % (name, shape))
+        self.device = h1.device
+        h = ctypes.c_void_p(0)
+        code = lib().afqmc_create(ctypes.byref(h), ctypes.byref(d), _ptr(h1, torch.complex128),
+                                  _ptr(L, torch.complex128), _ptr(psi_t, torch.complex128), _stream())
+        _check(code, "afqmc_create")
+        self._h = h
+
+    def close(self):
+        if self._h:
+            lib().afqmc_destroy(self._h)
+            self._h = ctypes.c_void_p(0)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- helpers -------------------------------------------------------------------------
+    def _empty(self, shape, dtype=torch.complex128):
+        return torch.empty(shape, dtype=dtype, device=self.device)
+
+    def launch_count(self) -> int:
+        return int(lib().afqmc_launch_count(self._h))
+
+    def exchange_flops(self, nw) -> float:
+        return float(lib().afqmc_exchange_flops(self._h, int(nw)))
+
+    def set_option(self, name: str, value: int):
+        _check(lib().afqmc_set_option(self._h, name.encode(), int(value)), "afqmc_set_option")
+
+    # ---- the six step calls ----------------------------------------------------------------
+    def overlap(self, phi, logdet=None, info=None):
+        nw = phi.shape[0]
+        logdet = self._empty((nw,)) if logdet is None else logdet
+        info = self._empty((nw,), torch.int32) if info is None else info
+        _check(lib().afqmc_overlap(self._h, _ptr(phi, torch.complex128), nw, _ptr(logdet), _ptr(info, torch.int32),
+                                   _stream()), "afqmc_overlap")
+        return logdet, info
+
+    def green(self, phi, theta=None, logdet=None, info=None):
+        nw = phi.shape[0]
+        theta = self._empty((nw, self.N, self.M)) if theta is None else theta
+        logdet = self._empty((nw,)) if logdet is None else logdet
+        info = self._empty((nw,), torch.int32) if info is None else info
+        _check(lib().afqmc_green(self._h, _ptr(phi, torch.complex128), nw, _ptr(theta, torch.complex128),
+                                 _ptr(logdet), _ptr(info, torch.int32), _stream()), "afqmc_green")
+        return theta, logdet, info
+
+    def force_bias(self, theta, vbias=None):
+        nw = theta.shape[0]
+        vbias = self._empty((nw, self.nk, self.nchol)) if vbias is None else vbias
+        _check(lib().afqmc_force_bias(self._h, _ptr(theta, torch.complex128), nw, _ptr(vbias, torch.complex128),
+                                      _stream()), "afqmc_force_bias")
+        return vbias
+
+    def vhs(self, x, vbias, dtau, vhs=None):
+        nw = x.shape[0]
+        vhs = self._empty((nw, self.M, self.M)) if vhs is None else vhs
+        _check(lib().afqmc_vhs(self._h, _ptr(x, torch.float64), _ptr(vbias, torch.complex128, optional=True),
+                               float(dtau), nw, _ptr(vhs, torch.complex128), _stream()), "afqmc_vhs")
+        return vhs
+
+    def propagate(self, vhs, dtau, order, phi):
+        nw = phi.shape[0]
+        _check(lib().afqmc_propagate(self._h, _ptr(vhs, torch.complex128), float(dtau), int(order),
+                                     _ptr(phi, torch.complex128), nw, _stream()), "afqmc_propagate")
+        return phi
+
+    def local_energy(self, theta, energy=None):
+        nw = theta.shape[0]
+        energy = self._empty((nw, 3)) if energy is None else energy
+        _check(lib().afqmc_local_energy(self._h, _ptr(theta, torch.complex128), nw, _ptr(energy, torch.complex128),
+                                        _stream()), "afqmc_local_energy")
+        return energy
+
+    # ---- the whole step ------------------------------------------------------------------------
+    def step(self, phi, x, dtau, order, energy=None, logdet=None, info=None):
+        nw = phi.shape[0]
+        energy = self._empty((nw, 3)) if energy is None else energy
+        logdet = self._empty((nw,)) if logdet is None else logdet
+        info = self._empty((nw,), torch.int32) if info is None else info
+        _check(lib().afqmc_step(self._h, _ptr(phi, torch.complex128), _ptr(x, torch.float64), float(dtau), int(order),
+                                nw, _ptr(energy), _ptr(logdet), _ptr(info, torch.int32), _stream()), "afqmc_step")
+        return energy, logdet, info
+
+    def step_host(self, phi_host, x_host, dtau, order, energy_host, logdet_host=None, info_host=None):
+        """Host (ideally pinned) tensors in and out; H2D/D2H copies happen inside the call."""
+        nw = phi_host.shape[0]
+        for t in (phi_host, x_host, energy_host):
+            if t.is_cuda:
+                raise ValueError("step_host takes host tensors")
+        _check(lib().afqmc_step_host(self._h, _ptr(phi_host, torch.complex128), _ptr(x_host, torch.float64),
+                                     float(dtau), int(order), nw, _ptr(energy_host, torch.complex128),
+                                     _ptr(logdet_host, optional=True), _ptr(info_host, optional=True), _stream()),
+               "afqmc_step_host")
+        return energy_host
+
+
+def from_problem(pb, max_walkers=None, device="cuda"):
+    """Builds a context from a `synth.Problem` (host numpy arrays -> device tensors)."""
+    cfg = pb.cfg
+    dev = torch.device(device)
+    h1 = torch.from_numpy(pb.h1).to(dev)
+    L = torch.from_numpy(pb.L).to(dev)
+    psi_t = torch.from_numpy(pb.psi_t).to(dev)
+    ctx = Afqmc(cfg.mesh, cfg.m, cfg.n, cfg.nchol, h1, L, psi_t, max_walkers or pb.phi.shape[0])
+    del L
+    return ctx

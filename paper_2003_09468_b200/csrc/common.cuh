@@ -1,0 +1,129 @@
+// Internal declarations shared by the translation units of libafqmc (not part of the ABI).
+// Hardware target: sm_100a (B200).  FP64 tensor-core op used throughout: mma.sync m8n8k4 f64
+// (SASS DMMA.8x8x4); tcgen05 has no f64 kind, so TMEM/UMMA do not apply to this path.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/afqmc.h"
+
+#define AFQMC_MAX_NK 512
+// exported C-ABI entry points (everything else in the library has hidden visibility)
+#define AFQMC_API extern "C" __attribute__((visibility("default")))
+
+// ----------------------------------------------------------------------------------------
+// Dimensions and derived sizes (host + device POD)
+// ----------------------------------------------------------------------------------------
+struct Dims {
+    int g[3];
+    int Nk, m, n, nchol;
+    int M, N;      // Nk*m, Nk*n
+    int KS;        // k-steps (of 4 reals) covering one complex row of length m: ceil(2m/4)
+    int NAG;       // groups of 4 occupied orbitals: ceil(n/4)
+    int GP;        // pairs of Cholesky vectors: ceil(nchol/2)   (exchange M-tiles; also vHS k-steps)
+    int GT;        // octets of Cholesky vectors: ceil(nchol/8)  (force-bias M-tiles)
+    int PRT;       // octets of (p,r) pairs: ceil(m*m/8)         (vHS M-tiles)
+};
+
+// The context.  All pointers are device memory owned by the context.
+struct afqmc_ctx {
+    Dims d;
+    int max_walkers;
+    // static tables
+    int* kminus;   // [Nk(k)][Nk(Q)] -> index of k-Q
+    int* kplus;    // [Nk(k)][Nk(Q)] -> index of k+Q
+    int* kneg;     // [Nk]           -> index of -Q
+    int* units;    // exchange work units, int4-packed (Q,k,k2,mult) [nunits]
+    int nunits;
+    // static tensors
+    double2* psi_t; // [Nk][m][n]
+    double2* ht;    // [Nk][n][m]   half-rotated one-body
+    double* Lx;     // exchange fragment layout  [Q][k][ag][gp][s][lane]
+    double* Lf;     // force-bias fragment layout [Q][gt][k][a][s][lane]
+    double* Lv;     // vHS fragment layout        [Q][k][prt][s][lane]
+    // workspace (sized by max_walkers)
+    double2* ws_O;      // [nw][N][LD]  elimination workspace when the matrix does not fit shared memory
+    double2* ws_oinvT;  // [nw][N][N]   transposed inverse overlap
+    double2* ws_theta;  // [nw][N][M]
+    double2* ws_vbias;  // [nw][Nk][nchol]
+    double2* ws_xi;     // [nw][Nk][nchol]
+    double2* ws_vhs;    // [nw][M][M]
+    double2* ws_T;      // [2][nw][M][N] Taylor ping-pong
+    double2* ws_expart; // [nunits][nw]  exchange partial sums
+    double* ws_x;       // [nw][Nk][nchol] (host-entry staging)
+    double2* ws_phi;    // [nw][M][N]     (host-entry staging)
+    double2* ws_energy; // [nw][3]
+    double2* ws_logdet; // [nw]
+    int* ws_info;       // [nw]
+    long long launches;
+    int opt_exchange;   // 0 default, 1 simple
+    int smem_optin;     // max dynamic shared memory per block (bytes)
+    int num_sms;
+};
+
+// ----------------------------------------------------------------------------------------
+// Device helpers
+// ----------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+
+// D(8x8) += A(8x4, row) * B(4x8, col), FP64.  Fragments (lane l):
+//   a = A[l>>2][l&3];  b = B[l&3][l>>2];  c0,c1 = C[l>>2][2*(l&3) + {0,1}]
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+// Real embedding of a complex GEMM  C = A*B  (8 real flops per complex multiply-add, exact):
+//   A row -> [Re a_0, Im a_0, Re a_1, Im a_1, ...]            (interleaved storage as is)
+//   B     -> for the real-part output column (d=0):  [Re b_k, -Im b_k];  for d=1: [Im b_k, Re b_k]
+// A B-fragment lane with K parity c (0: multiplies Re a, 1: multiplies Im a) and output part d
+// therefore reads component (c^d) of b and flips its sign iff (c==1 && d==0).
+__device__ __forceinline__ double flip_sign(double v, unsigned mask) {
+    return __hiloint2double(__double2hiint(v) ^ (int)mask, __double2loint(v));
+}
+
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) {
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ double2 cfma(double2 a, double2 b, double2 c) {  // a*b + c
+    c.x = fma(a.x, b.x, c.x); c.x = fma(-a.y, b.y, c.x);
+    c.y = fma(a.x, b.y, c.y); c.y = fma(a.y, b.x, c.y);
+    return c;
+}
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+#endif  // __CUDACC__
+
+// ----------------------------------------------------------------------------------------
+// Host-side helpers
+// ----------------------------------------------------------------------------------------
+#define AFQMC_CUDA_TRY(expr)                           \
+    do {                                               \
+        cudaError_t e__ = (expr);                      \
+        if (e__ != cudaSuccess) {                      \
+            (void)cudaGetLastError();                  \
+            return (e__ == cudaErrorMemoryAllocation) ? AFQMC_OUT_OF_MEMORY : AFQMC_CUDA_ERROR; \
+        }                                              \
+    } while (0)
+
+#define AFQMC_LAUNCH_CHECK(ctx)                        \
+    do {                                               \
+        (ctx)->launches++;                             \
+        cudaError_t e__ = cudaGetLastError();          \
+        if (e__ != cudaSuccess) return AFQMC_CUDA_ERROR; \
+    } while (0)
+
+static inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+// internal entry points used across translation units (all asynchronous on `st`)
+int afqmc_i_green(afqmc_ctx* c, const double2* phi, int nw, double2* theta, double2* logdet,
+                  int* info, cudaStream_t st);
+int afqmc_i_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias, cudaStream_t st);
+int afqmc_i_vhs(afqmc_ctx* c, const double* x, const double2* vbias, double dtau, int nw,
+                double2* vhs, cudaStream_t st);
+int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, double2* phi, int nw,
+                      cudaStream_t st);
+int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* energy, cudaStream_t st);

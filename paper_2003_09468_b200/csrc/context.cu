@@ -1,0 +1,294 @@
+// Context creation (a0 setup: half-rotation + repack into DMMA fragment layouts), destruction,
+// error strings, options.  Setup is once per simulation and is not timed.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#include "common.cuh"
+
+AFQMC_API const char* afqmc_strerror(int code) {
+    switch (code) {
+        case AFQMC_OK: return "ok";
+        case AFQMC_INVALID_ARGUMENT: return "invalid argument";
+        case AFQMC_UNSUPPORTED: return "unsupported configuration";
+        case AFQMC_CUDA_ERROR: return "CUDA error";
+        case AFQMC_OUT_OF_MEMORY: return "out of device memory";
+        default: return "unknown error code";
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// Fragment layouts.  In all three the innermost 32 doubles are one DMMA A-fragment in lane
+// order: lane l holds A[row = l>>2][kk = l&3]; the k-step s covers reals 4s..4s+3 of the
+// real-embedded K index (complex index j>>1, part j&1 with j = 4s+kk).
+//
+//  Lx (exchange, a9):   [Q][k][ag][gp][s][lane]   rows (gl = row>>2, al = row&3):
+//                        gamma = 2gp+gl, a = 4ag+al;  K = (r, part) of Lh[Q][k][a][gamma][r]
+//  Lf (force bias, a4): [Q][gt][k][a][s][lane]    rows gamma = 8gt+row;  K = (r, part), per (k,a)
+//  Lv (vHS, a5):        [Q][k][prt][s][lane]      rows pr = 8prt+row (p = pr/m, r = pr%m);
+//                        K = (gamma, part) of L[Q][k][gamma][p][r]
+// Out-of-range rows / K entries are stored as zeros, so kernels never branch on tails.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ double2 half_rot_elem(const double2* __restrict__ L, const double2* __restrict__ psi_t,
+                                                 const Dims& d, int Q, int k, int a, int gam, int r) {
+    // Lh[Q][k][a][gam][r] = sum_p conj(A_k[p][a]) L[Q][k][gam][p][r]
+    const double2* Lb = L + (((size_t)(Q * d.Nk + k) * d.nchol + gam) * d.m) * d.m + r;
+    const double2* Ab = psi_t + (size_t)k * d.m * d.n + a;
+    double2 acc = make_double2(0.0, 0.0);
+    for (int p = 0; p < d.m; ++p) {
+        double2 av = Ab[(size_t)p * d.n];
+        av.y = -av.y;
+        acc = cfma(av, Lb[(size_t)p * d.m], acc);
+    }
+    return acc;
+}
+
+__global__ void pack_Lx_kernel(Dims d, const double2* __restrict__ L, const double2* __restrict__ psi_t,
+                               double* __restrict__ Lx, size_t total) {
+    for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total;
+         idx += (size_t)gridDim.x * blockDim.x) {
+        size_t t = idx;
+        int lane = (int)(t & 31); t >>= 5;
+        int s = (int)(t % d.KS); t /= d.KS;
+        int gp = (int)(t % d.GP); t /= d.GP;
+        int ag = (int)(t % d.NAG); t /= d.NAG;
+        int k = (int)(t % d.Nk);
+        int Q = (int)(t / d.Nk);
+        int row = lane >> 2, kk = lane & 3;
+        int gam = 2 * gp + (row >> 2), a = 4 * ag + (row & 3);
+        int j = 4 * s + kk, r = j >> 1, c = j & 1;
+        double v = 0.0;
+        if (a < d.n && gam < d.nchol && r < d.m) {
+            double2 z = half_rot_elem(L, psi_t, d, Q, k, a, gam, r);
+            v = c ? z.y : z.x;
+        }
+        Lx[idx] = v;
+    }
+}
+
+__global__ void pack_Lf_kernel(Dims d, const double2* __restrict__ L, const double2* __restrict__ psi_t,
+                               double* __restrict__ Lf, size_t total) {
+    for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total;
+         idx += (size_t)gridDim.x * blockDim.x) {
+        size_t t = idx;
+        int lane = (int)(t & 31); t >>= 5;
+        int s = (int)(t % d.KS); t /= d.KS;
+        int a = (int)(t % d.n); t /= d.n;
+        int k = (int)(t % d.Nk); t /= d.Nk;
+        int gt = (int)(t % d.GT);
+        int Q = (int)(t / d.GT);
+        int row = lane >> 2, kk = lane & 3;
+        int gam = 8 * gt + row;
+        int j = 4 * s + kk, r = j >> 1, c = j & 1;
+        double v = 0.0;
+        if (gam < d.nchol && r < d.m) {
+            double2 z = half_rot_elem(L, psi_t, d, Q, k, a, gam, r);
+            v = c ? z.y : z.x;
+        }
+        Lf[idx] = v;
+    }
+}
+
+__global__ void pack_Lv_kernel(Dims d, const double2* __restrict__ L, double* __restrict__ Lv, size_t total) {
+    for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total;
+         idx += (size_t)gridDim.x * blockDim.x) {
+        size_t t = idx;
+        int lane = (int)(t & 31); t >>= 5;
+        int s = (int)(t % d.GP); t /= d.GP;
+        int prt = (int)(t % d.PRT); t /= d.PRT;   // t = Q*Nk + k
+        int row = lane >> 2, kk = lane & 3;
+        int pr = 8 * prt + row;
+        int j = 4 * s + kk, gam = j >> 1, c = j & 1;
+        double v = 0.0;
+        if (pr < d.m * d.m && gam < d.nchol) {
+            double2 z = L[((size_t)t * d.nchol + gam) * d.m * d.m + pr];
+            v = c ? z.y : z.x;
+        }
+        Lv[idx] = v;
+    }
+}
+
+__global__ void half_rot_h_kernel(Dims d, const double2* __restrict__ h1, const double2* __restrict__ psi_t,
+                                  double2* __restrict__ ht) {
+    // ht[k][a][q] = sum_p conj(A_k[p][a]) h_k[p][q]     (first line of Eq. 49)
+    int total = d.Nk * d.n * d.m;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
+        int q = idx % d.m, a = (idx / d.m) % d.n, k = idx / (d.m * d.n);
+        double2 acc = make_double2(0.0, 0.0);
+        for (int p = 0; p < d.m; ++p) {
+            double2 av = psi_t[((size_t)k * d.m + p) * d.n + a];
+            av.y = -av.y;
+            acc = cfma(av, h1[((size_t)k * d.m + p) * d.m + q], acc);
+        }
+        ht[idx] = acc;
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+static int kidx(const int* g, int a, int b, int c) {
+    a = ((a % g[0]) + g[0]) % g[0];
+    b = ((b % g[1]) + g[1]) % g[1];
+    c = ((c % g[2]) + g[2]) % g[2];
+    return (a * g[1] + b) * g[2] + c;
+}
+
+template <typename T>
+static int dev_alloc(T** p, size_t count) {
+    *p = nullptr;
+    if (count == 0) count = 1;
+    cudaError_t e = cudaMalloc((void**)p, count * sizeof(T));
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        *p = nullptr;
+        return (e == cudaErrorMemoryAllocation) ? AFQMC_OUT_OF_MEMORY : AFQMC_CUDA_ERROR;
+    }
+    return AFQMC_OK;
+}
+
+AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
+    if (!c) return;
+    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lx, c->Lf, c->Lv,
+                    c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T,
+                    c->ws_expart, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info};
+    for (void* p : ptrs)
+        if (p) cudaFree(p);
+    delete c;
+}
+
+AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* h1, const void* L,
+                            const void* psi_t, void* stream) {
+    if (!out) return AFQMC_INVALID_ARGUMENT;
+    *out = nullptr;
+    if (!dims || !h1 || !L || !psi_t) return AFQMC_INVALID_ARGUMENT;
+    if (dims->g[0] < 1 || dims->g[1] < 1 || dims->g[2] < 1 || dims->m < 1 || dims->n < 1 ||
+        dims->n > dims->m || dims->nchol < 1 || dims->max_walkers < 1)
+        return AFQMC_INVALID_ARGUMENT;
+    long long nk_ll = (long long)dims->g[0] * dims->g[1] * dims->g[2];
+    if (nk_ll > AFQMC_MAX_NK) return AFQMC_INVALID_ARGUMENT;
+    if (dims->closed_shell != 1) return AFQMC_UNSUPPORTED;
+    if (dims->precision != 0) return AFQMC_UNSUPPORTED;
+    cudaStream_t st = (cudaStream_t)stream;
+
+    afqmc_ctx* c = new afqmc_ctx();
+    memset(c, 0, sizeof(*c));
+    Dims& d = c->d;
+    for (int i = 0; i < 3; ++i) d.g[i] = dims->g[i];
+    d.Nk = (int)nk_ll; d.m = dims->m; d.n = dims->n; d.nchol = dims->nchol;
+    d.M = d.Nk * d.m; d.N = d.Nk * d.n;
+    d.KS = (2 * d.m + 3) / 4;
+    d.NAG = (d.n + 3) / 4;
+    d.GP = (d.nchol + 1) / 2;
+    d.GT = (d.nchol + 7) / 8;
+    d.PRT = (d.m * d.m + 7) / 8;
+    c->max_walkers = dims->max_walkers;
+    const int nw = c->max_walkers;
+
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { delete c; return AFQMC_CUDA_ERROR; }
+    cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
+
+    // ---- k-point tables and exchange work units (host) ----
+    const int Nk = d.Nk;
+    std::vector<int> kminus(Nk * Nk), kplus(Nk * Nk), kneg(Nk);
+    for (int k = 0; k < Nk; ++k) {
+        int k1 = k / (d.g[1] * d.g[2]), k2 = (k / d.g[2]) % d.g[1], k3 = k % d.g[2];
+        kneg[k] = kidx(d.g, -k1, -k2, -k3);
+        for (int Q = 0; Q < Nk; ++Q) {
+            int q1 = Q / (d.g[1] * d.g[2]), q2 = (Q / d.g[2]) % d.g[1], q3 = Q % d.g[2];
+            kminus[k * Nk + Q] = kidx(d.g, k1 - q1, k2 - q2, k3 - q3);
+            kplus[k * Nk + Q] = kidx(d.g, k1 + q1, k2 + q2, k3 + q3);
+        }
+    }
+    // unit (Q,k,k2): T^Q[(k,a),(k2,b),g] contracted with its partner T^{-Q}[(k2,b),(k,a),g];
+    // the partner unit is (-Q,k2,k) (an involution), so each unordered pair is computed once.
+    std::vector<int> units;
+    for (int Q = 0; Q < Nk; ++Q)
+        for (int k = 0; k < Nk; ++k)
+            for (int k2 = 0; k2 < Nk; ++k2) {
+                int Qp = kneg[Q], kp = k2, k2p = k;
+                long long me = ((long long)Q * Nk + k) * Nk + k2, pa = ((long long)Qp * Nk + kp) * Nk + k2p;
+                if (pa < me) continue;
+                units.push_back(Q); units.push_back(k); units.push_back(k2);
+                units.push_back(pa == me ? 1 : 2);
+            }
+    c->nunits = (int)(units.size() / 4);
+
+    int rc = AFQMC_OK;
+    auto A = [&](int r) { if (rc == AFQMC_OK) rc = r; };
+    const size_t nLx = (size_t)Nk * Nk * d.NAG * d.GP * d.KS * 32;
+    const size_t nLf = (size_t)Nk * d.GT * Nk * d.n * d.KS * 32;
+    const size_t nLv = (size_t)Nk * Nk * d.PRT * d.GP * 32;
+    const int LD = d.N | 1;
+    A(dev_alloc(&c->kminus, (size_t)Nk * Nk));
+    A(dev_alloc(&c->kplus, (size_t)Nk * Nk));
+    A(dev_alloc(&c->kneg, (size_t)Nk));
+    A(dev_alloc(&c->units, units.size()));
+    A(dev_alloc(&c->psi_t, (size_t)Nk * d.m * d.n));
+    A(dev_alloc(&c->ht, (size_t)Nk * d.n * d.m));
+    A(dev_alloc(&c->Lx, nLx));
+    A(dev_alloc(&c->Lf, nLf));
+    A(dev_alloc(&c->Lv, nLv));
+    A(dev_alloc(&c->ws_O, (size_t)nw * d.N * LD));
+    A(dev_alloc(&c->ws_oinvT, (size_t)nw * d.N * d.N));
+    A(dev_alloc(&c->ws_theta, (size_t)nw * d.N * d.M));
+    A(dev_alloc(&c->ws_vbias, (size_t)nw * Nk * d.nchol));
+    A(dev_alloc(&c->ws_xi, (size_t)Nk * d.GP * ((nw + 3) / 4) * 16));   // expanded fragments: 32 doubles each
+    A(dev_alloc(&c->ws_vhs, (size_t)nw * d.M * d.M));
+    A(dev_alloc(&c->ws_T, (size_t)2 * nw * d.M * d.N));
+    A(dev_alloc(&c->ws_expart, (size_t)c->nunits * nw));
+    A(dev_alloc(&c->ws_x, (size_t)nw * Nk * d.nchol));
+    A(dev_alloc(&c->ws_phi, (size_t)nw * d.M * d.N));
+    A(dev_alloc(&c->ws_energy, (size_t)nw * 3));
+    A(dev_alloc(&c->ws_logdet, (size_t)nw));
+    A(dev_alloc(&c->ws_info, (size_t)nw));
+    if (rc != AFQMC_OK) { afqmc_destroy(c); return rc; }
+
+    auto H2D = [&](void* dst, const void* src, size_t bytes) {
+        if (rc == AFQMC_OK && cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
+            rc = AFQMC_CUDA_ERROR;
+    };
+    H2D(c->kminus, kminus.data(), kminus.size() * sizeof(int));
+    H2D(c->kplus, kplus.data(), kplus.size() * sizeof(int));
+    H2D(c->kneg, kneg.data(), kneg.size() * sizeof(int));
+    H2D(c->units, units.data(), units.size() * sizeof(int));
+    if (rc == AFQMC_OK &&
+        cudaMemcpyAsync(c->psi_t, psi_t, (size_t)Nk * d.m * d.n * sizeof(double2), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+        rc = AFQMC_CUDA_ERROR;
+    if (rc == AFQMC_OK) {
+        const int T = 256;
+        auto grid = [&](size_t total) { return (int)((total + T - 1) / T > 148 * 64 ? 148 * 64 : (total + T - 1) / T); };
+        half_rot_h_kernel<<<grid((size_t)Nk * d.n * d.m), T, 0, st>>>(d, (const double2*)h1, c->psi_t, c->ht);
+        pack_Lx_kernel<<<grid(nLx), T, 0, st>>>(d, (const double2*)L, c->psi_t, c->Lx, nLx);
+        pack_Lf_kernel<<<grid(nLf), T, 0, st>>>(d, (const double2*)L, c->psi_t, c->Lf, nLf);
+        pack_Lv_kernel<<<grid(nLv), T, 0, st>>>(d, (const double2*)L, c->Lv, nLv);
+        c->launches += 4;
+        if (cudaGetLastError() != cudaSuccess) rc = AFQMC_CUDA_ERROR;
+    }
+    // host vectors must outlive the async copies; the caller may free its arrays after return
+    if (cudaStreamSynchronize(st) != cudaSuccess && rc == AFQMC_OK) rc = AFQMC_CUDA_ERROR;
+    if (rc != AFQMC_OK) { (void)cudaGetLastError(); afqmc_destroy(c); return rc; }
+    *out = c;
+    return AFQMC_OK;
+}
+
+AFQMC_API long long afqmc_launch_count(const afqmc_ctx* c) { return c ? c->launches : 0; }
+
+AFQMC_API double afqmc_exchange_flops(const afqmc_ctx* c, int nw) {
+    if (!c) return 0.0;
+    const Dims& d = c->d;
+    // per unit and walker: two complex GEMMs (n x m)(m x n) per gamma = 2 * 8*n*n*m*nchol real flops,
+    // plus the complex contraction 8*n*n*nchol.
+    double per = 16.0 * d.n * d.n * d.m * d.nchol + 8.0 * d.n * d.n * d.nchol;
+    return per * (double)c->nunits * (double)nw;
+}
+
+AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
+    if (!c || !name) return AFQMC_INVALID_ARGUMENT;
+    if (strcmp(name, "exchange_variant") == 0) {
+        if (value < 0 || value > 1) return AFQMC_INVALID_ARGUMENT;
+        c->opt_exchange = value;
+        return AFQMC_OK;
+    }
+    return AFQMC_INVALID_ARGUMENT;
+}

@@ -1,0 +1,237 @@
+// a7 one-body, a8 Coulomb, a9 exchange energy (Eq. 49; recipe PAPER.md:306-319).
+//
+// Exchange.  With T^Q[(k,a),(k2,b),g] = sum_r Lh[Q][k][a][g][r] theta[(k2,b),(k-Q,r)] the paper's
+// T1(Q,k,k')[b,a,g] is T^Q[(k,a),(k'-Q,b),g] and T2(Q,k,k')[a,b,g] is T^{-Q}[(k'-Q,b),(k,a),g]
+// (it uses Lh[-Q][k'-Q], which is Lbar of Eq. 40 under the (Q,-Q) identity of PAPER.md:216), so
+//     EX = - sum_{Q,k,k2} X(Q,k,k2),   X = sum_{a,b,g} T^Q[(k,a),(k2,b),g] T^{-Q}[(k2,b),(k,a),g]
+// and X(Q,k,k2) = X(-Q,k2,k): the map is an involution, so only one unit of each pair is computed
+// (weight 2; fixed points weight 1).  The T tensors never leave the SM: a work unit forms both
+// n x n x gamma blocks with DMMA (rows = (gamma pair, a), cols = (b, re/im), K = (r, re/im)),
+// transposes one of them across lanes with a shuffle, and contracts in registers.  This replaces
+// the paper's T1/T2 global buffers and its separate contraction kernel.
+#include "common.cuh"
+
+namespace {
+
+constexpr int EX_WARPS = 8;
+
+// lane' holding the (a,b)-transposed element inside a 16-lane group of a C fragment
+__device__ __forceinline__ int transpose_lane(int lane) { return (lane & 16) | ((lane & 3) << 2) | ((lane >> 2) & 3); }
+
+// ---------------------------------------------------------------------------------------------
+// Variant 1 ("simple"): B fragments (theta blocks, real-embedded) staged once per CTA in shared
+// memory; A fragments (Lx tiles) loaded straight from global/L2 in lane order.
+// CTA = (unit, group of NT walkers); warps split the gamma-pair tiles in groups of MT.
+// ---------------------------------------------------------------------------------------------
+template <int MT, int NT>
+__global__ void __launch_bounds__(32 * EX_WARPS) exchange_simple_kernel(
+    Dims d, int nw, const int* __restrict__ units, const int* __restrict__ kminus, const int* __restrict__ kplus,
+    const int* __restrict__ kneg, const double* __restrict__ Lx, const double2* __restrict__ theta,
+    double2* __restrict__ partial) {
+    extern __shared__ __align__(16) double ex_smem[];
+    // Bs1/Bs2: [bg or ag][s][j][lane]
+    const int u = blockIdx.x, w0 = blockIdx.y * NT;
+    const int Q = units[4 * u], k = units[4 * u + 1], k2 = units[4 * u + 2];
+    const int mQ = kneg[Q];
+    const int kq = kminus[k * d.Nk + Q];        // k - Q   : column block of theta for T^Q rows k
+    const int k2pq = kplus[k2 * d.Nk + Q];      // k2 + Q  : column block of theta for T^{-Q} rows k2
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int KS = d.KS, NAG = d.NAG;
+    double* Bs1 = ex_smem;                                  // theta[(k2,b),(k-Q,r)]
+    double* Bs2 = ex_smem + (size_t)NAG * KS * NT * 32;     // theta[(k,a),(k2+Q,s)]
+
+    // ---- stage B fragments: value for (grp, s, j, lane) ----
+    for (int e = tid; e < 2 * NAG * KS * NT * 32; e += blockDim.x) {
+        int which = e / (NAG * KS * NT * 32);
+        int rem = e % (NAG * KS * NT * 32);
+        int ln = rem & 31;
+        int j = (rem >> 5) % NT;
+        int s = ((rem >> 5) / NT) % KS;
+        int grp = (rem >> 5) / (NT * KS);
+        int kkk = ln & 3, col = ln >> 2;
+        int orb = 4 * grp + (col >> 1), dd = col & 1, cc = kkk & 1;
+        int r = 2 * s + (kkk >> 1);
+        int w = w0 + j;
+        double v = 0.0;
+        if (orb < d.n && r < d.m && w < nw) {
+            int rowblk = which == 0 ? k2 : k, colblk = which == 0 ? kq : k2pq;
+            const double* src = reinterpret_cast<const double*>(
+                theta + ((size_t)w * d.N + rowblk * d.n + orb) * d.M + (size_t)colblk * d.m + r);
+            v = src[cc ^ dd];
+            if (cc && !dd) v = -v;
+        }
+        ex_smem[e] = v;
+    }
+    __syncthreads();
+
+    double er[NT], ei[NT];
+#pragma unroll
+    for (int j = 0; j < NT; ++j) er[j] = ei[j] = 0.0;
+    const int srcl = transpose_lane(lane);
+    const int ngrp = (d.GP + MT - 1) / MT;
+    const size_t tile = (size_t)KS * 32;
+
+    for (int ag = 0; ag < NAG; ++ag)
+        for (int bg = 0; bg < NAG; ++bg)
+            for (int mg = warp; mg < ngrp; mg += EX_WARPS) {
+                const double* a1 = Lx + ((((size_t)Q * d.Nk + k) * NAG + ag) * d.GP + (size_t)mg * MT) * tile + lane;
+                const double* a2 = Lx + ((((size_t)mQ * d.Nk + k2) * NAG + bg) * d.GP + (size_t)mg * MT) * tile + lane;
+                const double* b1 = Bs1 + (size_t)bg * KS * NT * 32 + lane;
+                const double* b2 = Bs2 + (size_t)ag * KS * NT * 32 + lane;
+                bool ok[MT];
+#pragma unroll
+                for (int i = 0; i < MT; ++i) ok[i] = mg * MT + i < d.GP;
+                double acc1[MT][NT][2], acc2[MT][NT][2];
+#pragma unroll
+                for (int i = 0; i < MT; ++i)
+#pragma unroll
+                    for (int j = 0; j < NT; ++j) acc1[i][j][0] = acc1[i][j][1] = acc2[i][j][0] = acc2[i][j][1] = 0.0;
+                double fa1[MT], fa2[MT];
+#pragma unroll
+                for (int i = 0; i < MT; ++i) {
+                    fa1[i] = ok[i] ? __ldg(a1 + i * tile) : 0.0;
+                    fa2[i] = ok[i] ? __ldg(a2 + i * tile) : 0.0;
+                }
+                for (int s = 0; s < KS; ++s) {
+                    double ca1[MT], ca2[MT];
+#pragma unroll
+                    for (int i = 0; i < MT; ++i) { ca1[i] = fa1[i]; ca2[i] = fa2[i]; }
+                    if (s + 1 < KS) {
+#pragma unroll
+                        for (int i = 0; i < MT; ++i) {
+                            fa1[i] = ok[i] ? __ldg(a1 + i * tile + (s + 1) * 32) : 0.0;
+                            fa2[i] = ok[i] ? __ldg(a2 + i * tile + (s + 1) * 32) : 0.0;
+                        }
+                    }
+                    double fb1[NT], fb2[NT];
+#pragma unroll
+                    for (int j = 0; j < NT; ++j) {
+                        fb1[j] = b1[(s * NT + j) * 32];
+                        fb2[j] = b2[(s * NT + j) * 32];
+                    }
+#pragma unroll
+                    for (int i = 0; i < MT; ++i)
+#pragma unroll
+                        for (int j = 0; j < NT; ++j) {
+                            dmma884(acc1[i][j][0], acc1[i][j][1], ca1[i], fb1[j]);
+                            dmma884(acc2[i][j][0], acc2[i][j][1], ca2[i], fb2[j]);
+                        }
+                }
+                // contract: lane holds T1[(g,a),(b)]; fetch T2[(g,b),(a)] from the transposed lane
+#pragma unroll
+                for (int i = 0; i < MT; ++i)
+#pragma unroll
+                    for (int j = 0; j < NT; ++j) {
+                        double t2r = __shfl_sync(0xffffffffu, acc2[i][j][0], srcl);
+                        double t2i = __shfl_sync(0xffffffffu, acc2[i][j][1], srcl);
+                        er[j] = fma(acc1[i][j][0], t2r, er[j]);
+                        er[j] = fma(-acc1[i][j][1], t2i, er[j]);
+                        ei[j] = fma(acc1[i][j][0], t2i, ei[j]);
+                        ei[j] = fma(acc1[i][j][1], t2r, ei[j]);
+                    }
+            }
+
+    // ---- reduce over lanes and warps (deterministic) ----
+    __syncthreads();
+    double* red = ex_smem;   // reuse: [warp][NT][2]
+#pragma unroll
+    for (int j = 0; j < NT; ++j) {
+        double r = warp_sum(er[j]), i = warp_sum(ei[j]);
+        if (lane == 0) { red[(warp * NT + j) * 2] = r; red[(warp * NT + j) * 2 + 1] = i; }
+    }
+    __syncthreads();
+    if (tid < NT && w0 + tid < nw) {
+        double r = 0.0, i = 0.0;
+        for (int x = 0; x < EX_WARPS; ++x) { r += red[(x * NT + tid) * 2]; i += red[(x * NT + tid) * 2 + 1]; }
+        partial[(size_t)u * nw + w0 + tid] = make_double2(r, i);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Final reduction: one CTA per walker.  E1 (a7), EC from the force bias (a8), EX from the unit partials.
+// ---------------------------------------------------------------------------------------------
+__device__ double2 block_sum2(double2 v, double* scratch /* >= 64 doubles */) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    v.x = warp_sum(v.x); v.y = warp_sum(v.y);
+    __syncthreads();
+    if (lane == 0) { scratch[warp] = v.x; scratch[32 + warp] = v.y; }
+    __syncthreads();
+    double2 r = make_double2(0.0, 0.0);
+    for (int x = 0; x < nwarps; ++x) { r.x += scratch[x]; r.y += scratch[32 + x]; }
+    return r;
+}
+
+__global__ void __launch_bounds__(256) energy_finalize_kernel(
+    Dims d, int nw, int nunits, const int* __restrict__ units, const int* __restrict__ kneg,
+    const double2* __restrict__ ht, const double2* __restrict__ theta, const double2* __restrict__ vbias,
+    const double2* __restrict__ partial, double2* __restrict__ energy) {
+    __shared__ double scratch[64];
+    const int w = blockIdx.x, tid = threadIdx.x;
+    // E1 = 2 sum_k sum_{a,q} ht[k][a][q] theta[(k,a),(k,q)]
+    double2 e1 = make_double2(0.0, 0.0);
+    for (int e = tid; e < d.Nk * d.n * d.m; e += blockDim.x) {
+        int q = e % d.m, ka = e / d.m, k = ka / d.n;
+        e1 = cfma(ht[e], theta[((size_t)w * d.N + ka) * d.M + (size_t)k * d.m + q], e1);
+    }
+    e1 = block_sum2(e1, scratch);
+    // EC = 1/2 sum_Q sum_g v[Q][g] v[-Q][g]
+    double2 ec = make_double2(0.0, 0.0);
+    for (int e = tid; e < d.Nk * d.nchol; e += blockDim.x) {
+        int g = e % d.nchol, Q = e / d.nchol;
+        ec = cfma(vbias[((size_t)w * d.Nk + Q) * d.nchol + g], vbias[((size_t)w * d.Nk + kneg[Q]) * d.nchol + g], ec);
+    }
+    ec = block_sum2(ec, scratch);
+    // EX = - sum_units mult * X(unit)
+    double2 ex = make_double2(0.0, 0.0);
+    for (int u = tid; u < nunits; u += blockDim.x) {
+        double mult = (double)units[4 * u + 3];
+        double2 p = partial[(size_t)u * nw + w];
+        ex.x += mult * p.x; ex.y += mult * p.y;
+    }
+    ex = block_sum2(ex, scratch);
+    if (tid == 0) {
+        energy[w * 3 + 0] = make_double2(2.0 * e1.x, 2.0 * e1.y);
+        energy[w * 3 + 1] = make_double2(0.5 * ec.x, 0.5 * ec.y);
+        energy[w * 3 + 2] = make_double2(-ex.x, -ex.y);
+    }
+}
+
+template <int MT, int NT>
+int launch_exchange_simple(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+    const Dims& d = c->d;
+    size_t smem = (size_t)2 * d.NAG * d.KS * NT * 32 * sizeof(double);
+    if (smem < (size_t)EX_WARPS * NT * 2 * sizeof(double)) smem = (size_t)EX_WARPS * NT * 2 * sizeof(double);
+    auto kern = exchange_simple_kernel<MT, NT>;
+    static size_t attr_set = 0;
+    if (smem > 48 * 1024 && smem > attr_set) {
+        if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+            return AFQMC_CUDA_ERROR;
+        attr_set = smem;
+    }
+    dim3 grid(c->nunits, (nw + NT - 1) / NT);
+    kern<<<grid, 32 * EX_WARPS, smem, st>>>(d, nw, c->units, c->kminus, c->kplus, c->kneg, c->Lx, theta, c->ws_expart);
+    AFQMC_LAUNCH_CHECK(c);
+    return AFQMC_OK;
+}
+
+}  // namespace
+
+int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* energy, cudaStream_t st) {
+    const Dims& d = c->d;
+    int rc = afqmc_i_force_bias(c, theta, nw, c->ws_vbias, st);     // steps 2(d): the traces are the force bias
+    if (rc != AFQMC_OK) return rc;
+    if (nw >= 3) rc = launch_exchange_simple<2, 4>(c, theta, nw, st);
+    else rc = launch_exchange_simple<2, 2>(c, theta, nw, st);
+    if (rc != AFQMC_OK) return rc;
+    energy_finalize_kernel<<<nw, 256, 0, st>>>(d, nw, c->nunits, c->units, c->kneg, c->ht, theta, c->ws_vbias,
+                                              c->ws_expart, energy);
+    AFQMC_LAUNCH_CHECK(c);
+    return AFQMC_OK;
+}
+
+AFQMC_API int afqmc_local_energy(afqmc_ctx* c, const void* theta, int nw, void* energy, void* stream) {
+    if (!c || !theta || !energy || nw < 0 || nw > c->max_walkers) return AFQMC_INVALID_ARGUMENT;
+    if (nw == 0) return AFQMC_OK;
+    return afqmc_i_local_energy(c, (const double2*)theta, nw, (double2*)energy, (cudaStream_t)stream);
+}

@@ -1,0 +1,232 @@
+// a1 overlap, a2 elimination (log-det, inverse), a3 half-rotated Green's function.
+//
+// One CTA per walker: O = A^dagger Phi (N x N, Eq. 27-28; assembled as Nk row
+// blocks because the trial is block diagonal) is built in shared memory when it
+// fits (N <= 118), otherwise in a context-owned global workspace, and inverted in place by
+// Gauss-Jordan elimination with partial (row) pivoting -- the same pivot sequence as an LU with
+// partial pivoting, so det O = sign * prod(pivots).  The transposed inverse goes to workspace and
+// Theta = (Phi O^{-1})^T = O^{-T} Phi^T (Eq. 30) is one batched DMMA GEMM.
+#include <math_constants.h>
+#include "zgemm.cuh"
+
+namespace {
+
+constexpr int GJ_THREADS = 1024;
+
+struct GJShared {
+    double best_val[32];
+    double red2[32];
+    int best_idx[32];
+    int piv_row;
+    int info;
+    int nswaps;
+    int pad_;
+};
+
+// shared-memory carve-up (bytes, every section 16-byte aligned):
+//   rowbuf[N], colbuf[N], pivs[N] (double2) | prow[N], qperm[N] (int) | GJShared | matrix N x LD (double2)
+__host__ __device__ inline size_t gj_off_ints(int N) { return (size_t)3 * N * 16; }
+__host__ __device__ inline size_t gj_off_sh(int N) { return gj_off_ints(N) + (((size_t)2 * N * 4 + 15) / 16) * 16; }
+__host__ __device__ inline size_t gj_off_mat(int N) { return gj_off_sh(N) + ((sizeof(GJShared) + 15) / 16) * 16; }
+
+// O and the elimination live at `a` (leading dimension LD), in shared or global memory.
+__global__ void __launch_bounds__(GJ_THREADS) overlap_inverse_kernel(
+    Dims d, int LD, int use_smem, const double2* __restrict__ psi_t, const double2* __restrict__ phi,
+    double2* __restrict__ ws_O, double2* __restrict__ oinvT /*nullable*/, double2* __restrict__ logdet /*nullable*/,
+    int* __restrict__ info /*nullable*/) {
+    extern __shared__ __align__(16) unsigned char gj_smem_raw[];
+    const int N = d.N, w = blockIdx.x, tid = threadIdx.x, nthr = blockDim.x;
+    double2* rowbuf = reinterpret_cast<double2*>(gj_smem_raw);
+    double2* colbuf = rowbuf + N;
+    double2* pivs = colbuf + N;
+    int* prow = reinterpret_cast<int*>(gj_smem_raw + gj_off_ints(N));
+    int* qperm = prow + N;
+    GJShared* sh = reinterpret_cast<GJShared*>(gj_smem_raw + gj_off_sh(N));
+    double2* a = use_smem ? reinterpret_cast<double2*>(gj_smem_raw + gj_off_mat(N)) : ws_O + (size_t)w * N * LD;
+    const double2* ph = phi + (size_t)w * d.M * d.N;
+
+    // ---- a1: O[(k,a)][j] = sum_p conj(A_k[p][a]) Phi[(k,p)][j] ----
+    for (int e = tid; e < N * N; e += nthr) {
+        int j = e % N, i = e / N, k = i / d.n, aa = i % d.n;
+        const double2* Ab = psi_t + (size_t)k * d.m * d.n + aa;
+        const double2* Pb = ph + (size_t)k * d.m * N + j;
+        double2 acc = make_double2(0.0, 0.0);
+        for (int p = 0; p < d.m; ++p) {
+            double2 av = Ab[p * d.n];
+            av.y = -av.y;
+            acc = cfma(av, Pb[(size_t)p * N], acc);
+        }
+        a[i * LD + j] = acc;
+    }
+    if (tid == 0) { sh->info = 0; sh->nswaps = 0; }
+    __syncthreads();
+
+    // ---- a2: in-place Gauss-Jordan inversion with partial pivoting ----
+    const int lane = tid & 31, warp = tid >> 5;
+    for (int j = 0; j < N; ++j) {
+        // pivot search over rows j..N-1 of column j (largest modulus, smallest index on ties)
+        {
+            double bv = -1.0;
+            int bi = 0x7fffffff;
+            for (int i = j + tid; i < N; i += nthr) {
+                double2 v = a[i * LD + j];
+                double mag = v.x * v.x + v.y * v.y;
+                if (mag > bv) { bv = mag; bi = i; }
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                double ov = __shfl_xor_sync(0xffffffffu, bv, o);
+                int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+                if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+            }
+            if (lane == 0) { sh->best_val[warp] = bv; sh->best_idx[warp] = bi; }
+            __syncthreads();
+            if (warp == 0) {
+                int nwarps = nthr >> 5;
+                bv = lane < nwarps ? sh->best_val[lane] : -1.0;
+                bi = lane < nwarps ? sh->best_idx[lane] : 0x7fffffff;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    double ov = __shfl_xor_sync(0xffffffffu, bv, o);
+                    int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+                    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+                }
+                if (lane == 0) {
+                    if (bi == 0x7fffffff) bi = j;   // column of NaNs: keep indices in range, flag below
+                    sh->piv_row = bi;
+                    prow[j] = bi;
+                    if (!(bv > 0.0) && sh->info == 0) sh->info = j + 1;   // exactly-zero (or NaN) pivot
+                    if (bi != j) sh->nswaps++;
+                }
+            }
+            __syncthreads();
+        }
+        const int p = sh->piv_row;
+        const double2 pv = a[p * LD + j];
+        pivs[j] = pv;   // every thread writes the same value
+        // 1/pivot
+        double den = pv.x * pv.x + pv.y * pv.y;
+        double2 ip = (den > 0.0) ? make_double2(pv.x / den, -pv.y / den) : make_double2(0.0, 0.0);
+        __syncthreads();   // all threads have read a[p][j] before the row swap overwrites it
+        // swap rows j <-> p, build the scaled pivot row
+        for (int c = tid; c < N; c += nthr) {
+            double2 rj = a[p * LD + c];
+            if (p != j) a[p * LD + c] = a[j * LD + c];
+            rowbuf[c] = (c == j) ? ip : cmul(rj, ip);
+        }
+        __syncthreads();
+        for (int i = tid; i < N; i += nthr) colbuf[i] = (i == j) ? make_double2(0.0, 0.0) : a[i * LD + j];
+        __syncthreads();
+        // rank-1 update of the whole matrix
+        for (int e = tid; e < N * N; e += nthr) {
+            int c = e % N, i = e / N;
+            double2 r = rowbuf[c];
+            if (i == j) {
+                a[i * LD + c] = r;
+            } else {
+                double2 f = colbuf[i];
+                double2 cur = (c == j) ? make_double2(0.0, 0.0) : a[i * LD + c];
+                f.x = -f.x; f.y = -f.y;
+                a[i * LD + c] = cfma(f, r, cur);
+            }
+        }
+        __syncthreads();
+    }
+
+    // ---- log det O = sum log(pivot) + i*pi*(#swaps odd) ----
+    if (logdet) {
+        double lr = 0.0, li = 0.0;
+        for (int j = tid; j < N; j += nthr) {
+            double2 pv = pivs[j];
+            lr += log(hypot(pv.x, pv.y));
+            li += atan2(pv.y, pv.x);
+        }
+        lr = warp_sum(lr);
+        li = warp_sum(li);
+        __syncthreads();
+        if (lane == 0) { sh->best_val[warp] = lr; sh->red2[warp] = li; }
+        __syncthreads();
+        if (tid == 0) {
+            double sr = 0.0, si = 0.0;
+            for (int x = 0; x < (nthr >> 5); ++x) { sr += sh->best_val[x]; si += sh->red2[x]; }
+            if (sh->nswaps & 1) si += CUDART_PI;
+            // wrap to (-pi, pi]
+            si = si - 2.0 * CUDART_PI * ceil((si - CUDART_PI) / (2.0 * CUDART_PI));
+            logdet[w] = make_double2(sr, si);
+        }
+    }
+    if (info && tid == 0) info[w] = sh->info;
+
+    // ---- undo the row swaps as a column permutation and write O^{-T} ----
+    if (oinvT) {
+        __syncthreads();
+        if (tid == 0) {
+            for (int c = 0; c < N; ++c) qperm[c] = c;
+            for (int j = N - 1; j >= 0; --j) {
+                int pj = prow[j];
+                if (pj != j) { int t = qperm[j]; qperm[j] = qperm[pj]; qperm[pj] = t; }
+            }
+        }
+        __syncthreads();
+        double2* out = oinvT + (size_t)w * N * N;
+        for (int e = tid; e < N * N; e += nthr) {
+            int i = e % N, c = e / N;            // out[c][i] = Oinv[i][c] = a[i][q[c]]
+            out[(size_t)c * N + i] = a[i * LD + qperm[c]];
+        }
+    }
+}
+
+size_t gj_fixed_smem(int N) { return gj_off_mat(N); }
+
+int run_overlap_inverse(afqmc_ctx* c, const double2* phi, int nw, double2* oinvT, double2* logdet, int* info,
+                        cudaStream_t st) {
+    const Dims& d = c->d;
+    const int LD = d.N | 1;
+    size_t fixed = gj_fixed_smem(d.N);
+    size_t mat = (size_t)d.N * LD * sizeof(double2);
+    int use_smem = (fixed + mat <= (size_t)c->smem_optin) ? 1 : 0;
+    size_t smem = fixed + (use_smem ? mat : 0);
+    static size_t attr_set = 0;
+    if (smem > 48 * 1024 && smem > attr_set) {
+        if (cudaFuncSetAttribute(overlap_inverse_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+            return AFQMC_CUDA_ERROR;
+        attr_set = smem;
+    }
+    int threads = GJ_THREADS;
+    if (d.N * d.N < 4096) threads = 256;
+    overlap_inverse_kernel<<<nw, threads, smem, st>>>(d, LD, use_smem, c->psi_t, phi, c->ws_O, oinvT, logdet, info);
+    AFQMC_LAUNCH_CHECK(c);
+    return AFQMC_OK;
+}
+
+}  // namespace
+
+int afqmc_i_green(afqmc_ctx* c, const double2* phi, int nw, double2* theta, double2* logdet, int* info,
+                  cudaStream_t st) {
+    const Dims& d = c->d;
+    int rc = run_overlap_inverse(c, phi, nw, theta ? c->ws_oinvT : nullptr, logdet, info, st);
+    if (rc != AFQMC_OK || !theta) return rc;
+    // Theta[i][q] = sum_j OinvT[i][j] * Phi[q][j]   (B is K-contiguous: element (k=j, col=q) at phi[q*N + j])
+    zg::Args a;
+    a.A = c->ws_oinvT; a.strideA = (long long)d.N * d.N; a.lda = d.N;
+    a.B = phi; a.strideB = (long long)d.M * d.N; a.ldb = d.N;
+    a.C = theta; a.strideC = (long long)d.N * d.M; a.ldc = d.M;
+    a.D = nullptr; a.strideD = 0; a.ldd = 0;
+    a.M = d.N; a.N = d.M; a.K = d.N; a.alpha = 1.0;
+    if (zg::launch<true>(a, nw, st) != cudaSuccess) return AFQMC_CUDA_ERROR;
+    c->launches++;
+    return AFQMC_OK;
+}
+
+AFQMC_API int afqmc_overlap(afqmc_ctx* c, const void* phi, int nw, void* logdet, int* info, void* stream) {
+    if (!c || !phi || !logdet || nw < 0 || nw > c->max_walkers) return AFQMC_INVALID_ARGUMENT;
+    if (nw == 0) return AFQMC_OK;
+    return afqmc_i_green(c, (const double2*)phi, nw, nullptr, (double2*)logdet, info, (cudaStream_t)stream);
+}
+
+AFQMC_API int afqmc_green(afqmc_ctx* c, const void* phi, int nw, void* theta, void* logdet, int* info,
+                           void* stream) {
+    if (!c || !phi || !theta || nw < 0 || nw > c->max_walkers) return AFQMC_INVALID_ARGUMENT;
+    if (nw == 0) return AFQMC_OK;
+    return afqmc_i_green(c, (const double2*)phi, nw, (double2*)theta, (double2*)logdet, info, (cudaStream_t)stream);
+}

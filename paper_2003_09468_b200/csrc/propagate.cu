@@ -1,0 +1,36 @@
+// a6 propagation:  phi_w <- sum_{j=0..order} (s V_w)^j / j!  phi_w,  s = -sqrt(dtau)
+// (truncated Taylor series of PAPER.md:160), by the recurrence T_0 = phi, T_j = (s/j) V T_{j-1},
+// phi += T_j.  Each order is one batched DMMA GEMM (zgemm.cuh) over all walkers with the scale and
+// the running sum fused in its epilogue; T ping-pongs between two workspace buffers, so phi is
+// never read by a GEMM that other CTAs are updating.
+#include "zgemm.cuh"
+
+int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, double2* phi, int nw,
+                      cudaStream_t st) {
+    const Dims& d = c->d;
+    if (order == 0) return AFQMC_OK;
+    const size_t per = (size_t)d.M * d.N;
+    double2* T[2] = {c->ws_T, c->ws_T + (size_t)c->max_walkers * per};
+    if (cudaMemcpyAsync(T[0], phi, (size_t)nw * per * sizeof(double2), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+        return AFQMC_CUDA_ERROR;
+    const double s = -sqrt(dtau);
+    for (int j = 1; j <= order; ++j) {
+        zg::Args a;
+        a.A = vhs; a.strideA = (long long)d.M * d.M; a.lda = d.M;
+        a.B = T[(j - 1) & 1]; a.strideB = (long long)per; a.ldb = d.N;
+        a.C = T[j & 1]; a.strideC = (long long)per; a.ldc = d.N;
+        a.D = phi; a.strideD = (long long)per; a.ldd = d.N;
+        a.M = d.M; a.N = d.N; a.K = d.M; a.alpha = s / (double)j;
+        if (zg::launch<false>(a, nw, st) != cudaSuccess) return AFQMC_CUDA_ERROR;
+        c->launches++;
+    }
+    return AFQMC_OK;
+}
+
+AFQMC_API int afqmc_propagate(afqmc_ctx* c, const void* vhs, double dtau, int order, void* phi, int nw,
+                               void* stream) {
+    if (!c || !vhs || !phi || nw < 0 || nw > c->max_walkers || order < 0 || order > 32 || !(dtau >= 0.0))
+        return AFQMC_INVALID_ARGUMENT;
+    if (nw == 0) return AFQMC_OK;
+    return afqmc_i_propagate(c, (const double2*)vhs, dtau, order, (double2*)phi, nw, (cudaStream_t)stream);
+}

@@ -1,0 +1,42 @@
+// The timed composition: the propagation step of
+// PAPER.md:87-107/:142-160 on phi, then the energy evaluation of PAPER.md:306-319 on the new phi.
+#include "common.cuh"
+
+AFQMC_API int afqmc_step(afqmc_ctx* c, void* phi, const double* x, double dtau, int order, int nw,
+                          void* energy, void* logdet, int* info, void* stream) {
+    if (!c || !phi || !x || !energy || nw < 0 || nw > c->max_walkers || order < 0 || order > 32 || !(dtau >= 0.0))
+        return AFQMC_INVALID_ARGUMENT;
+    if (nw == 0) return AFQMC_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    double2* ph = (double2*)phi;
+    int rc;
+    if ((rc = afqmc_i_green(c, ph, nw, c->ws_theta, nullptr, nullptr, st)) != AFQMC_OK) return rc;
+    if ((rc = afqmc_i_force_bias(c, c->ws_theta, nw, c->ws_vbias, st)) != AFQMC_OK) return rc;
+    if ((rc = afqmc_i_vhs(c, x, c->ws_vbias, dtau, nw, c->ws_vhs, st)) != AFQMC_OK) return rc;
+    if ((rc = afqmc_i_propagate(c, c->ws_vhs, dtau, order, ph, nw, st)) != AFQMC_OK) return rc;
+    if ((rc = afqmc_i_green(c, ph, nw, c->ws_theta, (double2*)logdet, info, st)) != AFQMC_OK) return rc;
+    if ((rc = afqmc_i_local_energy(c, c->ws_theta, nw, (double2*)energy, st)) != AFQMC_OK) return rc;
+    return AFQMC_OK;
+}
+
+AFQMC_API int afqmc_step_host(afqmc_ctx* c, void* phi_host, const double* x_host, double dtau, int order,
+                               int nw, void* energy_host, void* logdet_host, int* info_host, void* stream) {
+    if (!c || !phi_host || !x_host || !energy_host || nw < 0 || nw > c->max_walkers) return AFQMC_INVALID_ARGUMENT;
+    if (nw == 0) return AFQMC_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Dims& d = c->d;
+    const size_t phi_bytes = (size_t)nw * d.M * d.N * sizeof(double2);
+    const size_t x_bytes = (size_t)nw * d.Nk * d.nchol * sizeof(double);
+    AFQMC_CUDA_TRY(cudaMemcpyAsync(c->ws_phi, phi_host, phi_bytes, cudaMemcpyHostToDevice, st));
+    AFQMC_CUDA_TRY(cudaMemcpyAsync(c->ws_x, x_host, x_bytes, cudaMemcpyHostToDevice, st));
+    int rc = afqmc_step(c, c->ws_phi, c->ws_x, dtau, order, nw, c->ws_energy, c->ws_logdet, c->ws_info, stream);
+    if (rc != AFQMC_OK) return rc;
+    AFQMC_CUDA_TRY(cudaMemcpyAsync(phi_host, c->ws_phi, phi_bytes, cudaMemcpyDeviceToHost, st));
+    AFQMC_CUDA_TRY(cudaMemcpyAsync(energy_host, c->ws_energy, (size_t)nw * 3 * sizeof(double2), cudaMemcpyDeviceToHost, st));
+    if (logdet_host)
+        AFQMC_CUDA_TRY(cudaMemcpyAsync(logdet_host, c->ws_logdet, (size_t)nw * sizeof(double2), cudaMemcpyDeviceToHost, st));
+    if (info_host)
+        AFQMC_CUDA_TRY(cudaMemcpyAsync(info_host, c->ws_info, (size_t)nw * sizeof(int), cudaMemcpyDeviceToHost, st));
+    AFQMC_CUDA_TRY(cudaStreamSynchronize(st));
+    return AFQMC_OK;
+}

@@ -1,0 +1,293 @@
+"""GPU parity: every C-ABI step call against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star, metric of SURVEY.md P16): relative 1e-10 in complex128 --
+tensors: max|gpu-ref| / max|ref| per walker; scalars: |gpu-ref| / |ref|; logdet: real part
+relative to max(1,|ref|), phase modulo 2 pi.  Each stage is fed the GPU output of the previous
+stage (downloaded), and the oracle evaluates the same stage on exactly those inputs, so a stage's
+error is not hidden or amplified by its predecessors.
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import afqmc_oracle as orc
+from paper_2003_09468_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-10
+
+
+def relerr(a, b):
+    a, b = np.asarray(a), np.asarray(b)
+    den = max(float(np.max(np.abs(b))), 1e-300)
+    return float(np.max(np.abs(a - b)) / den)
+
+
+def phase_diff(a, b):
+    return abs(np.angle(np.exp(1j * (a - b))))
+
+
+def _to_dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+class Case:
+    def __init__(self, cfg, nw=None):
+        from paper_2003_09468_b200 import binding
+        self.cfg = cfg
+        self.pb = synth.make_problem(cfg, nw)
+        self.nw = self.pb.phi.shape[0]
+        self.ctx = binding.from_problem(self.pb)
+        self.Lh, self.ht = orc.half_rotate(self.pb.L, self.pb.psi_t, self.pb.h1)
+
+    def close(self):
+        self.ctx.close()
+
+
+def run_chain_and_compare(case, sample, tol=RTOL, check_energy=True):
+    cfg, pb, ctx = case.cfg, case.pb, case.ctx
+    mesh = cfg.mesh
+    phi_d = _to_dev(pb.phi)
+    x_d = _to_dev(pb.x)
+
+    # a1-a3
+    theta_d, logdet_d, info_d = ctx.green(phi_d)
+    theta, logdet, info = theta_d.cpu().numpy(), logdet_d.cpu().numpy(), info_d.cpu().numpy()
+    assert np.all(info == 0)
+    ld2, info2 = ctx.overlap(phi_d)
+    assert np.array_equal(ld2.cpu().numpy(), logdet)          # same kernel, same result
+    for w in sample:
+        th_o, ld_o, inf_o = orc.green(pb.psi_t, pb.phi[w])
+        assert inf_o == 0
+        assert relerr(theta[w], th_o) < tol, ("theta", w, relerr(theta[w], th_o))
+        assert abs(logdet[w].real - ld_o.real) < tol * max(1.0, abs(ld_o.real)), ("logdet", w)
+        assert phase_diff(logdet[w].imag, ld_o.imag) < 1e-9, ("phase", w)
+
+    # a4
+    vb_d = ctx.force_bias(theta_d)
+    vb = vb_d.cpu().numpy()
+    for w in sample:
+        vb_o = orc.force_bias(mesh, case.Lh, theta[w])
+        assert relerr(vb[w], vb_o) < tol, ("vbias", w, relerr(vb[w], vb_o))
+
+    # a5 (with and without the force-bias shift)
+    vhs_d = ctx.vhs(x_d, vb_d, cfg.dtau)
+    vhs0_d = ctx.vhs(x_d, None, cfg.dtau)
+    for w in sample:
+        V = vhs_d[w].cpu().numpy()
+        V_o = orc.vhs(mesh, pb.L, orc.assemble_fields(mesh, pb.x[w], vb[w], cfg.dtau))
+        assert relerr(V, V_o) < tol, ("vhs", w, relerr(V, V_o))
+        V0 = vhs0_d[w].cpu().numpy()
+        V0_o = orc.vhs(mesh, pb.L, orc.assemble_fields(mesh, pb.x[w], None, cfg.dtau))
+        assert relerr(V0, V0_o) < tol, ("vhs0", w)
+        assert relerr(V0, -np.conj(V0.T)) < 1e-13              # anti-Hermitian without the shift
+    del vhs0_d
+
+    # a6
+    phi2_d = phi_d.clone()
+    ctx.propagate(vhs_d, cfg.dtau, cfg.order, phi2_d)
+    phi2 = phi2_d.cpu().numpy()
+    for w in sample:
+        p_o = orc.propagate(vhs_d[w].cpu().numpy(), pb.phi[w], cfg.dtau, cfg.order)
+        assert relerr(phi2[w], p_o) < tol, ("propagate", w, relerr(phi2[w], p_o))
+    phi0_d = phi_d.clone()
+    ctx.propagate(vhs_d, cfg.dtau, 0, phi0_d)
+    assert torch.equal(phi0_d, phi_d)                          # order 0 = identity
+    del vhs_d
+
+    # a1-a3 on the propagated walker, then a7-a9
+    theta2_d, logdet2_d, info2_d = ctx.green(phi2_d)
+    theta2 = theta2_d.cpu().numpy()
+    assert np.all(info2_d.cpu().numpy() == 0)
+    for w in sample:
+        th_o, ld_o, _ = orc.green(pb.psi_t, phi2[w])
+        assert relerr(theta2[w], th_o) < 1e-8, ("theta2", w, relerr(theta2[w], th_o))   # cond(O') enters here
+    e_d = ctx.local_energy(theta2_d)
+    e = e_d.cpu().numpy()
+    if check_energy:
+        for w in sample:
+            e_o = orc.local_energy(mesh, case.Lh, case.ht, theta2[w])
+            for i, name in enumerate(("E1", "EC", "EX")):
+                assert abs(e[w, i] - e_o[i]) < tol * abs(e_o[i]), (name, w, e[w, i], e_o[i])
+
+    # whole step == the chain above, bit for bit, on device and through the host entry
+    phi3_d = phi_d.clone()
+    e3_d, ld3_d, info3_d = ctx.step(phi3_d, x_d, cfg.dtau, cfg.order)
+    assert torch.equal(phi3_d, phi2_d)
+    assert torch.equal(e3_d, e_d)
+    assert torch.equal(ld3_d, logdet2_d)
+    phi_h = torch.from_numpy(pb.phi.copy()).pin_memory()
+    x_h = torch.from_numpy(pb.x.copy()).pin_memory()
+    e_h = torch.empty((case.nw, 3), dtype=torch.complex128).pin_memory()
+    ctx.step_host(phi_h, x_h, cfg.dtau, cfg.order, e_h)
+    assert torch.equal(phi_h, phi2_d.cpu())
+    assert torch.equal(e_h, e_d.cpu())
+    return e
+
+
+# ------------------------------------------------------------------------------------------
+# small and ragged shapes: all walkers checked
+# ------------------------------------------------------------------------------------------
+RAGGED = [
+    dict(mesh=(2, 3, 1), m=5, n=3, nchol=7, nw=5),      # odd m, n<4, odd nchol, nw not a multiple of 4
+    dict(mesh=(1, 1, 1), m=7, n=5, nchol=9, nw=1),      # single k-point, two a-groups, one walker
+    dict(mesh=(2, 2, 2), m=6, n=4, nchol=16, nw=9),     # every Q self-inverse
+    dict(mesh=(3, 1, 2), m=4, n=2, nchol=3, nw=2),
+    dict(mesh=(3, 3, 1), m=9, n=6, nchol=21, nw=3),     # n=6: padded second a-group
+]
+
+
+@pytest.mark.parametrize("kw", RAGGED, ids=lambda k: "x".join(map(str, k["mesh"])) + "_m%d_n%d_c%d_w%d" % (k["m"], k["n"], k["nchol"], k["nw"]))
+def test_ragged_small(kw):
+    cfg = synth.tiny_config(seed=2, **kw)
+    case = Case(cfg)
+    try:
+        run_chain_and_compare(case, range(case.nw))
+    finally:
+        case.close()
+
+
+def test_config_C1_all_walkers():
+    case = Case(synth.CONFIGS["C1"])
+    try:
+        run_chain_and_compare(case, range(case.nw))
+    finally:
+        case.close()
+
+
+def test_config_C2_sampled():
+    case = Case(synth.CONFIGS["C2"])
+    try:
+        run_chain_and_compare(case, [0, 37, 63])
+    finally:
+        case.close()
+
+
+def test_config_C3_headline_sampled():
+    case = Case(synth.CONFIGS["C3"])
+    try:
+        run_chain_and_compare(case, [0, 31])
+    finally:
+        case.close()
+
+
+@pytest.mark.slow
+@pytest.mark.skipif(os.environ.get("AFQMC_SKIP_LARGE") == "1", reason="AFQMC_SKIP_LARGE=1")
+def test_config_C4_sampled():
+    case = Case(synth.CONFIGS["C4"])
+    try:
+        run_chain_and_compare(case, [15])
+    finally:
+        case.close()
+
+
+@pytest.mark.slow
+@pytest.mark.skipif(os.environ.get("AFQMC_SKIP_LARGE") == "1", reason="AFQMC_SKIP_LARGE=1")
+def test_config_C5_sampled():
+    case = Case(synth.CONFIGS["C5"])
+    try:
+        run_chain_and_compare(case, [7])
+    finally:
+        case.close()
+
+
+# ------------------------------------------------------------------------------------------
+# degenerate and edge cases
+# ------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def small_case():
+    case = Case(synth.tiny_config(mesh=(2, 2, 1), m=6, n=4, nchol=10, nw=4, seed=5))
+    yield case
+    case.close()
+
+
+def test_trial_walker_unit_overlap(small_case):
+    case = small_case
+    A = orc.supercell_trial(case.pb.psi_t)
+    phi_d = _to_dev(np.stack([A, A]))
+    theta_d, ld_d, info_d = case.ctx.green(phi_d)
+    ld = ld_d.cpu().numpy()
+    assert np.max(np.abs(ld)) < 1e-12                      # det = 1
+    assert relerr(theta_d[0].cpu().numpy(), A.T) < 1e-12   # Theta = A^T
+    e = case.ctx.local_energy(theta_d).cpu().numpy()
+    assert np.max(np.abs(e.imag)) < 1e-12 * np.max(np.abs(e.real))
+    assert e[0, 1].real > 0 and e[0, 2].real < 0
+    vb = case.ctx.force_bias(theta_d).cpu().numpy()
+    assert abs(e[0, 1] - 0.5 * np.sum(np.abs(vb[0]) ** 2)) < 1e-12 * abs(e[0, 1])
+
+
+def test_block_diagonal_walker_momentum_conservation(small_case):
+    case, cfg = small_case, small_case.cfg
+    rng = np.random.default_rng(3)
+    phi = np.zeros((1, cfg.M, cfg.N), dtype=complex)
+    for k in range(cfg.nk):
+        phi[0, k * cfg.m:(k + 1) * cfg.m, k * cfg.n:(k + 1) * cfg.n] = \
+            rng.standard_normal((cfg.m, cfg.n)) + 1j * rng.standard_normal((cfg.m, cfg.n))
+    theta_d, ld_d, _ = case.ctx.green(_to_dev(phi))
+    vb = case.ctx.force_bias(theta_d).cpu().numpy()[0]
+    assert np.max(np.abs(vb[1:])) < 1e-12 * np.max(np.abs(vb[0]))
+    # det O = prod_k det(A_k^dagger phi_k)
+    tot = 0
+    for k in range(cfg.nk):
+        s, la = np.linalg.slogdet(np.conj(case.pb.psi_t[k]).T @ phi[0, k * cfg.m:(k + 1) * cfg.m, k * cfg.n:(k + 1) * cfg.n])
+        tot += la + 1j * np.angle(s)
+    ld = ld_d.cpu().numpy()[0]
+    assert abs(ld.real - tot.real) < 1e-10 and phase_diff(ld.imag, tot.imag) < 1e-10
+
+
+def test_singular_overlap_reports_info(small_case):
+    case = small_case
+    phi = case.pb.phi[:2].copy()
+    phi[1][:, 3] = 0.0                       # zero column -> O has a zero column
+    _, info_d = case.ctx.overlap(_to_dev(phi))
+    info = info_d.cpu().numpy()
+    assert info[0] == 0 and info[1] > 0
+
+
+def test_gauge_invariance_on_gpu(small_case):
+    case, cfg = small_case, small_case.cfg
+    rng = np.random.default_rng(4)
+    R = rng.standard_normal((cfg.N, cfg.N)) + 1j * rng.standard_normal((cfg.N, cfg.N))
+    phi = np.stack([case.pb.phi[0], case.pb.phi[0] @ R])
+    theta_d, _, _ = case.ctx.green(_to_dev(phi))
+    th = theta_d.cpu().numpy()
+    assert relerr(th[1], th[0]) < 1e-9
+    e = case.ctx.local_energy(theta_d).cpu().numpy()
+    assert relerr(e[1], e[0]) < 1e-9
+
+
+def test_argument_errors(small_case):
+    from paper_2003_09468_b200 import binding
+    case = small_case
+    lib = binding.lib()
+    phi_d = _to_dev(case.pb.phi)
+    # nw = 0 is a no-op
+    assert lib.afqmc_green(case.ctx._h, phi_d.data_ptr(), 0, phi_d.data_ptr(), None, None, None) == 0
+    # nw > max_walkers, null pointers, bad order
+    assert lib.afqmc_green(case.ctx._h, phi_d.data_ptr(), case.nw + 1, phi_d.data_ptr(), None, None, None) == 1
+    assert lib.afqmc_green(case.ctx._h, None, 1, phi_d.data_ptr(), None, None, None) == 1
+    assert lib.afqmc_propagate(case.ctx._h, phi_d.data_ptr(), 0.005, -1, phi_d.data_ptr(), 1, None) == 1
+    assert lib.afqmc_propagate(case.ctx._h, phi_d.data_ptr(), 0.005, 33, phi_d.data_ptr(), 1, None) == 1
+    import ctypes
+    h = ctypes.c_void_p(0)
+    d = binding.Dims((ctypes.c_int * 3)(2, 2, 1), 6, 4, 10, 0, 0, 4)       # open shell
+    assert lib.afqmc_create(ctypes.byref(h), ctypes.byref(d), phi_d.data_ptr(), phi_d.data_ptr(), phi_d.data_ptr(), None) == 2
+    d = binding.Dims((ctypes.c_int * 3)(2, 2, 1), 6, 4, 10, 1, 1, 4)       # complex64 not built yet
+    assert lib.afqmc_create(ctypes.byref(h), ctypes.byref(d), phi_d.data_ptr(), phi_d.data_ptr(), phi_d.data_ptr(), None) == 2
+    d = binding.Dims((ctypes.c_int * 3)(2, 2, 1), 6, 7, 10, 1, 0, 4)       # n > m
+    assert lib.afqmc_create(ctypes.byref(h), ctypes.byref(d), phi_d.data_ptr(), phi_d.data_ptr(), phi_d.data_ptr(), None) == 1
+
+
+def test_subbatch_equals_full_batch(small_case):
+    """nw < max_walkers: results for the first walkers do not depend on the batch size."""
+    case = small_case
+    phi_d = _to_dev(case.pb.phi)
+    th_all, _, _ = case.ctx.green(phi_d)
+    th_3, _, _ = case.ctx.green(phi_d[:3].contiguous())
+    assert torch.equal(th_all[:3], th_3)
+    e_all = case.ctx.local_energy(th_all)
+    e_3 = case.ctx.local_energy(th_3)
+    assert torch.equal(e_all[:3], e_3)
