@@ -1,0 +1,296 @@
+#!/usr/bin/env python
+"""bench.py -- walker-steps/s (incl. local energy) of the k-point ph-AFQMC step on B200.
+
+One "step" = one pass of the whole hot path over the walker batch (afqmc_step: green, force bias,
+vHS, 6th-order Taylor propagation, green on the new walkers, local energy with the exchange
+contraction).  Workload at N=1: BASELINE.json config C3 (3x3x3 k-mesh,
+m=26, n=4, nchol=200, 32 walkers, complex128), the config the metric is quoted on; seeded synthetic
+inputs (paper_2003_09468_b200/synth.py).  N>1: independent replicas, one per GPU/rank, walkers
+sharded by rank with no data-path collective (weak scaling).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C3] [--impl ours|reference]
+
+Prints ONE JSON line on rank 0.  `--impl reference` times the CPU oracle (oracle/afqmc_oracle.py, as
+it stands) on the host cores on a bounded sample (one walker per "step").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "walker-steps/s incl. local energy"
+UNIT = "walker-steps/s"
+
+
+def load_measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p))
+        except Exception:
+            pass
+    return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks / throttle reasons every 200 ms while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index = index
+        self.samples = []
+        self._halt = threading.Event()
+
+    def run(self):
+        while not self._halt.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                f = [v.strip() for v in out.strip().split(",")]
+                if len(f) >= 7:
+                    self.samples.append(f)
+            except Exception:
+                pass
+            self._halt.wait(0.2)
+
+    def stop(self):
+        self._halt.set()
+        self.join(timeout=3)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unsampled"]}
+        sm = sorted(float(s[0]) for s in self.samples)
+        reasons = []
+        for i, name in enumerate(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")):
+            if any(s[3 + i].lower().startswith("active") for s in self.samples):
+                reasons.append(name)
+        pw = max(float(s[2]) for s in self.samples)
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.samples[0][1]), "power_w_max": pw,
+                "samples": len(sm), "reasons": reasons}
+
+
+def oracle_walker_step(orc, cfg, pb, Lh, ht, w):
+    t0 = time.perf_counter()
+    orc.step(cfg.mesh, pb.L, Lh, ht, pb.psi_t, pb.phi[w:w + 1], pb.x[w:w + 1], cfg.dtau, cfg.order)
+    return time.perf_counter() - t0
+
+
+def run_reference(args):
+    """The CPU oracle as the reference arm: each 'step' is the full step for ONE walker of the config."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np  # noqa: F401
+    from threadpoolctl import threadpool_limits
+    from oracle import afqmc_oracle as orc
+    from paper_2003_09468_b200 import synth
+    cfg = synth.CONFIGS[args.config]
+    nsamp = max(1, min(cfg.nw, args.steps + args.warmup))
+    pb = synth.make_problem(cfg, nw=nsamp)
+    with threadpool_limits(limits=1):
+        Lh, ht = orc.half_rotate(pb.L, pb.psi_t, pb.h1)
+        for i in range(args.warmup):
+            oracle_walker_step(orc, cfg, pb, Lh, ht, i % nsamp)
+        tot = 0.0
+        for i in range(args.steps):
+            tot += oracle_walker_step(orc, cfg, pb, Lh, ht, (args.warmup + i) % nsamp)
+    value = args.steps / tot
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "c128", "data": "synthetic",
+        "config": {"workload": "%s: %dx%dx%d k-mesh, m=%d, n=%d, nchol=%d, complex128; one walker per step"
+                               % ((cfg.name,) + tuple(cfg.mesh) + (cfg.m, cfg.n, cfg.nchol))},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": "%d timed full steps (overlap..local energy), one walker each, numpy, 1 thread" % args.steps},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2003_09468_b200 import binding, synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    cfg = synth.CONFIGS[args.config]
+    # replicas: every rank has the same Hamiltonian and its own seeded walkers/fields (weak scaling)
+    pb = synth.make_problem(cfg)
+    if rank > 0:
+        rng = np.random.default_rng(cfg.seed + 1000 + rank)
+        pb.phi = synth.make_walkers(cfg, pb.psi_t, rng)
+        pb.x = rng.standard_normal(pb.x.shape)
+    nw = cfg.nw
+    ctx = binding.from_problem(pb)
+    ctx.set_option("timers", 1)
+    phi0 = torch.from_numpy(pb.phi).cuda()
+    phi = phi0.clone()
+    x = torch.from_numpy(pb.x).cuda()
+    energy = torch.empty((nw, 3), dtype=torch.complex128, device="cuda")
+    logdet = torch.empty((nw,), dtype=torch.complex128, device="cuda")
+    info = torch.empty((nw,), dtype=torch.int32, device="cuda")
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---------------- device-resident timing ----------------
+    for _ in range(args.warmup):
+        phi.copy_(phi0)
+        ctx.step(phi, x, cfg.dtau, cfg.order, energy, logdet, info)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    stage_acc = {k: 0.0 for k in ctx.STAGES}
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    l0 = ctx.launch_count()
+    barrier()
+    t_wall0 = time.perf_counter()
+    for i in range(args.steps):
+        phi.copy_(phi0)                       # restore the walkers (outside the event pair)
+        ev[i][0].record()
+        ctx.step(phi, x, cfg.dtau, cfg.order, energy, logdet, info)
+        ev[i][1].record()
+        ev[i][1].synchronize()
+        for k, v in ctx.stage_times().items():
+            stage_acc[k] += v
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    launches = ctx.launch_count() - l0
+    dev_ms = sum(a.elapsed_time(b) for a, b in ev)
+    assert int(info.abs().sum().item()) == 0
+    e_dev = energy.cpu().numpy().copy()
+
+    # ---------------- end to end through the host-buffer C-ABI call ----------------
+    phi_h0 = torch.from_numpy(pb.phi).pin_memory()
+    phi_h = torch.empty_like(phi_h0).pin_memory()
+    x_h = torch.from_numpy(pb.x).pin_memory()
+    e_h = torch.empty((nw, 3), dtype=torch.complex128).pin_memory()
+    ld_h = torch.empty((nw,), dtype=torch.complex128).pin_memory()
+    info_h = torch.empty((nw,), dtype=torch.int32).pin_memory()
+    e2e_t = 0.0
+    for i in range(max(1, args.warmup // 2) + args.steps):
+        phi_h.copy_(phi_h0)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ctx.step_host(phi_h, x_h, cfg.dtau, cfg.order, e_h, ld_h, info_h)   # synchronises before returning
+        dt = time.perf_counter() - t0
+        if i >= max(1, args.warmup // 2):
+            e2e_t += dt
+    sampler.stop()
+    assert np.array_equal(e_h.numpy(), e_dev), "host-entry step disagrees with the device step"
+    h2d = phi_h.numel() * 16 + x_h.numel() * 8
+    d2h = phi_h.numel() * 16 + e_h.numel() * 16 + ld_h.numel() * 16 + info_h.numel() * 4
+
+    # max over ranks
+    times = torch.tensor([dev_ms, e2e_t * 1e3], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    dev_ms_max, e2e_ms_max = float(times[0]), float(times[1])
+
+    if rank == 0:
+        total_walkers = nw * world
+        value = total_walkers * args.steps / (dev_ms_max * 1e-3)
+        e2e_value = total_walkers * args.steps / (e2e_ms_max * 1e-3)
+        # ---- roofline of the dominant kernel (exchange contraction, a9) ----
+        ex_ms = stage_acc["exchange"] / args.steps
+        ex_flops = ctx.exchange_flops(nw)
+        achieved = ex_flops / (ex_ms * 1e-3) / 1e12
+        peak_probe = binding.probe_fp64(1, 20000)          # DMMA issue-rate probe, this GPU, now
+        peaks = load_measured_peaks()
+        roofline = {
+            "kernel": "exchange (a9), afqmc_local_energy", "bound": "tensor", "achieved": achieved,
+            "peak": peak_probe, "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": None,
+            "peak_source": "live FP64 DMMA.8x8x4 probe (afqmc_probe_fp64); MEASURED_PEAKS.json has no FP64 entry",
+            "flops_per_launch": ex_flops, "ms_per_launch": ex_ms,
+            "share_of_step": ex_ms / (dev_ms_max / args.steps),
+        }
+        if peaks and "bf16_tflops" in peaks:
+            roofline["peak_alt_bf16_ratio"] = peaks["bf16_tflops"] * 45.0 / 2250.0
+        stages = {k: v / args.steps for k, v in stage_acc.items()}
+        # ---- CPU baseline: the oracle on a bounded sample (rank 0, N=1 only) ----
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            from threadpoolctl import threadpool_limits
+            from oracle import afqmc_oracle as orc
+            with threadpool_limits(limits=1):
+                Lh, ht = orc.half_rotate(pb.L, pb.psi_t, pb.h1)
+                nsamp = 2 if cfg.name in ("C3",) else 1
+                if cfg.name in ("C1", "C2"):
+                    nsamp = min(cfg.nw, 8)
+                t = sum(oracle_walker_step(orc, cfg, pb, Lh, ht, w) for w in range(nsamp))
+            cpu = {"value": nsamp / t, "unit": UNIT, "cores": 1, "kind": "oracle",
+                   "sample": "%d of %d walkers of %s, full step each (work is linear in walkers), numpy 1 thread, %.1f s"
+                             % (nsamp, nw, cfg.name, t)}
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "c128", "data": "synthetic",
+            "config": {"workload": "%s: %dx%dx%d k-mesh, m=%d, n=%d, nchol=%d, %d walkers/GPU, complex128, "
+                                   "dtau=%g, Taylor order %d; step = green+force_bias+vhs+propagate+green+local_energy"
+                                   % ((cfg.name,) + tuple(cfg.mesh) + (cfg.m, cfg.n, cfg.nchol, nw, cfg.dtau, cfg.order)),
+                       "l2": "inputs larger than L2 (L %.2f GB, packed Lh %.2f GB, vhs %.2f GB per step)"
+                             % (pb.L.nbytes / 1e9, 2 * cfg.nk ** 2 * cfg.n * cfg.nchol * cfg.m * 16 / 1e9,
+                                nw * cfg.M ** 2 * 16 / 1e9),
+                       "parallelism": "replicas x%d (walkers sharded by rank, no collective)" % world},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "gpu_launches": int(launches),
+            "clocks": sampler.summary(),
+            "roofline": roofline,
+            "stage_ms": stages,
+            "exchange_tflops": achieved,
+            "wall_s_timed_region": t_wall,
+        }
+        if cpu is not None:
+            line["cpu_baseline"] = cpu
+        print(json.dumps(line), flush=True)
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C3")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -157,8 +157,18 @@ long long afqmc_launch_count(const afqmc_ctx* ctx);
  * walkers, as the kernel executes it (pairs (Q,k,k') ~ (-Q,k'-Q,k-Q) computed once). */
 double afqmc_exchange_flops(const afqmc_ctx* ctx, int nw);
 
-/* Selects the exchange-kernel variant: 0 = default (best), 1 = simple direct-load variant. */
+/* Options: "exchange_variant" (0 = default/best, 1 = simple direct-load kernel);
+ * "timers" (1 = afqmc_step records a CUDA event after each stage, see afqmc_stage_times). */
 int afqmc_set_option(afqmc_ctx* ctx, const char* name, int value);
+
+/*
+ * Per-stage device times (milliseconds, CUDA events on the step's stream) of the most recent
+ * afqmc_step, valid after that stream was synchronised and only with option "timers" = 1:
+ * ms[0] green(phi), [1] force_bias, [2] vhs (fields + contraction), [3] propagate, [4] green(phi'),
+ * [5] force bias inside local_energy, [6] the exchange kernel alone, [7] energy finalisation.
+ */
+#define AFQMC_NUM_STAGES 8
+int afqmc_stage_times(afqmc_ctx* ctx, float* ms /* host, [AFQMC_NUM_STAGES] */);
 
 /*
  * FP64 peak probes (measurement aid, no AFQMC arithmetic): runs a register-resident loop of

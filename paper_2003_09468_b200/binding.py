@@ -31,7 +31,7 @@ class Dims(ctypes.Structure):
 
 EXPORTS = ["afqmc_strerror", "afqmc_create", "afqmc_destroy", "afqmc_overlap", "afqmc_green", "afqmc_force_bias",
            "afqmc_vhs", "afqmc_propagate", "afqmc_local_energy", "afqmc_step", "afqmc_step_host",
-           "afqmc_launch_count", "afqmc_exchange_flops", "afqmc_set_option", "afqmc_probe_fp64"]
+           "afqmc_launch_count", "afqmc_exchange_flops", "afqmc_set_option", "afqmc_stage_times", "afqmc_probe_fp64"]
 
 
 def lib():
@@ -63,6 +63,7 @@ def lib():
     L.afqmc_exchange_flops.restype = cd
     L.afqmc_set_option.argtypes = [vp, ctypes.c_char_p, ci]
     L.afqmc_probe_fp64.argtypes = [ci, ci, ctypes.POINTER(cd)]
+    L.afqmc_stage_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
     for name in EXPORTS:
         if name not in ("afqmc_strerror", "afqmc_destroy", "afqmc_launch_count", "afqmc_exchange_flops"):
             getattr(L, name).restype = ci
@@ -143,6 +144,14 @@ class Afqmc:
 
     def set_option(self, name: str, value: int):
         _check(lib().afqmc_set_option(self._h, name.encode(), int(value)), "afqmc_set_option")
+
+    STAGES = ("green", "force_bias", "vhs", "propagate", "green2", "force_bias2", "exchange", "finalize")
+
+    def stage_times(self):
+        """Per-stage ms of the last step() (needs set_option('timers', 1) and a synchronised stream)."""
+        buf = (ctypes.c_float * 8)()
+        _check(lib().afqmc_stage_times(self._h, buf), "afqmc_stage_times")
+        return dict(zip(self.STAGES, [float(v) for v in buf]))
 
     # ---- the six step calls ----------------------------------------------------------------
     def overlap(self, phi, logdet=None, info=None):

@@ -56,6 +56,9 @@ struct afqmc_ctx {
     int* ws_info;       // [nw]
     long long launches;
     int opt_exchange;   // 0 default, 1 simple
+    int opt_timers;     // record stage events in afqmc_step
+    cudaEvent_t ev[AFQMC_NUM_STAGES + 1];
+    int ev_valid;
     int smem_optin;     // max dynamic shared memory per block (bytes)
     int num_sms;
 };
@@ -127,3 +130,7 @@ int afqmc_i_vhs(afqmc_ctx* c, const double* x, const double2* vbias, double dtau
 int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, double2* phi, int nw,
                       cudaStream_t st);
 int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* energy, cudaStream_t st);
+// records stage event i on st when timers are on
+static inline void afqmc_mark(afqmc_ctx* c, int i, cudaStream_t st) {
+    if (c->opt_timers && c->ev[i]) cudaEventRecord(c->ev[i], st);
+}

@@ -152,6 +152,8 @@ AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
                     c->ws_expart, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info};
     for (void* p : ptrs)
         if (p) cudaFree(p);
+    for (cudaEvent_t e : c->ev)
+        if (e) cudaEventDestroy(e);
     delete c;
 }
 
@@ -290,5 +292,23 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
         c->opt_exchange = value;
         return AFQMC_OK;
     }
+    if (strcmp(name, "timers") == 0) {
+        if (value && !c->ev[0])
+            for (int i = 0; i <= AFQMC_NUM_STAGES; ++i)
+                if (cudaEventCreate(&c->ev[i]) != cudaSuccess) return AFQMC_CUDA_ERROR;
+        c->opt_timers = value ? 1 : 0;
+        c->ev_valid = 0;
+        return AFQMC_OK;
+    }
     return AFQMC_INVALID_ARGUMENT;
+}
+
+AFQMC_API int afqmc_stage_times(afqmc_ctx* c, float* ms) {
+    if (!c || !ms || !c->opt_timers || !c->ev_valid) return AFQMC_INVALID_ARGUMENT;
+    for (int i = 0; i < AFQMC_NUM_STAGES; ++i)
+        if (cudaEventElapsedTime(&ms[i], c->ev[i], c->ev[i + 1]) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return AFQMC_CUDA_ERROR;
+        }
+    return AFQMC_OK;
 }

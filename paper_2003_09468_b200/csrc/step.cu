@@ -10,12 +10,20 @@ AFQMC_API int afqmc_step(afqmc_ctx* c, void* phi, const double* x, double dtau, 
     cudaStream_t st = (cudaStream_t)stream;
     double2* ph = (double2*)phi;
     int rc;
+    afqmc_mark(c, 0, st);
     if ((rc = afqmc_i_green(c, ph, nw, c->ws_theta, nullptr, nullptr, st)) != AFQMC_OK) return rc;
+    afqmc_mark(c, 1, st);
     if ((rc = afqmc_i_force_bias(c, c->ws_theta, nw, c->ws_vbias, st)) != AFQMC_OK) return rc;
+    afqmc_mark(c, 2, st);
     if ((rc = afqmc_i_vhs(c, x, c->ws_vbias, dtau, nw, c->ws_vhs, st)) != AFQMC_OK) return rc;
+    afqmc_mark(c, 3, st);
     if ((rc = afqmc_i_propagate(c, c->ws_vhs, dtau, order, ph, nw, st)) != AFQMC_OK) return rc;
+    afqmc_mark(c, 4, st);
     if ((rc = afqmc_i_green(c, ph, nw, c->ws_theta, (double2*)logdet, info, st)) != AFQMC_OK) return rc;
+    afqmc_mark(c, 5, st);
     if ((rc = afqmc_i_local_energy(c, c->ws_theta, nw, (double2*)energy, st)) != AFQMC_OK) return rc;
+    afqmc_mark(c, 8, st);      // marks 6 and 7 are recorded around the exchange kernel inside local_energy
+    if (c->opt_timers) c->ev_valid = 1;
     return AFQMC_OK;
 }
 

@@ -118,7 +118,7 @@ def make_hamiltonian(cfg: Config, rng):
             else:
                 L[Q, k] = blk
                 L[Qp, kp] = np.conj(np.swapaxes(blk, -1, -2))
-    return h1, psi_t, L
+    return np.ascontiguousarray(h1), np.ascontiguousarray(psi_t), L
 
 
 def make_walkers(cfg: Config, psi_t, rng, nw=None, noise=0.1):
