@@ -13,56 +13,55 @@
 
 namespace {
 
-constexpr int EX_WARPS = 8;
 
 // lane' holding the (a,b)-transposed element inside a 16-lane group of a C fragment
 __device__ __forceinline__ int transpose_lane(int lane) { return (lane & 16) | ((lane & 3) << 2) | ((lane >> 2) & 3); }
 
 // ---------------------------------------------------------------------------------------------
 // Variant 1 ("simple"): B fragments (theta blocks, real-embedded) staged once per CTA in shared
-// memory; A fragments (Lx tiles) loaded straight from global/L2 in lane order.
-// CTA = (unit, group of NT walkers); warps split the gamma-pair tiles in groups of MT.
+// memory; A fragments (Lx tiles) loaded straight from global/L2 in lane order, software-pipelined
+// one k-step ahead ACROSS tasks so that no task starts with an exposed L2 round trip.
+// CTA = (unit, group of NT walkers), WPC warps.  A warp task is a group of MT gamma-pair tiles; the
+// host picks WPC so that the tasks divide evenly over the warps (no tail at the final barrier).
+// Walker groups of one unit are adjacent in the grid so that the Lx blocks of a unit are fetched
+// from HBM once and shared through L2.
 // ---------------------------------------------------------------------------------------------
-template <int MT, int NT>
-__global__ void __launch_bounds__(32 * EX_WARPS) exchange_simple_kernel(
+template <int MT, int NT, int WPC>
+__global__ void __launch_bounds__(32 * WPC, 16 / WPC) exchange_simple_kernel(
     Dims d, int nw, const int* __restrict__ units, const int* __restrict__ kminus, const int* __restrict__ kplus,
     const int* __restrict__ kneg, const double* __restrict__ Lx, const double2* __restrict__ theta,
     double2* __restrict__ partial) {
     extern __shared__ __align__(16) double ex_smem[];
-    // Bs1/Bs2: [bg or ag][s][j][lane]
-    const int u = blockIdx.x, w0 = blockIdx.y * NT;
+    const int u = blockIdx.y, w0 = blockIdx.x * NT;
     const int Q = units[4 * u], k = units[4 * u + 1], k2 = units[4 * u + 2];
     const int mQ = kneg[Q];
     const int kq = kminus[k * d.Nk + Q];        // k - Q   : column block of theta for T^Q rows k
     const int k2pq = kplus[k2 * d.Nk + Q];      // k2 + Q  : column block of theta for T^{-Q} rows k2
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int KS = d.KS, NAG = d.NAG;
-    double* Bs1 = ex_smem;                                  // theta[(k2,b),(k-Q,r)]
-    double* Bs2 = ex_smem + (size_t)NAG * KS * NT * 32;     // theta[(k,a),(k2+Q,s)]
+    // Bs[which][grp][s][j][lane]: which = 0 -> theta[(k2,b),(k-Q,r)], 1 -> theta[(k,a),(k2+Q,s)]
+    const size_t bs_half = (size_t)NAG * KS * NT * 32;
 
-    // ---- stage B fragments: value for (grp, s, j, lane) ----
-    for (int e = tid; e < 2 * NAG * KS * NT * 32; e += blockDim.x) {
-        int which = e / (NAG * KS * NT * 32);
-        int rem = e % (NAG * KS * NT * 32);
-        int ln = rem & 31;
-        int j = (rem >> 5) % NT;
-        int s = ((rem >> 5) / NT) % KS;
-        int grp = (rem >> 5) / (NT * KS);
-        int kkk = ln & 3, col = ln >> 2;
-        int orb = 4 * grp + (col >> 1), dd = col & 1, cc = kkk & 1;
-        int r = 2 * s + (kkk >> 1);
-        int w = w0 + j;
-        double v = 0.0;
-        if (orb < d.n && r < d.m && w < nw) {
-            int rowblk = which == 0 ? k2 : k, colblk = which == 0 ? kq : k2pq;
+    // ---- stage B fragments: one (which, grp, walker) fragment column per warp pass, lane = fragment lane ----
+    {
+        const int kkk = lane & 3, col = lane >> 2;
+        const int dd = col & 1, cc = kkk & 1;
+        const bool neg = cc && !dd;
+        for (int c = warp; c < 2 * NAG * NT; c += WPC) {
+            const int jw = c % NT, grp = (c / NT) % NAG, which = c / (NT * NAG);
+            const int orb = 4 * grp + (col >> 1), w = w0 + jw;
+            const int rowblk = which == 0 ? k2 : k, colblk = which == 0 ? kq : k2pq;
+            const bool ok = orb < d.n && w < nw;
             const double* src = reinterpret_cast<const double*>(
-                theta + ((size_t)w * d.N + rowblk * d.n + orb) * d.M + (size_t)colblk * d.m + r);
-            v = src[cc ^ dd];
-            if (cc && !dd) v = -v;
+                theta + ((size_t)(ok ? w : 0) * d.N + rowblk * d.n + (ok ? orb : 0)) * d.M + (size_t)colblk * d.m + (kkk >> 1)) + (cc ^ dd);
+            double* dst = ex_smem + which * bs_half + ((size_t)grp * KS * NT + jw) * 32 + lane;
+            for (int s = 0; s < KS; ++s) {
+                double v = 0.0;
+                if (ok && 2 * s + (kkk >> 1) < d.m) v = __ldg(src + 4 * s);
+                dst[(size_t)s * NT * 32] = neg ? -v : v;
+            }
         }
-        ex_smem[e] = v;
     }
-    __syncthreads();
 
     double er[NT], ei[NT];
 #pragma unroll
@@ -70,66 +69,91 @@ __global__ void __launch_bounds__(32 * EX_WARPS) exchange_simple_kernel(
     const int srcl = transpose_lane(lane);
     const int ngrp = (d.GP + MT - 1) / MT;
     const size_t tile = (size_t)KS * 32;
+    // flattened task list of this warp: t = warp, warp+WPC, ... < NAG*NAG*ngrp ; t -> (ag, bg, mg)
+    const int ntask = NAG * NAG * ngrp;
+    auto task_ptrs = [&](int t, const double*& a1, const double*& a2, int& ag, int& bg, int& mg) {
+        mg = t % ngrp;
+        const int ab = t / ngrp;
+        bg = ab % NAG; ag = ab / NAG;
+        a1 = Lx + ((((size_t)Q * d.Nk + k) * NAG + ag) * d.GP + (size_t)mg * MT) * tile + lane;
+        a2 = Lx + ((((size_t)mQ * d.Nk + k2) * NAG + bg) * d.GP + (size_t)mg * MT) * tile + lane;
+    };
+    const double *a1 = nullptr, *a2 = nullptr;
+    int ag = 0, bg = 0, mg = 0;
+    double fa1[MT], fa2[MT];
+    int t = warp;
+    if (t < ntask) {
+        task_ptrs(t, a1, a2, ag, bg, mg);
+#pragma unroll
+        for (int i = 0; i < MT; ++i) {
+            const bool ok = mg * MT + i < d.GP;
+            fa1[i] = ok ? __ldg(a1 + i * tile) : 0.0;
+            fa2[i] = ok ? __ldg(a2 + i * tile) : 0.0;
+        }
+    }
+    __syncthreads();   // B fragments staged
 
-    for (int ag = 0; ag < NAG; ++ag)
-        for (int bg = 0; bg < NAG; ++bg)
-            for (int mg = warp; mg < ngrp; mg += EX_WARPS) {
-                const double* a1 = Lx + ((((size_t)Q * d.Nk + k) * NAG + ag) * d.GP + (size_t)mg * MT) * tile + lane;
-                const double* a2 = Lx + ((((size_t)mQ * d.Nk + k2) * NAG + bg) * d.GP + (size_t)mg * MT) * tile + lane;
-                const double* b1 = Bs1 + (size_t)bg * KS * NT * 32 + lane;
-                const double* b2 = Bs2 + (size_t)ag * KS * NT * 32 + lane;
-                bool ok[MT];
+    for (; t < ntask; t += WPC) {
+        const double* b1 = ex_smem + (size_t)bg * KS * NT * 32 + lane;
+        const double* b2 = ex_smem + bs_half + (size_t)ag * KS * NT * 32 + lane;
+        // pointers of the next task (for the cross-task prefetch at the last k-step)
+        const double *n1 = a1, *n2 = a2;
+        int nag = ag, nbg = bg, nmg = mg;
+        const bool has_next = t + WPC < ntask;
+        if (has_next) task_ptrs(t + WPC, n1, n2, nag, nbg, nmg);
+        double acc1[MT][NT][2], acc2[MT][NT][2];
 #pragma unroll
-                for (int i = 0; i < MT; ++i) ok[i] = mg * MT + i < d.GP;
-                double acc1[MT][NT][2], acc2[MT][NT][2];
+        for (int i = 0; i < MT; ++i)
 #pragma unroll
-                for (int i = 0; i < MT; ++i)
+            for (int j = 0; j < NT; ++j) acc1[i][j][0] = acc1[i][j][1] = acc2[i][j][0] = acc2[i][j][1] = 0.0;
+        for (int s = 0; s < KS; ++s) {
+            double ca1[MT], ca2[MT];
 #pragma unroll
-                    for (int j = 0; j < NT; ++j) acc1[i][j][0] = acc1[i][j][1] = acc2[i][j][0] = acc2[i][j][1] = 0.0;
-                double fa1[MT], fa2[MT];
+            for (int i = 0; i < MT; ++i) { ca1[i] = fa1[i]; ca2[i] = fa2[i]; }
+            if (s + 1 < KS) {
 #pragma unroll
                 for (int i = 0; i < MT; ++i) {
-                    fa1[i] = ok[i] ? __ldg(a1 + i * tile) : 0.0;
-                    fa2[i] = ok[i] ? __ldg(a2 + i * tile) : 0.0;
+                    const bool ok = mg * MT + i < d.GP;
+                    fa1[i] = ok ? __ldg(a1 + i * tile + (s + 1) * 32) : 0.0;
+                    fa2[i] = ok ? __ldg(a2 + i * tile + (s + 1) * 32) : 0.0;
                 }
-                for (int s = 0; s < KS; ++s) {
-                    double ca1[MT], ca2[MT];
+            } else if (has_next) {
 #pragma unroll
-                    for (int i = 0; i < MT; ++i) { ca1[i] = fa1[i]; ca2[i] = fa2[i]; }
-                    if (s + 1 < KS) {
-#pragma unroll
-                        for (int i = 0; i < MT; ++i) {
-                            fa1[i] = ok[i] ? __ldg(a1 + i * tile + (s + 1) * 32) : 0.0;
-                            fa2[i] = ok[i] ? __ldg(a2 + i * tile + (s + 1) * 32) : 0.0;
-                        }
-                    }
-                    double fb1[NT], fb2[NT];
-#pragma unroll
-                    for (int j = 0; j < NT; ++j) {
-                        fb1[j] = b1[(s * NT + j) * 32];
-                        fb2[j] = b2[(s * NT + j) * 32];
-                    }
-#pragma unroll
-                    for (int i = 0; i < MT; ++i)
-#pragma unroll
-                        for (int j = 0; j < NT; ++j) {
-                            dmma884(acc1[i][j][0], acc1[i][j][1], ca1[i], fb1[j]);
-                            dmma884(acc2[i][j][0], acc2[i][j][1], ca2[i], fb2[j]);
-                        }
+                for (int i = 0; i < MT; ++i) {
+                    const bool ok = nmg * MT + i < d.GP;
+                    fa1[i] = ok ? __ldg(n1 + i * tile) : 0.0;
+                    fa2[i] = ok ? __ldg(n2 + i * tile) : 0.0;
                 }
-                // contract: lane holds T1[(g,a),(b)]; fetch T2[(g,b),(a)] from the transposed lane
-#pragma unroll
-                for (int i = 0; i < MT; ++i)
-#pragma unroll
-                    for (int j = 0; j < NT; ++j) {
-                        double t2r = __shfl_sync(0xffffffffu, acc2[i][j][0], srcl);
-                        double t2i = __shfl_sync(0xffffffffu, acc2[i][j][1], srcl);
-                        er[j] = fma(acc1[i][j][0], t2r, er[j]);
-                        er[j] = fma(-acc1[i][j][1], t2i, er[j]);
-                        ei[j] = fma(acc1[i][j][0], t2i, ei[j]);
-                        ei[j] = fma(acc1[i][j][1], t2r, ei[j]);
-                    }
             }
+            double fb1[NT], fb2[NT];
+#pragma unroll
+            for (int j = 0; j < NT; ++j) {
+                fb1[j] = b1[((size_t)s * NT + j) * 32];
+                fb2[j] = b2[((size_t)s * NT + j) * 32];
+            }
+#pragma unroll
+            for (int i = 0; i < MT; ++i)
+#pragma unroll
+                for (int j = 0; j < NT; ++j) dmma884(acc1[i][j][0], acc1[i][j][1], ca1[i], fb1[j]);
+#pragma unroll
+            for (int i = 0; i < MT; ++i)
+#pragma unroll
+                for (int j = 0; j < NT; ++j) dmma884(acc2[i][j][0], acc2[i][j][1], ca2[i], fb2[j]);
+        }
+        // contract: lane holds T1[(g,a),(b)]; fetch T2[(g,b),(a)] from the transposed lane
+#pragma unroll
+        for (int i = 0; i < MT; ++i)
+#pragma unroll
+            for (int j = 0; j < NT; ++j) {
+                double t2r = __shfl_sync(0xffffffffu, acc2[i][j][0], srcl);
+                double t2i = __shfl_sync(0xffffffffu, acc2[i][j][1], srcl);
+                er[j] = fma(acc1[i][j][0], t2r, er[j]);
+                er[j] = fma(-acc1[i][j][1], t2i, er[j]);
+                ei[j] = fma(acc1[i][j][0], t2i, ei[j]);
+                ei[j] = fma(acc1[i][j][1], t2r, ei[j]);
+            }
+        a1 = n1; a2 = n2; ag = nag; bg = nbg; mg = nmg;
+    }
 
     // ---- reduce over lanes and warps (deterministic) ----
     __syncthreads();
@@ -142,7 +166,7 @@ __global__ void __launch_bounds__(32 * EX_WARPS) exchange_simple_kernel(
     __syncthreads();
     if (tid < NT && w0 + tid < nw) {
         double r = 0.0, i = 0.0;
-        for (int x = 0; x < EX_WARPS; ++x) { r += red[(x * NT + tid) * 2]; i += red[(x * NT + tid) * 2 + 1]; }
+        for (int x = 0; x < WPC; ++x) { r += red[(x * NT + tid) * 2]; i += red[(x * NT + tid) * 2 + 1]; }
         partial[(size_t)u * nw + w0 + tid] = make_double2(r, i);
     }
 }
@@ -196,12 +220,12 @@ __global__ void __launch_bounds__(256) energy_finalize_kernel(
     }
 }
 
-template <int MT, int NT>
-int launch_exchange_simple(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+template <int MT, int NT, int WPC>
+int launch_exchange_simple_w(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     const Dims& d = c->d;
     size_t smem = (size_t)2 * d.NAG * d.KS * NT * 32 * sizeof(double);
-    if (smem < (size_t)EX_WARPS * NT * 2 * sizeof(double)) smem = (size_t)EX_WARPS * NT * 2 * sizeof(double);
-    auto kern = exchange_simple_kernel<MT, NT>;
+    if (smem < (size_t)WPC * NT * 2 * sizeof(double)) smem = (size_t)WPC * NT * 2 * sizeof(double);
+    auto kern = exchange_simple_kernel<MT, NT, WPC>;
     static size_t attr_set = 0;
     if (smem > 48 * 1024 && smem > attr_set) {
         if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
@@ -209,10 +233,30 @@ int launch_exchange_simple(afqmc_ctx* c, const double2* theta, int nw, cudaStrea
             return AFQMC_CUDA_ERROR;
         attr_set = smem;
     }
-    dim3 grid(c->nunits, (nw + NT - 1) / NT);
-    kern<<<grid, 32 * EX_WARPS, smem, st>>>(d, nw, c->units, c->kminus, c->kplus, c->kneg, c->Lx, theta, c->ws_expart);
+    dim3 grid((nw + NT - 1) / NT, c->nunits);
+    kern<<<grid, 32 * WPC, smem, st>>>(d, nw, c->units, c->kminus, c->kplus, c->kneg, c->Lx, theta, c->ws_expart);
     AFQMC_LAUNCH_CHECK(c);
     return AFQMC_OK;
+}
+
+// warps per CTA in {4,5,6,8}: the count that leaves the smallest tail when the tasks are dealt out
+template <int MT, int NT>
+int launch_exchange_simple(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+    const Dims& d = c->d;
+    const int ntask = d.NAG * d.NAG * ((d.GP + MT - 1) / MT);
+    int best = 8;
+    double bestc = 1e30;
+    const int cand[4] = {8, 6, 5, 4};
+    for (int w : cand) {
+        double cost = (double)((ntask + w - 1) / w) * w / ntask;   // >= 1, 1 = perfectly even
+        if (cost < bestc - 1e-9) { bestc = cost; best = w; }
+    }
+    switch (best) {
+        case 4: return launch_exchange_simple_w<MT, NT, 4>(c, theta, nw, st);
+        case 5: return launch_exchange_simple_w<MT, NT, 5>(c, theta, nw, st);
+        case 6: return launch_exchange_simple_w<MT, NT, 6>(c, theta, nw, st);
+        default: return launch_exchange_simple_w<MT, NT, 8>(c, theta, nw, st);
+    }
 }
 
 }  // namespace
