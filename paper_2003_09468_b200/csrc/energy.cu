@@ -32,7 +32,8 @@ __global__ void __launch_bounds__(32 * WPC, 16 / WPC) exchange_simple_kernel(
     const int* __restrict__ kneg, const double* __restrict__ Lx, const double2* __restrict__ theta,
     double2* __restrict__ partial) {
     extern __shared__ __align__(16) double ex_smem[];
-    const int u = blockIdx.y, w0 = blockIdx.x * NT;
+    const int nwg = (nw + NT - 1) / NT;             // walker groups of one unit are adjacent in the grid
+    const int u = blockIdx.x / nwg, w0 = (blockIdx.x % nwg) * NT;
     const int Q = units[4 * u], k = units[4 * u + 1], k2 = units[4 * u + 2];
     const int mQ = kneg[Q];
     const int kq = kminus[k * d.Nk + Q];        // k - Q   : column block of theta for T^Q rows k
@@ -233,7 +234,9 @@ int launch_exchange_simple_w(afqmc_ctx* c, const double2* theta, int nw, cudaStr
             return AFQMC_CUDA_ERROR;
         attr_set = smem;
     }
-    dim3 grid((nw + NT - 1) / NT, c->nunits);
+    const long long nblocks = (long long)((nw + NT - 1) / NT) * c->nunits;   // x only: y/z are capped at 65535
+    if (nblocks > 0x7fffffffLL) return AFQMC_UNSUPPORTED;
+    dim3 grid((unsigned)nblocks);
     kern<<<grid, 32 * WPC, smem, st>>>(d, nw, c->units, c->kminus, c->kplus, c->kneg, c->Lx, theta, c->ws_expart);
     AFQMC_LAUNCH_CHECK(c);
     return AFQMC_OK;
