@@ -157,7 +157,8 @@ long long afqmc_launch_count(const afqmc_ctx* ctx);
  * walkers, as the kernel executes it (pairs (Q,k,k') ~ (-Q,k'-Q,k-Q) computed once). */
 double afqmc_exchange_flops(const afqmc_ctx* ctx, int nw);
 
-/* Options: "exchange_variant" (0 = default/best, 1 = simple direct-load kernel);
+/* Options: "exchange_warps" (0 = automatic, or 4/5/6/8 warps per CTA of the exchange kernel; tuning aid);
+ * "exchange_depth" (0/3 or 2: k-steps of register prefetch in the exchange kernel; tuning aid);
  * "timers" (1 = afqmc_step records a CUDA event after each stage, see afqmc_stage_times). */
 int afqmc_set_option(afqmc_ctx* ctx, const char* name, int value);
 

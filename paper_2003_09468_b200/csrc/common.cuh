@@ -7,6 +7,7 @@
 #include "../../include/afqmc.h"
 
 #define AFQMC_MAX_NK 512
+#define AFQMC_LX_PAD 1024   // doubles of zero padding after Lx (the exchange kernel prefetches up to 4 k-steps ahead)
 // exported C-ABI entry points (everything else in the library has hidden visibility)
 #define AFQMC_API extern "C" __attribute__((visibility("default")))
 
@@ -19,7 +20,8 @@ struct Dims {
     int M, N;      // Nk*m, Nk*n
     int KS;        // k-steps (of 4 reals) covering one complex row of length m: ceil(2m/4)
     int NAG;       // groups of 4 occupied orbitals: ceil(n/4)
-    int GP;        // pairs of Cholesky vectors: ceil(nchol/2)   (exchange M-tiles; also vHS k-steps)
+    int GP;        // pairs of Cholesky vectors: ceil(nchol/2)   (vHS k-steps)
+    int GQ;        // quads of Cholesky vectors: ceil(nchol/4)   (exchange tasks: two M-tiles each)
     int GT;        // octets of Cholesky vectors: ceil(nchol/8)  (force-bias M-tiles)
     int PRT;       // octets of (p,r) pairs: ceil(m*m/8)         (vHS M-tiles)
 };
@@ -37,7 +39,7 @@ struct afqmc_ctx {
     // static tensors
     double2* psi_t; // [Nk][m][n]
     double2* ht;    // [Nk][n][m]   half-rotated one-body
-    double* Lx;     // exchange fragment layout  [Q][k][ag][gp][s][lane]
+    double* Lx;     // exchange fragment layout  [Q][k][ag][gq][s][lane][2]
     double* Lf;     // force-bias fragment layout [Q][gt][k][a][s][lane]
     double* Lv;     // vHS fragment layout        [Q][k][prt][s][lane]
     // workspace (sized by max_walkers)
@@ -55,11 +57,14 @@ struct afqmc_ctx {
     double2* ws_logdet; // [nw]
     int* ws_info;       // [nw]
     long long launches;
-    int opt_exchange;   // 0 default, 1 simple
+    int opt_exchange_depth; // 0/3 = three k-steps of fragment prefetch, 2 = two
+    int opt_exchange_minb;  // tuning aid: 1 = ask for more resident CTAs per SM
+    int opt_exchange_wpc;   // 0 = automatic, else warps per CTA of the exchange kernel (4,5,6,8)
     int opt_timers;     // record stage events in afqmc_step
     cudaEvent_t ev[AFQMC_NUM_STAGES + 1];
     int ev_valid;
     int smem_optin;     // max dynamic shared memory per block (bytes)
+    int smem_sm;        // shared memory per SM (bytes)
     int num_sms;
 };
 

@@ -22,8 +22,10 @@ AFQMC_API const char* afqmc_strerror(int code) {
 // order: lane l holds A[row = l>>2][kk = l&3]; the k-step s covers reals 4s..4s+3 of the
 // real-embedded K index (complex index j>>1, part j&1 with j = 4s+kk).
 //
-//  Lx (exchange, a9):   [Q][k][ag][gp][s][lane]   rows (gl = row>>2, al = row&3):
-//                        gamma = 2gp+gl, a = 4ag+al;  K = (r, part) of Lh[Q][k][a][gamma][r]
+//  Lx (exchange, a9):   [Q][k][ag][gq][s][lane][i]  two M-tiles i = 0,1 per gamma-quad gq, interleaved
+//                        per lane (one LDG.128 feeds both); rows (gl = row>>2, al = row&3):
+//                        gamma = 4gq+2i+gl, a = 4ag+al;  K = (r, part) of Lh[Q][k][a][gamma][r]
+//                        (+ AFQMC_LX_PAD zero doubles at the end: the kernel's prefetch may run past the last task)
 //  Lf (force bias, a4): [Q][gt][k][a][s][lane]    rows gamma = 8gt+row;  K = (r, part), per (k,a)
 //  Lv (vHS, a5):        [Q][k][prt][s][lane]      rows pr = 8prt+row (p = pr/m, r = pr%m);
 //                        K = (gamma, part) of L[Q][k][gamma][p][r]
@@ -48,17 +50,18 @@ __global__ void pack_Lx_kernel(Dims d, const double2* __restrict__ L, const doub
     for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total;
          idx += (size_t)gridDim.x * blockDim.x) {
         size_t t = idx;
+        int i = (int)(t & 1); t >>= 1;
         int lane = (int)(t & 31); t >>= 5;
         int s = (int)(t % d.KS); t /= d.KS;
-        int gp = (int)(t % d.GP); t /= d.GP;
+        int gq = (int)(t % d.GQ); t /= d.GQ;
         int ag = (int)(t % d.NAG); t /= d.NAG;
         int k = (int)(t % d.Nk);
         int Q = (int)(t / d.Nk);
         int row = lane >> 2, kk = lane & 3;
-        int gam = 2 * gp + (row >> 2), a = 4 * ag + (row & 3);
+        int gam = 4 * gq + 2 * i + (row >> 2), a = 4 * ag + (row & 3);
         int j = 4 * s + kk, r = j >> 1, c = j & 1;
         double v = 0.0;
-        if (a < d.n && gam < d.nchol && r < d.m) {
+        if (Q < d.Nk && a < d.n && gam < d.nchol && r < d.m) {   // Q >= Nk: the zero pad
             double2 z = half_rot_elem(L, psi_t, d, Q, k, a, gam, r);
             v = c ? z.y : z.x;
         }
@@ -180,6 +183,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     d.KS = (2 * d.m + 3) / 4;
     d.NAG = (d.n + 3) / 4;
     d.GP = (d.nchol + 1) / 2;
+    d.GQ = (d.nchol + 3) / 4;
     d.GT = (d.nchol + 7) / 8;
     d.PRT = (d.m * d.m + 7) / 8;
     c->max_walkers = dims->max_walkers;
@@ -189,6 +193,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     if (cudaGetDevice(&dev) != cudaSuccess) { delete c; return AFQMC_CUDA_ERROR; }
     cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&c->smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
 
     // ---- k-point tables and exchange work units (host) ----
     const int Nk = d.Nk;
@@ -218,7 +223,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
 
     int rc = AFQMC_OK;
     auto A = [&](int r) { if (rc == AFQMC_OK) rc = r; };
-    const size_t nLx = (size_t)Nk * Nk * d.NAG * d.GP * d.KS * 32;
+    const size_t nLx = (size_t)Nk * Nk * d.NAG * d.GQ * d.KS * 64 + AFQMC_LX_PAD;
     const size_t nLf = (size_t)Nk * d.GT * Nk * d.n * d.KS * 32;
     const size_t nLv = (size_t)Nk * Nk * d.PRT * d.GP * 32;
     const int LD = d.N | 1;
@@ -287,9 +292,18 @@ AFQMC_API double afqmc_exchange_flops(const afqmc_ctx* c, int nw) {
 
 AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
     if (!c || !name) return AFQMC_INVALID_ARGUMENT;
-    if (strcmp(name, "exchange_variant") == 0) {
-        if (value < 0 || value > 1) return AFQMC_INVALID_ARGUMENT;
-        c->opt_exchange = value;
+    if (strcmp(name, "exchange_warps") == 0) {
+        if (value != 0 && value != 2 && value != 4 && value != 5 && value != 6 && value != 8) return AFQMC_INVALID_ARGUMENT;
+        c->opt_exchange_wpc = value;
+        return AFQMC_OK;
+    }
+    if (strcmp(name, "exchange_minblocks") == 0) {
+        c->opt_exchange_minb = value ? 1 : 0;
+        return AFQMC_OK;
+    }
+    if (strcmp(name, "exchange_depth") == 0) {
+        if (value != 0 && value != 2 && value != 3) return AFQMC_INVALID_ARGUMENT;
+        c->opt_exchange_depth = value;
         return AFQMC_OK;
     }
     if (strcmp(name, "timers") == 0) {

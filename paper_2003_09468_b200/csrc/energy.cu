@@ -18,16 +18,23 @@ namespace {
 __device__ __forceinline__ int transpose_lane(int lane) { return (lane & 16) | ((lane & 3) << 2) | ((lane >> 2) & 3); }
 
 // ---------------------------------------------------------------------------------------------
-// Variant 1 ("simple"): B fragments (theta blocks, real-embedded) staged once per CTA in shared
-// memory; A fragments (Lx tiles) loaded straight from global/L2 in lane order, software-pipelined
-// one k-step ahead ACROSS tasks so that no task starts with an exposed L2 round trip.
-// CTA = (unit, group of NT walkers), WPC warps.  A warp task is a group of MT gamma-pair tiles; the
-// host picks WPC so that the tasks divide evenly over the warps (no tail at the final barrier).
-// Walker groups of one unit are adjacent in the grid so that the Lx blocks of a unit are fetched
-// from HBM once and shared through L2.
+// Exchange kernel.  CTA = (unit, group of NT walkers), WPC warps.
+//  * B fragments (the two theta blocks of the unit, real-embedded) are staged once per CTA in
+//    shared memory in fragment order.
+//  * A fragments (Lx) are a LINEAR stream per warp: a warp task is one gamma-quad (two DMMA m-tiles,
+//    rows (gamma pair, a)) and the layout Lx[Q][k][ag][gq][s][lane][2] makes every k-step of a task one
+//    coalesced 512-byte LDG.128 per operand; consecutive tasks of a warp are consecutive in memory.
+//  * Both fragment streams run D k-steps ahead of the DMMAs in statically rotated register buffers
+//    (the loop over the warp's flattened (task, k-step) sequence is unrolled by D), so neither the L2
+//    round trip of A nor the shared-memory latency of B is exposed, also across task boundaries.
+//    With n <= 4 (LINEAR) the refill is branch-free pointer arithmetic, so the loads of a k-step are
+//    scheduled between its DMMAs; the refill may run up to D k-steps past the warp's last task, into
+//    the next block or the zero pad after Lx (loaded, never used).
+//  * The host picks WPC so that the tasks divide evenly over the warps; walker groups of one unit are
+//    adjacent in the grid so that the Lx blocks of a unit are fetched from HBM once and shared in L2.
 // ---------------------------------------------------------------------------------------------
-template <int MT, int NT, int WPC>
-__global__ void __launch_bounds__(32 * WPC, 16 / WPC) exchange_simple_kernel(
+template <int NT, int WPC, int D, bool LINEAR, int MINB>
+__global__ void __launch_bounds__(32 * WPC, MINB) exchange_kernel(
     Dims d, int nw, const int* __restrict__ units, const int* __restrict__ kminus, const int* __restrict__ kplus,
     const int* __restrict__ kneg, const double* __restrict__ Lx, const double2* __restrict__ theta,
     double2* __restrict__ partial) {
@@ -39,28 +46,91 @@ __global__ void __launch_bounds__(32 * WPC, 16 / WPC) exchange_simple_kernel(
     const int kq = kminus[k * d.Nk + Q];        // k - Q   : column block of theta for T^Q rows k
     const int k2pq = kplus[k2 * d.Nk + Q];      // k2 + Q  : column block of theta for T^{-Q} rows k2
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int KS = d.KS, NAG = d.NAG;
+    const int KS = d.KS, NAG = d.NAG, GQ = d.GQ;
     // Bs[which][grp][s][j][lane]: which = 0 -> theta[(k2,b),(k-Q,r)], 1 -> theta[(k,a),(k2+Q,s)]
-    const size_t bs_half = (size_t)NAG * KS * NT * 32;
+    const int bs_step = NT * 32, bs_grp = KS * bs_step, bs_half = NAG * bs_grp;
 
-    // ---- stage B fragments: one (which, grp, walker) fragment column per warp pass, lane = fragment lane ----
-    {
-        const int kkk = lane & 3, col = lane >> 2;
-        const int dd = col & 1, cc = kkk & 1;
-        const bool neg = cc && !dd;
-        for (int c = warp; c < 2 * NAG * NT; c += WPC) {
-            const int jw = c % NT, grp = (c / NT) % NAG, which = c / (NT * NAG);
-            const int orb = 4 * grp + (col >> 1), w = w0 + jw;
-            const int rowblk = which == 0 ? k2 : k, colblk = which == 0 ? kq : k2pq;
-            const bool ok = orb < d.n && w < nw;
-            const double* src = reinterpret_cast<const double*>(
-                theta + ((size_t)(ok ? w : 0) * d.N + rowblk * d.n + (ok ? orb : 0)) * d.M + (size_t)colblk * d.m + (kkk >> 1)) + (cc ^ dd);
-            double* dst = ex_smem + which * bs_half + ((size_t)grp * KS * NT + jw) * 32 + lane;
-            for (int s = 0; s < KS; ++s) {
-                double v = 0.0;
-                if (ok && 2 * s + (kkk >> 1) < d.m) v = __ldg(src + 4 * s);
-                dst[(size_t)s * NT * 32] = neg ? -v : v;
+    // ---- this warp's contiguous share of the CTA's tasks t = (ag*NAG + bg)*GQ + gq ----
+    const int ntask = NAG * NAG * GQ;
+    const int t_begin = (int)((long long)warp * ntask / WPC), t_end = (int)((long long)(warp + 1) * ntask / WPC);
+    const int total = (t_end - t_begin) * KS;                       // k-steps of this warp
+    const size_t blk1 = ((size_t)Q * d.Nk + k) * NAG, blk2 = ((size_t)mQ * d.Nk + k2) * NAG;
+    const size_t task_doubles = (size_t)KS * 64;
+    // loader state: runs D k-steps ahead of the compute state
+    int lt = t_begin, ls = 0, lg = 0;
+    const double2 *la1, *la2;
+    const double *lb1, *lb2;
+    auto task_ptrs = [&](int t) {
+        const int gq = t % GQ, ab = t / GQ, bg = ab % NAG, ag = ab / NAG;
+        la1 = reinterpret_cast<const double2*>(Lx + ((blk1 + ag) * GQ + gq) * task_doubles) + lane;
+        la2 = reinterpret_cast<const double2*>(Lx + ((blk2 + bg) * GQ + gq) * task_doubles) + lane;
+        lb1 = ex_smem + bg * bs_grp + lane;
+        lb2 = ex_smem + bs_half + ag * bs_grp + lane;
+    };
+    auto loader_advance = [&]() {
+        if (LINEAR) {                    // one (ag,bg): A is contiguous across tasks, B wraps every KS steps
+            la1 += 32; la2 += 32;
+            const bool wrap = ++ls == KS;
+            const int db = wrap ? -(KS - 1) * bs_step : bs_step;
+            lb1 += db; lb2 += db;
+            ls = wrap ? 0 : ls;
+        } else {
+            ++lg;
+            if (++ls == KS) {
+                ls = 0; ++lt;
+                if (lg < total) task_ptrs(lt);
+            } else {
+                la1 += 32; la2 += 32; lb1 += bs_step; lb2 += bs_step;
             }
+        }
+    };
+    double2 fa1[D], fa2[D];
+    double fb1[D][NT], fb2[D][NT];
+    task_ptrs(total > 0 ? lt : 0);
+    // A prologue: the global loads are issued before the staging below, which hides their latency
+#pragma unroll
+    for (int q = 0; q < D; ++q) {
+        fa1[q] = fa2[q] = make_double2(0.0, 0.0);
+        if (LINEAR) {
+            if (total > 0) { fa1[q] = __ldg(la1 + q * 32); fa2[q] = __ldg(la2 + q * 32); }
+        } else if (q < total) {         // D <= KS is guaranteed by the host, so the prologue stays in task lt
+            fa1[q] = __ldg(la1 + q * 32); fa2[q] = __ldg(la2 + q * 32);
+        }
+    }
+
+    // ---- stage B fragments.  One thread per complex theta element (b, r): all loads of the CTA are
+    // independent (one L2 round trip in total), and each element feeds the four fragment entries
+    //   (kk = 2(r&1)+c, col = 2(b&3)+d):  d=0: (re, -im) for c = 0,1;  d=1: (im, re).
+    {
+        const int per_which = NAG * 4 * NT * 2 * KS;             // padded (orb, walker, r) space
+        for (int e = tid; e < 2 * per_which; e += 32 * WPC) {
+            const int which = e / per_which;
+            int x = e - which * per_which;
+            const int bl = x & 3; x >>= 2;                       // orbital inside its group of 4
+            const int jw = x % NT; x /= NT;
+            const int grp = x % NAG, r = x / NAG;                // r < 2*KS
+            const int orb = 4 * grp + bl, w = w0 + jw;
+            const int rowblk = which == 0 ? k2 : k, colblk = which == 0 ? kq : k2pq;
+            double2 v = make_double2(0.0, 0.0);
+            if (orb < d.n && w < nw && r < d.m)
+                v = __ldg(theta + ((size_t)w * d.N + rowblk * d.n + orb) * d.M + (size_t)colblk * d.m + r);
+            double* dst = ex_smem + which * bs_half + ((grp * KS + (r >> 1)) * NT + jw) * 32 + bl * 8 + 2 * (r & 1);
+            *reinterpret_cast<double2*>(dst) = make_double2(v.x, -v.y);       // d = 0: lanes (kk = 2(r&1)+{0,1}, col = 2bl)
+            *reinterpret_cast<double2*>(dst + 4) = make_double2(v.y, v.x);    // d = 1: col = 2bl+1
+        }
+    }
+    __syncthreads();   // B fragments staged
+
+    // B prologue, and bring the loader state to step D
+#pragma unroll
+    for (int q = 0; q < D; ++q) {
+        if (LINEAR || q < total) {
+#pragma unroll
+            for (int j = 0; j < NT; ++j) { fb1[q][j] = lb1[j * 32]; fb2[q][j] = lb2[j * 32]; }
+            loader_advance();
+        } else {
+#pragma unroll
+            for (int j = 0; j < NT; ++j) fb1[q][j] = fb2[q][j] = 0.0;
         }
     }
 
@@ -68,93 +138,56 @@ __global__ void __launch_bounds__(32 * WPC, 16 / WPC) exchange_simple_kernel(
 #pragma unroll
     for (int j = 0; j < NT; ++j) er[j] = ei[j] = 0.0;
     const int srcl = transpose_lane(lane);
-    const int ngrp = (d.GP + MT - 1) / MT;
-    const size_t tile = (size_t)KS * 32;
-    // flattened task list of this warp: t = warp, warp+WPC, ... < NAG*NAG*ngrp ; t -> (ag, bg, mg)
-    const int ntask = NAG * NAG * ngrp;
-    auto task_ptrs = [&](int t, const double*& a1, const double*& a2, int& ag, int& bg, int& mg) {
-        mg = t % ngrp;
-        const int ab = t / ngrp;
-        bg = ab % NAG; ag = ab / NAG;
-        a1 = Lx + ((((size_t)Q * d.Nk + k) * NAG + ag) * d.GP + (size_t)mg * MT) * tile + lane;
-        a2 = Lx + ((((size_t)mQ * d.Nk + k2) * NAG + bg) * d.GP + (size_t)mg * MT) * tile + lane;
-    };
-    const double *a1 = nullptr, *a2 = nullptr;
-    int ag = 0, bg = 0, mg = 0;
-    double fa1[MT], fa2[MT];
-    int t = warp;
-    if (t < ntask) {
-        task_ptrs(t, a1, a2, ag, bg, mg);
+    double acc1[2][NT][2], acc2[2][NT][2];
 #pragma unroll
-        for (int i = 0; i < MT; ++i) {
-            const bool ok = mg * MT + i < d.GP;
-            fa1[i] = ok ? __ldg(a1 + i * tile) : 0.0;
-            fa2[i] = ok ? __ldg(a2 + i * tile) : 0.0;
-        }
-    }
-    __syncthreads();   // B fragments staged
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int j = 0; j < NT; ++j) acc1[i][j][0] = acc1[i][j][1] = acc2[i][j][0] = acc2[i][j][1] = 0.0;
 
-    for (; t < ntask; t += WPC) {
-        const double* b1 = ex_smem + (size_t)bg * KS * NT * 32 + lane;
-        const double* b2 = ex_smem + bs_half + (size_t)ag * KS * NT * 32 + lane;
-        // pointers of the next task (for the cross-task prefetch at the last k-step)
-        const double *n1 = a1, *n2 = a2;
-        int nag = ag, nbg = bg, nmg = mg;
-        const bool has_next = t + WPC < ntask;
-        if (has_next) task_ptrs(t + WPC, n1, n2, nag, nbg, nmg);
-        double acc1[MT][NT][2], acc2[MT][NT][2];
+    int cs = 0;   // k-step of the compute state inside its task
+    // one k-step on register buffer q: 4*NT DMMAs, refill of the buffer, contraction at the end of a task
+    auto kstep = [&](const int q) {
 #pragma unroll
-        for (int i = 0; i < MT; ++i)
-#pragma unroll
-            for (int j = 0; j < NT; ++j) acc1[i][j][0] = acc1[i][j][1] = acc2[i][j][0] = acc2[i][j][1] = 0.0;
-        for (int s = 0; s < KS; ++s) {
-            double ca1[MT], ca2[MT];
-#pragma unroll
-            for (int i = 0; i < MT; ++i) { ca1[i] = fa1[i]; ca2[i] = fa2[i]; }
-            if (s + 1 < KS) {
-#pragma unroll
-                for (int i = 0; i < MT; ++i) {
-                    const bool ok = mg * MT + i < d.GP;
-                    fa1[i] = ok ? __ldg(a1 + i * tile + (s + 1) * 32) : 0.0;
-                    fa2[i] = ok ? __ldg(a2 + i * tile + (s + 1) * 32) : 0.0;
-                }
-            } else if (has_next) {
-#pragma unroll
-                for (int i = 0; i < MT; ++i) {
-                    const bool ok = nmg * MT + i < d.GP;
-                    fa1[i] = ok ? __ldg(n1 + i * tile) : 0.0;
-                    fa2[i] = ok ? __ldg(n2 + i * tile) : 0.0;
-                }
-            }
-            double fb1[NT], fb2[NT];
-#pragma unroll
-            for (int j = 0; j < NT; ++j) {
-                fb1[j] = b1[((size_t)s * NT + j) * 32];
-                fb2[j] = b2[((size_t)s * NT + j) * 32];
-            }
-#pragma unroll
-            for (int i = 0; i < MT; ++i)
-#pragma unroll
-                for (int j = 0; j < NT; ++j) dmma884(acc1[i][j][0], acc1[i][j][1], ca1[i], fb1[j]);
-#pragma unroll
-            for (int i = 0; i < MT; ++i)
-#pragma unroll
-                for (int j = 0; j < NT; ++j) dmma884(acc2[i][j][0], acc2[i][j][1], ca2[i], fb2[j]);
+        for (int j = 0; j < NT; ++j) {
+            dmma884(acc1[0][j][0], acc1[0][j][1], fa1[q].x, fb1[q][j]);
+            dmma884(acc1[1][j][0], acc1[1][j][1], fa1[q].y, fb1[q][j]);
         }
-        // contract: lane holds T1[(g,a),(b)]; fetch T2[(g,b),(a)] from the transposed lane
 #pragma unroll
-        for (int i = 0; i < MT; ++i)
+        for (int j = 0; j < NT; ++j) {
+            dmma884(acc2[0][j][0], acc2[0][j][1], fa2[q].x, fb2[q][j]);
+            dmma884(acc2[1][j][0], acc2[1][j][1], fa2[q].y, fb2[q][j]);
+        }
+        if (LINEAR || lg < total) {      // refill buffer q with the k-step D ahead
+            fa1[q] = __ldg(la1); fa2[q] = __ldg(la2);
 #pragma unroll
-            for (int j = 0; j < NT; ++j) {
-                double t2r = __shfl_sync(0xffffffffu, acc2[i][j][0], srcl);
-                double t2i = __shfl_sync(0xffffffffu, acc2[i][j][1], srcl);
-                er[j] = fma(acc1[i][j][0], t2r, er[j]);
-                er[j] = fma(-acc1[i][j][1], t2i, er[j]);
-                ei[j] = fma(acc1[i][j][0], t2i, ei[j]);
-                ei[j] = fma(acc1[i][j][1], t2r, ei[j]);
-            }
-        a1 = n1; a2 = n2; ag = nag; bg = nbg; mg = nmg;
+            for (int j = 0; j < NT; ++j) { fb1[q][j] = lb1[j * 32]; fb2[q][j] = lb2[j * 32]; }
+            loader_advance();
+        }
+        if (++cs == KS) {
+            cs = 0;
+            // contract: lane holds T1[(g,a),(b)]; fetch T2[(g,b),(a)] from the transposed lane
+#pragma unroll
+            for (int i = 0; i < 2; ++i)
+#pragma unroll
+                for (int j = 0; j < NT; ++j) {
+                    double t2r = __shfl_sync(0xffffffffu, acc2[i][j][0], srcl);
+                    double t2i = __shfl_sync(0xffffffffu, acc2[i][j][1], srcl);
+                    er[j] = fma(acc1[i][j][0], t2r, er[j]);
+                    er[j] = fma(-acc1[i][j][1], t2i, er[j]);
+                    ei[j] = fma(acc1[i][j][0], t2i, ei[j]);
+                    ei[j] = fma(acc1[i][j][1], t2r, ei[j]);
+                    acc1[i][j][0] = acc1[i][j][1] = acc2[i][j][0] = acc2[i][j][1] = 0.0;
+                }
+        }
+    };
+    const int nfull = total - total % D;
+    for (int g0 = 0; g0 < nfull; g0 += D) {
+#pragma unroll
+        for (int q = 0; q < D; ++q) kstep(q);
     }
+#pragma unroll
+    for (int q = 0; q < D - 1; ++q)
+        if (nfull + q < total) kstep(q);
 
     // ---- reduce over lanes and warps (deterministic) ----
     __syncthreads();
@@ -221,12 +254,12 @@ __global__ void __launch_bounds__(256) energy_finalize_kernel(
     }
 }
 
-template <int MT, int NT, int WPC>
-int launch_exchange_simple_w(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+template <int NT, int WPC, int D, bool LINEAR, int MINB>
+int launch_exchange_cfg(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     const Dims& d = c->d;
     size_t smem = (size_t)2 * d.NAG * d.KS * NT * 32 * sizeof(double);
     if (smem < (size_t)WPC * NT * 2 * sizeof(double)) smem = (size_t)WPC * NT * 2 * sizeof(double);
-    auto kern = exchange_simple_kernel<MT, NT, WPC>;
+    auto kern = exchange_kernel<NT, WPC, D, LINEAR, MINB>;
     static size_t attr_set = 0;
     if (smem > 48 * 1024 && smem > attr_set) {
         if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
@@ -242,23 +275,51 @@ int launch_exchange_simple_w(afqmc_ctx* c, const double2* theta, int nw, cudaStr
     return AFQMC_OK;
 }
 
-// warps per CTA in {4,5,6,8}: the count that leaves the smallest tail when the tasks are dealt out
-template <int MT, int NT>
-int launch_exchange_simple(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+template <int NT, int WPC, int MINB>
+int launch_exchange_wm(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+    const bool linear = c->d.NAG == 1;
+    const int depth = (c->opt_exchange_depth == 3 && c->d.KS >= 3) ? 3 : (c->d.KS >= 2 ? 2 : 1);
+    if (depth == 3) return linear ? launch_exchange_cfg<NT, WPC, 3, true, MINB>(c, theta, nw, st)
+                                  : launch_exchange_cfg<NT, WPC, 3, false, MINB>(c, theta, nw, st);
+    if (depth == 2) return linear ? launch_exchange_cfg<NT, WPC, 2, true, MINB>(c, theta, nw, st)
+                                  : launch_exchange_cfg<NT, WPC, 2, false, MINB>(c, theta, nw, st);
+    return launch_exchange_cfg<NT, WPC, 1, false, MINB>(c, theta, nw, st);     // m = 1: a single k-step per task
+}
+
+template <int NT, int WPC>
+int launch_exchange_w(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+    constexpr int MB0 = WPC == 2 ? 4 : (WPC > 6 ? 1 : 2), MB1 = WPC == 2 ? 6 : (WPC == 4 ? 3 : MB0);
+    if (c->opt_exchange_minb == 1) return launch_exchange_wm<NT, WPC, MB1>(c, theta, nw, st);
+    return launch_exchange_wm<NT, WPC, MB0>(c, theta, nw, st);
+}
+
+// Warps per CTA: the count in {2,4,6} that keeps the most warps resident per SM (up to 12 = 3 per
+// scheduler; limited by the staged theta blocks in shared memory and by ~160 registers per thread),
+// then the one that deals the tasks out most evenly, then the smallest (small CTAs drift out of
+// lockstep, so their prologues overlap other CTAs' DMMAs).
+template <int NT>
+int launch_exchange(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     const Dims& d = c->d;
-    const int ntask = d.NAG * d.NAG * ((d.GP + MT - 1) / MT);
-    int best = 8;
-    double bestc = 1e30;
-    const int cand[4] = {8, 6, 5, 4};
-    for (int w : cand) {
-        double cost = (double)((ntask + w - 1) / w) * w / ntask;   // >= 1, 1 = perfectly even
-        if (cost < bestc - 1e-9) { bestc = cost; best = w; }
+    const int ntask = d.NAG * d.NAG * d.GQ;
+    int best = c->opt_exchange_wpc;
+    if (best == 0) {
+        const size_t smem = (size_t)2 * d.NAG * d.KS * NT * 32 * sizeof(double) + 1024;
+        double bests = -1.0;
+        const int cand[3] = {2, 4, 6};
+        for (int w : cand) {
+            const int by_smem = (int)((size_t)c->smem_sm / smem), by_regs = 65536 / (160 * 32 * w);
+            const int warps = (by_smem < by_regs ? by_smem : by_regs) * w;
+            const double cost = (double)((ntask + w - 1) / w) * w / ntask;   // >= 1, 1 = perfectly even
+            const double score = (warps < 12 ? warps : 12) / cost;
+            if (score > bests + 1e-9) { bests = score; best = w; }
+        }
     }
     switch (best) {
-        case 4: return launch_exchange_simple_w<MT, NT, 4>(c, theta, nw, st);
-        case 5: return launch_exchange_simple_w<MT, NT, 5>(c, theta, nw, st);
-        case 6: return launch_exchange_simple_w<MT, NT, 6>(c, theta, nw, st);
-        default: return launch_exchange_simple_w<MT, NT, 8>(c, theta, nw, st);
+        case 2: return launch_exchange_w<NT, 2>(c, theta, nw, st);
+        case 4: return launch_exchange_w<NT, 4>(c, theta, nw, st);
+        case 5: return launch_exchange_w<NT, 5>(c, theta, nw, st);
+        case 8: return launch_exchange_w<NT, 8>(c, theta, nw, st);
+        default: return launch_exchange_w<NT, 6>(c, theta, nw, st);
     }
 }
 
@@ -269,8 +330,8 @@ int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* en
     int rc = afqmc_i_force_bias(c, theta, nw, c->ws_vbias, st);     // steps 2(d): the traces are the force bias
     if (rc != AFQMC_OK) return rc;
     afqmc_mark(c, 6, st);
-    if (nw >= 3) rc = launch_exchange_simple<2, 4>(c, theta, nw, st);
-    else rc = launch_exchange_simple<2, 2>(c, theta, nw, st);
+    if (nw >= 3) rc = launch_exchange<4>(c, theta, nw, st);
+    else rc = launch_exchange<2>(c, theta, nw, st);
     if (rc != AFQMC_OK) return rc;
     afqmc_mark(c, 7, st);
     energy_finalize_kernel<<<nw, 256, 0, st>>>(d, nw, c->nunits, c->units, c->kneg, c->ht, theta, c->ws_vbias,
