@@ -7,6 +7,7 @@
 #include "../../include/afqmc.h"
 
 #define AFQMC_MAX_NK 512
+#define AFQMC_FB_MAXKC 16   // max K chunks of the force-bias kernel (sizes its partial-sum workspace)
 #define AFQMC_LX_PAD 1024   // doubles of zero padding after Lx (the exchange kernel prefetches up to 4 k-steps ahead)
 // exported C-ABI entry points (everything else in the library has hidden visibility)
 #define AFQMC_API extern "C" __attribute__((visibility("default")))
@@ -22,7 +23,7 @@ struct Dims {
     int NAG;       // groups of 4 occupied orbitals: ceil(n/4)
     int GP;        // pairs of Cholesky vectors: ceil(nchol/2)   (vHS k-steps)
     int GQ;        // quads of Cholesky vectors: ceil(nchol/4)   (exchange tasks: two M-tiles each)
-    int GT;        // octets of Cholesky vectors: ceil(nchol/8)  (force-bias M-tiles)
+    int GT2;       // 16-groups of Cholesky vectors: ceil(nchol/16) (force-bias M-tile pairs)
     int PRT;       // octets of (p,r) pairs: ceil(m*m/8)         (vHS M-tiles)
 };
 
@@ -40,7 +41,7 @@ struct afqmc_ctx {
     double2* psi_t; // [Nk][m][n]
     double2* ht;    // [Nk][n][m]   half-rotated one-body
     double* Lx;     // exchange fragment layout  [Q][k][ag][gq][s][lane][2]
-    double* Lf;     // force-bias fragment layout [Q][gt][k][a][s][lane]
+    double* Lf;     // force-bias fragment layout [Q][gtp][k][a][s][lane][2]
     double* Lv;     // vHS fragment layout        [Q][k][prt][s][lane]
     // workspace (sized by max_walkers)
     double2* ws_O;      // [nw][N][LD]  elimination workspace when the matrix does not fit shared memory
@@ -51,6 +52,7 @@ struct afqmc_ctx {
     double2* ws_vhs;    // [nw][M][M]
     double2* ws_T;      // [2][nw][M][N] Taylor ping-pong
     double2* ws_expart; // [nunits][nw]  exchange partial sums
+    double2* ws_fbpart; // [AFQMC_FB_MAXKC][nw][Nk][nchol] force-bias K-chunk partial sums
     double* ws_x;       // [nw][Nk][nchol] (host-entry staging)
     double2* ws_phi;    // [nw][M][N]     (host-entry staging)
     double2* ws_energy; // [nw][3]
@@ -58,6 +60,8 @@ struct afqmc_ctx {
     int* ws_info;       // [nw]
     long long launches;
     int opt_exchange_depth; // 0/3 = three k-steps of fragment prefetch, 2 = two
+    int opt_fb_tile;        // tuning aid: warp tile of the force-bias kernel for > 16 walkers (0: 2x8, 1: 4x8, 2: 4x4 m x n tiles)
+    int opt_fb_pf;          // L2 prefetch distance (k-steps) of the Lf stream in the force-bias kernel
     int opt_exchange_minb;  // tuning aid: 1 = ask for more resident CTAs per SM
     int opt_exchange_wpc;   // 0 = automatic, else warps per CTA of the exchange kernel (4,5,6,8)
     int opt_timers;     // record stage events in afqmc_step

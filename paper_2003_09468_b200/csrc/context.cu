@@ -26,7 +26,8 @@ AFQMC_API const char* afqmc_strerror(int code) {
 //                        per lane (one LDG.128 feeds both); rows (gl = row>>2, al = row&3):
 //                        gamma = 4gq+2i+gl, a = 4ag+al;  K = (r, part) of Lh[Q][k][a][gamma][r]
 //                        (+ AFQMC_LX_PAD zero doubles at the end: the kernel's prefetch may run past the last task)
-//  Lf (force bias, a4): [Q][gt][k][a][s][lane]    rows gamma = 8gt+row;  K = (r, part), per (k,a)
+//  Lf (force bias, a4): [Q][gtp][k][a][s][lane][i] two M-tiles i = 0,1 per 16 gammas, interleaved per lane;
+//                        rows gamma = 16gtp+8i+row;  K = (r, part), per (k,a); one contiguous K stream per gtp
 //  Lv (vHS, a5):        [Q][k][prt][s][lane]      rows pr = 8prt+row (p = pr/m, r = pr%m);
 //                        K = (gamma, part) of L[Q][k][gamma][p][r]
 // Out-of-range rows / K entries are stored as zeros, so kernels never branch on tails.
@@ -74,14 +75,15 @@ __global__ void pack_Lf_kernel(Dims d, const double2* __restrict__ L, const doub
     for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total;
          idx += (size_t)gridDim.x * blockDim.x) {
         size_t t = idx;
+        int i = (int)(t & 1); t >>= 1;
         int lane = (int)(t & 31); t >>= 5;
         int s = (int)(t % d.KS); t /= d.KS;
         int a = (int)(t % d.n); t /= d.n;
         int k = (int)(t % d.Nk); t /= d.Nk;
-        int gt = (int)(t % d.GT);
-        int Q = (int)(t / d.GT);
+        int gtp = (int)(t % d.GT2);
+        int Q = (int)(t / d.GT2);
         int row = lane >> 2, kk = lane & 3;
-        int gam = 8 * gt + row;
+        int gam = 16 * gtp + 8 * i + row;
         int j = 4 * s + kk, r = j >> 1, c = j & 1;
         double v = 0.0;
         if (gam < d.nchol && r < d.m) {
@@ -152,7 +154,7 @@ AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     if (!c) return;
     void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lx, c->Lf, c->Lv,
                     c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T,
-                    c->ws_expart, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info};
+                    c->ws_expart, c->ws_fbpart, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     for (cudaEvent_t e : c->ev)
@@ -184,9 +186,10 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     d.NAG = (d.n + 3) / 4;
     d.GP = (d.nchol + 1) / 2;
     d.GQ = (d.nchol + 3) / 4;
-    d.GT = (d.nchol + 7) / 8;
+    d.GT2 = (d.nchol + 15) / 16;
     d.PRT = (d.m * d.m + 7) / 8;
     c->max_walkers = dims->max_walkers;
+    c->opt_fb_pf = 8;
     const int nw = c->max_walkers;
 
     int dev = 0;
@@ -224,7 +227,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     int rc = AFQMC_OK;
     auto A = [&](int r) { if (rc == AFQMC_OK) rc = r; };
     const size_t nLx = (size_t)Nk * Nk * d.NAG * d.GQ * d.KS * 64 + AFQMC_LX_PAD;
-    const size_t nLf = (size_t)Nk * d.GT * Nk * d.n * d.KS * 32;
+    const size_t nLf = (size_t)Nk * d.GT2 * Nk * d.n * d.KS * 64;
     const size_t nLv = (size_t)Nk * Nk * d.PRT * d.GP * 32;
     const int LD = d.N | 1;
     A(dev_alloc(&c->kminus, (size_t)Nk * Nk));
@@ -244,6 +247,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     A(dev_alloc(&c->ws_vhs, (size_t)nw * d.M * d.M));
     A(dev_alloc(&c->ws_T, (size_t)2 * nw * d.M * d.N));
     A(dev_alloc(&c->ws_expart, (size_t)c->nunits * nw));
+    A(dev_alloc(&c->ws_fbpart, (size_t)AFQMC_FB_MAXKC * nw * Nk * d.nchol));
     A(dev_alloc(&c->ws_x, (size_t)nw * Nk * d.nchol));
     A(dev_alloc(&c->ws_phi, (size_t)nw * d.M * d.N));
     A(dev_alloc(&c->ws_energy, (size_t)nw * 3));
@@ -295,6 +299,16 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
     if (strcmp(name, "exchange_warps") == 0) {
         if (value != 0 && value != 2 && value != 4 && value != 5 && value != 6 && value != 8) return AFQMC_INVALID_ARGUMENT;
         c->opt_exchange_wpc = value;
+        return AFQMC_OK;
+    }
+    if (strcmp(name, "force_bias_tile") == 0) {
+        if (value < 0 || value > 2) return AFQMC_INVALID_ARGUMENT;
+        c->opt_fb_tile = value;
+        return AFQMC_OK;
+    }
+    if (strcmp(name, "force_bias_prefetch") == 0) {
+        if (value < 0 || value > 256) return AFQMC_INVALID_ARGUMENT;
+        c->opt_fb_pf = value;
         return AFQMC_OK;
     }
     if (strcmp(name, "exchange_minblocks") == 0) {

@@ -2,134 +2,235 @@
 // (the half-rotated contraction of Eq. 47; = 2 X_g of Eq. 37).
 //
 // Per Q this is a real-embedded complex GEMM on the FP64 tensor pipe:
-//   rows   = gamma (8 per DMMA m-tile, packed layout Lf, see context.cu)
-//   K      = (k, a, r, re/im)  = Nk*n*2m reals
+//   rows   = gamma (8 per DMMA m-tile; two m-tiles interleaved per lane in the packed layout Lf, context.cu)
+//   K      = (k, a, r, re/im)  = Nk*n*KS k-steps of 4 reals, one contiguous stream per m-tile pair
 //   cols   = (walker, re/im)   = 4 walkers per DMMA n-tile
-// CTA = (Q, group of MT gamma-octets, group of NT walker-quads).  The 8 warps split K (the (k,a)
-// items), each keeping an MT x NT accumulator tile set in registers; A fragments stream from HBM in
-// lane order (one coalesced 256-byte LDG.64 per fragment), B fragments are read straight from theta
-// (4 full 32-byte sectors per LDG.64) with the real embedding applied as a component select + sign
-// flip.  Lf is read exactly once per call when all walkers fit one walker group.  The K-split
-// partial tiles are combined deterministically through shared memory (no atomics).
+// CTA = (Q, K chunk, walker group, group of m-tile pairs); its 4 warps split the K chunk evenly.  A warp
+// keeps an (MP pairs x NT n-tiles) accumulator set in registers and runs both fragment streams D k-steps
+// ahead in statically rotated register buffers, with branch-free pointer updates, so the loads of a
+// k-step are issued between its DMMAs:
+//   A: one coalesced 512-byte LDG.128 per m-tile pair per k-step, straight from HBM (read once per call
+//      when all walkers fit one walker group);
+//   B: straight from theta (4 full 32-byte sectors per LDG.64, L1/L2 hits: CTAs that differ only in the
+//      m-tile group are adjacent in the grid), real embedding = component select + sign flip.
+// The K split (warps, then chunks) is combined deterministically: shared-memory tree inside the CTA,
+// then a fixed-order sum over chunks in force_bias_reduce_kernel.  No atomics.
 #include "common.cuh"
 
 namespace {
 
-constexpr int FB_WARPS = 8;
+constexpr int FB_WARPS = 4;
+constexpr int FB_D = 2;
 
-template <int MT, int NT>
+template <int MP, int NT>
 __global__ void __launch_bounds__(32 * FB_WARPS) force_bias_kernel(
-    Dims d, int nw, const int* __restrict__ kminus, const double* __restrict__ Lf,
-    const double2* __restrict__ theta, double2* __restrict__ vbias) {
-    __shared__ double red[FB_WARPS / 2][MT * NT * 64];
-    const int Q = blockIdx.x, gt0 = blockIdx.y * MT, t0 = blockIdx.z * NT;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    Dims d, int nw, int KC, int nmg, int nwgrp, int pf, const int* __restrict__ kminus, const double* __restrict__ Lf,
+    const double2* __restrict__ theta, double2* __restrict__ out, int out_is_partial) {
+    extern __shared__ __align__(16) double fb_smem[];
+    // blockIdx.x = ((Q*KC + kc)*nwgrp + wgrp)*nmg + mg
+    int bx = blockIdx.x;
+    const int mg = bx % nmg; bx /= nmg;
+    const int wgrp = bx % nwgrp; bx /= nwgrp;
+    const int kc = bx % KC, Q = bx / KC;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int kk = lane & 3, col = lane >> 2;
     const int cpar = kk & 1, dpar = col & 1;
-    const int comp = cpar ^ dpar;
     const unsigned smask = (cpar && !dpar) ? 0x80000000u : 0u;
     const int roff = kk >> 1;                  // complex r offset inside a k-step
+    const int KS = d.KS, nitems = d.Nk * d.n;
+    const int S = nitems * KS;                 // k-steps of the whole K range
 
-    double acc[MT][NT][2];
+    // item -> offset (in doubles) of theta[(k,a)][(k-Q)*m] inside one walker; one pad entry
+    int* offtab = reinterpret_cast<int*>(fb_smem);
+    for (int it = tid; it <= nitems; it += 32 * FB_WARPS) {
+        const int item = it < nitems ? it : nitems - 1;
+        const int k = item / d.n;
+        offtab[it] = 2 * (item * d.M + kminus[k * d.Nk + Q] * d.m);
+    }
+    double* red = fb_smem + ((nitems + 1 + 1) / 2 + 1) / 2 * 2;     // 16-byte aligned, after the table
+
+    // this warp's K range
+    const int c0 = (int)((long long)kc * S / KC), c1 = (int)((long long)(kc + 1) * S / KC);
+    const int g_begin = c0 + (int)((long long)warp * (c1 - c0) / FB_WARPS);
+    const int g_end = c0 + (int)((long long)(warp + 1) * (c1 - c0) / FB_WARPS);
+
+    const double2* ap[MP];
+    bool aok[MP];
 #pragma unroll
-    for (int i = 0; i < MT; ++i)
+    for (int i = 0; i < MP; ++i) {
+        const int gtp = mg * MP + i;
+        aok[i] = gtp < d.GT2;
+        ap[i] = reinterpret_cast<const double2*>(Lf + (((size_t)Q * d.GT2 + (aok[i] ? gtp : d.GT2 - 1)) * S + g_begin) * 64) + lane;
+    }
+    const double* bw[NT];
+    bool bok[NT];
+#pragma unroll
+    for (int j = 0; j < NT; ++j) {
+        const int w = (wgrp * NT + j) * 4 + (col >> 1);
+        bok[j] = w < nw;
+        bw[j] = reinterpret_cast<const double*>(theta + (size_t)(bok[j] ? w : 0) * d.N * d.M) + 2 * roff + (cpar ^ dpar);
+    }
+    __syncthreads();   // offtab ready
+
+    double acc[2 * MP][NT][2];
+#pragma unroll
+    for (int i = 0; i < 2 * MP; ++i)
 #pragma unroll
         for (int j = 0; j < NT; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-    const int nitems = d.Nk * d.n;
-    for (int item = warp; item < nitems; item += FB_WARPS) {
-        const int k = item / d.n, a = item % d.n;
-        const int kq = kminus[k * d.Nk + Q];
-        const double* bptr[NT];
-        bool bok[NT];
+    // loader state (runs FB_D k-steps ahead; stops advancing at g_end, so nothing is read out of range)
+    int lg = g_begin, item = g_begin / KS, ls = g_begin - item * KS;
+    int boff = offtab[item] + 4 * ls;
+    double2 fa[FB_D][MP];
+    double fb[FB_D][NT];
+    auto refill = [&](const int q) {
+        const bool rok = 2 * ls + roff < d.m;
+#pragma unroll
+        for (int i = 0; i < MP; ++i) {
+            fa[q][i] = __ldg(ap[i]);
+            // pull the HBM stream into L2 `pf` k-steps ahead of the register loads (stays inside this warp's range)
+            if (lg + pf < g_end) asm volatile("prefetch.global.L2 [%0];" ::"l"(ap[i] + pf * 32));
+        }
 #pragma unroll
         for (int j = 0; j < NT; ++j) {
-            int w = (t0 + j) * 4 + (col >> 1);
-            bok[j] = w < nw;
-            bptr[j] = reinterpret_cast<const double*>(theta + ((size_t)(bok[j] ? w : 0) * d.N + k * d.n + a) * d.M +
-                                                      (size_t)kq * d.m + roff) + comp;
+            fb[q][j] = (bok[j] && rok) ? __ldg(bw[j] + boff) : 0.0;   // raw: the sign flip waits until use
         }
-        const double* aptr[MT];
-        bool aok[MT];
+        const bool adv = lg + 1 < g_end;
+        const bool wrap = ls + 1 == KS;
+        lg += adv ? 1 : 0;
 #pragma unroll
-        for (int i = 0; i < MT; ++i) {
-            aok[i] = gt0 + i < d.GT;
-            aptr[i] = Lf + ((((size_t)Q * d.GT + (aok[i] ? gt0 + i : 0)) * d.Nk + k) * d.n + a) * d.KS * 32 + lane;
-        }
-#pragma unroll 2
-        for (int s = 0; s < d.KS; ++s) {
-            double af[MT], bf[NT];
+        for (int i = 0; i < MP; ++i) ap[i] += adv ? 32 : 0;
+        ls = adv ? (wrap ? 0 : ls + 1) : ls;
+        item += (adv && wrap) ? 1 : 0;
+        boff = offtab[item] + 4 * ls;
+    };
+    auto kstep = [&](const int q) {
+        double b[NT];
 #pragma unroll
-            for (int i = 0; i < MT; ++i) af[i] = aok[i] ? __ldg(aptr[i] + s * 32) : 0.0;
-            const bool rok = 2 * s + roff < d.m;
+        for (int j = 0; j < NT; ++j) b[j] = flip_sign(fb[q][j], smask);      // real embedding: -Im for (c=1, d=0)
 #pragma unroll
-            for (int j = 0; j < NT; ++j) bf[j] = (bok[j] && rok) ? flip_sign(__ldg(bptr[j] + 4 * s), smask) : 0.0;
+        for (int i = 0; i < MP; ++i)
 #pragma unroll
-            for (int i = 0; i < MT; ++i)
+            for (int j = 0; j < NT; ++j) {
+                dmma884(acc[2 * i][j][0], acc[2 * i][j][1], fa[q][i].x, b[j]);
+                dmma884(acc[2 * i + 1][j][0], acc[2 * i + 1][j][1], fa[q][i].y, b[j]);
+            }
+        refill(q);
+    };
+    const int total = g_end - g_begin;
+    if (total > 0) {
 #pragma unroll
-                for (int j = 0; j < NT; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
-        }
+        for (int q = 0; q < FB_D; ++q) refill(q);     // steps g_begin .. g_begin+D-1 (repeats the last one if total < D)
     }
+    const int nfull = total - total % FB_D;
+    for (int g0 = 0; g0 < nfull; g0 += FB_D) {
+#pragma unroll
+        for (int q = 0; q < FB_D; ++q) kstep(q);
+    }
+#pragma unroll
+    for (int q = 0; q < FB_D - 1; ++q)
+        if (nfull + q < total) kstep(q);
 
     // deterministic tree reduction over the K-split warps
+    constexpr int TILE = 2 * MP * NT * 64;
 #pragma unroll
     for (int half = FB_WARPS / 2; half >= 1; half >>= 1) {
         if (warp >= half && warp < 2 * half) {
 #pragma unroll
-            for (int i = 0; i < MT; ++i)
+            for (int i = 0; i < 2 * MP; ++i)
 #pragma unroll
                 for (int j = 0; j < NT; ++j) {
-                    red[warp - half][(i * NT + j) * 64 + lane] = acc[i][j][0];
-                    red[warp - half][(i * NT + j) * 64 + 32 + lane] = acc[i][j][1];
+                    red[(warp - half) * TILE + (i * NT + j) * 64 + lane] = acc[i][j][0];
+                    red[(warp - half) * TILE + (i * NT + j) * 64 + 32 + lane] = acc[i][j][1];
                 }
         }
         __syncthreads();
         if (warp < half) {
 #pragma unroll
-            for (int i = 0; i < MT; ++i)
+            for (int i = 0; i < 2 * MP; ++i)
 #pragma unroll
                 for (int j = 0; j < NT; ++j) {
-                    acc[i][j][0] += red[warp][(i * NT + j) * 64 + lane];
-                    acc[i][j][1] += red[warp][(i * NT + j) * 64 + 32 + lane];
+                    acc[i][j][0] += red[warp * TILE + (i * NT + j) * 64 + lane];
+                    acc[i][j][1] += red[warp * TILE + (i * NT + j) * 64 + 32 + lane];
                 }
         }
         __syncthreads();
     }
     if (warp == 0) {
+        const double scale = out_is_partial ? 1.0 : 2.0;
+        double2* dst = out + (out_is_partial ? (size_t)kc * nw * d.Nk * d.nchol : 0);
 #pragma unroll
-        for (int i = 0; i < MT; ++i) {
-            int gam = (gt0 + i) * 8 + (lane >> 2);
-            if (gt0 + i >= d.GT || gam >= d.nchol) continue;
+        for (int i = 0; i < 2 * MP; ++i) {
+            const int gam = ((mg * MP + (i >> 1)) * 2 + (i & 1)) * 8 + (lane >> 2);
+            if (!aok[i >> 1] || gam >= d.nchol) continue;
 #pragma unroll
             for (int j = 0; j < NT; ++j) {
-                int w = (t0 + j) * 4 + (lane & 3);
+                const int w = (wgrp * NT + j) * 4 + (lane & 3);
                 if (w < nw)
-                    vbias[((size_t)w * d.Nk + Q) * d.nchol + gam] = make_double2(2.0 * acc[i][j][0], 2.0 * acc[i][j][1]);
+                    dst[((size_t)w * d.Nk + Q) * d.nchol + gam] = make_double2(scale * acc[i][j][0], scale * acc[i][j][1]);
             }
         }
     }
 }
 
+// vbias = 2 * sum over K chunks of the partial results, in chunk order
+__global__ void force_bias_reduce_kernel(size_t n, int KC, const double2* __restrict__ part, double2* __restrict__ vbias) {
+    for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        double2 s = part[e];
+        for (int c = 1; c < KC; ++c) { const double2 p = part[(size_t)c * n + e]; s.x += p.x; s.y += p.y; }
+        vbias[e] = make_double2(2.0 * s.x, 2.0 * s.y);
+    }
+}
+
+template <int MP, int NT>
+int launch_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias, cudaStream_t st) {
+    const Dims& d = c->d;
+    const int ntq = (nw + 3) / 4;
+    const int nmg = (d.GT2 + MP - 1) / MP, nwgrp = (ntq + NT - 1) / NT;
+    const long long base = (long long)d.Nk * nmg * nwgrp;
+    const int S = d.Nk * d.n * d.KS;
+    // K chunks: the count (<= AFQMC_FB_MAXKC, every warp keeps >= 8 k-steps) that fills the SMs most evenly
+    int KC = 1;
+    double best = -1.0;
+    for (int kc = 1; kc <= AFQMC_FB_MAXKC; ++kc) {
+        if (kc > 1 && S / (kc * FB_WARPS) < 8) break;
+        const double n = (double)base * kc, waves = n / c->num_sms;
+        const double eff = waves / (double)(long long)(waves + 0.999999) - 0.004 * kc;
+        if (eff > best) { best = eff; KC = kc; }
+    }
+    const size_t smem = (size_t)(((d.Nk * d.n + 2) / 2 + 1) / 2 * 2 + (FB_WARPS / 2) * 2 * MP * NT * 64) * sizeof(double);
+    auto kern = force_bias_kernel<MP, NT>;
+    static size_t attr_set = 0;
+    if (smem > 48 * 1024 && smem > attr_set) {
+        if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+            return AFQMC_CUDA_ERROR;
+        attr_set = smem;
+    }
+    kern<<<(unsigned)(base * KC), 32 * FB_WARPS, smem, st>>>(d, nw, KC, nmg, nwgrp, c->opt_fb_pf, c->kminus, c->Lf, theta,
+                                                             KC > 1 ? c->ws_fbpart : vbias, KC > 1 ? 1 : 0);
+    AFQMC_LAUNCH_CHECK(c);
+    if (KC > 1) {
+        const size_t n = (size_t)nw * d.Nk * d.nchol;
+        int G = (int)((n + 255) / 256);
+        if (G > c->num_sms * 8) G = c->num_sms * 8;
+        force_bias_reduce_kernel<<<G, 256, 0, st>>>(n, KC, c->ws_fbpart, vbias);
+        AFQMC_LAUNCH_CHECK(c);
+    }
+    return AFQMC_OK;
+}
+
 }  // namespace
 
 int afqmc_i_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias, cudaStream_t st) {
-    const Dims& d = c->d;
     const int ntq = (nw + 3) / 4;   // walker quads
-    if (ntq >= 4 || ntq == 3) {
-        constexpr int MT = 5, NT = 4;
-        dim3 grid(d.Nk, (d.GT + MT - 1) / MT, (ntq + NT - 1) / NT);
-        force_bias_kernel<MT, NT><<<grid, 32 * FB_WARPS, 0, st>>>(d, nw, c->kminus, c->Lf, theta, vbias);
-    } else if (ntq == 2) {
-        constexpr int MT = 5, NT = 2;
-        dim3 grid(d.Nk, (d.GT + MT - 1) / MT, 1);
-        force_bias_kernel<MT, NT><<<grid, 32 * FB_WARPS, 0, st>>>(d, nw, c->kminus, c->Lf, theta, vbias);
-    } else {
-        constexpr int MT = 5, NT = 1;
-        dim3 grid(d.Nk, (d.GT + MT - 1) / MT, 1);
-        force_bias_kernel<MT, NT><<<grid, 32 * FB_WARPS, 0, st>>>(d, nw, c->kminus, c->Lf, theta, vbias);
-    }
-    AFQMC_LAUNCH_CHECK(c);
-    return AFQMC_OK;
+    // 16 DMMAs per k-step and warp in every shape; all walkers in one group up to 32 walkers
+    if (ntq >= 5) return c->opt_fb_tile == 1 ? launch_force_bias<2, 8>(c, theta, nw, vbias, st)
+                     : c->opt_fb_tile == 2 ? launch_force_bias<2, 4>(c, theta, nw, vbias, st)
+                                           : launch_force_bias<1, 8>(c, theta, nw, vbias, st);
+    if (ntq >= 3) return launch_force_bias<2, 4>(c, theta, nw, vbias, st);
+    if (ntq == 2) return launch_force_bias<4, 2>(c, theta, nw, vbias, st);
+    return launch_force_bias<4, 1>(c, theta, nw, vbias, st);
 }
 
 AFQMC_API int afqmc_force_bias(afqmc_ctx* c, const void* theta, int nw, void* vbias, void* stream) {
