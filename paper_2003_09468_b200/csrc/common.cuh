@@ -65,6 +65,7 @@ struct afqmc_ctx {
     int opt_exchange_minb;  // tuning aid: 1 = ask for more resident CTAs per SM
     int opt_exchange_wpc;   // 0 = automatic, else warps per CTA of the exchange kernel (4,5,6,8)
     int opt_timers;     // record stage events in afqmc_step
+    int opt_green_legacy;   // testing aid: 1 = shared/global-memory elimination kernel instead of the register-resident one
     cudaEvent_t ev[AFQMC_NUM_STAGES + 1];
     int ev_valid;
     int smem_optin;     // max dynamic shared memory per block (bytes)

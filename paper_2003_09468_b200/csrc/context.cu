@@ -320,6 +320,10 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
         c->opt_exchange_depth = value;
         return AFQMC_OK;
     }
+    if (strcmp(name, "green_legacy") == 0) {
+        c->opt_green_legacy = value ? 1 : 0;
+        return AFQMC_OK;
+    }
     if (strcmp(name, "timers") == 0) {
         if (value && !c->ev[0])
             for (int i = 0; i <= AFQMC_NUM_STAGES; ++i)

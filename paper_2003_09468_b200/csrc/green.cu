@@ -6,6 +6,7 @@
 // Gauss-Jordan elimination with partial (row) pivoting -- the same pivot sequence as an LU with
 // partial pivoting, so det O = sign * prod(pivots).  The transposed inverse goes to workspace and
 // Theta = (Phi O^{-1})^T = O^{-T} Phi^T (Eq. 30) is one batched DMMA GEMM.
+#include <cooperative_groups.h>
 #include <math_constants.h>
 #include "zgemm.cuh"
 
@@ -176,11 +177,247 @@ __global__ void __launch_bounds__(GJ_THREADS) overlap_inverse_kernel(
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Register-resident elimination (N <= 32*RT rows, N <= CS*NWARP*CT columns).
+//
+// The whole N x N overlap lives in registers: lane l of every warp owns rows {l, l+32, ...} (RT of
+// them), warp gw (numbered across the CS CTAs of a thread-block cluster) owns columns
+// [gw*CT, gw*CT+CT).  Gauss-Jordan with IMPLICIT partial pivoting: rows are never swapped; step j
+// picks the largest |a[i][j]| among the rows not yet used as pivots (the same pivot values as LU
+// with partial pivoting up to the row labelling), so the stored matrix ends as
+//     stored[sigma(i)][c] = (Pi O)^{-1}[i][c],   sigma(j) = pivot row of step j
+//     =>  O^{-1}[i][c] = stored[sigma(i)][sigma^{-1}(c)],   det O = sign(sigma) * prod_j pivot_j.
+// Per step only ONE warp (the owner of column j) searches the pivot (warp shuffles) and publishes
+// {pivot row, 1/pivot, the column of multipliers} to the shared memory of every CTA of the cluster
+// (double-buffered by step parity); after ONE barrier (CTA or cluster) every warp fetches the pivot
+// row segment of its own columns by shuffles from the lane that owns it and applies the rank-1 update
+// to its registers.  No matrix traffic through shared or global memory at all.
+// ---------------------------------------------------------------------------------------------
+namespace cg = cooperative_groups;
+
+template <int RT, int CT>
+struct GJRegShared {
+    double2 f[2][32 * RT];      // multipliers (column j before the update), by step parity
+    double2 ipiv[2];
+    double2 piv[2];
+    int prow_cur[2];
+    int zero[2];
+    double2 pivs[32 * RT];      // pivots, for log det
+    int prow[32 * RT];          // sigma
+    int sinv[32 * RT];          // sigma^{-1}
+    double red[3][32];
+    int info;
+};
+
+template <int RT, int CT, int NWARP, int CS>
+__global__ void __launch_bounds__(32 * NWARP, 1) overlap_inverse_reg_kernel(
+    Dims d, const double2* __restrict__ psi_t, const double2* __restrict__ phi, double2* __restrict__ oinvT /*nullable*/,
+    double2* __restrict__ logdet /*nullable*/, int* __restrict__ info /*nullable*/) {
+    __shared__ GJRegShared<RT, CT> sh;
+    const int N = d.N, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int w = blockIdx.x / CS;
+    unsigned rank = 0;
+    if (CS > 1) rank = cg::this_cluster().block_rank();
+    const int gw = (int)rank * NWARP + warp;          // global warp = column group
+    const int c0 = gw * CT;
+    const double2* ph = phi + (size_t)w * d.M * N;
+
+    // ---- a1: O[(k,a)][c] = sum_p conj(A_k[p][a]) Phi[(k,p)][c] for my rows x my columns ----
+    double2 a[RT][CT];
+#pragma unroll
+    for (int t = 0; t < RT; ++t) {
+#pragma unroll
+        for (int cc = 0; cc < CT; ++cc) a[t][cc] = make_double2(0.0, 0.0);
+        const int i = lane + 32 * t;
+        if (i < N && c0 < N) {
+            const int k = i / d.n, aa = i - k * d.n;
+            const double2* Ab = psi_t + (size_t)k * d.m * d.n + aa;
+            const double2* Pb = ph + (size_t)k * d.m * N + c0;
+#pragma unroll 2
+            for (int p = 0; p < d.m; ++p) {
+                double2 av = __ldg(Ab + (size_t)p * d.n);
+                av.y = -av.y;
+#pragma unroll
+                for (int cc = 0; cc < CT; ++cc)
+                    if (c0 + cc < N) a[t][cc] = cfma(av, __ldg(Pb + (size_t)p * N + cc), a[t][cc]);
+            }
+        }
+    }
+    if (tid == 0) sh.info = 0;
+    unsigned used = 0;                                 // bit t: my row lane+32t has been a pivot row
+    if (CS > 1) cg::this_cluster().sync(); else __syncthreads();
+
+    // ---- a2: N elimination steps ----
+    for (int j = 0; j < N; ++j) {
+        const int buf = j & 1;
+        const int jw = j / CT, tj = j - jw * CT;       // owner warp and its local column
+        if (gw == jw) {
+            // column j of my rows
+            double2 col[RT];
+#pragma unroll
+            for (int t = 0; t < RT; ++t) {
+                col[t] = a[t][0];
+#pragma unroll
+                for (int cc = 1; cc < CT; ++cc) if (cc == tj) col[t] = a[t][cc];
+            }
+            double bv = -2.0;
+            int bi = 0x7fffffff;
+#pragma unroll
+            for (int t = 0; t < RT; ++t) {
+                const int i = lane + 32 * t;
+                if (i < N && !((used >> t) & 1u)) {
+                    double mag = col[t].x * col[t].x + col[t].y * col[t].y;
+                    if (!(mag >= 0.0)) mag = -1.0;                 // NaN: never preferred, still a valid row
+                    if (mag > bv) { bv = mag; bi = i; }
+                }
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const double ov = __shfl_xor_sync(0xffffffffu, bv, o);
+                const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+                if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+            }
+            const int p = bi, pl = p & 31, pt = p >> 5;
+            double2 pvl = col[0];
+#pragma unroll
+            for (int t = 1; t < RT; ++t) if (t == pt) pvl = col[t];
+            double2 pv;
+            pv.x = __shfl_sync(0xffffffffu, pvl.x, pl);
+            pv.y = __shfl_sync(0xffffffffu, pvl.y, pl);
+            const double den = pv.x * pv.x + pv.y * pv.y;
+            const bool ok = den > 0.0;
+            const double2 ip = ok ? make_double2(pv.x / den, -pv.y / den) : make_double2(0.0, 0.0);
+            // publish to every CTA of the cluster
+#pragma unroll 1
+            for (int q = 0; q < CS; ++q) {
+                GJRegShared<RT, CT>* dst = &sh;
+                if (CS > 1) dst = cg::this_cluster().map_shared_rank(&sh, q);
+#pragma unroll
+                for (int t = 0; t < RT; ++t) dst->f[buf][lane + 32 * t] = col[t];
+                if (lane == 0) { dst->ipiv[buf] = ip; dst->piv[buf] = pv; dst->prow_cur[buf] = p; dst->zero[buf] = ok ? 0 : 1; }
+            }
+        }
+        if (CS > 1) cg::this_cluster().sync(); else __syncthreads();
+
+        const int p = sh.prow_cur[buf], pl = p & 31, pt = p >> 5;
+        const double2 ip = sh.ipiv[buf];
+        if (tid == 0) {
+            sh.prow[j] = p;
+            sh.pivs[j] = sh.piv[buf];
+            if (sh.zero[buf] && sh.info == 0) sh.info = j + 1;
+        }
+        if (lane == pl) used |= 1u << pt;
+        // scaled pivot row for my columns: r[cc] = a[p][c] / pivot  (column j itself -> 1/pivot)
+        double2 r[CT];
+#pragma unroll
+        for (int cc = 0; cc < CT; ++cc) {
+            double2 v = a[0][cc];
+#pragma unroll
+            for (int t = 1; t < RT; ++t) if (t == pt) v = a[t][cc];
+            v.x = __shfl_sync(0xffffffffu, v.x, pl);
+            v.y = __shfl_sync(0xffffffffu, v.y, pl);
+            r[cc] = cmul(v, ip);
+        }
+        if (gw == jw) {
+#pragma unroll
+            for (int cc = 0; cc < CT; ++cc)
+                if (cc == tj) {
+                    r[cc] = ip;
+#pragma unroll
+                    for (int t = 0; t < RT; ++t) a[t][cc] = make_double2(0.0, 0.0);
+                }
+        }
+#pragma unroll
+        for (int t = 0; t < RT; ++t) {
+            const bool isp = (lane == pl) && (t == pt);
+            double2 f = sh.f[buf][lane + 32 * t];
+            f.x = isp ? 0.0 : -f.x;
+            f.y = isp ? 0.0 : -f.y;
+#pragma unroll
+            for (int cc = 0; cc < CT; ++cc) {
+                const double2 u = cfma(f, r[cc], a[t][cc]);
+                a[t][cc] = isp ? r[cc] : u;
+            }
+        }
+    }
+    if (CS > 1) cg::this_cluster().sync(); else __syncthreads();
+
+    // ---- sigma^{-1}, log det O = sum log(pivot) + i*pi*(sigma odd), info ----
+    for (int j = tid; j < N; j += 32 * NWARP) sh.sinv[sh.prow[j]] = j;
+    if (rank == 0) {
+        double lr = 0.0, li = 0.0, inv = 0.0;
+        for (int j = tid; j < N; j += 32 * NWARP) {
+            const double2 pv = sh.pivs[j];
+            lr += log(hypot(pv.x, pv.y));
+            li += atan2(pv.y, pv.x);
+            const int sj = sh.prow[j];
+            int cnt = 0;
+            for (int i = 0; i < j; ++i) cnt += sh.prow[i] > sj;      // inversions of sigma
+            inv += (double)cnt;
+        }
+        lr = warp_sum(lr); li = warp_sum(li); inv = warp_sum(inv);
+        if (lane == 0) { sh.red[0][warp] = lr; sh.red[1][warp] = li; sh.red[2][warp] = inv; }
+    }
+    __syncthreads();
+    if (rank == 0 && tid == 0) {
+        double sr = 0.0, si = 0.0, sv = 0.0;
+        for (int x = 0; x < NWARP; ++x) { sr += sh.red[0][x]; si += sh.red[1][x]; sv += sh.red[2][x]; }
+        if (((long long)sv) & 1LL) si += CUDART_PI;
+        si = si - 2.0 * CUDART_PI * ceil((si - CUDART_PI) / (2.0 * CUDART_PI));     // wrap to (-pi, pi]
+        if (logdet) logdet[w] = make_double2(sr, si);
+        if (info) info[w] = sh.info;
+    }
+    // ---- O^{-T}[sigma(k)][sigma^{-1}(rho)] = stored[rho][k] ----
+    if (oinvT) {
+        double2* out = oinvT + (size_t)w * N * N;
+#pragma unroll
+        for (int cc = 0; cc < CT; ++cc) {
+            const int k = c0 + cc;
+            if (k < N) {
+                const size_t rowoff = (size_t)sh.prow[k] * N;
+#pragma unroll
+                for (int t = 0; t < RT; ++t) {
+                    const int rho = lane + 32 * t;
+                    if (rho < N) out[rowoff + sh.sinv[rho]] = a[t][cc];
+                }
+            }
+        }
+    }
+}
+
+template <int RT, int CT, int NWARP, int CS>
+int launch_gj_reg(afqmc_ctx* c, const double2* phi, int nw, double2* oinvT, double2* logdet, int* info, cudaStream_t st) {
+    auto kern = overlap_inverse_reg_kernel<RT, CT, NWARP, CS>;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(nw * CS));
+    cfg.blockDim = dim3(32 * NWARP);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CS; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (cudaLaunchKernelEx(&cfg, kern, c->d, (const double2*)c->psi_t, phi, oinvT, logdet, info) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return AFQMC_CUDA_ERROR;
+    }
+    AFQMC_LAUNCH_CHECK(c);
+    return AFQMC_OK;
+}
+
 size_t gj_fixed_smem(int N) { return gj_off_mat(N); }
 
 int run_overlap_inverse(afqmc_ctx* c, const double2* phi, int nw, double2* oinvT, double2* logdet, int* info,
                         cudaStream_t st) {
     const Dims& d = c->d;
+    if (!c->opt_green_legacy) {
+        // register-resident elimination: one CTA for N <= 64, a cluster of two for N <= 128, of eight for N <= 256
+        if (d.N <= 32) return launch_gj_reg<1, 2, 16, 1>(c, phi, nw, oinvT, logdet, info, st);
+        if (d.N <= 64) return launch_gj_reg<2, 4, 16, 1>(c, phi, nw, oinvT, logdet, info, st);
+        if (d.N <= 128) return launch_gj_reg<4, 4, 16, 2>(c, phi, nw, oinvT, logdet, info, st);
+        if (d.N <= 256) return launch_gj_reg<8, 2, 16, 8>(c, phi, nw, oinvT, logdet, info, st);
+    }
     const int LD = d.N | 1;
     size_t fixed = gj_fixed_smem(d.N);
     size_t mat = (size_t)d.N * LD * sizeof(double2);

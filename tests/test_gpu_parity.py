@@ -291,3 +291,36 @@ def test_subbatch_equals_full_batch(small_case):
     e_all = case.ctx.local_energy(th_all)
     e_3 = case.ctx.local_energy(th_3)
     assert torch.equal(e_all[:3], e_3)
+
+
+def test_green_register_kernel_equals_legacy_kernel(small_case):
+    """The register-resident elimination and the shared-memory one agree to rounding (both exact up to pivot order)."""
+    case = small_case
+    phi_d = _to_dev(case.pb.phi)
+    th_new, ld_new, _ = case.ctx.green(phi_d)
+    case.ctx.set_option("green_legacy", 1)
+    try:
+        th_old, ld_old, _ = case.ctx.green(phi_d)
+    finally:
+        case.ctx.set_option("green_legacy", 0)
+    assert relerr(th_new.cpu().numpy(), th_old.cpu().numpy()) < 1e-12
+    assert np.max(np.abs(ld_new.cpu().numpy().real - ld_old.cpu().numpy().real)) < 1e-12
+    assert np.max(phase_diff(ld_new.cpu().numpy().imag, ld_old.cpu().numpy().imag)) < 1e-12
+
+
+@pytest.mark.parametrize("mesh,n", [((4, 4, 3), 6), ((4, 3, 3), 7), ((5, 5, 1), 5)], ids=["N288_legacy", "N252_cluster8", "N125_cluster2"])
+def test_green_large_N(mesh, n):
+    """Overlap sizes that select the cluster kernels (N <= 128: 2 CTAs, N <= 256: 8 CTAs) and the legacy path (N > 256)."""
+    cfg = synth.tiny_config(mesh=mesh, m=n + 2, n=n, nchol=2, nw=3, seed=11)
+    case = Case(cfg)
+    try:
+        theta_d, ld_d, info_d = case.ctx.green(_to_dev(case.pb.phi))
+        assert np.all(info_d.cpu().numpy() == 0)
+        theta, ld = theta_d.cpu().numpy(), ld_d.cpu().numpy()
+        for w in range(case.nw):
+            th_o, ld_o, _ = orc.green(case.pb.psi_t, case.pb.phi[w])
+            assert relerr(theta[w], th_o) < RTOL
+            assert abs(ld[w].real - ld_o.real) < RTOL * max(1.0, abs(ld_o.real))
+            assert phase_diff(ld[w].imag, ld_o.imag) < 1e-9
+    finally:
+        case.close()
