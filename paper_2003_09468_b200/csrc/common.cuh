@@ -50,7 +50,8 @@ struct afqmc_ctx {
     double2* ws_vbias;  // [nw][Nk][nchol]
     double2* ws_xi;     // [nw][Nk][nchol]
     double2* ws_vhs;    // [nw][M][M]
-    double2* ws_T;      // [2][nw][M][N] Taylor ping-pong
+    double2* ws_T;      // [2][nw][M][N] Taylor ping-pong (legacy GEMM path)
+    double* ws_Tx;      // [2][nw][expanded] Taylor ping-pong in the expanded B-fragment layout of tgemm.cuh
     double2* ws_expart; // [nunits][nw]  exchange partial sums
     double2* ws_fbpart; // [AFQMC_FB_MAXKC][nw][Nk][nchol] force-bias K-chunk partial sums
     double* ws_x;       // [nw][Nk][nchol] (host-entry staging)
@@ -65,6 +66,7 @@ struct afqmc_ctx {
     int opt_exchange_minb;  // tuning aid: 1 = ask for more resident CTAs per SM
     int opt_exchange_wpc;   // 0 = automatic, else warps per CTA of the exchange kernel (4,5,6,8)
     int opt_timers;     // record stage events in afqmc_step
+    int opt_taylor_legacy;  // testing aid: 1 = shared-memory-tiled zgemm for the Taylor chain
     int opt_green_legacy;   // testing aid: 1 = shared/global-memory elimination kernel instead of the register-resident one
     cudaEvent_t ev[AFQMC_NUM_STAGES + 1];
     int ev_valid;
@@ -140,6 +142,7 @@ int afqmc_i_vhs(afqmc_ctx* c, const double* x, const double2* vbias, double dtau
 int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, double2* phi, int nw,
                       cudaStream_t st);
 int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* energy, cudaStream_t st);
+size_t afqmc_i_taylor_ws_doubles(const Dims& d);   // per-walker doubles of one expanded Taylor buffer
 // records stage event i on st when timers are on
 static inline void afqmc_mark(afqmc_ctx* c, int i, cudaStream_t st) {
     if (c->opt_timers && c->ev[i]) cudaEventRecord(c->ev[i], st);

@@ -153,7 +153,7 @@ static int dev_alloc(T** p, size_t count) {
 AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     if (!c) return;
     void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lx, c->Lf, c->Lv,
-                    c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T,
+                    c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T, c->ws_Tx,
                     c->ws_expart, c->ws_fbpart, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -246,6 +246,8 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     A(dev_alloc(&c->ws_xi, (size_t)Nk * d.GP * ((nw + 3) / 4) * 16));   // expanded fragments: 32 doubles each
     A(dev_alloc(&c->ws_vhs, (size_t)nw * d.M * d.M));
     A(dev_alloc(&c->ws_T, (size_t)2 * nw * d.M * d.N));
+    const size_t nTx = (size_t)2 * nw * afqmc_i_taylor_ws_doubles(d);
+    A(dev_alloc(&c->ws_Tx, nTx));
     A(dev_alloc(&c->ws_expart, (size_t)c->nunits * nw));
     A(dev_alloc(&c->ws_fbpart, (size_t)AFQMC_FB_MAXKC * nw * Nk * d.nchol));
     A(dev_alloc(&c->ws_x, (size_t)nw * Nk * d.nchol));
@@ -259,6 +261,8 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
         if (rc == AFQMC_OK && cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
             rc = AFQMC_CUDA_ERROR;
     };
+    // the padding tiles of the expanded Taylor buffers are read but never written by the GEMM epilogue
+    if (cudaMemsetAsync(c->ws_Tx, 0, nTx * sizeof(double), st) != cudaSuccess) rc = AFQMC_CUDA_ERROR;
     H2D(c->kminus, kminus.data(), kminus.size() * sizeof(int));
     H2D(c->kplus, kplus.data(), kplus.size() * sizeof(int));
     H2D(c->kneg, kneg.data(), kneg.size() * sizeof(int));
@@ -318,6 +322,10 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
     if (strcmp(name, "exchange_depth") == 0) {
         if (value != 0 && value != 2 && value != 3) return AFQMC_INVALID_ARGUMENT;
         c->opt_exchange_depth = value;
+        return AFQMC_OK;
+    }
+    if (strcmp(name, "taylor_legacy") == 0) {
+        c->opt_taylor_legacy = value ? 1 : 0;
         return AFQMC_OK;
     }
     if (strcmp(name, "green_legacy") == 0) {

@@ -1,0 +1,298 @@
+// Batched complex128 GEMM for tall-skinny right-hand sides on the FP64 tensor pipe (DMMA m8n8k4),
+// used by a6 (Taylor propagation) and a3 (Green's function, Eq. 30):
+//
+//   C_b[i][j] = alpha * sum_k A_b[i][k] * B_b[k][j],     A: M x K (big, streamed once),  B: K x N (small)
+//
+// Design (B200): the big operand A is read straight from its natural row-major layout into DMMA
+// A-fragments, the small operand B lives in an EXPANDED fragment-major layout that is staged into shared
+// memory by bulk asynchronous copies (cp.async.bulk + mbarrier pipeline, SASS UBLKCP), so the inner loop is
+// LDG.128 (A, prefetched in registers) + LDS.64 (B, conflict-free) + DMMA only.
+//
+//  * K pairing.  The real embedding of a complex GEMM (common.cuh) needs K index (k, part).  The K order is
+//    free as long as A and B agree, so a PAIR of DMMA k-steps covers four complex k = 4t..4t+3:
+//        even step 2t  : A-fragment = Re A[i][4t+c],  B rows (T_re | T_im)
+//        odd  step 2t+1: A-fragment = Im A[i][4t+c],  B rows (-T_im | T_re)
+//    so lane (row r, c) gets both of its A values with ONE 16-byte load of the complex element A[i][4t+c].
+//  * Expanded B ("Bx"): [batch][g][s = 2t+parity][nt < NTA][32 doubles], g = column group (<= NTA n-tiles of 4
+//    complex columns), innermost 32 doubles = one DMMA B-fragment in lane order (lane = (2*jj+d)*4 + c: column jj
+//    of the tile, d = re/im output part, c = k inside the pair).  K is padded to a multiple of 4*KC and unused
+//    tiles/columns/rows are ZERO, so the kernel has no tails: A loads are clamped (finite * 0).
+//  * The epilogue can (a) accumulate alpha*C into a natural-layout D (D += alpha*C), (b) write alpha*C in the
+//    expanded layout of the NEXT product's B operand (rows of C become its K index), (c) store alpha*C
+//    transposed in natural layout.  With (b) the Taylor chain T_j = (s/j) V T_{j-1} never converts layouts.
+//  * CTA = 4 warps x (16 rows x one column group); the warps share the staged B chunks.  Grid = (groups, row
+//    blocks, batch): CTAs of the same rows and walker are adjacent, so A is fetched from HBM once and shared
+//    through L2 by the column groups.
+#pragma once
+#include "common.cuh"
+
+namespace tg {
+
+constexpr int KC = 4;        // k-step PAIRS per shared-memory stage
+constexpr int STAGES = 3;
+constexpr int WPC = 4;       // warps per CTA
+constexpr int BM = 16 * WPC;
+
+struct Args {
+    const double2* A; long long strideA; int lda;      // [batch][M][lda], K contiguous
+    const double* Bx; long long strideBx;              // expanded B operand (see above), K = this product's K
+    double* Cx; long long strideCx;                    // nullable: alpha*C expanded as the next product's B (its K = M)
+    double2* D; long long strideD; int ldd;            // nullable: D[i][j] += alpha*C[i][j]
+    double2* Ct; long long strideCt; int ldct;         // nullable: Ct[j][i]  = alpha*C[i][j]
+    int M, N, K;
+    int G, nt_base, nt_rem;                            // column groups: group g has nt_base + (g < nt_rem) n-tiles
+    int NPp;                                           // padded k-step pairs of this product: roundup(ceil(K/4), KC)
+    int NPcp;                                          // padded k-step pairs of the Cx layout: roundup(ceil(M/4), KC)
+    double alpha;
+};
+
+// column-group geometry shared by host and device
+struct Groups { int G, nt_base, nt_rem, NTA; };
+__host__ __device__ inline int group_tile0(int g, int nt_base, int nt_rem) { return g * nt_base + (g < nt_rem ? g : nt_rem); }
+__host__ __device__ inline int group_tiles(int g, int nt_base, int nt_rem) { return nt_base + (g < nt_rem ? 1 : 0); }
+
+// instantiated tile counts per column group (template NTA); a group with fewer tiles is zero padded
+static inline int round_nta(int nt) {
+    const int avail[] = {2, 4, 6, 8, 10, 12, 13, 14};
+    for (int a : avail) if (nt <= a) return a;
+    return 14;
+}
+static inline Groups make_groups(int N) {
+    Groups gr;
+    const int nt = (N + 3) / 4;
+    gr.G = (nt + 13) / 14;
+    gr.nt_base = nt / gr.G;
+    gr.nt_rem = nt % gr.G;
+    gr.NTA = round_nta(gr.nt_base + (gr.nt_rem ? 1 : 0));
+    return gr;
+}
+static inline int padded_pairs(int K) { return (((K + 3) / 4 + KC - 1) / KC) * KC; }
+// doubles of one batch entry of an expanded operand with K rows and N columns
+static inline size_t expanded_doubles(int K, int N) {
+    const Groups gr = make_groups(N);
+    return (size_t)gr.G * 2 * padded_pairs(K) * gr.NTA * 32;
+}
+
+// ---- natural [K][N] (ldb) -> expanded; also the zero fill of all padding ----
+// CONJ_T: the source is read as B[k][j] = src[j][k] (transposed, K contiguous), as a3 needs for Phi^T.
+template <bool TRANS>
+__global__ void expand_kernel(const double2* __restrict__ src, long long strideS, int lds, double* __restrict__ Bx,
+                              long long strideBx, int K, int N, int G, int nt_base, int nt_rem, int NTA, int NPp) {
+    const size_t per = (size_t)G * 2 * NPp * NTA * 32;
+    const int b = blockIdx.y;
+    const double2* S = src + (size_t)b * strideS;
+    double* out = Bx + (size_t)b * strideBx;
+    for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < per; idx += (size_t)gridDim.x * blockDim.x) {
+        size_t t = idx;
+        const int l = (int)(t & 31); t >>= 5;
+        const int nt = (int)(t % NTA); t /= NTA;
+        const int s = (int)(t % (2 * NPp));
+        const int g = (int)(t / (2 * NPp));
+        const int par = s & 1, col = l >> 2, jj = col >> 1, dd = col & 1;
+        const int k = 4 * (s >> 1) + (l & 3);
+        const int j = (group_tile0(g, nt_base, nt_rem) + nt) * 4 + jj;
+        double v = 0.0;
+        if (k < K && j < N && nt < group_tiles(g, nt_base, nt_rem)) {
+            const double2 z = TRANS ? S[(size_t)j * lds + k] : S[(size_t)k * lds + j];
+            v = par == 0 ? (dd ? z.y : z.x) : (dd ? z.x : -z.y);
+        }
+        out[idx] = v;
+    }
+}
+
+// ---- mbarrier / bulk-copy primitives (PTX) ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n.reg .pred p;\nWAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}\n" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// ---- the GEMM body for a column group of NT (<= NTA) n-tiles ----
+template <int NT, int NTA, int D>
+__device__ __forceinline__ void body(const Args& p, const double* stage0, uint64_t* full, uint64_t* empty, int g, int b) {
+    static_assert(KC % D == 0, "A prefetch depth must divide the chunk");
+    constexpr uint32_t STAGE_DOUBLES = KC * 2 * NTA * 32, STAGE_BYTES = STAGE_DOUBLES * 8;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int row0 = blockIdx.y * BM + warp * 16;
+    const int r = lane >> 2, c = lane & 3;
+    const double2* A = p.A + (size_t)b * p.strideA;
+    const int i0 = min(row0 + r, p.M - 1), i1 = min(row0 + 8 + r, p.M - 1);   // clamped rows: finite data, discarded
+    const double2* pa0 = A + (size_t)i0 * p.lda;
+    const double2* pa1 = A + (size_t)i1 * p.lda;
+    const int Km1 = p.K - 1;
+    double2 fa0[D], fa1[D];
+#pragma unroll
+    for (int q = 0; q < D; ++q) {
+        const int k = min(4 * q + c, Km1);               // clamped k: the matching B rows are zero
+        fa0[q] = __ldg(pa0 + k);
+        fa1[q] = __ldg(pa1 + k);
+    }
+    double acc[2][NT][2];
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
+
+    const int nchunks = p.NPp / KC;
+    const double* Bsrc = p.Bx + (size_t)b * p.strideBx + (size_t)g * 2 * p.NPp * NTA * 32;
+    if (tid == 0) {
+        for (int c0 = 0; c0 < STAGES - 1 && c0 < nchunks; ++c0) {
+            mbar_expect_tx(&full[c0], STAGE_BYTES);
+            bulk_g2s(const_cast<double*>(stage0) + (size_t)c0 * STAGE_DOUBLES, Bsrc + (size_t)c0 * STAGE_DOUBLES, STAGE_BYTES, &full[c0]);
+        }
+    }
+    for (int ch = 0; ch < nchunks; ++ch) {
+        const int st = ch % STAGES;
+        mbar_wait(&full[st], (uint32_t)((ch / STAGES) & 1));
+        const double* bs = stage0 + (size_t)st * STAGE_DOUBLES + lane;
+#pragma unroll
+        for (int q = 0; q < KC; ++q) {
+            constexpr int dummy = 0; (void)dummy;
+            const int buf = q % D;
+            double bf[NT];
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) bf[nt] = bs[((2 * q) * NTA + nt) * 32];
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+                dmma884(acc[0][nt][0], acc[0][nt][1], fa0[buf].x, bf[nt]);
+                dmma884(acc[1][nt][0], acc[1][nt][1], fa1[buf].x, bf[nt]);
+            }
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) bf[nt] = bs[((2 * q + 1) * NTA + nt) * 32];
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+                dmma884(acc[0][nt][0], acc[0][nt][1], fa0[buf].y, bf[nt]);
+                dmma884(acc[1][nt][0], acc[1][nt][1], fa1[buf].y, bf[nt]);
+            }
+            {   // refill this register buffer with the pair D ahead
+                const int k = min(4 * (ch * KC + q + D) + c, Km1);
+                fa0[buf] = __ldg(pa0 + k);
+                fa1[buf] = __ldg(pa1 + k);
+            }
+            if (q == 1 && tid == 0) {   // producer duty: refill the stage consumed in the previous iteration
+                const int nxt = ch + STAGES - 1;
+                if (nxt < nchunks) {
+                    const int s2 = nxt % STAGES;
+                    mbar_wait(&empty[s2], (uint32_t)(((nxt / STAGES) & 1) ^ 1));
+                    mbar_expect_tx(&full[s2], STAGE_BYTES);
+                    bulk_g2s(const_cast<double*>(stage0) + (size_t)s2 * STAGE_DOUBLES, Bsrc + (size_t)nxt * STAGE_DOUBLES, STAGE_BYTES, &full[s2]);
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[st]);
+    }
+
+    // ---- epilogue: lane holds complex (row = r, column = 4*tile + c) of each 8x4 tile ----
+    const int tile0 = group_tile0(g, p.nt_base, p.nt_rem);
+    const int ntg = group_tiles(g, p.nt_base, p.nt_rem);
+    double2* Dm = p.D ? p.D + (size_t)b * p.strideD : nullptr;
+    double2* Ct = p.Ct ? p.Ct + (size_t)b * p.strideCt : nullptr;
+    double* Cx = p.Cx ? p.Cx + (size_t)b * p.strideCx + (size_t)g * 2 * p.NPcp * NTA * 32 : nullptr;
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt) {
+        const int i = row0 + mt * 8 + r;
+        const bool iok = i < p.M;
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            const int j = (tile0 + nt) * 4 + c;
+            double2 v = make_double2(p.alpha * acc[mt][nt][0], p.alpha * acc[mt][nt][1]);
+            if (iok && j < p.N && nt < ntg) {
+                if (Dm) {
+                    double2 o = Dm[(size_t)i * p.ldd + j];
+                    o.x += v.x; o.y += v.y;
+                    Dm[(size_t)i * p.ldd + j] = o;
+                }
+                if (Ct) Ct[(size_t)j * p.ldct + i] = v;
+            }
+            if (Cx && i < 4 * p.NPcp) {
+                if (!iok) v = make_double2(0.0, 0.0);     // K padding of the next product
+                double* f = Cx + ((size_t)(2 * (i >> 2)) * NTA + nt) * 32 + 8 * c + (i & 3);
+                f[0] = v.x; f[4] = v.y;                   // even step: (re | im)
+                f += NTA * 32;
+                f[0] = -v.y; f[4] = v.x;                  // odd step: (-im | re)
+            }
+        }
+    }
+}
+
+template <int NTA, int D>
+__global__ void __launch_bounds__(32 * WPC, 2) tgemm_kernel(Args p) {
+    extern __shared__ __align__(128) double tg_smem[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(tg_smem + (size_t)STAGES * KC * 2 * NTA * 32);
+    uint64_t* empty = full + STAGES;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], WPC); }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+    }
+    __syncthreads();
+    const int g = blockIdx.x, b = blockIdx.z;
+    if (group_tiles(g, p.nt_base, p.nt_rem) == NTA) body<NTA, NTA, D>(p, tg_smem, full, empty, g, b);
+    else body<NTA - 1, NTA, D>(p, tg_smem, full, empty, g, b);
+}
+
+template <int NTA, int D>
+static inline cudaError_t launch_cfg(const Args& a, int batch, cudaStream_t st) {
+    auto kern = tgemm_kernel<NTA, D>;
+    const int smem = STAGES * KC * 2 * NTA * 32 * 8 + 2 * STAGES * 8;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    dim3 grid(a.G, (a.M + BM - 1) / BM, batch);
+    kern<<<grid, 32 * WPC, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+// fills the group fields of `a` from N and launches; `a.NPp`/`a.NPcp` are derived from K and M
+static inline cudaError_t launch(Args a, int batch, cudaStream_t st) {
+    const Groups gr = make_groups(a.N);
+    a.G = gr.G; a.nt_base = gr.nt_base; a.nt_rem = gr.nt_rem;
+    a.NPp = padded_pairs(a.K);
+    a.NPcp = padded_pairs(a.M);
+    switch (gr.NTA) {
+        case 2: return launch_cfg<2, 2>(a, batch, st);
+        case 4: return launch_cfg<4, 2>(a, batch, st);
+        case 6: return launch_cfg<6, 2>(a, batch, st);
+        case 8: return launch_cfg<8, 2>(a, batch, st);
+        case 10: return launch_cfg<10, 2>(a, batch, st);
+        case 12: return launch_cfg<12, 2>(a, batch, st);
+        case 13: return launch_cfg<13, 2>(a, batch, st);
+        default: return launch_cfg<14, 2>(a, batch, st);
+    }
+}
+
+template <bool TRANS>
+static inline cudaError_t launch_expand(const double2* src, long long strideS, int lds, double* Bx, int K, int N,
+                                        int batch, cudaStream_t st) {
+    const Groups gr = make_groups(N);
+    const int NPp = padded_pairs(K);
+    const size_t per = (size_t)gr.G * 2 * NPp * gr.NTA * 32;
+    int bx = (int)((per + 255) / 256);
+    if (bx > 148 * 8) bx = 148 * 8;
+    expand_kernel<TRANS><<<dim3(bx, batch), 256, 0, st>>>(src, strideS, lds, Bx, (long long)per, K, N, gr.G, gr.nt_base,
+                                                           gr.nt_rem, gr.NTA, NPp);
+    return cudaGetLastError();
+}
+
+}  // namespace tg
