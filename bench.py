@@ -30,6 +30,11 @@ if ROOT not in sys.path:
 METRIC = "walker-steps/s incl. local energy"
 UNIT = "walker-steps/s"
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE exchange-kernel launch, from the committed
+# `ncu --set full` capture of this same command (profiles/r01c_ncu_full_metrics.txt); bench.py cannot
+# measure DRAM traffic itself.  Only the configuration that was captured has a value.
+EXCHANGE_DRAM_TRAFFIC = {"C3": {"bytes": 389.341e6 + 9.110e6, "source": "profiles/r01c_ncu_full_metrics.txt"}}
+
 
 def load_measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -223,10 +228,16 @@ def run_ours(args):
         ex_flops = ctx.exchange_flops(nw)
         achieved = ex_flops / (ex_ms * 1e-3) / 1e12
         peak_probe = binding.probe_fp64(1, 20000)          # DMMA issue-rate probe, this GPU, now
+        # algorithmic bytes of one exchange launch: packed Lh once + theta once + partial sums
+        ctx_alg_bytes = cfg.nk ** 2 * cfg.n * cfg.nchol * cfg.m * 16 + nw * cfg.N * cfg.M * 16
         peaks = load_measured_peaks()
         roofline = {
             "kernel": "exchange (a9), afqmc_local_energy", "bound": "tensor", "achieved": achieved,
-            "peak": peak_probe, "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": None,
+            "peak": peak_probe, "unit": "TFLOP/s", "frac": achieved / peak_probe,
+            "traffic": EXCHANGE_DRAM_TRAFFIC.get(cfg.name, {}).get("bytes"),
+            "traffic_unit": "bytes per launch (DRAM read+write)",
+            "traffic_source": EXCHANGE_DRAM_TRAFFIC.get(cfg.name, {}).get("source"),
+            "algorithmic_bytes": float(ctx_alg_bytes),
             "peak_source": "live FP64 DMMA.8x8x4 probe (afqmc_probe_fp64); MEASURED_PEAKS.json has no FP64 entry",
             "flops_per_launch": ex_flops, "ms_per_launch": ex_ms,
             "share_of_step": ex_ms / (dev_ms_max / args.steps),
