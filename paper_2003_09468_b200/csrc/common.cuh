@@ -67,6 +67,8 @@ struct afqmc_ctx {
     int opt_exchange_wpc;   // 0 = automatic, else warps per CTA of the exchange kernel (4,5,6,8)
     int opt_timers;     // record stage events in afqmc_step
     int opt_taylor_legacy;  // testing aid: 1 = shared-memory-tiled zgemm for the Taylor chain
+    int opt_taylor_wpc;     // tuning aid: 0 = automatic, else 3/4/5 warps per CTA of the Taylor GEMM
+    int opt_taylor_groups;  // tuning aid: 0 = automatic, else the number of column groups of the Taylor GEMM
     int opt_green_legacy;   // testing aid: 1 = shared/global-memory elimination kernel instead of the register-resident one
     cudaEvent_t ev[AFQMC_NUM_STAGES + 1];
     int ev_valid;

@@ -328,6 +328,16 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
         c->opt_taylor_legacy = value ? 1 : 0;
         return AFQMC_OK;
     }
+    if (strcmp(name, "taylor_warps") == 0) {
+        if (value != 0 && (value < 3 || value > 5)) return AFQMC_INVALID_ARGUMENT;
+        c->opt_taylor_wpc = value;
+        return AFQMC_OK;
+    }
+    if (strcmp(name, "taylor_groups") == 0) {
+        if (value < 0 || value > 64) return AFQMC_INVALID_ARGUMENT;
+        c->opt_taylor_groups = value;
+        return AFQMC_OK;
+    }
     if (strcmp(name, "green_legacy") == 0) {
         c->opt_green_legacy = value ? 1 : 0;
         return AFQMC_OK;

@@ -7,7 +7,7 @@
 #include "tgemm.cuh"
 #include "zgemm.cuh"
 
-size_t afqmc_i_taylor_ws_doubles(const Dims& d) { return tg::expanded_doubles(d.M, d.N); }
+size_t afqmc_i_taylor_ws_doubles(const Dims& d) { return tg::expanded_doubles_max(d.M, d.N); }
 
 int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, double2* phi, int nw,
                       cudaStream_t st) {
@@ -31,9 +31,11 @@ int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, 
         }
         return AFQMC_OK;
     }
-    const size_t perx = tg::expanded_doubles(d.M, d.N);
-    double* Tx[2] = {c->ws_Tx, c->ws_Tx + (size_t)c->max_walkers * perx};
-    if (tg::launch_expand<false>(phi, (long long)per, d.N, Tx[0], d.M, d.N, nw, st) != cudaSuccess) return AFQMC_CUDA_ERROR;
+    const int G = c->opt_taylor_groups > 0 ? c->opt_taylor_groups : tg::pick_groups(d.M, d.N, nw);
+    const size_t perx = tg::expanded_doubles(d.M, d.N, G);
+    if (perx > afqmc_i_taylor_ws_doubles(d)) return AFQMC_INVALID_ARGUMENT;   // a forced group count the workspace was not sized for
+    double* Tx[2] = {c->ws_Tx, c->ws_Tx + (size_t)c->max_walkers * afqmc_i_taylor_ws_doubles(d)};
+    if (tg::launch_expand<false>(phi, (long long)per, d.N, Tx[0], d.M, d.N, nw, st, G) != cudaSuccess) return AFQMC_CUDA_ERROR;
     c->launches++;
     for (int j = 1; j <= order; ++j) {
         tg::Args a = {};
@@ -43,7 +45,8 @@ int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, 
         a.D = phi; a.strideD = (long long)per; a.ldd = d.N;
         a.Ct = nullptr; a.strideCt = 0; a.ldct = 0;
         a.M = d.M; a.N = d.N; a.K = d.M; a.alpha = s / (double)j;
-        if (tg::launch(a, nw, st) != cudaSuccess) return AFQMC_CUDA_ERROR;
+        a.wpc = c->opt_taylor_wpc;
+        if (tg::launch(a, nw, st, G) != cudaSuccess) return AFQMC_CUDA_ERROR;
         c->launches++;
     }
     return AFQMC_OK;

@@ -20,9 +20,9 @@
 //  * The epilogue can (a) accumulate alpha*C into a natural-layout D (D += alpha*C), (b) write alpha*C in the
 //    expanded layout of the NEXT product's B operand (rows of C become its K index), (c) store alpha*C
 //    transposed in natural layout.  With (b) the Taylor chain T_j = (s/j) V T_{j-1} never converts layouts.
-//  * CTA = 4 warps x (16 rows x one column group); the warps share the staged B chunks.  Grid = (groups, row
+//  * CTA = WPC warps x (16 rows x one column group); the warps share the staged B chunks.  Grid = (groups, row
 //    blocks, batch): CTAs of the same rows and walker are adjacent, so A is fetched from HBM once and shared
-//    through L2 by the column groups.
+//    through L2 by the column groups.  WPC = 4 (see launch_cfg).
 #pragma once
 #include "common.cuh"
 
@@ -30,8 +30,7 @@ namespace tg {
 
 constexpr int KC = 4;        // k-step PAIRS per shared-memory stage
 constexpr int STAGES = 3;
-constexpr int WPC = 4;       // warps per CTA
-constexpr int BM = 16 * WPC;
+// warps per CTA (WPC, 16 rows each) is a template parameter chosen per launch: see launch_cfg()
 
 struct Args {
     const double2* A; long long strideA; int lda;      // [batch][M][lda], K contiguous
@@ -44,6 +43,7 @@ struct Args {
     int NPp;                                           // padded k-step pairs of this product: roundup(ceil(K/4), KC)
     int NPcp;                                          // padded k-step pairs of the Cx layout: roundup(ceil(M/4), KC)
     double alpha;
+    int wpc;                                           // 0 = automatic, else 3/4/5 warps per CTA (tuning aid)
 };
 
 // column-group geometry shared by host and device
@@ -57,20 +57,33 @@ static inline int round_nta(int nt) {
     for (int a : avail) if (nt <= a) return a;
     return 14;
 }
-static inline Groups make_groups(int N) {
+// G = 0: the fewest groups (<= 14 tiles each); G > 0: that many groups (clamped to what the tile count allows)
+static inline Groups make_groups(int N, int G = 0) {
     Groups gr;
     const int nt = (N + 3) / 4;
-    gr.G = (nt + 13) / 14;
+    const int gmin = (nt + 13) / 14;
+    gr.G = G < gmin ? gmin : (G > nt ? nt : G);
     gr.nt_base = nt / gr.G;
     gr.nt_rem = nt % gr.G;
     gr.NTA = round_nta(gr.nt_base + (gr.nt_rem ? 1 : 0));
     return gr;
 }
+constexpr int GROUP_CHOICES = 3;   // pick_groups() considers gmin .. gmin + GROUP_CHOICES - 1 groups
 static inline int padded_pairs(int K) { return (((K + 3) / 4 + KC - 1) / KC) * KC; }
 // doubles of one batch entry of an expanded operand with K rows and N columns
-static inline size_t expanded_doubles(int K, int N) {
-    const Groups gr = make_groups(N);
+static inline size_t expanded_doubles(int K, int N, int G = 0) {
+    const Groups gr = make_groups(N, G);
     return (size_t)gr.G * 2 * padded_pairs(K) * gr.NTA * 32;
+}
+// the largest expanded operand over the group counts pick_groups() may choose (workspace sizing)
+static inline size_t expanded_doubles_max(int K, int N) {
+    const int gmin = make_groups(N).G;
+    size_t mx = 0;
+    for (int g = gmin; g < gmin + GROUP_CHOICES; ++g) {
+        const size_t e = expanded_doubles(K, N, g);
+        if (e > mx) mx = e;
+    }
+    return mx;
 }
 
 // ---- natural [K][N] (ldb) -> expanded; also the zero fill of all padding ----
@@ -125,12 +138,12 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 }
 
 // ---- the GEMM body for a column group of NT (<= NTA) n-tiles ----
-template <int NT, int NTA, int D>
+template <int NT, int NTA, int D, int WPC>
 __device__ __forceinline__ void body(const Args& p, const double* stage0, uint64_t* full, uint64_t* empty, int g, int b) {
     static_assert(KC % D == 0, "A prefetch depth must divide the chunk");
     constexpr uint32_t STAGE_DOUBLES = KC * 2 * NTA * 32, STAGE_BYTES = STAGE_DOUBLES * 8;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int row0 = blockIdx.y * BM + warp * 16;
+    const int row0 = blockIdx.y * (16 * WPC) + warp * 16;
     const int r = lane >> 2, c = lane & 3;
     const double2* A = p.A + (size_t)b * p.strideA;
     const int i0 = min(row0 + r, p.M - 1), i1 = min(row0 + 8 + r, p.M - 1);   // clamped rows: finite data, discarded
@@ -233,7 +246,7 @@ __device__ __forceinline__ void body(const Args& p, const double* stage0, uint64
     }
 }
 
-template <int NTA, int D>
+template <int NTA, int D, int WPC>
 __global__ void __launch_bounds__(32 * WPC, 2) tgemm_kernel(Args p) {
     extern __shared__ __align__(128) double tg_smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(tg_smem + (size_t)STAGES * KC * 2 * NTA * 32);
@@ -245,47 +258,115 @@ __global__ void __launch_bounds__(32 * WPC, 2) tgemm_kernel(Args p) {
     }
     __syncthreads();
     const int g = blockIdx.x, b = blockIdx.z;
-    if (group_tiles(g, p.nt_base, p.nt_rem) == NTA) body<NTA, NTA, D>(p, tg_smem, full, empty, g, b);
-    else body<NTA - 1, NTA, D>(p, tg_smem, full, empty, g, b);
+    if (group_tiles(g, p.nt_base, p.nt_rem) == NTA) body<NTA, NTA, D, WPC>(p, tg_smem, full, empty, g, b);
+    else body<NTA - 1, NTA, D, WPC>(p, tg_smem, full, empty, g, b);
 }
 
-template <int NTA, int D>
-static inline cudaError_t launch_cfg(const Args& a, int batch, cudaStream_t st) {
-    auto kern = tgemm_kernel<NTA, D>;
+template <int NTA, int D, int WPC>
+static inline cudaError_t launch_wpc(const Args& a, int batch, cudaStream_t st, int* occ_out) {
+    auto kern = tgemm_kernel<NTA, D, WPC>;
     const int smem = STAGES * KC * 2 * NTA * 32 * 8 + 2 * STAGES * 8;
-    static bool attr_done = false;
-    if (!attr_done) {
+    static int occ = -1;
+    if (occ < 0) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        int o = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kern, 32 * WPC, smem);
+        if (e != cudaSuccess) return e;
+        occ = o > 0 ? o : 1;
     }
-    dim3 grid(a.G, (a.M + BM - 1) / BM, batch);
+    if (occ_out) { *occ_out = occ; return cudaSuccess; }      // query only
+    dim3 grid(a.G, (a.M + 16 * WPC - 1) / (16 * WPC), batch);
     kern<<<grid, 32 * WPC, smem, st>>>(a);
     return cudaGetLastError();
 }
 
-// fills the group fields of `a` from N and launches; `a.NPp`/`a.NPcp` are derived from K and M
-static inline cudaError_t launch(Args a, int batch, cudaStream_t st) {
-    const Groups gr = make_groups(a.N);
+static inline int device_sms() {
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+            sms = 148;
+    }
+    return sms;
+}
+
+// Warps per CTA.  The DMMA pipe is per SM sub-partition, so resident warps must divide evenly over the four
+// sub-partitions: measured at C3 (r01c notes), 2 CTAs x 4 warps run 6 sub-partition rounds in 3.35 ms, while
+// 2 x 5 warps (1.95 waves instead of 2.38, but 3+3+2+2 warps per sub-partition) take 3.90 ms and 3 warps 4.39 ms.
+// 4 is therefore the default; 3 and 5 stay selectable as a tuning aid (option "taylor_warps").
+template <int NTA, int D>
+static inline cudaError_t launch_cfg(const Args& a, int batch, cudaStream_t st) {
+    int best = 4;
+    if (a.wpc >= 3 && a.wpc <= 5) best = a.wpc;
+    switch (best) {
+        case 3: return launch_wpc<NTA, D, 3>(a, batch, st, nullptr);
+        case 5: return launch_wpc<NTA, D, 5>(a, batch, st, nullptr);
+        default: return launch_wpc<NTA, D, 4>(a, batch, st, nullptr);
+    }
+}
+
+#define TG_NTA_SWITCH(NTA_VALUE, CALL)                         \
+    switch (NTA_VALUE) {                                       \
+        case 2: return CALL(2);                                \
+        case 4: return CALL(4);                                \
+        case 6: return CALL(6);                                \
+        case 8: return CALL(8);                                \
+        case 10: return CALL(10);                              \
+        case 12: return CALL(12);                              \
+        case 13: return CALL(13);                              \
+        default: return CALL(14);                              \
+    }
+
+// resident CTAs per SM of the 4-warp kernel instantiated for NTA tiles per group
+static inline cudaError_t query_occupancy(int NTA, int* occ) {
+    Args a = {};
+#define TG_CALL(n) launch_wpc<n, 2, 4>(a, 1, nullptr, occ)
+    TG_NTA_SWITCH(NTA, TG_CALL)
+#undef TG_CALL
+}
+
+// Number of column groups for a product with M rows, N columns and `batch` entries.  More groups mean narrower
+// warp tiles (fewer accumulators, A re-read from L2 by more CTAs) but a finer grid: the cost model is
+//   rounds of resident CTAs x resident CTAs per SM x tiles a warp executes per k-step,
+// i.e. the DMMA time of one SM (the kernel is tensor-pipe bound).  At C3 (27 n-tiles, 704 row blocks) two groups
+// of 14/13 tiles run 2.38 -> 3 rounds (cost 84), three groups of 9 run 3.57 -> 4 rounds (cost 72), four of 7 run 4.76 -> 5 rounds (cost 70): measured 3.35, 2.78, 2.71 ms.
+static inline int pick_groups(int M, int N, int batch) {
+    const int gmin = make_groups(N).G;
+    const int sms = device_sms();
+    int best = gmin; long long best_cost = -1;
+    for (int g = gmin; g < gmin + GROUP_CHOICES; ++g) {
+        const Groups gr = make_groups(N, g);
+        if (gr.G != g) break;
+        int occ = 1;
+        if (query_occupancy(gr.NTA, &occ) != cudaSuccess) { (void)cudaGetLastError(); continue; }
+        const long long ctas = (long long)gr.G * ((M + 63) / 64) * batch;
+        const long long slots = (long long)occ * sms;
+        const long long rounds = (ctas + slots - 1) / slots;
+        const int nt_exec = gr.nt_base + (gr.nt_rem ? 1 : 0);
+        // 2 % per extra group for the A re-reads and the shorter DMMA runs between fragment loads
+        const long long cost = rounds * occ * nt_exec * (100 + 2 * (g - gmin));
+        if (best_cost < 0 || cost < best_cost) { best = g; best_cost = cost; }
+    }
+    return best;
+}
+
+// fills the group fields of `a` from N (and the group count G, 0 = fewest) and launches; `a.NPp`/`a.NPcp` are
+// derived from K and M.  The expanded operands must have been written with the same G.
+static inline cudaError_t launch(Args a, int batch, cudaStream_t st, int G = 0) {
+    const Groups gr = make_groups(a.N, G);
     a.G = gr.G; a.nt_base = gr.nt_base; a.nt_rem = gr.nt_rem;
     a.NPp = padded_pairs(a.K);
     a.NPcp = padded_pairs(a.M);
-    switch (gr.NTA) {
-        case 2: return launch_cfg<2, 2>(a, batch, st);
-        case 4: return launch_cfg<4, 2>(a, batch, st);
-        case 6: return launch_cfg<6, 2>(a, batch, st);
-        case 8: return launch_cfg<8, 2>(a, batch, st);
-        case 10: return launch_cfg<10, 2>(a, batch, st);
-        case 12: return launch_cfg<12, 2>(a, batch, st);
-        case 13: return launch_cfg<13, 2>(a, batch, st);
-        default: return launch_cfg<14, 2>(a, batch, st);
-    }
+#define TG_CALL(n) launch_cfg<n, 2>(a, batch, st)
+    TG_NTA_SWITCH(gr.NTA, TG_CALL)
+#undef TG_CALL
 }
 
 template <bool TRANS>
 static inline cudaError_t launch_expand(const double2* src, long long strideS, int lds, double* Bx, int K, int N,
-                                        int batch, cudaStream_t st) {
-    const Groups gr = make_groups(N);
+                                        int batch, cudaStream_t st, int G = 0) {
+    const Groups gr = make_groups(N, G);
     const int NPp = padded_pairs(K);
     const size_t per = (size_t)gr.G * 2 * NPp * gr.NTA * 32;
     int bx = (int)((per + 255) / 256);
