@@ -376,3 +376,210 @@ def step(mesh, L, Lh, ht, psi_t, phi, x, dtau, order):
         energy[w] = local_energy(mesh, Lh, ht, th2)
         logdet[w] = ld
     return phi_new, energy, logdet
+
+
+# ======================================================================================
+# The AFQMC block around the step:  one-body half steps (Eq. 7, 13,
+# PAPER.md:54, :85), hybrid importance function and phaseless weight update (Eq. 15-19,
+# PAPER.md:93-105), walker orthogonalisation and the mixed estimator (Eq. 34-35);
+# "a block is 20 iterations of the propagation step followed by an energy evaluation and walker
+# orthogonalization ... the 'hybrid' method is used for propagation".
+# ======================================================================================
+
+# ---- level D: the real-field (Hermitian) basis of the Hubbard-Stratonovich operators ----
+def hermitian_hs_operators(mesh, Lsc, nchol):
+    """One HERMITIAN M x M matrix v_j per real field x[Q][gamma] (j = Q*nchol + gamma), so that
+    H2' = (1/2) sum_Gamma rho_Gamma rho_Gamma^dagger = (1/2) sum_j v_j^2 (Eq. 8-9, with
+    the paper's v_hat = i v) and sum_j x_j v_j = sum_Gamma z_Gamma L_Gamma with the z of
+    `assemble_fields`:
+        -Q == Q          : v = L_Q                             (Hermitian by the (Q,-Q) identity)
+        idx(Q) < idx(-Q) : v_Q = (L_Q + L_{-Q})/sqrt2,  v_{-Q} = i (L_Q - L_{-Q})/sqrt2.
+    rho_Gamma = sum_pr L_{pr,Gamma} c_p^dag c_r and rho_{(-Q,gamma)} = rho_{(Q,gamma)}^dagger."""
+    nk = mesh[0] * mesh[1] * mesh[2]
+    Mdim = Lsc.shape[0]
+    v = np.zeros((nk * nchol, Mdim, Mdim), dtype=C128)
+    for Q in range(nk):
+        mq = k_neg(mesh, Q)
+        for g in range(nchol):
+            LQ = Lsc[:, :, Q * nchol + g]
+            LmQ = Lsc[:, :, mq * nchol + g]
+            if mq == Q:
+                v[Q * nchol + g] = LQ
+            elif Q < mq:
+                v[Q * nchol + g] = (LQ + LmQ) / np.sqrt(2.0)
+                v[mq * nchol + g] = 1j * (LQ - LmQ) / np.sqrt(2.0)
+    return v
+
+
+def dense_expm_hermitian(Hm, scale):
+    """exp(scale * Hm) for a Hermitian matrix by eigendecomposition."""
+    w, U = np.linalg.eigh(Hm)
+    return (U * np.exp(scale * w)) @ np.conj(U.T)
+
+
+def dense_hybrid_step(A, vops, B1, phi_w, x_flat, dtau, order, xbar_override=None):
+    """Level D of one hybrid propagation step for one walker, entirely in the real-field basis; `B1` is the
+    DENSE M x M one-body half-step propagator (`supercell_h1` of the per-k blocks)
+    (Eq. 13, 15-19; closed shell, both spins share phi):
+        G      = Green's function of phi (Eq. 29);   <v_j> = 2 sum_pr (v_j)_pr G_pr
+        xbar_j = -i sqrt(dtau) <v_j>                  (Eq. 17 with v_hat_j = i v_j)
+        B(x - xbar) = B1 * Taylor_order( i sqrt(dtau) sum_j (x_j - xbar_j) v_j ) * B1   (Eq. 13)
+        ratio  = [det(A^dag phi') / det(A^dag phi)]^2                          (two spin channels)
+        I      = ratio * exp(x.xbar - xbar.xbar/2)                             (Eq. 16)
+        dtheta = arg(ratio)                                                     (Eq. 19)
+        factor = |I| max(0, cos dtheta)                                         (Eq. 18)
+    `xbar_override` replaces the force-bias shift by any (complex) shift: Eq. 12 and 15-16 describe the same
+    integral for every shift, which is what the quadrature pin checks.
+    Returns (phi', I, dtheta, factor)."""
+    G = dense_green(A, phi_w)
+    vavg = 2.0 * np.einsum('jpr,pr->j', vops, G)
+    xbar = -1j * np.sqrt(dtau) * vavg
+    if xbar_override is not None:
+        xbar = np.asarray(xbar_override, dtype=C128)
+    xs = x_flat - xbar
+    V = np.einsum('j,jpr->pr', xs, vops)
+    t = B1 @ phi_w
+    # Taylor series of exp(i sqrt(dtau) V) applied to t
+    term = t.copy()
+    out = t.copy()
+    for j in range(1, order + 1):
+        term = (1j * np.sqrt(dtau) / j) * (V @ term)
+        out = out + term
+    phi_new = B1 @ out
+    d_old = np.linalg.det(dense_overlap(A, phi_w))
+    d_new = np.linalg.det(dense_overlap(A, phi_new))
+    ratio = (d_new / d_old) ** 2
+    I = ratio * np.exp(np.sum(x_flat * xbar) - 0.5 * np.sum(xbar * xbar))
+    dtheta = float(np.angle(ratio))
+    factor = float(np.abs(I) * max(0.0, np.cos(dtheta)))
+    return phi_new, I, dtheta, factor
+
+
+def dense_h2prime_mixed(vops, G):
+    """<Psi_T| (1/2) sum_j v_j^2 |phi> / <Psi_T|phi> for a closed shell by Wick's theorem with
+    G_pr = <c_p^dag c_r> (per spin):  <c_p^dag c_r c_q^dag c_s> = G_pr G_qs + G_ps (delta_rq - G_qr), so
+    <v^2> = (2 tr_pr v G)^2 + 2 sum v_pr v_rs G_ps - 2 sum v_pr v_qs G_ps G_qr."""
+    tot = 0.0 + 0.0j
+    for v in vops:
+        t1 = 2.0 * np.einsum('pr,pr->', v, G)
+        t2 = 2.0 * np.einsum('pr,rs,ps->', v, v, G)
+        t3 = 2.0 * np.einsum('pr,qs,ps,qr->', v, v, G, G)
+        tot += 0.5 * (t1 * t1 + t2 - t3)
+    return tot
+
+
+# ---- level P: what the GPU library computes ----
+def onebody_half_propagator(h1p, dtau):
+    """B1[k] = exp(-dtau/2 * h1p[k]) per k-point (H1' is block diagonal in k, Eq. 45, PAPER.md:210;
+    the half steps of Eq. 7/13).  `h1p` is whatever one-body operator the caller propagates with
+    (the paper's H1' = H1 + v0, Eq. 10; v0 is outside this build's scope)."""
+    return np.stack([dense_expm_hermitian(h1p[k], -0.5 * dtau) for k in range(h1p.shape[0])])
+
+
+def apply_onebody(B1, phi_w):
+    """Phi[(k,:), :] <- B1[k] Phi[(k,:), :]  (block-diagonal one-body propagator, Eq. 13)."""
+    nk, m, _ = B1.shape
+    out = np.empty_like(phi_w)
+    for k in range(nk):
+        out[k * m:(k + 1) * m, :] = B1[k] @ phi_w[k * m:(k + 1) * m, :]
+    return out
+
+
+def hybrid_weight(mesh, x_w, vbias_w, dtau, logdet_old, logdet_new):
+    """Eq. 16, 18, 19 in the (Q,gamma) field basis of `assemble_fields`:
+    with z, zbar as there (zbar_{Q} = -i sqrt(dtau) vbias_{-Q}),
+        x.xbar = sum_{Q,gamma} z_Q zbar_{-Q},   xbar.xbar = sum_{Q,gamma} zbar_Q zbar_{-Q}
+    (the real-field bilinear forms written in the complex basis; pinned against level D),
+        log ratio = 2 (logdet_new - logdet_old)          (closed shell: both spin channels)
+        log I = log ratio + x.xbar - xbar.xbar/2;  dtheta = Im log ratio wrapped to (-pi, pi];
+        factor = |I| max(0, cos dtheta).
+    Returns (log I (complex), dtheta, factor)."""
+    nk = x_w.shape[0]
+    z = np.zeros(x_w.shape, dtype=C128)
+    for Q in range(nk):
+        mq = k_neg(mesh, Q)
+        if mq == Q:
+            z[Q] = x_w[Q]
+        elif Q < mq:
+            z[Q] = (x_w[Q] + 1j * x_w[mq]) / np.sqrt(2.0)
+            z[mq] = np.conj(z[Q])
+    zbar = np.zeros_like(z)
+    for Q in range(nk):
+        zbar[Q] = -1j * np.sqrt(dtau) * vbias_w[k_neg(mesh, Q)]
+    xxb = 0.0 + 0.0j
+    xbxb = 0.0 + 0.0j
+    for Q in range(nk):
+        mq = k_neg(mesh, Q)
+        xxb += np.sum(z[Q] * zbar[mq])
+        xbxb += np.sum(zbar[Q] * zbar[mq])
+    logratio = 2.0 * (logdet_new - logdet_old)
+    logI = logratio + xxb - 0.5 * xbxb
+    dtheta = float((logratio.imag + np.pi) % (2 * np.pi) - np.pi)
+    if dtheta == -np.pi:
+        dtheta = np.pi
+    factor = float(np.exp(logI.real) * max(0.0, np.cos(dtheta)))
+    return logI, dtheta, factor
+
+
+def orthogonalize(phi_w):
+    """Walker orthogonalisation: thin QR  Phi = Q R  with R upper triangular and a
+    REAL POSITIVE diagonal (which makes Q unique), by modified Gram-Schmidt column by column.
+    Returns (Q [M][N], log det R = sum_j log r_jj, real).  The Slater determinant changes only by the
+    factor det R: Theta, vbias and the local energy are invariant (gauge invariance, R14)."""
+    q = phi_w.astype(C128).copy()
+    nn = q.shape[1]
+    logdet_r = 0.0
+    for j in range(nn):
+        for i in range(j):
+            rij = np.vdot(q[:, i], q[:, j])           # q_i^dagger a_j
+            q[:, j] = q[:, j] - rij * q[:, i]
+        rjj = np.sqrt(np.vdot(q[:, j], q[:, j]).real)
+        q[:, j] = q[:, j] / rjj
+        logdet_r += np.log(rjj)
+    return q, logdet_r
+
+
+def mixed_estimator(weight, energy):
+    """Eq. 35: E_mixed = sum_w weight_w E_L[phi_w] / sum_w weight_w, E_L = E1 + EC + EX.
+    Returns (numerator [3] complex = sum_w weight_w (E1, EC, EX)_w, denominator = sum_w weight_w)."""
+    num = np.einsum('w,wc->c', weight.astype(np.float64), energy)
+    return num, float(np.sum(weight))
+
+
+def hybrid_step(mesh, L, Lh, psi_t, B1, phi_w, x_w, dtau, order):
+    """One hybrid propagation step for one walker (Eq. 13, 15-19): force bias, vHS, B1 * Taylor * B1,
+    overlap ratio and weight factor.  Returns (phi', log I, dtheta, factor, info)."""
+    th, ld_old, info = green(psi_t, phi_w)
+    vb = force_bias(mesh, Lh, th)
+    xi = assemble_fields(mesh, x_w, vb, dtau)
+    V = vhs(mesh, L, xi)
+    t = apply_onebody(B1, phi_w)
+    t = propagate(V, t, dtau, order)
+    phi_new = apply_onebody(B1, t)
+    lu, perm, sign, info2 = lu_factor(overlap(psi_t, phi_new))
+    ld_new = lu_logdet(lu, sign)
+    logI, dtheta, factor = hybrid_weight(mesh, x_w, vb, dtau, ld_old, ld_new)
+    return phi_new, logI, dtheta, factor, max(info, info2)
+
+
+def block(mesh, L, Lh, ht, psi_t, B1, phi, weight, x, dtau, order):
+    """One AFQMC block: x.shape[0] hybrid propagation steps, then the local energy of
+    every walker and the mixed estimator, then walker orthogonalisation.
+      phi [nw][M][N], weight [nw] real, x [nsteps][nw][Nk][nchol] real.
+    Returns (phi_out, weight_out, energy [nw][3], (num, den) of Eq. 35, logdetR [nw])."""
+    nsteps, nw = x.shape[0], phi.shape[0]
+    phi = phi.astype(C128).copy()
+    weight = weight.astype(np.float64).copy()
+    for s in range(nsteps):
+        for w in range(nw):
+            phi[w], _, _, factor, _ = hybrid_step(mesh, L, Lh, psi_t, B1, phi[w], x[s, w], dtau, order)
+            weight[w] *= factor
+    energy = np.empty((nw, 3), dtype=C128)
+    logdet_r = np.empty(nw)
+    for w in range(nw):
+        th, _, _ = green(psi_t, phi[w])
+        energy[w] = local_energy(mesh, Lh, ht, th)
+    num, den = mixed_estimator(weight, energy)
+    for w in range(nw):
+        phi[w], logdet_r[w] = orthogonalize(phi[w])
+    return phi, weight, energy, (num, den), logdet_r

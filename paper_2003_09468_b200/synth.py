@@ -145,3 +145,12 @@ def make_problem(cfg: Config, nw=None) -> Problem:
 def tiny_config(mesh=(2, 3, 1), m=3, n=2, nchol=4, nw=2, seed=1, dtau=0.005, order=6):
     """Small configs for the definition-level (dense 4-index) oracle checks."""
     return Config("tiny%dx%dx%d" % tuple(mesh), tuple(mesh), m, n, nchol, nw, dtau, order, seed)
+
+
+def make_block_fields(cfg: Config, nsteps: int, nw=None, seed_offset=7):
+    """Auxiliary fields for one AFQMC block (a block = `nsteps` propagation steps, 20 in the
+    paper): x[nsteps][nw][Nk][nchol] ~ N(0,1), from their own stream `seed + seed_offset` so the single-step
+    inputs of `make_problem` are unchanged.  Initial weights are 1 (the caller's array)."""
+    nw = cfg.nw if nw is None else nw
+    rng = np.random.default_rng(cfg.seed + seed_offset)
+    return rng.standard_normal((nsteps, nw, cfg.nk, cfg.nchol))
