@@ -150,6 +150,69 @@ int afqmc_step(afqmc_ctx* ctx, void* phi, const double* x, double dtau, int orde
 int afqmc_step_host(afqmc_ctx* ctx, void* phi_host, const double* x_host, double dtau, int order,
                     int nw, void* energy_host, void* logdet_host, int* info_host, void* stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * The AFQMC block around the step: one-body half steps, hybrid importance
+ * function with the phaseless weight update, walker orthogonalisation, mixed estimator.
+ * "A block is 20 iterations of the propagation step followed by an energy evaluation and walker
+ * orthogonalization; the 'hybrid' method is used for propagation".
+ * ------------------------------------------------------------------------------------------------ */
+
+/*
+ * One-body half-step propagator of Eq. 7/13:  B1[k] = exp(-dtau/2 * h1p[k]) per k-point
+ * (H1' is block diagonal in k, Eq. 45), by scaling and squaring of a Taylor series on the
+ * device; stored in the context for afqmc_apply_onebody / afqmc_block.
+ *   h1p [Nk][m][m] device, complex128: the one-body operator to propagate with (the paper's H1' = H1 + v0,
+ *       Eq. 10; building v0 is outside this library).  Need not be Hermitian.
+ *   b1_out: device [Nk][m][m] or NULL; receives a copy of B1.
+ */
+int afqmc_set_onebody(afqmc_ctx* ctx, const void* h1p, double dtau, void* b1_out, void* stream);
+
+/* phi_w[(k,:), :] <- B1[k] phi_w[(k,:), :] for every walker and k-point, in place (Eq. 13).
+ * AFQMC_INVALID_ARGUMENT if afqmc_set_onebody was never called.   phi: device [nw][M][N]. */
+int afqmc_apply_onebody(afqmc_ctx* ctx, void* phi, int nw, void* stream);
+
+/*
+ * Hybrid importance function and phaseless weight update, Eq. 16, 18, 19, for the step
+ * whose fields were x and whose force bias was vbias (the arrays given to afqmc_vhs):
+ *   z, zbar as in afqmc_vhs;   x.xbar = sum_{Q,g} z_{Q g} zbar_{-Q g},   xbar.xbar = sum_{Q,g} zbar_{Q g} zbar_{-Q g}
+ *   log I_w  = 2 (logdet_new[w] - logdet_old[w]) + x.xbar - xbar.xbar/2      (closed shell: two spin channels)
+ *   dtheta_w = Im 2 (logdet_new[w] - logdet_old[w]) wrapped to (-pi, pi]        (Eq. 19)
+ *   weight[w] <- weight[w] * |I_w| * max(0, cos dtheta_w)                       (Eq. 18)
+ *   x [nw][Nk][nchol] double, vbias [nw][Nk][nchol] complex, logdet_old/new [nw] complex (afqmc_overlap of the
+ *   walker before / after the propagation), weight [nw] double in/out, log_i [nw] complex out or NULL: device.
+ */
+int afqmc_hybrid_weight(afqmc_ctx* ctx, const double* x, const void* vbias, double dtau, const void* logdet_old,
+                        const void* logdet_new, int nw, double* weight, void* log_i, void* stream);
+
+/*
+ * Walker orthogonalisation: phi_w <- Q_w of the thin QR  phi_w = Q_w R_w  with R_w upper
+ * triangular and a real positive diagonal (unique), by two passes of Cholesky-QR on the device
+ * (Gram matrix, Cholesky factor, phi R^{-1}).  logdet_r[w] = log det R_w (real; device double [nw] or NULL).
+ * info[w] (device int32 [nw] or NULL): 0, or j > 0 if the Gram matrix was not positive definite at column j
+ * (rank-deficient walker; phi_w is then undefined).  In place.
+ */
+int afqmc_orthogonalize(afqmc_ctx* ctx, void* phi, int nw, double* logdet_r, int* info, void* stream);
+
+/*
+ * Mixed estimator, Eq. 35:  out[0..2] = sum_w weight[w] * energy[w][0..2],  out[3] = sum_w weight[w]
+ * (E_mixed = (out[0]+out[1]+out[2]) / out[3]), summed in walker order (deterministic).
+ *   energy [nw][3] complex, weight [nw] double, out [4] complex: device.
+ */
+int afqmc_mixed_estimator(afqmc_ctx* ctx, const void* energy, const double* weight, int nw, void* out, void* stream);
+
+/*
+ * One block on DEVICE buffers: for s < nsteps:  green(phi) -> force_bias -> vhs(x[s], vbias, dtau) ->
+ * B1, Taylor(order), B1 on phi -> overlap(phi') -> hybrid weight update;   then green + local_energy on the
+ * final walkers, the mixed estimator with the final weights, and afqmc_orthogonalize.  The overlap of step s's
+ * new walker is the green() of step s+1 (computed once).
+ *   phi [nw][M][N] in/out; weight [nw] double in/out; x [nsteps][nw][Nk][nchol] double;
+ *   energy [nw][3], emixed [4] complex out; logdet_r [nw] double out or NULL; info [nw] int32 out or NULL
+ *   (first non-zero of: singular overlap at any step, non positive definite Gram matrix): device.
+ * Needs afqmc_set_onebody.
+ */
+int afqmc_block(afqmc_ctx* ctx, void* phi, double* weight, const double* x, double dtau, int order, int nsteps,
+                int nw, void* energy, void* emixed, double* logdet_r, int* info, void* stream);
+
 /* Number of kernels the context has launched so far (for bench.py's gpu_launches). */
 long long afqmc_launch_count(const afqmc_ctx* ctx);
 

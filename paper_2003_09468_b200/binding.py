@@ -31,7 +31,9 @@ class Dims(ctypes.Structure):
 
 EXPORTS = ["afqmc_strerror", "afqmc_create", "afqmc_destroy", "afqmc_overlap", "afqmc_green", "afqmc_force_bias",
            "afqmc_vhs", "afqmc_propagate", "afqmc_local_energy", "afqmc_step", "afqmc_step_host",
-           "afqmc_launch_count", "afqmc_exchange_flops", "afqmc_set_option", "afqmc_stage_times", "afqmc_probe_fp64"]
+           "afqmc_launch_count", "afqmc_exchange_flops", "afqmc_set_option", "afqmc_stage_times", "afqmc_probe_fp64",
+           "afqmc_set_onebody", "afqmc_apply_onebody", "afqmc_hybrid_weight", "afqmc_orthogonalize",
+           "afqmc_mixed_estimator", "afqmc_block"]
 
 
 def lib():
@@ -64,6 +66,12 @@ def lib():
     L.afqmc_set_option.argtypes = [vp, ctypes.c_char_p, ci]
     L.afqmc_probe_fp64.argtypes = [ci, ci, ctypes.POINTER(cd)]
     L.afqmc_stage_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+    L.afqmc_set_onebody.argtypes = [vp, vp, cd, vp, vp]
+    L.afqmc_apply_onebody.argtypes = [vp, vp, ci, vp]
+    L.afqmc_hybrid_weight.argtypes = [vp, vp, vp, cd, vp, vp, ci, vp, vp, vp]
+    L.afqmc_orthogonalize.argtypes = [vp, vp, ci, vp, vp, vp]
+    L.afqmc_mixed_estimator.argtypes = [vp, vp, vp, ci, vp, vp]
+    L.afqmc_block.argtypes = [vp, vp, vp, vp, cd, ci, ci, ci, vp, vp, vp, vp, vp]
     for name in EXPORTS:
         if name not in ("afqmc_strerror", "afqmc_destroy", "afqmc_launch_count", "afqmc_exchange_flops"):
             getattr(L, name).restype = ci
@@ -219,6 +227,58 @@ class Afqmc:
                                      _ptr(logdet_host, optional=True), _ptr(info_host, optional=True), _stream()),
                "afqmc_step_host")
         return energy_host
+
+
+    # ---- the AFQMC block (include/afqmc.h "The AFQMC block") ----------------------------------------
+    def set_onebody(self, h1p, dtau, b1_out=None):
+        """B1[k] = exp(-dtau/2 h1p[k]) computed on the device and kept in the context; returns a copy."""
+        if tuple(h1p.shape) != (self.nk, self.m, self.m):
+            raise ValueError("h1p must have shape (Nk, m, m)")
+        b1_out = self._empty((self.nk, self.m, self.m)) if b1_out is None else b1_out
+        _check(lib().afqmc_set_onebody(self._h, _ptr(h1p, torch.complex128), float(dtau), _ptr(b1_out, torch.complex128),
+                                       _stream()), "afqmc_set_onebody")
+        return b1_out
+
+    def apply_onebody(self, phi):
+        _check(lib().afqmc_apply_onebody(self._h, _ptr(phi, torch.complex128), phi.shape[0], _stream()),
+               "afqmc_apply_onebody")
+        return phi
+
+    def hybrid_weight(self, x, vbias, dtau, logdet_old, logdet_new, weight, log_i=None):
+        nw = x.shape[0]
+        log_i = self._empty((nw,)) if log_i is None else log_i
+        _check(lib().afqmc_hybrid_weight(self._h, _ptr(x, torch.float64), _ptr(vbias, torch.complex128), float(dtau),
+                                         _ptr(logdet_old, torch.complex128), _ptr(logdet_new, torch.complex128), nw,
+                                         _ptr(weight, torch.float64), _ptr(log_i, torch.complex128), _stream()),
+               "afqmc_hybrid_weight")
+        return weight, log_i
+
+    def orthogonalize(self, phi, logdet_r=None, info=None):
+        nw = phi.shape[0]
+        logdet_r = self._empty((nw,), torch.float64) if logdet_r is None else logdet_r
+        info = self._empty((nw,), torch.int32) if info is None else info
+        _check(lib().afqmc_orthogonalize(self._h, _ptr(phi, torch.complex128), nw, _ptr(logdet_r, torch.float64),
+                                         _ptr(info, torch.int32), _stream()), "afqmc_orthogonalize")
+        return phi, logdet_r, info
+
+    def mixed_estimator(self, energy, weight, out=None):
+        out = self._empty((4,)) if out is None else out
+        _check(lib().afqmc_mixed_estimator(self._h, _ptr(energy, torch.complex128), _ptr(weight, torch.float64),
+                                           energy.shape[0], _ptr(out, torch.complex128), _stream()), "afqmc_mixed_estimator")
+        return out
+
+    def block(self, phi, weight, x, dtau, order, energy=None, emixed=None, logdet_r=None, info=None):
+        """x [nsteps][nw][Nk][nchol]; phi and weight are updated in place."""
+        nsteps, nw = int(x.shape[0]), int(phi.shape[0])
+        energy = self._empty((nw, 3)) if energy is None else energy
+        emixed = self._empty((4,)) if emixed is None else emixed
+        logdet_r = self._empty((nw,), torch.float64) if logdet_r is None else logdet_r
+        info = self._empty((nw,), torch.int32) if info is None else info
+        _check(lib().afqmc_block(self._h, _ptr(phi, torch.complex128), _ptr(weight, torch.float64),
+                                 _ptr(x, torch.float64), float(dtau), int(order), nsteps, nw,
+                                 _ptr(energy, torch.complex128), _ptr(emixed, torch.complex128),
+                                 _ptr(logdet_r, torch.float64), _ptr(info, torch.int32), _stream()), "afqmc_block")
+        return energy, emixed, logdet_r, info
 
 
 def from_problem(pb, max_walkers=None, device="cuda"):

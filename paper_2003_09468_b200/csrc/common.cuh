@@ -59,6 +59,15 @@ struct afqmc_ctx {
     double2* ws_energy; // [nw][3]
     double2* ws_logdet; // [nw]
     int* ws_info;       // [nw]
+    // the block (block.cu)
+    double2* b1;        // [Nk][m][m] one-body half-step propagator exp(-dtau/2 h1p); valid iff b1_set
+    double2* ws_b1tmp;  // [Nk][3][m][m] scratch of the matrix exponential
+    double2* ws_gram;   // [nw][N][N] Gram matrix / Cholesky factor of the orthogonalisation
+    double2* ws_rinv;   // [nw][N][N] inverse of the triangular factor
+    double2* ws_logdet2;// [nw] overlap of the walker before the propagation
+    double* ws_ldr;     // [2][nw] log det R of the two Cholesky-QR passes
+    int* ws_info2;      // [2][nw] status of the two Cholesky passes
+    int b1_set;
     long long launches;
     int opt_exchange_depth; // 0/3 = three k-steps of fragment prefetch, 2 = two
     int opt_fb_tile;        // tuning aid: warp tile of the force-bias kernel for > 16 walkers (0: 2x8, 1: 4x8, 2: 4x4 m x n tiles)
@@ -144,6 +153,7 @@ int afqmc_i_vhs(afqmc_ctx* c, const double* x, const double2* vbias, double dtau
 int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, double2* phi, int nw,
                       cudaStream_t st);
 int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* energy, cudaStream_t st);
+int afqmc_i_apply_onebody(afqmc_ctx* c, double2* phi, int nw, cudaStream_t st);
 size_t afqmc_i_taylor_ws_doubles(const Dims& d);   // per-walker doubles of one expanded Taylor buffer
 // records stage event i on st when timers are on
 static inline void afqmc_mark(afqmc_ctx* c, int i, cudaStream_t st) {

@@ -154,7 +154,8 @@ AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     if (!c) return;
     void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lx, c->Lf, c->Lv,
                     c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T, c->ws_Tx,
-                    c->ws_expart, c->ws_fbpart, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info};
+                    c->ws_expart, c->ws_fbpart, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
+                    c->b1, c->ws_b1tmp, c->ws_gram, c->ws_rinv, c->ws_logdet2, c->ws_ldr, c->ws_info2};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     for (cudaEvent_t e : c->ev)
@@ -255,6 +256,13 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     A(dev_alloc(&c->ws_energy, (size_t)nw * 3));
     A(dev_alloc(&c->ws_logdet, (size_t)nw));
     A(dev_alloc(&c->ws_info, (size_t)nw));
+    A(dev_alloc(&c->b1, (size_t)Nk * d.m * d.m));
+    A(dev_alloc(&c->ws_b1tmp, (size_t)Nk * 3 * d.m * d.m));
+    A(dev_alloc(&c->ws_gram, (size_t)nw * d.N * d.N));
+    A(dev_alloc(&c->ws_rinv, (size_t)nw * d.N * d.N));
+    A(dev_alloc(&c->ws_logdet2, (size_t)nw));
+    A(dev_alloc(&c->ws_ldr, (size_t)2 * nw));
+    A(dev_alloc(&c->ws_info2, (size_t)2 * nw));
     if (rc != AFQMC_OK) { afqmc_destroy(c); return rc; }
 
     auto H2D = [&](void* dst, const void* src, size_t bytes) {

@@ -134,9 +134,16 @@ def make_walkers(cfg: Config, psi_t, rng, nw=None, noise=0.1):
     return phi
 
 
-def make_problem(cfg: Config, nw=None) -> Problem:
+def make_problem(cfg: Config, nw=None, l_scale=1.0) -> Problem:
+    """`l_scale` multiplies L after the draw (same random stream).  1.0 is BASELINE.json's recipe, whose
+    sqrt(dtau)*vHS has norm 2-16 (R9): every kernel is tested there, but in a hybrid AFQMC block such
+    steps rotate the overlap phase by more than pi/2 and the phaseless projection sets most weights to 0.  The
+    block tests and the block bench therefore also use a 'physically scaled' L (l_scale ~ 0.05-0.1, steps of
+    norm < 1), as SURVEY.md P9 suggests; shapes and structure are unchanged."""
     rng = np.random.default_rng(cfg.seed)
     h1, psi_t, L = make_hamiltonian(cfg, rng)
+    if l_scale != 1.0:
+        L *= l_scale
     phi = make_walkers(cfg, psi_t, rng, nw)
     x = rng.standard_normal((phi.shape[0], cfg.nk, cfg.nchol))
     return Problem(cfg, h1, psi_t, L, phi, x)
