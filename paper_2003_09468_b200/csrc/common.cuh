@@ -41,6 +41,7 @@ struct afqmc_ctx {
     double2* psi_t; // [Nk][m][n]
     double2* ht;    // [Nk][n][m]   half-rotated one-body
     double* Lx;     // exchange fragment layout  [Q][k][ag][gq][s][lane][2]
+    double* Lx3;    // exchange, 3M products      [Q][k][ag][gq][ks][prod][lane][2]   (exchange3m.cu; n <= 4 only, else NULL)
     double* Lf;     // force-bias fragment layout [Q][gtp][k][a][s][lane][2]
     double* Lv;     // vHS fragment layout        [Q][k][prt][s][lane]
     // workspace (sized by max_walkers)
@@ -73,6 +74,7 @@ struct afqmc_ctx {
     int opt_fb_tile;        // tuning aid: warp tile of the force-bias kernel for > 16 walkers (0: 2x8, 1: 4x8, 2: 4x4 m x n tiles)
     int opt_fb_pf;          // L2 prefetch distance (k-steps) of the Lf stream in the force-bias kernel
     int opt_exchange_minb;  // tuning aid: 1 = ask for more resident CTAs per SM
+    int opt_exchange_3m;    // 1 (default) = 3M exchange kernel when n <= 4, 0 = the 4M kernel of energy.cu
     int opt_exchange_wpc;   // 0 = automatic, else warps per CTA of the exchange kernel (4,5,6,8)
     int opt_timers;     // record stage events in afqmc_step
     int opt_taylor_legacy;  // testing aid: 1 = shared-memory-tiled zgemm for the Taylor chain
@@ -153,6 +155,9 @@ int afqmc_i_vhs(afqmc_ctx* c, const double* x, const double2* vbias, double dtau
 int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, double2* phi, int nw,
                       cudaStream_t st);
 int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* energy, cudaStream_t st);
+int afqmc_i_exchange3m(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st);   // AFQMC_UNSUPPORTED if n > 4
+int afqmc_i_pack_lx3(afqmc_ctx* c, const double2* L, cudaStream_t st);
+size_t afqmc_i_lx3_doubles(const Dims& d);
 int afqmc_i_apply_onebody(afqmc_ctx* c, double2* phi, int nw, cudaStream_t st);
 size_t afqmc_i_taylor_ws_doubles(const Dims& d);   // per-walker doubles of one expanded Taylor buffer
 // records stage event i on st when timers are on

@@ -152,7 +152,7 @@ static int dev_alloc(T** p, size_t count) {
 
 AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     if (!c) return;
-    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lx, c->Lf, c->Lv,
+    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lx, c->Lx3, c->Lf, c->Lv,
                     c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T, c->ws_Tx,
                     c->ws_expart, c->ws_fbpart, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
                     c->b1, c->ws_b1tmp, c->ws_gram, c->ws_rinv, c->ws_logdet2, c->ws_ldr, c->ws_info2};
@@ -191,6 +191,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     d.PRT = (d.m * d.m + 7) / 8;
     c->max_walkers = dims->max_walkers;
     c->opt_fb_pf = 8;
+    c->opt_exchange_3m = 1;
     const int nw = c->max_walkers;
 
     int dev = 0;
@@ -238,6 +239,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     A(dev_alloc(&c->psi_t, (size_t)Nk * d.m * d.n));
     A(dev_alloc(&c->ht, (size_t)Nk * d.n * d.m));
     A(dev_alloc(&c->Lx, nLx));
+    if (d.NAG == 1) A(dev_alloc(&c->Lx3, afqmc_i_lx3_doubles(d)));
     A(dev_alloc(&c->Lf, nLf));
     A(dev_alloc(&c->Lv, nLv));
     A(dev_alloc(&c->ws_O, (size_t)nw * d.N * LD));
@@ -287,6 +289,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
         pack_Lv_kernel<<<grid(nLv), T, 0, st>>>(d, (const double2*)L, c->Lv, nLv);
         c->launches += 4;
         if (cudaGetLastError() != cudaSuccess) rc = AFQMC_CUDA_ERROR;
+        if (rc == AFQMC_OK && c->Lx3) rc = afqmc_i_pack_lx3(c, (const double2*)L, st);
     }
     // host vectors must outlive the async copies; the caller may free its arrays after return
     if (cudaStreamSynchronize(st) != cudaSuccess && rc == AFQMC_OK) rc = AFQMC_CUDA_ERROR;
@@ -300,9 +303,11 @@ AFQMC_API long long afqmc_launch_count(const afqmc_ctx* c) { return c ? c->launc
 AFQMC_API double afqmc_exchange_flops(const afqmc_ctx* c, int nw) {
     if (!c) return 0.0;
     const Dims& d = c->d;
-    // per unit and walker: two complex GEMMs (n x m)(m x n) per gamma = 2 * 8*n*n*m*nchol real flops,
-    // plus the complex contraction 8*n*n*nchol.
+    // per unit and walker: two complex GEMMs (n x m)(m x n) per gamma, plus the complex contraction 8*n*n*nchol.
+    // 4M kernel: 8 real flops per complex multiply-add = 2 * 8*n*n*m*nchol.  3M kernel (exchange3m.cu): 6 real
+    // flops per complex multiply-add = 2 * 6*n*n*m*nchol, plus 3 additions per element of both T tensors.
     double per = 16.0 * d.n * d.n * d.m * d.nchol + 8.0 * d.n * d.n * d.nchol;
+    if (c->opt_exchange_3m && c->Lx3) per = 12.0 * d.n * d.n * d.m * d.nchol + 6.0 * d.n * d.n * d.nchol + 8.0 * d.n * d.n * d.nchol;
     return per * (double)c->nunits * (double)nw;
 }
 
@@ -321,6 +326,10 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
     if (strcmp(name, "force_bias_prefetch") == 0) {
         if (value < 0 || value > 256) return AFQMC_INVALID_ARGUMENT;
         c->opt_fb_pf = value;
+        return AFQMC_OK;
+    }
+    if (strcmp(name, "exchange_3m") == 0) {
+        c->opt_exchange_3m = value ? 1 : 0;
         return AFQMC_OK;
     }
     if (strcmp(name, "exchange_minblocks") == 0) {
