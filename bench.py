@@ -31,9 +31,9 @@ METRIC = "walker-steps/s incl. local energy"
 UNIT = "walker-steps/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE exchange-kernel launch, from the committed
-# `ncu --set full` capture of this same command (profiles/r01c_ncu_full_metrics.txt); bench.py cannot
-# measure DRAM traffic itself.  Only the configuration that was captured has a value.
-EXCHANGE_DRAM_TRAFFIC = {"C3": {"bytes": 389.341e6 + 9.110e6, "source": "profiles/r01c_ncu_full_metrics.txt"}}
+# `ncu --set full` capture of this same command (profiles/r01d_ncu_full_metrics.txt, the default 3M kernel); bench.py
+# cannot measure DRAM traffic itself.  Only the configuration that was captured has a value.
+EXCHANGE_DRAM_TRAFFIC = {"C3": {"bytes": 719.947e6 + 11.857e6, "source": "profiles/r01d_ncu_full_metrics.txt"}}
 
 
 def load_measured_peaks():
@@ -192,6 +192,21 @@ def run_ours(args):
     assert int(info.abs().sum().item()) == 0
     e_dev = energy.cpu().numpy().copy()
 
+    # ---------------- the 4M exchange kernel (energy.cu) for comparison: a few untimed-for-the-metric steps -------------
+    ex_flops_default = ctx.exchange_flops(nw)
+    ctx.set_option("exchange_3m", 0)
+    ex_flops_4m = ctx.exchange_flops(nw)
+    ex4_ms = 0.0
+    for i in range(4):
+        phi.copy_(phi0)
+        ctx.step(phi, x, cfg.dtau, cfg.order, energy, logdet, info)
+        torch.cuda.synchronize()
+        if i > 0:
+            ex4_ms += ctx.stage_times()["exchange"] / 3
+    e_4m = energy.cpu().numpy().copy()
+    ctx.set_option("exchange_3m", 1)
+    assert np.max(np.abs(e_4m - e_dev) / np.abs(e_dev)) < 1e-10, "3M and 4M exchange kernels disagree"
+
     # ---------------- end to end through the host-buffer C-ABI call ----------------
     phi_h0 = torch.from_numpy(pb.phi).pin_memory()
     phi_h = torch.empty_like(phi_h0).pin_memory()
@@ -225,11 +240,12 @@ def run_ours(args):
         e2e_value = total_walkers * args.steps / (e2e_ms_max * 1e-3)
         # ---- roofline of the dominant kernel (exchange contraction, a9) ----
         ex_ms = stage_acc["exchange"] / args.steps
-        ex_flops = ctx.exchange_flops(nw)
+        ex_flops = ex_flops_default
         achieved = ex_flops / (ex_ms * 1e-3) / 1e12
         peak_probe = binding.probe_fp64(1, 20000)          # DMMA issue-rate probe, this GPU, now
-        # algorithmic bytes of one exchange launch: packed Lh once + theta once + partial sums
-        ctx_alg_bytes = cfg.nk ** 2 * cfg.n * cfg.nchol * cfg.m * 16 + nw * cfg.N * cfg.M * 16
+        # algorithmic bytes of one exchange launch: the packed operand once (Lx3 of the 3M kernel: Re+Im, Re, Im of
+        # Lh with r padded to a multiple of 4 = 24 bytes per complex element) + theta once
+        ctx_alg_bytes = cfg.nk ** 2 * cfg.n * cfg.nchol * (4 * ((cfg.m + 3) // 4)) * 24 + nw * cfg.N * cfg.M * 16
         peaks = load_measured_peaks()
         roofline = {
             "kernel": "exchange (a9), afqmc_local_energy", "bound": "tensor", "achieved": achieved,
@@ -240,6 +256,11 @@ def run_ours(args):
             "algorithmic_bytes": float(ctx_alg_bytes),
             "peak_source": "live FP64 DMMA.8x8x4 probe (afqmc_probe_fp64); MEASURED_PEAKS.json has no FP64 entry",
             "flops_per_launch": ex_flops, "ms_per_launch": ex_ms,
+            "flops_note": "EXECUTED real flops of the default kernel (3M complex product when n <= 4: 6 per complex "
+                          "multiply-add, unpadded; the K = m padding to 4 is not counted)",
+            "variant_4m": {"ms_per_launch": ex4_ms, "flops_per_launch": ex_flops_4m,
+                           "achieved": ex_flops_4m / (ex4_ms * 1e-3) / 1e12, "frac": ex_flops_4m / (ex4_ms * 1e-3) / 1e12 / peak_probe,
+                           "note": "one real GEMM with 8 flops per complex multiply-add (energy.cu), option exchange_3m=0"},
             "share_of_step": ex_ms / (dev_ms_max / args.steps),
         }
         if peaks and "bf16_tflops" in peaks:

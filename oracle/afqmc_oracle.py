@@ -28,6 +28,11 @@ Phi -> Phi R).  No function here is "parity unpinned"; the field-assembly rule
 (`assemble_fields`, reading R7) and the Taylor order (R8) are conventions pinned
 only by level D of this file, as DESIGN.md states.
 
+The AFQMC-block functions at the end of the file (one-body half steps, hybrid weight,
+orthogonalisation, mixed estimator, block) are pinned by tests/test_oracle_block_pins.py (real-field Hermitian
+restatement, Gauss-Hermite quadrature of Eq. 12/16, Wick's theorem, scipy expm, numpy QR); none is "parity
+unpinned".  `numpy.linalg.det` / `inv` appear only in level D.
+
 Layouts (row-major, last index fastest):
   L[Q][k][gamma][p][r]   p at k-point k, r at k-Q
   psi_t[k][p][a]         trial, block diagonal in k

@@ -337,7 +337,7 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
         return AFQMC_OK;
     }
     if (strcmp(name, "exchange_depth") == 0) {
-        if (value != 0 && value != 2 && value != 3) return AFQMC_INVALID_ARGUMENT;
+        if (value != 0 && value != 2 && value != 3 && value != 6) return AFQMC_INVALID_ARGUMENT;
         c->opt_exchange_depth = value;
         return AFQMC_OK;
     }

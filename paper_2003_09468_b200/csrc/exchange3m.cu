@@ -2,22 +2,24 @@
 //
 //   T = Lh * theta^T  is a complex GEMM.  energy.cu embeds it in ONE real GEMM with K = (r, re/im) and columns
 //   (b, re/im): 8 real flops per complex multiply-add (4 real products).  Here every complex product is formed
-//   from THREE real products (Karatsuba / "3M"):
-//       P0 = Ar Br,  P1 = Ai Bi,  P2 = (Ar+Ai)(Br+Bi);      Re T = P0 - P1,   Im T = P2 - P0 - P1
+//   from THREE real products (Gauss's form of the "3M" product: two additions per result instead of Karatsuba's three,
+//   which matters because DADD shares the FP64 units with DMMA):
+//       P0 = (Ar+Ai) Br,  P1 = Ar (Bi-Br),  P2 = Ai (Br+Bi);      Re T = P0 - P2,   Im T = P0 + P1
 //   i.e. three real GEMMs with K = r and columns b: 6 real flops per complex multiply-add, 25 % fewer DMMAs
 //   (19 % at m = 26, where K = 26 pads to 7 k-steps of 4).  The tensor pipe is the bound of this kernel
 //   (89 % DMMA issue, r01c profile), so fewer DMMAs is the only lever left.  Rounding: Im T carries the error of
 //   (|Ar|+|Ai|)(|Br|+|Bi|) instead of |A||B|: a small constant factor, far inside the 1e-10 tolerance.
 //
 // Layout of the static operand (written once in afqmc_create):
-//   Lx3[Q][k][ag][gq][ks][prod][lane][i]   prod = 0: Re Lh, 1: Im Lh, 2: Re + Im;  two M-tiles i = 0,1 per gamma-quad
+//   Lx3[Q][k][ag][gq][ks][prod][lane][i]   prod = 0: Re + Im of Lh, 1: Re, 2: Im;  two M-tiles i = 0,1 per gamma-quad
 //   rows (gl = row>>2, al = row&3): gamma = 4gq+2i+gl, a = 4ag+al;  K: r = 4ks + (lane&3);  zeros outside.
 // A warp task is one gamma-quad: 3*KS3 "micro-steps" (ks-major, product-minor), each ONE coalesced 512-byte LDG.128
 // of A, consecutive in memory across micro-steps and tasks.  DMMA columns are (walker of a pair, b): one n-tile
 // serves two walkers, a CTA handles 2*NP walkers.  The three products keep separate accumulators; the register
 // pipeline is 3 deep and unrolled by 3, so buffer q always belongs to product q (static register indexing).
-// At the end of a task the products are combined, the partner tile is transposed across lanes by shuffles and
-// contracted in registers, exactly as in energy.cu.  Only n <= 4 (one a-group) is handled here; larger n uses
+// At the end of a task the products are combined and contracted in registers.  The partner tile is computed with
+// the DMMA operands swapped (theta as A, Lh as B: the two fragment lane layouts coincide), which yields it already
+// transposed in (a,b); one shuffle per value (lane bits 4 and 1 exchanged) then aligns gamma and walker.  Only n <= 4 (one a-group) is handled here; larger n uses
 // the 4M kernel.
 #include "common.cuh"
 
@@ -49,9 +51,9 @@ __global__ void pack_Lx3_kernel(Dims d, int KS3, const double2* __restrict__ L, 
         }
         // [..][ks][prod][lane][i]
         const size_t base = ((((((size_t)Q * d.Nk + k) * d.NAG + ag) * d.GQ + gq) * KS3 + ks) * 3) * 64 + lane * 2 + i;
-        Lx3[base] = z.x;
-        Lx3[base + 64] = z.y;
-        Lx3[base + 128] = z.x + z.y;
+        Lx3[base] = z.x + z.y;
+        Lx3[base + 64] = z.x;
+        Lx3[base + 128] = z.y;
     }
     // zero pad after the last block (the kernel's prefetch may run 3 micro-steps past the last task)
     const size_t body = total_in * 3;
@@ -81,7 +83,8 @@ int afqmc_i_pack_lx3(afqmc_ctx* c, const double2* L, cudaStream_t st) {
 namespace {
 
 // CTA = (unit, group of 2*NP walkers), WPC warps; see the header comment.  n <= 4 only (NAG == 1).
-template <int NP, int WPC, int MINB>
+// DA = micro-steps of register prefetch of the A (Lx3, L2-resident) stream: 3 or 6; B (shared memory) runs 3 ahead.
+template <int NP, int WPC, int MINB, int DA>
 __global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_kernel(
     Dims d, int KS3, int nw, const int* __restrict__ units, const int* __restrict__ kminus, const int* __restrict__ kplus,
     const int* __restrict__ kneg, const double* __restrict__ Lx3, const double2* __restrict__ theta,
@@ -110,20 +113,21 @@ __global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_kernel(
     const double* lb2 = ex3_smem + bs_half + lane;
     int ls = 0;
     auto loader_advance = [&]() {        // A is contiguous across micro-steps and tasks, B wraps every MS micro-steps
-        la1 += 32; la2 += 32;
         const bool wrap = ++ls == MS;
         const int db = wrap ? -(MS - 1) * bs_step : bs_step;
         lb1 += db; lb2 += db;
         ls = wrap ? 0 : ls;
     };
-    double2 fa1[3], fa2[3];
+    static_assert(DA == 3 || DA == 6, "A depth is a multiple of the three products");
+    double2 fa1[DA], fa2[DA];
     double fb1[3][NP], fb2[3][NP];
     // A prologue: issued before the staging below, which hides the L2 round trip
 #pragma unroll
-    for (int q = 0; q < 3; ++q) {
+    for (int q = 0; q < DA; ++q) {
         fa1[q] = fa2[q] = make_double2(0.0, 0.0);
         if (total > 0) { fa1[q] = __ldg(la1 + q * 32); fa2[q] = __ldg(la2 + q * 32); }
     }
+    la1 += DA * 32; la2 += DA * 32;
 
     // ---- stage the B fragments: one thread per complex theta element (b, walker, r) ----
     //   lane of a B fragment = (col << 2) | kk,  col = 4*(w&1) + b,  kk = r & 3;  micro-step = 3*(r>>2) + prod
@@ -141,7 +145,7 @@ __global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_kernel(
                 v = __ldg(theta + ((size_t)w * d.N + rowblk * d.n + b) * d.M + (size_t)colblk * d.m + r);
             double* dst = ex3_smem + which * bs_half + ((3 * (r >> 2)) * NP + (wl >> 1)) * 32 + (((wl & 1) * 4 + b) << 2) + (r & 3);
             dst[0] = v.x;
-            dst[bs_step] = v.y;
+            dst[bs_step] = v.y - v.x;
             dst[2 * bs_step] = v.x + v.y;
         }
     }
@@ -158,13 +162,12 @@ __global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_kernel(
     double er[NP], ei[NP];
 #pragma unroll
     for (int j = 0; j < NP; ++j) er[j] = ei[j] = 0.0;
-    // lane geometry of a C fragment: row = lane>>2 = (gamma in pair, a), columns 2c, 2c+1 with c = lane&3:
-    // walker-in-pair wp = c>>1, b = 2*(c&1) + e for register e.  The partner element T2[(g,b),(wp,a)] is register
-    // (a&1) of lane (row' = (g, b), c' = 2wp + (a>>1)).
-    const int a_l = (lane >> 2) & 3, c_l = lane & 3;
-    const int src0 = (lane & 16) | ((2 * (c_l & 1) + 0) << 2) | (2 * (c_l >> 1) + (a_l >> 1));
-    const int src1 = (lane & 16) | ((2 * (c_l & 1) + 1) << 2) | (2 * (c_l >> 1) + (a_l >> 1));
-    const bool asel = (a_l & 1) != 0;
+    // lane geometry of the C fragments (row = lane>>2, columns 2c+e with c = lane&3, register e):
+    //   T1   : row (gamma of pair g, a),   columns (walker of pair wp = c>>1, b = 2(c&1)+e)
+    //   T2^T : row (walker of pair wp, a), columns (gamma of pair g = c>>1,  b = 2(c&1)+e)
+    // The contraction sum_{a,b} T1[(g,a),(wp,b)] T2[(g,b),(wp,a)] = sum T1[(g,a),(wp,b)] T2^T[(wp,a),(g,b)] pairs
+    // register e of lane (g, a | wp, c&1) with register e of lane (wp, a | g, c&1): lane bits 4 and 1 exchanged.
+    const int srcl = (lane & ~0x12) | ((lane & 16) >> 3) | ((lane & 2) << 3);
     double acc1[3][2][NP][2], acc2[3][2][NP][2];
 #pragma unroll
     for (int p = 0; p < 3; ++p)
@@ -175,19 +178,24 @@ __global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_kernel(
                 acc1[p][i][j][0] = acc1[p][i][j][1] = acc2[p][i][j][0] = acc2[p][i][j][1] = 0.0;
 
     int cs = 0;   // micro-step of the compute state inside its task
-    auto mstep = [&](const int q) {      // buffer q == product q
+    auto mstep = [&](const int qa) {     // A buffer qa; product and B buffer q = qa % 3
+        const int q = qa % 3;
 #pragma unroll
         for (int j = 0; j < NP; ++j) {
-            dmma884(acc1[q][0][j][0], acc1[q][0][j][1], fa1[q].x, fb1[q][j]);
-            dmma884(acc1[q][1][j][0], acc1[q][1][j][1], fa1[q].y, fb1[q][j]);
+            dmma884(acc1[q][0][j][0], acc1[q][0][j][1], fa1[qa].x, fb1[q][j]);
+            dmma884(acc1[q][1][j][0], acc1[q][1][j][1], fa1[qa].y, fb1[q][j]);
         }
+        // partner tile with the operands swapped: theta is the A fragment and Lh the B fragment (their lane
+        // layouts coincide), so the result is T2^T with rows (walker of pair, a) and columns (gamma of pair, b)
 #pragma unroll
         for (int j = 0; j < NP; ++j) {
-            dmma884(acc2[q][0][j][0], acc2[q][0][j][1], fa2[q].x, fb2[q][j]);
-            dmma884(acc2[q][1][j][0], acc2[q][1][j][1], fa2[q].y, fb2[q][j]);
+            dmma884(acc2[q][0][j][0], acc2[q][0][j][1], fb2[q][j], fa2[qa].x);
+            dmma884(acc2[q][1][j][0], acc2[q][1][j][1], fb2[q][j], fa2[qa].y);
         }
-        // refill buffer q with the micro-step 3 ahead (may run past the warp's last task: loaded, never used)
-        fa1[q] = __ldg(la1); fa2[q] = __ldg(la2);
+        // refill the buffers with the micro-steps DA (A) and 3 (B) ahead (may run past the warp's last task:
+        // loaded, never used)
+        fa1[qa] = __ldg(la1); fa2[qa] = __ldg(la2);
+        la1 += 32; la2 += 32;
 #pragma unroll
         for (int j = 0; j < NP; ++j) { fb1[q][j] = lb1[j * 32]; fb2[q][j] = lb2[j * 32]; }
         loader_advance();
@@ -202,17 +210,14 @@ __global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_kernel(
                         double t1r[2], t1i[2], t2r[2], t2i[2];
 #pragma unroll
                         for (int e = 0; e < 2; ++e) {
-                            t1r[e] = acc1[0][i][j][e] - acc1[1][i][j][e];
-                            t1i[e] = acc1[2][i][j][e] - acc1[0][i][j][e] - acc1[1][i][j][e];
-                            t2r[e] = acc2[0][i][j][e] - acc2[1][i][j][e];
-                            t2i[e] = acc2[2][i][j][e] - acc2[0][i][j][e] - acc2[1][i][j][e];
+                            t1r[e] = acc1[0][i][j][e] - acc1[2][i][j][e];
+                            t1i[e] = acc1[0][i][j][e] + acc1[1][i][j][e];
+                            t2r[e] = acc2[0][i][j][e] - acc2[2][i][j][e];
+                            t2i[e] = acc2[0][i][j][e] + acc2[1][i][j][e];
                         }
-                        const double r00 = __shfl_sync(0xffffffffu, t2r[0], src0), r01 = __shfl_sync(0xffffffffu, t2r[1], src0);
-                        const double i00 = __shfl_sync(0xffffffffu, t2i[0], src0), i01 = __shfl_sync(0xffffffffu, t2i[1], src0);
-                        const double r10 = __shfl_sync(0xffffffffu, t2r[0], src1), r11 = __shfl_sync(0xffffffffu, t2r[1], src1);
-                        const double i10 = __shfl_sync(0xffffffffu, t2i[0], src1), i11 = __shfl_sync(0xffffffffu, t2i[1], src1);
-                        const double pr0 = asel ? r01 : r00, pi0 = asel ? i01 : i00;     // partner of register 0 (b = 2(c&1))
-                        const double pr1 = asel ? r11 : r10, pi1 = asel ? i11 : i10;     // partner of register 1 (b = 2(c&1)+1)
+                        // T1 lane (g, a | wp, bp) pairs with T2^T lane (wp, a | g, bp), same register: swap lane bits 4 and 1
+                        const double pr0 = __shfl_sync(0xffffffffu, t2r[0], srcl), pi0 = __shfl_sync(0xffffffffu, t2i[0], srcl);
+                        const double pr1 = __shfl_sync(0xffffffffu, t2r[1], srcl), pi1 = __shfl_sync(0xffffffffu, t2i[1], srcl);
                         er[j] = fma(t1r[0], pr0, er[j]); er[j] = fma(-t1i[0], pi0, er[j]);
                         ei[j] = fma(t1r[0], pi0, ei[j]); ei[j] = fma(t1i[0], pr0, ei[j]);
                         er[j] = fma(t1r[1], pr1, er[j]); er[j] = fma(-t1i[1], pi1, er[j]);
@@ -226,6 +231,11 @@ __global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_kernel(
     };
     for (int g0 = 0; g0 < total; g0 += 3) {
         mstep(0); mstep(1); mstep(2);
+        if (DA == 6) {
+            if (g0 + 3 >= total) break;
+            g0 += 3;
+            mstep(DA - 3); mstep(DA - 2); mstep(DA - 1);
+        }
     }
 
     // ---- reduce over the lanes of each walker-in-pair (lane bit 1), then over warps (deterministic) ----
@@ -253,13 +263,13 @@ __global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_kernel(
     }
 }
 
-template <int NP, int WPC, int MINB>
+template <int NP, int WPC, int MINB, int DA>
 int launch_exchange3m_cfg(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     const Dims& d = c->d;
     const int KS3 = (d.m + 3) / 4;
     size_t smem = (size_t)2 * 3 * KS3 * NP * 32 * sizeof(double);
     if (smem < (size_t)WPC * 2 * NP * 2 * sizeof(double)) smem = (size_t)WPC * 2 * NP * 2 * sizeof(double);
-    auto kern = exchange3m_kernel<NP, WPC, MINB>;
+    auto kern = exchange3m_kernel<NP, WPC, MINB, DA>;
     static size_t attr_set = 0;
     if (smem > 48 * 1024 && smem > attr_set) {
         if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
@@ -281,6 +291,10 @@ int afqmc_i_exchange3m(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t 
     const Dims& d = c->d;
     if (d.NAG != 1 || !c->Lx3) return AFQMC_UNSUPPORTED;
     const int wpc = c->opt_exchange_wpc == 4 ? 4 : 2;
-    if (nw >= 3) return wpc == 4 ? launch_exchange3m_cfg<2, 4, 3>(c, theta, nw, st) : launch_exchange3m_cfg<2, 2, 6>(c, theta, nw, st);
-    return wpc == 4 ? launch_exchange3m_cfg<1, 4, 3>(c, theta, nw, st) : launch_exchange3m_cfg<1, 2, 6>(c, theta, nw, st);
+    const bool deep = c->opt_exchange_depth == 6;
+    if (nw >= 3) {
+        if (deep) return wpc == 4 ? launch_exchange3m_cfg<2, 4, 2, 6>(c, theta, nw, st) : launch_exchange3m_cfg<2, 2, 4, 6>(c, theta, nw, st);
+        return wpc == 4 ? launch_exchange3m_cfg<2, 4, 3, 3>(c, theta, nw, st) : launch_exchange3m_cfg<2, 2, 6, 3>(c, theta, nw, st);
+    }
+    return wpc == 4 ? launch_exchange3m_cfg<1, 4, 3, 3>(c, theta, nw, st) : launch_exchange3m_cfg<1, 2, 6, 3>(c, theta, nw, st);
 }

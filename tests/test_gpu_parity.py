@@ -308,6 +308,34 @@ def test_green_register_kernel_equals_legacy_kernel(small_case):
     assert np.max(phase_diff(ld_new.cpu().numpy().imag, ld_old.cpu().numpy().imag)) < 1e-12
 
 
+@pytest.mark.parametrize("kw", [dict(mesh=(2, 2, 1), m=6, n=4, nchol=10, nw=4), dict(mesh=(2, 3, 1), m=5, n=3, nchol=7, nw=5),
+                                dict(mesh=(1, 2, 2), m=9, n=1, nchol=5, nw=2), dict(mesh=(3, 1, 1), m=26, n=4, nchol=18, nw=7)],
+                         ids=["n4", "n3_odd", "n1_two_walkers", "m26_seven_walkers"])
+def test_exchange_3m_and_4m_kernels_against_the_oracle(kw):
+    """Both exchange kernels (exchange3m.cu: default for n <= 4; energy.cu: option exchange_3m=0) on the same theta,
+    each against the oracle, and against each other; the deep-prefetch variants of the 3M kernel too."""
+    case = Case(synth.tiny_config(seed=13, **kw))
+    try:
+        theta_d, _, _ = case.ctx.green(_to_dev(case.pb.phi))
+        theta = theta_d.cpu().numpy()
+        e_o = np.array([orc.local_energy(case.cfg.mesh, case.Lh, case.ht, theta[w]) for w in range(case.nw)])
+        res = {}
+        for name, opts in (("3m", {}), ("4m", {"exchange_3m": 0}), ("3m_deep", {"exchange_depth": 6}),
+                           ("3m_4warps", {"exchange_warps": 4}), ("3m_deep_4warps", {"exchange_depth": 6, "exchange_warps": 4})):
+            for k, v in opts.items():
+                case.ctx.set_option(k, v)
+            res[name] = case.ctx.local_energy(theta_d).cpu().numpy()
+            case.ctx.set_option("exchange_3m", 1)
+            case.ctx.set_option("exchange_depth", 0)
+            case.ctx.set_option("exchange_warps", 0)
+        for name, e in res.items():
+            for w in range(case.nw):
+                assert np.max(np.abs(e[w] - e_o[w]) / np.abs(e_o[w])) < RTOL, (name, w, e[w], e_o[w])
+        assert relerr(res["3m"], res["4m"]) < 1e-12
+    finally:
+        case.close()
+
+
 @pytest.mark.parametrize("mesh,n", [((4, 4, 3), 6), ((4, 3, 3), 7), ((5, 5, 1), 5)], ids=["N288_legacy", "N252_cluster8", "N125_cluster2"])
 def test_green_large_N(mesh, n):
     """Overlap sizes that select the cluster kernels (N <= 128: 2 CTAs, N <= 256: 8 CTAs) and the legacy path (N > 256)."""
