@@ -20,10 +20,10 @@
 namespace {
 
 constexpr int FB_WARPS = 4;
-constexpr int FB_D = 2;
+constexpr int FB_D = 3;   // k-steps of register prefetch (3 CTAs of 4 warps stay resident at 168 registers)
 
 template <int MP, int NT>
-__global__ void __launch_bounds__(32 * FB_WARPS) force_bias_kernel(
+__global__ void __launch_bounds__(32 * FB_WARPS, (MP * NT > 8 ? 2 : 3)) force_bias_kernel(
     Dims d, int nw, int KC, int nmg, int nwgrp, int pf, const int* __restrict__ kminus, const double* __restrict__ Lf,
     const double2* __restrict__ theta, double2* __restrict__ out, int out_is_partial) {
     extern __shared__ __align__(16) double fb_smem[];
