@@ -43,7 +43,10 @@ struct afqmc_ctx {
     double* Lx;     // exchange fragment layout  [Q][k][ag][gq][s][lane][2]
     double* Lx3;    // exchange, 3M products      [Q][k][ag][gq][ks][prod][lane][2]   (exchange3m.cu; n <= 4 only, else NULL)
     double* Lf;     // force-bias fragment layout [Q][gtp][k][a][s][lane][2]
-    double* Lv;     // vHS fragment layout        [Q][k][prt][s][lane]
+    double2* Lv3;   // vHS operand [unit][prt][ks][lane] complex fragments (vhs.cu); one block per (Q,-Q) pair if vhs_paired
+    int* vunits;    // vHS work units, int4-packed (Q, k, kind, 0) [nvunits]; kind 1 = block + its (-Q,k-Q) partner
+    int nvunits;
+    int vhs_paired; // 1 = the caller's L satisfies the (Q,-Q) identity (checked in afqmc_create): one block per pair stored
     // workspace (sized by max_walkers)
     double2* ws_O;      // [nw][N][LD]  elimination workspace when the matrix does not fit shared memory
     double2* ws_oinvT;  // [nw][N][N]   transposed inverse overlap
@@ -159,7 +162,8 @@ int afqmc_i_exchange3m(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t 
 int afqmc_i_pack_lx3(afqmc_ctx* c, const double2* L, cudaStream_t st);
 size_t afqmc_i_lx3_doubles(const Dims& d);
 int afqmc_i_apply_onebody(afqmc_ctx* c, double2* phi, int nw, cudaStream_t st);
-size_t afqmc_i_taylor_ws_doubles(const Dims& d);   // per-walker doubles of one expanded Taylor buffer
+size_t afqmc_i_taylor_ws_doubles(const Dims& d);
+size_t afqmc_i_vhs_field_doubles(const Dims& d, int nw);   // doubles of the expanded field operand (workspace ws_xi)   // per-walker doubles of one expanded Taylor buffer
 // records stage event i on st when timers are on
 static inline void afqmc_mark(afqmc_ctx* c, int i, cudaStream_t st) {
     if (c->opt_timers && c->ev[i]) cudaEventRecord(c->ev[i], st);

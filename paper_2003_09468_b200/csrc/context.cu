@@ -6,6 +6,9 @@
 #include <vector>
 #include "common.cuh"
 
+int afqmc_i_vhs_setup(afqmc_ctx* c, const double2* L, const std::vector<int>& kminus, const std::vector<int>& kneg,
+                      cudaStream_t st);   // vhs.cu
+
 AFQMC_API const char* afqmc_strerror(int code) {
     switch (code) {
         case AFQMC_OK: return "ok";
@@ -28,8 +31,7 @@ AFQMC_API const char* afqmc_strerror(int code) {
 //                        (+ AFQMC_LX_PAD zero doubles at the end: the kernel's prefetch may run past the last task)
 //  Lf (force bias, a4): [Q][gtp][k][a][s][lane][i] two M-tiles i = 0,1 per 16 gammas, interleaved per lane;
 //                        rows gamma = 16gtp+8i+row;  K = (r, part), per (k,a); one contiguous K stream per gtp
-//  Lv (vHS, a5):        [Q][k][prt][s][lane]      rows pr = 8prt+row (p = pr/m, r = pr%m);
-//                        K = (gamma, part) of L[Q][k][gamma][p][r]
+//  (the vHS operand Lv3 and the 3M exchange operand Lx3 are described and packed in vhs.cu / exchange3m.cu)
 // Out-of-range rows / K entries are stored as zeros, so kernels never branch on tails.
 // ---------------------------------------------------------------------------------------
 __device__ __forceinline__ double2 half_rot_elem(const double2* __restrict__ L, const double2* __restrict__ psi_t,
@@ -94,25 +96,6 @@ __global__ void pack_Lf_kernel(Dims d, const double2* __restrict__ L, const doub
     }
 }
 
-__global__ void pack_Lv_kernel(Dims d, const double2* __restrict__ L, double* __restrict__ Lv, size_t total) {
-    for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total;
-         idx += (size_t)gridDim.x * blockDim.x) {
-        size_t t = idx;
-        int lane = (int)(t & 31); t >>= 5;
-        int s = (int)(t % d.GP); t /= d.GP;
-        int prt = (int)(t % d.PRT); t /= d.PRT;   // t = Q*Nk + k
-        int row = lane >> 2, kk = lane & 3;
-        int pr = 8 * prt + row;
-        int j = 4 * s + kk, gam = j >> 1, c = j & 1;
-        double v = 0.0;
-        if (pr < d.m * d.m && gam < d.nchol) {
-            double2 z = L[((size_t)t * d.nchol + gam) * d.m * d.m + pr];
-            v = c ? z.y : z.x;
-        }
-        Lv[idx] = v;
-    }
-}
-
 __global__ void half_rot_h_kernel(Dims d, const double2* __restrict__ h1, const double2* __restrict__ psi_t,
                                   double2* __restrict__ ht) {
     // ht[k][a][q] = sum_p conj(A_k[p][a]) h_k[p][q]     (first line of Eq. 49)
@@ -152,7 +135,7 @@ static int dev_alloc(T** p, size_t count) {
 
 AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     if (!c) return;
-    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lx, c->Lx3, c->Lf, c->Lv,
+    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lx, c->Lx3, c->Lf, c->Lv3, c->vunits,
                     c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T, c->ws_Tx,
                     c->ws_expart, c->ws_fbpart, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
                     c->b1, c->ws_b1tmp, c->ws_gram, c->ws_rinv, c->ws_logdet2, c->ws_ldr, c->ws_info2};
@@ -230,7 +213,6 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     auto A = [&](int r) { if (rc == AFQMC_OK) rc = r; };
     const size_t nLx = (size_t)Nk * Nk * d.NAG * d.GQ * d.KS * 64 + AFQMC_LX_PAD;
     const size_t nLf = (size_t)Nk * d.GT2 * Nk * d.n * d.KS * 64;
-    const size_t nLv = (size_t)Nk * Nk * d.PRT * d.GP * 32;
     const int LD = d.N | 1;
     A(dev_alloc(&c->kminus, (size_t)Nk * Nk));
     A(dev_alloc(&c->kplus, (size_t)Nk * Nk));
@@ -241,12 +223,11 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     A(dev_alloc(&c->Lx, nLx));
     if (d.NAG == 1) A(dev_alloc(&c->Lx3, afqmc_i_lx3_doubles(d)));
     A(dev_alloc(&c->Lf, nLf));
-    A(dev_alloc(&c->Lv, nLv));
     A(dev_alloc(&c->ws_O, (size_t)nw * d.N * LD));
     A(dev_alloc(&c->ws_oinvT, (size_t)nw * d.N * d.N));
     A(dev_alloc(&c->ws_theta, (size_t)nw * d.N * d.M));
     A(dev_alloc(&c->ws_vbias, (size_t)nw * Nk * d.nchol));
-    A(dev_alloc(&c->ws_xi, (size_t)Nk * d.GP * ((nw + 3) / 4) * 16));   // expanded fragments: 32 doubles each
+    A(dev_alloc(&c->ws_xi, (afqmc_i_vhs_field_doubles(d, nw) + 1) / 2));   // expanded field fragments (vhs.cu)
     A(dev_alloc(&c->ws_vhs, (size_t)nw * d.M * d.M));
     A(dev_alloc(&c->ws_T, (size_t)2 * nw * d.M * d.N));
     const size_t nTx = (size_t)2 * nw * afqmc_i_taylor_ws_doubles(d);
@@ -286,10 +267,10 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
         half_rot_h_kernel<<<grid((size_t)Nk * d.n * d.m), T, 0, st>>>(d, (const double2*)h1, c->psi_t, c->ht);
         pack_Lx_kernel<<<grid(nLx), T, 0, st>>>(d, (const double2*)L, c->psi_t, c->Lx, nLx);
         pack_Lf_kernel<<<grid(nLf), T, 0, st>>>(d, (const double2*)L, c->psi_t, c->Lf, nLf);
-        pack_Lv_kernel<<<grid(nLv), T, 0, st>>>(d, (const double2*)L, c->Lv, nLv);
-        c->launches += 4;
+        c->launches += 3;
         if (cudaGetLastError() != cudaSuccess) rc = AFQMC_CUDA_ERROR;
         if (rc == AFQMC_OK && c->Lx3) rc = afqmc_i_pack_lx3(c, (const double2*)L, st);
+        if (rc == AFQMC_OK) rc = afqmc_i_vhs_setup(c, (const double2*)L, kminus, kneg, st);
     }
     // host vectors must outlive the async copies; the caller may free its arrays after return
     if (cudaStreamSynchronize(st) != cudaSuccess && rc == AFQMC_OK) rc = AFQMC_CUDA_ERROR;

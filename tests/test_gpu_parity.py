@@ -308,6 +308,28 @@ def test_green_register_kernel_equals_legacy_kernel(small_case):
     assert np.max(phase_diff(ld_new.cpu().numpy().imag, ld_old.cpu().numpy().imag)) < 1e-12
 
 
+@pytest.mark.parametrize("nw", [3, 11, 37])
+def test_vhs_without_the_pair_identity_falls_back_to_all_blocks(nw):
+    """vhs.cu stores one L block per (Q,-Q) pair only if afqmc_create finds the identity of PAPER.md:216 in the caller's
+    L; an L that violates it must still give the exact contraction of Eq. 48 (all blocks stored, no pairing).  Several
+    batch sizes exercise the 1-, 2- and 4-tile kernels and more than one walker group."""
+    from paper_2003_09468_b200 import binding
+    cfg = synth.tiny_config(mesh=(2, 3, 1), m=5, n=3, nchol=7, nw=nw, seed=17)
+    pb = synth.make_problem(cfg)
+    rng = np.random.default_rng(99)
+    for Lcase, paired in ((pb.L, True), (pb.L + 0.3 * (rng.standard_normal(pb.L.shape) + 1j * rng.standard_normal(pb.L.shape)), False)):
+        pb2 = synth.Problem(cfg, pb.h1, pb.psi_t, np.ascontiguousarray(Lcase), pb.phi, pb.x)
+        ctx = binding.from_problem(pb2)
+        try:
+            vb = rng.standard_normal((nw, cfg.nk, cfg.nchol)) + 1j * rng.standard_normal((nw, cfg.nk, cfg.nchol))
+            V = ctx.vhs(_to_dev(pb.x), _to_dev(vb), cfg.dtau).cpu().numpy()
+            for w in range(nw):
+                V_o = orc.vhs(cfg.mesh, pb2.L, orc.assemble_fields(cfg.mesh, pb.x[w], vb[w], cfg.dtau))
+                assert relerr(V[w], V_o) < RTOL, (paired, w, relerr(V[w], V_o))
+        finally:
+            ctx.close()
+
+
 @pytest.mark.parametrize("kw", [dict(mesh=(2, 2, 1), m=6, n=4, nchol=10, nw=4), dict(mesh=(2, 3, 1), m=5, n=3, nchol=7, nw=5),
                                 dict(mesh=(1, 2, 2), m=9, n=1, nchol=5, nw=2), dict(mesh=(3, 1, 1), m=26, n=4, nchol=18, nw=7)],
                          ids=["n4", "n3_odd", "n1_two_walkers", "m26_seven_walkers"])
