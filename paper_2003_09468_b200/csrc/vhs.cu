@@ -32,7 +32,6 @@ namespace {
 constexpr int V3_KC = 2;        // k-steps per shared-memory stage
 constexpr int V3_STAGES = 3;
 constexpr int V3_WARPS = 4;
-constexpr int V3_D = 3;         // k-steps of register prefetch of the A stream
 
 // max |L[-Q][k-Q][g][r][p] - conj(L[Q][k][g][p][r])| and max |L| (both as ordered-int atomics on the bit patterns of
 // non-negative doubles, which is exact and order independent)
@@ -198,7 +197,11 @@ __device__ __forceinline__ void v3_bulk_g2s(void* dst, const void* src, uint32_t
 }
 
 // ---- the contraction kernel: see the header comment ----
-template <int NT>
+// NT = n-tiles (8 walkers each) of one column set.  MERGED (small batches, NT <= 2): one warp computes BOTH column
+// sets of its row slice (2 NT n-tiles), so the A stream is read once without relying on L1 and every fragment feeds
+// twice as many DMMAs; otherwise warps 0-1 take the block and warps 2-3 its partner.  D = k-steps of A register prefetch
+// (deeper for small batches, where the kernel is bound by the HBM stream of L and needs more bytes in flight).
+template <int NT, bool MERGED, int D>
 __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
     Dims d, int KS4, int KS4p, int nw, int nwg, int nsg, const int* __restrict__ vunits, const int* __restrict__ kminus,
     const double2* __restrict__ Lv3, const double* __restrict__ Bx3, double2* __restrict__ vhs) {
@@ -212,13 +215,14 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
     const int Q = vunits[4 * u], k = vunits[4 * u + 1], kind = vunits[4 * u + 2];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nslices = (d.PRT + 1) / 2;
-    const int spc = kind ? V3_WARPS / 2 : V3_WARPS;           // row slices per CTA
+    constexpr int NTT = MERGED ? 2 * NT : NT;                 // n-tiles of one warp
+    const int spc = (kind && !MERGED) ? V3_WARPS / 2 : V3_WARPS;   // row slices per CTA
     const int slice0 = sg * spc;
     if (slice0 >= nslices) return;                            // (single-block units need fewer CTAs than paired ones)
-    const int set = kind ? warp / spc : 0;
-    const int slice = slice0 + (kind ? warp % spc : warp);
+    const int set = (kind && !MERGED) ? warp / spc : 0;       // column set of this warp (MERGED: both)
+    const int slice = slice0 + warp % spc;
     int nactive = 0;
-    for (int wv = 0; wv < V3_WARPS; ++wv) nactive += (slice0 + (kind ? wv % spc : wv)) < nslices ? 1 : 0;
+    for (int wv = 0; wv < V3_WARPS; ++wv) nactive += (slice0 + wv % spc) < nslices ? 1 : 0;
     if (tid == 0) {
         for (int s = 0; s < V3_STAGES; ++s) { v3_mbar_init(&full[s], 1); v3_mbar_init(&empty[s], nactive); }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
@@ -245,20 +249,21 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
     const int prt0 = 2 * slice, prt1 = min(prt0 + 1, d.PRT - 1);
     const double2* pa0 = Lv3 + (((size_t)u * d.PRT + prt0) * KS4) * 32 + lane;
     const double2* pa1 = Lv3 + (((size_t)u * d.PRT + prt1) * KS4) * 32 + lane;
-    double2 fa0[V3_D], fa1[V3_D];
+    static_assert(D == 3 || D == 6, "the ring switch below enumerates 3 or 6 entries");
+    double2 fa0[D], fa1[D];
 #pragma unroll
-    for (int q = 0; q < V3_D; ++q) {
+    for (int q = 0; q < D; ++q) {
         const int ks = min(q, KS4 - 1);
         fa0[q] = __ldg(pa0 + (size_t)ks * 32);
         fa1[q] = __ldg(pa1 + (size_t)ks * 32);
     }
-    double acc[3][2][NT][2];
+    double acc[3][2][NTT][2];
 #pragma unroll
     for (int p = 0; p < 3; ++p)
 #pragma unroll
         for (int i = 0; i < 2; ++i)
 #pragma unroll
-            for (int j = 0; j < NT; ++j) acc[p][i][j][0] = acc[p][i][j][1] = 0.0;
+            for (int j = 0; j < NTT; ++j) acc[p][i][j][0] = acc[p][i][j][1] = 0.0;
 
     int ksg = 0;        // global k-step
     auto kstep = [&](const double* bs, const int qa) {
@@ -266,21 +271,20 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
         const double a1[3] = {fa1[qa].x + fa1[qa].y, fa1[qa].x, fa1[qa].y};
 #pragma unroll
         for (int p = 0; p < 3; ++p) {
-            double bf[NT];
+            double bf[NTT];
 #pragma unroll
-            for (int j = 0; j < NT; ++j) bf[j] = bs[(p * NT + j) * 32];
+            for (int j = 0; j < NTT; ++j) bf[j] = bs[(j / NT) * SET_DOUBLES + (p * NT + j % NT) * 32];
 #pragma unroll
-            for (int j = 0; j < NT; ++j) {
+            for (int j = 0; j < NTT; ++j) {
                 dmma884(acc[p][0][j][0], acc[p][0][j][1], a0[p], bf[j]);
                 dmma884(acc[p][1][j][0], acc[p][1][j][1], a1[p], bf[j]);
             }
         }
-        const int nk = min(ksg + V3_D, KS4 - 1);          // clamped: the matching B rows are zero
+        const int nk = min(ksg + D, KS4 - 1);          // clamped: the matching B rows are zero
         fa0[qa] = __ldg(pa0 + (size_t)nk * 32);
         fa1[qa] = __ldg(pa1 + (size_t)nk * 32);
         ++ksg;
     };
-    static_assert(V3_D == 3, "the switch below enumerates the three entries of the A register ring");
     int qa = 0;
     for (int ch = 0; ch < nchunks; ++ch) {
         const int s = ch % V3_STAGES;
@@ -288,13 +292,16 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
         const double* bs = v3_smem + (size_t)s * STAGE_DOUBLES + set * SET_DOUBLES + lane;
 #pragma unroll
         for (int q = 0; q < V3_KC; ++q) {
-            // the A register ring has V3_D entries; qa cycles 0..V3_D-1 (a switch keeps the indices static)
+            // the A register ring has D entries; qa cycles 0..D-1 (a switch keeps the register indices static)
             switch (qa) {
                 case 0: kstep(bs + q * 3 * NT * 32, 0); break;
                 case 1: kstep(bs + q * 3 * NT * 32, 1); break;
-                default: kstep(bs + q * 3 * NT * 32, 2); break;
+                case 2: kstep(bs + q * 3 * NT * 32, 2); break;
+                case 3: kstep(bs + q * 3 * NT * 32, D > 3 ? 3 : 0); break;
+                case 4: kstep(bs + q * 3 * NT * 32, D > 3 ? 4 : 0); break;
+                default: kstep(bs + q * 3 * NT * 32, D > 3 ? 5 : 0); break;
             }
-            qa = qa + 1 == V3_D ? 0 : qa + 1;
+            qa = qa + 1 == D ? 0 : qa + 1;
             if (q == 0 && tid == 0) {   // producer duty: refill the stage consumed in the previous iteration
                 const int nxt = ch + V3_STAGES - 1;
                 if (nxt < nchunks) {
@@ -316,31 +323,34 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
         const int pr = 8 * prt + (lane >> 2);
         if (prt >= d.PRT || pr >= mm) continue;
         const int p = pr / d.m, r = pr % d.m;
-        const size_t off = set == 0 ? ((size_t)k * d.m + p) * d.M + (size_t)kq * d.m + r
-                                    : ((size_t)kq * d.m + r) * d.M + (size_t)k * d.m + p;
+        const size_t off_own = ((size_t)k * d.m + p) * d.M + (size_t)kq * d.m + r;
+        const size_t off_par = ((size_t)kq * d.m + r) * d.M + (size_t)k * d.m + p;
 #pragma unroll
-        for (int j = 0; j < NT; ++j)
+        for (int j = 0; j < NTT; ++j) {
+            const int sj = MERGED ? j / NT : set;                 // column set of this n-tile
+            if (sj == 1 && !kind) continue;                       // a self-partner block has no second set
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-                const int w = (wg * NT + j) * 8 + 2 * (lane & 3) + e;
+                const int w = (wg * NT + j % NT) * 8 + 2 * (lane & 3) + e;
                 if (w >= nw) continue;
                 const double re = acc[0][i][j][e] - acc[2][i][j][e];
                 const double im = acc[0][i][j][e] + acc[1][i][j][e];
-                vhs[(size_t)w * d.M * d.M + off] = make_double2(re, set == 0 ? im : -im);
+                vhs[(size_t)w * d.M * d.M + (sj == 0 ? off_own : off_par)] = make_double2(re, sj == 0 ? im : -im);
             }
+        }
     }
 }
 
-template <int NT>
+template <int NT, bool MERGED, int D>
 int launch_vhs3(afqmc_ctx* c, int nw, int KS4, int KS4p, double2* vhs, cudaStream_t st) {
     const Dims& d = c->d;
     const int nwg = (nw + 8 * NT - 1) / (8 * NT);
     const int nslices = (d.PRT + 1) / 2;
-    const int nsg = c->vhs_paired ? (nslices + V3_WARPS / 2 - 1) / (V3_WARPS / 2) : (nslices + V3_WARPS - 1) / V3_WARPS;
+    const int nsg = (c->vhs_paired && !MERGED) ? (nslices + V3_WARPS / 2 - 1) / (V3_WARPS / 2) : (nslices + V3_WARPS - 1) / V3_WARPS;
     const size_t smem = (size_t)V3_STAGES * 2 * V3_KC * 3 * NT * 32 * sizeof(double) + 2 * V3_STAGES * sizeof(uint64_t);
     const long long gx = (long long)c->nvunits * nsg;
     if (gx > 0x7fffffffLL || nwg > 65535) return AFQMC_UNSUPPORTED;
-    vhs3_kernel<NT><<<dim3((unsigned)gx, nwg), 32 * V3_WARPS, smem, st>>>(d, KS4, KS4p, nw, nwg, nsg, c->vunits, c->kminus, c->Lv3,
+    vhs3_kernel<NT, MERGED, D><<<dim3((unsigned)gx, nwg), 32 * V3_WARPS, smem, st>>>(d, KS4, KS4p, nw, nwg, nsg, c->vunits, c->kminus, c->Lv3,
                                                                         reinterpret_cast<const double*>(c->ws_xi), vhs);
     AFQMC_LAUNCH_CHECK(c);
     return AFQMC_OK;
@@ -368,9 +378,9 @@ int afqmc_i_vhs(afqmc_ctx* c, const double* x, const double2* vbias, double dtau
         fields3_kernel<<<G, T, 0, st>>>(d, nw, NT, nwg, KS4p, c->kneg, x, vbias, sqrt(dtau), reinterpret_cast<double*>(c->ws_xi));
         AFQMC_LAUNCH_CHECK(c);
     }
-    if (NT == 4) return launch_vhs3<4>(c, nw, KS4, KS4p, vhs, st);
-    if (NT == 2) return launch_vhs3<2>(c, nw, KS4, KS4p, vhs, st);
-    return launch_vhs3<1>(c, nw, KS4, KS4p, vhs, st);
+    if (NT == 4) return launch_vhs3<4, false, 3>(c, nw, KS4, KS4p, vhs, st);
+    if (NT == 2) return c->vhs_paired ? launch_vhs3<2, true, 6>(c, nw, KS4, KS4p, vhs, st) : launch_vhs3<2, false, 6>(c, nw, KS4, KS4p, vhs, st);
+    return c->vhs_paired ? launch_vhs3<1, true, 6>(c, nw, KS4, KS4p, vhs, st) : launch_vhs3<1, false, 6>(c, nw, KS4, KS4p, vhs, st);
 }
 
 AFQMC_API int afqmc_vhs(afqmc_ctx* c, const double* x, const void* vbias, double dtau, int nw, void* vhs,
