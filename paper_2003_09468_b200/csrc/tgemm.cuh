@@ -1,35 +1,37 @@
-// Batched complex128 GEMM for tall-skinny right-hand sides on the FP64 tensor pipe (DMMA m8n8k4),
-// used by a6 (Taylor propagation) and a3 (Green's function, Eq. 30):
+// Batched complex128 GEMM for tall-skinny right-hand sides on the FP64 tensor pipe (DMMA m8n8k4), used by a6
+// (Taylor propagation):
 //
 //   C_b[i][j] = alpha * sum_k A_b[i][k] * B_b[k][j],     A: M x K (big, streamed once),  B: K x N (small)
 //
-// Design (B200): the big operand A is read straight from its natural row-major layout into DMMA
-// A-fragments, the small operand B lives in an EXPANDED fragment-major layout that is staged into shared
-// memory by bulk asynchronous copies (cp.async.bulk + mbarrier pipeline, SASS UBLKCP), so the inner loop is
-// LDG.128 (A, prefetched in registers) + LDS.64 (B, conflict-free) + DMMA only.
+// Design (B200): the big operand A is read straight from its natural row-major layout into DMMA A-fragments, the
+// small operand B lives in an EXPANDED fragment-major layout that is staged into shared memory by bulk asynchronous
+// copies (cp.async.bulk + mbarrier pipeline, SASS UBLKCP), so the inner loop is LDG.128 (A, prefetched in
+// registers) + LDS.64 (B, conflict-free) + DMMA only.
 //
-//  * K pairing.  The real embedding of a complex GEMM (common.cuh) needs K index (k, part).  The K order is
-//    free as long as A and B agree, so a PAIR of DMMA k-steps covers four complex k = 4t..4t+3:
-//        even step 2t  : A-fragment = Re A[i][4t+c],  B rows (T_re | T_im)
-//        odd  step 2t+1: A-fragment = Im A[i][4t+c],  B rows (-T_im | T_re)
-//    so lane (row r, c) gets both of its A values with ONE 16-byte load of the complex element A[i][4t+c].
-//  * Expanded B ("Bx"): [batch][g][s = 2t+parity][nt < NTA][32 doubles], g = column group (<= NTA n-tiles of 4
-//    complex columns), innermost 32 doubles = one DMMA B-fragment in lane order (lane = (2*jj+d)*4 + c: column jj
-//    of the tile, d = re/im output part, c = k inside the pair).  K is padded to a multiple of 4*KC and unused
-//    tiles/columns/rows are ZERO, so the kernel has no tails: A loads are clamped (finite * 0).
+//  * 3M complex product (Gauss's form, as in exchange3m.cu and vhs.cu):
+//        P0 = (Ar+Ai) Br,  P1 = Ar (Bi-Br),  P2 = Ai (Br+Bi);      Re C = P0 - P2,   Im C = P0 + P1
+//    three real GEMMs with K = k and ONE real column per complex column of B: 6 real flops per complex multiply-add
+//    instead of the 8 of the real embedding, 22 % fewer DMMAs at N = 108 (14 n-tiles of 8 columns x 3 products
+//    against 27 n-tiles of 4 complex columns x 2 k-parities).  Lane (row r, c) gets Re and Im of A[i][4t+c] with ONE
+//    16-byte load; Ar+Ai is one DADD per fragment.
+//  * Expanded B ("Bx"): [batch][g][t][prod][nt < NTA][32 doubles], g = column group (<= NTA n-tiles of 8 columns),
+//    t = group of 4 consecutive k, prod = 0: Br, 1: Bi-Br, 2: Br+Bi; innermost 32 doubles = one DMMA B-fragment in lane
+//    order (lane = col*4 + c: column col of the tile, c = k inside the group).  K is padded to a multiple of 4*KC and
+//    unused tiles/columns/rows are ZERO, so the kernel has no tails: A loads are clamped (finite * 0).
 //  * The epilogue can (a) accumulate alpha*C into a natural-layout D (D += alpha*C), (b) write alpha*C in the
 //    expanded layout of the NEXT product's B operand (rows of C become its K index), (c) store alpha*C
 //    transposed in natural layout.  With (b) the Taylor chain T_j = (s/j) V T_{j-1} never converts layouts.
-//  * CTA = WPC warps x (16 rows x one column group); the warps share the staged B chunks.  Grid = (groups, row
+//  * CTA = 4 warps x (16 rows x one column group); the warps share the staged B chunks.  Grid = (groups, row
 //    blocks, batch): CTAs of the same rows and walker are adjacent, so A is fetched from HBM once and shared
-//    through L2 by the column groups.  WPC = 4 (see launch_cfg).
+//    through L2 by the column groups.
 #pragma once
 #include "common.cuh"
 
 namespace tg {
 
-constexpr int KC = 4;        // k-step PAIRS per shared-memory stage
+constexpr int KC = 4;        // k-groups (of 4 complex k) per shared-memory stage
 constexpr int STAGES = 3;
+constexpr int NTMAX = 4;     // n-tiles (8 columns) per column group: 3 products x 2 m-tiles x 4 tiles x 2 = 48 accumulators
 // warps per CTA (WPC, 16 rows each) is a template parameter chosen per launch: see launch_cfg()
 
 struct Args {
@@ -40,8 +42,8 @@ struct Args {
     double2* Ct; long long strideCt; int ldct;         // nullable: Ct[j][i]  = alpha*C[i][j]
     int M, N, K;
     int G, nt_base, nt_rem;                            // column groups: group g has nt_base + (g < nt_rem) n-tiles
-    int NPp;                                           // padded k-step pairs of this product: roundup(ceil(K/4), KC)
-    int NPcp;                                          // padded k-step pairs of the Cx layout: roundup(ceil(M/4), KC)
+    int NPp;                                           // padded k-groups of this product: roundup(ceil(K/4), KC)
+    int NPcp;                                          // padded k-groups of the Cx layout: roundup(ceil(M/4), KC)
     double alpha;
     int wpc;                                           // 0 = automatic, else 3/4/5 warps per CTA (tuning aid)
 };
@@ -51,21 +53,15 @@ struct Groups { int G, nt_base, nt_rem, NTA; };
 __host__ __device__ inline int group_tile0(int g, int nt_base, int nt_rem) { return g * nt_base + (g < nt_rem ? g : nt_rem); }
 __host__ __device__ inline int group_tiles(int g, int nt_base, int nt_rem) { return nt_base + (g < nt_rem ? 1 : 0); }
 
-// instantiated tile counts per column group (template NTA); a group with fewer tiles is zero padded
-static inline int round_nta(int nt) {
-    const int avail[] = {2, 4, 6, 8, 10, 12, 13, 14};
-    for (int a : avail) if (nt <= a) return a;
-    return 14;
-}
-// G = 0: the fewest groups (<= 14 tiles each); G > 0: that many groups (clamped to what the tile count allows)
+// G = 0: the fewest groups (<= NTMAX tiles each); G > 0: that many groups (clamped to what the tile count allows)
 static inline Groups make_groups(int N, int G = 0) {
     Groups gr;
-    const int nt = (N + 3) / 4;
-    const int gmin = (nt + 13) / 14;
+    const int nt = (N + 7) / 8;
+    const int gmin = (nt + NTMAX - 1) / NTMAX;
     gr.G = G < gmin ? gmin : (G > nt ? nt : G);
     gr.nt_base = nt / gr.G;
     gr.nt_rem = nt % gr.G;
-    gr.NTA = round_nta(gr.nt_base + (gr.nt_rem ? 1 : 0));
+    gr.NTA = gr.nt_base + (gr.nt_rem ? 1 : 0);         // 1..NTMAX; a group with one tile fewer is zero padded
     return gr;
 }
 constexpr int GROUP_CHOICES = 3;   // pick_groups() considers gmin .. gmin + GROUP_CHOICES - 1 groups
@@ -73,7 +69,7 @@ static inline int padded_pairs(int K) { return (((K + 3) / 4 + KC - 1) / KC) * K
 // doubles of one batch entry of an expanded operand with K rows and N columns
 static inline size_t expanded_doubles(int K, int N, int G = 0) {
     const Groups gr = make_groups(N, G);
-    return (size_t)gr.G * 2 * padded_pairs(K) * gr.NTA * 32;
+    return (size_t)gr.G * padded_pairs(K) * 3 * gr.NTA * 32;
 }
 // the largest expanded operand over the group counts pick_groups() may choose (workspace sizing)
 static inline size_t expanded_doubles_max(int K, int N) {
@@ -87,29 +83,29 @@ static inline size_t expanded_doubles_max(int K, int N) {
 }
 
 // ---- natural [K][N] (ldb) -> expanded; also the zero fill of all padding ----
-// CONJ_T: the source is read as B[k][j] = src[j][k] (transposed, K contiguous), as a3 needs for Phi^T.
+// TRANS: the source is read as B[k][j] = src[j][k] (transposed, K contiguous).
 template <bool TRANS>
 __global__ void expand_kernel(const double2* __restrict__ src, long long strideS, int lds, double* __restrict__ Bx,
                               long long strideBx, int K, int N, int G, int nt_base, int nt_rem, int NTA, int NPp) {
-    const size_t per = (size_t)G * 2 * NPp * NTA * 32;
+    const size_t per_in = (size_t)G * NPp * NTA * 32;          // without the product index
     const int b = blockIdx.y;
     const double2* S = src + (size_t)b * strideS;
     double* out = Bx + (size_t)b * strideBx;
-    for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < per; idx += (size_t)gridDim.x * blockDim.x) {
+    for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < per_in; idx += (size_t)gridDim.x * blockDim.x) {
         size_t t = idx;
         const int l = (int)(t & 31); t >>= 5;
         const int nt = (int)(t % NTA); t /= NTA;
-        const int s = (int)(t % (2 * NPp));
-        const int g = (int)(t / (2 * NPp));
-        const int par = s & 1, col = l >> 2, jj = col >> 1, dd = col & 1;
-        const int k = 4 * (s >> 1) + (l & 3);
-        const int j = (group_tile0(g, nt_base, nt_rem) + nt) * 4 + jj;
-        double v = 0.0;
-        if (k < K && j < N && nt < group_tiles(g, nt_base, nt_rem)) {
-            const double2 z = TRANS ? S[(size_t)j * lds + k] : S[(size_t)k * lds + j];
-            v = par == 0 ? (dd ? z.y : z.x) : (dd ? z.x : -z.y);
-        }
-        out[idx] = v;
+        const int tt = (int)(t % NPp);
+        const int g = (int)(t / NPp);
+        const int col = l >> 2;
+        const int k = 4 * tt + (l & 3);
+        const int j = (group_tile0(g, nt_base, nt_rem) + nt) * 8 + col;
+        double2 z = make_double2(0.0, 0.0);
+        if (k < K && j < N && nt < group_tiles(g, nt_base, nt_rem)) z = TRANS ? S[(size_t)j * lds + k] : S[(size_t)k * lds + j];
+        double* f = out + ((((size_t)g * NPp + tt) * 3) * NTA + nt) * 32 + l;
+        f[0] = z.x;
+        f[(size_t)NTA * 32] = z.y - z.x;
+        f[(size_t)2 * NTA * 32] = z.x + z.y;
     }
 }
 
@@ -141,7 +137,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 template <int NT, int NTA, int D, int WPC>
 __device__ __forceinline__ void body(const Args& p, const double* stage0, uint64_t* full, uint64_t* empty, int g, int b) {
     static_assert(KC % D == 0, "A prefetch depth must divide the chunk");
-    constexpr uint32_t STAGE_DOUBLES = KC * 2 * NTA * 32, STAGE_BYTES = STAGE_DOUBLES * 8;
+    constexpr uint32_t STAGE_DOUBLES = KC * 3 * NTA * 32, STAGE_BYTES = STAGE_DOUBLES * 8;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int row0 = blockIdx.y * (16 * WPC) + warp * 16;
     const int r = lane >> 2, c = lane & 3;
@@ -157,14 +153,16 @@ __device__ __forceinline__ void body(const Args& p, const double* stage0, uint64
         fa0[q] = __ldg(pa0 + k);
         fa1[q] = __ldg(pa1 + k);
     }
-    double acc[2][NT][2];
+    double acc[3][2][NT][2];
 #pragma unroll
-    for (int mt = 0; mt < 2; ++mt)
+    for (int pr = 0; pr < 3; ++pr)
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
+        for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) acc[pr][mt][nt][0] = acc[pr][mt][nt][1] = 0.0;
 
     const int nchunks = p.NPp / KC;
-    const double* Bsrc = p.Bx + (size_t)b * p.strideBx + (size_t)g * 2 * p.NPp * NTA * 32;
+    const double* Bsrc = p.Bx + (size_t)b * p.strideBx + (size_t)g * p.NPp * 3 * NTA * 32;
     if (tid == 0) {
         for (int c0 = 0; c0 < STAGES - 1 && c0 < nchunks; ++c0) {
             mbar_expect_tx(&full[c0], STAGE_BYTES);
@@ -177,24 +175,21 @@ __device__ __forceinline__ void body(const Args& p, const double* stage0, uint64
         const double* bs = stage0 + (size_t)st * STAGE_DOUBLES + lane;
 #pragma unroll
         for (int q = 0; q < KC; ++q) {
-            constexpr int dummy = 0; (void)dummy;
             const int buf = q % D;
-            double bf[NT];
+            const double a0[3] = {fa0[buf].x + fa0[buf].y, fa0[buf].x, fa0[buf].y};     // Ar+Ai, Ar, Ai
+            const double a1[3] = {fa1[buf].x + fa1[buf].y, fa1[buf].x, fa1[buf].y};
 #pragma unroll
-            for (int nt = 0; nt < NT; ++nt) bf[nt] = bs[((2 * q) * NTA + nt) * 32];
+            for (int pr = 0; pr < 3; ++pr) {
+                double bf[NT];
 #pragma unroll
-            for (int nt = 0; nt < NT; ++nt) {
-                dmma884(acc[0][nt][0], acc[0][nt][1], fa0[buf].x, bf[nt]);
-                dmma884(acc[1][nt][0], acc[1][nt][1], fa1[buf].x, bf[nt]);
+                for (int nt = 0; nt < NT; ++nt) bf[nt] = bs[((q * 3 + pr) * NTA + nt) * 32];
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) {
+                    dmma884(acc[pr][0][nt][0], acc[pr][0][nt][1], a0[pr], bf[nt]);
+                    dmma884(acc[pr][1][nt][0], acc[pr][1][nt][1], a1[pr], bf[nt]);
+                }
             }
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt) bf[nt] = bs[((2 * q + 1) * NTA + nt) * 32];
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt) {
-                dmma884(acc[0][nt][0], acc[0][nt][1], fa0[buf].y, bf[nt]);
-                dmma884(acc[1][nt][0], acc[1][nt][1], fa1[buf].y, bf[nt]);
-            }
-            {   // refill this register buffer with the pair D ahead
+            {   // refill this register buffer with the k-group D ahead
                 const int k = min(4 * (ch * KC + q + D) + c, Km1);
                 fa0[buf] = __ldg(pa0 + k);
                 fa1[buf] = __ldg(pa1 + k);
@@ -213,34 +208,38 @@ __device__ __forceinline__ void body(const Args& p, const double* stage0, uint64
         if (lane == 0) mbar_arrive(&empty[st]);
     }
 
-    // ---- epilogue: lane holds complex (row = r, column = 4*tile + c) of each 8x4 tile ----
+    // ---- epilogue: lane holds rows r, r+8 and columns 8*tile + 2c + e of each 8x8 tile; Re = P0 - P2, Im = P0 + P1 ----
     const int tile0 = group_tile0(g, p.nt_base, p.nt_rem);
     const int ntg = group_tiles(g, p.nt_base, p.nt_rem);
     double2* Dm = p.D ? p.D + (size_t)b * p.strideD : nullptr;
     double2* Ct = p.Ct ? p.Ct + (size_t)b * p.strideCt : nullptr;
-    double* Cx = p.Cx ? p.Cx + (size_t)b * p.strideCx + (size_t)g * 2 * p.NPcp * NTA * 32 : nullptr;
+    double* Cx = p.Cx ? p.Cx + (size_t)b * p.strideCx + (size_t)g * p.NPcp * 3 * NTA * 32 : nullptr;
 #pragma unroll
     for (int mt = 0; mt < 2; ++mt) {
         const int i = row0 + mt * 8 + r;
         const bool iok = i < p.M;
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt) {
-            const int j = (tile0 + nt) * 4 + c;
-            double2 v = make_double2(p.alpha * acc[mt][nt][0], p.alpha * acc[mt][nt][1]);
-            if (iok && j < p.N && nt < ntg) {
-                if (Dm) {
-                    double2 o = Dm[(size_t)i * p.ldd + j];
-                    o.x += v.x; o.y += v.y;
-                    Dm[(size_t)i * p.ldd + j] = o;
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int j = (tile0 + nt) * 8 + 2 * c + e;
+                double2 v = make_double2(p.alpha * (acc[0][mt][nt][e] - acc[2][mt][nt][e]),
+                                         p.alpha * (acc[0][mt][nt][e] + acc[1][mt][nt][e]));
+                if (iok && j < p.N && nt < ntg) {
+                    if (Dm) {
+                        double2 o = Dm[(size_t)i * p.ldd + j];
+                        o.x += v.x; o.y += v.y;
+                        Dm[(size_t)i * p.ldd + j] = o;
+                    }
+                    if (Ct) Ct[(size_t)j * p.ldct + i] = v;
                 }
-                if (Ct) Ct[(size_t)j * p.ldct + i] = v;
-            }
-            if (Cx && i < 4 * p.NPcp) {
-                if (!iok) v = make_double2(0.0, 0.0);     // K padding of the next product
-                double* f = Cx + ((size_t)(2 * (i >> 2)) * NTA + nt) * 32 + 8 * c + (i & 3);
-                f[0] = v.x; f[4] = v.y;                   // even step: (re | im)
-                f += NTA * 32;
-                f[0] = -v.y; f[4] = v.x;                  // odd step: (-im | re)
+                if (Cx && i < 4 * p.NPcp) {
+                    if (!iok) v = make_double2(0.0, 0.0);     // K padding of the next product
+                    double* f = Cx + (((size_t)(i >> 2) * 3) * NTA + nt) * 32 + (2 * c + e) * 4 + (i & 3);
+                    f[0] = v.x;                               // Br
+                    f[NTA * 32] = v.y - v.x;                  // Bi - Br
+                    f[2 * NTA * 32] = v.x + v.y;              // Br + Bi
+                }
             }
         }
     }
@@ -249,7 +248,7 @@ __device__ __forceinline__ void body(const Args& p, const double* stage0, uint64
 template <int NTA, int D, int WPC>
 __global__ void __launch_bounds__(32 * WPC, 2) tgemm_kernel(Args p) {
     extern __shared__ __align__(128) double tg_smem[];
-    uint64_t* full = reinterpret_cast<uint64_t*>(tg_smem + (size_t)STAGES * KC * 2 * NTA * 32);
+    uint64_t* full = reinterpret_cast<uint64_t*>(tg_smem + (size_t)STAGES * KC * 3 * NTA * 32);
     uint64_t* empty = full + STAGES;
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], WPC); }
@@ -258,14 +257,14 @@ __global__ void __launch_bounds__(32 * WPC, 2) tgemm_kernel(Args p) {
     }
     __syncthreads();
     const int g = blockIdx.x, b = blockIdx.z;
-    if (group_tiles(g, p.nt_base, p.nt_rem) == NTA) body<NTA, NTA, D, WPC>(p, tg_smem, full, empty, g, b);
-    else body<NTA - 1, NTA, D, WPC>(p, tg_smem, full, empty, g, b);
+    if (NTA == 1 || group_tiles(g, p.nt_base, p.nt_rem) == NTA) body<NTA, NTA, D, WPC>(p, tg_smem, full, empty, g, b);
+    else body<(NTA > 1 ? NTA - 1 : 1), NTA, D, WPC>(p, tg_smem, full, empty, g, b);
 }
 
 template <int NTA, int D, int WPC>
 static inline cudaError_t launch_wpc(const Args& a, int batch, cudaStream_t st, int* occ_out) {
     auto kern = tgemm_kernel<NTA, D, WPC>;
-    const int smem = STAGES * KC * 2 * NTA * 32 * 8 + 2 * STAGES * 8;
+    const int smem = STAGES * KC * 3 * NTA * 32 * 8 + 2 * STAGES * 8;
     static int occ = -1;
     if (occ < 0) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -292,9 +291,9 @@ static inline int device_sms() {
 }
 
 // Warps per CTA.  The DMMA pipe is per SM sub-partition, so resident warps must divide evenly over the four
-// sub-partitions: measured at C3 (r01c notes), 2 CTAs x 4 warps run 6 sub-partition rounds in 3.35 ms, while
-// 2 x 5 warps (1.95 waves instead of 2.38, but 3+3+2+2 warps per sub-partition) take 3.90 ms and 3 warps 4.39 ms.
-// 4 is therefore the default; 3 and 5 stay selectable as a tuning aid (option "taylor_warps").
+// sub-partitions: measured at C3 (r01c notes, 4M version of this kernel), 2 CTAs x 4 warps ran 6 sub-partition rounds in
+// 3.35 ms, while 2 x 5 warps (1.95 waves instead of 2.38, but 3+3+2+2 warps per sub-partition) took 3.90 ms and 3
+// warps 4.39 ms.  4 is therefore the default; 3 and 5 stay selectable as a tuning aid (option "taylor_warps").
 template <int NTA, int D>
 static inline cudaError_t launch_cfg(const Args& a, int batch, cudaStream_t st) {
     int best = 4;
@@ -308,14 +307,10 @@ static inline cudaError_t launch_cfg(const Args& a, int batch, cudaStream_t st) 
 
 #define TG_NTA_SWITCH(NTA_VALUE, CALL)                         \
     switch (NTA_VALUE) {                                       \
+        case 1: return CALL(1);                                \
         case 2: return CALL(2);                                \
-        case 4: return CALL(4);                                \
-        case 6: return CALL(6);                                \
-        case 8: return CALL(8);                                \
-        case 10: return CALL(10);                              \
-        case 12: return CALL(12);                              \
-        case 13: return CALL(13);                              \
-        default: return CALL(14);                              \
+        case 3: return CALL(3);                                \
+        default: return CALL(4);                               \
     }
 
 // resident CTAs per SM of the 4-warp kernel instantiated for NTA tiles per group
@@ -329,8 +324,7 @@ static inline cudaError_t query_occupancy(int NTA, int* occ) {
 // Number of column groups for a product with M rows, N columns and `batch` entries.  More groups mean narrower
 // warp tiles (fewer accumulators, A re-read from L2 by more CTAs) but a finer grid: the cost model is
 //   rounds of resident CTAs x resident CTAs per SM x tiles a warp executes per k-step,
-// i.e. the DMMA time of one SM (the kernel is tensor-pipe bound).  At C3 (27 n-tiles, 704 row blocks) two groups
-// of 14/13 tiles run 2.38 -> 3 rounds (cost 84), three groups of 9 run 3.57 -> 4 rounds (cost 72), four of 7 run 4.76 -> 5 rounds (cost 70): measured 3.35, 2.78, 2.71 ms.
+// i.e. the DMMA time of one SM (the kernel is tensor-pipe bound), plus 2 % per extra group for the A re-reads.
 static inline int pick_groups(int M, int N, int batch) {
     const int gmin = make_groups(N).G;
     const int sms = device_sms();
@@ -343,9 +337,7 @@ static inline int pick_groups(int M, int N, int batch) {
         const long long ctas = (long long)gr.G * ((M + 63) / 64) * batch;
         const long long slots = (long long)occ * sms;
         const long long rounds = (ctas + slots - 1) / slots;
-        const int nt_exec = gr.nt_base + (gr.nt_rem ? 1 : 0);
-        // 2 % per extra group for the A re-reads and the shorter DMMA runs between fragment loads
-        const long long cost = rounds * occ * nt_exec * (100 + 2 * (g - gmin));
+        const long long cost = rounds * occ * gr.NTA * (100 + 2 * (g - gmin));
         if (best_cost < 0 || cost < best_cost) { best = g; best_cost = cost; }
     }
     return best;
@@ -368,8 +360,8 @@ static inline cudaError_t launch_expand(const double2* src, long long strideS, i
                                         int batch, cudaStream_t st, int G = 0) {
     const Groups gr = make_groups(N, G);
     const int NPp = padded_pairs(K);
-    const size_t per = (size_t)gr.G * 2 * NPp * gr.NTA * 32;
-    int bx = (int)((per + 255) / 256);
+    const size_t per = (size_t)gr.G * NPp * 3 * gr.NTA * 32;
+    int bx = (int)((per / 3 + 255) / 256);
     if (bx > 148 * 8) bx = 148 * 8;
     expand_kernel<TRANS><<<dim3(bx, batch), 256, 0, st>>>(src, strideS, lds, Bx, (long long)per, K, N, gr.G, gr.nt_base,
                                                            gr.nt_rem, gr.NTA, NPp);

@@ -29,8 +29,17 @@
 
 namespace {
 
-constexpr int V3_KC = 2;        // k-steps per shared-memory stage
-constexpr int V3_STAGES = 3;
+#ifndef AFQMC_V3_KC
+#define AFQMC_V3_KC 2
+#endif
+#ifndef AFQMC_V3_STAGES
+#define AFQMC_V3_STAGES 3
+#endif
+#ifndef AFQMC_V3_D4
+#define AFQMC_V3_D4 3
+#endif
+constexpr int V3_KC = AFQMC_V3_KC;        // k-steps per shared-memory stage
+constexpr int V3_STAGES = AFQMC_V3_STAGES;
 constexpr int V3_WARPS = 4;
 
 // max |L[-Q][k-Q][g][r][p] - conj(L[Q][k][g][p][r])| and max |L| (both as ordered-int atomics on the bit patterns of
@@ -350,6 +359,12 @@ int launch_vhs3(afqmc_ctx* c, int nw, int KS4, int KS4p, double2* vhs, cudaStrea
     const size_t smem = (size_t)V3_STAGES * 2 * V3_KC * 3 * NT * 32 * sizeof(double) + 2 * V3_STAGES * sizeof(uint64_t);
     const long long gx = (long long)c->nvunits * nsg;
     if (gx > 0x7fffffffLL || nwg > 65535) return AFQMC_UNSUPPORTED;
+    static bool attr_done = false;
+    if (!attr_done && smem > 48 * 1024) {
+        if (cudaFuncSetAttribute(vhs3_kernel<NT, MERGED, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+            return AFQMC_CUDA_ERROR;
+        attr_done = true;
+    }
     vhs3_kernel<NT, MERGED, D><<<dim3((unsigned)gx, nwg), 32 * V3_WARPS, smem, st>>>(d, KS4, KS4p, nw, nwg, nsg, c->vunits, c->kminus, c->Lv3,
                                                                         reinterpret_cast<const double*>(c->ws_xi), vhs);
     AFQMC_LAUNCH_CHECK(c);
@@ -378,7 +393,7 @@ int afqmc_i_vhs(afqmc_ctx* c, const double* x, const double2* vbias, double dtau
         fields3_kernel<<<G, T, 0, st>>>(d, nw, NT, nwg, KS4p, c->kneg, x, vbias, sqrt(dtau), reinterpret_cast<double*>(c->ws_xi));
         AFQMC_LAUNCH_CHECK(c);
     }
-    if (NT == 4) return launch_vhs3<4, false, 3>(c, nw, KS4, KS4p, vhs, st);
+    if (NT == 4) return launch_vhs3<4, false, AFQMC_V3_D4>(c, nw, KS4, KS4p, vhs, st);
     if (NT == 2) return c->vhs_paired ? launch_vhs3<2, true, 6>(c, nw, KS4, KS4p, vhs, st) : launch_vhs3<2, false, 6>(c, nw, KS4, KS4p, vhs, st);
     return c->vhs_paired ? launch_vhs3<1, true, 6>(c, nw, KS4, KS4p, vhs, st) : launch_vhs3<1, false, 6>(c, nw, KS4, KS4p, vhs, st);
 }
