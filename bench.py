@@ -266,6 +266,13 @@ def run_ours(args):
         if peaks and "bf16_tflops" in peaks:
             roofline["peak_alt_bf16_ratio"] = peaks["bf16_tflops"] * 45.0 / 2250.0
         stages = {k: v / args.steps for k, v in stage_acc.items()}
+        # the other kernel the north_star names: force bias (a4), 8 Nk^2 n m nchol real flops per walker (4M real embedding);
+        # the stage time includes its small chunk-reduction kernel
+        fb_flops = 8.0 * nw * cfg.nk ** 2 * cfg.n * cfg.m * cfg.nchol
+        fb_ms = stages["force_bias"]
+        force_bias_roofline = {"kernel": "force bias (a4), afqmc_force_bias", "bound": "tensor", "flops_per_launch": fb_flops,
+                               "ms_per_launch": fb_ms, "achieved": fb_flops / (fb_ms * 1e-3) / 1e12, "peak": peak_probe,
+                               "unit": "TFLOP/s", "frac": fb_flops / (fb_ms * 1e-3) / 1e12 / peak_probe}
         # ---- CPU baseline: the oracle on a bounded sample (rank 0, N=1 only) ----
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
@@ -295,6 +302,7 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "clocks": sampler.summary(),
             "roofline": roofline,
+            "force_bias_roofline": force_bias_roofline,
             "stage_ms": stages,
             "exchange_tflops": achieved,
             "wall_s_timed_region": t_wall,

@@ -74,7 +74,7 @@ struct afqmc_ctx {
     int b1_set;
     long long launches;
     int opt_exchange_depth; // 0/3 = three k-steps of fragment prefetch, 2 = two
-    int opt_fb_tile;        // tuning aid: warp tile of the force-bias kernel for > 16 walkers (0: 2x8, 1: 4x8, 2: 4x4 m x n tiles)
+    int opt_fb_tile;        // tuning aid: warp tile of the force-bias kernel for > 16 walkers (0: 4x4, 1: 4x8, 2: 2x8 m x n tiles)
     int opt_fb_pf;          // L2 prefetch distance (k-steps) of the Lf stream in the force-bias kernel
     int opt_exchange_minb;  // tuning aid: 1 = ask for more resident CTAs per SM
     int opt_exchange_3m;    // 1 (default) = 3M exchange kernel when n <= 4, 0 = the 4M kernel of energy.cu

@@ -225,9 +225,11 @@ int launch_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias
 int afqmc_i_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias, cudaStream_t st) {
     const int ntq = (nw + 3) / 4;   // walker quads
     // 16 DMMAs per k-step and warp in every shape; all walkers in one group up to 32 walkers
+    // > 16 walkers: 2 m-tile pairs x 4 n-tiles per warp (16 walkers per CTA, 2 A loads + 4 B loads per 16 DMMAs) measured
+    // fastest with the 3-deep prefetch (C3: 0.1725 ms against 0.1800 ms for 1 x 8 and 0.1964 ms for 2 x 8)
     if (ntq >= 5) return c->opt_fb_tile == 1 ? launch_force_bias<2, 8>(c, theta, nw, vbias, st)
-                     : c->opt_fb_tile == 2 ? launch_force_bias<2, 4>(c, theta, nw, vbias, st)
-                                           : launch_force_bias<1, 8>(c, theta, nw, vbias, st);
+                     : c->opt_fb_tile == 2 ? launch_force_bias<1, 8>(c, theta, nw, vbias, st)
+                                           : launch_force_bias<2, 4>(c, theta, nw, vbias, st);
     if (ntq >= 3) return launch_force_bias<2, 4>(c, theta, nw, vbias, st);
     if (ntq == 2) return launch_force_bias<4, 2>(c, theta, nw, vbias, st);
     return launch_force_bias<4, 1>(c, theta, nw, vbias, st);
