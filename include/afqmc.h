@@ -71,7 +71,10 @@ const char* afqmc_strerror(int code);
  *   h1    [Nk][m][m]            device, complex128, Hermitian blocks (Eq. 45)
  *   L     [Nk][Nk][nchol][m][m] device, complex128: L[Q][k][g][p][r], p at k, r at k-Q.
  *         The (Q,-Q) identity L[-Q][k-Q][g][r][p] = conj(L[Q][k][g][p][r]) is ASSUMED
- *         by afqmc_local_energy (it is what lets Lbar of Eq. 40 be read from Lh); it is not checked.
+ *         by afqmc_local_energy (it is what lets Lbar of Eq. 40 be read from Lh).  afqmc_create measures
+ *         the deviation from it: if it is below 1e-13 max|L| the library keeps ONE block of every pair for
+ *         afqmc_vhs ("only one of the pair needs to be stored": half the bytes of L);
+ *         otherwise afqmc_vhs keeps all blocks and stays exact for such an L.
  *   psi_t [Nk][m][n]            device, complex128 (trial block-diagonal in k)
  */
 int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* h1, const void* L,
@@ -222,6 +225,7 @@ double afqmc_exchange_flops(const afqmc_ctx* ctx, int nw);
 
 /* Options: "exchange_warps" (0 = automatic, or 4/5/6/8 warps per CTA of the exchange kernel; tuning aid);
  * "exchange_depth" (0/3 or 2: k-steps of register prefetch in the exchange kernel; tuning aid);
+ * "exchange_3m" (1 = default: three real products per complex product when n <= 4, 0 = the 4M kernel);
  * "timers" (1 = afqmc_step records a CUDA event after each stage, see afqmc_stage_times). */
 int afqmc_set_option(afqmc_ctx* ctx, const char* name, int value);
 
