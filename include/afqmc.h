@@ -147,7 +147,8 @@ int afqmc_step(afqmc_ctx* ctx, void* phi, const double* x, double dtau, int orde
 
 /*
  * The same step on HOST buffers: copies phi and x to the device, runs afqmc_step, copies phi',
- * energy (and logdet, info if not NULL) back and synchronises `stream` before returning.
+ * energy (and logdet, info if not NULL) back and synchronises `stream` before returning.  The download of phi'
+ * runs on a stream of the context, concurrently with the energy evaluation of phi'.
  * Host buffers should be pinned for full copy bandwidth; pageable memory also works.
  */
 int afqmc_step_host(afqmc_ctx* ctx, void* phi_host, const double* x_host, double dtau, int order,

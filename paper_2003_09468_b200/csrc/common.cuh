@@ -84,6 +84,8 @@ struct afqmc_ctx {
     int opt_taylor_wpc;     // tuning aid: 0 = automatic, else 3/4/5 warps per CTA of the Taylor GEMM
     int opt_taylor_groups;  // tuning aid: 0 = automatic, else the number of column groups of the Taylor GEMM
     int opt_green_legacy;   // testing aid: 1 = shared/global-memory elimination kernel instead of the register-resident one
+    cudaStream_t copy_stream;   // afqmc_step_host: downloads the propagated walkers during the energy evaluation
+    cudaEvent_t ev_copy[2];
     cudaEvent_t ev[AFQMC_NUM_STAGES + 1];
     int ev_valid;
     int smem_optin;     // max dynamic shared memory per block (bytes)

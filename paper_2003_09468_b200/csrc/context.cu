@@ -143,6 +143,9 @@ AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
         if (p) cudaFree(p);
     for (cudaEvent_t e : c->ev)
         if (e) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->ev_copy)
+        if (e) cudaEventDestroy(e);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     delete c;
 }
 

@@ -29,22 +29,47 @@ AFQMC_API int afqmc_step(afqmc_ctx* c, void* phi, const double* x, double dtau, 
 
 AFQMC_API int afqmc_step_host(afqmc_ctx* c, void* phi_host, const double* x_host, double dtau, int order,
                                int nw, void* energy_host, void* logdet_host, int* info_host, void* stream) {
-    if (!c || !phi_host || !x_host || !energy_host || nw < 0 || nw > c->max_walkers) return AFQMC_INVALID_ARGUMENT;
+    if (!c || !phi_host || !x_host || !energy_host || nw < 0 || nw > c->max_walkers || order < 0 || order > 32 || !(dtau >= 0.0))
+        return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
     cudaStream_t st = (cudaStream_t)stream;
     const Dims& d = c->d;
     const size_t phi_bytes = (size_t)nw * d.M * d.N * sizeof(double2);
     const size_t x_bytes = (size_t)nw * d.Nk * d.nchol * sizeof(double);
+    // a second stream carries the download of the propagated walkers while the energy of those walkers is evaluated
+    if (!c->copy_stream) {
+        AFQMC_CUDA_TRY(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        AFQMC_CUDA_TRY(cudaEventCreateWithFlags(&c->ev_copy[0], cudaEventDisableTiming));
+        AFQMC_CUDA_TRY(cudaEventCreateWithFlags(&c->ev_copy[1], cudaEventDisableTiming));
+    }
     AFQMC_CUDA_TRY(cudaMemcpyAsync(c->ws_phi, phi_host, phi_bytes, cudaMemcpyHostToDevice, st));
     AFQMC_CUDA_TRY(cudaMemcpyAsync(c->ws_x, x_host, x_bytes, cudaMemcpyHostToDevice, st));
-    int rc = afqmc_step(c, c->ws_phi, c->ws_x, dtau, order, nw, c->ws_energy, c->ws_logdet, c->ws_info, stream);
-    if (rc != AFQMC_OK) return rc;
-    AFQMC_CUDA_TRY(cudaMemcpyAsync(phi_host, c->ws_phi, phi_bytes, cudaMemcpyDeviceToHost, st));
+    int rc;
+    // the same composition as afqmc_step (stage marks included)
+    afqmc_mark(c, 0, st);
+    if ((rc = afqmc_i_green(c, c->ws_phi, nw, c->ws_theta, nullptr, nullptr, st)) != AFQMC_OK) return rc;
+    afqmc_mark(c, 1, st);
+    if ((rc = afqmc_i_force_bias(c, c->ws_theta, nw, c->ws_vbias, st)) != AFQMC_OK) return rc;
+    afqmc_mark(c, 2, st);
+    if ((rc = afqmc_i_vhs(c, c->ws_x, c->ws_vbias, dtau, nw, c->ws_vhs, st)) != AFQMC_OK) return rc;
+    afqmc_mark(c, 3, st);
+    if ((rc = afqmc_i_propagate(c, c->ws_vhs, dtau, order, c->ws_phi, nw, st)) != AFQMC_OK) return rc;
+    afqmc_mark(c, 4, st);
+    AFQMC_CUDA_TRY(cudaEventRecord(c->ev_copy[0], st));                      // phi' is final here
+    AFQMC_CUDA_TRY(cudaStreamWaitEvent(c->copy_stream, c->ev_copy[0], 0));
+    AFQMC_CUDA_TRY(cudaMemcpyAsync(phi_host, c->ws_phi, phi_bytes, cudaMemcpyDeviceToHost, c->copy_stream));
+    AFQMC_CUDA_TRY(cudaEventRecord(c->ev_copy[1], c->copy_stream));
+    if ((rc = afqmc_i_green(c, c->ws_phi, nw, c->ws_theta, c->ws_logdet, c->ws_info, st)) != AFQMC_OK) return rc;
+    afqmc_mark(c, 5, st);
+    if ((rc = afqmc_i_local_energy(c, c->ws_theta, nw, c->ws_energy, st)) != AFQMC_OK) return rc;
+    afqmc_mark(c, 8, st);
+    if (c->opt_timers) c->ev_valid = 1;
     AFQMC_CUDA_TRY(cudaMemcpyAsync(energy_host, c->ws_energy, (size_t)nw * 3 * sizeof(double2), cudaMemcpyDeviceToHost, st));
     if (logdet_host)
         AFQMC_CUDA_TRY(cudaMemcpyAsync(logdet_host, c->ws_logdet, (size_t)nw * sizeof(double2), cudaMemcpyDeviceToHost, st));
     if (info_host)
         AFQMC_CUDA_TRY(cudaMemcpyAsync(info_host, c->ws_info, (size_t)nw * sizeof(int), cudaMemcpyDeviceToHost, st));
+    AFQMC_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_copy[1], 0));               // the caller's stream owns the whole result
     AFQMC_CUDA_TRY(cudaStreamSynchronize(st));
     return AFQMC_OK;
 }
