@@ -42,6 +42,7 @@ struct afqmc_ctx {
     double2* ht;    // [Nk][n][m]   half-rotated one-body
     double* Lx;     // exchange fragment layout  [Q][k][ag][gq][s][lane][2]
     double* Lx3;    // exchange, 3M products      [Q][k][ag][gq][ks][prod][lane][2]   (exchange3m.cu; n <= 4 only, else NULL)
+    float* LxT;     // exchange, TF32 fragments       [Q][k][gq][ks][lane][4]             (exchange_tf32.cu; n <= 4 only, else NULL)
     double* Lf;     // force-bias fragment layout [Q][gtp][k][a][s][lane][2]
     double2* Lv3;   // vHS operand [unit][prt][ks][lane] complex fragments (vhs.cu); one block per (Q,-Q) pair if vhs_paired
     int* vunits;    // vHS work units, int4-packed (Q, k, kind, 0) [nvunits]; kind 1 = block + its (-Q,k-Q) partner
@@ -77,6 +78,7 @@ struct afqmc_ctx {
     int opt_fb_tile;        // tuning aid: warp tile of the force-bias kernel for > 16 walkers (0: 4x4, 1: 4x8, 2: 2x8 m x n tiles)
     int opt_fb_pf;          // L2 prefetch distance (k-steps) of the Lf stream in the force-bias kernel
     int opt_exchange_minb;  // tuning aid: 1 = ask for more resident CTAs per SM
+    int opt_exchange_prec;  // 0 (default) = FP64 exchange kernels; mixed precision on the TF32 tensor cores (n <= 4): 1 = 3xTF32 split, 2 = 1xTF32
     int opt_exchange_3m;    // 1 (default) = 3M exchange kernel when n <= 4, 0 = the 4M kernel of energy.cu
     int opt_exchange_wpc;   // 0 = automatic, else warps per CTA of the exchange kernel (4,5,6,8)
     int opt_timers;     // record stage events in afqmc_step
@@ -162,6 +164,9 @@ int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, 
 int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* energy, cudaStream_t st);
 int afqmc_i_exchange3m(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st);   // AFQMC_UNSUPPORTED if n > 4
 int afqmc_i_pack_lx3(afqmc_ctx* c, const double2* L, cudaStream_t st);
+int afqmc_i_exchange_tf32(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st);  // AFQMC_UNSUPPORTED if n > 4
+int afqmc_i_pack_lxt(afqmc_ctx* c, const double2* L, cudaStream_t st);
+size_t afqmc_i_lxt_floats(const Dims& d);
 size_t afqmc_i_lx3_doubles(const Dims& d);
 int afqmc_i_apply_onebody(afqmc_ctx* c, double2* phi, int nw, cudaStream_t st);
 size_t afqmc_i_taylor_ws_doubles(const Dims& d);

@@ -135,7 +135,7 @@ static int dev_alloc(T** p, size_t count) {
 
 AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     if (!c) return;
-    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lx, c->Lx3, c->Lf, c->Lv3, c->vunits,
+    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lx, c->Lx3, c->LxT, c->Lf, c->Lv3, c->vunits,
                     c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T, c->ws_Tx,
                     c->ws_expart, c->ws_fbpart, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
                     c->b1, c->ws_b1tmp, c->ws_gram, c->ws_rinv, c->ws_logdet2, c->ws_ldr, c->ws_info2};
@@ -225,6 +225,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     A(dev_alloc(&c->ht, (size_t)Nk * d.n * d.m));
     A(dev_alloc(&c->Lx, nLx));
     if (d.NAG == 1) A(dev_alloc(&c->Lx3, afqmc_i_lx3_doubles(d)));
+    if (d.NAG == 1) A(dev_alloc(&c->LxT, afqmc_i_lxt_floats(d)));
     A(dev_alloc(&c->Lf, nLf));
     A(dev_alloc(&c->ws_O, (size_t)nw * d.N * LD));
     A(dev_alloc(&c->ws_oinvT, (size_t)nw * d.N * d.N));
@@ -273,6 +274,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
         c->launches += 3;
         if (cudaGetLastError() != cudaSuccess) rc = AFQMC_CUDA_ERROR;
         if (rc == AFQMC_OK && c->Lx3) rc = afqmc_i_pack_lx3(c, (const double2*)L, st);
+        if (rc == AFQMC_OK && c->LxT) rc = afqmc_i_pack_lxt(c, (const double2*)L, st);
         if (rc == AFQMC_OK) rc = afqmc_i_vhs_setup(c, (const double2*)L, kminus, kneg, st);
     }
     // host vectors must outlive the async copies; the caller may free its arrays after return
@@ -291,6 +293,7 @@ AFQMC_API double afqmc_exchange_flops(const afqmc_ctx* c, int nw) {
     // 4M kernel: 8 real flops per complex multiply-add = 2 * 8*n*n*m*nchol.  3M kernel (exchange3m.cu): 6 real
     // flops per complex multiply-add = 2 * 6*n*n*m*nchol, plus 3 additions per element of both T tensors.
     double per = 16.0 * d.n * d.n * d.m * d.nchol + 8.0 * d.n * d.n * d.nchol;
+    if (c->opt_exchange_prec != 0 && c->LxT) return (c->opt_exchange_prec == 1 ? 3.0 : 1.0) * per * (double)c->nunits * (double)nw;      // TF32 kernel: the 4M real embedding
     if (c->opt_exchange_3m && c->Lx3) per = 12.0 * d.n * d.n * d.m * d.nchol + 6.0 * d.n * d.n * d.nchol + 8.0 * d.n * d.n * d.nchol;
     return per * (double)c->nunits * (double)nw;
 }
@@ -310,6 +313,12 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
     if (strcmp(name, "force_bias_prefetch") == 0) {
         if (value < 0 || value > 256) return AFQMC_INVALID_ARGUMENT;
         c->opt_fb_pf = value;
+        return AFQMC_OK;
+    }
+    if (strcmp(name, "exchange_precision") == 0) {
+        if (value < 0 || value > 2) return AFQMC_INVALID_ARGUMENT;
+        if (value != 0 && !c->LxT) return AFQMC_UNSUPPORTED;        // n > 4
+        c->opt_exchange_prec = value;
         return AFQMC_OK;
     }
     if (strcmp(name, "exchange_3m") == 0) {

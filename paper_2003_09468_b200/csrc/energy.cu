@@ -330,7 +330,8 @@ int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* en
     int rc = afqmc_i_force_bias(c, theta, nw, c->ws_vbias, st);     // steps 2(d): the traces are the force bias
     if (rc != AFQMC_OK) return rc;
     afqmc_mark(c, 6, st);
-    rc = c->opt_exchange_3m ? afqmc_i_exchange3m(c, theta, nw, st) : AFQMC_UNSUPPORTED;
+    rc = c->opt_exchange_prec != 0 ? afqmc_i_exchange_tf32(c, theta, nw, st)
+         : c->opt_exchange_3m    ? afqmc_i_exchange3m(c, theta, nw, st) : AFQMC_UNSUPPORTED;
     if (rc == AFQMC_UNSUPPORTED) {          // n > 4, or the 4M kernel was asked for
         if (nw >= 3) rc = launch_exchange<4>(c, theta, nw, st);
         else rc = launch_exchange<2>(c, theta, nw, st);

@@ -358,6 +358,61 @@ def test_exchange_3m_and_4m_kernels_against_the_oracle(kw):
         case.close()
 
 
+@pytest.mark.parametrize("kw", [dict(mesh=(2, 2, 1), m=6, n=4, nchol=10, nw=4), dict(mesh=(2, 3, 1), m=5, n=3, nchol=7, nw=5),
+                                dict(mesh=(1, 2, 2), m=9, n=1, nchol=5, nw=2), dict(mesh=(3, 1, 1), m=26, n=4, nchol=18, nw=7)],
+                         ids=["n4", "n3_odd", "n1_two_walkers", "m26_seven_walkers"])
+def test_mixed_precision_exchange_against_the_oracle(kw):
+    """Option exchange_precision (exchange_tf32.cu), the analogue of the paper's single-precision mode and
+    of the north_star's optional complex64 path (tolerance 1e-4): mode 1 (3xTF32 split) is held to 1e-5 relative on EX
+    against the FP64 oracle, mode 2 (operands rounded once to TF32) only to 1e-2 (it is documented as outside the 1e-4
+    tolerance).  E1 and EC must not change at all."""
+    case = Case(synth.tiny_config(seed=19, **kw))
+    try:
+        theta_d, _, _ = case.ctx.green(_to_dev(case.pb.phi))
+        theta = theta_d.cpu().numpy()
+        e_o = np.array([orc.local_energy(case.cfg.mesh, case.Lh, case.ht, theta[w]) for w in range(case.nw)])
+        e64 = case.ctx.local_energy(theta_d).cpu().numpy()
+        for mode, tol in ((1, 1e-5), (2, 1e-2)):
+            case.ctx.set_option("exchange_precision", mode)
+            try:
+                e = case.ctx.local_energy(theta_d).cpu().numpy()
+            finally:
+                case.ctx.set_option("exchange_precision", 0)
+            assert np.array_equal(e[:, :2], e64[:, :2])
+            for w in range(case.nw):
+                assert abs(e[w, 2] - e_o[w, 2]) / abs(e_o[w, 2]) < tol, (mode, w, e[w, 2], e_o[w, 2])
+    finally:
+        case.close()
+
+
+def test_mixed_precision_exchange_is_unsupported_for_more_than_four_orbitals():
+    from paper_2003_09468_b200 import binding
+    case = Case(synth.tiny_config(mesh=(1, 1, 1), m=7, n=5, nchol=9, nw=1, seed=3))
+    try:
+        with pytest.raises(binding.AfqmcError) as e:
+            case.ctx.set_option("exchange_precision", 1)
+        assert e.value.code == 2
+    finally:
+        case.close()
+
+
+def test_mixed_precision_exchange_c3_full_size():
+    """C3 at full size: 3xTF32 against the FP64 kernel on every walker (the FP64 kernel is checked against the oracle in
+    test_config_C3_headline_sampled), and against the oracle on one walker."""
+    case = Case(synth.CONFIGS["C3"])
+    try:
+        theta_d, _, _ = case.ctx.green(_to_dev(case.pb.phi))
+        e64 = case.ctx.local_energy(theta_d).cpu().numpy()
+        case.ctx.set_option("exchange_precision", 1)
+        e = case.ctx.local_energy(theta_d).cpu().numpy()
+        case.ctx.set_option("exchange_precision", 0)
+        assert np.max(np.abs(e[:, 2] - e64[:, 2]) / np.abs(e64[:, 2])) < 1e-5
+        e_o = orc.local_energy(case.cfg.mesh, case.Lh, case.ht, theta_d[5].cpu().numpy())
+        assert abs(e[5, 2] - e_o[2]) / abs(e_o[2]) < 1e-5
+    finally:
+        case.close()
+
+
 @pytest.mark.parametrize("mesh,n", [((4, 4, 3), 6), ((4, 3, 3), 7), ((5, 5, 1), 5)], ids=["N288_legacy", "N252_cluster8", "N125_cluster2"])
 def test_green_large_N(mesh, n):
     """Overlap sizes that select the cluster kernels (N <= 128: 2 CTAs, N <= 256: 8 CTAs) and the legacy path (N > 256)."""
