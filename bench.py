@@ -210,7 +210,11 @@ def run_ours(args):
     # ---------------- optional mixed-precision exchange (exchange_tf32.cu): extra information, NOT the headline ----------
     mixed = {}
     for mode, label in ((1, "3xTF32"), (2, "1xTF32")):
-        ctx.set_option("exchange_precision", mode)
+        try:
+            ctx.set_option("exchange_precision", mode)
+        except binding.AfqmcError:            # more than 4 occupied orbitals per k-point: FP64 kernels only
+            mixed[label] = None
+            continue
         tot = exm = 0.0
         for i in range(4):
             phi.copy_(phi0)
