@@ -85,6 +85,7 @@ struct afqmc_ctx {
     int opt_taylor_legacy;  // testing aid: 1 = shared-memory-tiled zgemm for the Taylor chain
     int opt_taylor_wpc;     // tuning aid: 0 = automatic, else 3/4/5 warps per CTA of the Taylor GEMM
     int opt_taylor_groups;  // tuning aid: 0 = automatic, else the number of column groups of the Taylor GEMM
+    int opt_green_cs;       // tuning aid: 4 = cluster of four CTAs per walker for 64 < N <= 128 (default two)
     int opt_green_legacy;   // testing aid: 1 = shared/global-memory elimination kernel instead of the register-resident one
     cudaStream_t copy_stream;   // afqmc_step_host: downloads the propagated walkers during the energy evaluation
     cudaEvent_t ev_copy[2];

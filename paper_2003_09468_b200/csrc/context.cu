@@ -348,6 +348,11 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
         c->opt_taylor_groups = value;
         return AFQMC_OK;
     }
+    if (strcmp(name, "green_cluster") == 0) {
+        if (value != 0 && value != 2 && value != 4) return AFQMC_INVALID_ARGUMENT;
+        c->opt_green_cs = value;
+        return AFQMC_OK;
+    }
     if (strcmp(name, "green_legacy") == 0) {
         c->opt_green_legacy = value ? 1 : 0;
         return AFQMC_OK;

@@ -415,7 +415,13 @@ int run_overlap_inverse(afqmc_ctx* c, const double2* phi, int nw, double2* oinvT
         // register-resident elimination: one CTA for N <= 64, a cluster of two for N <= 128, of eight for N <= 256
         if (d.N <= 32) return launch_gj_reg<1, 2, 16, 1>(c, phi, nw, oinvT, logdet, info, st);
         if (d.N <= 64) return launch_gj_reg<2, 4, 16, 1>(c, phi, nw, oinvT, logdet, info, st);
-        if (d.N <= 128) return launch_gj_reg<4, 4, 16, 2>(c, phi, nw, oinvT, logdet, info, st);
+        if (d.N <= 128) {
+            // four CTAs per walker when they all fit one wave (the update is instruction-bound on the SMs that hold a
+            // walker: C3 0.388 -> 0.355 ms), else two
+            const bool four = c->opt_green_cs == 4 || (c->opt_green_cs == 0 && 4 * nw <= c->num_sms);
+            return four ? launch_gj_reg<4, 2, 16, 4>(c, phi, nw, oinvT, logdet, info, st)
+                        : launch_gj_reg<4, 4, 16, 2>(c, phi, nw, oinvT, logdet, info, st);
+        }
         if (d.N <= 256) return launch_gj_reg<8, 2, 16, 8>(c, phi, nw, oinvT, logdet, info, st);
     }
     const int LD = d.N | 1;
