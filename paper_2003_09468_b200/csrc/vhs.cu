@@ -29,17 +29,11 @@
 
 namespace {
 
-#ifndef AFQMC_V3_KC
-#define AFQMC_V3_KC 2
-#endif
-#ifndef AFQMC_V3_STAGES
-#define AFQMC_V3_STAGES 3
-#endif
-#ifndef AFQMC_V3_D4
-#define AFQMC_V3_D4 3
-#endif
-constexpr int V3_KC = AFQMC_V3_KC;        // k-steps per shared-memory stage
-constexpr int V3_STAGES = AFQMC_V3_STAGES;
+constexpr int V3_STAGES = 3;
+// k-steps per shared-memory stage = the depth D of the A register ring (template parameter of the kernel), so that
+// ring entry q always serves k-step q of a stage (static register indexing, no dispatch on a running ring index:
+// C3 0.777 -> 0.636 ms)
+constexpr int V3_DMAX = 6;
 constexpr int V3_WARPS = 4;
 
 // max |L[-Q][k-Q][g][r][p] - conj(L[Q][k][g][p][r])| and max |L| (both as ordered-int atomics on the bit patterns of
@@ -215,7 +209,8 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
     Dims d, int KS4, int KS4p, int nw, int nwg, int nsg, const int* __restrict__ vunits, const int* __restrict__ kminus,
     const double2* __restrict__ Lv3, const double* __restrict__ Bx3, double2* __restrict__ vhs) {
     extern __shared__ __align__(128) double v3_smem[];
-    constexpr int SET_DOUBLES = V3_KC * 3 * NT * 32;          // one column set of one stage
+    constexpr int KC = D;                                     // k-steps per stage
+    constexpr int SET_DOUBLES = KC * 3 * NT * 32;             // one column set of one stage
     constexpr int STAGE_DOUBLES = 2 * SET_DOUBLES;
     uint64_t* full = reinterpret_cast<uint64_t*>(v3_smem + (size_t)V3_STAGES * STAGE_DOUBLES);
     uint64_t* empty = full + V3_STAGES;
@@ -241,7 +236,7 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
     if (slice >= nslices) return;
 
     const int nsets = kind ? 2 : 1;
-    const int nchunks = KS4p / V3_KC;
+    const int nchunks = KS4p / KC;
     const double* bsrc0 = Bx3 + ((((size_t)Q * 2 + 0) * nwg + wg) * KS4p) * 3 * NT * 32;
     const double* bsrc1 = Bx3 + ((((size_t)Q * 2 + 1) * nwg + wg) * KS4p) * 3 * NT * 32;
     auto produce = [&](int ch) {       // thread 0 only
@@ -258,7 +253,6 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
     const int prt0 = 2 * slice, prt1 = min(prt0 + 1, d.PRT - 1);
     const double2* pa0 = Lv3 + (((size_t)u * d.PRT + prt0) * KS4) * 32 + lane;
     const double2* pa1 = Lv3 + (((size_t)u * d.PRT + prt1) * KS4) * 32 + lane;
-    static_assert(D == 3 || D == 6, "the ring switch below enumerates 3 or 6 entries");
     double2 fa0[D], fa1[D];
 #pragma unroll
     for (int q = 0; q < D; ++q) {
@@ -294,23 +288,13 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
         fa1[qa] = __ldg(pa1 + (size_t)nk * 32);
         ++ksg;
     };
-    int qa = 0;
     for (int ch = 0; ch < nchunks; ++ch) {
         const int s = ch % V3_STAGES;
         v3_mbar_wait(&full[s], (uint32_t)((ch / V3_STAGES) & 1));
         const double* bs = v3_smem + (size_t)s * STAGE_DOUBLES + set * SET_DOUBLES + lane;
 #pragma unroll
-        for (int q = 0; q < V3_KC; ++q) {
-            // the A register ring has D entries; qa cycles 0..D-1 (a switch keeps the register indices static)
-            switch (qa) {
-                case 0: kstep(bs + q * 3 * NT * 32, 0); break;
-                case 1: kstep(bs + q * 3 * NT * 32, 1); break;
-                case 2: kstep(bs + q * 3 * NT * 32, 2); break;
-                case 3: kstep(bs + q * 3 * NT * 32, D > 3 ? 3 : 0); break;
-                case 4: kstep(bs + q * 3 * NT * 32, D > 3 ? 4 : 0); break;
-                default: kstep(bs + q * 3 * NT * 32, D > 3 ? 5 : 0); break;
-            }
-            qa = qa + 1 == D ? 0 : qa + 1;
+        for (int q = 0; q < KC; ++q) {
+            kstep(bs + q * 3 * NT * 32, q);
             if (q == 0 && tid == 0) {   // producer duty: refill the stage consumed in the previous iteration
                 const int nxt = ch + V3_STAGES - 1;
                 if (nxt < nchunks) {
@@ -356,7 +340,7 @@ int launch_vhs3(afqmc_ctx* c, int nw, int KS4, int KS4p, double2* vhs, cudaStrea
     const int nwg = (nw + 8 * NT - 1) / (8 * NT);
     const int nslices = (d.PRT + 1) / 2;
     const int nsg = (c->vhs_paired && !MERGED) ? (nslices + V3_WARPS / 2 - 1) / (V3_WARPS / 2) : (nslices + V3_WARPS - 1) / V3_WARPS;
-    const size_t smem = (size_t)V3_STAGES * 2 * V3_KC * 3 * NT * 32 * sizeof(double) + 2 * V3_STAGES * sizeof(uint64_t);
+    const size_t smem = (size_t)V3_STAGES * 2 * D * 3 * NT * 32 * sizeof(double) + 2 * V3_STAGES * sizeof(uint64_t);
     const long long gx = (long long)c->nvunits * nsg;
     if (gx > 0x7fffffffLL || nwg > 65535) return AFQMC_UNSUPPORTED;
     static bool attr_done = false;
@@ -375,7 +359,7 @@ int launch_vhs3(afqmc_ctx* c, int nw, int KS4, int KS4p, double2* vhs, cudaStrea
 
 // doubles of the expanded field operand for up to nw walkers (workspace sizing; the largest over the NT choices)
 size_t afqmc_i_vhs_field_doubles(const Dims& d, int nw) {
-    const int KS4 = (d.nchol + 3) / 4, KS4p = (KS4 + V3_KC - 1) / V3_KC * V3_KC;
+    const int KS4 = (d.nchol + 3) / 4, KS4p = KS4 + V3_DMAX;          // covers the padding to a multiple of any ring depth
     const int ntiles = (nw + 7) / 8;
     return (size_t)d.Nk * 2 * KS4p * 3 * (size_t)((ntiles + 3) / 4 * 4) * 32;
 }
@@ -383,8 +367,9 @@ size_t afqmc_i_vhs_field_doubles(const Dims& d, int nw) {
 int afqmc_i_vhs(afqmc_ctx* c, const double* x, const double2* vbias, double dtau, int nw, double2* vhs,
                 cudaStream_t st) {
     const Dims& d = c->d;
-    const int KS4 = (d.nchol + 3) / 4, KS4p = (KS4 + V3_KC - 1) / V3_KC * V3_KC;
     const int NT = nw > 16 ? 4 : (nw > 8 ? 2 : 1);
+    const int D = NT == 4 ? 3 : 6;                                       // ring depth = k-steps per stage of the kernel chosen below
+    const int KS4 = (d.nchol + 3) / 4, KS4p = (KS4 + D - 1) / D * D;
     const int nwg = (nw + 8 * NT - 1) / (8 * NT);
     {
         const size_t total = (size_t)d.Nk * 2 * nwg * KS4p * NT * 32;
@@ -393,7 +378,7 @@ int afqmc_i_vhs(afqmc_ctx* c, const double* x, const double2* vbias, double dtau
         fields3_kernel<<<G, T, 0, st>>>(d, nw, NT, nwg, KS4p, c->kneg, x, vbias, sqrt(dtau), reinterpret_cast<double*>(c->ws_xi));
         AFQMC_LAUNCH_CHECK(c);
     }
-    if (NT == 4) return launch_vhs3<4, false, AFQMC_V3_D4>(c, nw, KS4, KS4p, vhs, st);
+    if (NT == 4) return launch_vhs3<4, false, 3>(c, nw, KS4, KS4p, vhs, st);
     if (NT == 2) return c->vhs_paired ? launch_vhs3<2, true, 6>(c, nw, KS4, KS4p, vhs, st) : launch_vhs3<2, false, 6>(c, nw, KS4, KS4p, vhs, st);
     return c->vhs_paired ? launch_vhs3<1, true, 6>(c, nw, KS4, KS4p, vhs, st) : launch_vhs3<1, false, 6>(c, nw, KS4, KS4p, vhs, st);
 }
