@@ -31,9 +31,9 @@ METRIC = "walker-steps/s incl. local energy"
 UNIT = "walker-steps/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE exchange-kernel launch, from the committed
-# `ncu --set full` capture of this same command (profiles/r01f_ncu_full_metrics.txt, the default 3M kernel); bench.py
+# `ncu --set full` capture of this same command (profiles/r01g_ncu_full_metrics.txt, the default 3M kernel); bench.py
 # cannot measure DRAM traffic itself.  Only the configuration that was captured has a value.
-EXCHANGE_DRAM_TRAFFIC = {"C3": {"bytes": 718.598e6 + 9.912e6, "source": "profiles/r01f_ncu_full_metrics.txt"}}
+EXCHANGE_DRAM_TRAFFIC = {"C3": {"bytes": 722.316e6 + 9.972e6, "source": "profiles/r01g_ncu_full_metrics.txt"}}
 
 
 def load_measured_peaks():

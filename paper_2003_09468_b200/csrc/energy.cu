@@ -219,7 +219,7 @@ __device__ double2 block_sum2(double2 v, double* scratch /* >= 64 doubles */) {
     return r;
 }
 
-__global__ void __launch_bounds__(256) energy_finalize_kernel(
+__global__ void __launch_bounds__(1024) energy_finalize_kernel(
     Dims d, int nw, int nunits, const int* __restrict__ units, const int* __restrict__ kneg,
     const double2* __restrict__ ht, const double2* __restrict__ theta, const double2* __restrict__ vbias,
     const double2* __restrict__ partial, double2* __restrict__ energy) {
@@ -338,7 +338,7 @@ int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* en
     }
     if (rc != AFQMC_OK) return rc;
     afqmc_mark(c, 7, st);
-    energy_finalize_kernel<<<nw, 256, 0, st>>>(d, nw, c->nunits, c->units, c->kneg, c->ht, theta, c->ws_vbias,
+    energy_finalize_kernel<<<nw, 1024, 0, st>>>(d, nw, c->nunits, c->units, c->kneg, c->ht, theta, c->ws_vbias,
                                               c->ws_expart, energy);
     AFQMC_LAUNCH_CHECK(c);
     return AFQMC_OK;

@@ -29,8 +29,18 @@
 
 namespace tg {
 
-constexpr int KC = 4;        // k-groups (of 4 complex k) per shared-memory stage
-constexpr int STAGES = 3;
+#ifndef AFQMC_TG_KC
+#define AFQMC_TG_KC 4
+#endif
+#ifndef AFQMC_TG_STAGES
+#define AFQMC_TG_STAGES 3
+#endif
+#ifndef AFQMC_TG_D
+#define AFQMC_TG_D 2
+#endif
+constexpr int KC = AFQMC_TG_KC;        // k-groups (of 4 complex k) per shared-memory stage
+constexpr int STAGES = AFQMC_TG_STAGES;
+constexpr int DEPTH = AFQMC_TG_D;      // k-groups of register prefetch of the A stream (divides KC)
 constexpr int NTMAX = 4;     // n-tiles (8 columns) per column group: 3 products x 2 m-tiles x 4 tiles x 2 = 48 accumulators
 // warps per CTA (WPC, 16 rows each) is a template parameter chosen per launch: see launch_cfg()
 
@@ -316,7 +326,7 @@ static inline cudaError_t launch_cfg(const Args& a, int batch, cudaStream_t st) 
 // resident CTAs per SM of the 4-warp kernel instantiated for NTA tiles per group
 static inline cudaError_t query_occupancy(int NTA, int* occ) {
     Args a = {};
-#define TG_CALL(n) launch_wpc<n, 2, 4>(a, 1, nullptr, occ)
+#define TG_CALL(n) launch_wpc<n, DEPTH, 4>(a, 1, nullptr, occ)
     TG_NTA_SWITCH(NTA, TG_CALL)
 #undef TG_CALL
 }
@@ -350,7 +360,7 @@ static inline cudaError_t launch(Args a, int batch, cudaStream_t st, int G = 0) 
     a.G = gr.G; a.nt_base = gr.nt_base; a.nt_rem = gr.nt_rem;
     a.NPp = padded_pairs(a.K);
     a.NPcp = padded_pairs(a.M);
-#define TG_CALL(n) launch_cfg<n, 2>(a, batch, st)
+#define TG_CALL(n) launch_cfg<n, DEPTH>(a, batch, st)
     TG_NTA_SWITCH(gr.NTA, TG_CALL)
 #undef TG_CALL
 }
