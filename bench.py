@@ -373,6 +373,31 @@ def run_ours(args):
             "e_mixed": [float((em[0] + em[1] + em[2]).real / em[3].real) if em[3].real > 0 else None][0],
         }
         bctx.close()
+    # ---- the optional complex64 boundary (afqmc_dims.precision = 1): extra information, N=1 only ----
+    if world == 1 and rank == 0 and not args.no_block:
+        torch.cuda.empty_cache()
+        pb64 = synth.make_problem(cfg)
+        c64 = binding.from_problem(pb64, precision=1)
+        phi64_0 = torch.from_numpy(pb64.phi).to(torch.complex64).cuda()
+        x32 = torch.from_numpy(pb64.x).to(torch.float32).cuda()
+        ms64 = []
+        for it in range(4):
+            p64 = phi64_0.clone()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            e64, _, _ = c64.step(p64, x32, cfg.dtau, cfg.order)
+            e1.record()
+            torch.cuda.synchronize()
+            if it > 0:
+                ms64.append(e0.elapsed_time(e1))
+        err = np.abs(e64.cpu().numpy().astype(np.complex128) - e_dev) / np.abs(e_dev)
+        line["complex64_path"] = {"ms_per_step": sum(ms64) / len(ms64), "walker_steps_per_s": nw / (sum(ms64) / len(ms64) * 1e-3),
+                                  "max_rel_diff_vs_complex128": [float(err[:, i].max()) for i in range(3)],
+                                  "note": "afqmc_dims.precision = 1: complex64 arrays at the boundary, FP64 small algebra, 3xTF32 "
+                                          "exchange; extra information (the energies are those of the polynomial-propagated walkers, "
+                                          "whose FP32 storage error is amplified by the synthetic step size, DESIGN.md R9)"}
+        c64.close()
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:

@@ -23,6 +23,13 @@
  *   energy[nw][3]         complex (E1, EC, EX);  logdet[nw] complex = log|det O| + i arg det O of
  *                         ONE spin channel, arg in (-pi, pi];  info[nw] int32.
  *
+ * Precision 1 (optional complex64 path; the paper's production runs are single precision): with
+ * afqmc_dims.precision = 1 EVERY complex array of afqmc_create, of the six step calls, of afqmc_step and of
+ * afqmc_step_host is complex64 (float re, im) and every real array (x) is float32; shapes and layouts are unchanged.
+ * Inside, the small algebra runs in FP64 on widened copies and the exchange contraction on the TF32 tensor cores with a
+ * high/low operand split (option "exchange_precision" = 1).  Results agree with the FP64 path to FP32 input/output
+ * accuracy (tolerance 1e-4).  The AFQMC-block calls return AFQMC_UNSUPPORTED in this mode.
+ *
  * Errors: every call returns an int; 0 = AFQMC_OK.  No exceptions cross the ABI, there is no
  * global state.  A singular overlap cannot be a return code of an asynchronous call: it is
  * reported LAPACK-style in the device array info[w] (0 ok, j>0 = exactly-zero pivot at
@@ -47,14 +54,14 @@ typedef struct {
     int n;            /* occupied orbitals per k-point per spin                      */
     int nchol;        /* Cholesky vectors per Q             */
     int closed_shell; /* must be 1 (else AFQMC_UNSUPPORTED)                          */
-    int precision;    /* 0 = complex128 (only value supported so far)               */
+    int precision;    /* 0 = complex128; 1 = complex64 boundary (see "Precision 1" below)  */
     int max_walkers;  /* workspace is sized for this many walkers                    */
 } afqmc_dims;
 
 enum {
     AFQMC_OK = 0,
     AFQMC_INVALID_ARGUMENT = 1, /* null pointer, nw < 0 or > max_walkers, bad dims, bad order */
-    AFQMC_UNSUPPORTED = 2,      /* open shell, precision != 0                                 */
+    AFQMC_UNSUPPORTED = 2,      /* open shell, precision > 1, block calls with precision 1 ...  */
     AFQMC_CUDA_ERROR = 3,       /* a CUDA runtime call or launch failed                       */
     AFQMC_OUT_OF_MEMORY = 4     /* device allocation failed                                   */
 };

@@ -116,6 +116,10 @@ class Afqmc:
         self.m, self.n, self.nchol = int(m), int(n), int(nchol)
         self.M, self.N = self.nk * self.m, self.nk * self.n
         self.max_walkers = int(max_walkers)
+        self.precision = int(precision)
+        # dtypes at the boundary: complex128/float64, or complex64/float32 with precision = 1 (include/afqmc.h "Precision 1")
+        self.cdtype = torch.complex64 if self.precision == 1 else torch.complex128
+        self.rdtype = torch.float32 if self.precision == 1 else torch.float64
         d = Dims((ctypes.c_int * 3)(*self.mesh), self.m, self.n, self.nchol, closed_shell, precision, self.max_walkers)
         for name, t, shape in (("h1", h1, (self.nk, self.m, self.m)),
                                ("L", L, (self.nk, self.nk, self.nchol, self.m, self.m)),
@@ -124,8 +128,8 @@ class Afqmc:
                 raise ValueError("%s must be a CUDA tensor of shape %s" % (name, shape))
         self.device = h1.device
         h = ctypes.c_void_p(0)
-        code = lib().afqmc_create(ctypes.byref(h), ctypes.byref(d), _ptr(h1, torch.complex128),
-                                  _ptr(L, torch.complex128), _ptr(psi_t, torch.complex128), _stream())
+        code = lib().afqmc_create(ctypes.byref(h), ctypes.byref(d), _ptr(h1, self.cdtype),
+                                  _ptr(L, self.cdtype), _ptr(psi_t, self.cdtype), _stream())
         _check(code, "afqmc_create")
         self._h = h
 
@@ -141,8 +145,8 @@ class Afqmc:
             pass
 
     # ---- helpers -------------------------------------------------------------------------
-    def _empty(self, shape, dtype=torch.complex128):
-        return torch.empty(shape, dtype=dtype, device=self.device)
+    def _empty(self, shape, dtype=None):
+        return torch.empty(shape, dtype=self.cdtype if dtype is None else dtype, device=self.device)
 
     def launch_count(self) -> int:
         return int(lib().afqmc_launch_count(self._h))
@@ -166,7 +170,7 @@ class Afqmc:
         nw = phi.shape[0]
         logdet = self._empty((nw,)) if logdet is None else logdet
         info = self._empty((nw,), torch.int32) if info is None else info
-        _check(lib().afqmc_overlap(self._h, _ptr(phi, torch.complex128), nw, _ptr(logdet), _ptr(info, torch.int32),
+        _check(lib().afqmc_overlap(self._h, _ptr(phi, self.cdtype), nw, _ptr(logdet), _ptr(info, torch.int32),
                                    _stream()), "afqmc_overlap")
         return logdet, info
 
@@ -175,34 +179,34 @@ class Afqmc:
         theta = self._empty((nw, self.N, self.M)) if theta is None else theta
         logdet = self._empty((nw,)) if logdet is None else logdet
         info = self._empty((nw,), torch.int32) if info is None else info
-        _check(lib().afqmc_green(self._h, _ptr(phi, torch.complex128), nw, _ptr(theta, torch.complex128),
+        _check(lib().afqmc_green(self._h, _ptr(phi, self.cdtype), nw, _ptr(theta, self.cdtype),
                                  _ptr(logdet), _ptr(info, torch.int32), _stream()), "afqmc_green")
         return theta, logdet, info
 
     def force_bias(self, theta, vbias=None):
         nw = theta.shape[0]
         vbias = self._empty((nw, self.nk, self.nchol)) if vbias is None else vbias
-        _check(lib().afqmc_force_bias(self._h, _ptr(theta, torch.complex128), nw, _ptr(vbias, torch.complex128),
+        _check(lib().afqmc_force_bias(self._h, _ptr(theta, self.cdtype), nw, _ptr(vbias, self.cdtype),
                                       _stream()), "afqmc_force_bias")
         return vbias
 
     def vhs(self, x, vbias, dtau, vhs=None):
         nw = x.shape[0]
         vhs = self._empty((nw, self.M, self.M)) if vhs is None else vhs
-        _check(lib().afqmc_vhs(self._h, _ptr(x, torch.float64), _ptr(vbias, torch.complex128, optional=True),
-                               float(dtau), nw, _ptr(vhs, torch.complex128), _stream()), "afqmc_vhs")
+        _check(lib().afqmc_vhs(self._h, _ptr(x, self.rdtype), _ptr(vbias, self.cdtype, optional=True),
+                               float(dtau), nw, _ptr(vhs, self.cdtype), _stream()), "afqmc_vhs")
         return vhs
 
     def propagate(self, vhs, dtau, order, phi):
         nw = phi.shape[0]
-        _check(lib().afqmc_propagate(self._h, _ptr(vhs, torch.complex128), float(dtau), int(order),
-                                     _ptr(phi, torch.complex128), nw, _stream()), "afqmc_propagate")
+        _check(lib().afqmc_propagate(self._h, _ptr(vhs, self.cdtype), float(dtau), int(order),
+                                     _ptr(phi, self.cdtype), nw, _stream()), "afqmc_propagate")
         return phi
 
     def local_energy(self, theta, energy=None):
         nw = theta.shape[0]
         energy = self._empty((nw, 3)) if energy is None else energy
-        _check(lib().afqmc_local_energy(self._h, _ptr(theta, torch.complex128), nw, _ptr(energy, torch.complex128),
+        _check(lib().afqmc_local_energy(self._h, _ptr(theta, self.cdtype), nw, _ptr(energy, self.cdtype),
                                         _stream()), "afqmc_local_energy")
         return energy
 
@@ -212,7 +216,7 @@ class Afqmc:
         energy = self._empty((nw, 3)) if energy is None else energy
         logdet = self._empty((nw,)) if logdet is None else logdet
         info = self._empty((nw,), torch.int32) if info is None else info
-        _check(lib().afqmc_step(self._h, _ptr(phi, torch.complex128), _ptr(x, torch.float64), float(dtau), int(order),
+        _check(lib().afqmc_step(self._h, _ptr(phi, self.cdtype), _ptr(x, self.rdtype), float(dtau), int(order),
                                 nw, _ptr(energy), _ptr(logdet), _ptr(info, torch.int32), _stream()), "afqmc_step")
         return energy, logdet, info
 
@@ -222,8 +226,8 @@ class Afqmc:
         for t in (phi_host, x_host, energy_host):
             if t.is_cuda:
                 raise ValueError("step_host takes host tensors")
-        _check(lib().afqmc_step_host(self._h, _ptr(phi_host, torch.complex128), _ptr(x_host, torch.float64),
-                                     float(dtau), int(order), nw, _ptr(energy_host, torch.complex128),
+        _check(lib().afqmc_step_host(self._h, _ptr(phi_host, self.cdtype), _ptr(x_host, self.rdtype),
+                                     float(dtau), int(order), nw, _ptr(energy_host, self.cdtype),
                                      _ptr(logdet_host, optional=True), _ptr(info_host, optional=True), _stream()),
                "afqmc_step_host")
         return energy_host
@@ -281,13 +285,14 @@ class Afqmc:
         return energy, emixed, logdet_r, info
 
 
-def from_problem(pb, max_walkers=None, device="cuda"):
-    """Builds a context from a `synth.Problem` (host numpy arrays -> device tensors)."""
+def from_problem(pb, max_walkers=None, device="cuda", precision=0):
+    """Builds a context from a `synth.Problem` (host numpy arrays -> device tensors; complex64 with precision = 1)."""
     cfg = pb.cfg
     dev = torch.device(device)
-    h1 = torch.from_numpy(pb.h1).to(dev)
-    L = torch.from_numpy(pb.L).to(dev)
-    psi_t = torch.from_numpy(pb.psi_t).to(dev)
-    ctx = Afqmc(cfg.mesh, cfg.m, cfg.n, cfg.nchol, h1, L, psi_t, max_walkers or pb.phi.shape[0])
+    cd = torch.complex64 if precision == 1 else torch.complex128
+    h1 = torch.from_numpy(pb.h1).to(dev).to(cd)
+    L = torch.from_numpy(pb.L).to(dev).to(cd)
+    psi_t = torch.from_numpy(pb.psi_t).to(dev).to(cd)
+    ctx = Afqmc(cfg.mesh, cfg.m, cfg.n, cfg.nchol, h1, L, psi_t, max_walkers or pb.phi.shape[0], precision=precision)
     del L
     return ctx

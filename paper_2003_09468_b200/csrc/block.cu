@@ -139,6 +139,7 @@ int afqmc_i_apply_onebody(afqmc_ctx* c, double2* phi, int nw, cudaStream_t st) {
 }
 
 AFQMC_API int afqmc_set_onebody(afqmc_ctx* c, const void* h1p, double dtau, void* b1_out, void* stream) {
+    if (c && c->prec32) return AFQMC_UNSUPPORTED;      // the block calls are FP64-only (boundary32.cu)
     if (!c || !h1p || !(dtau >= 0.0)) return AFQMC_INVALID_ARGUMENT;
     const Dims& d = c->d;
     cudaStream_t st = (cudaStream_t)stream;
@@ -151,6 +152,7 @@ AFQMC_API int afqmc_set_onebody(afqmc_ctx* c, const void* h1p, double dtau, void
 }
 
 AFQMC_API int afqmc_apply_onebody(afqmc_ctx* c, void* phi, int nw, void* stream) {
+    if (c && c->prec32) return AFQMC_UNSUPPORTED;      // the block calls are FP64-only (boundary32.cu)
     if (!c || !phi || nw < 0 || nw > c->max_walkers) return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
     return afqmc_i_apply_onebody(c, (double2*)phi, nw, (cudaStream_t)stream);
@@ -241,6 +243,7 @@ static int hybrid_weight_i(afqmc_ctx* c, const double* x, const double2* vbias, 
 
 AFQMC_API int afqmc_hybrid_weight(afqmc_ctx* c, const double* x, const void* vbias, double dtau, const void* logdet_old,
                                    const void* logdet_new, int nw, double* weight, void* log_i, void* stream) {
+    if (c && c->prec32) return AFQMC_UNSUPPORTED;      // the block calls are FP64-only (boundary32.cu)
     if (!c || !x || !vbias || !logdet_old || !logdet_new || !weight || nw < 0 || nw > c->max_walkers || !(dtau >= 0.0))
         return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
@@ -250,6 +253,7 @@ AFQMC_API int afqmc_hybrid_weight(afqmc_ctx* c, const double* x, const void* vbi
 
 AFQMC_API int afqmc_mixed_estimator(afqmc_ctx* c, const void* energy, const double* weight, int nw, void* out,
                                      void* stream) {
+    if (c && c->prec32) return AFQMC_UNSUPPORTED;      // the block calls are FP64-only (boundary32.cu)
     if (!c || !energy || !weight || !out || nw < 0) return AFQMC_INVALID_ARGUMENT;
     mixed_estimator_kernel<<<1, 32, 0, (cudaStream_t)stream>>>(nw, (const double2*)energy, weight, (double2*)out);
     AFQMC_LAUNCH_CHECK(c);
@@ -436,6 +440,7 @@ static int orthogonalize_i(afqmc_ctx* c, double2* phi, int nw, double* logdet_r,
 }
 
 AFQMC_API int afqmc_orthogonalize(afqmc_ctx* c, void* phi, int nw, double* logdet_r, int* info, void* stream) {
+    if (c && c->prec32) return AFQMC_UNSUPPORTED;      // the block calls are FP64-only (boundary32.cu)
     if (!c || !phi || nw < 0 || nw > c->max_walkers) return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
     return orthogonalize_i(c, (double2*)phi, nw, logdet_r, info, 0, (cudaStream_t)stream);
@@ -455,6 +460,7 @@ __global__ void info_merge_kernel(int nw, int first, const int* __restrict__ ste
 
 AFQMC_API int afqmc_block(afqmc_ctx* c, void* phi, double* weight, const double* x, double dtau, int order, int nsteps,
                            int nw, void* energy, void* emixed, double* logdet_r, int* info, void* stream) {
+    if (c && c->prec32) return AFQMC_UNSUPPORTED;      // the block calls are FP64-only (boundary32.cu)
     if (!c || !phi || !weight || !energy || !emixed || nw < 0 || nw > c->max_walkers || nsteps < 0 || order < 0 ||
         order > 32 || !(dtau >= 0.0) || (nsteps > 0 && !x))
         return AFQMC_INVALID_ARGUMENT;

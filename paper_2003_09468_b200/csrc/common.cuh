@@ -73,6 +73,8 @@ struct afqmc_ctx {
     double* ws_ldr;     // [2][nw] log det R of the two Cholesky-QR passes
     int* ws_info2;      // [2][nw] status of the two Cholesky passes
     int b1_set;
+    int prec32;         // 1 = complex64 boundary (afqmc_dims.precision = 1, boundary32.cu)
+    float* ws_f32;      // precision 1: device staging of afqmc_step_host ([nw][M][N][2] + x + energy + logdet floats)
     long long launches;
     int opt_exchange_depth; // 0/3 = three k-steps of fragment prefetch, 2 = two
     int opt_fb_tile;        // tuning aid: warp tile of the force-bias kernel for > 16 walkers (0: 4x4, 1: 4x8, 2: 2x8 m x n tiles)
@@ -170,6 +172,19 @@ int afqmc_i_pack_lxt(afqmc_ctx* c, const double2* L, cudaStream_t st);
 size_t afqmc_i_lxt_floats(const Dims& d);
 size_t afqmc_i_lx3_doubles(const Dims& d);
 int afqmc_i_apply_onebody(afqmc_ctx* c, double2* phi, int nw, cudaStream_t st);
+int afqmc_i_step(afqmc_ctx* c, double2* phi, const double* x, double dtau, int order, int nw, double2* energy,
+                 double2* logdet, int* info, cudaStream_t st);
+// complex64 boundary (boundary32.cu): same calls on float arrays, staged through the FP64 workspace
+int afqmc32_widen_alloc(afqmc_ctx* c, const void* in, size_t ndoubles, double** out, cudaStream_t st);
+int afqmc32_green(afqmc_ctx* c, const void* phi, int nw, void* theta, void* logdet, int* info, cudaStream_t st);
+int afqmc32_force_bias(afqmc_ctx* c, const void* theta, int nw, void* vbias, cudaStream_t st);
+int afqmc32_vhs(afqmc_ctx* c, const void* x, const void* vbias, double dtau, int nw, void* vhs, cudaStream_t st);
+int afqmc32_propagate(afqmc_ctx* c, const void* vhs, double dtau, int order, void* phi, int nw, cudaStream_t st);
+int afqmc32_local_energy(afqmc_ctx* c, const void* theta, int nw, void* energy, cudaStream_t st);
+int afqmc32_step(afqmc_ctx* c, void* phi, const void* x, double dtau, int order, int nw, void* energy, void* logdet,
+                 int* info, cudaStream_t st);
+int afqmc32_step_host(afqmc_ctx* c, void* phi_host, const void* x_host, double dtau, int order, int nw, void* energy_host,
+                      void* logdet_host, int* info_host, cudaStream_t st);
 size_t afqmc_i_taylor_ws_doubles(const Dims& d);
 size_t afqmc_i_vhs_field_doubles(const Dims& d, int nw);   // doubles of the expanded field operand (workspace ws_xi)   // per-walker doubles of one expanded Taylor buffer
 // records stage event i on st when timers are on

@@ -138,7 +138,7 @@ AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lx, c->Lx3, c->LxT, c->Lf, c->Lv3, c->vunits,
                     c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T, c->ws_Tx,
                     c->ws_expart, c->ws_fbpart, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
-                    c->b1, c->ws_b1tmp, c->ws_gram, c->ws_rinv, c->ws_logdet2, c->ws_ldr, c->ws_info2};
+                    c->ws_f32, c->b1, c->ws_b1tmp, c->ws_gram, c->ws_rinv, c->ws_logdet2, c->ws_ldr, c->ws_info2};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     for (cudaEvent_t e : c->ev)
@@ -160,7 +160,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     long long nk_ll = (long long)dims->g[0] * dims->g[1] * dims->g[2];
     if (nk_ll > AFQMC_MAX_NK) return AFQMC_INVALID_ARGUMENT;
     if (dims->closed_shell != 1) return AFQMC_UNSUPPORTED;
-    if (dims->precision != 0) return AFQMC_UNSUPPORTED;
+    if (dims->precision != 0 && dims->precision != 1) return AFQMC_UNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
 
     afqmc_ctx* c = new afqmc_ctx();
@@ -176,6 +176,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     d.GT2 = (d.nchol + 15) / 16;
     d.PRT = (d.m * d.m + 7) / 8;
     c->max_walkers = dims->max_walkers;
+    c->prec32 = dims->precision == 1 ? 1 : 0;
     c->opt_fb_pf = 8;
     c->opt_exchange_3m = 1;
     const int nw = c->max_walkers;
@@ -250,7 +251,17 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     A(dev_alloc(&c->ws_logdet2, (size_t)nw));
     A(dev_alloc(&c->ws_ldr, (size_t)2 * nw));
     A(dev_alloc(&c->ws_info2, (size_t)2 * nw));
+    if (c->prec32) A(dev_alloc(&c->ws_f32, (size_t)nw * ((size_t)d.M * d.N * 2 + (size_t)Nk * d.nchol + 8)));
     if (rc != AFQMC_OK) { afqmc_destroy(c); return rc; }
+    // complex64 boundary: the static inputs are widened once into FP64 temporaries (freed before returning)
+    double *h1w = nullptr, *Lw = nullptr, *psiw = nullptr;
+    if (c->prec32) {
+        A(afqmc32_widen_alloc(c, h1, (size_t)Nk * d.m * d.m * 2, &h1w, st));
+        A(afqmc32_widen_alloc(c, L, (size_t)Nk * Nk * d.nchol * d.m * d.m * 2, &Lw, st));
+        A(afqmc32_widen_alloc(c, psi_t, (size_t)Nk * d.m * d.n * 2, &psiw, st));
+        if (rc != AFQMC_OK) { cudaFree(h1w); cudaFree(Lw); cudaFree(psiw); afqmc_destroy(c); return rc; }
+        h1 = h1w; L = Lw; psi_t = psiw;
+    }
 
     auto H2D = [&](void* dst, const void* src, size_t bytes) {
         if (rc == AFQMC_OK && cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
@@ -279,7 +290,9 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     }
     // host vectors must outlive the async copies; the caller may free its arrays after return
     if (cudaStreamSynchronize(st) != cudaSuccess && rc == AFQMC_OK) rc = AFQMC_CUDA_ERROR;
+    cudaFree(h1w); cudaFree(Lw); cudaFree(psiw);
     if (rc != AFQMC_OK) { (void)cudaGetLastError(); afqmc_destroy(c); return rc; }
+    if (c->prec32 && c->LxT) c->opt_exchange_prec = 1;      // complex64 boundary: 3xTF32 exchange by default
     *out = c;
     return AFQMC_OK;
 }

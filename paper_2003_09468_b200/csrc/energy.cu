@@ -347,5 +347,6 @@ int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* en
 AFQMC_API int afqmc_local_energy(afqmc_ctx* c, const void* theta, int nw, void* energy, void* stream) {
     if (!c || !theta || !energy || nw < 0 || nw > c->max_walkers) return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
+    if (c->prec32) return afqmc32_local_energy(c, theta, nw, energy, (cudaStream_t)stream);
     return afqmc_i_local_energy(c, (const double2*)theta, nw, (double2*)energy, (cudaStream_t)stream);
 }

@@ -238,5 +238,6 @@ int afqmc_i_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbia
 AFQMC_API int afqmc_force_bias(afqmc_ctx* c, const void* theta, int nw, void* vbias, void* stream) {
     if (!c || !theta || !vbias || nw < 0 || nw > c->max_walkers) return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
+    if (c->prec32) return afqmc32_force_bias(c, theta, nw, vbias, (cudaStream_t)stream);
     return afqmc_i_force_bias(c, (const double2*)theta, nw, (double2*)vbias, (cudaStream_t)stream);
 }

@@ -2,13 +2,8 @@
 // PAPER.md:87-107/:142-160 on phi, then the energy evaluation of PAPER.md:306-319 on the new phi.
 #include "common.cuh"
 
-AFQMC_API int afqmc_step(afqmc_ctx* c, void* phi, const double* x, double dtau, int order, int nw,
-                          void* energy, void* logdet, int* info, void* stream) {
-    if (!c || !phi || !x || !energy || nw < 0 || nw > c->max_walkers || order < 0 || order > 32 || !(dtau >= 0.0))
-        return AFQMC_INVALID_ARGUMENT;
-    if (nw == 0) return AFQMC_OK;
-    cudaStream_t st = (cudaStream_t)stream;
-    double2* ph = (double2*)phi;
+int afqmc_i_step(afqmc_ctx* c, double2* ph, const double* x, double dtau, int order, int nw, double2* energy,
+                 double2* logdet, int* info, cudaStream_t st) {
     int rc;
     afqmc_mark(c, 0, st);
     if ((rc = afqmc_i_green(c, ph, nw, c->ws_theta, nullptr, nullptr, st)) != AFQMC_OK) return rc;
@@ -19,12 +14,21 @@ AFQMC_API int afqmc_step(afqmc_ctx* c, void* phi, const double* x, double dtau, 
     afqmc_mark(c, 3, st);
     if ((rc = afqmc_i_propagate(c, c->ws_vhs, dtau, order, ph, nw, st)) != AFQMC_OK) return rc;
     afqmc_mark(c, 4, st);
-    if ((rc = afqmc_i_green(c, ph, nw, c->ws_theta, (double2*)logdet, info, st)) != AFQMC_OK) return rc;
+    if ((rc = afqmc_i_green(c, ph, nw, c->ws_theta, logdet, info, st)) != AFQMC_OK) return rc;
     afqmc_mark(c, 5, st);
-    if ((rc = afqmc_i_local_energy(c, c->ws_theta, nw, (double2*)energy, st)) != AFQMC_OK) return rc;
+    if ((rc = afqmc_i_local_energy(c, c->ws_theta, nw, energy, st)) != AFQMC_OK) return rc;
     afqmc_mark(c, 8, st);      // marks 6 and 7 are recorded around the exchange kernel inside local_energy
     if (c->opt_timers) c->ev_valid = 1;
     return AFQMC_OK;
+}
+
+AFQMC_API int afqmc_step(afqmc_ctx* c, void* phi, const double* x, double dtau, int order, int nw,
+                          void* energy, void* logdet, int* info, void* stream) {
+    if (!c || !phi || !x || !energy || nw < 0 || nw > c->max_walkers || order < 0 || order > 32 || !(dtau >= 0.0))
+        return AFQMC_INVALID_ARGUMENT;
+    if (nw == 0) return AFQMC_OK;
+    if (c->prec32) return afqmc32_step(c, phi, x, dtau, order, nw, energy, logdet, info, (cudaStream_t)stream);
+    return afqmc_i_step(c, (double2*)phi, x, dtau, order, nw, (double2*)energy, (double2*)logdet, info, (cudaStream_t)stream);
 }
 
 AFQMC_API int afqmc_step_host(afqmc_ctx* c, void* phi_host, const double* x_host, double dtau, int order,
@@ -33,6 +37,7 @@ AFQMC_API int afqmc_step_host(afqmc_ctx* c, void* phi_host, const double* x_host
         return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
     cudaStream_t st = (cudaStream_t)stream;
+    if (c->prec32) return afqmc32_step_host(c, phi_host, x_host, dtau, order, nw, energy_host, logdet_host, info_host, st);
     const Dims& d = c->d;
     const size_t phi_bytes = (size_t)nw * d.M * d.N * sizeof(double2);
     const size_t x_bytes = (size_t)nw * d.Nk * d.nchol * sizeof(double);

@@ -387,5 +387,6 @@ AFQMC_API int afqmc_vhs(afqmc_ctx* c, const double* x, const void* vbias, double
                          void* stream) {
     if (!c || !x || !vhs || nw < 0 || nw > c->max_walkers || !(dtau >= 0.0)) return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
+    if (c->prec32) return afqmc32_vhs(c, x, vbias, dtau, nw, vhs, (cudaStream_t)stream);
     return afqmc_i_vhs(c, x, (const double2*)vbias, dtau, nw, (double2*)vhs, (cudaStream_t)stream);
 }
