@@ -275,7 +275,7 @@ def test_argument_errors(small_case):
     h = ctypes.c_void_p(0)
     d = binding.Dims((ctypes.c_int * 3)(2, 2, 1), 6, 4, 10, 0, 0, 4)       # open shell
     assert lib.afqmc_create(ctypes.byref(h), ctypes.byref(d), phi_d.data_ptr(), phi_d.data_ptr(), phi_d.data_ptr(), None) == 2
-    d = binding.Dims((ctypes.c_int * 3)(2, 2, 1), 6, 4, 10, 1, 1, 4)       # complex64 not built yet
+    d = binding.Dims((ctypes.c_int * 3)(2, 2, 1), 6, 4, 10, 1, 2, 4)       # precision: only 0 (complex128) and 1 (complex64) exist
     assert lib.afqmc_create(ctypes.byref(h), ctypes.byref(d), phi_d.data_ptr(), phi_d.data_ptr(), phi_d.data_ptr(), None) == 2
     d = binding.Dims((ctypes.c_int * 3)(2, 2, 1), 6, 7, 10, 1, 0, 4)       # n > m
     assert lib.afqmc_create(ctypes.byref(h), ctypes.byref(d), phi_d.data_ptr(), phi_d.data_ptr(), phi_d.data_ptr(), None) == 1
