@@ -238,7 +238,7 @@ double afqmc_exchange_flops(const afqmc_ctx* ctx, int nw);
  *   (else AFQMC_UNSUPPORTED):  1 = "3xTF32": operands split into TF32 high + low parts, three MMAs per product, FP32
  *   accumulation per task, FP64 sums: EX agrees with FP64 to ~1e-6 relative (tolerance 1e-4);  2 = "1xTF32": operands
  *   rounded once to TF32, fastest, EX error 2e-5 typical / 2e-3 worst measured: outside the 1e-4 tolerance);
- * "exchange_3m" (1 = default: three real products per complex product when n <= 4, 0 = the 4M kernel);
+ * "exchange_3m" (1 = default: three real products per complex product, 0 = the 4M kernel);
  * "timers" (1 = afqmc_step records a CUDA event after each stage, see afqmc_stage_times). */
 int afqmc_set_option(afqmc_ctx* ctx, const char* name, int value);
 

@@ -225,7 +225,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     A(dev_alloc(&c->psi_t, (size_t)Nk * d.m * d.n));
     A(dev_alloc(&c->ht, (size_t)Nk * d.n * d.m));
     A(dev_alloc(&c->Lx, nLx));
-    if (d.NAG == 1) A(dev_alloc(&c->Lx3, afqmc_i_lx3_doubles(d)));
+    A(dev_alloc(&c->Lx3, afqmc_i_lx3_doubles(d)));
     if (d.NAG == 1) A(dev_alloc(&c->LxT, afqmc_i_lxt_floats(d)));
     A(dev_alloc(&c->Lf, nLf));
     A(dev_alloc(&c->ws_O, (size_t)nw * d.N * LD));

@@ -19,8 +19,9 @@
 // pipeline is 3 deep and unrolled by 3, so buffer q always belongs to product q (static register indexing).
 // At the end of a task the products are combined and contracted in registers.  The partner tile is computed with
 // the DMMA operands swapped (theta as A, Lh as B: the two fragment lane layouts coincide), which yields it already
-// transposed in (a,b); one shuffle per value (lane bits 4 and 1 exchanged) then aligns gamma and walker.  Only n <= 4 (one a-group) is handled here; larger n uses
-// the 4M kernel.
+// transposed in (a,b); one shuffle per value (lane bits 4 and 1 exchanged) then aligns gamma and walker.  n <= 4 (one
+// a-group) uses the tuned kernel below; larger n the multi-group variant after it (falls back to the 4M kernel only if
+// the theta blocks of all a-groups do not fit shared memory).
 #include "common.cuh"
 
 namespace {
@@ -263,6 +264,186 @@ __global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_kernel(
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// The same kernel for MORE THAN FOUR occupied orbitals per k-point (NAG = ceil(n/4) > 1 a-groups).  The (ag, bg)
+// pairs of a-groups are processed one after the other; inside a pair everything is as above (linear A streams of the
+// rows ag of Lh[Q][k] and bg of Lh[-Q][k2], B fragments of the theta rows bg of k2 and ag of k).  The theta blocks of
+// ALL groups are staged once per CTA: Bs[which][grp][ms][j][lane].
+// ---------------------------------------------------------------------------------------------------------------
+template <int NP, int WPC, int MINB>
+__global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_multi_kernel(
+    Dims d, int KS3, int nw, const int* __restrict__ units, const int* __restrict__ kminus, const int* __restrict__ kplus,
+    const int* __restrict__ kneg, const double* __restrict__ Lx3, const double2* __restrict__ theta,
+    double2* __restrict__ partial) {
+    extern __shared__ __align__(16) double ex3_smem[];
+    constexpr int NWC = 2 * NP;
+    const int nwg = (nw + NWC - 1) / NWC;
+    const int u = blockIdx.x / nwg, w0 = (blockIdx.x % nwg) * NWC;
+    const int Q = units[4 * u], k = units[4 * u + 1], k2 = units[4 * u + 2];
+    const int mQ = kneg[Q];
+    const int kq = kminus[k * d.Nk + Q];
+    const int k2pq = kplus[k2 * d.Nk + Q];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int GQ = d.GQ, NAG = d.NAG, MS = 3 * KS3;
+    constexpr int bs_step = NP * 32;
+    const int bs_grp = MS * bs_step, bs_half = NAG * bs_grp;
+    const size_t task_doubles = (size_t)MS * 64;
+
+    // ---- stage the B fragments of every a-group: one thread per complex theta element (orbital, walker, r) ----
+    {
+        const int per_which = NAG * 4 * NWC * 4 * KS3;
+        for (int e = tid; e < 2 * per_which; e += 32 * WPC) {
+            const int which = e / per_which;
+            int x = e - which * per_which;
+            const int b = x & 3; x >>= 2;
+            const int wl = x % NWC; x /= NWC;
+            const int grp = x % NAG, r = x / NAG;                // r < 4*KS3
+            const int orb = 4 * grp + b, w = w0 + wl;
+            const int rowblk = which == 0 ? k2 : k, colblk = which == 0 ? kq : k2pq;
+            double2 v = make_double2(0.0, 0.0);
+            if (orb < d.n && w < nw && r < d.m)
+                v = __ldg(theta + ((size_t)w * d.N + rowblk * d.n + orb) * d.M + (size_t)colblk * d.m + r);
+            double* dst = ex3_smem + which * bs_half + grp * bs_grp + ((3 * (r >> 2)) * NP + (wl >> 1)) * 32 +
+                          (((wl & 1) * 4 + b) << 2) + (r & 3);
+            dst[0] = v.x;
+            dst[bs_step] = v.y - v.x;
+            dst[2 * bs_step] = v.x + v.y;
+        }
+    }
+    __syncthreads();
+
+    const int t_begin = (int)((long long)warp * GQ / WPC), t_end = (int)((long long)(warp + 1) * GQ / WPC);
+    const int total = (t_end - t_begin) * MS;
+    const int srcl = (lane & ~0x12) | ((lane & 16) >> 3) | ((lane & 2) << 3);
+    double er[NP], ei[NP];
+#pragma unroll
+    for (int j = 0; j < NP; ++j) er[j] = ei[j] = 0.0;
+
+    for (int ab = 0; ab < NAG * NAG; ++ab) {
+        const int ag = ab / NAG, bg = ab % NAG;
+        const double2* la1 = reinterpret_cast<const double2*>(Lx3 + ((((size_t)Q * d.Nk + k) * NAG + ag) * GQ + t_begin) * task_doubles) + lane;
+        const double2* la2 = reinterpret_cast<const double2*>(Lx3 + ((((size_t)mQ * d.Nk + k2) * NAG + bg) * GQ + t_begin) * task_doubles) + lane;
+        const double* lb1 = ex3_smem + bg * bs_grp + lane;                 // theta rows bg of k2
+        const double* lb2 = ex3_smem + bs_half + ag * bs_grp + lane;       // theta rows ag of k
+        int ls = 0;
+        auto loader_advance = [&]() {
+            const bool wrap = ++ls == MS;
+            const int db = wrap ? -(MS - 1) * bs_step : bs_step;
+            lb1 += db; lb2 += db;
+            ls = wrap ? 0 : ls;
+        };
+        double2 fa1[3], fa2[3];
+        double fb1[3][NP], fb2[3][NP];
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            fa1[q] = fa2[q] = make_double2(0.0, 0.0);
+            if (total > 0) { fa1[q] = __ldg(la1 + q * 32); fa2[q] = __ldg(la2 + q * 32); }
+#pragma unroll
+            for (int j = 0; j < NP; ++j) { fb1[q][j] = lb1[j * 32]; fb2[q][j] = lb2[j * 32]; }
+            loader_advance();
+        }
+        la1 += 96; la2 += 96;
+        double acc1[3][2][NP][2], acc2[3][2][NP][2];
+#pragma unroll
+        for (int p = 0; p < 3; ++p)
+#pragma unroll
+            for (int i = 0; i < 2; ++i)
+#pragma unroll
+                for (int j = 0; j < NP; ++j)
+                    acc1[p][i][j][0] = acc1[p][i][j][1] = acc2[p][i][j][0] = acc2[p][i][j][1] = 0.0;
+        int cs = 0;
+        auto mstep = [&](const int q) {
+#pragma unroll
+            for (int j = 0; j < NP; ++j) {
+                dmma884(acc1[q][0][j][0], acc1[q][0][j][1], fa1[q].x, fb1[q][j]);
+                dmma884(acc1[q][1][j][0], acc1[q][1][j][1], fa1[q].y, fb1[q][j]);
+            }
+#pragma unroll
+            for (int j = 0; j < NP; ++j) {
+                dmma884(acc2[q][0][j][0], acc2[q][0][j][1], fb2[q][j], fa2[q].x);
+                dmma884(acc2[q][1][j][0], acc2[q][1][j][1], fb2[q][j], fa2[q].y);
+            }
+            fa1[q] = __ldg(la1); fa2[q] = __ldg(la2);      // may run up to 3 micro-steps past this pair's last task
+            la1 += 32; la2 += 32;
+#pragma unroll
+            for (int j = 0; j < NP; ++j) { fb1[q][j] = lb1[j * 32]; fb2[q][j] = lb2[j * 32]; }
+            loader_advance();
+            if (q == 2) {
+                cs += 3;
+                if (cs == MS) {
+                    cs = 0;
+#pragma unroll
+                    for (int i = 0; i < 2; ++i)
+#pragma unroll
+                        for (int j = 0; j < NP; ++j) {
+                            double t1r[2], t1i[2], t2r[2], t2i[2];
+#pragma unroll
+                            for (int e = 0; e < 2; ++e) {
+                                t1r[e] = acc1[0][i][j][e] - acc1[2][i][j][e];
+                                t1i[e] = acc1[0][i][j][e] + acc1[1][i][j][e];
+                                t2r[e] = acc2[0][i][j][e] - acc2[2][i][j][e];
+                                t2i[e] = acc2[0][i][j][e] + acc2[1][i][j][e];
+                            }
+                            const double pr0 = __shfl_sync(0xffffffffu, t2r[0], srcl), pi0 = __shfl_sync(0xffffffffu, t2i[0], srcl);
+                            const double pr1 = __shfl_sync(0xffffffffu, t2r[1], srcl), pi1 = __shfl_sync(0xffffffffu, t2i[1], srcl);
+                            er[j] = fma(t1r[0], pr0, er[j]); er[j] = fma(-t1i[0], pi0, er[j]);
+                            ei[j] = fma(t1r[0], pi0, ei[j]); ei[j] = fma(t1i[0], pr0, ei[j]);
+                            er[j] = fma(t1r[1], pr1, er[j]); er[j] = fma(-t1i[1], pi1, er[j]);
+                            ei[j] = fma(t1r[1], pi1, ei[j]); ei[j] = fma(t1i[1], pr1, ei[j]);
+#pragma unroll
+                            for (int p = 0; p < 3; ++p)
+                                acc1[p][i][j][0] = acc1[p][i][j][1] = acc2[p][i][j][0] = acc2[p][i][j][1] = 0.0;
+                        }
+                }
+            }
+        };
+        for (int g0 = 0; g0 < total; g0 += 3) { mstep(0); mstep(1); mstep(2); }
+    }
+
+    __syncthreads();
+    double* red = ex3_smem;
+#pragma unroll
+    for (int j = 0; j < NP; ++j) {
+        double r = er[j], i = ei[j];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            if (o == 2) continue;
+            r += __shfl_xor_sync(0xffffffffu, r, o);
+            i += __shfl_xor_sync(0xffffffffu, i, o);
+        }
+        if (lane == 0 || lane == 2) {
+            const int wl = 2 * j + (lane >> 1);
+            red[(warp * NWC + wl) * 2] = r; red[(warp * NWC + wl) * 2 + 1] = i;
+        }
+    }
+    __syncthreads();
+    if (tid < NWC && w0 + tid < nw) {
+        double r = 0.0, i = 0.0;
+        for (int x = 0; x < WPC; ++x) { r += red[(x * NWC + tid) * 2]; i += red[(x * NWC + tid) * 2 + 1]; }
+        partial[(size_t)u * nw + w0 + tid] = make_double2(r, i);
+    }
+}
+
+template <int NP, int WPC, int MINB>
+int launch_exchange3m_multi(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+    const Dims& d = c->d;
+    const int KS3 = (d.m + 3) / 4;
+    size_t smem = (size_t)2 * d.NAG * 3 * KS3 * NP * 32 * sizeof(double);
+    if (smem < (size_t)WPC * 2 * NP * 2 * sizeof(double)) smem = (size_t)WPC * 2 * NP * 2 * sizeof(double);
+    if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
+    auto kern = exchange3m_multi_kernel<NP, WPC, MINB>;
+    static size_t attr_set = 0;
+    if (smem > 48 * 1024 && smem > attr_set) {
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return AFQMC_CUDA_ERROR;
+        attr_set = smem;
+    }
+    const long long nblocks = (long long)((nw + 2 * NP - 1) / (2 * NP)) * c->nunits;
+    if (nblocks > 0x7fffffffLL) return AFQMC_UNSUPPORTED;
+    kern<<<(unsigned)nblocks, 32 * WPC, smem, st>>>(d, KS3, nw, c->units, c->kminus, c->kplus, c->kneg, c->Lx3, theta, c->ws_expart);
+    AFQMC_LAUNCH_CHECK(c);
+    return AFQMC_OK;
+}
+
 template <int NP, int WPC, int MINB, int DA>
 int launch_exchange3m_cfg(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     const Dims& d = c->d;
@@ -286,10 +467,13 @@ int launch_exchange3m_cfg(afqmc_ctx* c, const double2* theta, int nw, cudaStream
 
 }  // namespace
 
-// Writes the unit partial sums into ws_expart like the 4M kernel.  Returns AFQMC_UNSUPPORTED for n > 4 (caller falls back).
+// Writes the unit partial sums into ws_expart like the 4M kernel.  Returns AFQMC_UNSUPPORTED (caller falls back to the 4M
+// kernel) only if the staged theta blocks do not fit shared memory.
 int afqmc_i_exchange3m(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     const Dims& d = c->d;
-    if (d.NAG != 1 || !c->Lx3) return AFQMC_UNSUPPORTED;
+    if (!c->Lx3) return AFQMC_UNSUPPORTED;
+    if (d.NAG != 1)      // more than four occupied orbitals per k-point
+        return nw >= 3 ? launch_exchange3m_multi<2, 2, 6>(c, theta, nw, st) : launch_exchange3m_multi<1, 2, 6>(c, theta, nw, st);
     const int wpc = c->opt_exchange_wpc == 4 ? 4 : 2;
     const bool deep = c->opt_exchange_depth == 6;
     if (nw >= 3) {

@@ -331,8 +331,9 @@ def test_vhs_without_the_pair_identity_falls_back_to_all_blocks(nw):
 
 
 @pytest.mark.parametrize("kw", [dict(mesh=(2, 2, 1), m=6, n=4, nchol=10, nw=4), dict(mesh=(2, 3, 1), m=5, n=3, nchol=7, nw=5),
-                                dict(mesh=(1, 2, 2), m=9, n=1, nchol=5, nw=2), dict(mesh=(3, 1, 1), m=26, n=4, nchol=18, nw=7)],
-                         ids=["n4", "n3_odd", "n1_two_walkers", "m26_seven_walkers"])
+                                dict(mesh=(1, 2, 2), m=9, n=1, nchol=5, nw=2), dict(mesh=(3, 1, 1), m=26, n=4, nchol=18, nw=7),
+                                dict(mesh=(2, 2, 1), m=9, n=6, nchol=11, nw=5), dict(mesh=(1, 1, 2), m=14, n=9, nchol=6, nw=2)],
+                         ids=["n4", "n3_odd", "n1_two_walkers", "m26_seven_walkers", "n6_two_groups", "n9_three_groups"])
 def test_exchange_3m_and_4m_kernels_against_the_oracle(kw):
     """Both exchange kernels (exchange3m.cu: default for n <= 4; energy.cu: option exchange_3m=0) on the same theta,
     each against the oracle, and against each other; the deep-prefetch variants of the 3M kernel too."""
