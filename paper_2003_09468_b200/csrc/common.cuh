@@ -37,6 +37,8 @@ struct afqmc_ctx {
     int* kneg;     // [Nk]           -> index of -Q
     int* units;    // exchange work units, int4-packed (Q,k,k2,mult) [nunits]
     int nunits;
+    int ex_parts;     // partial sums per exchange unit written by the last exchange launch (1, or NAG^2 * chunks: exchange3m.cu)
+    int ex_parts_max; // ... that ws_expart was sized for
     // static tensors
     double2* psi_t; // [Nk][m][n]
     double2* ht;    // [Nk][n][m]   half-rotated one-body

@@ -237,7 +237,13 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     A(dev_alloc(&c->ws_T, (size_t)2 * nw * d.M * d.N));
     const size_t nTx = (size_t)2 * nw * afqmc_i_taylor_ws_doubles(d);
     A(dev_alloc(&c->ws_Tx, nTx));
-    A(dev_alloc(&c->ws_expart, (size_t)c->nunits * nw));
+    {   // exchange partial sums: one per unit and walker, or NAG^2 * (up to 8 chunks) when the theta blocks of all a-groups
+        // do not fit one CTA's shared memory (large n*m per k-point: exchange3m_big_kernel)
+        const size_t multi_smem = (size_t)2 * d.NAG * 3 * ((d.m + 3) / 4) * 2 * 32 * sizeof(double);
+        c->ex_parts_max = (d.NAG > 1 && multi_smem > (size_t)c->smem_optin) ? d.NAG * d.NAG * 8 : 1;
+        c->ex_parts = 1;
+        A(dev_alloc(&c->ws_expart, (size_t)c->nunits * nw * c->ex_parts_max));
+    }
     A(dev_alloc(&c->ws_fbpart, (size_t)AFQMC_FB_MAXKC * nw * Nk * d.nchol));
     A(dev_alloc(&c->ws_x, (size_t)nw * Nk * d.nchol));
     A(dev_alloc(&c->ws_phi, (size_t)nw * d.M * d.N));

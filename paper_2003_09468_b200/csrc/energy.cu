@@ -220,7 +220,7 @@ __device__ double2 block_sum2(double2 v, double* scratch /* >= 64 doubles */) {
 }
 
 __global__ void __launch_bounds__(1024) energy_finalize_kernel(
-    Dims d, int nw, int nunits, const int* __restrict__ units, const int* __restrict__ kneg,
+    Dims d, int nw, int nunits, int parts, const int* __restrict__ units, const int* __restrict__ kneg,
     const double2* __restrict__ ht, const double2* __restrict__ theta, const double2* __restrict__ vbias,
     const double2* __restrict__ partial, double2* __restrict__ energy) {
     __shared__ double scratch[64];
@@ -241,9 +241,9 @@ __global__ void __launch_bounds__(1024) energy_finalize_kernel(
     ec = block_sum2(ec, scratch);
     // EX = - sum_units mult * X(unit)
     double2 ex = make_double2(0.0, 0.0);
-    for (int u = tid; u < nunits; u += blockDim.x) {
-        double mult = (double)units[4 * u + 3];
-        double2 p = partial[(size_t)u * nw + w];
+    for (int idx = tid; idx < nunits * parts; idx += blockDim.x) {     // `parts` partial sums per unit (1 except for large blocks)
+        double mult = (double)units[4 * (idx / parts) + 3];
+        double2 p = partial[(size_t)idx * nw + w];
         ex.x += mult * p.x; ex.y += mult * p.y;
     }
     ex = block_sum2(ex, scratch);
@@ -330,6 +330,7 @@ int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* en
     int rc = afqmc_i_force_bias(c, theta, nw, c->ws_vbias, st);     // steps 2(d): the traces are the force bias
     if (rc != AFQMC_OK) return rc;
     afqmc_mark(c, 6, st);
+    c->ex_parts = 1;
     rc = c->opt_exchange_prec != 0 ? afqmc_i_exchange_tf32(c, theta, nw, st)
          : c->opt_exchange_3m    ? afqmc_i_exchange3m(c, theta, nw, st) : AFQMC_UNSUPPORTED;
     if (rc == AFQMC_UNSUPPORTED) {          // n > 4, or the 4M kernel was asked for
@@ -338,7 +339,7 @@ int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* en
     }
     if (rc != AFQMC_OK) return rc;
     afqmc_mark(c, 7, st);
-    energy_finalize_kernel<<<nw, 1024, 0, st>>>(d, nw, c->nunits, c->units, c->kneg, c->ht, theta, c->ws_vbias,
+    energy_finalize_kernel<<<nw, 1024, 0, st>>>(d, nw, c->nunits, c->ex_parts, c->units, c->kneg, c->ht, theta, c->ws_vbias,
                                               c->ws_expart, energy);
     AFQMC_LAUNCH_CHECK(c);
     return AFQMC_OK;

@@ -424,6 +424,200 @@ __global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_multi_kernel(
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// The variant for LARGE blocks (the theta blocks of all a-groups of a unit do not fit shared memory: many occupied
+// orbitals and/or bands per k-point, e.g. the dense Gamma-point supercell shape of SURVEY.md 8(f) NEXT-4).  The pair
+// (ag, bg) of a-groups and a chunk of the gamma-quads move from loops inside the CTA into the grid: a CTA stages only
+// the theta rows of its two groups, and a unit contributes NAG^2 * nchunk partial sums (summed by the finalisation).
+// ---------------------------------------------------------------------------------------------------------------
+template <int NP, int WPC, int MINB>
+__global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_big_kernel(
+    Dims d, int KS3, int nchunk, int nw, const int* __restrict__ units, const int* __restrict__ kminus, const int* __restrict__ kplus,
+    const int* __restrict__ kneg, const double* __restrict__ Lx3, const double2* __restrict__ theta,
+    double2* __restrict__ partial) {
+    extern __shared__ __align__(16) double ex3_smem[];
+    constexpr int NWC = 2 * NP;
+    const int nwg = (nw + NWC - 1) / NWC;
+    const int npairs = d.NAG * d.NAG;
+    // blockIdx.x = ((u * nwg + walker group) * npairs + ab) * nchunk + chunk
+    int bx = blockIdx.x;
+    const int chunk = bx % nchunk; bx /= nchunk;
+    const int ab = bx % npairs; bx /= npairs;
+    const int w0 = (bx % nwg) * NWC, u = bx / nwg;
+    const int ag = ab / d.NAG, bg = ab % d.NAG;
+    const int Q = units[4 * u], k = units[4 * u + 1], k2 = units[4 * u + 2];
+    const int mQ = kneg[Q];
+    const int kq = kminus[k * d.Nk + Q];
+    const int k2pq = kplus[k2 * d.Nk + Q];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int GQ = d.GQ, NAG = d.NAG, MS = 3 * KS3;
+    (void)NAG;
+    constexpr int bs_step = NP * 32;
+    const int bs_half = MS * bs_step;
+    const size_t task_doubles = (size_t)MS * 64;
+
+    // ---- stage the B fragments of the two a-groups of this CTA: theta rows bg of k2 and rows ag of k ----
+    {
+        const int per_which = 4 * NWC * 4 * KS3;
+        for (int e = tid; e < 2 * per_which; e += 32 * WPC) {
+            const int which = e / per_which;
+            int x = e - which * per_which;
+            const int b = x & 3; x >>= 2;
+            const int wl = x % NWC, r = x / NWC;                 // r < 4*KS3
+            const int orb = 4 * (which == 0 ? bg : ag) + b, w = w0 + wl;
+            const int rowblk = which == 0 ? k2 : k, colblk = which == 0 ? kq : k2pq;
+            double2 v = make_double2(0.0, 0.0);
+            if (orb < d.n && w < nw && r < d.m)
+                v = __ldg(theta + ((size_t)w * d.N + rowblk * d.n + orb) * d.M + (size_t)colblk * d.m + r);
+            double* dst = ex3_smem + which * bs_half + ((3 * (r >> 2)) * NP + (wl >> 1)) * 32 + (((wl & 1) * 4 + b) << 2) + (r & 3);
+            dst[0] = v.x;
+            dst[bs_step] = v.y - v.x;
+            dst[2 * bs_step] = v.x + v.y;
+        }
+    }
+    __syncthreads();
+
+    const int q_begin = (int)((long long)chunk * GQ / nchunk), q_end = (int)((long long)(chunk + 1) * GQ / nchunk);
+    const int t_begin = q_begin + (int)((long long)warp * (q_end - q_begin) / WPC);
+    const int t_end = q_begin + (int)((long long)(warp + 1) * (q_end - q_begin) / WPC);
+    const int total = (t_end - t_begin) * MS;
+    const int srcl = (lane & ~0x12) | ((lane & 16) >> 3) | ((lane & 2) << 3);
+    double er[NP], ei[NP];
+#pragma unroll
+    for (int j = 0; j < NP; ++j) er[j] = ei[j] = 0.0;
+
+    {
+        const double2* la1 = reinterpret_cast<const double2*>(Lx3 + ((((size_t)Q * d.Nk + k) * NAG + ag) * GQ + t_begin) * task_doubles) + lane;
+        const double2* la2 = reinterpret_cast<const double2*>(Lx3 + ((((size_t)mQ * d.Nk + k2) * NAG + bg) * GQ + t_begin) * task_doubles) + lane;
+        const double* lb1 = ex3_smem + lane;                 // theta rows bg of k2
+        const double* lb2 = ex3_smem + bs_half + lane;       // theta rows ag of k
+        int ls = 0;
+        auto loader_advance = [&]() {
+            const bool wrap = ++ls == MS;
+            const int db = wrap ? -(MS - 1) * bs_step : bs_step;
+            lb1 += db; lb2 += db;
+            ls = wrap ? 0 : ls;
+        };
+        double2 fa1[3], fa2[3];
+        double fb1[3][NP], fb2[3][NP];
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            fa1[q] = fa2[q] = make_double2(0.0, 0.0);
+            if (total > 0) { fa1[q] = __ldg(la1 + q * 32); fa2[q] = __ldg(la2 + q * 32); }
+#pragma unroll
+            for (int j = 0; j < NP; ++j) { fb1[q][j] = lb1[j * 32]; fb2[q][j] = lb2[j * 32]; }
+            loader_advance();
+        }
+        la1 += 96; la2 += 96;
+        double acc1[3][2][NP][2], acc2[3][2][NP][2];
+#pragma unroll
+        for (int p = 0; p < 3; ++p)
+#pragma unroll
+            for (int i = 0; i < 2; ++i)
+#pragma unroll
+                for (int j = 0; j < NP; ++j)
+                    acc1[p][i][j][0] = acc1[p][i][j][1] = acc2[p][i][j][0] = acc2[p][i][j][1] = 0.0;
+        int cs = 0;
+        auto mstep = [&](const int q) {
+#pragma unroll
+            for (int j = 0; j < NP; ++j) {
+                dmma884(acc1[q][0][j][0], acc1[q][0][j][1], fa1[q].x, fb1[q][j]);
+                dmma884(acc1[q][1][j][0], acc1[q][1][j][1], fa1[q].y, fb1[q][j]);
+            }
+#pragma unroll
+            for (int j = 0; j < NP; ++j) {
+                dmma884(acc2[q][0][j][0], acc2[q][0][j][1], fb2[q][j], fa2[q].x);
+                dmma884(acc2[q][1][j][0], acc2[q][1][j][1], fb2[q][j], fa2[q].y);
+            }
+            fa1[q] = __ldg(la1); fa2[q] = __ldg(la2);      // may run up to 3 micro-steps past this pair's last task
+            la1 += 32; la2 += 32;
+#pragma unroll
+            for (int j = 0; j < NP; ++j) { fb1[q][j] = lb1[j * 32]; fb2[q][j] = lb2[j * 32]; }
+            loader_advance();
+            if (q == 2) {
+                cs += 3;
+                if (cs == MS) {
+                    cs = 0;
+#pragma unroll
+                    for (int i = 0; i < 2; ++i)
+#pragma unroll
+                        for (int j = 0; j < NP; ++j) {
+                            double t1r[2], t1i[2], t2r[2], t2i[2];
+#pragma unroll
+                            for (int e = 0; e < 2; ++e) {
+                                t1r[e] = acc1[0][i][j][e] - acc1[2][i][j][e];
+                                t1i[e] = acc1[0][i][j][e] + acc1[1][i][j][e];
+                                t2r[e] = acc2[0][i][j][e] - acc2[2][i][j][e];
+                                t2i[e] = acc2[0][i][j][e] + acc2[1][i][j][e];
+                            }
+                            const double pr0 = __shfl_sync(0xffffffffu, t2r[0], srcl), pi0 = __shfl_sync(0xffffffffu, t2i[0], srcl);
+                            const double pr1 = __shfl_sync(0xffffffffu, t2r[1], srcl), pi1 = __shfl_sync(0xffffffffu, t2i[1], srcl);
+                            er[j] = fma(t1r[0], pr0, er[j]); er[j] = fma(-t1i[0], pi0, er[j]);
+                            ei[j] = fma(t1r[0], pi0, ei[j]); ei[j] = fma(t1i[0], pr0, ei[j]);
+                            er[j] = fma(t1r[1], pr1, er[j]); er[j] = fma(-t1i[1], pi1, er[j]);
+                            ei[j] = fma(t1r[1], pi1, ei[j]); ei[j] = fma(t1i[1], pr1, ei[j]);
+#pragma unroll
+                            for (int p = 0; p < 3; ++p)
+                                acc1[p][i][j][0] = acc1[p][i][j][1] = acc2[p][i][j][0] = acc2[p][i][j][1] = 0.0;
+                        }
+                }
+            }
+        };
+        for (int g0 = 0; g0 < total; g0 += 3) { mstep(0); mstep(1); mstep(2); }
+    }
+
+    __syncthreads();
+    double* red = ex3_smem;
+#pragma unroll
+    for (int j = 0; j < NP; ++j) {
+        double r = er[j], i = ei[j];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            if (o == 2) continue;
+            r += __shfl_xor_sync(0xffffffffu, r, o);
+            i += __shfl_xor_sync(0xffffffffu, i, o);
+        }
+        if (lane == 0 || lane == 2) {
+            const int wl = 2 * j + (lane >> 1);
+            red[(warp * NWC + wl) * 2] = r; red[(warp * NWC + wl) * 2 + 1] = i;
+        }
+    }
+    __syncthreads();
+    if (tid < NWC && w0 + tid < nw) {
+        double r = 0.0, i = 0.0;
+        for (int x = 0; x < WPC; ++x) { r += red[(x * NWC + tid) * 2]; i += red[(x * NWC + tid) * 2 + 1]; }
+        partial[(((size_t)u * npairs + ab) * nchunk + chunk) * nw + w0 + tid] = make_double2(r, i);
+    }
+}
+
+template <int NP, int WPC>
+int launch_exchange3m_big(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+    const Dims& d = c->d;
+    const int KS3 = (d.m + 3) / 4;
+    size_t smem = (size_t)2 * 3 * KS3 * NP * 32 * sizeof(double);
+    if (smem < (size_t)WPC * 2 * NP * 2 * sizeof(double)) smem = (size_t)WPC * 2 * NP * 2 * sizeof(double);
+    if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
+    auto kern = exchange3m_big_kernel<NP, WPC, 1>;
+    static size_t attr_set = 0;
+    if (smem > 48 * 1024 && smem > attr_set) {
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return AFQMC_CUDA_ERROR;
+        attr_set = smem;
+    }
+    const int nwg = (nw + 2 * NP - 1) / (2 * NP), npairs = d.NAG * d.NAG;
+    // chunks of gamma-quads: enough CTAs for ~4 waves, every warp keeps at least 2 quads, at most ex_parts_max parts per unit
+    int nchunk = (int)((4LL * c->num_sms + (long long)c->nunits * nwg * npairs - 1) / ((long long)c->nunits * nwg * npairs));
+    if (nchunk > d.GQ / (2 * WPC)) nchunk = d.GQ / (2 * WPC);
+    if (nchunk * npairs > c->ex_parts_max) nchunk = c->ex_parts_max / npairs;
+    if (nchunk < 1) nchunk = 1;
+    if (npairs * nchunk > c->ex_parts_max) return AFQMC_UNSUPPORTED;
+    const long long nblocks = (long long)c->nunits * nwg * npairs * nchunk;
+    if (nblocks > 0x7fffffffLL) return AFQMC_UNSUPPORTED;
+    kern<<<(unsigned)nblocks, 32 * WPC, smem, st>>>(d, KS3, nchunk, nw, c->units, c->kminus, c->kplus, c->kneg, c->Lx3, theta, c->ws_expart);
+    AFQMC_LAUNCH_CHECK(c);
+    c->ex_parts = npairs * nchunk;
+    return AFQMC_OK;
+}
+
 template <int NP, int WPC, int MINB>
 int launch_exchange3m_multi(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     const Dims& d = c->d;
@@ -472,8 +666,15 @@ int launch_exchange3m_cfg(afqmc_ctx* c, const double2* theta, int nw, cudaStream
 int afqmc_i_exchange3m(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     const Dims& d = c->d;
     if (!c->Lx3) return AFQMC_UNSUPPORTED;
-    if (d.NAG != 1)      // more than four occupied orbitals per k-point
-        return nw >= 3 ? launch_exchange3m_multi<2, 2, 6>(c, theta, nw, st) : launch_exchange3m_multi<1, 2, 6>(c, theta, nw, st);
+    c->ex_parts = 1;
+    if (d.NAG != 1) {    // more than four occupied orbitals per k-point
+        int rc = nw >= 3 ? launch_exchange3m_multi<2, 2, 6>(c, theta, nw, st) : launch_exchange3m_multi<1, 2, 6>(c, theta, nw, st);
+        if (rc == AFQMC_UNSUPPORTED && c->ex_parts_max > 1) {       // blocks too large for one CTA's shared memory
+            rc = nw >= 3 ? launch_exchange3m_big<2, 8>(c, theta, nw, st) : AFQMC_UNSUPPORTED;
+            if (rc == AFQMC_UNSUPPORTED) rc = launch_exchange3m_big<1, 8>(c, theta, nw, st);
+        }
+        return rc;
+    }
     const int wpc = c->opt_exchange_wpc == 4 ? 4 : 2;
     const bool deep = c->opt_exchange_depth == 6;
     if (nw >= 3) {

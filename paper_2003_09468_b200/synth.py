@@ -57,6 +57,10 @@ CONFIGS = {
     "C3": Config("C3", (3, 3, 3), 26, 4, 200, 32),
     "C4": Config("C4", (3, 3, 3), 52, 4, 400, 16),
     "C5": Config("C5", (4, 4, 4), 26, 4, 200, 8),
+    # NOT a BASELINE.json config: the dense Gamma-point supercell shape of SURVEY.md 8(f) NEXT-4 (one k-point, large m and n:
+    # the 2x2x2 cell of C2 written as a single cell), which runs the same kernels at a very different
+    # tile shape (n = 32 occupied orbitals: eight a-groups in the exchange kernel, N = 32, M = 208).
+    "G1": Config("G1", (1, 1, 1), 208, 32, 1040, 16),
 }
 
 

@@ -166,6 +166,16 @@ def test_config_C2_sampled():
         case.close()
 
 
+def test_gamma_point_supercell_shape_sampled():
+    """SURVEY.md 8(f) NEXT-4: the dense Gamma-point representation = one k-point with large m and n (synth config G1);
+    its theta blocks do not fit one CTA's shared memory, so the exchange runs the large-block 3M kernel."""
+    case = Case(synth.CONFIGS["G1"])
+    try:
+        run_chain_and_compare(case, [0, 9])
+    finally:
+        case.close()
+
+
 def test_config_C3_headline_sampled():
     case = Case(synth.CONFIGS["C3"])
     try:
