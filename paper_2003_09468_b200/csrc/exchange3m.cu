@@ -445,6 +445,15 @@ __global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_big_kernel(
     const int ab = bx % npairs; bx /= npairs;
     const int w0 = (bx % nwg) * NWC, u = bx / nwg;
     const int ag = ab / d.NAG, bg = ab % d.NAG;
+    // A unit that is its own partner under (Q,k,k2) -> (-Q,k2,k) (multiplicity 1; every unit at the Gamma point) has
+    // T2 = T1, so the contributions of the pairs (ag,bg) and (bg,ag) are equal: compute ag <= bg only, twice for ag < bg.
+    const bool self_unit = units[4 * u + 3] == 1;
+    if (self_unit && ag > bg) {
+        if (threadIdx.x < 2 * NP && w0 + (int)threadIdx.x < nw)
+            partial[(((size_t)u * npairs + ab) * nchunk + chunk) * nw + w0 + threadIdx.x] = make_double2(0.0, 0.0);
+        return;
+    }
+    const double pair_weight = (self_unit && ag < bg) ? 2.0 : 1.0;
     const int Q = units[4 * u], k = units[4 * u + 1], k2 = units[4 * u + 2];
     const int mQ = kneg[Q];
     const int kq = kminus[k * d.Nk + Q];
@@ -586,7 +595,7 @@ __global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_big_kernel(
     if (tid < NWC && w0 + tid < nw) {
         double r = 0.0, i = 0.0;
         for (int x = 0; x < WPC; ++x) { r += red[(x * NWC + tid) * 2]; i += red[(x * NWC + tid) * 2 + 1]; }
-        partial[(((size_t)u * npairs + ab) * nchunk + chunk) * nw + w0 + tid] = make_double2(r, i);
+        partial[(((size_t)u * npairs + ab) * nchunk + chunk) * nw + w0 + tid] = make_double2(pair_weight * r, pair_weight * i);
     }
 }
 

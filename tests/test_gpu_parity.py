@@ -137,6 +137,8 @@ RAGGED = [
     dict(mesh=(2, 2, 2), m=6, n=4, nchol=16, nw=9),     # every Q self-inverse
     dict(mesh=(3, 1, 2), m=4, n=2, nchol=3, nw=2),
     dict(mesh=(3, 3, 1), m=9, n=6, nchol=21, nw=3),     # n=6: padded second a-group
+    dict(mesh=(2, 1, 1), m=104, n=10, nchol=6, nw=3),   # theta blocks too large for one CTA: large-block exchange kernel,
+                                                        # self-partner and paired units, padded third a-group
 ]
 
 
