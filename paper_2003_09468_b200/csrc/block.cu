@@ -106,11 +106,22 @@ __global__ void __launch_bounds__(OB_THREADS) onebody_kernel(Dims d, int CT, con
         Xs[r * CT + j] = X[(size_t)r * d.N + j];
     }
     __syncthreads();
-    for (int e = threadIdx.x; e < d.m * ct; e += OB_THREADS) {
-        const int p = e / ct, j = e % ct;
-        double2 s = make_double2(0.0, 0.0);
-        for (int r = 0; r < d.m; ++r) s = cfma(Bs[p * d.m + r], Xs[r * CT + j], s);
-        X[(size_t)p * d.N + j] = s;
+    // a thread computes 4 rows of one column: every element of the staged block feeds 4 complex FMAs per load
+    const int npg = (d.m + 3) / 4;
+    for (int e = threadIdx.x; e < npg * ct; e += OB_THREADS) {
+        const int pg = e / ct, j = e % ct;
+        const int p0 = 4 * pg;
+        double2 s[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) s[i] = make_double2(0.0, 0.0);
+        for (int r = 0; r < d.m; ++r) {
+            const double2 xv = Xs[r * CT + j];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) s[i] = cfma(Bs[min(p0 + i, d.m - 1) * d.m + r], xv, s[i]);
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            if (p0 + i < d.m) X[(size_t)(p0 + i) * d.N + j] = s[i];
     }
 }
 
