@@ -442,3 +442,36 @@ def test_green_large_N(mesh, n):
             assert phase_diff(ld[w].imag, ld_o.imag) < 1e-9
     finally:
         case.close()
+
+
+def test_gpu_step_against_the_stored_oracle_fixture():
+    """The GPU step on the tiny seeded system of tests/golden/tiny_step.txt (written by the oracle alone) reproduces the
+    stored values: a parity check that does not execute the oracle at test time."""
+    import importlib.util
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    stored = {}
+    for line in open(os.path.join(here, "tiny_step.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        name, re_, im_ = line.split()
+        stored[name] = complex(float(re_), float(im_))
+    case = Case(synth.tiny_config(**mg.CFG))
+    try:
+        cfg, pb, ctx = case.cfg, case.pb, case.ctx
+        phi_d, x_d = _to_dev(pb.phi), _to_dev(pb.x)
+        theta_d, ld0_d, _ = ctx.green(phi_d)
+        vb = ctx.force_bias(theta_d).cpu().numpy()
+        energy, logdet, info = ctx.step(phi_d, x_d, cfg.dtau, cfg.order)
+        e, ld1, ld0, phi_new = energy.cpu().numpy(), logdet.cpu().numpy(), ld0_d.cpu().numpy(), phi_d.cpu().numpy()
+        for w in range(cfg.nw):
+            got = {"vbias_sum[%d]" % w: complex(np.sum(vb[w])), "E1[%d]" % w: e[w, 0], "EC[%d]" % w: e[w, 1],
+                   "EX[%d]" % w: e[w, 2], "phi_new_sum[%d]" % w: complex(np.sum(phi_new[w]))}
+            for name, z in got.items():
+                assert abs(z - stored[name]) <= 1e-9 * max(1.0, abs(stored[name])), (name, z, stored[name])
+            for name, z in (("logdet0[%d]" % w, ld0[w]), ("logdet1[%d]" % w, ld1[w])):
+                assert abs(z.real - stored[name].real) < 1e-9 and phase_diff(z.imag, stored[name].imag) < 1e-9, name
+    finally:
+        case.close()

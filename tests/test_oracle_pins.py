@@ -441,3 +441,25 @@ def test_full_step_runs_and_is_consistent(tiny):
     assert phi2.shape == pb.phi.shape and e.shape == (cfg.nw, 3) and np.all(np.isfinite(e))
     th2, ld2, _ = orc.green(pb.psi_t, phi2[1])
     assert abs(ld2 - ld[1]) < 1e-12
+
+
+# ---------------------------------------------------------------- stored fixture (regression guard of the oracle)
+def test_oracle_reproduces_the_stored_tiny_step():
+    """tests/golden/tiny_step.txt was written by tests/golden/make_golden.py from the oracle alone; the oracle must keep
+    reproducing it (a deliberate change of the oracle's arithmetic regenerates the file and cites its reason)."""
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    stored = {}
+    for line in open(os.path.join(here, "tiny_step.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        name, re_, im_ = line.split()
+        stored[name] = complex(float(re_), float(im_))
+    rows = dict(mg.compute())
+    assert set(rows) == set(stored)
+    for name, z in rows.items():
+        assert abs(z - stored[name]) <= 1e-12 * max(1.0, abs(stored[name])), name
