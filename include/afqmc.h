@@ -179,7 +179,9 @@ int afqmc_step_host(afqmc_ctx* ctx, void* phi_host, const double* x_host, double
 int afqmc_set_onebody(afqmc_ctx* ctx, const void* h1p, double dtau, void* b1_out, void* stream);
 
 /* phi_w[(k,:), :] <- B1[k] phi_w[(k,:), :] for every walker and k-point, in place (Eq. 13).
- * AFQMC_INVALID_ARGUMENT if afqmc_set_onebody was never called.   phi: device [nw][M][N]. */
+ * AFQMC_INVALID_ARGUMENT if afqmc_set_onebody was never called.   phi: device [nw][M][N].
+ * B1[k] is staged in shared memory when it fits (m up to ~116); larger m (the Gamma-point supercell shape) runs one
+ * batched tensor-core GEMM per k-point through the context's Taylor workspace instead: same result, no size limit. */
 int afqmc_apply_onebody(afqmc_ctx* ctx, void* phi, int nw, void* stream);
 
 /*
@@ -189,6 +191,8 @@ int afqmc_apply_onebody(afqmc_ctx* ctx, void* phi, int nw, void* stream);
  *   log I_w  = 2 (logdet_new[w] - logdet_old[w]) + x.xbar - xbar.xbar/2      (closed shell: two spin channels)
  *   dtheta_w = Im 2 (logdet_new[w] - logdet_old[w]) wrapped to (-pi, pi]        (Eq. 19)
  *   weight[w] <- weight[w] * |I_w| * max(0, cos dtheta_w)                       (Eq. 18)
+ *   A walker whose weight is 0 stays at 0, and a walker whose log det is not finite (singular overlap: logdet is
+ *   undefined when info != 0) or whose factor overflows is KILLED (weight 0): no NaN or 0*inf reaches the weights.
  *   x [nw][Nk][nchol] double, vbias [nw][Nk][nchol] complex, logdet_old/new [nw] complex (afqmc_overlap of the
  *   walker before / after the propagation), weight [nw] double in/out, log_i [nw] complex out or NULL: device.
  */
@@ -206,7 +210,9 @@ int afqmc_orthogonalize(afqmc_ctx* ctx, void* phi, int nw, double* logdet_r, int
 
 /*
  * Mixed estimator, Eq. 35:  out[0..2] = sum_w weight[w] * energy[w][0..2],  out[3] = sum_w weight[w]
- * (E_mixed = (out[0]+out[1]+out[2]) / out[3]), summed in walker order (deterministic).
+ * (E_mixed = (out[0]+out[1]+out[2]) / out[3]), summed in walker order (deterministic).  Walkers with weight 0
+ * (killed by the phaseless projection) and walkers whose local energy is not finite are left out of all four sums,
+ * so one dead walker cannot turn the block estimate into NaN.
  *   energy [nw][3] complex, weight [nw] double, out [4] complex: device.
  */
 int afqmc_mixed_estimator(afqmc_ctx* ctx, const void* energy, const double* weight, int nw, void* out, void* stream);
@@ -219,6 +225,7 @@ int afqmc_mixed_estimator(afqmc_ctx* ctx, const void* energy, const double* weig
  *   phi [nw][M][N] in/out; weight [nw] double in/out; x [nsteps][nw][Nk][nchol] double;
  *   energy [nw][3], emixed [4] complex out; logdet_r [nw] double out or NULL; info [nw] int32 out or NULL
  *   (first non-zero of: singular overlap at any step, non positive definite Gram matrix): device.
+ *   A walker with a singular overlap at some step gets weight 0 there and stays dead (it is still propagated).
  * Needs afqmc_set_onebody.
  */
 int afqmc_block(afqmc_ctx* ctx, void* phi, double* weight, const double* x, double dtau, int order, int nsteps,

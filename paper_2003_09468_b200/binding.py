@@ -127,9 +127,13 @@ class Afqmc:
             if not t.is_cuda or tuple(t.shape) != shape:
                 raise ValueError("%s must be a CUDA tensor of shape %s" % (name, shape))
         self.device = h1.device
+        for t in (L, psi_t):
+            if t.device != self.device:
+                raise ValueError("h1, L and psi_t must live on the same CUDA device")
         h = ctypes.c_void_p(0)
-        code = lib().afqmc_create(ctypes.byref(h), ctypes.byref(d), _ptr(h1, self.cdtype),
-                                  _ptr(L, self.cdtype), _ptr(psi_t, self.cdtype), _stream())
+        with torch.cuda.device(self.device):       # the library allocates its workspace on the CURRENT device
+            code = lib().afqmc_create(ctypes.byref(h), ctypes.byref(d), _ptr(h1, self.cdtype),
+                                      _ptr(L, self.cdtype), _ptr(psi_t, self.cdtype), _stream())
         _check(code, "afqmc_create")
         self._h = h
 
@@ -147,6 +151,41 @@ class Afqmc:
     # ---- helpers -------------------------------------------------------------------------
     def _empty(self, shape, dtype=None):
         return torch.empty(shape, dtype=self.cdtype if dtype is None else dtype, device=self.device)
+
+    def _nw(self, t, name):
+        """Batch size of a per-walker tensor; the library would read past `max_walkers` worth of workspace otherwise."""
+        nw = int(t.shape[0])
+        if nw > self.max_walkers:
+            raise ValueError("%s: %d walkers > max_walkers = %d" % (name, nw, self.max_walkers))
+        return nw
+
+    def _dev(self, t, shape, dtype, name, optional=False):
+        """Marshals one DEVICE tensor: exact shape, dtype, contiguity and device are checked here, because past this
+        point the tensor is a raw pointer (a wrong shape would be a silent out-of-bounds access in a kernel)."""
+        if t is None:
+            if optional:
+                return ctypes.c_void_p(0)
+            raise ValueError("%s is required" % name)
+        if not t.is_cuda or t.device != self.device:
+            raise ValueError("%s must be a CUDA tensor on %s (got %s)" % (name, self.device, t.device))
+        if tuple(t.shape) != tuple(shape):
+            raise ValueError("%s must have shape %s (got %s)" % (name, tuple(shape), tuple(t.shape)))
+        return _ptr(t, dtype)
+
+    def _host(self, t, shape, dtype, name, optional=False):
+        if t is None:
+            if optional:
+                return ctypes.c_void_p(0)
+            raise ValueError("%s is required" % name)
+        if t.is_cuda:
+            raise ValueError("%s must be a host tensor" % name)
+        if tuple(t.shape) != tuple(shape):
+            raise ValueError("%s must have shape %s (got %s)" % (name, tuple(shape), tuple(t.shape)))
+        return _ptr(t, dtype)
+
+    def _call(self, fn, *args):
+        with torch.cuda.device(self.device):
+            return fn(self._h, *args, _stream())
 
     def launch_count(self) -> int:
         return int(lib().afqmc_launch_count(self._h))
@@ -167,121 +206,132 @@ class Afqmc:
 
     # ---- the six step calls ----------------------------------------------------------------
     def overlap(self, phi, logdet=None, info=None):
-        nw = phi.shape[0]
+        nw = self._nw(phi, "phi")
         logdet = self._empty((nw,)) if logdet is None else logdet
         info = self._empty((nw,), torch.int32) if info is None else info
-        _check(lib().afqmc_overlap(self._h, _ptr(phi, self.cdtype), nw, _ptr(logdet), _ptr(info, torch.int32),
-                                   _stream()), "afqmc_overlap")
+        _check(self._call(lib().afqmc_overlap, self._dev(phi, (nw, self.M, self.N), self.cdtype, "phi"), nw,
+                          self._dev(logdet, (nw,), self.cdtype, "logdet"), self._dev(info, (nw,), torch.int32, "info")),
+               "afqmc_overlap")
         return logdet, info
 
     def green(self, phi, theta=None, logdet=None, info=None):
-        nw = phi.shape[0]
+        nw = self._nw(phi, "phi")
         theta = self._empty((nw, self.N, self.M)) if theta is None else theta
         logdet = self._empty((nw,)) if logdet is None else logdet
         info = self._empty((nw,), torch.int32) if info is None else info
-        _check(lib().afqmc_green(self._h, _ptr(phi, self.cdtype), nw, _ptr(theta, self.cdtype),
-                                 _ptr(logdet), _ptr(info, torch.int32), _stream()), "afqmc_green")
+        _check(self._call(lib().afqmc_green, self._dev(phi, (nw, self.M, self.N), self.cdtype, "phi"), nw,
+                          self._dev(theta, (nw, self.N, self.M), self.cdtype, "theta"),
+                          self._dev(logdet, (nw,), self.cdtype, "logdet"), self._dev(info, (nw,), torch.int32, "info")),
+               "afqmc_green")
         return theta, logdet, info
 
     def force_bias(self, theta, vbias=None):
-        nw = theta.shape[0]
+        nw = self._nw(theta, "theta")
         vbias = self._empty((nw, self.nk, self.nchol)) if vbias is None else vbias
-        _check(lib().afqmc_force_bias(self._h, _ptr(theta, self.cdtype), nw, _ptr(vbias, self.cdtype),
-                                      _stream()), "afqmc_force_bias")
+        _check(self._call(lib().afqmc_force_bias, self._dev(theta, (nw, self.N, self.M), self.cdtype, "theta"), nw,
+                          self._dev(vbias, (nw, self.nk, self.nchol), self.cdtype, "vbias")), "afqmc_force_bias")
         return vbias
 
     def vhs(self, x, vbias, dtau, vhs=None):
-        nw = x.shape[0]
+        nw = self._nw(x, "x")
         vhs = self._empty((nw, self.M, self.M)) if vhs is None else vhs
-        _check(lib().afqmc_vhs(self._h, _ptr(x, self.rdtype), _ptr(vbias, self.cdtype, optional=True),
-                               float(dtau), nw, _ptr(vhs, self.cdtype), _stream()), "afqmc_vhs")
+        _check(self._call(lib().afqmc_vhs, self._dev(x, (nw, self.nk, self.nchol), self.rdtype, "x"),
+                          self._dev(vbias, (nw, self.nk, self.nchol), self.cdtype, "vbias", optional=True),
+                          float(dtau), nw, self._dev(vhs, (nw, self.M, self.M), self.cdtype, "vhs")), "afqmc_vhs")
         return vhs
 
     def propagate(self, vhs, dtau, order, phi):
-        nw = phi.shape[0]
-        _check(lib().afqmc_propagate(self._h, _ptr(vhs, self.cdtype), float(dtau), int(order),
-                                     _ptr(phi, self.cdtype), nw, _stream()), "afqmc_propagate")
+        nw = self._nw(phi, "phi")
+        _check(self._call(lib().afqmc_propagate, self._dev(vhs, (nw, self.M, self.M), self.cdtype, "vhs"), float(dtau),
+                          int(order), self._dev(phi, (nw, self.M, self.N), self.cdtype, "phi"), nw), "afqmc_propagate")
         return phi
 
     def local_energy(self, theta, energy=None):
-        nw = theta.shape[0]
+        nw = self._nw(theta, "theta")
         energy = self._empty((nw, 3)) if energy is None else energy
-        _check(lib().afqmc_local_energy(self._h, _ptr(theta, self.cdtype), nw, _ptr(energy, self.cdtype),
-                                        _stream()), "afqmc_local_energy")
+        _check(self._call(lib().afqmc_local_energy, self._dev(theta, (nw, self.N, self.M), self.cdtype, "theta"), nw,
+                          self._dev(energy, (nw, 3), self.cdtype, "energy")), "afqmc_local_energy")
         return energy
 
     # ---- the whole step ------------------------------------------------------------------------
     def step(self, phi, x, dtau, order, energy=None, logdet=None, info=None):
-        nw = phi.shape[0]
+        nw = self._nw(phi, "phi")
         energy = self._empty((nw, 3)) if energy is None else energy
         logdet = self._empty((nw,)) if logdet is None else logdet
         info = self._empty((nw,), torch.int32) if info is None else info
-        _check(lib().afqmc_step(self._h, _ptr(phi, self.cdtype), _ptr(x, self.rdtype), float(dtau), int(order),
-                                nw, _ptr(energy), _ptr(logdet), _ptr(info, torch.int32), _stream()), "afqmc_step")
+        _check(self._call(lib().afqmc_step, self._dev(phi, (nw, self.M, self.N), self.cdtype, "phi"),
+                          self._dev(x, (nw, self.nk, self.nchol), self.rdtype, "x"), float(dtau), int(order), nw,
+                          self._dev(energy, (nw, 3), self.cdtype, "energy"), self._dev(logdet, (nw,), self.cdtype, "logdet"),
+                          self._dev(info, (nw,), torch.int32, "info")), "afqmc_step")
         return energy, logdet, info
 
     def step_host(self, phi_host, x_host, dtau, order, energy_host, logdet_host=None, info_host=None):
         """Host (ideally pinned) tensors in and out; H2D/D2H copies happen inside the call."""
-        nw = phi_host.shape[0]
-        for t in (phi_host, x_host, energy_host):
-            if t.is_cuda:
-                raise ValueError("step_host takes host tensors")
-        _check(lib().afqmc_step_host(self._h, _ptr(phi_host, self.cdtype), _ptr(x_host, self.rdtype),
-                                     float(dtau), int(order), nw, _ptr(energy_host, self.cdtype),
-                                     _ptr(logdet_host, optional=True), _ptr(info_host, optional=True), _stream()),
-               "afqmc_step_host")
+        nw = self._nw(phi_host, "phi_host")
+        _check(self._call(lib().afqmc_step_host, self._host(phi_host, (nw, self.M, self.N), self.cdtype, "phi_host"),
+                          self._host(x_host, (nw, self.nk, self.nchol), self.rdtype, "x_host"), float(dtau), int(order), nw,
+                          self._host(energy_host, (nw, 3), self.cdtype, "energy_host"),
+                          self._host(logdet_host, (nw,), self.cdtype, "logdet_host", optional=True),
+                          self._host(info_host, (nw,), torch.int32, "info_host", optional=True)), "afqmc_step_host")
         return energy_host
-
 
     # ---- the AFQMC block (include/afqmc.h "The AFQMC block") ----------------------------------------
     def set_onebody(self, h1p, dtau, b1_out=None):
         """B1[k] = exp(-dtau/2 h1p[k]) computed on the device and kept in the context; returns a copy."""
-        if tuple(h1p.shape) != (self.nk, self.m, self.m):
-            raise ValueError("h1p must have shape (Nk, m, m)")
-        b1_out = self._empty((self.nk, self.m, self.m)) if b1_out is None else b1_out
-        _check(lib().afqmc_set_onebody(self._h, _ptr(h1p, torch.complex128), float(dtau), _ptr(b1_out, torch.complex128),
-                                       _stream()), "afqmc_set_onebody")
+        shp = (self.nk, self.m, self.m)
+        b1_out = self._empty(shp) if b1_out is None else b1_out
+        _check(self._call(lib().afqmc_set_onebody, self._dev(h1p, shp, torch.complex128, "h1p"), float(dtau),
+                          self._dev(b1_out, shp, torch.complex128, "b1_out")), "afqmc_set_onebody")
         return b1_out
 
     def apply_onebody(self, phi):
-        _check(lib().afqmc_apply_onebody(self._h, _ptr(phi, torch.complex128), phi.shape[0], _stream()),
+        nw = self._nw(phi, "phi")
+        _check(self._call(lib().afqmc_apply_onebody, self._dev(phi, (nw, self.M, self.N), torch.complex128, "phi"), nw),
                "afqmc_apply_onebody")
         return phi
 
     def hybrid_weight(self, x, vbias, dtau, logdet_old, logdet_new, weight, log_i=None):
-        nw = x.shape[0]
+        nw = self._nw(x, "x")
         log_i = self._empty((nw,)) if log_i is None else log_i
-        _check(lib().afqmc_hybrid_weight(self._h, _ptr(x, torch.float64), _ptr(vbias, torch.complex128), float(dtau),
-                                         _ptr(logdet_old, torch.complex128), _ptr(logdet_new, torch.complex128), nw,
-                                         _ptr(weight, torch.float64), _ptr(log_i, torch.complex128), _stream()),
+        fld = (nw, self.nk, self.nchol)
+        _check(self._call(lib().afqmc_hybrid_weight, self._dev(x, fld, torch.float64, "x"),
+                          self._dev(vbias, fld, torch.complex128, "vbias"), float(dtau),
+                          self._dev(logdet_old, (nw,), torch.complex128, "logdet_old"),
+                          self._dev(logdet_new, (nw,), torch.complex128, "logdet_new"), nw,
+                          self._dev(weight, (nw,), torch.float64, "weight"), self._dev(log_i, (nw,), torch.complex128, "log_i")),
                "afqmc_hybrid_weight")
         return weight, log_i
 
     def orthogonalize(self, phi, logdet_r=None, info=None):
-        nw = phi.shape[0]
+        nw = self._nw(phi, "phi")
         logdet_r = self._empty((nw,), torch.float64) if logdet_r is None else logdet_r
         info = self._empty((nw,), torch.int32) if info is None else info
-        _check(lib().afqmc_orthogonalize(self._h, _ptr(phi, torch.complex128), nw, _ptr(logdet_r, torch.float64),
-                                         _ptr(info, torch.int32), _stream()), "afqmc_orthogonalize")
+        _check(self._call(lib().afqmc_orthogonalize, self._dev(phi, (nw, self.M, self.N), torch.complex128, "phi"), nw,
+                          self._dev(logdet_r, (nw,), torch.float64, "logdet_r"), self._dev(info, (nw,), torch.int32, "info")),
+               "afqmc_orthogonalize")
         return phi, logdet_r, info
 
     def mixed_estimator(self, energy, weight, out=None):
+        nw = int(energy.shape[0])
         out = self._empty((4,)) if out is None else out
-        _check(lib().afqmc_mixed_estimator(self._h, _ptr(energy, torch.complex128), _ptr(weight, torch.float64),
-                                           energy.shape[0], _ptr(out, torch.complex128), _stream()), "afqmc_mixed_estimator")
+        _check(self._call(lib().afqmc_mixed_estimator, self._dev(energy, (nw, 3), torch.complex128, "energy"),
+                          self._dev(weight, (nw,), torch.float64, "weight"), nw, self._dev(out, (4,), torch.complex128, "out")),
+               "afqmc_mixed_estimator")
         return out
 
     def block(self, phi, weight, x, dtau, order, energy=None, emixed=None, logdet_r=None, info=None):
         """x [nsteps][nw][Nk][nchol]; phi and weight are updated in place."""
-        nsteps, nw = int(x.shape[0]), int(phi.shape[0])
+        nsteps, nw = int(x.shape[0]), self._nw(phi, "phi")
         energy = self._empty((nw, 3)) if energy is None else energy
         emixed = self._empty((4,)) if emixed is None else emixed
         logdet_r = self._empty((nw,), torch.float64) if logdet_r is None else logdet_r
         info = self._empty((nw,), torch.int32) if info is None else info
-        _check(lib().afqmc_block(self._h, _ptr(phi, torch.complex128), _ptr(weight, torch.float64),
-                                 _ptr(x, torch.float64), float(dtau), int(order), nsteps, nw,
-                                 _ptr(energy, torch.complex128), _ptr(emixed, torch.complex128),
-                                 _ptr(logdet_r, torch.float64), _ptr(info, torch.int32), _stream()), "afqmc_block")
+        _check(self._call(lib().afqmc_block, self._dev(phi, (nw, self.M, self.N), torch.complex128, "phi"),
+                          self._dev(weight, (nw,), torch.float64, "weight"),
+                          self._dev(x, (nsteps, nw, self.nk, self.nchol), torch.float64, "x"), float(dtau), int(order), nsteps, nw,
+                          self._dev(energy, (nw, 3), torch.complex128, "energy"), self._dev(emixed, (4,), torch.complex128, "emixed"),
+                          self._dev(logdet_r, (nw,), torch.float64, "logdet_r"), self._dev(info, (nw,), torch.int32, "info")),
+               "afqmc_block")
         return energy, emixed, logdet_r, info
 
 

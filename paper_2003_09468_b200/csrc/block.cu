@@ -134,16 +134,27 @@ int afqmc_i_apply_onebody(afqmc_ctx* c, double2* phi, int nw, cudaStream_t st) {
     int CT = d.N;
     const size_t budget = 96 * 1024;
     const size_t fixed = (size_t)d.m * d.m * sizeof(double2);
-    if (fixed + (size_t)d.m * 8 * sizeof(double2) > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
+    if (fixed + (size_t)d.m * 8 * sizeof(double2) > (size_t)c->smem_optin) {
+        // B1[k] does not fit one CTA's shared memory (m above ~116, e.g. the Gamma-point supercell shape): one batched DMMA
+        // GEMM per k-point, out of place into the Taylor workspace, then copied back
+        const size_t per = (size_t)d.M * d.N;
+        for (int k = 0; k < d.Nk; ++k) {
+            zg::Args a;
+            a.A = c->b1 + (size_t)k * d.m * d.m; a.strideA = 0; a.lda = d.m;
+            a.B = phi + (size_t)k * d.m * d.N; a.strideB = (long long)per; a.ldb = d.N;
+            a.C = c->ws_T + (size_t)k * d.m * d.N; a.strideC = (long long)per; a.ldc = d.N;
+            a.D = nullptr; a.strideD = 0; a.ldd = 0;
+            a.M = d.m; a.N = d.N; a.K = d.m; a.alpha = 1.0;
+            if (zg::launch<false>(c, a, nw, st) != cudaSuccess) return AFQMC_CUDA_ERROR;
+            c->launches++;
+        }
+        AFQMC_CUDA_TRY(cudaMemcpyAsync(phi, c->ws_T, (size_t)nw * per * sizeof(double2), cudaMemcpyDeviceToDevice, st));
+        return AFQMC_OK;
+    }
     while (CT > 8 && (fixed + (size_t)d.m * CT * sizeof(double2) > budget || (long long)nw * d.Nk * ceil_div(d.N, CT) < 2LL * c->num_sms))
         CT = (CT + 1) / 2;
     const size_t smem = fixed + (size_t)d.m * CT * sizeof(double2);
-    static size_t attr_set = 0;
-    if (smem > 48 * 1024 && smem > attr_set) {
-        if (cudaFuncSetAttribute(onebody_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return AFQMC_CUDA_ERROR;
-        attr_set = smem;
-    }
+    if (int rc = afqmc_smem_optin(c, (const void*)onebody_kernel, smem)) return rc;
     onebody_kernel<<<dim3(ceil_div(d.N, CT), d.Nk, nw), OB_THREADS, smem, st>>>(d, CT, c->b1, phi);
     AFQMC_LAUNCH_CHECK(c);
     return AFQMC_OK;
@@ -180,6 +191,7 @@ constexpr int HW_THREADS = 256;
 __global__ void __launch_bounds__(HW_THREADS) hybrid_weight_kernel(
     Dims d, const int* __restrict__ kneg, const double* __restrict__ x, const double2* __restrict__ vbias,
     double sqrt_dtau, const double2* __restrict__ ld_old, const double2* __restrict__ ld_new,
+    const int* __restrict__ info /* nullable: status of the two overlap factorisations */,
     double* __restrict__ weight, double2* __restrict__ log_i) {
     __shared__ double red[4][HW_THREADS];
     const int w = blockIdx.x;
@@ -225,7 +237,12 @@ __global__ void __launch_bounds__(HW_THREADS) hybrid_weight_kernel(
         dth -= pi;
         if (dth == -pi) dth = pi;
         const double c = cos(dth);
-        weight[w] *= exp(li_r) * (c > 0.0 ? c : 0.0);
+        // A walker that is already dead stays dead, and a walker whose overlap is singular or not finite (log det
+        // undefined, include/afqmc.h) is killed: 0 * inf or a NaN phase never reaches the weight.
+        const double w_old = weight[w];
+        const bool bad = (info && info[w] != 0) || !isfinite(lr_r) || !isfinite(lr_i) || !isfinite(li_r);
+        const double f = exp(li_r) * (c > 0.0 ? c : 0.0);
+        weight[w] = (w_old == 0.0 || bad || !isfinite(f)) ? 0.0 : w_old * f;
         if (log_i) log_i[w] = make_double2(li_r, li_i);
     }
 }
@@ -237,8 +254,13 @@ __global__ void mixed_estimator_kernel(int nw, const double2* __restrict__ energ
     if (c >= 4) return;
     double2 s = make_double2(0.0, 0.0);
     for (int w = 0; w < nw; ++w) {
-        if (c < 3) { s.x += weight[w] * energy[w * 3 + c].x; s.y += weight[w] * energy[w * 3 + c].y; }
-        else s.x += weight[w];
+        // dead walkers (weight 0) and walkers without a finite local energy do not enter either sum of Eq. 35
+        const double wt = weight[w];
+        bool ok = wt != 0.0 && isfinite(wt);
+        for (int q = 0; q < 3; ++q) ok = ok && isfinite(energy[w * 3 + q].x) && isfinite(energy[w * 3 + q].y);
+        if (!ok) continue;
+        if (c < 3) { s.x += wt * energy[w * 3 + c].x; s.y += wt * energy[w * 3 + c].y; }
+        else s.x += wt;
     }
     out[c] = s;
 }
@@ -246,8 +268,8 @@ __global__ void mixed_estimator_kernel(int nw, const double2* __restrict__ energ
 }  // namespace
 
 static int hybrid_weight_i(afqmc_ctx* c, const double* x, const double2* vbias, double dtau, const double2* ld_old,
-                           const double2* ld_new, int nw, double* weight, double2* log_i, cudaStream_t st) {
-    hybrid_weight_kernel<<<nw, HW_THREADS, 0, st>>>(c->d, c->kneg, x, vbias, sqrt(dtau), ld_old, ld_new, weight, log_i);
+                           const double2* ld_new, const int* info, int nw, double* weight, double2* log_i, cudaStream_t st) {
+    hybrid_weight_kernel<<<nw, HW_THREADS, 0, st>>>(c->d, c->kneg, x, vbias, sqrt(dtau), ld_old, ld_new, info, weight, log_i);
     AFQMC_LAUNCH_CHECK(c);
     return AFQMC_OK;
 }
@@ -258,7 +280,7 @@ AFQMC_API int afqmc_hybrid_weight(afqmc_ctx* c, const double* x, const void* vbi
     if (!c || !x || !vbias || !logdet_old || !logdet_new || !weight || nw < 0 || nw > c->max_walkers || !(dtau >= 0.0))
         return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
-    return hybrid_weight_i(c, x, (const double2*)vbias, dtau, (const double2*)logdet_old, (const double2*)logdet_new, nw,
+    return hybrid_weight_i(c, x, (const double2*)vbias, dtau, (const double2*)logdet_old, (const double2*)logdet_new, nullptr, nw,
                            weight, (double2*)log_i, (cudaStream_t)stream);
 }
 
@@ -420,12 +442,8 @@ static int orthogonalize_i(afqmc_ctx* c, double2* phi, int nw, double* logdet_r,
     const Dims& d = c->d;
     const size_t mat = (size_t)d.N * d.N * sizeof(double2);
     const int use_smem = mat + 1024 <= (size_t)c->smem_optin;
-    static size_t attr_set = 0;
-    if (use_smem && mat > 48 * 1024 && mat > attr_set) {
-        if (cudaFuncSetAttribute(cholesky_inverse_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mat) != cudaSuccess)
-            return AFQMC_CUDA_ERROR;
-        attr_set = mat;
-    }
+    if (use_smem)
+        if (int rc = afqmc_smem_optin(c, (const void*)cholesky_inverse_kernel, mat)) return rc;
     const size_t per = (size_t)d.M * d.N;
     for (int pass = 0; pass < 2; ++pass) {
         gram_kernel<<<dim3(ceil_div(d.N, GR_T), ceil_div(d.N, GR_T), nw), GR_THREADS, 0, st>>>(d.M, d.N, phi, c->ws_gram);
@@ -439,7 +457,7 @@ static int orthogonalize_i(afqmc_ctx* c, double2* phi, int nw, double* logdet_r,
         a.C = c->ws_T; a.strideC = (long long)per; a.ldc = d.N;
         a.D = nullptr; a.strideD = 0; a.ldd = 0;
         a.M = d.M; a.N = d.N; a.K = d.N; a.alpha = 1.0;
-        if (zg::launch<false>(a, nw, st) != cudaSuccess) return AFQMC_CUDA_ERROR;
+        if (zg::launch<false>(c, a, nw, st) != cudaSuccess) return AFQMC_CUDA_ERROR;
         c->launches++;
         AFQMC_CUDA_TRY(cudaMemcpyAsync(phi, c->ws_T, (size_t)nw * per * sizeof(double2), cudaMemcpyDeviceToDevice, st));
     }
@@ -501,7 +519,7 @@ AFQMC_API int afqmc_block(afqmc_ctx* c, void* phi, double* weight, const double*
         // overlap of the new walker = Green's function of the next step (or of the energy evaluation)
         if ((rc = afqmc_i_green(c, ph, nw, c->ws_theta, ld[(s + 1) & 1], c->ws_info, st)) != AFQMC_OK) return rc;
         if ((rc = merge(0)) != AFQMC_OK) return rc;
-        if ((rc = hybrid_weight_i(c, xs, c->ws_vbias, dtau, ld[s & 1], ld[(s + 1) & 1], nw, weight, nullptr, st)) != AFQMC_OK)
+        if ((rc = hybrid_weight_i(c, xs, c->ws_vbias, dtau, ld[s & 1], ld[(s + 1) & 1], c->ws_info, nw, weight, nullptr, st)) != AFQMC_OK)
             return rc;
     }
     if ((rc = afqmc_i_local_energy(c, c->ws_theta, nw, (double2*)energy, st)) != AFQMC_OK) return rc;

@@ -91,7 +91,7 @@ int afqmc32_step(afqmc_ctx* c, void* phi, const void* x, double dtau, int order,
     const Dims& d = c->d;
     TRY32(widen(c, phi, c->ws_phi, (size_t)nw * d.M * d.N * 2, st));
     TRY32(widen(c, x, c->ws_x, (size_t)nw * d.Nk * d.nchol, st));
-    TRY32(afqmc_i_step(c, c->ws_phi, c->ws_x, dtau, order, nw, c->ws_energy, logdet ? c->ws_logdet : nullptr, info, st));
+    TRY32(afqmc_i_step(c, c->ws_phi, c->ws_x, dtau, order, nw, c->ws_energy, logdet ? c->ws_logdet : nullptr, info, st, nullptr));
     TRY32(narrow(c, c->ws_phi, phi, (size_t)nw * d.M * d.N * 2, st));
     TRY32(narrow(c, c->ws_energy, energy, (size_t)nw * 3 * 2, st));
     if (logdet) TRY32(narrow(c, c->ws_logdet, logdet, (size_t)nw * 2, st));

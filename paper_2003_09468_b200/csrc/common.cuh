@@ -27,6 +27,11 @@ struct Dims {
     int PRT;       // octets of (p,r) pairs: ceil(m*m/8)         (vHS M-tiles)
 };
 
+// Kernel attributes that were set / queried for this context.  A function attribute belongs to the (function, device)
+// pair and a context lives on one device, so the record is per CONTEXT: nothing in the library is process-wide state.
+struct FuncAttr { const void* fn; int smem; int occ; };
+#define AFQMC_MAX_FATTR 128
+
 // The context.  All pointers are device memory owned by the context.
 struct afqmc_ctx {
     Dims d;
@@ -95,6 +100,9 @@ struct afqmc_ctx {
     cudaEvent_t ev_copy[2];
     cudaEvent_t ev[AFQMC_NUM_STAGES + 1];
     int ev_valid;
+    FuncAttr fattr[AFQMC_MAX_FATTR];   // see afqmc_smem_optin()
+    int nfattr;
+    int device;         // the CUDA device the context was created on
     int smem_optin;     // max dynamic shared memory per block (bytes)
     int smem_sm;        // shared memory per SM (bytes)
     int num_sms;
@@ -158,6 +166,34 @@ __device__ __forceinline__ double warp_sum(double v) {
 
 static inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 
+// Makes sure kernel `fn` may be launched with `smem` bytes of dynamic shared memory on the context's device.  The limit is
+// only ever RAISED (it is shared by every context on the device), and what was done is remembered in the context, not in
+// function-local statics: a second context on another device, or a context created after another one was destroyed,
+// opts in again.  Returns AFQMC_UNSUPPORTED if the device cannot give that much.
+static inline FuncAttr* afqmc_fattr(afqmc_ctx* c, const void* fn) {
+    for (int i = 0; i < c->nfattr; ++i)
+        if (c->fattr[i].fn == fn) return &c->fattr[i];
+    if (c->nfattr == AFQMC_MAX_FATTR) return nullptr;
+    FuncAttr* f = &c->fattr[c->nfattr++];
+    f->fn = fn; f->smem = 0; f->occ = -1;
+    return f;
+}
+static inline int afqmc_smem_optin(afqmc_ctx* c, const void* fn, size_t smem) {
+    if (smem <= 48 * 1024) return AFQMC_OK;
+    if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
+    FuncAttr* f = afqmc_fattr(c, fn);
+    if (f && (size_t)f->smem >= smem) return AFQMC_OK;
+    cudaFuncAttributes fa;
+    if (cudaFuncGetAttributes(&fa, fn) != cudaSuccess) { (void)cudaGetLastError(); return AFQMC_CUDA_ERROR; }
+    if ((size_t)fa.maxDynamicSharedSizeBytes < smem &&
+        cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return AFQMC_CUDA_ERROR;
+    }
+    if (f) { f->smem = (int)smem; f->occ = -1; }
+    return AFQMC_OK;
+}
+
 // internal entry points used across translation units (all asynchronous on `st`)
 int afqmc_i_green(afqmc_ctx* c, const double2* phi, int nw, double2* theta, double2* logdet,
                   int* info, cudaStream_t st);
@@ -175,7 +211,7 @@ size_t afqmc_i_lxt_floats(const Dims& d);
 size_t afqmc_i_lx3_doubles(const Dims& d);
 int afqmc_i_apply_onebody(afqmc_ctx* c, double2* phi, int nw, cudaStream_t st);
 int afqmc_i_step(afqmc_ctx* c, double2* phi, const double* x, double dtau, int order, int nw, double2* energy,
-                 double2* logdet, int* info, cudaStream_t st);
+                 double2* logdet, int* info, cudaStream_t st, cudaEvent_t phi_final /* nullable: recorded after the propagation */);
 // complex64 boundary (boundary32.cu): same calls on float arrays, staged through the FP64 workspace
 int afqmc32_widen_alloc(afqmc_ctx* c, const void* in, size_t ndoubles, double** out, cudaStream_t st);
 int afqmc32_green(afqmc_ctx* c, const void* phi, int nw, void* theta, void* logdet, int* info, cudaStream_t st);

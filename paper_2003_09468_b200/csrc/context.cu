@@ -183,6 +183,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
 
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { delete c; return AFQMC_CUDA_ERROR; }
+    c->device = dev;
     cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&c->smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);

@@ -260,13 +260,7 @@ int launch_exchange_cfg(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t
     size_t smem = (size_t)2 * d.NAG * d.KS * NT * 32 * sizeof(double);
     if (smem < (size_t)WPC * NT * 2 * sizeof(double)) smem = (size_t)WPC * NT * 2 * sizeof(double);
     auto kern = exchange_kernel<NT, WPC, D, LINEAR, MINB>;
-    static size_t attr_set = 0;
-    if (smem > 48 * 1024 && smem > attr_set) {
-        if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return AFQMC_CUDA_ERROR;
-        attr_set = smem;
-    }
+    if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
     const long long nblocks = (long long)((nw + NT - 1) / NT) * c->nunits;   // x only: y/z are capped at 65535
     if (nblocks > 0x7fffffffLL) return AFQMC_UNSUPPORTED;
     dim3 grid((unsigned)nblocks);

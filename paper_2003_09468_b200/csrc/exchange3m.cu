@@ -607,11 +607,7 @@ int launch_exchange3m_big(afqmc_ctx* c, const double2* theta, int nw, cudaStream
     if (smem < (size_t)WPC * 2 * NP * 2 * sizeof(double)) smem = (size_t)WPC * 2 * NP * 2 * sizeof(double);
     if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
     auto kern = exchange3m_big_kernel<NP, WPC, 1>;
-    static size_t attr_set = 0;
-    if (smem > 48 * 1024 && smem > attr_set) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return AFQMC_CUDA_ERROR;
-        attr_set = smem;
-    }
+    if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
     const int nwg = (nw + 2 * NP - 1) / (2 * NP), npairs = d.NAG * d.NAG;
     // chunks of gamma-quads: enough CTAs for ~4 waves, every warp keeps at least 2 quads, at most ex_parts_max parts per unit
     int nchunk = (int)((4LL * c->num_sms + (long long)c->nunits * nwg * npairs - 1) / ((long long)c->nunits * nwg * npairs));
@@ -635,11 +631,7 @@ int launch_exchange3m_multi(afqmc_ctx* c, const double2* theta, int nw, cudaStre
     if (smem < (size_t)WPC * 2 * NP * 2 * sizeof(double)) smem = (size_t)WPC * 2 * NP * 2 * sizeof(double);
     if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
     auto kern = exchange3m_multi_kernel<NP, WPC, MINB>;
-    static size_t attr_set = 0;
-    if (smem > 48 * 1024 && smem > attr_set) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return AFQMC_CUDA_ERROR;
-        attr_set = smem;
-    }
+    if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
     const long long nblocks = (long long)((nw + 2 * NP - 1) / (2 * NP)) * c->nunits;
     if (nblocks > 0x7fffffffLL) return AFQMC_UNSUPPORTED;
     kern<<<(unsigned)nblocks, 32 * WPC, smem, st>>>(d, KS3, nw, c->units, c->kminus, c->kplus, c->kneg, c->Lx3, theta, c->ws_expart);
@@ -654,13 +646,7 @@ int launch_exchange3m_cfg(afqmc_ctx* c, const double2* theta, int nw, cudaStream
     size_t smem = (size_t)2 * 3 * KS3 * NP * 32 * sizeof(double);
     if (smem < (size_t)WPC * 2 * NP * 2 * sizeof(double)) smem = (size_t)WPC * 2 * NP * 2 * sizeof(double);
     auto kern = exchange3m_kernel<NP, WPC, MINB, DA>;
-    static size_t attr_set = 0;
-    if (smem > 48 * 1024 && smem > attr_set) {
-        if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return AFQMC_CUDA_ERROR;
-        attr_set = smem;
-    }
+    if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
     const long long nblocks = (long long)((nw + 2 * NP - 1) / (2 * NP)) * c->nunits;
     if (nblocks > 0x7fffffffLL) return AFQMC_UNSUPPORTED;
     kern<<<(unsigned)nblocks, 32 * WPC, smem, st>>>(d, KS3, nw, c->units, c->kminus, c->kplus, c->kneg, c->Lx3, theta, c->ws_expart);

@@ -235,14 +235,8 @@ int afqmc_i_exchange_tf32(afqmc_ctx* c, const double2* theta, int nw, cudaStream
     const size_t plane = (size_t)d.Nk * d.Nk * d.GQ * KS8 * 128 + XT_PAD;
     size_t smem = (size_t)(split ? 4 : 2) * KS8 * XT_NT * 64 * sizeof(float);
     if (smem < (size_t)XT_WARPS * XT_NT * 2 * sizeof(double)) smem = (size_t)XT_WARPS * XT_NT * 2 * sizeof(double);
-    static size_t attr_set = 0;
-    if (smem > 48 * 1024 && smem > attr_set) {
-        if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
-        if (cudaFuncSetAttribute(exchange_tf32_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-            cudaFuncSetAttribute(exchange_tf32_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return AFQMC_CUDA_ERROR;
-        attr_set = smem;
-    }
+    if (int rc = afqmc_smem_optin(c, (const void*)exchange_tf32_kernel<true>, smem)) return rc;
+    if (int rc = afqmc_smem_optin(c, (const void*)exchange_tf32_kernel<false>, smem)) return rc;
     const long long nblocks = (long long)((nw + XT_NT - 1) / XT_NT) * c->nunits;
     if (nblocks > 0x7fffffffLL) return AFQMC_UNSUPPORTED;
     if (split)

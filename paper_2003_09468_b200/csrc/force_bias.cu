@@ -200,13 +200,7 @@ int launch_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias
     }
     const size_t smem = (size_t)(((d.Nk * d.n + 2) / 2 + 1) / 2 * 2 + (FB_WARPS / 2) * 2 * MP * NT * 64) * sizeof(double);
     auto kern = force_bias_kernel<MP, NT>;
-    static size_t attr_set = 0;
-    if (smem > 48 * 1024 && smem > attr_set) {
-        if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return AFQMC_CUDA_ERROR;
-        attr_set = smem;
-    }
+    if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
     kern<<<(unsigned)(base * KC), 32 * FB_WARPS, smem, st>>>(d, nw, KC, nmg, nwgrp, c->opt_fb_pf, c->kminus, c->Lf, theta,
                                                              KC > 1 ? c->ws_fbpart : vbias, KC > 1 ? 1 : 0);
     AFQMC_LAUNCH_CHECK(c);

@@ -429,12 +429,7 @@ int run_overlap_inverse(afqmc_ctx* c, const double2* phi, int nw, double2* oinvT
     size_t mat = (size_t)d.N * LD * sizeof(double2);
     int use_smem = (fixed + mat <= (size_t)c->smem_optin) ? 1 : 0;
     size_t smem = fixed + (use_smem ? mat : 0);
-    static size_t attr_set = 0;
-    if (smem > 48 * 1024 && smem > attr_set) {
-        if (cudaFuncSetAttribute(overlap_inverse_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return AFQMC_CUDA_ERROR;
-        attr_set = smem;
-    }
+    if (int rc = afqmc_smem_optin(c, (const void*)overlap_inverse_kernel, smem)) return rc;
     int threads = GJ_THREADS;
     if (d.N * d.N < 4096) threads = 256;
     overlap_inverse_kernel<<<nw, threads, smem, st>>>(d, LD, use_smem, c->psi_t, phi, c->ws_O, oinvT, logdet, info);
@@ -456,7 +451,7 @@ int afqmc_i_green(afqmc_ctx* c, const double2* phi, int nw, double2* theta, doub
     a.C = theta; a.strideC = (long long)d.N * d.M; a.ldc = d.M;
     a.D = nullptr; a.strideD = 0; a.ldd = 0;
     a.M = d.N; a.N = d.M; a.K = d.N; a.alpha = 1.0;
-    if (zg::launch<true>(a, nw, st) != cudaSuccess) return AFQMC_CUDA_ERROR;
+    if (zg::launch<true>(c, a, nw, st) != cudaSuccess) return AFQMC_CUDA_ERROR;
     c->launches++;
     return AFQMC_OK;
 }

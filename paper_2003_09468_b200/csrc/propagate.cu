@@ -26,12 +26,12 @@ int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, 
             a.C = T[j & 1]; a.strideC = (long long)per; a.ldc = d.N;
             a.D = phi; a.strideD = (long long)per; a.ldd = d.N;
             a.M = d.M; a.N = d.N; a.K = d.M; a.alpha = s / (double)j;
-            if (zg::launch<false>(a, nw, st) != cudaSuccess) return AFQMC_CUDA_ERROR;
+            if (zg::launch<false>(c, a, nw, st) != cudaSuccess) return AFQMC_CUDA_ERROR;
             c->launches++;
         }
         return AFQMC_OK;
     }
-    const int G = c->opt_taylor_groups > 0 ? c->opt_taylor_groups : tg::pick_groups(d.M, d.N, nw);
+    const int G = c->opt_taylor_groups > 0 ? c->opt_taylor_groups : tg::pick_groups(c, d.M, d.N, nw);
     const size_t perx = tg::expanded_doubles(d.M, d.N, G);
     if (perx > afqmc_i_taylor_ws_doubles(d)) return AFQMC_INVALID_ARGUMENT;   // a forced group count the workspace was not sized for
     double* Tx[2] = {c->ws_Tx, c->ws_Tx + (size_t)c->max_walkers * afqmc_i_taylor_ws_doubles(d)};
@@ -46,7 +46,7 @@ int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, 
         a.Ct = nullptr; a.strideCt = 0; a.ldct = 0;
         a.M = d.M; a.N = d.N; a.K = d.M; a.alpha = s / (double)j;
         a.wpc = c->opt_taylor_wpc;
-        if (tg::launch(a, nw, st, G) != cudaSuccess) return AFQMC_CUDA_ERROR;
+        if (tg::launch(c, a, nw, st, G) != cudaSuccess) return AFQMC_CUDA_ERROR;
         c->launches++;
     }
     return AFQMC_OK;

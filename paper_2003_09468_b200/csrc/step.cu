@@ -3,7 +3,7 @@
 #include "common.cuh"
 
 int afqmc_i_step(afqmc_ctx* c, double2* ph, const double* x, double dtau, int order, int nw, double2* energy,
-                 double2* logdet, int* info, cudaStream_t st) {
+                 double2* logdet, int* info, cudaStream_t st, cudaEvent_t phi_final) {
     int rc;
     afqmc_mark(c, 0, st);
     if ((rc = afqmc_i_green(c, ph, nw, c->ws_theta, nullptr, nullptr, st)) != AFQMC_OK) return rc;
@@ -14,6 +14,7 @@ int afqmc_i_step(afqmc_ctx* c, double2* ph, const double* x, double dtau, int or
     afqmc_mark(c, 3, st);
     if ((rc = afqmc_i_propagate(c, c->ws_vhs, dtau, order, ph, nw, st)) != AFQMC_OK) return rc;
     afqmc_mark(c, 4, st);
+    if (phi_final) AFQMC_CUDA_TRY(cudaEventRecord(phi_final, st));      // the propagated walkers are final from here on
     if ((rc = afqmc_i_green(c, ph, nw, c->ws_theta, logdet, info, st)) != AFQMC_OK) return rc;
     afqmc_mark(c, 5, st);
     if ((rc = afqmc_i_local_energy(c, c->ws_theta, nw, energy, st)) != AFQMC_OK) return rc;
@@ -28,7 +29,7 @@ AFQMC_API int afqmc_step(afqmc_ctx* c, void* phi, const double* x, double dtau, 
         return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
     if (c->prec32) return afqmc32_step(c, phi, x, dtau, order, nw, energy, logdet, info, (cudaStream_t)stream);
-    return afqmc_i_step(c, (double2*)phi, x, dtau, order, nw, (double2*)energy, (double2*)logdet, info, (cudaStream_t)stream);
+    return afqmc_i_step(c, (double2*)phi, x, dtau, order, nw, (double2*)energy, (double2*)logdet, info, (cudaStream_t)stream, nullptr);
 }
 
 AFQMC_API int afqmc_step_host(afqmc_ctx* c, void* phi_host, const double* x_host, double dtau, int order,
@@ -49,32 +50,25 @@ AFQMC_API int afqmc_step_host(afqmc_ctx* c, void* phi_host, const double* x_host
     }
     AFQMC_CUDA_TRY(cudaMemcpyAsync(c->ws_phi, phi_host, phi_bytes, cudaMemcpyHostToDevice, st));
     AFQMC_CUDA_TRY(cudaMemcpyAsync(c->ws_x, x_host, x_bytes, cudaMemcpyHostToDevice, st));
-    int rc;
-    // the same composition as afqmc_step (stage marks included)
-    afqmc_mark(c, 0, st);
-    if ((rc = afqmc_i_green(c, c->ws_phi, nw, c->ws_theta, nullptr, nullptr, st)) != AFQMC_OK) return rc;
-    afqmc_mark(c, 1, st);
-    if ((rc = afqmc_i_force_bias(c, c->ws_theta, nw, c->ws_vbias, st)) != AFQMC_OK) return rc;
-    afqmc_mark(c, 2, st);
-    if ((rc = afqmc_i_vhs(c, c->ws_x, c->ws_vbias, dtau, nw, c->ws_vhs, st)) != AFQMC_OK) return rc;
-    afqmc_mark(c, 3, st);
-    if ((rc = afqmc_i_propagate(c, c->ws_vhs, dtau, order, c->ws_phi, nw, st)) != AFQMC_OK) return rc;
-    afqmc_mark(c, 4, st);
-    AFQMC_CUDA_TRY(cudaEventRecord(c->ev_copy[0], st));                      // phi' is final here
-    AFQMC_CUDA_TRY(cudaStreamWaitEvent(c->copy_stream, c->ev_copy[0], 0));
-    AFQMC_CUDA_TRY(cudaMemcpyAsync(phi_host, c->ws_phi, phi_bytes, cudaMemcpyDeviceToHost, c->copy_stream));
-    AFQMC_CUDA_TRY(cudaEventRecord(c->ev_copy[1], c->copy_stream));
-    if ((rc = afqmc_i_green(c, c->ws_phi, nw, c->ws_theta, c->ws_logdet, c->ws_info, st)) != AFQMC_OK) return rc;
-    afqmc_mark(c, 5, st);
-    if ((rc = afqmc_i_local_energy(c, c->ws_theta, nw, c->ws_energy, st)) != AFQMC_OK) return rc;
-    afqmc_mark(c, 8, st);
-    if (c->opt_timers) c->ev_valid = 1;
-    AFQMC_CUDA_TRY(cudaMemcpyAsync(energy_host, c->ws_energy, (size_t)nw * 3 * sizeof(double2), cudaMemcpyDeviceToHost, st));
-    if (logdet_host)
-        AFQMC_CUDA_TRY(cudaMemcpyAsync(logdet_host, c->ws_logdet, (size_t)nw * sizeof(double2), cudaMemcpyDeviceToHost, st));
-    if (info_host)
-        AFQMC_CUDA_TRY(cudaMemcpyAsync(info_host, c->ws_info, (size_t)nw * sizeof(int), cudaMemcpyDeviceToHost, st));
-    AFQMC_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_copy[1], 0));               // the caller's stream owns the whole result
-    AFQMC_CUDA_TRY(cudaStreamSynchronize(st));
+    // the same composition as afqmc_step; ev_copy[0] is recorded when the propagated walkers are final, so that their
+    // download (second stream) runs while the energy of those walkers is evaluated
+    int rc = afqmc_i_step(c, c->ws_phi, c->ws_x, dtau, order, nw, c->ws_energy, c->ws_logdet, c->ws_info, st, c->ev_copy[0]);
+    if (rc != AFQMC_OK) {                          // nothing of this call may still be in flight when it returns
+        cudaStreamSynchronize(st);
+        (void)cudaGetLastError();
+        return rc;
+    }
+    cudaError_t e = cudaStreamWaitEvent(c->copy_stream, c->ev_copy[0], 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(phi_host, c->ws_phi, phi_bytes, cudaMemcpyDeviceToHost, c->copy_stream);
+    if (e == cudaSuccess) e = cudaEventRecord(c->ev_copy[1], c->copy_stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(energy_host, c->ws_energy, (size_t)nw * 3 * sizeof(double2), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && logdet_host)
+        e = cudaMemcpyAsync(logdet_host, c->ws_logdet, (size_t)nw * sizeof(double2), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && info_host)
+        e = cudaMemcpyAsync(info_host, c->ws_info, (size_t)nw * sizeof(int), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, c->ev_copy[1], 0);     // the caller's stream owns the whole result
+    // both streams are drained on every path: the caller's host buffers are never written after the call returns
+    cudaError_t e1 = cudaStreamSynchronize(c->copy_stream), e2 = cudaStreamSynchronize(st);
+    if (e != cudaSuccess || e1 != cudaSuccess || e2 != cudaSuccess) { (void)cudaGetLastError(); return AFQMC_CUDA_ERROR; }
     return AFQMC_OK;
 }

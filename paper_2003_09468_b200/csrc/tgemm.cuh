@@ -272,32 +272,26 @@ __global__ void __launch_bounds__(32 * WPC, 2) tgemm_kernel(Args p) {
 }
 
 template <int NTA, int D, int WPC>
-static inline cudaError_t launch_wpc(const Args& a, int batch, cudaStream_t st, int* occ_out) {
+static inline cudaError_t launch_wpc(afqmc_ctx* c, const Args& a, int batch, cudaStream_t st, int* occ_out) {
     auto kern = tgemm_kernel<NTA, D, WPC>;
     const int smem = STAGES * KC * 3 * NTA * 32 * 8 + 2 * STAGES * 8;
-    static int occ = -1;
-    if (occ < 0) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        int o = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kern, 32 * WPC, smem);
-        if (e != cudaSuccess) return e;
-        occ = o > 0 ? o : 1;
+    if (afqmc_smem_optin(c, (const void*)kern, smem) != AFQMC_OK) return cudaErrorInvalidValue;
+    if (occ_out) {      // query only: resident CTAs per SM, remembered in the context (per device)
+        FuncAttr* f = afqmc_fattr(c, (const void*)kern);
+        int occ = f ? f->occ : -1;
+        if (occ < 0) {
+            int o = 0;
+            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kern, 32 * WPC, smem);
+            if (e != cudaSuccess) return e;
+            occ = o > 0 ? o : 1;
+            if (f) f->occ = occ;
+        }
+        *occ_out = occ;
+        return cudaSuccess;
     }
-    if (occ_out) { *occ_out = occ; return cudaSuccess; }      // query only
     dim3 grid(a.G, (a.M + 16 * WPC - 1) / (16 * WPC), batch);
     kern<<<grid, 32 * WPC, smem, st>>>(a);
     return cudaGetLastError();
-}
-
-static inline int device_sms() {
-    static int sms = 0;
-    if (!sms) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
-            sms = 148;
-    }
-    return sms;
 }
 
 // Warps per CTA.  The DMMA pipe is per SM sub-partition, so resident warps must divide evenly over the four
@@ -305,13 +299,13 @@ static inline int device_sms() {
 // 3.35 ms, while 2 x 5 warps (1.95 waves instead of 2.38, but 3+3+2+2 warps per sub-partition) took 3.90 ms and 3
 // warps 4.39 ms.  4 is therefore the default; 3 and 5 stay selectable as a tuning aid (option "taylor_warps").
 template <int NTA, int D>
-static inline cudaError_t launch_cfg(const Args& a, int batch, cudaStream_t st) {
+static inline cudaError_t launch_cfg(afqmc_ctx* c, const Args& a, int batch, cudaStream_t st) {
     int best = 4;
     if (a.wpc >= 3 && a.wpc <= 5) best = a.wpc;
     switch (best) {
-        case 3: return launch_wpc<NTA, D, 3>(a, batch, st, nullptr);
-        case 5: return launch_wpc<NTA, D, 5>(a, batch, st, nullptr);
-        default: return launch_wpc<NTA, D, 4>(a, batch, st, nullptr);
+        case 3: return launch_wpc<NTA, D, 3>(c, a, batch, st, nullptr);
+        case 5: return launch_wpc<NTA, D, 5>(c, a, batch, st, nullptr);
+        default: return launch_wpc<NTA, D, 4>(c, a, batch, st, nullptr);
     }
 }
 
@@ -324,9 +318,9 @@ static inline cudaError_t launch_cfg(const Args& a, int batch, cudaStream_t st) 
     }
 
 // resident CTAs per SM of the 4-warp kernel instantiated for NTA tiles per group
-static inline cudaError_t query_occupancy(int NTA, int* occ) {
+static inline cudaError_t query_occupancy(afqmc_ctx* c, int NTA, int* occ) {
     Args a = {};
-#define TG_CALL(n) launch_wpc<n, DEPTH, 4>(a, 1, nullptr, occ)
+#define TG_CALL(n) launch_wpc<n, DEPTH, 4>(c, a, 1, nullptr, occ)
     TG_NTA_SWITCH(NTA, TG_CALL)
 #undef TG_CALL
 }
@@ -335,15 +329,15 @@ static inline cudaError_t query_occupancy(int NTA, int* occ) {
 // warp tiles (fewer accumulators, A re-read from L2 by more CTAs) but a finer grid: the cost model is
 //   rounds of resident CTAs x resident CTAs per SM x tiles a warp executes per k-step,
 // i.e. the DMMA time of one SM (the kernel is tensor-pipe bound), plus 2 % per extra group for the A re-reads.
-static inline int pick_groups(int M, int N, int batch) {
+static inline int pick_groups(afqmc_ctx* c, int M, int N, int batch) {
     const int gmin = make_groups(N).G;
-    const int sms = device_sms();
+    const int sms = c->num_sms;
     int best = gmin; long long best_cost = -1;
     for (int g = gmin; g < gmin + GROUP_CHOICES; ++g) {
         const Groups gr = make_groups(N, g);
         if (gr.G != g) break;
         int occ = 1;
-        if (query_occupancy(gr.NTA, &occ) != cudaSuccess) { (void)cudaGetLastError(); continue; }
+        if (query_occupancy(c, gr.NTA, &occ) != cudaSuccess) { (void)cudaGetLastError(); continue; }
         const long long ctas = (long long)gr.G * ((M + 63) / 64) * batch;
         const long long slots = (long long)occ * sms;
         const long long rounds = (ctas + slots - 1) / slots;
@@ -355,12 +349,12 @@ static inline int pick_groups(int M, int N, int batch) {
 
 // fills the group fields of `a` from N (and the group count G, 0 = fewest) and launches; `a.NPp`/`a.NPcp` are
 // derived from K and M.  The expanded operands must have been written with the same G.
-static inline cudaError_t launch(Args a, int batch, cudaStream_t st, int G = 0) {
+static inline cudaError_t launch(afqmc_ctx* c, Args a, int batch, cudaStream_t st, int G = 0) {
     const Groups gr = make_groups(a.N, G);
     a.G = gr.G; a.nt_base = gr.nt_base; a.nt_rem = gr.nt_rem;
     a.NPp = padded_pairs(a.K);
     a.NPcp = padded_pairs(a.M);
-#define TG_CALL(n) launch_cfg<n, DEPTH>(a, batch, st)
+#define TG_CALL(n) launch_cfg<n, DEPTH>(c, a, batch, st)
     TG_NTA_SWITCH(gr.NTA, TG_CALL)
 #undef TG_CALL
 }

@@ -343,12 +343,7 @@ int launch_vhs3(afqmc_ctx* c, int nw, int KS4, int KS4p, double2* vhs, cudaStrea
     const size_t smem = (size_t)V3_STAGES * 2 * D * 3 * NT * 32 * sizeof(double) + 2 * V3_STAGES * sizeof(uint64_t);
     const long long gx = (long long)c->nvunits * nsg;
     if (gx > 0x7fffffffLL || nwg > 65535) return AFQMC_UNSUPPORTED;
-    static bool attr_done = false;
-    if (!attr_done && smem > 48 * 1024) {
-        if (cudaFuncSetAttribute(vhs3_kernel<NT, MERGED, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return AFQMC_CUDA_ERROR;
-        attr_done = true;
-    }
+    if (int rc = afqmc_smem_optin(c, (const void*)vhs3_kernel<NT, MERGED, D>, smem)) return rc;
     vhs3_kernel<NT, MERGED, D><<<dim3((unsigned)gx, nwg), 32 * V3_WARPS, smem, st>>>(d, KS4, KS4p, nw, nwg, nsg, c->vunits, c->kminus, c->Lv3,
                                                                         reinterpret_cast<const double*>(c->ws_xi), vhs);
     AFQMC_LAUNCH_CHECK(c);

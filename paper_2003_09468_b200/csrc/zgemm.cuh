@@ -151,15 +151,10 @@ __global__ void __launch_bounds__(32 * WGM) zgemm_kernel(Args p) {
 }
 
 template <int WGM, int NT, bool B_KCONTIG>
-static inline cudaError_t launch_one(const Args& a, int batch, cudaStream_t st) {
+static inline cudaError_t launch_one(afqmc_ctx* c, const Args& a, int batch, cudaStream_t st) {
     using C_ = Cfg<WGM, NT>;
     auto kern = zgemm_kernel<WGM, NT, B_KCONTIG>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C_::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    if (afqmc_smem_optin(c, (const void*)kern, C_::SMEM_BYTES) != AFQMC_OK) return cudaErrorInvalidValue;
     dim3 grid((a.N + C_::BN - 1) / C_::BN, (a.M + C_::BM - 1) / C_::BM, batch);
     kern<<<grid, C_::NTHR, C_::SMEM_BYTES, st>>>(a);
     return cudaGetLastError();
@@ -167,7 +162,7 @@ static inline cudaError_t launch_one(const Args& a, int batch, cudaStream_t st) 
 
 // Picks the column-tile width (NT in {7,8,9} quads) that wastes the fewest padded columns.
 template <bool B_KCONTIG>
-static inline cudaError_t launch(const Args& a, int batch, cudaStream_t st) {
+static inline cudaError_t launch(afqmc_ctx* c, const Args& a, int batch, cudaStream_t st) {
     int best = 8;
     long long bestw = -1;
     for (int nt = 7; nt <= 9; ++nt) {
@@ -175,9 +170,9 @@ static inline cudaError_t launch(const Args& a, int batch, cudaStream_t st) {
         if (bestw < 0 || padded < bestw || (padded == bestw && nt > best)) { bestw = padded; best = nt; }
     }
     switch (best) {
-        case 7: return launch_one<4, 7, B_KCONTIG>(a, batch, st);
-        case 9: return launch_one<4, 9, B_KCONTIG>(a, batch, st);
-        default: return launch_one<4, 8, B_KCONTIG>(a, batch, st);
+        case 7: return launch_one<4, 7, B_KCONTIG>(c, a, batch, st);
+        case 9: return launch_one<4, 9, B_KCONTIG>(c, a, batch, st);
+        default: return launch_one<4, 8, B_KCONTIG>(c, a, batch, st);
     }
 }
 

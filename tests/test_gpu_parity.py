@@ -47,9 +47,54 @@ class Case:
         self.ctx.close()
 
 
-def run_chain_and_compare(case, sample, tol=RTOL, check_energy=True):
+_JOB = {}
+
+
+def _energy_job(w):
+    j = _JOB
+    return orc.local_energy(j["mesh"], j["Lh"], j["ht"], j["theta"][w])
+
+
+def oracle_energies(mesh, Lh, ht, theta, walkers):
+    """orc.local_energy for several walkers, one forked worker process per walker when there is more than one (the
+    oracle itself stays plain and single-threaded; the children run numpy only and never touch CUDA)."""
+    walkers = list(walkers)
+    _JOB.update(mesh=mesh, Lh=Lh, ht=ht, theta=theta)
+    try:
+        if len(walkers) > 1 and (os.cpu_count() or 1) > 1 and Lh.nbytes > (64 << 20):
+            import multiprocessing as mp
+            try:
+                with mp.get_context("fork").Pool(min(len(walkers), os.cpu_count())) as pool:
+                    return dict(zip(walkers, pool.map_async(_energy_job, walkers).get(timeout=900)))
+            except Exception as exc:           # noqa: BLE001 - fall back to the plain loop
+                print("oracle pool failed (%r): serial evaluation" % (exc,))
+        return {w: _energy_job(w) for w in walkers}
+    finally:
+        _JOB.clear()
+
+
+def cond_overlap(psi_t, phi_w):
+    """2-norm condition number of O = A^dagger Phi (numpy SVD; used only to DERIVE a tolerance, never as a reference value)."""
+    return float(np.linalg.cond(orc.overlap(psi_t, phi_w)))
+
+
+def theta2_bound(cond):
+    """Tolerance of quantities that pass through the inversion of the PROPAGATED walker's overlap O':
+    north_star's 1e-10, unless cond(O') is so large that a backward-stable inversion cannot reach it; then
+    100 * cond(O') * 2^-53 (elimination with partial pivoting: forward error <~ c(N) * cond * u, c(N) <~ 100 for
+    N <= 256).  On the synthetic walkers cond(O') is 1e1..1e4, so the bound is 1e-10 at every config (printed)."""
+    return max(RTOL, 100.0 * cond * 2.0 ** -53)
+
+
+def run_chain_and_compare(case, sample=None, tol=RTOL, energy_sample=None):
+    """Stages a1..a9 on ALL walkers of the case against the oracle; `sample` restricts the walkers (None = all) and
+    `energy_sample` the walkers whose local energy the oracle evaluates (the oracle's exchange recipe costs seconds
+    per walker at the full-size configs); every walker outside `energy_sample` has its energies cross-checked between
+    the two independent exchange kernels (3M, exchange3m.cu; 4M, energy.cu) at 1e-12."""
     cfg, pb, ctx = case.cfg, case.pb, case.ctx
     mesh = cfg.mesh
+    sample = list(range(case.nw)) if sample is None else list(sample)
+    energy_sample = sample if energy_sample is None else list(energy_sample)
     phi_d = _to_dev(pb.phi)
     x_d = _to_dev(pb.x)
 
@@ -98,20 +143,46 @@ def run_chain_and_compare(case, sample, tol=RTOL, check_energy=True):
     assert torch.equal(phi0_d, phi_d)                          # order 0 = identity
     del vhs_d
 
-    # a1-a3 on the propagated walker, then a7-a9
+    # a1-a3 on the propagated walker: held to north_star's 1e-10 unless cond(O') forbids it (derived, printed)
     theta2_d, logdet2_d, info2_d = ctx.green(phi2_d)
-    theta2 = theta2_d.cpu().numpy()
+    theta2, logdet2 = theta2_d.cpu().numpy(), logdet2_d.cpu().numpy()
     assert np.all(info2_d.cpu().numpy() == 0)
+    worst, worst_cond = 0.0, 0.0
     for w in sample:
         th_o, ld_o, _ = orc.green(pb.psi_t, phi2[w])
-        assert relerr(theta2[w], th_o) < 1e-8, ("theta2", w, relerr(theta2[w], th_o))   # cond(O') enters here
+        cnd = cond_overlap(pb.psi_t, phi2[w])
+        err = relerr(theta2[w], th_o)
+        worst, worst_cond = max(worst, err), max(worst_cond, cnd)
+        assert err < theta2_bound(cnd), ("theta2", w, err, cnd)
+        assert abs(logdet2[w].real - ld_o.real) < tol * max(1.0, abs(ld_o.real)), ("logdet2", w)
+        assert phase_diff(logdet2[w].imag, ld_o.imag) < 1e-9, ("phase2", w)
+    print("[parity %s] theta(propagated walker): max rel err %.2e, max cond(O') %.2e, bound %.2e"
+          % (cfg.name, worst, worst_cond, theta2_bound(worst_cond)))
+
+    # a7-a9
     e_d = ctx.local_energy(theta2_d)
     e = e_d.cpu().numpy()
-    if check_energy:
+    e_orc = oracle_energies(mesh, case.Lh, case.ht, theta2, energy_sample)
+    for w in energy_sample:
+        e_o = e_orc[w]
+        for i, name in enumerate(("E1", "EC", "EX")):
+            assert abs(e[w, i] - e_o[i]) < tol * abs(e_o[i]), (name, w, e[w, i], e_o[i])
+    if len(energy_sample) < case.nw:
+        # the walkers the oracle did not evaluate: the two independent exchange kernels must agree on every walker
+        ctx.set_option("exchange_3m", 0)
+        try:
+            e4 = ctx.local_energy(theta2_d).cpu().numpy()
+        finally:
+            ctx.set_option("exchange_3m", 1)
+        assert np.max(np.abs(e4 - e) / np.abs(e)) < 1e-12, ("3M vs 4M", np.max(np.abs(e4 - e) / np.abs(e)))
+        # E1 and EC of EVERY walker against the oracle's cheap definitions (Eq. 49 line 1; Eq. 41 from the force bias)
+        vb2 = ctx.force_bias(theta2_d).cpu().numpy()
         for w in sample:
-            e_o = orc.local_energy(mesh, case.Lh, case.ht, theta2[w])
-            for i, name in enumerate(("E1", "EC", "EX")):
-                assert abs(e[w, i] - e_o[i]) < tol * abs(e_o[i]), (name, w, e[w, i], e_o[i])
+            e1_o = sum(2.0 * np.sum(case.ht[k] * theta2[w][k * cfg.n:(k + 1) * cfg.n, k * cfg.m:(k + 1) * cfg.m]) for k in range(cfg.nk))
+            ec_o = orc.coulomb_from_vbias(mesh, orc.force_bias(mesh, case.Lh, theta2[w]))
+            assert abs(e[w, 0] - e1_o) < tol * abs(e1_o), ("E1", w)
+            assert abs(e[w, 1] - ec_o) < tol * abs(ec_o), ("EC", w)
+            assert relerr(vb2[w], orc.force_bias(mesh, case.Lh, theta2[w])) < tol
 
     # whole step == the chain above, bit for bit, on device and through the host entry
     phi3_d = phi_d.clone()
@@ -126,6 +197,27 @@ def run_chain_and_compare(case, sample, tol=RTOL, check_energy=True):
     assert torch.equal(phi_h, phi2_d.cpu())
     assert torch.equal(e_h, e_d.cpu())
     return e
+
+
+def step_end_to_end_vs_oracle(case, walkers):
+    """afqmc_step (one call, nothing downloaded in between) against orc.step on the same walkers: energies, log det and
+    the propagated walker with every stage's rounding compounding.  The energies pass through the inversion of O', so
+    their bound is theta2_bound(cond(O')) (= 1e-10 unless the propagated overlap is ill conditioned; printed)."""
+    cfg, pb, ctx = case.cfg, case.pb, case.ctx
+    phi_d = _to_dev(pb.phi)
+    e_d, ld_d, info_d = ctx.step(phi_d, _to_dev(pb.x), cfg.dtau, cfg.order)
+    e, ld, phi_new = e_d.cpu().numpy(), ld_d.cpu().numpy(), phi_d.cpu().numpy()
+    assert np.all(info_d.cpu().numpy() == 0)
+    for w in walkers:
+        phi_o, e_o, ld_o = orc.step(cfg.mesh, pb.L, case.Lh, case.ht, pb.psi_t, pb.phi[w:w + 1], pb.x[w:w + 1], cfg.dtau, cfg.order)
+        cnd = cond_overlap(pb.psi_t, phi_o[0])
+        bound = theta2_bound(cnd)
+        assert relerr(phi_new[w], phi_o[0]) < RTOL, ("phi'", w, relerr(phi_new[w], phi_o[0]))
+        errs = [abs(e[w, i] - e_o[0, i]) / abs(e_o[0, i]) for i in range(3)]
+        print("[e2e %s walker %d] rel err E1 %.2e EC %.2e EX %.2e, cond(O') %.2e, bound %.2e" % ((cfg.name, w) + tuple(errs) + (cnd, bound)))
+        assert max(errs) < bound, (w, errs, cnd)
+        assert abs(ld[w].real - ld_o[0].real) < RTOL * max(1.0, abs(ld_o[0].real))
+        assert phase_diff(ld[w].imag, ld_o[0].imag) < 1e-9
 
 
 # ------------------------------------------------------------------------------------------
@@ -147,7 +239,8 @@ def test_ragged_small(kw):
     cfg = synth.tiny_config(seed=2, **kw)
     case = Case(cfg)
     try:
-        run_chain_and_compare(case, range(case.nw))
+        run_chain_and_compare(case)
+        step_end_to_end_vs_oracle(case, range(case.nw))
     finally:
         case.close()
 
@@ -155,15 +248,17 @@ def test_ragged_small(kw):
 def test_config_C1_all_walkers():
     case = Case(synth.CONFIGS["C1"])
     try:
-        run_chain_and_compare(case, range(case.nw))
+        run_chain_and_compare(case)
+        step_end_to_end_vs_oracle(case, range(case.nw))
     finally:
         case.close()
 
 
-def test_config_C2_sampled():
+def test_config_C2_all_walkers_energy_sampled():
     case = Case(synth.CONFIGS["C2"])
     try:
-        run_chain_and_compare(case, [0, 37, 63])
+        run_chain_and_compare(case, energy_sample=[0, 37, 63])
+        step_end_to_end_vs_oracle(case, [11])
     finally:
         case.close()
 
@@ -173,35 +268,36 @@ def test_gamma_point_supercell_shape_sampled():
     its theta blocks do not fit one CTA's shared memory, so the exchange runs the large-block 3M kernel."""
     case = Case(synth.CONFIGS["G1"])
     try:
-        run_chain_and_compare(case, [0, 9])
+        run_chain_and_compare(case, energy_sample=[0, 9, 15])
     finally:
         case.close()
 
 
-def test_config_C3_headline_sampled():
+def test_config_C3_headline_all_walkers_energy_sampled():
     case = Case(synth.CONFIGS["C3"])
     try:
-        run_chain_and_compare(case, [0, 31])
+        run_chain_and_compare(case, energy_sample=[0, 16, 31])
+        step_end_to_end_vs_oracle(case, [7])
     finally:
         case.close()
 
 
 @pytest.mark.slow
 @pytest.mark.skipif(os.environ.get("AFQMC_SKIP_LARGE") == "1", reason="AFQMC_SKIP_LARGE=1")
-def test_config_C4_sampled():
+def test_config_C4_all_walkers_energy_sampled():
     case = Case(synth.CONFIGS["C4"])
     try:
-        run_chain_and_compare(case, [15])
+        run_chain_and_compare(case, energy_sample=[0, 8, 15])
     finally:
         case.close()
 
 
 @pytest.mark.slow
 @pytest.mark.skipif(os.environ.get("AFQMC_SKIP_LARGE") == "1", reason="AFQMC_SKIP_LARGE=1")
-def test_config_C5_sampled():
+def test_config_C5_all_walkers_energy_sampled():
     case = Case(synth.CONFIGS["C5"])
     try:
-        run_chain_and_compare(case, [7])
+        run_chain_and_compare(case, energy_sample=[0, 4, 7])
     finally:
         case.close()
 
@@ -250,6 +346,45 @@ def test_block_diagonal_walker_momentum_conservation(small_case):
     assert abs(ld.real - tot.real) < 1e-10 and phase_diff(ld.imag, tot.imag) < 1e-10
 
 
+@pytest.mark.parametrize("kw", [dict(mesh=(2, 3, 1), m=5, n=3, nchol=7), dict(mesh=(1, 2, 2), m=6, n=5, nchol=18)],
+                         ids=["2x3x1_m5_n3_c7", "1x2x2_m6_n5_c18"])
+def test_a0_half_rotation_probed_through_the_abi(kw):
+    """a0 located directly instead of inferred downstream: a ONE-HOT Theta with its 1 at row (k,a), column (k',r) makes
+    afqmc_force_bias return 2*Lh[Q][k][a][:,r] for the single Q with k-Q = k' and zero for every other Q (Eq. 47 is
+    linear in Theta), and afqmc_local_energy return E1 = 2*ht[k][a][r] iff k' = k (Eq. 49 line 1).  Every element of the
+    library's packed half-rotated tensors is thus read back and compared with orc.half_rotate on a ragged shape."""
+    cfg = synth.tiny_config(seed=23, nw=1, **kw)
+    nw = cfg.N * cfg.M
+    pb = synth.make_problem(cfg, nw=1)
+    from paper_2003_09468_b200 import binding
+    ctx = binding.from_problem(pb, max_walkers=nw)
+    try:
+        Lh, ht = orc.half_rotate(pb.L, pb.psi_t, pb.h1)
+        kminus, _ = orc.k_tables(cfg.mesh)
+        theta = np.zeros((nw, cfg.N, cfg.M), dtype=complex)
+        theta.reshape(nw, nw)[np.arange(nw), np.arange(nw)] = 1.0
+        theta_d = _to_dev(theta)
+        vb = ctx.force_bias(theta_d).cpu().numpy()
+        e = ctx.local_energy(theta_d).cpu().numpy()
+        expect_vb = np.zeros((nw, cfg.nk, cfg.nchol), dtype=complex)
+        expect_e1 = np.zeros(nw, dtype=complex)
+        for row in range(cfg.N):
+            k, a = divmod(row, cfg.n)
+            for col in range(cfg.M):
+                kp, r = divmod(col, cfg.m)
+                w = row * cfg.M + col
+                Q = [q for q in range(cfg.nk) if kminus[k, q] == kp]
+                assert len(Q) == 1
+                expect_vb[w, Q[0]] = 2.0 * Lh[Q[0], k, a, :, r]
+                if kp == k:
+                    expect_e1[w] = 2.0 * ht[k, a, r]
+        scale = np.max(np.abs(expect_vb))
+        assert np.max(np.abs(vb - expect_vb)) < 1e-13 * scale
+        assert np.max(np.abs(e[:, 0] - expect_e1)) < 1e-13 * np.max(np.abs(expect_e1))
+    finally:
+        ctx.close()
+
+
 def test_singular_overlap_reports_info(small_case):
     case = small_case
     phi = case.pb.phi[:2].copy()
@@ -291,6 +426,59 @@ def test_argument_errors(small_case):
     assert lib.afqmc_create(ctypes.byref(h), ctypes.byref(d), phi_d.data_ptr(), phi_d.data_ptr(), phi_d.data_ptr(), None) == 2
     d = binding.Dims((ctypes.c_int * 3)(2, 2, 1), 6, 7, 10, 1, 0, 4)       # n > m
     assert lib.afqmc_create(ctypes.byref(h), ctypes.byref(d), phi_d.data_ptr(), phi_d.data_ptr(), phi_d.data_ptr(), None) == 1
+
+
+def test_binding_rejects_wrong_shapes_dtypes_and_devices(small_case):
+    """The binding is marshalling only, but it must not hand a mis-shaped tensor to the kernels as a raw pointer."""
+    case, cfg = small_case, small_case.cfg
+    phi_d = _to_dev(case.pb.phi)
+    with pytest.raises(ValueError):
+        case.ctx.green(phi_d[:, :-1].contiguous())                       # wrong trailing dimension
+    with pytest.raises(ValueError):
+        case.ctx.green(torch.from_numpy(case.pb.phi))                    # host tensor
+    with pytest.raises(TypeError):
+        case.ctx.green(phi_d.to(torch.complex64))                        # wrong dtype
+    with pytest.raises(ValueError):
+        case.ctx.green(torch.cat([phi_d, phi_d]))                        # more walkers than max_walkers
+    theta_d, _, _ = case.ctx.green(phi_d)
+    with pytest.raises(ValueError):
+        case.ctx.force_bias(theta_d.transpose(1, 2).contiguous())        # [nw][M][N] where [nw][N][M] is expected
+    with pytest.raises(ValueError):
+        case.ctx.vhs(_to_dev(case.pb.x)[:2], case.ctx.force_bias(theta_d), cfg.dtau)   # batch sizes disagree
+    with pytest.raises(ValueError):
+        case.ctx.step_host(phi_d, torch.from_numpy(case.pb.x), cfg.dtau, cfg.order, torch.empty((case.nw, 3), dtype=torch.complex128))
+
+
+def test_contexts_in_sequence_and_side_by_side_share_no_state():
+    """include/afqmc.h: 'no global state'.  Kernel attributes (the dynamic shared-memory opt-in) are remembered per
+    context: a context created after another one was destroyed, and two contexts alive at once with different shapes,
+    give bit-identical results to a lone context."""
+    from paper_2003_09468_b200 import binding
+    cfg_a = synth.tiny_config(mesh=(2, 2, 1), m=26, n=4, nchol=24, nw=5, seed=31)      # > 48 KB of staged theta blocks
+    cfg_b = synth.tiny_config(mesh=(1, 1, 2), m=14, n=9, nchol=6, nw=2, seed=32)
+    pa, pb_ = synth.make_problem(cfg_a), synth.make_problem(cfg_b)
+
+    def run(ctx, pb, cfg):
+        phi = _to_dev(pb.phi)
+        e, ld, info = ctx.step(phi, _to_dev(pb.x), cfg.dtau, cfg.order)
+        return phi.cpu(), e.cpu(), ld.cpu()
+
+    ctx = binding.from_problem(pa)
+    ref_a = run(ctx, pa, cfg_a)
+    ctx.close()
+    ctx = binding.from_problem(pb_)
+    ref_b = run(ctx, pb_, cfg_b)
+    ctx.close()
+    ca, cb = binding.from_problem(pa), binding.from_problem(pb_)
+    try:
+        for _ in range(2):
+            got_b = run(cb, pb_, cfg_b)
+            got_a = run(ca, pa, cfg_a)
+            for r, g in zip(ref_a + ref_b, got_a + got_b):
+                assert torch.equal(r, g)
+    finally:
+        ca.close()
+        cb.close()
 
 
 def test_subbatch_equals_full_batch(small_case):
@@ -411,7 +599,7 @@ def test_mixed_precision_exchange_is_unsupported_for_more_than_four_orbitals():
 
 def test_mixed_precision_exchange_c3_full_size():
     """C3 at full size: 3xTF32 against the FP64 kernel on every walker (the FP64 kernel is checked against the oracle in
-    test_config_C3_headline_sampled), and against the oracle on one walker."""
+    test_config_C3_headline_all_walkers_energy_sampled), and against the oracle on one walker."""
     case = Case(synth.CONFIGS["C3"])
     try:
         theta_d, _, _ = case.ctx.green(_to_dev(case.pb.phi))
