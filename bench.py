@@ -88,40 +88,87 @@ class ClockSampler(threading.Thread):
                 "samples": len(sm), "reasons": reasons}
 
 
-def oracle_walker_step(orc, cfg, pb, Lh, ht, w):
-    t0 = time.perf_counter()
-    orc.step(cfg.mesh, pb.L, Lh, ht, pb.psi_t, pb.phi[w:w + 1], pb.x[w:w + 1], cfg.dtau, cfg.order)
-    return time.perf_counter() - t0
+# ---- the CPU oracle on the host cores: one worker PROCESS per core, one walker per worker call.  The oracle itself is
+# untouched (plain single-threaded numpy); the pool only runs several walkers side by side, which is how the step shards
+# (walkers are independent).  Workers are forked BEFORE this process touches CUDA, inherit the problem copy-on-write and
+# run numpy only.
+_ORC = {}
+
+
+def _oracle_job(w):
+    from threadpoolctl import threadpool_limits
+    o = _ORC
+    with threadpool_limits(limits=1):
+        t0 = time.perf_counter()
+        o["orc"].step(o["cfg"].mesh, o["pb"].L, o["Lh"], o["ht"], o["pb"].psi_t, o["pb"].phi[w:w + 1], o["pb"].x[w:w + 1],
+                      o["cfg"].dtau, o["cfg"].order)
+        return time.perf_counter() - t0
+
+
+def host_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+class OraclePool:
+    """`cores` forked workers that each run orc.step for one walker at a time."""
+
+    def __init__(self, cfg, pb, cores):
+        import multiprocessing as mp
+        from threadpoolctl import threadpool_limits
+        from oracle import afqmc_oracle as orc
+        with threadpool_limits(limits=1):
+            Lh, ht = orc.half_rotate(pb.L, pb.psi_t, pb.h1)
+        _ORC.update(orc=orc, cfg=cfg, pb=pb, Lh=Lh, ht=ht)
+        self.cores = max(1, int(cores))
+        self.pool = mp.get_context("fork").Pool(self.cores) if self.cores > 1 else None
+
+    def run(self, walkers):
+        """Wall seconds to do one full oracle step for each walker of `walkers`, `cores` at a time."""
+        t0 = time.perf_counter()
+        if self.pool is None:
+            for w in walkers:
+                _oracle_job(w)
+        else:
+            self.pool.map(_oracle_job, list(walkers), chunksize=1)
+        return time.perf_counter() - t0
+
+    def close(self):
+        if self.pool is not None:
+            self.pool.close()
+            self.pool.join()
+        _ORC.clear()
 
 
 def run_reference(args):
-    """The CPU oracle as the reference arm: each 'step' is the full step for ONE walker of the config."""
-    rank = int(os.environ.get("RANK", "0"))
+    """The CPU oracle as the reference arm: each 'step' is the full step (overlap .. local energy) for one walker per
+    host core in use, all cores side by side (bounded sample of the config's walker batch; work is linear in walkers)."""
+    from paper_2003_09468_b200 import replicas, synth
+    rank, _, world = replicas.rank_env()
     if rank != 0:
         return
-    import numpy as np  # noqa: F401
-    from threadpoolctl import threadpool_limits
-    from oracle import afqmc_oracle as orc
-    from paper_2003_09468_b200 import synth
     cfg = synth.CONFIGS[args.config]
-    nsamp = max(1, min(cfg.nw, args.steps + args.warmup))
-    pb = synth.make_problem(cfg, nw=nsamp)
-    with threadpool_limits(limits=1):
-        Lh, ht = orc.half_rotate(pb.L, pb.psi_t, pb.h1)
-        for i in range(args.warmup):
-            oracle_walker_step(orc, cfg, pb, Lh, ht, i % nsamp)
-        tot = 0.0
-        for i in range(args.steps):
-            tot += oracle_walker_step(orc, cfg, pb, Lh, ht, (args.warmup + i) % nsamp)
-    value = args.steps / tot
+    cores = min(host_cores() if args.cores <= 0 else args.cores, cfg.nw)
+    pb = synth.make_problem(cfg, nw=cores)
+    pool = OraclePool(cfg, pb, cores)
+    try:
+        for _ in range(args.warmup):
+            pool.run(range(cores))
+        tot = sum(pool.run(range(cores)) for _ in range(args.steps))
+    finally:
+        pool.close()
+    value = cores * args.steps / tot
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "c128", "data": "synthetic",
-        "config": {"workload": "%s: %dx%dx%d k-mesh, m=%d, n=%d, nchol=%d, complex128; one walker per step"
-                               % ((cfg.name,) + tuple(cfg.mesh) + (cfg.m, cfg.n, cfg.nchol))},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
-                         "sample": "%d timed full steps (overlap..local energy), one walker each, numpy, 1 thread" % args.steps},
+        "config": {"workload": "%s: %dx%dx%d k-mesh, m=%d, n=%d, nchol=%d, complex128; %d walkers per step (one per host core)"
+                               % ((cfg.name,) + tuple(cfg.mesh) + (cfg.m, cfg.n, cfg.nchol, cores))},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": "%d timed passes, each the full step (overlap..local energy) of %d walkers of %s side by side, "
+                                   "one single-threaded numpy oracle process per core" % (args.steps, cores, cfg.name)},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -130,27 +177,47 @@ def run_reference(args):
 
 def run_ours(args):
     import numpy as np
+    from paper_2003_09468_b200 import replicas, synth
+
+    rank, local_rank, world = replicas.rank_env()
+    cfg = synth.CONFIGS[args.config]
+    # replicas: every rank has the same Hamiltonian and its own seeded walkers/fields (weak scaling); rank r owns the
+    # global walkers [r*nw, (r+1)*nw) of the nw*world walkers of the job
+    pb = synth.make_problem(cfg)
+    nw = cfg.nw
+    w_lo, w_hi = replicas.shard_walkers(nw * world, rank, world)
+    assert w_hi - w_lo == nw
+    if rank > 0:
+        rng = np.random.default_rng(cfg.seed + 1000 + rank)
+        pb.phi = synth.make_walkers(cfg, pb.psi_t, rng)
+        pb.x = rng.standard_normal(pb.x.shape)
+
+    # ---- CPU baseline: the oracle on a bounded sample, on all host cores (rank 0, N=1 only); runs BEFORE CUDA is touched
+    # so that the worker processes can be forked safely ----
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cores = min(host_cores() if args.cores <= 0 else args.cores, nw)
+        pool = OraclePool(cfg, pb, cores)
+        try:
+            t1 = pool.run(range(cores))                       # one walker per core
+            passes = 1
+            while t1 < 8.0 and passes < 64:                   # small configs: repeat until ~10 s of wall time
+                t1 += pool.run(range(cores))
+                passes += 1
+        finally:
+            pool.close()
+        cpu = {"value": cores * passes / t1, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "%d pass(es) of %d of the %d walkers of %s, full step each (work is linear in walkers), one "
+                         "single-threaded numpy oracle process per host core, %.1f s wall" % (passes, cores, nw, cfg.name, t1)}
+
     import torch
     import torch.distributed as dist
-    from paper_2003_09468_b200 import binding, synth
-
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2003_09468_b200 import binding
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-
-    cfg = synth.CONFIGS[args.config]
-    # replicas: every rank has the same Hamiltonian and its own seeded walkers/fields (weak scaling)
-    pb = synth.make_problem(cfg)
-    if rank > 0:
-        rng = np.random.default_rng(cfg.seed + 1000 + rank)
-        pb.phi = synth.make_walkers(cfg, pb.psi_t, rng)
-        pb.x = rng.standard_normal(pb.x.shape)
-    nw = cfg.nw
     ctx = binding.from_problem(pb)
     ctx.set_option("timers", 1)
     phi0 = torch.from_numpy(pb.phi).cuda()
@@ -250,16 +317,13 @@ def run_ours(args):
     h2d = phi_h.numel() * 16 + x_h.numel() * 8
     d2h = phi_h.numel() * 16 + e_h.numel() * 16 + ld_h.numel() * 16 + info_h.numel() * 4
 
-    # max over ranks
-    times = torch.tensor([dev_ms, e2e_t * 1e3], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    dev_ms_max, e2e_ms_max = float(times[0]), float(times[1])
+    # max over ranks (the only torch.distributed traffic of the run besides the barriers)
+    dev_ms_max = replicas.max_over_ranks(dev_ms, device="cuda")
+    e2e_ms_max = replicas.max_over_ranks(e2e_t * 1e3, device="cuda")
 
     if rank == 0:
-        total_walkers = nw * world
-        value = total_walkers * args.steps / (dev_ms_max * 1e-3)
-        e2e_value = total_walkers * args.steps / (e2e_ms_max * 1e-3)
+        value = replicas.aggregate_throughput(nw, args.steps, world, dev_ms_max)
+        e2e_value = replicas.aggregate_throughput(nw, args.steps, world, e2e_ms_max)
         # ---- roofline of the dominant kernel (exchange contraction, a9) ----
         ex_ms = stage_acc["exchange"] / args.steps
         ex_flops = ex_flops_default
@@ -295,20 +359,6 @@ def run_ours(args):
         force_bias_roofline = {"kernel": "force bias (a4), afqmc_force_bias", "bound": "tensor", "flops_per_launch": fb_flops,
                                "ms_per_launch": fb_ms, "achieved": fb_flops / (fb_ms * 1e-3) / 1e12, "peak": peak_probe,
                                "unit": "TFLOP/s", "frac": fb_flops / (fb_ms * 1e-3) / 1e12 / peak_probe}
-        # ---- CPU baseline: the oracle on a bounded sample (rank 0, N=1 only) ----
-        cpu = None
-        if world == 1 and not args.no_cpu_baseline:
-            from threadpoolctl import threadpool_limits
-            from oracle import afqmc_oracle as orc
-            with threadpool_limits(limits=1):
-                Lh, ht = orc.half_rotate(pb.L, pb.psi_t, pb.h1)
-                nsamp = 2 if cfg.name in ("C3",) else 1
-                if cfg.name in ("C1", "C2"):
-                    nsamp = min(cfg.nw, 8)
-                t = sum(oracle_walker_step(orc, cfg, pb, Lh, ht, w) for w in range(nsamp))
-            cpu = {"value": nsamp / t, "unit": UNIT, "cores": 1, "kind": "oracle",
-                   "sample": "%d of %d walkers of %s, full step each (work is linear in walkers), numpy 1 thread, %.1f s"
-                             % (nsamp, nw, cfg.name, t)}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True,
@@ -412,10 +462,18 @@ def main():
     ap.add_argument("--config", default="C3")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cores", type=int, default=0, help="host cores for the CPU oracle (0 = all available to the process)")
     ap.add_argument("--no-block", action="store_true", help="skip the extra 20-step block measurement")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
+    from paper_2003_09468_b200 import replicas
+    if replicas.needs_launch(args.gpus):
+        # `python bench.py --gpus N` without torchrun: start the N ranks (one per GPU) and let rank 0 print the line
+        sys.exit(replicas.launch_ranks(os.path.abspath(__file__), sys.argv[1:], args.gpus))
+    _, _, world = replicas.rank_env()
+    if world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d" % (args.gpus, world))
     if args.impl == "reference":
         run_reference(args)
     else:

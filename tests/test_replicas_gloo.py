@@ -46,3 +46,38 @@ def test_two_rank_timing_is_max_over_ranks():
 
 def test_single_process_identity():
     assert replicas.max_over_ranks(3.5) == 3.5
+
+
+def test_launch_command_is_the_drivers_line():
+    cmd = replicas.launch_command("bench.py", ["--gpus", "2"], 2, port=29511)
+    assert cmd[1:4] == ["-m", "torch.distributed.run", "--nnodes=1"]
+    assert cmd[cmd.index("--nproc-per-node") + 1] == "2"
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "29511"
+    assert cmd[-3:] == ["bench.py", "--gpus", "2"]
+    assert replicas.rank_env() == (0, 0, 1) or "WORLD_SIZE" in os.environ
+
+
+def test_needs_launch_only_without_a_rank_environment(monkeypatch):
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    assert not replicas.needs_launch(1)
+    assert replicas.needs_launch(2)
+    monkeypatch.setenv("WORLD_SIZE", "2")
+    assert not replicas.needs_launch(2)
+
+
+def test_bench_gpus_2_starts_two_ranks_and_rank0_prints_one_line():
+    """`python bench.py --gpus 2` (no torchrun) must start the two ranks itself.  Driven here on CPU through the
+    reference arm (the CPU oracle: rank 0 works, the other rank exits 0), smallest config."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--impl", "reference", "--config", "C1",
+                        "--steps", "1", "--warmup", "0", "--cores", "2"], capture_output=True, text=True, timeout=600, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    rec = json.loads(lines[0])
+    assert rec["impl"] == "reference" and rec["n_gpus"] == 2 and rec["cpu_baseline"]["cores"] == 2
+    assert rec["value"] > 0 and rec["e2e"]["h2d_bytes_per_step"] == 0
