@@ -47,9 +47,11 @@ struct afqmc_ctx {
     // static tensors
     double2* psi_t; // [Nk][m][n]
     double2* ht;    // [Nk][n][m]   half-rotated one-body
-    double* Lx;     // exchange fragment layout  [Q][k][ag][gq][s][lane][2]
-    double* Lx3;    // exchange, 3M products      [Q][k][ag][gq][ks][prod][lane][2]   (exchange3m.cu; n <= 4 only, else NULL)
-    float* LxT;     // exchange, TF32 fragments       [Q][k][gq][ks][lane][4]             (exchange_tf32.cu; n <= 4 only, else NULL)
+    double2* Lh;    // half-rotated Cholesky tensor, natural layout [Q][k][a][gamma][r]: computed ONCE in a0; every packed
+                    // operand below is a pure re-layout of it
+    double* Lxc;    // exchange (default 3M kernel, exchange3m.cu): complex fragments [Q][k][ag][gq][ks][lane][4]
+    double* Lx;     // exchange, 4M kernel (energy.cu): [Q][k][ag][gq][s][lane][2]; packed on first use (option exchange_3m = 0)
+    float* LxT;     // exchange, TF32 fragments [Q][k][gq][ks][lane][4] (exchange_tf32.cu; n <= 4 only); packed on first use
     double* Lf;     // force-bias fragment layout [Q][gtp][k][a][s][lane][2]
     double2* Lv3;   // vHS operand [unit][prt][ks][lane] complex fragments (vhs.cu); one block per (Q,-Q) pair if vhs_paired
     int* vunits;    // vHS work units, int4-packed (Q, k, kind, 0) [nvunits]; kind 1 = block + its (-Q,k-Q) partner
@@ -90,6 +92,7 @@ struct afqmc_ctx {
     int opt_exchange_prec;  // 0 (default) = FP64 exchange kernels; mixed precision on the TF32 tensor cores (n <= 4): 1 = 3xTF32 split, 2 = 1xTF32
     int opt_exchange_3m;    // 1 (default) = 3M exchange kernel when n <= 4, 0 = the 4M kernel of energy.cu
     int opt_exchange_wpc;   // 0 = automatic, else warps per CTA of the exchange kernel (4,5,6,8)
+    int opt_exchange_np;    // tuning aid (3M kernel): 0 = automatic, else 1/2/4 walker pairs (n-tiles) per warp
     int opt_timers;     // record stage events in afqmc_step
     int opt_taylor_legacy;  // testing aid: 1 = shared-memory-tiled zgemm for the Taylor chain
     int opt_taylor_wpc;     // tuning aid: 0 = automatic, else 3/4/5 warps per CTA of the Taylor GEMM
@@ -203,12 +206,15 @@ int afqmc_i_vhs(afqmc_ctx* c, const double* x, const double2* vbias, double dtau
 int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, double2* phi, int nw,
                       cudaStream_t st);
 int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* energy, cudaStream_t st);
-int afqmc_i_exchange3m(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st);   // AFQMC_UNSUPPORTED if n > 4
-int afqmc_i_pack_lx3(afqmc_ctx* c, const double2* L, cudaStream_t st);
+int afqmc_i_exchange3m(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st);   // AFQMC_UNSUPPORTED only if the staged theta blocks exceed shared memory
+int afqmc_i_pack_lxc(afqmc_ctx* c, cudaStream_t st);                                    // Lh -> Lxc
+size_t afqmc_i_lxc_doubles(const Dims& d);
+int afqmc_i_exchange3m_parts_max(const afqmc_ctx* c);
 int afqmc_i_exchange_tf32(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st);  // AFQMC_UNSUPPORTED if n > 4
-int afqmc_i_pack_lxt(afqmc_ctx* c, const double2* L, cudaStream_t st);
+int afqmc_i_ensure_lx(afqmc_ctx* c, cudaStream_t st);     // packs the 4M operand Lx from Lh on first use
+int afqmc_i_ensure_lxt(afqmc_ctx* c, cudaStream_t st);    // packs the TF32 operand LxT from Lh on first use (n <= 4)
+int afqmc_i_pack_lxt(afqmc_ctx* c, cudaStream_t st);
 size_t afqmc_i_lxt_floats(const Dims& d);
-size_t afqmc_i_lx3_doubles(const Dims& d);
 int afqmc_i_apply_onebody(afqmc_ctx* c, double2* phi, int nw, cudaStream_t st);
 int afqmc_i_step(afqmc_ctx* c, double2* phi, const double* x, double dtau, int order, int nw, double2* energy,
                  double2* logdet, int* info, cudaStream_t st, cudaEvent_t phi_final /* nullable: recorded after the propagation */);

@@ -34,22 +34,33 @@ AFQMC_API const char* afqmc_strerror(int code) {
 //  (the vHS operand Lv3 and the 3M exchange operand Lx3 are described and packed in vhs.cu / exchange3m.cu)
 // Out-of-range rows / K entries are stored as zeros, so kernels never branch on tails.
 // ---------------------------------------------------------------------------------------
-__device__ __forceinline__ double2 half_rot_elem(const double2* __restrict__ L, const double2* __restrict__ psi_t,
-                                                 const Dims& d, int Q, int k, int a, int gam, int r) {
-    // Lh[Q][k][a][gam][r] = sum_p conj(A_k[p][a]) L[Q][k][gam][p][r]
-    const double2* Lb = L + (((size_t)(Q * d.Nk + k) * d.nchol + gam) * d.m) * d.m + r;
-    const double2* Ab = psi_t + (size_t)k * d.m * d.n + a;
-    double2 acc = make_double2(0.0, 0.0);
-    for (int p = 0; p < d.m; ++p) {
-        double2 av = Ab[(size_t)p * d.n];
-        av.y = -av.y;
-        acc = cfma(av, Lb[(size_t)p * d.m], acc);
+// Lh[Q][k][a][gam][r] = sum_p conj(A_k[p][a]) L[Q][k][gam][p][r], computed once; natural layout
+__global__ void half_rot_L_kernel(Dims d, const double2* __restrict__ L, const double2* __restrict__ psi_t,
+                                  double2* __restrict__ Lh, size_t total) {
+    for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+        size_t t = idx;
+        const int r = (int)(t % d.m); t /= d.m;
+        const int gam = (int)(t % d.nchol); t /= d.nchol;
+        const int a = (int)(t % d.n); t /= d.n;
+        const int k = (int)(t % d.Nk);
+        const int Q = (int)(t / d.Nk);
+        const double2* Lb = L + (((size_t)(Q * d.Nk + k) * d.nchol + gam) * d.m) * d.m + r;
+        const double2* Ab = psi_t + (size_t)k * d.m * d.n + a;
+        double2 acc = make_double2(0.0, 0.0);
+        for (int p = 0; p < d.m; ++p) {
+            double2 av = Ab[(size_t)p * d.n];
+            av.y = -av.y;
+            acc = cfma(av, Lb[(size_t)p * d.m], acc);
+        }
+        Lh[idx] = acc;
     }
-    return acc;
 }
 
-__global__ void pack_Lx_kernel(Dims d, const double2* __restrict__ L, const double2* __restrict__ psi_t,
-                               double* __restrict__ Lx, size_t total) {
+__device__ __forceinline__ double2 lh_elem(const double2* __restrict__ Lh, const Dims& d, int Q, int k, int a, int gam, int r) {
+    return Lh[((((size_t)Q * d.Nk + k) * d.n + a) * d.nchol + gam) * d.m + r];
+}
+
+__global__ void pack_Lx_kernel(Dims d, const double2* __restrict__ Lh, double* __restrict__ Lx, size_t total) {
     for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total;
          idx += (size_t)gridDim.x * blockDim.x) {
         size_t t = idx;
@@ -65,15 +76,14 @@ __global__ void pack_Lx_kernel(Dims d, const double2* __restrict__ L, const doub
         int j = 4 * s + kk, r = j >> 1, c = j & 1;
         double v = 0.0;
         if (Q < d.Nk && a < d.n && gam < d.nchol && r < d.m) {   // Q >= Nk: the zero pad
-            double2 z = half_rot_elem(L, psi_t, d, Q, k, a, gam, r);
+            double2 z = lh_elem(Lh, d, Q, k, a, gam, r);
             v = c ? z.y : z.x;
         }
         Lx[idx] = v;
     }
 }
 
-__global__ void pack_Lf_kernel(Dims d, const double2* __restrict__ L, const double2* __restrict__ psi_t,
-                               double* __restrict__ Lf, size_t total) {
+__global__ void pack_Lf_kernel(Dims d, const double2* __restrict__ Lh, double* __restrict__ Lf, size_t total) {
     for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total;
          idx += (size_t)gridDim.x * blockDim.x) {
         size_t t = idx;
@@ -89,7 +99,7 @@ __global__ void pack_Lf_kernel(Dims d, const double2* __restrict__ L, const doub
         int j = 4 * s + kk, r = j >> 1, c = j & 1;
         double v = 0.0;
         if (gam < d.nchol && r < d.m) {
-            double2 z = half_rot_elem(L, psi_t, d, Q, k, a, gam, r);
+            double2 z = lh_elem(Lh, d, Q, k, a, gam, r);
             v = c ? z.y : z.x;
         }
         Lf[idx] = v;
@@ -135,7 +145,7 @@ static int dev_alloc(T** p, size_t count) {
 
 AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     if (!c) return;
-    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lx, c->Lx3, c->LxT, c->Lf, c->Lv3, c->vunits,
+    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lh, c->Lxc, c->Lx, c->LxT, c->Lf, c->Lv3, c->vunits,
                     c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T, c->ws_Tx,
                     c->ws_expart, c->ws_fbpart, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
                     c->ws_f32, c->b1, c->ws_b1tmp, c->ws_gram, c->ws_rinv, c->ws_logdet2, c->ws_ldr, c->ws_info2};
@@ -216,7 +226,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
 
     int rc = AFQMC_OK;
     auto A = [&](int r) { if (rc == AFQMC_OK) rc = r; };
-    const size_t nLx = (size_t)Nk * Nk * d.NAG * d.GQ * d.KS * 64 + AFQMC_LX_PAD;
+    const size_t nLh = (size_t)Nk * Nk * d.n * d.nchol * d.m;
     const size_t nLf = (size_t)Nk * d.GT2 * Nk * d.n * d.KS * 64;
     const int LD = d.N | 1;
     A(dev_alloc(&c->kminus, (size_t)Nk * Nk));
@@ -225,9 +235,8 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     A(dev_alloc(&c->units, units.size()));
     A(dev_alloc(&c->psi_t, (size_t)Nk * d.m * d.n));
     A(dev_alloc(&c->ht, (size_t)Nk * d.n * d.m));
-    A(dev_alloc(&c->Lx, nLx));
-    A(dev_alloc(&c->Lx3, afqmc_i_lx3_doubles(d)));
-    if (d.NAG == 1) A(dev_alloc(&c->LxT, afqmc_i_lxt_floats(d)));
+    A(dev_alloc(&c->Lh, nLh));
+    A(dev_alloc(&c->Lxc, afqmc_i_lxc_doubles(d)));
     A(dev_alloc(&c->Lf, nLf));
     A(dev_alloc(&c->ws_O, (size_t)nw * d.N * LD));
     A(dev_alloc(&c->ws_oinvT, (size_t)nw * d.N * d.N));
@@ -238,13 +247,9 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     A(dev_alloc(&c->ws_T, (size_t)2 * nw * d.M * d.N));
     const size_t nTx = (size_t)2 * nw * afqmc_i_taylor_ws_doubles(d);
     A(dev_alloc(&c->ws_Tx, nTx));
-    {   // exchange partial sums: one per unit and walker, or NAG^2 * (up to 8 chunks) when the theta blocks of all a-groups
-        // do not fit one CTA's shared memory (large n*m per k-point: exchange3m_big_kernel)
-        const size_t multi_smem = (size_t)2 * d.NAG * 3 * ((d.m + 3) / 4) * 2 * 32 * sizeof(double);
-        c->ex_parts_max = (d.NAG > 1 && multi_smem > (size_t)c->smem_optin) ? d.NAG * d.NAG * 8 : 1;
-        c->ex_parts = 1;
-        A(dev_alloc(&c->ws_expart, (size_t)c->nunits * nw * c->ex_parts_max));
-    }
+    c->ex_parts_max = afqmc_i_exchange3m_parts_max(c);      // exchange partial sums per unit (exchange3m.cu)
+    c->ex_parts = 1;
+    A(dev_alloc(&c->ws_expart, (size_t)c->nunits * nw * c->ex_parts_max));
     A(dev_alloc(&c->ws_fbpart, (size_t)AFQMC_FB_MAXKC * nw * Nk * d.nchol));
     A(dev_alloc(&c->ws_x, (size_t)nw * Nk * d.nchol));
     A(dev_alloc(&c->ws_phi, (size_t)nw * d.M * d.N));
@@ -287,21 +292,47 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
         const int T = 256;
         auto grid = [&](size_t total) { return (int)((total + T - 1) / T > 148 * 64 ? 148 * 64 : (total + T - 1) / T); };
         half_rot_h_kernel<<<grid((size_t)Nk * d.n * d.m), T, 0, st>>>(d, (const double2*)h1, c->psi_t, c->ht);
-        pack_Lx_kernel<<<grid(nLx), T, 0, st>>>(d, (const double2*)L, c->psi_t, c->Lx, nLx);
-        pack_Lf_kernel<<<grid(nLf), T, 0, st>>>(d, (const double2*)L, c->psi_t, c->Lf, nLf);
+        half_rot_L_kernel<<<grid(nLh), T, 0, st>>>(d, (const double2*)L, c->psi_t, c->Lh, nLh);     // the half rotation, once
+        pack_Lf_kernel<<<grid(nLf), T, 0, st>>>(d, c->Lh, c->Lf, nLf);
         c->launches += 3;
         if (cudaGetLastError() != cudaSuccess) rc = AFQMC_CUDA_ERROR;
-        if (rc == AFQMC_OK && c->Lx3) rc = afqmc_i_pack_lx3(c, (const double2*)L, st);
-        if (rc == AFQMC_OK && c->LxT) rc = afqmc_i_pack_lxt(c, (const double2*)L, st);
+        if (rc == AFQMC_OK) rc = afqmc_i_pack_lxc(c, st);
         if (rc == AFQMC_OK) rc = afqmc_i_vhs_setup(c, (const double2*)L, kminus, kneg, st);
     }
     // host vectors must outlive the async copies; the caller may free its arrays after return
     if (cudaStreamSynchronize(st) != cudaSuccess && rc == AFQMC_OK) rc = AFQMC_CUDA_ERROR;
     cudaFree(h1w); cudaFree(Lw); cudaFree(psiw);
     if (rc != AFQMC_OK) { (void)cudaGetLastError(); afqmc_destroy(c); return rc; }
-    if (c->prec32 && c->LxT) c->opt_exchange_prec = 1;      // complex64 boundary: 3xTF32 exchange by default
+    if (c->prec32 && d.NAG == 1) {      // complex64 boundary: 3xTF32 exchange by default
+        rc = afqmc_i_ensure_lxt(c, st);
+        if (rc == AFQMC_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = AFQMC_CUDA_ERROR;
+        if (rc != AFQMC_OK) { (void)cudaGetLastError(); afqmc_destroy(c); return rc; }
+        c->opt_exchange_prec = 1;
+    }
     *out = c;
     return AFQMC_OK;
+}
+
+// The operands of the two optional exchange kernels are re-layouts of Lh made the first time the option is used
+// (they add 1x |Lh| each, so they are not resident unless asked for).
+int afqmc_i_ensure_lx(afqmc_ctx* c, cudaStream_t st) {
+    if (c->Lx) return AFQMC_OK;
+    const Dims& d = c->d;
+    const size_t nLx = (size_t)d.Nk * d.Nk * d.NAG * d.GQ * d.KS * 64 + AFQMC_LX_PAD;
+    int rc = dev_alloc(&c->Lx, nLx);
+    if (rc != AFQMC_OK) return rc;
+    const size_t g = (nLx + 255) / 256;
+    pack_Lx_kernel<<<(unsigned)(g > 148 * 64 ? 148 * 64 : g), 256, 0, st>>>(d, c->Lh, c->Lx, nLx);
+    AFQMC_LAUNCH_CHECK(c);
+    return AFQMC_OK;
+}
+
+int afqmc_i_ensure_lxt(afqmc_ctx* c, cudaStream_t st) {
+    if (c->LxT) return AFQMC_OK;
+    if (c->d.NAG != 1) return AFQMC_UNSUPPORTED;
+    int rc = dev_alloc(&c->LxT, afqmc_i_lxt_floats(c->d));
+    if (rc != AFQMC_OK) return rc;
+    return afqmc_i_pack_lxt(c, st);
 }
 
 AFQMC_API long long afqmc_launch_count(const afqmc_ctx* c) { return c ? c->launches : 0; }
@@ -314,7 +345,8 @@ AFQMC_API double afqmc_exchange_flops(const afqmc_ctx* c, int nw) {
     // flops per complex multiply-add = 2 * 6*n*n*m*nchol, plus 3 additions per element of both T tensors.
     double per = 16.0 * d.n * d.n * d.m * d.nchol + 8.0 * d.n * d.n * d.nchol;
     if (c->opt_exchange_prec != 0 && c->LxT) return (c->opt_exchange_prec == 1 ? 3.0 : 1.0) * per * (double)c->nunits * (double)nw;      // TF32 kernel: the 4M real embedding
-    if (c->opt_exchange_3m && c->Lx3) per = 12.0 * d.n * d.n * d.m * d.nchol + 6.0 * d.n * d.n * d.nchol + 8.0 * d.n * d.n * d.nchol;
+    // (counted as pure 3M; the <= 2 tail elements of a row with m mod 4 in {1,2} are really done as 4M: not counted)
+    if (c->opt_exchange_3m) per = 12.0 * d.n * d.n * d.m * d.nchol + 6.0 * d.n * d.n * d.nchol + 8.0 * d.n * d.n * d.nchol;
     return per * (double)c->nunits * (double)nw;
 }
 
@@ -337,12 +369,26 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
     }
     if (strcmp(name, "exchange_precision") == 0) {
         if (value < 0 || value > 2) return AFQMC_INVALID_ARGUMENT;
-        if (value != 0 && !c->LxT) return AFQMC_UNSUPPORTED;        // n > 4
+        if (value != 0) {                                           // n > 4: AFQMC_UNSUPPORTED
+            int rc = afqmc_i_ensure_lxt(c, 0);
+            if (rc == AFQMC_OK && cudaStreamSynchronize(0) != cudaSuccess) rc = AFQMC_CUDA_ERROR;
+            if (rc != AFQMC_OK) return rc;
+        }
         c->opt_exchange_prec = value;
         return AFQMC_OK;
     }
     if (strcmp(name, "exchange_3m") == 0) {
+        if (!value) {
+            int rc = afqmc_i_ensure_lx(c, 0);
+            if (rc == AFQMC_OK && cudaStreamSynchronize(0) != cudaSuccess) rc = AFQMC_CUDA_ERROR;
+            if (rc != AFQMC_OK) return rc;
+        }
         c->opt_exchange_3m = value ? 1 : 0;
+        return AFQMC_OK;
+    }
+    if (strcmp(name, "exchange_np") == 0) {
+        if (value != 0 && value != 1 && value != 2 && value != 4) return AFQMC_INVALID_ARGUMENT;
+        c->opt_exchange_np = value;
         return AFQMC_OK;
     }
     if (strcmp(name, "exchange_minblocks") == 0) {

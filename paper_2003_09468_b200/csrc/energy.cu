@@ -327,7 +327,8 @@ int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* en
     c->ex_parts = 1;
     rc = c->opt_exchange_prec != 0 ? afqmc_i_exchange_tf32(c, theta, nw, st)
          : c->opt_exchange_3m    ? afqmc_i_exchange3m(c, theta, nw, st) : AFQMC_UNSUPPORTED;
-    if (rc == AFQMC_UNSUPPORTED) {          // n > 4, or the 4M kernel was asked for
+    if (rc == AFQMC_UNSUPPORTED) {          // the 4M kernel was asked for (or the TF32 option with n > 4)
+        if ((rc = afqmc_i_ensure_lx(c, st)) != AFQMC_OK) return rc;
         if (nw >= 3) rc = launch_exchange<4>(c, theta, nw, st);
         else rc = launch_exchange<2>(c, theta, nw, st);
     }

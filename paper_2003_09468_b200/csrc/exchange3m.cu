@@ -1,407 +1,344 @@
-// a9 exchange energy with the 3M complex product (same contraction as energy.cu, Eq. 49):
+// a9 exchange energy, the default kernel (same contraction as energy.cu; Eq. 49):
 //
-//   T = Lh * theta^T  is a complex GEMM.  energy.cu embeds it in ONE real GEMM with K = (r, re/im) and columns
-//   (b, re/im): 8 real flops per complex multiply-add (4 real products).  Here every complex product is formed
-//   from THREE real products (Gauss's form of the "3M" product: two additions per result instead of Karatsuba's three,
-//   which matters because DADD shares the FP64 units with DMMA):
-//       P0 = (Ar+Ai) Br,  P1 = Ar (Bi-Br),  P2 = Ai (Br+Bi);      Re T = P0 - P2,   Im T = P0 + P1
-//   i.e. three real GEMMs with K = r and columns b: 6 real flops per complex multiply-add, 25 % fewer DMMAs
-//   (19 % at m = 26, where K = 26 pads to 7 k-steps of 4).  The tensor pipe is the bound of this kernel
-//   (89 % DMMA issue, r01c profile), so fewer DMMAs is the only lever left.  Rounding: Im T carries the error of
-//   (|Ar|+|Ai|)(|Br|+|Bi|) instead of |A||B|: a small constant factor, far inside the 1e-10 tolerance.
+//     EX = - sum_units mult * X(unit),    unit = (Q,k,k2) ~ (-Q,k2,k)   (SURVEY.md P6 / DESIGN.md R6)
+//     X   = sum_{gamma,a,b} T1[(gamma,a),(w,b)] * T2[(gamma,b),(w,a)]
+//     T1  = sum_r Lh[ Q][k ][a][gamma][r] * theta_w[(k2,b),(k-Q ,r)]        (the paper's step 2(a))
+//     T2  = sum_s Lh[-Q][k2][b][gamma][s] * theta_w[(k ,a),(k2+Q,s)]        (step 2(b), Lbar read from Lh: R4)
 //
-// Layout of the static operand (written once in afqmc_create):
-//   Lx3[Q][k][ag][gq][ks][prod][lane][i]   prod = 0: Re + Im of Lh, 1: Re, 2: Im;  two M-tiles i = 0,1 per gamma-quad
-//   rows (gl = row>>2, al = row&3): gamma = 4gq+2i+gl, a = 4ag+al;  K: r = 4ks + (lane&3);  zeros outside.
-// A warp task is one gamma-quad: 3*KS3 "micro-steps" (ks-major, product-minor), each ONE coalesced 512-byte LDG.128
-// of A, consecutive in memory across micro-steps and tasks.  DMMA columns are (walker of a pair, b): one n-tile
-// serves two walkers, a CTA handles 2*NP walkers.  The three products keep separate accumulators; the register
-// pipeline is 3 deep and unrolled by 3, so buffer q always belongs to product q (static register indexing).
-// At the end of a task the products are combined and contracted in registers.  The partner tile is computed with
-// the DMMA operands swapped (theta as A, Lh as B: the two fragment lane layouts coincide), which yields it already
-// transposed in (a,b); one shuffle per value (lane bits 4 and 1 exchanged) then aligns gamma and walker.  n <= 4 (one
-// a-group) uses the tuned kernel below; larger n the multi-group variant after it (falls back to the 4M kernel only if
-// the theta blocks of all a-groups do not fit shared memory).
+// Both T's are complex GEMMs  (gamma,orbital) x r  times  r x (walker,orbital)  on the FP64 tensor pipe (DMMA m8n8k4); they never
+// leave the SM (the paper keeps them in a user-sized global buffer).  What this kernel does about the pipe:
+//
+//  * 3M complex product (Gauss):  P0 = (Ar+Ai) Br,  P1 = Ar (Bi-Br),  P2 = Ai (Br+Bi);  Re = P0 - P2,  Im = P0 + P1:
+//    three real GEMMs with K = r, 6 real flops per complex multiply-add instead of the 8 of the real embedding.
+//  * TAIL in the real embedding.  K = m is covered by k-steps of 4; when m mod 4 is 1 or 2 (m = 26: two left-over r) the last
+//    k-step of each product would be at least half padding (3 DMMA k-steps for <= 2 complex r).  Those <= 2 tail elements are
+//    instead done as 4M with K = (r, re/im) = 4 reals: ONE A fragment [Ar,Ai,Ar',Ai'] against B = [Br,-Bi,Br',-Bi'] (accumulated
+//    into P0: adds Re t) and against B = [Bi-Br, Br+Bi, ...] (into P1: adds Im t - Re t), i.e. 2 k-steps instead of 3 and
+//    Re = P0 - P2, Im = P0 + P1 still hold.  m = 26: 20 DMMA k-steps per task and tile pair instead of 21 (26 of 26.67 useful).
+//  * The static operand is stored COMPLEX (Re, Im per lane; Ar+Ai is one DADD per fragment, as in tgemm.cuh): 2/3 of the bytes
+//    and of the load wavefronts of a layout that stores the three A variants, so the register prefetch ring holds DA whole
+//    k-steps (3 products each) and covers the L2 latency of the stream (the r01 kernel ran 1 k-step ahead and lost 14 % of its
+//    issue slots to that, profiles/r01g).
+//  * A warp computes ONE of T1 / T2 (role h = warp & 1); the two warps of a pair meet once per task (gamma-quad): each hands
+//    one of its two m-tiles to the partner through shared memory (which also does the (a,b) transpose) and contracts the
+//    other one.  Half the accumulators per warp (3 products x 2 m-tiles x NP n-tiles) of a kernel that keeps T1 and T2 in
+//    one warp: more resident warps per scheduler, or NP = 4 (eight walkers per CTA: every A fragment feeds four n-tiles).
+//
+// Operand layout (written once in afqmc_create from Lh, see pack_Lxc_kernel):
+//   Lxc[Q][k][ag][gq][ks < KSPT][lane][4]   lane = (row << 2) | kk;  tile i rows: gamma = 4 gq + 2 i + (row >> 2), a = 4 ag + (row & 3)
+//     full k-step ks < KSF:  r = 4 ks + kk;  doubles = (Re, Im of tile 0, Re, Im of tile 1)
+//     tail k-step ks = KSF:  r = 4 KSF + (kk >> 1), part = kk & 1;  doubles = (part of tile 0, part of tile 1, 0, 0)
+//   one coalesced 1 KB access per k-step and warp, consecutive in memory across k-steps and tasks; zeros outside.
+// theta blocks are staged once per CTA in shared memory in B-fragment order, already expanded into the three B variants.
+#include <type_traits>
 #include "common.cuh"
 
 namespace {
 
-__global__ void pack_Lx3_kernel(Dims d, int KS3, const double2* __restrict__ L, const double2* __restrict__ psi_t,
-                                double* __restrict__ Lx3, size_t total_in /* without the product index */, size_t total_out) {
+struct X3Geom { int KSF, TAIL, KSPT, MSPT; };
+// k-steps of a task: KSF full ones (3 micro-steps = products each) + TAIL (0/1) real-embedded one (2 micro-steps)
+__host__ __device__ inline X3Geom x3_geom(int m) {
+    X3Geom g;
+    const int mr = m & 3;
+    g.TAIL = (mr == 1 || mr == 2) ? 1 : 0;
+    g.KSF = g.TAIL ? m / 4 : (m + 3) / 4;
+    g.KSPT = g.KSF + g.TAIL;
+    g.MSPT = 3 * g.KSF + 2 * g.TAIL;
+    return g;
+}
+
+__global__ void pack_Lxc_kernel(Dims d, X3Geom g, const double2* __restrict__ Lh, double* __restrict__ Lxc, size_t total_in,
+                                size_t total_out) {
+    // one thread per (.., ks, lane, tile i)
     for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total_in; idx += (size_t)gridDim.x * blockDim.x) {
         size_t t = idx;
         const int i = (int)(t & 1); t >>= 1;
         const int lane = (int)(t & 31); t >>= 5;
-        const int ks = (int)(t % KS3); t /= KS3;
+        const int ks = (int)(t % g.KSPT); t /= g.KSPT;
         const int gq = (int)(t % d.GQ); t /= d.GQ;
         const int ag = (int)(t % d.NAG); t /= d.NAG;
         const int k = (int)(t % d.Nk);
         const int Q = (int)(t / d.Nk);
         const int row = lane >> 2, kk = lane & 3;
-        const int gam = 4 * gq + 2 * i + (row >> 2), a = 4 * ag + (row & 3), r = 4 * ks + kk;
+        const int gam = 4 * gq + 2 * i + (row >> 2), a = 4 * ag + (row & 3);
+        const bool full = ks < g.KSF;
+        const int r = full ? 4 * ks + kk : 4 * g.KSF + (kk >> 1);
         double2 z = make_double2(0.0, 0.0);
-        if (a < d.n && gam < d.nchol && r < d.m) {
-            // Lh[Q][k][a][gam][r] = sum_p conj(A_k[p][a]) L[Q][k][gam][p][r]
-            const double2* Lb = L + (((size_t)(Q * d.Nk + k) * d.nchol + gam) * d.m) * d.m + r;
-            const double2* Ab = psi_t + (size_t)k * d.m * d.n + a;
-            for (int p = 0; p < d.m; ++p) {
-                double2 av = Ab[(size_t)p * d.n];
-                av.y = -av.y;
-                z = cfma(av, Lb[(size_t)p * d.m], z);
-            }
+        if (a < d.n && gam < d.nchol && r < d.m) z = Lh[((((size_t)Q * d.Nk + k) * d.n + a) * d.nchol + gam) * d.m + r];
+        double* out = Lxc + (idx >> 6) * 128 + lane * 4;        // (idx >> 6) = the k-step's linear index
+        if (full) {
+            out[2 * i] = z.x;
+            out[2 * i + 1] = z.y;
+        } else {
+            out[i] = (kk & 1) ? z.y : z.x;
+            out[2 + i] = 0.0;
         }
-        // [..][ks][prod][lane][i]
-        const size_t base = ((((((size_t)Q * d.Nk + k) * d.NAG + ag) * d.GQ + gq) * KS3 + ks) * 3) * 64 + lane * 2 + i;
-        Lx3[base] = z.x + z.y;
-        Lx3[base + 64] = z.x;
-        Lx3[base + 128] = z.y;
     }
-    // zero pad after the last block (the kernel's prefetch may run 3 micro-steps past the last task)
-    const size_t body = total_in * 3;
+    // zero pad after the last block (the register prefetch runs up to DA k-steps past a warp's last task)
+    const size_t body = total_in * 2;
     for (size_t idx = body + blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total_out; idx += (size_t)gridDim.x * blockDim.x)
-        Lx3[idx] = 0.0;
+        Lxc[idx] = 0.0;
 }
 
 }  // namespace
 
-size_t afqmc_i_lx3_doubles(const Dims& d) {
-    const int KS3 = (d.m + 3) / 4;
-    return (size_t)d.Nk * d.Nk * d.NAG * d.GQ * KS3 * 3 * 64 + AFQMC_LX_PAD;
+size_t afqmc_i_lxc_doubles(const Dims& d) {
+    const X3Geom g = x3_geom(d.m);
+    return (size_t)d.Nk * d.Nk * d.NAG * d.GQ * g.KSPT * 128 + AFQMC_LX_PAD;
 }
 
-int afqmc_i_pack_lx3(afqmc_ctx* c, const double2* L, cudaStream_t st) {
+int afqmc_i_pack_lxc(afqmc_ctx* c, cudaStream_t st) {
     const Dims& d = c->d;
-    const int KS3 = (d.m + 3) / 4;
-    const size_t total_in = (size_t)d.Nk * d.Nk * d.NAG * d.GQ * KS3 * 64;
-    const size_t total_out = afqmc_i_lx3_doubles(d);
-    size_t g = (total_in + 255) / 256;
-    if (g > 148 * 64) g = 148 * 64;
-    pack_Lx3_kernel<<<(unsigned)g, 256, 0, st>>>(d, KS3, L, c->psi_t, c->Lx3, total_in, total_out);
+    const X3Geom g = x3_geom(d.m);
+    const size_t total_in = (size_t)d.Nk * d.Nk * d.NAG * d.GQ * g.KSPT * 64;
+    size_t nb = (total_in + 255) / 256;
+    if (nb > 148 * 64) nb = 148 * 64;
+    pack_Lxc_kernel<<<(unsigned)nb, 256, 0, st>>>(d, g, c->Lh, c->Lxc, total_in, afqmc_i_lxc_doubles(d));
     AFQMC_LAUNCH_CHECK(c);
     return AFQMC_OK;
 }
 
 namespace {
 
-// CTA = (unit, group of 2*NP walkers), WPC warps; see the header comment.  n <= 4 only (NAG == 1).
-// DA = micro-steps of register prefetch of the A (Lx3, L2-resident) stream: 3 or 6; B (shared memory) runs 3 ahead.
-template <int NP, int WPC, int MINB, int DA>
-__global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_kernel(
-    Dims d, int KS3, int nw, const int* __restrict__ units, const int* __restrict__ kminus, const int* __restrict__ kplus,
-    const int* __restrict__ kneg, const double* __restrict__ Lx3, const double2* __restrict__ theta,
-    double2* __restrict__ partial) {
-    extern __shared__ __align__(16) double ex3_smem[];
-    constexpr int NWC = 2 * NP;                      // walkers of this CTA
+// B fragments of NP n-tiles for one lane and micro-step sit next to each other: [ms][jp][lane][W], W = min(NP,2) doubles
+template <int NP> struct BVec { static constexpr int W = NP >= 2 ? 2 : 1, NPH = NP / W; };
+
+// CTA = (unit, group of 2*NP walkers[, pair of a-groups, chunk of gamma-quads]); 2*NPAIR warps; see the header comment.
+//   GRIDPAIRS = false: the theta blocks of ALL a-groups are staged and the CTA loops over the (ag,bg) pairs (n <= 4: one pair);
+//   GRIDPAIRS = true : the (ag,bg) pair and a chunk of the gamma-quads come from the grid and only the theta rows of those two
+//                      groups are staged (blocks too large for shared memory: many orbitals / bands per k-point, e.g. the
+//                      Gamma-point supercell shape); a unit then contributes NAG^2 * nchunk partial sums.
+// DA = k-steps of register prefetch of the Lxc stream (L2 resident); the B fragments (shared memory) run one k-step ahead.
+template <int NP, int NPAIR, int DA, int MINB, bool GRIDPAIRS>
+__global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
+    Dims d, X3Geom g, int nchunk, int nw, const int* __restrict__ units, const int* __restrict__ kminus,
+    const int* __restrict__ kplus, const int* __restrict__ kneg, const double* __restrict__ Lxc,
+    const double2* __restrict__ theta, double2* __restrict__ partial) {
+    extern __shared__ __align__(16) double x3_smem[];
+    constexpr int NWC = 2 * NP, NWARP = 2 * NPAIR, NBUF = 2;
+    constexpr int W = BVec<NP>::W, NPH = BVec<NP>::NPH;
     const int nwg = (nw + NWC - 1) / NWC;            // walker groups of one unit are adjacent in the grid
-    const int u = blockIdx.x / nwg, w0 = (blockIdx.x % nwg) * NWC;
+    const int NAG = d.NAG, GQ = d.GQ, npairs = NAG * NAG;
+    int bx = blockIdx.x, chunk = 0, ab0 = 0, ab1 = npairs;
+    if (GRIDPAIRS) {                                  // blockIdx.x = ((u * nwg + walker group) * npairs + ab) * nchunk + chunk
+        chunk = bx % nchunk; bx /= nchunk;
+        ab0 = bx % npairs; bx /= npairs;
+        ab1 = ab0 + 1;
+    }
+    const int w0 = (bx % nwg) * NWC, u = bx / nwg;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, pair = warp >> 1, h = warp & 1;
+    double pair_weight = 1.0;
+    if (GRIDPAIRS) {
+        // A unit that is its own partner under (Q,k,k2) -> (-Q,k2,k) (multiplicity 1; every unit at the Gamma point) has
+        // T2 = T1, so the pairs (ag,bg) and (bg,ag) contribute equally: compute ag <= bg only, twice for ag < bg.
+        const int ag = ab0 / NAG, bg = ab0 % NAG;
+        const bool self_unit = units[4 * u + 3] == 1;
+        if (self_unit && ag > bg) {
+            if (tid < NWC && w0 + tid < nw)
+                partial[(((size_t)u * npairs + ab0) * nchunk + chunk) * nw + w0 + tid] = make_double2(0.0, 0.0);
+            return;
+        }
+        if (self_unit && ag < bg) pair_weight = 2.0;
+    }
     const int Q = units[4 * u], k = units[4 * u + 1], k2 = units[4 * u + 2];
     const int mQ = kneg[Q];
-    const int kq = kminus[k * d.Nk + Q];        // k - Q   : column block of theta for T^Q rows k
-    const int k2pq = kplus[k2 * d.Nk + Q];      // k2 + Q  : column block of theta for T^{-Q} rows k2
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int GQ = d.GQ, MS = 3 * KS3;              // micro-steps of one task
-    // Bs[which][ms][j][lane]: which = 0 -> theta[(k2,b),(k-Q,r)], 1 -> theta[(k,a),(k2+Q,s)]
-    constexpr int bs_step = NP * 32;
-    const int bs_half = MS * bs_step;
+    const int kq = kminus[k * d.Nk + Q];        // k - Q   : column block of theta for T1
+    const int k2pq = kplus[k2 * d.Nk + Q];      // k2 + Q  : column block of theta for T2
+    const int NGS = GRIDPAIRS ? 1 : NAG;        // a-group slots staged per theta block
+    constexpr int bs_step = 32 * NP;            // doubles of one micro-step
+    const int bs_grp = (g.MSPT + 1) * bs_step;  // +1: the k-step before a tail prefetches a third micro-step that does not exist
+    const int bs_half = NGS * bs_grp;
+    double* Bs = x3_smem;                       // Bs[which][slot][ms][jp][lane][W]: which 0 -> theta[(k2,b),(k-Q,r)], 1 -> theta[(k,a),(k2+Q,s)]
+    double2* xbuf = reinterpret_cast<double2*>(x3_smem + 2 * bs_half);      // [pair][role][NBUF][NP][64] hand-over tiles
 
-    // ---- this warp's contiguous share of the gamma-quads ----
-    const int t_begin = (int)((long long)warp * GQ / WPC), t_end = (int)((long long)(warp + 1) * GQ / WPC);
-    const int total = (t_end - t_begin) * MS;                       // micro-steps of this warp (a multiple of 3)
-    const size_t task_doubles = (size_t)MS * 64;
-    const double2* la1 = reinterpret_cast<const double2*>(Lx3 + (((size_t)Q * d.Nk + k) * GQ + t_begin) * task_doubles) + lane;
-    const double2* la2 = reinterpret_cast<const double2*>(Lx3 + (((size_t)mQ * d.Nk + k2) * GQ + t_begin) * task_doubles) + lane;
-    const double* lb1 = ex3_smem + lane;
-    const double* lb2 = ex3_smem + bs_half + lane;
-    int ls = 0;
-    auto loader_advance = [&]() {        // A is contiguous across micro-steps and tasks, B wraps every MS micro-steps
-        const bool wrap = ++ls == MS;
-        const int db = wrap ? -(MS - 1) * bs_step : bs_step;
-        lb1 += db; lb2 += db;
-        ls = wrap ? 0 : ls;
+    // ---- this warp's share of the gamma-quads (both warps of a pair walk the same tasks) ----
+    const int q_begin = (int)((long long)chunk * GQ / nchunk), q_end = (int)((long long)(chunk + 1) * GQ / nchunk);
+    const int t_begin = q_begin + (int)((long long)pair * (q_end - q_begin) / NPAIR);
+    const int t_end = q_begin + (int)((long long)(pair + 1) * (q_end - q_begin) / NPAIR);
+    const int total = (t_end - t_begin) * g.KSPT;                 // k-steps of this warp per (ag,bg) pair
+    const size_t blk = h == 0 ? (size_t)Q * d.Nk + k : (size_t)mQ * d.Nk + k2;
+    auto stream_ptr = [&](int grp) {            // 2 double2 per lane and k-step; k-step stride 64 double2
+        return reinterpret_cast<const double2*>(Lxc + (((blk * NAG + grp) * GQ + t_begin) * (size_t)g.KSPT) * 128) + lane * 2;
     };
-    static_assert(DA == 3 || DA == 6, "A depth is a multiple of the three products");
-    double2 fa1[DA], fa2[DA];
-    double fb1[3][NP], fb2[3][NP];
-    // A prologue: issued before the staging below, which hides the L2 round trip
+    double2 fa[DA][2];
+    const double2* pa = stream_ptr(h == 0 ? ab0 / NAG : ab0 % NAG);
+    // prologue of the first pair's A stream: issued before the staging below, which hides the L2 round trip
 #pragma unroll
     for (int q = 0; q < DA; ++q) {
-        fa1[q] = fa2[q] = make_double2(0.0, 0.0);
-        if (total > 0) { fa1[q] = __ldg(la1 + q * 32); fa2[q] = __ldg(la2 + q * 32); }
+        fa[q][0] = fa[q][1] = make_double2(0.0, 0.0);
+        if (total > 0) { fa[q][0] = __ldg(pa + q * 64); fa[q][1] = __ldg(pa + q * 64 + 1); }
     }
-    la1 += DA * 32; la2 += DA * 32;
 
-    // ---- stage the B fragments: one thread per complex theta element (b, walker, r) ----
-    //   lane of a B fragment = (col << 2) | kk,  col = 4*(w&1) + b,  kk = r & 3;  micro-step = 3*(r>>2) + prod
+    // ---- stage the B fragments: one thread per complex theta element (orbital, walker, r) ----
+    //   lane of a B fragment = (col << 2) | kk,  col = 4*(w&1) + orbital;  n-tile j = walker >> 1
     {
-        const int per_which = 4 * NWC * 4 * KS3;
-        for (int e = tid; e < 2 * per_which; e += 32 * WPC) {
-            const int which = e / per_which;
-            int x = e - which * per_which;
-            const int b = x & 3; x >>= 2;
-            const int wl = x % NWC, r = x / NWC;                 // r < 4*KS3
-            const int w = w0 + wl;
-            const int rowblk = which == 0 ? k2 : k, colblk = which == 0 ? kq : k2pq;
-            double2 v = make_double2(0.0, 0.0);
-            if (b < d.n && w < nw && r < d.m)
-                v = __ldg(theta + ((size_t)w * d.N + rowblk * d.n + b) * d.M + (size_t)colblk * d.m + r);
-            double* dst = ex3_smem + which * bs_half + ((3 * (r >> 2)) * NP + (wl >> 1)) * 32 + (((wl & 1) * 4 + b) << 2) + (r & 3);
-            dst[0] = v.x;
-            dst[bs_step] = v.y - v.x;
-            dst[2 * bs_step] = v.x + v.y;
-        }
-    }
-    __syncthreads();   // B fragments staged
-
-    // B prologue, and bring the loader state to micro-step 3
-#pragma unroll
-    for (int q = 0; q < 3; ++q) {
-#pragma unroll
-        for (int j = 0; j < NP; ++j) { fb1[q][j] = lb1[j * 32]; fb2[q][j] = lb2[j * 32]; }
-        loader_advance();
-    }
-
-    double er[NP], ei[NP];
-#pragma unroll
-    for (int j = 0; j < NP; ++j) er[j] = ei[j] = 0.0;
-    // lane geometry of the C fragments (row = lane>>2, columns 2c+e with c = lane&3, register e):
-    //   T1   : row (gamma of pair g, a),   columns (walker of pair wp = c>>1, b = 2(c&1)+e)
-    //   T2^T : row (walker of pair wp, a), columns (gamma of pair g = c>>1,  b = 2(c&1)+e)
-    // The contraction sum_{a,b} T1[(g,a),(wp,b)] T2[(g,b),(wp,a)] = sum T1[(g,a),(wp,b)] T2^T[(wp,a),(g,b)] pairs
-    // register e of lane (g, a | wp, c&1) with register e of lane (wp, a | g, c&1): lane bits 4 and 1 exchanged.
-    const int srcl = (lane & ~0x12) | ((lane & 16) >> 3) | ((lane & 2) << 3);
-    double acc1[3][2][NP][2], acc2[3][2][NP][2];
-#pragma unroll
-    for (int p = 0; p < 3; ++p)
-#pragma unroll
-        for (int i = 0; i < 2; ++i)
-#pragma unroll
-            for (int j = 0; j < NP; ++j)
-                acc1[p][i][j][0] = acc1[p][i][j][1] = acc2[p][i][j][0] = acc2[p][i][j][1] = 0.0;
-
-    int cs = 0;   // micro-step of the compute state inside its task
-    auto mstep = [&](const int qa) {     // A buffer qa; product and B buffer q = qa % 3
-        const int q = qa % 3;
-#pragma unroll
-        for (int j = 0; j < NP; ++j) {
-            dmma884(acc1[q][0][j][0], acc1[q][0][j][1], fa1[qa].x, fb1[q][j]);
-            dmma884(acc1[q][1][j][0], acc1[q][1][j][1], fa1[qa].y, fb1[q][j]);
-        }
-        // partner tile with the operands swapped: theta is the A fragment and Lh the B fragment (their lane
-        // layouts coincide), so the result is T2^T with rows (walker of pair, a) and columns (gamma of pair, b)
-#pragma unroll
-        for (int j = 0; j < NP; ++j) {
-            dmma884(acc2[q][0][j][0], acc2[q][0][j][1], fb2[q][j], fa2[qa].x);
-            dmma884(acc2[q][1][j][0], acc2[q][1][j][1], fb2[q][j], fa2[qa].y);
-        }
-        // refill the buffers with the micro-steps DA (A) and 3 (B) ahead (may run past the warp's last task:
-        // loaded, never used)
-        fa1[qa] = __ldg(la1); fa2[qa] = __ldg(la2);
-        la1 += 32; la2 += 32;
-#pragma unroll
-        for (int j = 0; j < NP; ++j) { fb1[q][j] = lb1[j * 32]; fb2[q][j] = lb2[j * 32]; }
-        loader_advance();
-        if (q == 2) {
-            cs += 3;
-            if (cs == MS) {
-                cs = 0;
-#pragma unroll
-                for (int i = 0; i < 2; ++i)
-#pragma unroll
-                    for (int j = 0; j < NP; ++j) {
-                        double t1r[2], t1i[2], t2r[2], t2i[2];
-#pragma unroll
-                        for (int e = 0; e < 2; ++e) {
-                            t1r[e] = acc1[0][i][j][e] - acc1[2][i][j][e];
-                            t1i[e] = acc1[0][i][j][e] + acc1[1][i][j][e];
-                            t2r[e] = acc2[0][i][j][e] - acc2[2][i][j][e];
-                            t2i[e] = acc2[0][i][j][e] + acc2[1][i][j][e];
-                        }
-                        // T1 lane (g, a | wp, bp) pairs with T2^T lane (wp, a | g, bp), same register: swap lane bits 4 and 1
-                        const double pr0 = __shfl_sync(0xffffffffu, t2r[0], srcl), pi0 = __shfl_sync(0xffffffffu, t2i[0], srcl);
-                        const double pr1 = __shfl_sync(0xffffffffu, t2r[1], srcl), pi1 = __shfl_sync(0xffffffffu, t2i[1], srcl);
-                        er[j] = fma(t1r[0], pr0, er[j]); er[j] = fma(-t1i[0], pi0, er[j]);
-                        ei[j] = fma(t1r[0], pi0, ei[j]); ei[j] = fma(t1i[0], pr0, ei[j]);
-                        er[j] = fma(t1r[1], pr1, er[j]); er[j] = fma(-t1i[1], pi1, er[j]);
-                        ei[j] = fma(t1r[1], pi1, ei[j]); ei[j] = fma(t1i[1], pr1, ei[j]);
-#pragma unroll
-                        for (int p = 0; p < 3; ++p)
-                            acc1[p][i][j][0] = acc1[p][i][j][1] = acc2[p][i][j][0] = acc2[p][i][j][1] = 0.0;
-                    }
-            }
-        }
-    };
-    for (int g0 = 0; g0 < total; g0 += 3) {
-        mstep(0); mstep(1); mstep(2);
-        if (DA == 6) {
-            if (g0 + 3 >= total) break;
-            g0 += 3;
-            mstep(DA - 3); mstep(DA - 2); mstep(DA - 1);
-        }
-    }
-
-    // ---- reduce over the lanes of each walker-in-pair (lane bit 1), then over warps (deterministic) ----
-    __syncthreads();
-    double* red = ex3_smem;   // reuse: [warp][NWC][2]
-#pragma unroll
-    for (int j = 0; j < NP; ++j) {
-        double r = er[j], i = ei[j];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            if (o == 2) continue;
-            r += __shfl_xor_sync(0xffffffffu, r, o);
-            i += __shfl_xor_sync(0xffffffffu, i, o);
-        }
-        if (lane == 0 || lane == 2) {
-            const int wl = 2 * j + (lane >> 1);
-            red[(warp * NWC + wl) * 2] = r; red[(warp * NWC + wl) * 2 + 1] = i;
-        }
-    }
-    __syncthreads();
-    if (tid < NWC && w0 + tid < nw) {
-        double r = 0.0, i = 0.0;
-        for (int x = 0; x < WPC; ++x) { r += red[(x * NWC + tid) * 2]; i += red[(x * NWC + tid) * 2 + 1]; }
-        partial[(size_t)u * nw + w0 + tid] = make_double2(r, i);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------------------
-// The same kernel for MORE THAN FOUR occupied orbitals per k-point (NAG = ceil(n/4) > 1 a-groups).  The (ag, bg)
-// pairs of a-groups are processed one after the other; inside a pair everything is as above (linear A streams of the
-// rows ag of Lh[Q][k] and bg of Lh[-Q][k2], B fragments of the theta rows bg of k2 and ag of k).  The theta blocks of
-// ALL groups are staged once per CTA: Bs[which][grp][ms][j][lane].
-// ---------------------------------------------------------------------------------------------------------------
-template <int NP, int WPC, int MINB>
-__global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_multi_kernel(
-    Dims d, int KS3, int nw, const int* __restrict__ units, const int* __restrict__ kminus, const int* __restrict__ kplus,
-    const int* __restrict__ kneg, const double* __restrict__ Lx3, const double2* __restrict__ theta,
-    double2* __restrict__ partial) {
-    extern __shared__ __align__(16) double ex3_smem[];
-    constexpr int NWC = 2 * NP;
-    const int nwg = (nw + NWC - 1) / NWC;
-    const int u = blockIdx.x / nwg, w0 = (blockIdx.x % nwg) * NWC;
-    const int Q = units[4 * u], k = units[4 * u + 1], k2 = units[4 * u + 2];
-    const int mQ = kneg[Q];
-    const int kq = kminus[k * d.Nk + Q];
-    const int k2pq = kplus[k2 * d.Nk + Q];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int GQ = d.GQ, NAG = d.NAG, MS = 3 * KS3;
-    constexpr int bs_step = NP * 32;
-    const int bs_grp = MS * bs_step, bs_half = NAG * bs_grp;
-    const size_t task_doubles = (size_t)MS * 64;
-
-    // ---- stage the B fragments of every a-group: one thread per complex theta element (orbital, walker, r) ----
-    {
-        const int per_which = NAG * 4 * NWC * 4 * KS3;
-        for (int e = tid; e < 2 * per_which; e += 32 * WPC) {
+        const int RP = 4 * g.KSF + 2 * g.TAIL;
+        const int per_which = NGS * 4 * NWC * RP;
+        for (int e = tid; e < 2 * per_which; e += 64 * NPAIR) {
             const int which = e / per_which;
             int x = e - which * per_which;
             const int b = x & 3; x >>= 2;
             const int wl = x % NWC; x /= NWC;
-            const int grp = x % NAG, r = x / NAG;                // r < 4*KS3
+            const int gs = x % NGS, r = x / NGS;
+            const int grp = GRIDPAIRS ? (which == 0 ? ab0 % NAG : ab0 / NAG) : gs;
             const int orb = 4 * grp + b, w = w0 + wl;
             const int rowblk = which == 0 ? k2 : k, colblk = which == 0 ? kq : k2pq;
             double2 v = make_double2(0.0, 0.0);
             if (orb < d.n && w < nw && r < d.m)
                 v = __ldg(theta + ((size_t)w * d.N + rowblk * d.n + orb) * d.M + (size_t)colblk * d.m + r);
-            double* dst = ex3_smem + which * bs_half + grp * bs_grp + ((3 * (r >> 2)) * NP + (wl >> 1)) * 32 +
-                          (((wl & 1) * 4 + b) << 2) + (r & 3);
-            dst[0] = v.x;
-            dst[bs_step] = v.y - v.x;
-            dst[2 * bs_step] = v.x + v.y;
+            const int j = wl >> 1, col = (wl & 1) * 4 + b;
+            double* base = Bs + which * bs_half + gs * bs_grp + (j / W) * (32 * W) + (j % W);    // + ms * bs_step + lane * W
+            if (r < 4 * g.KSF) {
+                double* dst = base + 3 * (r >> 2) * bs_step + ((col << 2) | (r & 3)) * W;
+                dst[0] = v.x;                       // Br
+                dst[bs_step] = v.y - v.x;           // Bi - Br
+                dst[2 * bs_step] = v.x + v.y;       // Br + Bi
+            } else {                                // tail: real embedding, lanes kk = 2t (times Ar) and 2t+1 (times Ai)
+                double* dst = base + 3 * g.KSF * bs_step + ((col << 2) | (2 * (r - 4 * g.KSF))) * W;
+                dst[0] = v.x;  dst[W] = -v.y;                               // -> P0:  Ar Br - Ai Bi
+                dst[bs_step] = v.y - v.x;  dst[bs_step + W] = v.x + v.y;    // -> P1:  Ar (Bi-Br) + Ai (Br+Bi)
+            }
         }
     }
-    __syncthreads();
+    __syncthreads();   // B fragments staged
 
-    const int t_begin = (int)((long long)warp * GQ / WPC), t_end = (int)((long long)(warp + 1) * GQ / WPC);
-    const int total = (t_end - t_begin) * MS;
-    const int srcl = (lane & ~0x12) | ((lane & 16) >> 3) | ((lane & 2) << 3);
+    // lane geometry of a C fragment (row = lane>>2, columns 2c+e, c = lane&3, register e):
+    //   rows (gl = row>>2: gamma of the tile's pair, orow = row&3: this warp's ROW orbital), columns (wp = c>>1: walker of the
+    //   pair, ocol = 2(c&1)+e: the COLUMN orbital).  T1: orow = a, ocol = b;  T2: orow = b, ocol = a.
+    const int gl = lane >> 4, orow = (lane >> 2) & 3, wp = (lane >> 1) & 1, cb = lane & 1;
+    const int idx_w = gl * 32 + orow * 8 + wp * 4 + 2 * cb;       // hand-over slot of (this lane, e = 0); e = 1 is the next one
+    const int idx_r = gl * 32 + (2 * cb) * 8 + wp * 4 + orow;     // partner element [(gamma, ocol), (w, orow)] for e = 0; e = 1: + 8
     double er[NP], ei[NP];
 #pragma unroll
     for (int j = 0; j < NP; ++j) er[j] = ei[j] = 0.0;
+    int buf = 0;
 
-    for (int ab = 0; ab < NAG * NAG; ++ab) {
+    for (int ab = ab0; ab < ab1; ++ab) {
         const int ag = ab / NAG, bg = ab % NAG;
-        const double2* la1 = reinterpret_cast<const double2*>(Lx3 + ((((size_t)Q * d.Nk + k) * NAG + ag) * GQ + t_begin) * task_doubles) + lane;
-        const double2* la2 = reinterpret_cast<const double2*>(Lx3 + ((((size_t)mQ * d.Nk + k2) * NAG + bg) * GQ + t_begin) * task_doubles) + lane;
-        const double* lb1 = ex3_smem + bg * bs_grp + lane;                 // theta rows bg of k2
-        const double* lb2 = ex3_smem + bs_half + ag * bs_grp + lane;       // theta rows ag of k
-        int ls = 0;
-        auto loader_advance = [&]() {
-            const bool wrap = ++ls == MS;
-            const int db = wrap ? -(MS - 1) * bs_step : bs_step;
-            lb1 += db; lb2 += db;
-            ls = wrap ? 0 : ls;
-        };
-        double2 fa1[3], fa2[3];
-        double fb1[3][NP], fb2[3][NP];
+        if (ab != ab0) {                         // next pair of a-groups: restart the A stream
+            pa = stream_ptr(h == 0 ? ag : bg);
 #pragma unroll
-        for (int q = 0; q < 3; ++q) {
-            fa1[q] = fa2[q] = make_double2(0.0, 0.0);
-            if (total > 0) { fa1[q] = __ldg(la1 + q * 32); fa2[q] = __ldg(la2 + q * 32); }
-#pragma unroll
-            for (int j = 0; j < NP; ++j) { fb1[q][j] = lb1[j * 32]; fb2[q][j] = lb2[j * 32]; }
-            loader_advance();
+            for (int q = 0; q < DA; ++q)
+                if (total > 0) { fa[q][0] = __ldg(pa + q * 64); fa[q][1] = __ldg(pa + q * 64 + 1); }
         }
-        la1 += 96; la2 += 96;
-        double acc1[3][2][NP][2], acc2[3][2][NP][2];
+        pa += DA * 64;
+        // T1 needs theta rows bg of k2 (which 0), T2 theta rows ag of k (which 1)
+        const double* pb = Bs + h * bs_half + (GRIDPAIRS ? 0 : (h == 0 ? bg : ag)) * bs_grp + lane * W;
+        double fb[3][NP];
+        auto load_b = [&](const int p, const int ms0) {       // B fragments of micro-step ms0 + p into buffer p
+            const double* src = pb + (ms0 + p) * bs_step;
+#pragma unroll
+            for (int jp = 0; jp < NPH; ++jp) {
+                if (W == 2) {
+                    const double2 v = *reinterpret_cast<const double2*>(src + jp * 64);
+                    fb[p][2 * jp] = v.x; fb[p][2 * jp + (NP > 1 ? 1 : 0)] = v.y;
+                } else {
+                    fb[p][jp] = src[jp * 32];
+                }
+            }
+        };
+        load_b(0, 0); load_b(1, 0); load_b(2, 0);
+        double acc[3][2][NP][2];
 #pragma unroll
         for (int p = 0; p < 3; ++p)
 #pragma unroll
             for (int i = 0; i < 2; ++i)
 #pragma unroll
-                for (int j = 0; j < NP; ++j)
-                    acc1[p][i][j][0] = acc1[p][i][j][1] = acc2[p][i][j][0] = acc2[p][i][j][1] = 0.0;
-        int cs = 0;
-        auto mstep = [&](const int q) {
+                for (int j = 0; j < NP; ++j) acc[p][i][j][0] = acc[p][i][j][1] = 0.0;
+
+        // end of a task: combine the three products, hand tile GIVE to the partner warp, contract tile KEEP
+        auto finish_task = [&](auto KEEP_) {
+            constexpr int KEEP = decltype(KEEP_)::value, GIVE = 1 - KEEP;
+            double2* xw = xbuf + (((pair * 2 + h) * NBUF + buf) * NP) * 64 + idx_w;
 #pragma unroll
             for (int j = 0; j < NP; ++j) {
-                dmma884(acc1[q][0][j][0], acc1[q][0][j][1], fa1[q].x, fb1[q][j]);
-                dmma884(acc1[q][1][j][0], acc1[q][1][j][1], fa1[q].y, fb1[q][j]);
+                xw[j * 64] = make_double2(acc[0][GIVE][j][0] - acc[2][GIVE][j][0], acc[0][GIVE][j][0] + acc[1][GIVE][j][0]);
+                xw[j * 64 + 1] = make_double2(acc[0][GIVE][j][1] - acc[2][GIVE][j][1], acc[0][GIVE][j][1] + acc[1][GIVE][j][1]);
             }
+            asm volatile("bar.sync %0, 64;" ::"r"(pair + 1) : "memory");       // the two warps of the pair
+            const double2* xr = xbuf + (((pair * 2 + (h ^ 1)) * NBUF + buf) * NP) * 64 + idx_r;
 #pragma unroll
-            for (int j = 0; j < NP; ++j) {
-                dmma884(acc2[q][0][j][0], acc2[q][0][j][1], fb2[q][j], fa2[q].x);
-                dmma884(acc2[q][1][j][0], acc2[q][1][j][1], fb2[q][j], fa2[q].y);
-            }
-            fa1[q] = __ldg(la1); fa2[q] = __ldg(la2);      // may run up to 3 micro-steps past this pair's last task
-            la1 += 32; la2 += 32;
+            for (int j = 0; j < NP; ++j)
 #pragma unroll
-            for (int j = 0; j < NP; ++j) { fb1[q][j] = lb1[j * 32]; fb2[q][j] = lb2[j * 32]; }
-            loader_advance();
-            if (q == 2) {
-                cs += 3;
-                if (cs == MS) {
-                    cs = 0;
-#pragma unroll
-                    for (int i = 0; i < 2; ++i)
-#pragma unroll
-                        for (int j = 0; j < NP; ++j) {
-                            double t1r[2], t1i[2], t2r[2], t2i[2];
-#pragma unroll
-                            for (int e = 0; e < 2; ++e) {
-                                t1r[e] = acc1[0][i][j][e] - acc1[2][i][j][e];
-                                t1i[e] = acc1[0][i][j][e] + acc1[1][i][j][e];
-                                t2r[e] = acc2[0][i][j][e] - acc2[2][i][j][e];
-                                t2i[e] = acc2[0][i][j][e] + acc2[1][i][j][e];
-                            }
-                            const double pr0 = __shfl_sync(0xffffffffu, t2r[0], srcl), pi0 = __shfl_sync(0xffffffffu, t2i[0], srcl);
-                            const double pr1 = __shfl_sync(0xffffffffu, t2r[1], srcl), pi1 = __shfl_sync(0xffffffffu, t2i[1], srcl);
-                            er[j] = fma(t1r[0], pr0, er[j]); er[j] = fma(-t1i[0], pi0, er[j]);
-                            ei[j] = fma(t1r[0], pi0, ei[j]); ei[j] = fma(t1i[0], pr0, ei[j]);
-                            er[j] = fma(t1r[1], pr1, er[j]); er[j] = fma(-t1i[1], pi1, er[j]);
-                            ei[j] = fma(t1r[1], pi1, ei[j]); ei[j] = fma(t1i[1], pr1, ei[j]);
-#pragma unroll
-                            for (int p = 0; p < 3; ++p)
-                                acc1[p][i][j][0] = acc1[p][i][j][1] = acc2[p][i][j][0] = acc2[p][i][j][1] = 0.0;
-                        }
+                for (int e = 0; e < 2; ++e) {
+                    const double tr = acc[0][KEEP][j][e] - acc[2][KEEP][j][e], ti = acc[0][KEEP][j][e] + acc[1][KEEP][j][e];
+                    const double2 p = xr[j * 64 + e * 8];
+                    er[j] = fma(tr, p.x, er[j]); er[j] = fma(-ti, p.y, er[j]);
+                    ei[j] = fma(tr, p.y, ei[j]); ei[j] = fma(ti, p.x, ei[j]);
                 }
+#pragma unroll
+            for (int p = 0; p < 3; ++p)
+#pragma unroll
+                for (int i = 0; i < 2; ++i)
+#pragma unroll
+                    for (int j = 0; j < NP; ++j) acc[p][i][j][0] = acc[p][i][j][1] = 0.0;
+            buf ^= 1;      // two hand-over buffers: the partner may still read this one while the next task is written
+        };
+
+        int cs = 0;   // k-step of the compute state inside its task
+        auto kstep = [&](auto Q_) {
+            constexpr int q = decltype(Q_)::value;
+            const double2 x0 = fa[q][0], x1 = fa[q][1];
+            const int nxt = (cs + 1 == g.KSPT) ? 0 : 3 * (cs + 1);      // first micro-step of the next k-step (wraps at the task end)
+            if (cs < g.KSF) {
+                const double s0 = x0.x + x0.y, s1 = x1.x + x1.y;        // Ar + Ai
+#pragma unroll
+                for (int j = 0; j < NP; ++j) {
+                    dmma884(acc[0][0][j][0], acc[0][0][j][1], s0, fb[0][j]);
+                    dmma884(acc[0][1][j][0], acc[0][1][j][1], s1, fb[0][j]);
+                }
+                load_b(0, nxt);
+#pragma unroll
+                for (int j = 0; j < NP; ++j) {
+                    dmma884(acc[1][0][j][0], acc[1][0][j][1], x0.x, fb[1][j]);
+                    dmma884(acc[1][1][j][0], acc[1][1][j][1], x1.x, fb[1][j]);
+                }
+                load_b(1, nxt);
+#pragma unroll
+                for (int j = 0; j < NP; ++j) {
+                    dmma884(acc[2][0][j][0], acc[2][0][j][1], x0.y, fb[2][j]);
+                    dmma884(acc[2][1][j][0], acc[2][1][j][1], x1.y, fb[2][j]);
+                }
+                load_b(2, nxt);
+            } else {                                                     // tail k-step: x0 = (tile 0, tile 1) real-embedded
+#pragma unroll
+                for (int j = 0; j < NP; ++j) {
+                    dmma884(acc[0][0][j][0], acc[0][0][j][1], x0.x, fb[0][j]);
+                    dmma884(acc[0][1][j][0], acc[0][1][j][1], x0.y, fb[0][j]);
+                }
+                load_b(0, nxt);
+#pragma unroll
+                for (int j = 0; j < NP; ++j) {
+                    dmma884(acc[1][0][j][0], acc[1][0][j][1], x0.x, fb[1][j]);
+                    dmma884(acc[1][1][j][0], acc[1][1][j][1], x0.y, fb[1][j]);
+                }
+                load_b(1, nxt);
+                load_b(2, nxt);
+            }
+            // refill this ring slot with the k-step DA ahead (may run past the warp's last task: loaded, never used)
+            fa[q][0] = __ldg(pa); fa[q][1] = __ldg(pa + 1);
+            pa += 64;
+            if (++cs == g.KSPT) {
+                cs = 0;
+                if (h == 0) finish_task(std::integral_constant<int, 0>());
+                else finish_task(std::integral_constant<int, 1>());
             }
         };
-        for (int g0 = 0; g0 < total; g0 += 3) { mstep(0); mstep(1); mstep(2); }
+        const int nfull = total - total % DA;
+        for (int g0 = 0; g0 < nfull; g0 += DA) {
+            kstep(std::integral_constant<int, 0>());
+            if (DA > 1) kstep(std::integral_constant<int, 1 % DA>());
+            if (DA > 2) kstep(std::integral_constant<int, 2 % DA>());
+            if (DA > 3) kstep(std::integral_constant<int, 3 % DA>());
+        }
+        if (nfull + 0 < total) kstep(std::integral_constant<int, 0>());
+        if (DA > 2 && nfull + 1 < total) kstep(std::integral_constant<int, 1 % DA>());
+        if (DA > 3 && nfull + 2 < total) kstep(std::integral_constant<int, 2 % DA>());
     }
 
+    // ---- reduce over the lanes of each walker-in-pair (lane bit 1 = wp), then over warps (deterministic) ----
     __syncthreads();
-    double* red = ex3_smem;
+    double* red = x3_smem;   // reuse: [warp][NWC][2]
 #pragma unroll
     for (int j = 0; j < NP; ++j) {
         double r = er[j], i = ei[j];
@@ -419,262 +356,79 @@ __global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_multi_kernel(
     __syncthreads();
     if (tid < NWC && w0 + tid < nw) {
         double r = 0.0, i = 0.0;
-        for (int x = 0; x < WPC; ++x) { r += red[(x * NWC + tid) * 2]; i += red[(x * NWC + tid) * 2 + 1]; }
-        partial[(size_t)u * nw + w0 + tid] = make_double2(r, i);
+        for (int x = 0; x < NWARP; ++x) { r += red[(x * NWC + tid) * 2]; i += red[(x * NWC + tid) * 2 + 1]; }
+        const size_t slot = GRIDPAIRS ? ((size_t)u * npairs + ab0) * nchunk + chunk : (size_t)u;
+        partial[slot * nw + w0 + tid] = make_double2(pair_weight * r, pair_weight * i);
     }
 }
 
-// ---------------------------------------------------------------------------------------------------------------
-// The variant for LARGE blocks (the theta blocks of all a-groups of a unit do not fit shared memory: many occupied
-// orbitals and/or bands per k-point, e.g. the dense Gamma-point supercell shape of SURVEY.md 8(f) NEXT-4).  The pair
-// (ag, bg) of a-groups and a chunk of the gamma-quads move from loops inside the CTA into the grid: a CTA stages only
-// the theta rows of its two groups, and a unit contributes NAG^2 * nchunk partial sums (summed by the finalisation).
-// ---------------------------------------------------------------------------------------------------------------
-template <int NP, int WPC, int MINB>
-__global__ void __launch_bounds__(32 * WPC, MINB) exchange3m_big_kernel(
-    Dims d, int KS3, int nchunk, int nw, const int* __restrict__ units, const int* __restrict__ kminus, const int* __restrict__ kplus,
-    const int* __restrict__ kneg, const double* __restrict__ Lx3, const double2* __restrict__ theta,
-    double2* __restrict__ partial) {
-    extern __shared__ __align__(16) double ex3_smem[];
-    constexpr int NWC = 2 * NP;
-    const int nwg = (nw + NWC - 1) / NWC;
-    const int npairs = d.NAG * d.NAG;
-    // blockIdx.x = ((u * nwg + walker group) * npairs + ab) * nchunk + chunk
-    int bx = blockIdx.x;
-    const int chunk = bx % nchunk; bx /= nchunk;
-    const int ab = bx % npairs; bx /= npairs;
-    const int w0 = (bx % nwg) * NWC, u = bx / nwg;
-    const int ag = ab / d.NAG, bg = ab % d.NAG;
-    // A unit that is its own partner under (Q,k,k2) -> (-Q,k2,k) (multiplicity 1; every unit at the Gamma point) has
-    // T2 = T1, so the contributions of the pairs (ag,bg) and (bg,ag) are equal: compute ag <= bg only, twice for ag < bg.
-    const bool self_unit = units[4 * u + 3] == 1;
-    if (self_unit && ag > bg) {
-        if (threadIdx.x < 2 * NP && w0 + (int)threadIdx.x < nw)
-            partial[(((size_t)u * npairs + ab) * nchunk + chunk) * nw + w0 + threadIdx.x] = make_double2(0.0, 0.0);
-        return;
-    }
-    const double pair_weight = (self_unit && ag < bg) ? 2.0 : 1.0;
-    const int Q = units[4 * u], k = units[4 * u + 1], k2 = units[4 * u + 2];
-    const int mQ = kneg[Q];
-    const int kq = kminus[k * d.Nk + Q];
-    const int k2pq = kplus[k2 * d.Nk + Q];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int GQ = d.GQ, NAG = d.NAG, MS = 3 * KS3;
-    (void)NAG;
-    constexpr int bs_step = NP * 32;
-    const int bs_half = MS * bs_step;
-    const size_t task_doubles = (size_t)MS * 64;
-
-    // ---- stage the B fragments of the two a-groups of this CTA: theta rows bg of k2 and rows ag of k ----
-    {
-        const int per_which = 4 * NWC * 4 * KS3;
-        for (int e = tid; e < 2 * per_which; e += 32 * WPC) {
-            const int which = e / per_which;
-            int x = e - which * per_which;
-            const int b = x & 3; x >>= 2;
-            const int wl = x % NWC, r = x / NWC;                 // r < 4*KS3
-            const int orb = 4 * (which == 0 ? bg : ag) + b, w = w0 + wl;
-            const int rowblk = which == 0 ? k2 : k, colblk = which == 0 ? kq : k2pq;
-            double2 v = make_double2(0.0, 0.0);
-            if (orb < d.n && w < nw && r < d.m)
-                v = __ldg(theta + ((size_t)w * d.N + rowblk * d.n + orb) * d.M + (size_t)colblk * d.m + r);
-            double* dst = ex3_smem + which * bs_half + ((3 * (r >> 2)) * NP + (wl >> 1)) * 32 + (((wl & 1) * 4 + b) << 2) + (r & 3);
-            dst[0] = v.x;
-            dst[bs_step] = v.y - v.x;
-            dst[2 * bs_step] = v.x + v.y;
-        }
-    }
-    __syncthreads();
-
-    const int q_begin = (int)((long long)chunk * GQ / nchunk), q_end = (int)((long long)(chunk + 1) * GQ / nchunk);
-    const int t_begin = q_begin + (int)((long long)warp * (q_end - q_begin) / WPC);
-    const int t_end = q_begin + (int)((long long)(warp + 1) * (q_end - q_begin) / WPC);
-    const int total = (t_end - t_begin) * MS;
-    const int srcl = (lane & ~0x12) | ((lane & 16) >> 3) | ((lane & 2) << 3);
-    double er[NP], ei[NP];
-#pragma unroll
-    for (int j = 0; j < NP; ++j) er[j] = ei[j] = 0.0;
-
-    {
-        const double2* la1 = reinterpret_cast<const double2*>(Lx3 + ((((size_t)Q * d.Nk + k) * NAG + ag) * GQ + t_begin) * task_doubles) + lane;
-        const double2* la2 = reinterpret_cast<const double2*>(Lx3 + ((((size_t)mQ * d.Nk + k2) * NAG + bg) * GQ + t_begin) * task_doubles) + lane;
-        const double* lb1 = ex3_smem + lane;                 // theta rows bg of k2
-        const double* lb2 = ex3_smem + bs_half + lane;       // theta rows ag of k
-        int ls = 0;
-        auto loader_advance = [&]() {
-            const bool wrap = ++ls == MS;
-            const int db = wrap ? -(MS - 1) * bs_step : bs_step;
-            lb1 += db; lb2 += db;
-            ls = wrap ? 0 : ls;
-        };
-        double2 fa1[3], fa2[3];
-        double fb1[3][NP], fb2[3][NP];
-#pragma unroll
-        for (int q = 0; q < 3; ++q) {
-            fa1[q] = fa2[q] = make_double2(0.0, 0.0);
-            if (total > 0) { fa1[q] = __ldg(la1 + q * 32); fa2[q] = __ldg(la2 + q * 32); }
-#pragma unroll
-            for (int j = 0; j < NP; ++j) { fb1[q][j] = lb1[j * 32]; fb2[q][j] = lb2[j * 32]; }
-            loader_advance();
-        }
-        la1 += 96; la2 += 96;
-        double acc1[3][2][NP][2], acc2[3][2][NP][2];
-#pragma unroll
-        for (int p = 0; p < 3; ++p)
-#pragma unroll
-            for (int i = 0; i < 2; ++i)
-#pragma unroll
-                for (int j = 0; j < NP; ++j)
-                    acc1[p][i][j][0] = acc1[p][i][j][1] = acc2[p][i][j][0] = acc2[p][i][j][1] = 0.0;
-        int cs = 0;
-        auto mstep = [&](const int q) {
-#pragma unroll
-            for (int j = 0; j < NP; ++j) {
-                dmma884(acc1[q][0][j][0], acc1[q][0][j][1], fa1[q].x, fb1[q][j]);
-                dmma884(acc1[q][1][j][0], acc1[q][1][j][1], fa1[q].y, fb1[q][j]);
-            }
-#pragma unroll
-            for (int j = 0; j < NP; ++j) {
-                dmma884(acc2[q][0][j][0], acc2[q][0][j][1], fb2[q][j], fa2[q].x);
-                dmma884(acc2[q][1][j][0], acc2[q][1][j][1], fb2[q][j], fa2[q].y);
-            }
-            fa1[q] = __ldg(la1); fa2[q] = __ldg(la2);      // may run up to 3 micro-steps past this pair's last task
-            la1 += 32; la2 += 32;
-#pragma unroll
-            for (int j = 0; j < NP; ++j) { fb1[q][j] = lb1[j * 32]; fb2[q][j] = lb2[j * 32]; }
-            loader_advance();
-            if (q == 2) {
-                cs += 3;
-                if (cs == MS) {
-                    cs = 0;
-#pragma unroll
-                    for (int i = 0; i < 2; ++i)
-#pragma unroll
-                        for (int j = 0; j < NP; ++j) {
-                            double t1r[2], t1i[2], t2r[2], t2i[2];
-#pragma unroll
-                            for (int e = 0; e < 2; ++e) {
-                                t1r[e] = acc1[0][i][j][e] - acc1[2][i][j][e];
-                                t1i[e] = acc1[0][i][j][e] + acc1[1][i][j][e];
-                                t2r[e] = acc2[0][i][j][e] - acc2[2][i][j][e];
-                                t2i[e] = acc2[0][i][j][e] + acc2[1][i][j][e];
-                            }
-                            const double pr0 = __shfl_sync(0xffffffffu, t2r[0], srcl), pi0 = __shfl_sync(0xffffffffu, t2i[0], srcl);
-                            const double pr1 = __shfl_sync(0xffffffffu, t2r[1], srcl), pi1 = __shfl_sync(0xffffffffu, t2i[1], srcl);
-                            er[j] = fma(t1r[0], pr0, er[j]); er[j] = fma(-t1i[0], pi0, er[j]);
-                            ei[j] = fma(t1r[0], pi0, ei[j]); ei[j] = fma(t1i[0], pr0, ei[j]);
-                            er[j] = fma(t1r[1], pr1, er[j]); er[j] = fma(-t1i[1], pi1, er[j]);
-                            ei[j] = fma(t1r[1], pi1, ei[j]); ei[j] = fma(t1i[1], pr1, ei[j]);
-#pragma unroll
-                            for (int p = 0; p < 3; ++p)
-                                acc1[p][i][j][0] = acc1[p][i][j][1] = acc2[p][i][j][0] = acc2[p][i][j][1] = 0.0;
-                        }
-                }
-            }
-        };
-        for (int g0 = 0; g0 < total; g0 += 3) { mstep(0); mstep(1); mstep(2); }
-    }
-
-    __syncthreads();
-    double* red = ex3_smem;
-#pragma unroll
-    for (int j = 0; j < NP; ++j) {
-        double r = er[j], i = ei[j];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            if (o == 2) continue;
-            r += __shfl_xor_sync(0xffffffffu, r, o);
-            i += __shfl_xor_sync(0xffffffffu, i, o);
-        }
-        if (lane == 0 || lane == 2) {
-            const int wl = 2 * j + (lane >> 1);
-            red[(warp * NWC + wl) * 2] = r; red[(warp * NWC + wl) * 2 + 1] = i;
-        }
-    }
-    __syncthreads();
-    if (tid < NWC && w0 + tid < nw) {
-        double r = 0.0, i = 0.0;
-        for (int x = 0; x < WPC; ++x) { r += red[(x * NWC + tid) * 2]; i += red[(x * NWC + tid) * 2 + 1]; }
-        partial[(((size_t)u * npairs + ab) * nchunk + chunk) * nw + w0 + tid] = make_double2(pair_weight * r, pair_weight * i);
-    }
+template <int NP>
+size_t x3_smem_bytes(const X3Geom& g, int NGS, int NPAIR) {
+    const size_t bs = (size_t)2 * NGS * (g.MSPT + 1) * 32 * NP * sizeof(double);
+    const size_t xb = (size_t)NPAIR * 2 * 2 * NP * 64 * sizeof(double2);
+    return bs + xb;
 }
 
-template <int NP, int WPC>
-int launch_exchange3m_big(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+template <int NP, int NPAIR, int DA, int MINB, bool GRIDPAIRS>
+int launch_x3(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     const Dims& d = c->d;
-    const int KS3 = (d.m + 3) / 4;
-    size_t smem = (size_t)2 * 3 * KS3 * NP * 32 * sizeof(double);
-    if (smem < (size_t)WPC * 2 * NP * 2 * sizeof(double)) smem = (size_t)WPC * 2 * NP * 2 * sizeof(double);
-    if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
-    auto kern = exchange3m_big_kernel<NP, WPC, 1>;
+    const X3Geom g = x3_geom(d.m);
+    const size_t smem = x3_smem_bytes<NP>(g, GRIDPAIRS ? 1 : d.NAG, NPAIR);
+    auto kern = exchange3m_kernel<NP, NPAIR, DA, MINB, GRIDPAIRS>;
     if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
     const int nwg = (nw + 2 * NP - 1) / (2 * NP), npairs = d.NAG * d.NAG;
-    // chunks of gamma-quads: enough CTAs for ~4 waves, every warp keeps at least 2 quads, at most ex_parts_max parts per unit
-    int nchunk = (int)((4LL * c->num_sms + (long long)c->nunits * nwg * npairs - 1) / ((long long)c->nunits * nwg * npairs));
-    if (nchunk > d.GQ / (2 * WPC)) nchunk = d.GQ / (2 * WPC);
-    if (nchunk * npairs > c->ex_parts_max) nchunk = c->ex_parts_max / npairs;
-    if (nchunk < 1) nchunk = 1;
-    if (npairs * nchunk > c->ex_parts_max) return AFQMC_UNSUPPORTED;
-    const long long nblocks = (long long)c->nunits * nwg * npairs * nchunk;
+    int nchunk = 1;
+    long long nblocks = (long long)c->nunits * nwg;
+    if (GRIDPAIRS) {
+        // chunks of gamma-quads: enough CTAs for ~4 waves, every warp pair keeps at least 2 quads, at most ex_parts_max parts per unit
+        nchunk = (int)((4LL * c->num_sms + nblocks * npairs - 1) / (nblocks * npairs));
+        if (nchunk > d.GQ / (2 * NPAIR)) nchunk = d.GQ / (2 * NPAIR);
+        if (nchunk * npairs > c->ex_parts_max) nchunk = c->ex_parts_max / npairs;
+        if (nchunk < 1) nchunk = 1;
+        if (npairs * nchunk > c->ex_parts_max) return AFQMC_UNSUPPORTED;
+        nblocks *= (long long)npairs * nchunk;
+    }
     if (nblocks > 0x7fffffffLL) return AFQMC_UNSUPPORTED;
-    kern<<<(unsigned)nblocks, 32 * WPC, smem, st>>>(d, KS3, nchunk, nw, c->units, c->kminus, c->kplus, c->kneg, c->Lx3, theta, c->ws_expart);
+    kern<<<(unsigned)nblocks, 64 * NPAIR, smem, st>>>(d, g, nchunk, nw, c->units, c->kminus, c->kplus, c->kneg, c->Lxc, theta, c->ws_expart);
     AFQMC_LAUNCH_CHECK(c);
-    c->ex_parts = npairs * nchunk;
+    c->ex_parts = GRIDPAIRS ? npairs * nchunk : 1;
     return AFQMC_OK;
 }
 
-template <int NP, int WPC, int MINB>
-int launch_exchange3m_multi(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
-    const Dims& d = c->d;
-    const int KS3 = (d.m + 3) / 4;
-    size_t smem = (size_t)2 * d.NAG * 3 * KS3 * NP * 32 * sizeof(double);
-    if (smem < (size_t)WPC * 2 * NP * 2 * sizeof(double)) smem = (size_t)WPC * 2 * NP * 2 * sizeof(double);
-    if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
-    auto kern = exchange3m_multi_kernel<NP, WPC, MINB>;
-    if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
-    const long long nblocks = (long long)((nw + 2 * NP - 1) / (2 * NP)) * c->nunits;
-    if (nblocks > 0x7fffffffLL) return AFQMC_UNSUPPORTED;
-    kern<<<(unsigned)nblocks, 32 * WPC, smem, st>>>(d, KS3, nw, c->units, c->kminus, c->kplus, c->kneg, c->Lx3, theta, c->ws_expart);
-    AFQMC_LAUNCH_CHECK(c);
-    return AFQMC_OK;
+// n-tiles per warp: 2 (four walkers per CTA) unless there are at most two walkers; 4 (eight walkers per CTA) on request
+template <int NPAIR, int DA, bool GRIDPAIRS>
+int launch_x3_np(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+    int np = c->opt_exchange_np;
+    if (np == 0) np = nw <= 2 ? 1 : 2;
+    // resident CTAs asked of the compiler: the register budget per thread is 65536 / (MINB * 64 * NPAIR)
+    if (np == 1) return launch_x3<1, NPAIR, DA, (NPAIR == 1 ? 8 : 4), GRIDPAIRS>(c, theta, nw, st);
+    if (np == 4) return launch_x3<4, NPAIR, (DA > 2 ? 2 : DA), (NPAIR == 1 ? 5 : 2), GRIDPAIRS>(c, theta, nw, st);
+    return launch_x3<2, NPAIR, DA, (NPAIR == 1 ? 7 : 3), GRIDPAIRS>(c, theta, nw, st);
 }
 
-template <int NP, int WPC, int MINB, int DA>
-int launch_exchange3m_cfg(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
-    const Dims& d = c->d;
-    const int KS3 = (d.m + 3) / 4;
-    size_t smem = (size_t)2 * 3 * KS3 * NP * 32 * sizeof(double);
-    if (smem < (size_t)WPC * 2 * NP * 2 * sizeof(double)) smem = (size_t)WPC * 2 * NP * 2 * sizeof(double);
-    auto kern = exchange3m_kernel<NP, WPC, MINB, DA>;
-    if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
-    const long long nblocks = (long long)((nw + 2 * NP - 1) / (2 * NP)) * c->nunits;
-    if (nblocks > 0x7fffffffLL) return AFQMC_UNSUPPORTED;
-    kern<<<(unsigned)nblocks, 32 * WPC, smem, st>>>(d, KS3, nw, c->units, c->kminus, c->kplus, c->kneg, c->Lx3, theta, c->ws_expart);
-    AFQMC_LAUNCH_CHECK(c);
-    return AFQMC_OK;
+template <bool GRIDPAIRS>
+int launch_x3_cfg(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+    const bool two_pairs = GRIDPAIRS || c->opt_exchange_wpc == 4;         // option "exchange_warps" = 4: two warp pairs per CTA
+    const int da = c->opt_exchange_depth == 2 ? 2 : 3;                     // option "exchange_depth": k-steps of A prefetch
+    if (two_pairs) return da == 2 ? launch_x3_np<2, 2, GRIDPAIRS>(c, theta, nw, st) : launch_x3_np<2, 3, GRIDPAIRS>(c, theta, nw, st);
+    return da == 2 ? launch_x3_np<1, 2, GRIDPAIRS>(c, theta, nw, st) : launch_x3_np<1, 3, GRIDPAIRS>(c, theta, nw, st);
 }
 
 }  // namespace
 
-// Writes the unit partial sums into ws_expart like the 4M kernel.  Returns AFQMC_UNSUPPORTED (caller falls back to the 4M
-// kernel) only if the staged theta blocks do not fit shared memory.
-int afqmc_i_exchange3m(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+// Partial sums per unit that ws_expart must hold: 1, or NAG^2 * (up to 8 chunks) when the theta blocks of all a-groups do not
+// fit one CTA's shared memory (then the (ag,bg) pairs and chunks of gamma-quads are spread over the grid).
+int afqmc_i_exchange3m_parts_max(const afqmc_ctx* c) {
     const Dims& d = c->d;
-    if (!c->Lx3) return AFQMC_UNSUPPORTED;
+    if (d.NAG == 1) return 1;
+    return x3_smem_bytes<2>(x3_geom(d.m), d.NAG, 1) > (size_t)c->smem_optin ? d.NAG * d.NAG * 8 : 1;
+}
+
+// Writes the unit partial sums into ws_expart (ex_parts per unit) for energy_finalize_kernel.  Returns AFQMC_UNSUPPORTED only
+// if even the theta rows of two a-groups do not fit shared memory.
+int afqmc_i_exchange3m(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     c->ex_parts = 1;
-    if (d.NAG != 1) {    // more than four occupied orbitals per k-point
-        int rc = nw >= 3 ? launch_exchange3m_multi<2, 2, 6>(c, theta, nw, st) : launch_exchange3m_multi<1, 2, 6>(c, theta, nw, st);
-        if (rc == AFQMC_UNSUPPORTED && c->ex_parts_max > 1) {       // blocks too large for one CTA's shared memory
-            rc = nw >= 3 ? launch_exchange3m_big<2, 8>(c, theta, nw, st) : AFQMC_UNSUPPORTED;
-            if (rc == AFQMC_UNSUPPORTED) rc = launch_exchange3m_big<1, 8>(c, theta, nw, st);
-        }
-        return rc;
-    }
-    const int wpc = c->opt_exchange_wpc == 4 ? 4 : 2;
-    const bool deep = c->opt_exchange_depth == 6;
-    if (nw >= 3) {
-        if (deep) return wpc == 4 ? launch_exchange3m_cfg<2, 4, 2, 6>(c, theta, nw, st) : launch_exchange3m_cfg<2, 2, 4, 6>(c, theta, nw, st);
-        return wpc == 4 ? launch_exchange3m_cfg<2, 4, 3, 3>(c, theta, nw, st) : launch_exchange3m_cfg<2, 2, 6, 3>(c, theta, nw, st);
-    }
-    return wpc == 4 ? launch_exchange3m_cfg<1, 4, 3, 3>(c, theta, nw, st) : launch_exchange3m_cfg<1, 2, 6, 3>(c, theta, nw, st);
+    int rc = launch_x3_cfg<false>(c, theta, nw, st);
+    if (rc == AFQMC_UNSUPPORTED && c->d.NAG > 1 && c->ex_parts_max > 1) rc = launch_x3_cfg<true>(c, theta, nw, st);
+    return rc;
 }

@@ -30,8 +30,8 @@ __device__ __forceinline__ float tf32_of(float f) {
 }
 
 // LxT = [hi plane][pad][lo plane][pad]; plane stride = total_padded floats
-__global__ void pack_LxT_kernel(Dims d, int KS8, const double2* __restrict__ L, const double2* __restrict__ psi_t,
-                                float* __restrict__ LxT, size_t total, size_t total_padded) {
+__global__ void pack_LxT_kernel(Dims d, int KS8, const double2* __restrict__ Lh, float* __restrict__ LxT, size_t total,
+                                size_t total_padded) {
     for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
         size_t t_ = idx;
         const int e = (int)(t_ & 3); t_ >>= 2;                // register of the A fragment
@@ -45,15 +45,7 @@ __global__ void pack_LxT_kernel(Dims d, int KS8, const double2* __restrict__ L, 
         const int gam = 4 * gq + (row >> 2), a = row & 3, r = j >> 1, part = j & 1;
         float v = 0.f, vlo = 0.f;
         if (a < d.n && gam < d.nchol && r < d.m) {
-            // Lh[Q][k][a][gam][r] = sum_p conj(A_k[p][a]) L[Q][k][gam][p][r], in FP64, then rounded
-            const double2* Lb = L + (((size_t)(Q * d.Nk + k) * d.nchol + gam) * d.m) * d.m + r;
-            const double2* Ab = psi_t + (size_t)k * d.m * d.n + a;
-            double2 z = make_double2(0.0, 0.0);
-            for (int p = 0; p < d.m; ++p) {
-                double2 av = Ab[(size_t)p * d.n];
-                av.y = -av.y;
-                z = cfma(av, Lb[(size_t)p * d.m], z);
-            }
+            const double2 z = Lh[((((size_t)Q * d.Nk + k) * d.n + a) * d.nchol + gam) * d.m + r];     // FP64, then rounded
             const float f = (float)(part ? z.y : z.x);
             v = tf32_of(f);
             vlo = tf32_of(f - v);
@@ -215,13 +207,13 @@ size_t afqmc_i_lxt_floats(const Dims& d) {
     return 2 * ((size_t)d.Nk * d.Nk * d.GQ * KS8 * 128 + XT_PAD);      // hi and lo planes
 }
 
-int afqmc_i_pack_lxt(afqmc_ctx* c, const double2* L, cudaStream_t st) {
+int afqmc_i_pack_lxt(afqmc_ctx* c, cudaStream_t st) {
     const Dims& d = c->d;
     const int KS8 = (2 * d.m + 7) / 8;
     const size_t total = (size_t)d.Nk * d.Nk * d.GQ * KS8 * 128;
     size_t g = (total + 255) / 256;
     if (g > 148 * 64) g = 148 * 64;
-    pack_LxT_kernel<<<(unsigned)g, 256, 0, st>>>(d, KS8, L, c->psi_t, c->LxT, total, total + XT_PAD);
+    pack_LxT_kernel<<<(unsigned)g, 256, 0, st>>>(d, KS8, c->Lh, c->LxT, total, total + XT_PAD);
     AFQMC_LAUNCH_CHECK(c);
     return AFQMC_OK;
 }

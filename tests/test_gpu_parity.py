@@ -79,11 +79,12 @@ def cond_overlap(psi_t, phi_w):
 
 
 def theta2_bound(cond):
-    """Tolerance of quantities that pass through the inversion of the PROPAGATED walker's overlap O':
-    north_star's 1e-10, unless cond(O') is so large that a backward-stable inversion cannot reach it; then
-    100 * cond(O') * 2^-53 (elimination with partial pivoting: forward error <~ c(N) * cond * u, c(N) <~ 100 for
-    N <= 256).  On the synthetic walkers cond(O') is 1e1..1e4, so the bound is 1e-10 at every config (printed)."""
-    return max(RTOL, 100.0 * cond * 2.0 ** -53)
+    """Tolerance of quantities that pass through the inversion of the PROPAGATED walker's overlap O': north_star's 1e-10,
+    flat.  cond(O') is printed beside every measured error because it is what the error scales with (elimination with
+    partial pivoting: forward error <~ c(N) * cond * 2^-53); on the synthetic walkers cond(O') reaches 1e4 and the measured
+    error 3e-13, so the flat bound holds with two orders of margin at every config."""
+    del cond
+    return RTOL
 
 
 def run_chain_and_compare(case, sample=None, tol=RTOL, energy_sample=None):
