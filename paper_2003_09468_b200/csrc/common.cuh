@@ -49,7 +49,9 @@ struct afqmc_ctx {
     double2* ht;    // [Nk][n][m]   half-rotated one-body
     double2* Lh;    // half-rotated Cholesky tensor, natural layout [Q][k][a][gamma][r]: computed ONCE in a0; every packed
                     // operand below is a pure re-layout of it
-    double* Lxc;    // exchange (default 3M kernel, exchange3m.cu): complex fragments [Q][k][ag][gq][ks][lane][4]
+    double* Lxc;    // exchange, generic 3M kernel (exchange3m.cu; default for m > 28): complex fragments [Q][k][ag][gq][ks][lane][4]
+    double* Lx3t;   // exchange, register-B 3M kernel (default for m <= 28): the three A variants [Q][k][ag][gq][ml][lane][2]
+                    // (only the default one of Lxc / Lx3t is packed in a0; the other on first use)
     double* Lx;     // exchange, 4M kernel (energy.cu): [Q][k][ag][gq][s][lane][2]; packed on first use (option exchange_3m = 0)
     float* LxT;     // exchange, TF32 fragments [Q][k][gq][ks][lane][4] (exchange_tf32.cu; n <= 4 only); packed on first use
     double* Lf;     // force-bias fragment layout [Q][gtp][k][a][s][lane][2]
@@ -93,6 +95,7 @@ struct afqmc_ctx {
     int opt_exchange_3m;    // 1 (default) = 3M exchange kernel when n <= 4, 0 = the 4M kernel of energy.cu
     int opt_exchange_wpc;   // 0 = automatic, else warps per CTA of the exchange kernel (4,5,6,8)
     int opt_exchange_np;    // tuning aid (3M kernel): 0 = automatic, else 1/2/4 walker pairs (n-tiles) per warp
+    int opt_exchange_regb;  // 1 (default) = theta block of a warp in registers when m <= 28 (exchange3m_reg_kernel), 0 = generic kernel
     int opt_timers;     // record stage events in afqmc_step
     int opt_taylor_legacy;  // testing aid: 1 = shared-memory-tiled zgemm for the Taylor chain
     int opt_taylor_wpc;     // tuning aid: 0 = automatic, else 3/4/5 warps per CTA of the Taylor GEMM
@@ -141,6 +144,35 @@ __device__ __forceinline__ double2 cfma(double2 a, double2 b, double2 c) {  // a
     c.y = fma(a.x, b.y, c.y); c.y = fma(a.y, b.x, c.y);
     return c;
 }
+// ---- mbarrier / bulk asynchronous copy (TMA engine, SASS UBLKCP) primitives shared by the kernels that stage operands ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n.reg .pred p;\nWAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}\n" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// global -> shared, `bytes` a multiple of 16, both addresses 16-byte aligned; completion is counted on `bar`
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -207,7 +239,7 @@ int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, 
                       cudaStream_t st);
 int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* energy, cudaStream_t st);
 int afqmc_i_exchange3m(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st);   // AFQMC_UNSUPPORTED only if the staged theta blocks exceed shared memory
-int afqmc_i_pack_lxc(afqmc_ctx* c, cudaStream_t st);                                    // Lh -> Lxc
+int afqmc_i_pack_exchange_operand(afqmc_ctx* c, cudaStream_t st);                       // a0: Lh -> Lx3t (m <= 28) or Lxc
 size_t afqmc_i_lxc_doubles(const Dims& d);
 int afqmc_i_exchange3m_parts_max(const afqmc_ctx* c);
 int afqmc_i_exchange_tf32(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st);  // AFQMC_UNSUPPORTED if n > 4

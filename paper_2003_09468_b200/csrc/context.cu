@@ -145,7 +145,7 @@ static int dev_alloc(T** p, size_t count) {
 
 AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     if (!c) return;
-    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lh, c->Lxc, c->Lx, c->LxT, c->Lf, c->Lv3, c->vunits,
+    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lh, c->Lxc, c->Lx3t, c->Lx, c->LxT, c->Lf, c->Lv3, c->vunits,
                     c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T, c->ws_Tx,
                     c->ws_expart, c->ws_fbpart, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
                     c->ws_f32, c->b1, c->ws_b1tmp, c->ws_gram, c->ws_rinv, c->ws_logdet2, c->ws_ldr, c->ws_info2};
@@ -189,6 +189,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     c->prec32 = dims->precision == 1 ? 1 : 0;
     c->opt_fb_pf = 8;
     c->opt_exchange_3m = 1;
+    c->opt_exchange_regb = 1;
     const int nw = c->max_walkers;
 
     int dev = 0;
@@ -236,7 +237,6 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     A(dev_alloc(&c->psi_t, (size_t)Nk * d.m * d.n));
     A(dev_alloc(&c->ht, (size_t)Nk * d.n * d.m));
     A(dev_alloc(&c->Lh, nLh));
-    A(dev_alloc(&c->Lxc, afqmc_i_lxc_doubles(d)));
     A(dev_alloc(&c->Lf, nLf));
     A(dev_alloc(&c->ws_O, (size_t)nw * d.N * LD));
     A(dev_alloc(&c->ws_oinvT, (size_t)nw * d.N * d.N));
@@ -296,7 +296,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
         pack_Lf_kernel<<<grid(nLf), T, 0, st>>>(d, c->Lh, c->Lf, nLf);
         c->launches += 3;
         if (cudaGetLastError() != cudaSuccess) rc = AFQMC_CUDA_ERROR;
-        if (rc == AFQMC_OK) rc = afqmc_i_pack_lxc(c, st);
+        if (rc == AFQMC_OK) rc = afqmc_i_pack_exchange_operand(c, st);
         if (rc == AFQMC_OK) rc = afqmc_i_vhs_setup(c, (const double2*)L, kminus, kneg, st);
     }
     // host vectors must outlive the async copies; the caller may free its arrays after return
@@ -384,6 +384,10 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
             if (rc != AFQMC_OK) return rc;
         }
         c->opt_exchange_3m = value ? 1 : 0;
+        return AFQMC_OK;
+    }
+    if (strcmp(name, "exchange_regb") == 0) {
+        c->opt_exchange_regb = value ? 1 : 0;
         return AFQMC_OK;
     }
     if (strcmp(name, "exchange_np") == 0) {

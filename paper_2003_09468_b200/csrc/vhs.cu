@@ -176,28 +176,6 @@ __global__ void fields3_kernel(Dims d, int nw, int NT, int nwg, int KS4p, const 
 }
 
 // ---- mbarrier / bulk-copy primitives (PTX) ----
-__device__ __forceinline__ uint32_t v3_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void v3_mbar_init(uint64_t* bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(v3_smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void v3_mbar_wait(uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n.reg .pred p;\nWAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}\n" ::"r"(v3_smem_u32(bar)), "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void v3_mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(v3_smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void v3_mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(v3_smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void v3_bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(v3_smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(v3_smem_u32(bar))
-                 : "memory");
-}
 
 // ---- the contraction kernel: see the header comment ----
 // NT = n-tiles (8 walkers each) of one column set.  MERGED (small batches, NT <= 2): one warp computes BOTH column
@@ -228,7 +206,7 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
     int nactive = 0;
     for (int wv = 0; wv < V3_WARPS; ++wv) nactive += (slice0 + wv % spc) < nslices ? 1 : 0;
     if (tid == 0) {
-        for (int s = 0; s < V3_STAGES; ++s) { v3_mbar_init(&full[s], 1); v3_mbar_init(&empty[s], nactive); }
+        for (int s = 0; s < V3_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], nactive); }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
     }
@@ -241,10 +219,10 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
     const double* bsrc1 = Bx3 + ((((size_t)Q * 2 + 1) * nwg + wg) * KS4p) * 3 * NT * 32;
     auto produce = [&](int ch) {       // thread 0 only
         const int s = ch % V3_STAGES;
-        v3_mbar_expect_tx(&full[s], (uint32_t)(nsets * SET_DOUBLES * 8));
+        mbar_expect_tx(&full[s], (uint32_t)(nsets * SET_DOUBLES * 8));
         double* dst = v3_smem + (size_t)s * STAGE_DOUBLES;
-        v3_bulk_g2s(dst, bsrc0 + (size_t)ch * SET_DOUBLES, SET_DOUBLES * 8, &full[s]);
-        if (nsets == 2) v3_bulk_g2s(dst + SET_DOUBLES, bsrc1 + (size_t)ch * SET_DOUBLES, SET_DOUBLES * 8, &full[s]);
+        bulk_g2s(dst, bsrc0 + (size_t)ch * SET_DOUBLES, SET_DOUBLES * 8, &full[s]);
+        if (nsets == 2) bulk_g2s(dst + SET_DOUBLES, bsrc1 + (size_t)ch * SET_DOUBLES, SET_DOUBLES * 8, &full[s]);
     };
     if (tid == 0)
         for (int c0 = 0; c0 < V3_STAGES - 1 && c0 < nchunks; ++c0) produce(c0);
@@ -290,7 +268,7 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
     };
     for (int ch = 0; ch < nchunks; ++ch) {
         const int s = ch % V3_STAGES;
-        v3_mbar_wait(&full[s], (uint32_t)((ch / V3_STAGES) & 1));
+        mbar_wait(&full[s], (uint32_t)((ch / V3_STAGES) & 1));
         const double* bs = v3_smem + (size_t)s * STAGE_DOUBLES + set * SET_DOUBLES + lane;
 #pragma unroll
         for (int q = 0; q < KC; ++q) {
@@ -298,13 +276,13 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
             if (q == 0 && tid == 0) {   // producer duty: refill the stage consumed in the previous iteration
                 const int nxt = ch + V3_STAGES - 1;
                 if (nxt < nchunks) {
-                    if (nxt >= V3_STAGES) v3_mbar_wait(&empty[nxt % V3_STAGES], (uint32_t)(((nxt / V3_STAGES) & 1) ^ 1));
+                    if (nxt >= V3_STAGES) mbar_wait(&empty[nxt % V3_STAGES], (uint32_t)(((nxt / V3_STAGES) & 1) ^ 1));
                     produce(nxt);
                 }
             }
         }
         __syncwarp();
-        if (lane == 0) v3_mbar_arrive(&empty[s]);
+        if (lane == 0) mbar_arrive(&empty[s]);
     }
 
     // ---- epilogue: Re = P0 - P2, Im = P0 + P1 (conjugated and transposed for the partner block) ----
