@@ -536,22 +536,29 @@ def test_vhs_without_the_pair_identity_falls_back_to_all_blocks(nw):
                                 dict(mesh=(2, 2, 1), m=9, n=6, nchol=11, nw=5), dict(mesh=(1, 1, 2), m=14, n=9, nchol=6, nw=2)],
                          ids=["n4", "n3_odd", "n1_two_walkers", "m26_seven_walkers", "n6_two_groups", "n9_three_groups"])
 def test_exchange_3m_and_4m_kernels_against_the_oracle(kw):
-    """Both exchange kernels (exchange3m.cu: default for n <= 4; energy.cu: option exchange_3m=0) on the same theta,
-    each against the oracle, and against each other; the deep-prefetch variants of the 3M kernel too."""
+    """All exchange kernels (exchange3m.cu: register-B and generic 3M kernels; energy.cu: 4M, option exchange_3m=0) on the
+    same theta, each against the oracle, and against each other."""
     case = Case(synth.tiny_config(seed=13, **kw))
     try:
         theta_d, _, _ = case.ctx.green(_to_dev(case.pb.phi))
         theta = theta_d.cpu().numpy()
         e_o = np.array([orc.local_energy(case.cfg.mesh, case.Lh, case.ht, theta[w]) for w in range(case.nw)])
         res = {}
-        for name, opts in (("3m", {}), ("4m", {"exchange_3m": 0}), ("3m_deep", {"exchange_depth": 6}),
-                           ("3m_4warps", {"exchange_warps": 4}), ("3m_deep_4warps", {"exchange_depth": 6, "exchange_warps": 4})):
+        # "3m" is the default kernel of the shape (register-B persistent kernel for m <= 28, else the generic one); the other
+        # entries force the generic kernel in its variants (smem B fragments, 1 or 2 warp pairs, 2 or 3 k-steps of prefetch,
+        # 1/2/4 n-tiles per warp), the two-walker register-B kernel, and the 4M kernel
+        for name, opts in (("3m", {}), ("4m", {"exchange_3m": 0}), ("3m_generic", {"exchange_regb": 0}),
+                           ("3m_generic_depth2", {"exchange_regb": 0, "exchange_depth": 2}),
+                           ("3m_generic_4warps", {"exchange_warps": 4}), ("3m_generic_np4", {"exchange_np": 4}),
+                           ("3m_generic_np1_4warps", {"exchange_regb": 0, "exchange_np": 1, "exchange_warps": 4}),
+                           ("3m_two_walkers_per_cta", {"exchange_np": 1})):
             for k, v in opts.items():
                 case.ctx.set_option(k, v)
             res[name] = case.ctx.local_energy(theta_d).cpu().numpy()
+            for k in ("exchange_depth", "exchange_warps", "exchange_np"):
+                case.ctx.set_option(k, 0)
             case.ctx.set_option("exchange_3m", 1)
-            case.ctx.set_option("exchange_depth", 0)
-            case.ctx.set_option("exchange_warps", 0)
+            case.ctx.set_option("exchange_regb", 1)
         for name, e in res.items():
             for w in range(case.nw):
                 assert np.max(np.abs(e[w] - e_o[w]) / np.abs(e_o[w])) < RTOL, (name, w, e[w], e_o[w])
