@@ -33,6 +33,11 @@ orthogonalisation, mixed estimator, block) are pinned by tests/test_oracle_block
 restatement, Gauss-Hermite quadrature of Eq. 12/16, Wick's theorem, scipy expm, numpy QR); none is "parity
 unpinned".  `numpy.linalg.det` / `inv` appear only in level D.
 
+The OPEN-SHELL functions (two spin channels with N_up != N_dn; Eq. 36 and Eq. 49 with their
+explicit sigma, sigma' sums) follow the closed-shell ones section by section (`*_uhf`); they are
+pinned by tests/test_oracle_open_shell_pins.py (explicit p,q,r,s,sigma,sigma' loops, the one-electron self-interaction
+cancellation E_C + E_X = 0, the closed-shell limit, level P == level D); none is "parity unpinned".
+
 Layouts (row-major, last index fastest):
   L[Q][k][gamma][p][r]   p at k-point k, r at k-Q
   psi_t[k][p][a]         trial, block diagonal in k
@@ -588,3 +593,100 @@ def block(mesh, L, Lh, ht, psi_t, B1, phi, weight, x, dtau, order):
     for w in range(nw):
         phi[w], logdet_r[w] = orthogonalize(phi[w])
     return phi, weight, energy, (num, den), logdet_r
+
+
+# ======================================================================================
+# OPEN SHELL: two spin channels, N_up != N_dn allowed.
+# Eq. 36:  E = sum_{pq,s} h_pq G^s_pq + 1/2 sum_{pqrs} v_pqrs sum_{s,s'} [ G^s_pr G^s'_qs - delta_{ss'} G^s_ps G^s_qr ]
+# Eq. 49 is the same in k-blocked, half-rotated form with its explicit sigma sums.
+# A channel is (trial A^s [Nk][m][n_s], walker Phi^s [M][N_s]); the closed shell is the case A^up = A^dn, Phi^up = Phi^dn,
+# where these functions reduce to the closed-shell ones above (factors 2, 4, 2).
+# ======================================================================================
+
+# ---- level D ----
+def dense_vbias_uhf(Lsc, G_up, G_dn):
+    """v_Gamma = sum_sigma sum_pr L_{pr,Gamma} G^sigma_pr  (Eq. 25/37 summed over spin, no prefactor)."""
+    return np.einsum('prg,pr->g', Lsc, G_up) + np.einsum('prg,pr->g', Lsc, G_dn)
+
+
+def dense_energy_uhf(H, V, G_up, G_dn):
+    """Eq. 36 with both spin sums explicit:
+    E1 = sum_s sum_pq h_pq G^s_pq;  EC = 1/2 sum_{s,s'} sum v_pqrs G^s_pr G^s'_qs;
+    EX = -1/2 sum_s sum v_pqrs G^s_ps G^s_qr   (delta_{ss'}: exchange only between like spins)."""
+    e1 = 0.0 + 0.0j
+    ec = 0.0 + 0.0j
+    ex = 0.0 + 0.0j
+    for Gs in (G_up, G_dn):
+        e1 += np.einsum('pq,pq->', H, Gs)
+        ex += -0.5 * np.einsum('pqrs,ps,qr->', V, Gs, Gs)
+        for Gt in (G_up, G_dn):
+            ec += 0.5 * np.einsum('pqrs,pr,qs->', V, Gs, Gt)
+    return np.array([e1, ec, ex], dtype=C128)
+
+
+# ---- level P ----
+def force_bias_uhf(mesh, Lh_up, Lh_dn, theta_up, theta_dn):
+    """a4, open shell: vbias[Q][gamma] = sum_sigma sum_k sum_{a,r} Lh^sigma[Q][k][a][gamma][r] Theta^sigma[(k,a),(k-Q,r)]
+    (Eq. 47 with its spin sum).  `force_bias` above carries the closed-shell factor 2 = two equal channels."""
+    return 0.5 * (force_bias(mesh, Lh_up, theta_up) + force_bias(mesh, Lh_dn, theta_dn))
+
+
+def local_energy_uhf(mesh, Lh_s, ht_s, theta_s):
+    """a7-a9, open shell, by the paper's steps 1-3 with the loop over sigma of step 2 written out.
+    `Lh_s`, `ht_s`, `theta_s` are 2-tuples (up, dn).  The traces v_1, v_2 of step 2(d) are summed over BOTH spins before
+    step 3 multiplies them (the Coulomb term couples the channels: sigma, sigma' independent in Eq. 49), while the exchange
+    contribution of step 2(c) is accumulated per spin (delta_{sigma sigma'})."""
+    nk = Lh_s[0].shape[0]
+    nchol = Lh_s[0].shape[3]
+    e1 = 0.0 + 0.0j
+    ex = 0.0 + 0.0j
+    ec = 0.0 + 0.0j
+    G_s = []
+    for Lh, ht, theta_w in zip(Lh_s, ht_s, theta_s):
+        n, m = Lh.shape[2], Lh.shape[4]
+        G = reshape_theta(theta_w, nk, n, m)                # step 1, per spin
+        G_s.append(G)
+        for k in range(nk):                                 # Eq. 49 line 1
+            e1 += np.sum(ht[k] * G[k, k])
+    for Q in range(nk):
+        mQ = k_neg(mesh, Q)
+        v1 = np.zeros(nchol, dtype=C128)
+        v2 = np.zeros(nchol, dtype=C128)
+        for Lh, G in zip(Lh_s, G_s):                        # step 2: "for each (sigma, Q, k, k')"
+            for k in range(nk):
+                kq = k_sub(mesh, k, Q)
+                for kp in range(nk):
+                    kpq = k_sub(mesh, kp, Q)
+                    T1 = np.einsum('agr,br->bag', Lh[Q, k], G[kpq, kq])        # 2(a)
+                    T2 = np.einsum('bgs,as->abg', Lh[mQ, kpq], G[k, kp])       # 2(b)
+                    ex += -0.5 * np.einsum('bag,abg->', T1, T2)                # 2(c)
+                    if kpq == k:                                                # 2(d)
+                        v1 += np.einsum('aag->g', T1)
+                        v2 += np.einsum('aag->g', T2)
+        ec += 0.5 * np.sum(v1 * v2)                                            # step 3, summed over Q
+    return np.array([e1, ec, ex], dtype=C128)
+
+
+def step_uhf(mesh, L, Lh_s, ht_s, psi_t_s, phi_s, x, dtau, order):
+    """The timed composition for open-shell walkers: per walker, Green's function of both channels, the spin-summed force
+    bias, ONE vHS (spin independent), the same Taylor propagator on both channels, then overlap + Green + local energy of
+    the new walker.  phi_s = (phi_up [nw][M][N_up], phi_dn [nw][M][N_dn]).
+    Returns ((phi_up', phi_dn'), energy [nw][3], logdet [nw] = log det O_up + log det O_dn)."""
+    nw = phi_s[0].shape[0]
+    out = (np.empty_like(phi_s[0]), np.empty_like(phi_s[1]))
+    energy = np.empty((nw, 3), dtype=C128)
+    logdet = np.empty(nw, dtype=C128)
+    for w in range(nw):
+        th = [green(psi_t_s[s], phi_s[s][w])[0] for s in range(2)]
+        vb = force_bias_uhf(mesh, Lh_s[0], Lh_s[1], th[0], th[1])
+        xi = assemble_fields(mesh, x[w], vb, dtau)
+        V = vhs(mesh, L, xi)
+        th2, ld = [], 0.0 + 0.0j
+        for s in range(2):
+            out[s][w] = propagate(V, phi_s[s][w], dtau, order)
+            t2, l2, _ = green(psi_t_s[s], out[s][w])
+            th2.append(t2)
+            ld += l2
+        energy[w] = local_energy_uhf(mesh, Lh_s, ht_s, th2)
+        logdet[w] = complex(ld.real, (ld.imag + np.pi) % (2 * np.pi) - np.pi)
+    return out, energy, logdet

@@ -165,3 +165,21 @@ def make_block_fields(cfg: Config, nsteps: int, nw=None, seed_offset=7):
     nw = cfg.nw if nw is None else nw
     rng = np.random.default_rng(cfg.seed + seed_offset)
     return rng.standard_normal((nsteps, nw, cfg.nk, cfg.nchol))
+
+
+# ---- open-shell inputs: a second spin channel with its own occupied count ----
+def make_open_shell(cfg: Config, n_dn: int, nw=None, seed_offset=101):
+    """Adds a spin-DOWN channel with `n_dn` occupied orbitals per k-point to `make_problem(cfg)` (whose trial and walkers
+    become the spin-UP channel, n_up = cfg.n): an independent random orthonormal trial block per k and walkers drawn the same
+    way (trial + 0.1 CN(0,1), thin QR), from their own stream `seed + seed_offset`.  Returns (problem, psi_t_dn [Nk][m][n_dn],
+    phi_dn [nw][M][Nk*n_dn]); the Hamiltonian and the fields are shared by both channels."""
+    pb = make_problem(cfg, nw)
+    rng = np.random.default_rng(cfg.seed + seed_offset)
+    nk, m = cfg.nk, cfg.m
+    psi_dn = np.empty((nk, m, n_dn), dtype=np.complex128)
+    for k in range(nk):
+        q, _ = np.linalg.qr(_cn(rng, (m, n_dn), 1.0))
+        psi_dn[k] = q
+    cfg_dn = Config(cfg.name + "_dn", cfg.mesh, m, n_dn, cfg.nchol, pb.phi.shape[0], cfg.dtau, cfg.order, cfg.seed)
+    phi_dn = make_walkers(cfg_dn, psi_dn, rng, pb.phi.shape[0])
+    return pb, psi_dn, phi_dn
