@@ -53,18 +53,33 @@ typedef struct {
     int m;            /* bands per k-point                                          */
     int n;            /* occupied orbitals per k-point per spin                      */
     int nchol;        /* Cholesky vectors per Q             */
-    int closed_shell; /* must be 1 (else AFQMC_UNSUPPORTED)                          */
+    int closed_shell; /* 1 = closed shell (one walker matrix for both spins); 0 = open shell (see "Open shell") */
     int precision;    /* 0 = complex128; 1 = complex64 boundary (see "Precision 1" below)  */
     int max_walkers;  /* workspace is sized for this many walkers                    */
+    int n_dn;         /* open shell only: spin-down occupied orbitals per k-point (n is then the spin-up count) */
 } afqmc_dims;
 
 enum {
     AFQMC_OK = 0,
     AFQMC_INVALID_ARGUMENT = 1, /* null pointer, nw < 0 or > max_walkers, bad dims, bad order */
-    AFQMC_UNSUPPORTED = 2,      /* open shell, precision > 1, block calls with precision 1 ...  */
+    AFQMC_UNSUPPORTED = 2,      /* precision > 1, open shell or block calls with precision 1 ...   */
     AFQMC_CUDA_ERROR = 3,       /* a CUDA runtime call or launch failed                       */
     AFQMC_OUT_OF_MEMORY = 4     /* device allocation failed                                   */
-};
+}/*
+ * Open shell (closed_shell = 0; Eq. 36 / Eq. 49 with their explicit spin sums).  Two spin channels
+ * with n (spin up) and n_dn (spin down) occupied orbitals per k-point, N_up = Nk*n, N_dn = Nk*n_dn.  Every per-walker array
+ * that has an orbital index is SPIN-MAJOR: the spin-up block of all nw walkers followed by the spin-down block,
+ *     psi_t = [Nk][m][n]      then [Nk][m][n_dn]           phi   = [nw][M][N_up] then [nw][M][N_dn]
+ *     theta = [nw][N_up][M]   then [nw][N_dn][M]           (the offset of the second block depends on the call's nw)
+ * and the spin-independent ones are unchanged: vbias[nw][Nk][nchol] = vbias_up + vbias_dn (no factor 2), x, vhs[nw][M][M],
+ * energy[nw][3] = (E1 summed over spins, EC = 1/2 sum_Q v_Q v_-Q of the spin-summed v, EX = -1/2 sum_spin sum T T: exchange
+ * only between like spins), logdet[nw] = log det O_up + log det O_dn (phase wrapped to (-pi, pi]), info[nw] = first non-zero
+ * of the two channels.  All calls below take these layouts when the context is open shell; the hybrid weight then uses the
+ * overlap ratio det'_up det'_dn / (det_up det_dn) (closed shell: the squared ratio of the shared determinant).  Two equal
+ * channels reproduce the closed-shell results (tested).  The complex64 boundary (precision = 1) is closed-shell only.
+ */
+
+;
 
 /* Text for an error code (static storage, never NULL). */
 const char* afqmc_strerror(int code);

@@ -26,7 +26,8 @@ class AfqmcError(RuntimeError):
 
 class Dims(ctypes.Structure):
     _fields_ = [("g", ctypes.c_int * 3), ("m", ctypes.c_int), ("n", ctypes.c_int), ("nchol", ctypes.c_int),
-                ("closed_shell", ctypes.c_int), ("precision", ctypes.c_int), ("max_walkers", ctypes.c_int)]
+                ("closed_shell", ctypes.c_int), ("precision", ctypes.c_int), ("max_walkers", ctypes.c_int),
+                ("n_dn", ctypes.c_int)]
 
 
 EXPORTS = ["afqmc_strerror", "afqmc_create", "afqmc_destroy", "afqmc_overlap", "afqmc_green", "afqmc_force_bias",
@@ -109,21 +110,32 @@ def probe_fp64(kind: int, iters: int = 20000) -> float:
 class Afqmc:
     """Context of one Hamiltonian + trial on the current CUDA device (afqmc_create / afqmc_destroy)."""
 
-    def __init__(self, mesh, m, n, nchol, h1, L, psi_t, max_walkers, closed_shell=1, precision=0):
+    def __init__(self, mesh, m, n, nchol, h1, L, psi_t, max_walkers, closed_shell=1, precision=0, n_dn=0):
+        """Open shell (closed_shell=0): `n` is the spin-up and `n_dn` the spin-down occupied count per k-point, `psi_t` is the
+        pair (psi_up [Nk][m][n], psi_dn [Nk][m][n_dn]); walkers and Green's functions are then FLAT spin-major tensors (the
+        spin-up block of all walkers followed by the spin-down block, include/afqmc.h "Open shell"): see join_spin/split_*."""
         self._h = ctypes.c_void_p(0)
         self.mesh = tuple(int(v) for v in mesh)
         self.nk = self.mesh[0] * self.mesh[1] * self.mesh[2]
         self.m, self.n, self.nchol = int(m), int(n), int(nchol)
         self.M, self.N = self.nk * self.m, self.nk * self.n
+        self.open_shell = int(closed_shell) == 0
+        self.n_dn = int(n_dn) if self.open_shell else 0
+        self.N_dn = self.nk * self.n_dn
         self.max_walkers = int(max_walkers)
         self.precision = int(precision)
         # dtypes at the boundary: complex128/float64, or complex64/float32 with precision = 1 (include/afqmc.h "Precision 1")
         self.cdtype = torch.complex64 if self.precision == 1 else torch.complex128
         self.rdtype = torch.float32 if self.precision == 1 else torch.float64
-        d = Dims((ctypes.c_int * 3)(*self.mesh), self.m, self.n, self.nchol, closed_shell, precision, self.max_walkers)
+        d = Dims((ctypes.c_int * 3)(*self.mesh), self.m, self.n, self.nchol, closed_shell, precision, self.max_walkers, self.n_dn)
+        if self.open_shell:
+            psi_up, psi_dn = psi_t
+            if tuple(psi_up.shape) != (self.nk, self.m, self.n) or tuple(psi_dn.shape) != (self.nk, self.m, self.n_dn):
+                raise ValueError("open shell: psi_t must be the pair ([Nk][m][n], [Nk][m][n_dn])")
+            psi_t = torch.cat([psi_up.contiguous().reshape(-1), psi_dn.contiguous().reshape(-1)])
         for name, t, shape in (("h1", h1, (self.nk, self.m, self.m)),
                                ("L", L, (self.nk, self.nk, self.nchol, self.m, self.m)),
-                               ("psi_t", psi_t, (self.nk, self.m, self.n))):
+                               ("psi_t", psi_t, (psi_t.numel(),) if self.open_shell else (self.nk, self.m, self.n))):
             if not t.is_cuda or tuple(t.shape) != shape:
                 raise ValueError("%s must be a CUDA tensor of shape %s" % (name, shape))
         self.device = h1.device
@@ -152,9 +164,33 @@ class Afqmc:
     def _empty(self, shape, dtype=None):
         return torch.empty(shape, dtype=self.cdtype if dtype is None else dtype, device=self.device)
 
+    # ---- open shell: flat spin-major walker / Green's function tensors ----
+    def join_spin(self, up, dn):
+        """(up [nw][..][..], dn [nw][..][..]) -> the flat spin-major tensor the library takes."""
+        return torch.cat([up.contiguous().reshape(-1), dn.contiguous().reshape(-1)])
+
+    def split_phi(self, flat, nw):
+        a = nw * self.M * self.N
+        return flat[:a].view(nw, self.M, self.N), flat[a:].view(nw, self.M, self.N_dn)
+
+    def split_theta(self, flat, nw):
+        a = nw * self.N * self.M
+        return flat[:a].view(nw, self.N, self.M), flat[a:].view(nw, self.N_dn, self.M)
+
+    def _phi_shape(self, nw):
+        return (nw * self.M * (self.N + self.N_dn),) if self.open_shell else (nw, self.M, self.N)
+
+    def _theta_shape(self, nw):
+        return (nw * (self.N + self.N_dn) * self.M,) if self.open_shell else (nw, self.N, self.M)
+
     def _nw(self, t, name):
         """Batch size of a per-walker tensor; the library would read past `max_walkers` worth of workspace otherwise."""
         nw = int(t.shape[0])
+        if self.open_shell and t.dim() == 1 and name in ("phi", "theta", "phi_host"):
+            per = self.M * (self.N + self.N_dn)
+            if t.numel() % per != 0:
+                raise ValueError("%s: flat spin-major tensor of %d elements is not a multiple of M*(N_up+N_dn) = %d" % (name, t.numel(), per))
+            nw = t.numel() // per
         if nw > self.max_walkers:
             raise ValueError("%s: %d walkers > max_walkers = %d" % (name, nw, self.max_walkers))
         return nw
@@ -209,18 +245,18 @@ class Afqmc:
         nw = self._nw(phi, "phi")
         logdet = self._empty((nw,)) if logdet is None else logdet
         info = self._empty((nw,), torch.int32) if info is None else info
-        _check(self._call(lib().afqmc_overlap, self._dev(phi, (nw, self.M, self.N), self.cdtype, "phi"), nw,
+        _check(self._call(lib().afqmc_overlap, self._dev(phi, self._phi_shape(nw), self.cdtype, "phi"), nw,
                           self._dev(logdet, (nw,), self.cdtype, "logdet"), self._dev(info, (nw,), torch.int32, "info")),
                "afqmc_overlap")
         return logdet, info
 
     def green(self, phi, theta=None, logdet=None, info=None):
         nw = self._nw(phi, "phi")
-        theta = self._empty((nw, self.N, self.M)) if theta is None else theta
+        theta = self._empty(self._theta_shape(nw)) if theta is None else theta
         logdet = self._empty((nw,)) if logdet is None else logdet
         info = self._empty((nw,), torch.int32) if info is None else info
-        _check(self._call(lib().afqmc_green, self._dev(phi, (nw, self.M, self.N), self.cdtype, "phi"), nw,
-                          self._dev(theta, (nw, self.N, self.M), self.cdtype, "theta"),
+        _check(self._call(lib().afqmc_green, self._dev(phi, self._phi_shape(nw), self.cdtype, "phi"), nw,
+                          self._dev(theta, self._theta_shape(nw), self.cdtype, "theta"),
                           self._dev(logdet, (nw,), self.cdtype, "logdet"), self._dev(info, (nw,), torch.int32, "info")),
                "afqmc_green")
         return theta, logdet, info
@@ -228,7 +264,7 @@ class Afqmc:
     def force_bias(self, theta, vbias=None):
         nw = self._nw(theta, "theta")
         vbias = self._empty((nw, self.nk, self.nchol)) if vbias is None else vbias
-        _check(self._call(lib().afqmc_force_bias, self._dev(theta, (nw, self.N, self.M), self.cdtype, "theta"), nw,
+        _check(self._call(lib().afqmc_force_bias, self._dev(theta, self._theta_shape(nw), self.cdtype, "theta"), nw,
                           self._dev(vbias, (nw, self.nk, self.nchol), self.cdtype, "vbias")), "afqmc_force_bias")
         return vbias
 
@@ -243,13 +279,13 @@ class Afqmc:
     def propagate(self, vhs, dtau, order, phi):
         nw = self._nw(phi, "phi")
         _check(self._call(lib().afqmc_propagate, self._dev(vhs, (nw, self.M, self.M), self.cdtype, "vhs"), float(dtau),
-                          int(order), self._dev(phi, (nw, self.M, self.N), self.cdtype, "phi"), nw), "afqmc_propagate")
+                          int(order), self._dev(phi, self._phi_shape(nw), self.cdtype, "phi"), nw), "afqmc_propagate")
         return phi
 
     def local_energy(self, theta, energy=None):
         nw = self._nw(theta, "theta")
         energy = self._empty((nw, 3)) if energy is None else energy
-        _check(self._call(lib().afqmc_local_energy, self._dev(theta, (nw, self.N, self.M), self.cdtype, "theta"), nw,
+        _check(self._call(lib().afqmc_local_energy, self._dev(theta, self._theta_shape(nw), self.cdtype, "theta"), nw,
                           self._dev(energy, (nw, 3), self.cdtype, "energy")), "afqmc_local_energy")
         return energy
 
@@ -259,7 +295,7 @@ class Afqmc:
         energy = self._empty((nw, 3)) if energy is None else energy
         logdet = self._empty((nw,)) if logdet is None else logdet
         info = self._empty((nw,), torch.int32) if info is None else info
-        _check(self._call(lib().afqmc_step, self._dev(phi, (nw, self.M, self.N), self.cdtype, "phi"),
+        _check(self._call(lib().afqmc_step, self._dev(phi, self._phi_shape(nw), self.cdtype, "phi"),
                           self._dev(x, (nw, self.nk, self.nchol), self.rdtype, "x"), float(dtau), int(order), nw,
                           self._dev(energy, (nw, 3), self.cdtype, "energy"), self._dev(logdet, (nw,), self.cdtype, "logdet"),
                           self._dev(info, (nw,), torch.int32, "info")), "afqmc_step")
@@ -268,7 +304,7 @@ class Afqmc:
     def step_host(self, phi_host, x_host, dtau, order, energy_host, logdet_host=None, info_host=None):
         """Host (ideally pinned) tensors in and out; H2D/D2H copies happen inside the call."""
         nw = self._nw(phi_host, "phi_host")
-        _check(self._call(lib().afqmc_step_host, self._host(phi_host, (nw, self.M, self.N), self.cdtype, "phi_host"),
+        _check(self._call(lib().afqmc_step_host, self._host(phi_host, self._phi_shape(nw), self.cdtype, "phi_host"),
                           self._host(x_host, (nw, self.nk, self.nchol), self.rdtype, "x_host"), float(dtau), int(order), nw,
                           self._host(energy_host, (nw, 3), self.cdtype, "energy_host"),
                           self._host(logdet_host, (nw,), self.cdtype, "logdet_host", optional=True),
@@ -286,7 +322,7 @@ class Afqmc:
 
     def apply_onebody(self, phi):
         nw = self._nw(phi, "phi")
-        _check(self._call(lib().afqmc_apply_onebody, self._dev(phi, (nw, self.M, self.N), torch.complex128, "phi"), nw),
+        _check(self._call(lib().afqmc_apply_onebody, self._dev(phi, self._phi_shape(nw), torch.complex128, "phi"), nw),
                "afqmc_apply_onebody")
         return phi
 
@@ -306,7 +342,7 @@ class Afqmc:
         nw = self._nw(phi, "phi")
         logdet_r = self._empty((nw,), torch.float64) if logdet_r is None else logdet_r
         info = self._empty((nw,), torch.int32) if info is None else info
-        _check(self._call(lib().afqmc_orthogonalize, self._dev(phi, (nw, self.M, self.N), torch.complex128, "phi"), nw,
+        _check(self._call(lib().afqmc_orthogonalize, self._dev(phi, self._phi_shape(nw), torch.complex128, "phi"), nw,
                           self._dev(logdet_r, (nw,), torch.float64, "logdet_r"), self._dev(info, (nw,), torch.int32, "info")),
                "afqmc_orthogonalize")
         return phi, logdet_r, info
@@ -326,7 +362,7 @@ class Afqmc:
         emixed = self._empty((4,)) if emixed is None else emixed
         logdet_r = self._empty((nw,), torch.float64) if logdet_r is None else logdet_r
         info = self._empty((nw,), torch.int32) if info is None else info
-        _check(self._call(lib().afqmc_block, self._dev(phi, (nw, self.M, self.N), torch.complex128, "phi"),
+        _check(self._call(lib().afqmc_block, self._dev(phi, self._phi_shape(nw), torch.complex128, "phi"),
                           self._dev(weight, (nw,), torch.float64, "weight"),
                           self._dev(x, (nsteps, nw, self.nk, self.nchol), torch.float64, "x"), float(dtau), int(order), nsteps, nw,
                           self._dev(energy, (nw, 3), torch.complex128, "energy"), self._dev(emixed, (4,), torch.complex128, "emixed"),

@@ -177,7 +177,7 @@ AFQMC_API int afqmc_apply_onebody(afqmc_ctx* c, void* phi, int nw, void* stream)
     if (c && c->prec32) return AFQMC_UNSUPPORTED;      // the block calls are FP64-only (boundary32.cu)
     if (!c || !phi || nw < 0 || nw > c->max_walkers) return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
-    return afqmc_i_apply_onebody(c, (double2*)phi, nw, (cudaStream_t)stream);
+    return afqmc_x_apply_onebody(c, (double2*)phi, nw, (cudaStream_t)stream);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -190,7 +190,7 @@ constexpr int HW_THREADS = 256;
 
 __global__ void __launch_bounds__(HW_THREADS) hybrid_weight_kernel(
     Dims d, const int* __restrict__ kneg, const double* __restrict__ x, const double2* __restrict__ vbias,
-    double sqrt_dtau, const double2* __restrict__ ld_old, const double2* __restrict__ ld_new,
+    double sqrt_dtau, double spin_factor, const double2* __restrict__ ld_old, const double2* __restrict__ ld_new,
     const int* __restrict__ info /* nullable: status of the two overlap factorisations */,
     double* __restrict__ weight, double2* __restrict__ log_i) {
     __shared__ double red[4][HW_THREADS];
@@ -228,7 +228,8 @@ __global__ void __launch_bounds__(HW_THREADS) hybrid_weight_kernel(
         __syncthreads();
     }
     if (threadIdx.x == 0) {
-        const double lr_r = 2.0 * (ld_new[w].x - ld_old[w].x), lr_i = 2.0 * (ld_new[w].y - ld_old[w].y);
+        // closed shell: both spins share the walker (ratio squared); open shell: logdet already is the sum over channels
+        const double lr_r = spin_factor * (ld_new[w].x - ld_old[w].x), lr_i = spin_factor * (ld_new[w].y - ld_old[w].y);
         const double li_r = lr_r + red[0][0] - 0.5 * red[2][0];
         const double li_i = lr_i + red[1][0] - 0.5 * red[3][0];
         const double twopi = 6.283185307179586476925287, pi = 3.141592653589793238462643;
@@ -269,7 +270,7 @@ __global__ void mixed_estimator_kernel(int nw, const double2* __restrict__ energ
 
 static int hybrid_weight_i(afqmc_ctx* c, const double* x, const double2* vbias, double dtau, const double2* ld_old,
                            const double2* ld_new, const int* info, int nw, double* weight, double2* log_i, cudaStream_t st) {
-    hybrid_weight_kernel<<<nw, HW_THREADS, 0, st>>>(c->d, c->kneg, x, vbias, sqrt(dtau), ld_old, ld_new, info, weight, log_i);
+    hybrid_weight_kernel<<<nw, HW_THREADS, 0, st>>>(c->d, c->kneg, x, vbias, sqrt(dtau), c->spin_factor, ld_old, ld_new, info, weight, log_i);
     AFQMC_LAUNCH_CHECK(c);
     return AFQMC_OK;
 }
@@ -468,11 +469,35 @@ static int orthogonalize_i(afqmc_ctx* c, double2* phi, int nw, double* logdet_r,
     return AFQMC_OK;
 }
 
+namespace {
+__global__ void ortho_merge_kernel(int nw, const double* __restrict__ ldr_dn, const int* __restrict__ info_dn,
+                                   double* __restrict__ logdet_r, int* __restrict__ info) {
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= nw) return;
+    if (logdet_r) logdet_r[w] += ldr_dn[w];
+    if (info && info[w] == 0) info[w] = info_dn[w];
+}
+}  // namespace
+
+// closed shell: one channel; open shell: each spin channel is orthogonalised on its own (log det R = sum, first non-zero info)
+static int orthogonalize_x(afqmc_ctx* c, double2* phi, int nw, double* logdet_r, int* info, int keep_info, cudaStream_t st) {
+    int rc = orthogonalize_i(c, phi, nw, logdet_r, info, keep_info, st);
+    if (rc != AFQMC_OK || !c->dn) return rc;
+    afqmc_ctx* dn = c->dn;
+    rc = orthogonalize_i(dn, phi + (size_t)nw * c->d.M * c->d.N, nw, dn->ws_ldr_chan, dn->ws_info_chan, 0, st);
+    if (rc != AFQMC_OK) return rc;
+    if (logdet_r || info) {
+        ortho_merge_kernel<<<ceil_div(nw, 128), 128, 0, st>>>(nw, dn->ws_ldr_chan, dn->ws_info_chan, logdet_r, info);
+        AFQMC_LAUNCH_CHECK(c);
+    }
+    return AFQMC_OK;
+}
+
 AFQMC_API int afqmc_orthogonalize(afqmc_ctx* c, void* phi, int nw, double* logdet_r, int* info, void* stream) {
     if (c && c->prec32) return AFQMC_UNSUPPORTED;      // the block calls are FP64-only (boundary32.cu)
     if (!c || !phi || nw < 0 || nw > c->max_walkers) return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
-    return orthogonalize_i(c, (double2*)phi, nw, logdet_r, info, 0, (cudaStream_t)stream);
+    return orthogonalize_x(c, (double2*)phi, nw, logdet_r, info, 0, (cudaStream_t)stream);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -507,23 +532,23 @@ AFQMC_API int afqmc_block(afqmc_ctx* c, void* phi, double* weight, const double*
         AFQMC_LAUNCH_CHECK(c);
         return AFQMC_OK;
     };
-    if ((rc = afqmc_i_green(c, ph, nw, c->ws_theta, ld[0], c->ws_info, st)) != AFQMC_OK) return rc;
+    if ((rc = afqmc_x_green(c, ph, nw, c->ws_theta, ld[0], c->ws_info, st)) != AFQMC_OK) return rc;
     if ((rc = merge(1)) != AFQMC_OK) return rc;
     for (int s = 0; s < nsteps; ++s) {
         const double* xs = x + (size_t)s * xstride;
-        if ((rc = afqmc_i_force_bias(c, c->ws_theta, nw, c->ws_vbias, st)) != AFQMC_OK) return rc;
-        if ((rc = afqmc_i_vhs(c, xs, c->ws_vbias, dtau, nw, c->ws_vhs, st)) != AFQMC_OK) return rc;
-        if ((rc = afqmc_i_apply_onebody(c, ph, nw, st)) != AFQMC_OK) return rc;
-        if ((rc = afqmc_i_propagate(c, c->ws_vhs, dtau, order, ph, nw, st)) != AFQMC_OK) return rc;
-        if ((rc = afqmc_i_apply_onebody(c, ph, nw, st)) != AFQMC_OK) return rc;
+        if ((rc = afqmc_x_force_bias(c, c->ws_theta, nw, afqmc_x_vbias_ws(c), st)) != AFQMC_OK) return rc;
+        if ((rc = afqmc_i_vhs(c, xs, afqmc_x_vbias_ws(c), dtau, nw, c->ws_vhs, st)) != AFQMC_OK) return rc;
+        if ((rc = afqmc_x_apply_onebody(c, ph, nw, st)) != AFQMC_OK) return rc;
+        if ((rc = afqmc_x_propagate(c, c->ws_vhs, dtau, order, ph, nw, st)) != AFQMC_OK) return rc;
+        if ((rc = afqmc_x_apply_onebody(c, ph, nw, st)) != AFQMC_OK) return rc;
         // overlap of the new walker = Green's function of the next step (or of the energy evaluation)
-        if ((rc = afqmc_i_green(c, ph, nw, c->ws_theta, ld[(s + 1) & 1], c->ws_info, st)) != AFQMC_OK) return rc;
+        if ((rc = afqmc_x_green(c, ph, nw, c->ws_theta, ld[(s + 1) & 1], c->ws_info, st)) != AFQMC_OK) return rc;
         if ((rc = merge(0)) != AFQMC_OK) return rc;
-        if ((rc = hybrid_weight_i(c, xs, c->ws_vbias, dtau, ld[s & 1], ld[(s + 1) & 1], c->ws_info, nw, weight, nullptr, st)) != AFQMC_OK)
+        if ((rc = hybrid_weight_i(c, xs, afqmc_x_vbias_ws(c), dtau, ld[s & 1], ld[(s + 1) & 1], c->ws_info, nw, weight, nullptr, st)) != AFQMC_OK)
             return rc;
     }
     if ((rc = afqmc_i_local_energy(c, c->ws_theta, nw, (double2*)energy, st)) != AFQMC_OK) return rc;
     mixed_estimator_kernel<<<1, 32, 0, st>>>(nw, (const double2*)energy, weight, (double2*)emixed);
     AFQMC_LAUNCH_CHECK(c);
-    return orthogonalize_i(c, ph, nw, logdet_r, info, 1, st);
+    return orthogonalize_x(c, ph, nw, logdet_r, info, 1, st);
 }

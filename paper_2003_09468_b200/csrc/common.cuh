@@ -84,6 +84,16 @@ struct afqmc_ctx {
     double* ws_ldr;     // [2][nw] log det R of the two Cholesky-QR passes
     int* ws_info2;      // [2][nw] status of the two Cholesky passes
     int b1_set;
+    // open shell (afqmc_dims.closed_shell = 0): this context is the spin-UP channel and owns everything spin independent;
+    // `dn` is the spin-DOWN channel (is_child = 1: no vHS operand / workspace, b1 shared).  spin_factor = 2 for a closed
+    // shell (one channel stands for both spins: E1, vbias, EX carry it), 1 per channel of an open shell.
+    afqmc_ctx* dn;
+    int is_child;
+    double spin_factor;
+    double2* ws_vbtot;  // [nw][Nk][nchol] spin-summed force bias (open shell)
+    double2* ws_ld_chan; // [nw] this channel's log det (open shell: combined by openshell.cu)
+    int* ws_info_chan;  // [nw] this channel's status
+    double* ws_ldr_chan; // [nw] this channel's log det R of the orthogonalisation
     int prec32;         // 1 = complex64 boundary (afqmc_dims.precision = 1, boundary32.cu)
     float* ws_f32;      // precision 1: device staging of afqmc_step_host ([nw][M][N][2] + x + energy + logdet floats)
     long long launches;
@@ -250,6 +260,27 @@ size_t afqmc_i_lxt_floats(const Dims& d);
 int afqmc_i_apply_onebody(afqmc_ctx* c, double2* phi, int nw, cudaStream_t st);
 int afqmc_i_step(afqmc_ctx* c, double2* phi, const double* x, double dtau, int order, int nw, double2* energy,
                  double2* logdet, int* info, cudaStream_t st, cudaEvent_t phi_final /* nullable: recorded after the propagation */);
+// open shell (openshell.cu): `c` is the spin-up context, c->dn the spin-down one; arrays are spin-major (up block, dn block)
+int afqmc_os_green(afqmc_ctx* c, const double2* phi, int nw, double2* theta, double2* logdet, int* info, cudaStream_t st);
+int afqmc_os_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias, cudaStream_t st);
+int afqmc_os_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, double2* phi, int nw, cudaStream_t st);
+int afqmc_os_apply_onebody(afqmc_ctx* c, double2* phi, int nw, cudaStream_t st);
+// closed / open shell dispatch used by the compositions (step, block): same argument meaning, spin-major arrays when open
+static inline int afqmc_x_green(afqmc_ctx* c, const double2* phi, int nw, double2* theta, double2* logdet, int* info, cudaStream_t st) {
+    return c->dn ? afqmc_os_green(c, phi, nw, theta, logdet, info, st) : afqmc_i_green(c, phi, nw, theta, logdet, info, st);
+}
+static inline double2* afqmc_x_vbias_ws(afqmc_ctx* c) { return c->dn ? c->ws_vbtot : c->ws_vbias; }
+static inline int afqmc_x_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias, cudaStream_t st) {
+    return c->dn ? afqmc_os_force_bias(c, theta, nw, vbias, st) : afqmc_i_force_bias(c, theta, nw, vbias, st);
+}
+static inline int afqmc_x_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, double2* phi, int nw, cudaStream_t st) {
+    return c->dn ? afqmc_os_propagate(c, vhs, dtau, order, phi, nw, st) : afqmc_i_propagate(c, vhs, dtau, order, phi, nw, st);
+}
+static inline int afqmc_x_apply_onebody(afqmc_ctx* c, double2* phi, int nw, cudaStream_t st) {
+    return c->dn ? afqmc_os_apply_onebody(c, phi, nw, st) : afqmc_i_apply_onebody(c, phi, nw, st);
+}
+// complex numbers of one walker batch entry: all spin channels
+static inline size_t afqmc_x_phi_elems(const afqmc_ctx* c) { return (size_t)c->d.M * (c->d.N + (c->dn ? c->dn->d.N : 0)); }
 // complex64 boundary (boundary32.cu): same calls on float arrays, staged through the FP64 workspace
 int afqmc32_widen_alloc(afqmc_ctx* c, const void* in, size_t ndoubles, double** out, cudaStream_t st);
 int afqmc32_green(afqmc_ctx* c, const void* phi, int nw, void* theta, void* logdet, int* info, cudaStream_t st);

@@ -145,9 +145,11 @@ static int dev_alloc(T** p, size_t count) {
 
 AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     if (!c) return;
+    if (c->dn) { afqmc_destroy(c->dn); c->dn = nullptr; }
+    if (c->is_child) c->b1 = nullptr;        // owned by the spin-up context
     void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lh, c->Lxc, c->Lx3t, c->Lx, c->LxT, c->Lf, c->Lv3, c->vunits,
                     c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T, c->ws_Tx,
-                    c->ws_expart, c->ws_fbpart, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
+                    c->ws_expart, c->ws_fbpart, c->ws_vbtot, c->ws_ld_chan, c->ws_info_chan, c->ws_ldr_chan, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
                     c->ws_f32, c->b1, c->ws_b1tmp, c->ws_gram, c->ws_rinv, c->ws_logdet2, c->ws_ldr, c->ws_info2};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -159,25 +161,18 @@ AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     delete c;
 }
 
-AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* h1, const void* L,
-                            const void* psi_t, void* stream) {
-    if (!out) return AFQMC_INVALID_ARGUMENT;
+// One spin channel: the whole closed-shell context (n = `n_chan` occupied orbitals per k-point), or one of the two channels
+// of an open-shell context (spin_factor 1).  The spin-DOWN channel (`child`) has no vHS operand, no field / vHS workspace
+// and no one-body propagator of its own: those are spin independent and live in the spin-up (parent) context.
+static int create_channel(afqmc_ctx** out, const afqmc_dims* dims, int n_chan, int n_total, const void* h1, const void* L,
+                          const void* psi_t, cudaStream_t st, bool child, bool open_shell) {
     *out = nullptr;
-    if (!dims || !h1 || !L || !psi_t) return AFQMC_INVALID_ARGUMENT;
-    if (dims->g[0] < 1 || dims->g[1] < 1 || dims->g[2] < 1 || dims->m < 1 || dims->n < 1 ||
-        dims->n > dims->m || dims->nchol < 1 || dims->max_walkers < 1)
-        return AFQMC_INVALID_ARGUMENT;
-    long long nk_ll = (long long)dims->g[0] * dims->g[1] * dims->g[2];
-    if (nk_ll > AFQMC_MAX_NK) return AFQMC_INVALID_ARGUMENT;
-    if (dims->closed_shell != 1) return AFQMC_UNSUPPORTED;
-    if (dims->precision != 0 && dims->precision != 1) return AFQMC_UNSUPPORTED;
-    cudaStream_t st = (cudaStream_t)stream;
-
+    const long long nk_ll = (long long)dims->g[0] * dims->g[1] * dims->g[2];
     afqmc_ctx* c = new afqmc_ctx();
     memset(c, 0, sizeof(*c));
     Dims& d = c->d;
     for (int i = 0; i < 3; ++i) d.g[i] = dims->g[i];
-    d.Nk = (int)nk_ll; d.m = dims->m; d.n = dims->n; d.nchol = dims->nchol;
+    d.Nk = (int)nk_ll; d.m = dims->m; d.n = n_chan; d.nchol = dims->nchol;
     d.M = d.Nk * d.m; d.N = d.Nk * d.n;
     d.KS = (2 * d.m + 3) / 4;
     d.NAG = (d.n + 3) / 4;
@@ -190,6 +185,8 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     c->opt_fb_pf = 8;
     c->opt_exchange_3m = 1;
     c->opt_exchange_regb = 1;
+    c->spin_factor = open_shell ? 1.0 : 2.0;
+    c->is_child = child ? 1 : 0;
     const int nw = c->max_walkers;
 
     int dev = 0;
@@ -240,10 +237,13 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     A(dev_alloc(&c->Lf, nLf));
     A(dev_alloc(&c->ws_O, (size_t)nw * d.N * LD));
     A(dev_alloc(&c->ws_oinvT, (size_t)nw * d.N * d.N));
-    A(dev_alloc(&c->ws_theta, (size_t)nw * d.N * d.M));
+    A(dev_alloc(&c->ws_theta, (size_t)nw * (child ? d.N : Nk * n_total) * d.M));     // spin-up context: both channels, spin-major
     A(dev_alloc(&c->ws_vbias, (size_t)nw * Nk * d.nchol));
-    A(dev_alloc(&c->ws_xi, (afqmc_i_vhs_field_doubles(d, nw) + 1) / 2));   // expanded field fragments (vhs.cu)
-    A(dev_alloc(&c->ws_vhs, (size_t)nw * d.M * d.M));
+    if (!child) {
+        A(dev_alloc(&c->ws_xi, (afqmc_i_vhs_field_doubles(d, nw) + 1) / 2));   // expanded field fragments (vhs.cu)
+        A(dev_alloc(&c->ws_vhs, (size_t)nw * d.M * d.M));
+        if (open_shell) A(dev_alloc(&c->ws_vbtot, (size_t)nw * Nk * d.nchol));  // spin-summed force bias
+    }
     A(dev_alloc(&c->ws_T, (size_t)2 * nw * d.M * d.N));
     const size_t nTx = (size_t)2 * nw * afqmc_i_taylor_ws_doubles(d);
     A(dev_alloc(&c->ws_Tx, nTx));
@@ -251,18 +251,25 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
     c->ex_parts = 1;
     A(dev_alloc(&c->ws_expart, (size_t)c->nunits * nw * c->ex_parts_max));
     A(dev_alloc(&c->ws_fbpart, (size_t)AFQMC_FB_MAXKC * nw * Nk * d.nchol));
-    A(dev_alloc(&c->ws_x, (size_t)nw * Nk * d.nchol));
-    A(dev_alloc(&c->ws_phi, (size_t)nw * d.M * d.N));
+    if (!child) {      // host-entry staging: all channels of a walker batch
+        A(dev_alloc(&c->ws_x, (size_t)nw * Nk * d.nchol));
+        A(dev_alloc(&c->ws_phi, (size_t)nw * d.M * Nk * n_total));
+    }
     A(dev_alloc(&c->ws_energy, (size_t)nw * 3));
     A(dev_alloc(&c->ws_logdet, (size_t)nw));
     A(dev_alloc(&c->ws_info, (size_t)nw));
-    A(dev_alloc(&c->b1, (size_t)Nk * d.m * d.m));
-    A(dev_alloc(&c->ws_b1tmp, (size_t)Nk * 3 * d.m * d.m));
+    if (!child) {
+        A(dev_alloc(&c->b1, (size_t)Nk * d.m * d.m));
+        A(dev_alloc(&c->ws_b1tmp, (size_t)Nk * 3 * d.m * d.m));
+    }
     A(dev_alloc(&c->ws_gram, (size_t)nw * d.N * d.N));
     A(dev_alloc(&c->ws_rinv, (size_t)nw * d.N * d.N));
     A(dev_alloc(&c->ws_logdet2, (size_t)nw));
     A(dev_alloc(&c->ws_ldr, (size_t)2 * nw));
     A(dev_alloc(&c->ws_info2, (size_t)2 * nw));
+    A(dev_alloc(&c->ws_ld_chan, (size_t)nw));
+    A(dev_alloc(&c->ws_info_chan, (size_t)nw));
+    A(dev_alloc(&c->ws_ldr_chan, (size_t)nw));
     if (c->prec32) A(dev_alloc(&c->ws_f32, (size_t)nw * ((size_t)d.M * d.N * 2 + (size_t)Nk * d.nchol + 8)));
     if (rc != AFQMC_OK) { afqmc_destroy(c); return rc; }
     // complex64 boundary: the static inputs are widened once into FP64 temporaries (freed before returning)
@@ -297,7 +304,7 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
         c->launches += 3;
         if (cudaGetLastError() != cudaSuccess) rc = AFQMC_CUDA_ERROR;
         if (rc == AFQMC_OK) rc = afqmc_i_pack_exchange_operand(c, st);
-        if (rc == AFQMC_OK) rc = afqmc_i_vhs_setup(c, (const double2*)L, kminus, kneg, st);
+        if (rc == AFQMC_OK && !child) rc = afqmc_i_vhs_setup(c, (const double2*)L, kminus, kneg, st);
     }
     // host vectors must outlive the async copies; the caller may free its arrays after return
     if (cudaStreamSynchronize(st) != cudaSuccess && rc == AFQMC_OK) rc = AFQMC_CUDA_ERROR;
@@ -310,6 +317,35 @@ AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* 
         c->opt_exchange_prec = 1;
     }
     *out = c;
+    return AFQMC_OK;
+}
+
+AFQMC_API int afqmc_create(afqmc_ctx** out, const afqmc_dims* dims, const void* h1, const void* L,
+                            const void* psi_t, void* stream) {
+    if (!out) return AFQMC_INVALID_ARGUMENT;
+    *out = nullptr;
+    if (!dims || !h1 || !L || !psi_t) return AFQMC_INVALID_ARGUMENT;
+    if (dims->g[0] < 1 || dims->g[1] < 1 || dims->g[2] < 1 || dims->m < 1 || dims->n < 1 ||
+        dims->n > dims->m || dims->nchol < 1 || dims->max_walkers < 1)
+        return AFQMC_INVALID_ARGUMENT;
+    const long long nk_ll = (long long)dims->g[0] * dims->g[1] * dims->g[2];
+    if (nk_ll > AFQMC_MAX_NK) return AFQMC_INVALID_ARGUMENT;
+    if (dims->closed_shell != 0 && dims->closed_shell != 1) return AFQMC_INVALID_ARGUMENT;
+    if (dims->precision != 0 && dims->precision != 1) return AFQMC_UNSUPPORTED;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dims->closed_shell == 1) return create_channel(out, dims, dims->n, dims->n, h1, L, psi_t, st, false, false);
+    // open shell: n = spin-up, n_dn = spin-down occupied orbitals per k-point; psi_t = [Nk][m][n] then [Nk][m][n_dn]
+    if (dims->n_dn < 1 || dims->n_dn > dims->m) return AFQMC_INVALID_ARGUMENT;
+    if (dims->precision != 0) return AFQMC_UNSUPPORTED;        // the complex64 boundary is closed-shell only
+    afqmc_ctx *up = nullptr, *dn = nullptr;
+    int rc = create_channel(&up, dims, dims->n, dims->n + dims->n_dn, h1, L, psi_t, st, false, true);
+    if (rc != AFQMC_OK) return rc;
+    const double2* psi_dn = (const double2*)psi_t + (size_t)nk_ll * dims->m * dims->n;
+    rc = create_channel(&dn, dims, dims->n_dn, dims->n + dims->n_dn, h1, L, psi_dn, st, true, true);
+    if (rc != AFQMC_OK) { afqmc_destroy(up); return rc; }
+    dn->b1 = up->b1;            // shared (owned by the spin-up context)
+    up->dn = dn;
+    *out = up;
     return AFQMC_OK;
 }
 
@@ -339,6 +375,7 @@ AFQMC_API long long afqmc_launch_count(const afqmc_ctx* c) { return c ? c->launc
 
 AFQMC_API double afqmc_exchange_flops(const afqmc_ctx* c, int nw) {
     if (!c) return 0.0;
+    if (c->dn) { afqmc_ctx up = *c; up.dn = nullptr; return afqmc_exchange_flops(&up, nw) + afqmc_exchange_flops(c->dn, nw); }
     const Dims& d = c->d;
     // per unit and walker: two complex GEMMs (n x m)(m x n) per gamma, plus the complex contraction 8*n*n*nchol.
     // 4M kernel: 8 real flops per complex multiply-add = 2 * 8*n*n*m*nchol.  3M kernel (exchange3m.cu): 6 real
@@ -352,6 +389,10 @@ AFQMC_API double afqmc_exchange_flops(const afqmc_ctx* c, int nw) {
 
 AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
     if (!c || !name) return AFQMC_INVALID_ARGUMENT;
+    if (c->dn && strcmp(name, "timers") != 0) {     // tuning options apply to both spin channels
+        int rc = afqmc_set_option(c->dn, name, value);
+        if (rc != AFQMC_OK) return rc;
+    }
     if (strcmp(name, "exchange_warps") == 0) {
         if (value != 0 && value != 2 && value != 4 && value != 5 && value != 6 && value != 8) return AFQMC_INVALID_ARGUMENT;
         c->opt_exchange_wpc = value;

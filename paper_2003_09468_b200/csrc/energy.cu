@@ -219,38 +219,50 @@ __device__ double2 block_sum2(double2 v, double* scratch /* >= 64 doubles */) {
     return r;
 }
 
+// One spin channel's inputs of the final reduction
+struct FinChan {
+    int n, N, nunits, parts;
+    const int* units;
+    const double2 *ht, *theta, *vbias, *partial;      // vbias: this channel's force bias including its spin factor
+};
+
+// sf = spin factor (2: closed shell, one channel for both spins; 1: open shell, two channels):
+//   E1 = sf sum_ch sum ht theta;   EC = 1/2 sum_Q sum_g v[Q][g] v[-Q][g], v = sum_ch vbias_ch;   EX = -(sf/2) sum_ch sum_units mult X
 __global__ void __launch_bounds__(1024) energy_finalize_kernel(
-    Dims d, int nw, int nunits, int parts, const int* __restrict__ units, const int* __restrict__ kneg,
-    const double2* __restrict__ ht, const double2* __restrict__ theta, const double2* __restrict__ vbias,
-    const double2* __restrict__ partial, double2* __restrict__ energy) {
+    Dims d, int nw, int nchan, double sf, FinChan c0, FinChan c1, const int* __restrict__ kneg, double2* __restrict__ energy) {
     __shared__ double scratch[64];
     const int w = blockIdx.x, tid = threadIdx.x;
-    // E1 = 2 sum_k sum_{a,q} ht[k][a][q] theta[(k,a),(k,q)]
-    double2 e1 = make_double2(0.0, 0.0);
-    for (int e = tid; e < d.Nk * d.n * d.m; e += blockDim.x) {
-        int q = e % d.m, ka = e / d.m, k = ka / d.n;
-        e1 = cfma(ht[e], theta[((size_t)w * d.N + ka) * d.M + (size_t)k * d.m + q], e1);
+    double2 e1 = make_double2(0.0, 0.0), ex = make_double2(0.0, 0.0);
+    for (int ch = 0; ch < nchan; ++ch) {
+        const FinChan& c = ch == 0 ? c0 : c1;
+        // E1 = sum_k sum_{a,q} ht[k][a][q] theta[(k,a),(k,q)]
+        for (int e = tid; e < d.Nk * c.n * d.m; e += blockDim.x) {
+            int q = e % d.m, ka = e / d.m, k = ka / c.n;
+            e1 = cfma(c.ht[e], c.theta[((size_t)w * c.N + ka) * d.M + (size_t)k * d.m + q], e1);
+        }
+        // EX = - sum_units mult * X(unit); `parts` partial sums per unit (1 except for large blocks)
+        for (int idx = tid; idx < c.nunits * c.parts; idx += blockDim.x) {
+            double mult = (double)c.units[4 * (idx / c.parts) + 3];
+            double2 p = c.partial[(size_t)idx * nw + w];
+            ex.x += mult * p.x; ex.y += mult * p.y;
+        }
     }
     e1 = block_sum2(e1, scratch);
+    ex = block_sum2(ex, scratch);
     // EC = 1/2 sum_Q sum_g v[Q][g] v[-Q][g]
     double2 ec = make_double2(0.0, 0.0);
     for (int e = tid; e < d.Nk * d.nchol; e += blockDim.x) {
         int g = e % d.nchol, Q = e / d.nchol;
-        ec = cfma(vbias[((size_t)w * d.Nk + Q) * d.nchol + g], vbias[((size_t)w * d.Nk + kneg[Q]) * d.nchol + g], ec);
+        const size_t i0 = ((size_t)w * d.Nk + Q) * d.nchol + g, i1 = ((size_t)w * d.Nk + kneg[Q]) * d.nchol + g;
+        double2 a = c0.vbias[i0], b = c0.vbias[i1];
+        if (nchan > 1) { const double2 a1 = c1.vbias[i0], b1 = c1.vbias[i1]; a.x += a1.x; a.y += a1.y; b.x += b1.x; b.y += b1.y; }
+        ec = cfma(a, b, ec);
     }
     ec = block_sum2(ec, scratch);
-    // EX = - sum_units mult * X(unit)
-    double2 ex = make_double2(0.0, 0.0);
-    for (int idx = tid; idx < nunits * parts; idx += blockDim.x) {     // `parts` partial sums per unit (1 except for large blocks)
-        double mult = (double)units[4 * (idx / parts) + 3];
-        double2 p = partial[(size_t)idx * nw + w];
-        ex.x += mult * p.x; ex.y += mult * p.y;
-    }
-    ex = block_sum2(ex, scratch);
     if (tid == 0) {
-        energy[w * 3 + 0] = make_double2(2.0 * e1.x, 2.0 * e1.y);
+        energy[w * 3 + 0] = make_double2(sf * e1.x, sf * e1.y);
         energy[w * 3 + 1] = make_double2(0.5 * ec.x, 0.5 * ec.y);
-        energy[w * 3 + 2] = make_double2(-ex.x, -ex.y);
+        energy[w * 3 + 2] = make_double2(-0.5 * sf * ex.x, -0.5 * sf * ex.y);
     }
 }
 
@@ -319,11 +331,11 @@ int launch_exchange(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st)
 
 }  // namespace
 
-int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* energy, cudaStream_t st) {
-    const Dims& d = c->d;
+// force bias (the traces of steps 2(d)) and exchange partial sums of ONE spin channel, left in its workspace
+static int channel_energy_parts(afqmc_ctx* c, afqmc_ctx* timers, const double2* theta, int nw, cudaStream_t st) {
     int rc = afqmc_i_force_bias(c, theta, nw, c->ws_vbias, st);     // steps 2(d): the traces are the force bias
     if (rc != AFQMC_OK) return rc;
-    afqmc_mark(c, 6, st);
+    if (timers) afqmc_mark(timers, 6, st);
     c->ex_parts = 1;
     rc = c->opt_exchange_prec != 0 ? afqmc_i_exchange_tf32(c, theta, nw, st)
          : c->opt_exchange_3m    ? afqmc_i_exchange3m(c, theta, nw, st) : AFQMC_UNSUPPORTED;
@@ -332,10 +344,29 @@ int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* en
         if (nw >= 3) rc = launch_exchange<4>(c, theta, nw, st);
         else rc = launch_exchange<2>(c, theta, nw, st);
     }
+    return rc;
+}
+
+static FinChan fin_chan(const afqmc_ctx* c, const double2* theta) {
+    FinChan f;
+    f.n = c->d.n; f.N = c->d.N; f.nunits = c->nunits; f.parts = c->ex_parts;
+    f.units = c->units; f.ht = c->ht; f.theta = theta; f.vbias = c->ws_vbias; f.partial = c->ws_expart;
+    return f;
+}
+
+// theta: [nw][N][M]; open shell: the spin-up block followed by the spin-down block [nw][N_dn][M]
+int afqmc_i_local_energy(afqmc_ctx* c, const double2* theta, int nw, double2* energy, cudaStream_t st) {
+    const Dims& d = c->d;
+    int rc = channel_energy_parts(c, c->dn ? nullptr : c, theta, nw, st);
     if (rc != AFQMC_OK) return rc;
+    const double2* theta_dn = theta + (size_t)nw * d.N * d.M;
+    if (c->dn) {
+        if ((rc = channel_energy_parts(c->dn, nullptr, theta_dn, nw, st)) != AFQMC_OK) return rc;
+        afqmc_mark(c, 6, st);
+    }
     afqmc_mark(c, 7, st);
-    energy_finalize_kernel<<<nw, 1024, 0, st>>>(d, nw, c->nunits, c->ex_parts, c->units, c->kneg, c->ht, theta, c->ws_vbias,
-                                              c->ws_expart, energy);
+    const FinChan f0 = fin_chan(c, theta), f1 = c->dn ? fin_chan(c->dn, theta_dn) : f0;
+    energy_finalize_kernel<<<nw, 1024, 0, st>>>(d, nw, c->dn ? 2 : 1, c->spin_factor, f0, f1, c->kneg, energy);
     AFQMC_LAUNCH_CHECK(c);
     return AFQMC_OK;
 }

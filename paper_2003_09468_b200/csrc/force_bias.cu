@@ -1,4 +1,5 @@
-// a4 force bias:  vbias[w][Q][g] = 2 sum_k sum_{a,r} Lh[Q][k][a][g][r] theta_w[(k,a),(k-Q,r)]
+// a4 force bias:  vbias[w][Q][g] = f_s sum_k sum_{a,r} Lh[Q][k][a][g][r] theta_w[(k,a),(k-Q,r)]      (f_s = 2: closed shell;
+// open shell: f_s = 1 per spin channel and the two channels are added, openshell.cu)
 // (the half-rotated contraction of Eq. 47; = 2 X_g of Eq. 37).
 //
 // Per Q this is a real-embedded complex GEMM on the FP64 tensor pipe:
@@ -25,7 +26,7 @@ constexpr int FB_D = 3;   // k-steps of register prefetch (3 CTAs of 4 warps sta
 template <int MP, int NT>
 __global__ void __launch_bounds__(32 * FB_WARPS, (MP * NT > 8 ? 2 : 3)) force_bias_kernel(
     Dims d, int nw, int KC, int nmg, int nwgrp, int pf, const int* __restrict__ kminus, const double* __restrict__ Lf,
-    const double2* __restrict__ theta, double2* __restrict__ out, int out_is_partial) {
+    const double2* __restrict__ theta, double2* __restrict__ out, int out_is_partial, double spin_factor) {
     extern __shared__ __align__(16) double fb_smem[];
     // blockIdx.x = ((Q*KC + kc)*nwgrp + wgrp)*nmg + mg
     int bx = blockIdx.x;
@@ -157,7 +158,7 @@ __global__ void __launch_bounds__(32 * FB_WARPS, (MP * NT > 8 ? 2 : 3)) force_bi
         __syncthreads();
     }
     if (warp == 0) {
-        const double scale = out_is_partial ? 1.0 : 2.0;
+        const double scale = out_is_partial ? 1.0 : spin_factor;      // 2 = both spins of a closed shell, 1 = one channel
         double2* dst = out + (out_is_partial ? (size_t)kc * nw * d.Nk * d.nchol : 0);
 #pragma unroll
         for (int i = 0; i < 2 * MP; ++i) {
@@ -173,12 +174,12 @@ __global__ void __launch_bounds__(32 * FB_WARPS, (MP * NT > 8 ? 2 : 3)) force_bi
     }
 }
 
-// vbias = 2 * sum over K chunks of the partial results, in chunk order
-__global__ void force_bias_reduce_kernel(size_t n, int KC, const double2* __restrict__ part, double2* __restrict__ vbias) {
+// vbias = spin_factor * sum over K chunks of the partial results, in chunk order
+__global__ void force_bias_reduce_kernel(size_t n, int KC, double spin_factor, const double2* __restrict__ part, double2* __restrict__ vbias) {
     for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
         double2 s = part[e];
         for (int c = 1; c < KC; ++c) { const double2 p = part[(size_t)c * n + e]; s.x += p.x; s.y += p.y; }
-        vbias[e] = make_double2(2.0 * s.x, 2.0 * s.y);
+        vbias[e] = make_double2(spin_factor * s.x, spin_factor * s.y);
     }
 }
 
@@ -202,13 +203,13 @@ int launch_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias
     auto kern = force_bias_kernel<MP, NT>;
     if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
     kern<<<(unsigned)(base * KC), 32 * FB_WARPS, smem, st>>>(d, nw, KC, nmg, nwgrp, c->opt_fb_pf, c->kminus, c->Lf, theta,
-                                                             KC > 1 ? c->ws_fbpart : vbias, KC > 1 ? 1 : 0);
+                                                             KC > 1 ? c->ws_fbpart : vbias, KC > 1 ? 1 : 0, c->spin_factor);
     AFQMC_LAUNCH_CHECK(c);
     if (KC > 1) {
         const size_t n = (size_t)nw * d.Nk * d.nchol;
         int G = (int)((n + 255) / 256);
         if (G > c->num_sms * 8) G = c->num_sms * 8;
-        force_bias_reduce_kernel<<<G, 256, 0, st>>>(n, KC, c->ws_fbpart, vbias);
+        force_bias_reduce_kernel<<<G, 256, 0, st>>>(n, KC, c->spin_factor, c->ws_fbpart, vbias);
         AFQMC_LAUNCH_CHECK(c);
     }
     return AFQMC_OK;
@@ -233,5 +234,6 @@ AFQMC_API int afqmc_force_bias(afqmc_ctx* c, const void* theta, int nw, void* vb
     if (!c || !theta || !vbias || nw < 0 || nw > c->max_walkers) return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
     if (c->prec32) return afqmc32_force_bias(c, theta, nw, vbias, (cudaStream_t)stream);
+    if (c->dn) return afqmc_os_force_bias(c, (const double2*)theta, nw, (double2*)vbias, (cudaStream_t)stream);
     return afqmc_i_force_bias(c, (const double2*)theta, nw, (double2*)vbias, (cudaStream_t)stream);
 }

@@ -460,7 +460,7 @@ AFQMC_API int afqmc_overlap(afqmc_ctx* c, const void* phi, int nw, void* logdet,
     if (!c || !phi || !logdet || nw < 0 || nw > c->max_walkers) return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
     if (c->prec32) return afqmc32_green(c, phi, nw, nullptr, logdet, info, (cudaStream_t)stream);
-    return afqmc_i_green(c, (const double2*)phi, nw, nullptr, (double2*)logdet, info, (cudaStream_t)stream);
+    return afqmc_x_green(c, (const double2*)phi, nw, nullptr, (double2*)logdet, info, (cudaStream_t)stream);
 }
 
 AFQMC_API int afqmc_green(afqmc_ctx* c, const void* phi, int nw, void* theta, void* logdet, int* info,
@@ -468,5 +468,5 @@ AFQMC_API int afqmc_green(afqmc_ctx* c, const void* phi, int nw, void* theta, vo
     if (!c || !phi || !theta || nw < 0 || nw > c->max_walkers) return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
     if (c->prec32) return afqmc32_green(c, phi, nw, theta, logdet, info, (cudaStream_t)stream);
-    return afqmc_i_green(c, (const double2*)phi, nw, (double2*)theta, (double2*)logdet, info, (cudaStream_t)stream);
+    return afqmc_x_green(c, (const double2*)phi, nw, (double2*)theta, (double2*)logdet, info, (cudaStream_t)stream);
 }

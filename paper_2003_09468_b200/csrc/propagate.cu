@@ -58,5 +58,5 @@ AFQMC_API int afqmc_propagate(afqmc_ctx* c, const void* vhs, double dtau, int or
         return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
     if (c->prec32) return afqmc32_propagate(c, vhs, dtau, order, phi, nw, (cudaStream_t)stream);
-    return afqmc_i_propagate(c, (const double2*)vhs, dtau, order, (double2*)phi, nw, (cudaStream_t)stream);
+    return afqmc_x_propagate(c, (const double2*)vhs, dtau, order, (double2*)phi, nw, (cudaStream_t)stream);
 }

@@ -6,16 +6,16 @@ int afqmc_i_step(afqmc_ctx* c, double2* ph, const double* x, double dtau, int or
                  double2* logdet, int* info, cudaStream_t st, cudaEvent_t phi_final) {
     int rc;
     afqmc_mark(c, 0, st);
-    if ((rc = afqmc_i_green(c, ph, nw, c->ws_theta, nullptr, nullptr, st)) != AFQMC_OK) return rc;
+    if ((rc = afqmc_x_green(c, ph, nw, c->ws_theta, nullptr, nullptr, st)) != AFQMC_OK) return rc;
     afqmc_mark(c, 1, st);
-    if ((rc = afqmc_i_force_bias(c, c->ws_theta, nw, c->ws_vbias, st)) != AFQMC_OK) return rc;
+    if ((rc = afqmc_x_force_bias(c, c->ws_theta, nw, afqmc_x_vbias_ws(c), st)) != AFQMC_OK) return rc;
     afqmc_mark(c, 2, st);
-    if ((rc = afqmc_i_vhs(c, x, c->ws_vbias, dtau, nw, c->ws_vhs, st)) != AFQMC_OK) return rc;
+    if ((rc = afqmc_i_vhs(c, x, afqmc_x_vbias_ws(c), dtau, nw, c->ws_vhs, st)) != AFQMC_OK) return rc;
     afqmc_mark(c, 3, st);
-    if ((rc = afqmc_i_propagate(c, c->ws_vhs, dtau, order, ph, nw, st)) != AFQMC_OK) return rc;
+    if ((rc = afqmc_x_propagate(c, c->ws_vhs, dtau, order, ph, nw, st)) != AFQMC_OK) return rc;
     afqmc_mark(c, 4, st);
     if (phi_final) AFQMC_CUDA_TRY(cudaEventRecord(phi_final, st));      // the propagated walkers are final from here on
-    if ((rc = afqmc_i_green(c, ph, nw, c->ws_theta, logdet, info, st)) != AFQMC_OK) return rc;
+    if ((rc = afqmc_x_green(c, ph, nw, c->ws_theta, logdet, info, st)) != AFQMC_OK) return rc;
     afqmc_mark(c, 5, st);
     if ((rc = afqmc_i_local_energy(c, c->ws_theta, nw, energy, st)) != AFQMC_OK) return rc;
     afqmc_mark(c, 8, st);      // marks 6 and 7 are recorded around the exchange kernel inside local_energy
@@ -40,7 +40,7 @@ AFQMC_API int afqmc_step_host(afqmc_ctx* c, void* phi_host, const double* x_host
     cudaStream_t st = (cudaStream_t)stream;
     if (c->prec32) return afqmc32_step_host(c, phi_host, x_host, dtau, order, nw, energy_host, logdet_host, info_host, st);
     const Dims& d = c->d;
-    const size_t phi_bytes = (size_t)nw * d.M * d.N * sizeof(double2);
+    const size_t phi_bytes = (size_t)nw * afqmc_x_phi_elems(c) * sizeof(double2);
     const size_t x_bytes = (size_t)nw * d.Nk * d.nchol * sizeof(double);
     // a second stream carries the download of the propagated walkers while the energy of those walkers is evaluated
     if (!c->copy_stream) {

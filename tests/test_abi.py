@@ -39,7 +39,7 @@ def test_create_rejects_bad_arguments_before_touching_cuda():
     from paper_2003_09468_b200 import binding
     lib = binding.lib()
     h = ctypes.c_void_p(0)
-    d = binding.Dims((ctypes.c_int * 3)(2, 2, 2), 8, 4, 32, 1, 0, 4)
+    d = binding.Dims((ctypes.c_int * 3)(2, 2, 2), 8, 4, 32, 1, 0, 4, 0)
     assert lib.afqmc_create(ctypes.byref(h), ctypes.byref(d), None, None, None, None) == 1
     assert lib.afqmc_create(None, ctypes.byref(d), None, None, None, None) == 1
     lib.afqmc_destroy(None)

@@ -421,11 +421,11 @@ def test_argument_errors(small_case):
     assert lib.afqmc_propagate(case.ctx._h, phi_d.data_ptr(), 0.005, 33, phi_d.data_ptr(), 1, None) == 1
     import ctypes
     h = ctypes.c_void_p(0)
-    d = binding.Dims((ctypes.c_int * 3)(2, 2, 1), 6, 4, 10, 0, 0, 4)       # open shell
+    d = binding.Dims((ctypes.c_int * 3)(2, 2, 1), 6, 4, 10, 0, 0, 4, 0)    # open shell without a spin-down orbital count
+    assert lib.afqmc_create(ctypes.byref(h), ctypes.byref(d), phi_d.data_ptr(), phi_d.data_ptr(), phi_d.data_ptr(), None) == 1
+    d = binding.Dims((ctypes.c_int * 3)(2, 2, 1), 6, 4, 10, 1, 2, 4, 0)    # precision: only 0 (complex128) and 1 (complex64) exist
     assert lib.afqmc_create(ctypes.byref(h), ctypes.byref(d), phi_d.data_ptr(), phi_d.data_ptr(), phi_d.data_ptr(), None) == 2
-    d = binding.Dims((ctypes.c_int * 3)(2, 2, 1), 6, 4, 10, 1, 2, 4)       # precision: only 0 (complex128) and 1 (complex64) exist
-    assert lib.afqmc_create(ctypes.byref(h), ctypes.byref(d), phi_d.data_ptr(), phi_d.data_ptr(), phi_d.data_ptr(), None) == 2
-    d = binding.Dims((ctypes.c_int * 3)(2, 2, 1), 6, 7, 10, 1, 0, 4)       # n > m
+    d = binding.Dims((ctypes.c_int * 3)(2, 2, 1), 6, 7, 10, 1, 0, 4, 0)    # n > m
     assert lib.afqmc_create(ctypes.byref(h), ctypes.byref(d), phi_d.data_ptr(), phi_d.data_ptr(), phi_d.data_ptr(), None) == 1
 
 
