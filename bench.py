@@ -428,6 +428,7 @@ def run_ours(args):
         torch.cuda.empty_cache()
         pb64 = synth.make_problem(cfg)
         c64 = binding.from_problem(pb64, precision=1)
+        c64.set_option("timers", 1)
         phi64_0 = torch.from_numpy(pb64.phi).to(torch.complex64).cuda()
         x32 = torch.from_numpy(pb64.x).to(torch.float32).cuda()
         ms64 = []
@@ -441,10 +442,14 @@ def run_ours(args):
             torch.cuda.synchronize()
             if it > 0:
                 ms64.append(e0.elapsed_time(e1))
+        st64 = c64.stage_times()
         err = np.abs(e64.cpu().numpy().astype(np.complex128) - e_dev) / np.abs(e_dev)
         line["complex64_path"] = {"ms_per_step": sum(ms64) / len(ms64), "walker_steps_per_s": nw / (sum(ms64) / len(ms64) * 1e-3),
                                   "max_rel_diff_vs_complex128": [float(err[:, i].max()) for i in range(3)],
-                                  "note": "afqmc_dims.precision = 1: complex64 arrays at the boundary, FP64 small algebra, 3xTF32 "
+                                  "stage_ms": st64,
+                                  "stage_ms_complex128": {k: stages[k] for k in ("force_bias", "vhs", "exchange")},
+                                  "note": "afqmc_dims.precision = 1: complex64 arrays at the boundary, the vHS and force-bias operands "
+                                          "STORED in single precision (half the HBM bytes, FP64 accumulation), FP64 small algebra, 3xTF32 "
                                           "exchange; extra information (the energies are those of the polynomial-propagated walkers, "
                                           "whose FP32 storage error is amplified by the synthetic step size, DESIGN.md R9)"}
         c64.close()

@@ -55,6 +55,8 @@ struct afqmc_ctx {
     double* Lx;     // exchange, 4M kernel (energy.cu): [Q][k][ag][gq][s][lane][2]; packed on first use (option exchange_3m = 0)
     float* LxT;     // exchange, TF32 fragments [Q][k][gq][ks][lane][4] (exchange_tf32.cu; n <= 4 only); packed on first use
     double* Lf;     // force-bias fragment layout [Q][gtp][k][a][s][lane][2]
+    float* Lff;     // precision = 1: the force-bias operand in single precision (Lf is then NULL)
+    float2* Lv3f;   // precision = 1: the vHS operand in single precision (Lv3 is then NULL): half the bytes of the HBM-bound streams
     double2* Lv3;   // vHS operand [unit][prt][ks][lane] complex fragments (vhs.cu); one block per (Q,-Q) pair if vhs_paired
     int* vunits;    // vHS work units, int4-packed (Q, k, kind, 0) [nvunits]; kind 1 = block + its (-Q,k-Q) partner
     int nvunits;

@@ -83,7 +83,8 @@ __global__ void pack_Lx_kernel(Dims d, const double2* __restrict__ Lh, double* _
     }
 }
 
-__global__ void pack_Lf_kernel(Dims d, const double2* __restrict__ Lh, double* __restrict__ Lf, size_t total) {
+template <typename T>
+__global__ void pack_Lf_kernel(Dims d, const double2* __restrict__ Lh, T* __restrict__ Lf, size_t total) {
     for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total;
          idx += (size_t)gridDim.x * blockDim.x) {
         size_t t = idx;
@@ -102,7 +103,7 @@ __global__ void pack_Lf_kernel(Dims d, const double2* __restrict__ Lh, double* _
             double2 z = lh_elem(Lh, d, Q, k, a, gam, r);
             v = c ? z.y : z.x;
         }
-        Lf[idx] = v;
+        Lf[idx] = (T)v;
     }
 }
 
@@ -147,7 +148,7 @@ AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     if (!c) return;
     if (c->dn) { afqmc_destroy(c->dn); c->dn = nullptr; }
     if (c->is_child) c->b1 = nullptr;        // owned by the spin-up context
-    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lh, c->Lxc, c->Lx3t, c->Lx, c->LxT, c->Lf, c->Lv3, c->vunits,
+    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lh, c->Lxc, c->Lx3t, c->Lx, c->LxT, c->Lf, c->Lff, c->Lv3, c->Lv3f, c->vunits,
                     c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T, c->ws_Tx,
                     c->ws_expart, c->ws_fbpart, c->ws_vbtot, c->ws_ld_chan, c->ws_info_chan, c->ws_ldr_chan, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
                     c->ws_f32, c->b1, c->ws_b1tmp, c->ws_gram, c->ws_rinv, c->ws_logdet2, c->ws_ldr, c->ws_info2};
@@ -234,7 +235,8 @@ static int create_channel(afqmc_ctx** out, const afqmc_dims* dims, int n_chan, i
     A(dev_alloc(&c->psi_t, (size_t)Nk * d.m * d.n));
     A(dev_alloc(&c->ht, (size_t)Nk * d.n * d.m));
     A(dev_alloc(&c->Lh, nLh));
-    A(dev_alloc(&c->Lf, nLf));
+    if (c->prec32) A(dev_alloc(&c->Lff, nLf));      // single-precision storage of the force-bias operand
+    else A(dev_alloc(&c->Lf, nLf));
     A(dev_alloc(&c->ws_O, (size_t)nw * d.N * LD));
     A(dev_alloc(&c->ws_oinvT, (size_t)nw * d.N * d.N));
     A(dev_alloc(&c->ws_theta, (size_t)nw * (child ? d.N : Nk * n_total) * d.M));     // spin-up context: both channels, spin-major
@@ -300,7 +302,8 @@ static int create_channel(afqmc_ctx** out, const afqmc_dims* dims, int n_chan, i
         auto grid = [&](size_t total) { return (int)((total + T - 1) / T > 148 * 64 ? 148 * 64 : (total + T - 1) / T); };
         half_rot_h_kernel<<<grid((size_t)Nk * d.n * d.m), T, 0, st>>>(d, (const double2*)h1, c->psi_t, c->ht);
         half_rot_L_kernel<<<grid(nLh), T, 0, st>>>(d, (const double2*)L, c->psi_t, c->Lh, nLh);     // the half rotation, once
-        pack_Lf_kernel<<<grid(nLf), T, 0, st>>>(d, c->Lh, c->Lf, nLf);
+        if (c->prec32) pack_Lf_kernel<float><<<grid(nLf), T, 0, st>>>(d, c->Lh, c->Lff, nLf);
+        else pack_Lf_kernel<double><<<grid(nLf), T, 0, st>>>(d, c->Lh, c->Lf, nLf);
         c->launches += 3;
         if (cudaGetLastError() != cudaSuccess) rc = AFQMC_CUDA_ERROR;
         if (rc == AFQMC_OK) rc = afqmc_i_pack_exchange_operand(c, st);

@@ -23,9 +23,10 @@ namespace {
 constexpr int FB_WARPS = 4;
 constexpr int FB_D = 3;   // k-steps of register prefetch (3 CTAs of 4 warps stay resident at 168 registers)
 
-template <int MP, int NT>
+// AT = double2: FP64 storage of the operand; float2: single-precision storage (precision = 1), widened at use
+template <int MP, int NT, typename AT>
 __global__ void __launch_bounds__(32 * FB_WARPS, (MP * NT > 8 ? 2 : 3)) force_bias_kernel(
-    Dims d, int nw, int KC, int nmg, int nwgrp, int pf, const int* __restrict__ kminus, const double* __restrict__ Lf,
+    Dims d, int nw, int KC, int nmg, int nwgrp, int pf, const int* __restrict__ kminus, const AT* __restrict__ Lf,
     const double2* __restrict__ theta, double2* __restrict__ out, int out_is_partial, double spin_factor) {
     extern __shared__ __align__(16) double fb_smem[];
     // blockIdx.x = ((Q*KC + kc)*nwgrp + wgrp)*nmg + mg
@@ -55,13 +56,13 @@ __global__ void __launch_bounds__(32 * FB_WARPS, (MP * NT > 8 ? 2 : 3)) force_bi
     const int g_begin = c0 + (int)((long long)warp * (c1 - c0) / FB_WARPS);
     const int g_end = c0 + (int)((long long)(warp + 1) * (c1 - c0) / FB_WARPS);
 
-    const double2* ap[MP];
+    const AT* ap[MP];
     bool aok[MP];
 #pragma unroll
     for (int i = 0; i < MP; ++i) {
         const int gtp = mg * MP + i;
         aok[i] = gtp < d.GT2;
-        ap[i] = reinterpret_cast<const double2*>(Lf + (((size_t)Q * d.GT2 + (aok[i] ? gtp : d.GT2 - 1)) * S + g_begin) * 64) + lane;
+        ap[i] = Lf + (((size_t)Q * d.GT2 + (aok[i] ? gtp : d.GT2 - 1)) * S + g_begin) * 32 + lane;
     }
     const double* bw[NT];
     bool bok[NT];
@@ -82,7 +83,7 @@ __global__ void __launch_bounds__(32 * FB_WARPS, (MP * NT > 8 ? 2 : 3)) force_bi
     // loader state (runs FB_D k-steps ahead; stops advancing at g_end, so nothing is read out of range)
     int lg = g_begin, item = g_begin / KS, ls = g_begin - item * KS;
     int boff = offtab[item] + 4 * ls;
-    double2 fa[FB_D][MP];
+    AT fa[FB_D][MP];
     double fb[FB_D][NT];
     auto refill = [&](const int q) {
         const bool rok = 2 * ls + roff < d.m;
@@ -110,12 +111,14 @@ __global__ void __launch_bounds__(32 * FB_WARPS, (MP * NT > 8 ? 2 : 3)) force_bi
 #pragma unroll
         for (int j = 0; j < NT; ++j) b[j] = flip_sign(fb[q][j], smask);      // real embedding: -Im for (c=1, d=0)
 #pragma unroll
-        for (int i = 0; i < MP; ++i)
+        for (int i = 0; i < MP; ++i) {
+            const double ax = (double)fa[q][i].x, ay = (double)fa[q][i].y;
 #pragma unroll
             for (int j = 0; j < NT; ++j) {
-                dmma884(acc[2 * i][j][0], acc[2 * i][j][1], fa[q][i].x, b[j]);
-                dmma884(acc[2 * i + 1][j][0], acc[2 * i + 1][j][1], fa[q][i].y, b[j]);
+                dmma884(acc[2 * i][j][0], acc[2 * i][j][1], ax, b[j]);
+                dmma884(acc[2 * i + 1][j][0], acc[2 * i + 1][j][1], ay, b[j]);
             }
+        }
         refill(q);
     };
     const int total = g_end - g_begin;
@@ -183,8 +186,8 @@ __global__ void force_bias_reduce_kernel(size_t n, int KC, double spin_factor, c
     }
 }
 
-template <int MP, int NT>
-int launch_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias, cudaStream_t st) {
+template <int MP, int NT, typename AT>
+int launch_force_bias_t(afqmc_ctx* c, const AT* Lf, const double2* theta, int nw, double2* vbias, cudaStream_t st) {
     const Dims& d = c->d;
     const int ntq = (nw + 3) / 4;
     const int nmg = (d.GT2 + MP - 1) / MP, nwgrp = (ntq + NT - 1) / NT;
@@ -200,9 +203,9 @@ int launch_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias
         if (eff > best) { best = eff; KC = kc; }
     }
     const size_t smem = (size_t)(((d.Nk * d.n + 2) / 2 + 1) / 2 * 2 + (FB_WARPS / 2) * 2 * MP * NT * 64) * sizeof(double);
-    auto kern = force_bias_kernel<MP, NT>;
+    auto kern = force_bias_kernel<MP, NT, AT>;
     if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
-    kern<<<(unsigned)(base * KC), 32 * FB_WARPS, smem, st>>>(d, nw, KC, nmg, nwgrp, c->opt_fb_pf, c->kminus, c->Lf, theta,
+    kern<<<(unsigned)(base * KC), 32 * FB_WARPS, smem, st>>>(d, nw, KC, nmg, nwgrp, c->opt_fb_pf, c->kminus, Lf, theta,
                                                              KC > 1 ? c->ws_fbpart : vbias, KC > 1 ? 1 : 0, c->spin_factor);
     AFQMC_LAUNCH_CHECK(c);
     if (KC > 1) {
@@ -213,6 +216,12 @@ int launch_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias
         AFQMC_LAUNCH_CHECK(c);
     }
     return AFQMC_OK;
+}
+
+template <int MP, int NT>
+int launch_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias, cudaStream_t st) {
+    if (c->Lff) return launch_force_bias_t<MP, NT, float2>(c, reinterpret_cast<const float2*>(c->Lff), theta, nw, vbias, st);
+    return launch_force_bias_t<MP, NT, double2>(c, reinterpret_cast<const double2*>(c->Lf), theta, nw, vbias, st);
 }
 
 }  // namespace

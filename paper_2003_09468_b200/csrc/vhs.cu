@@ -22,6 +22,9 @@
 //    addresses at about the same time: L1 hits, so HBM sees every byte of L once).  The B fragments of the unit
 //    (both column sets) stream through a 3-stage shared-memory ring filled by bulk asynchronous copies
 //    (cp.async.bulk + mbarrier, SASS UBLKCP) and are shared by the 4 warps.
+//  * Single-precision STORAGE of L (precision = 1, the paper's production mode): the same
+//    fragments as float2 (Lv3f): half the bytes of the stream that bounds this kernel at small batches (C4, C5); the fragment
+//    is widened in registers (one F2F per component) and everything downstream is the FP64 path (FP64 accumulation).
 // Every (k,k') block of vhs is written exactly once, so no zero fill is needed.
 #include <cstring>
 #include <vector>
@@ -59,8 +62,14 @@ __global__ void pair_symmetry_kernel(Dims d, const int* __restrict__ kminus, con
     atomicMax(out + 1, (unsigned long long)__double_as_longlong(mx));
 }
 
+__device__ __forceinline__ void store_frag(double2* p, double2 z) { *p = z; }
+__device__ __forceinline__ void store_frag(float2* p, double2 z) { *p = make_float2((float)z.x, (float)z.y); }
+__device__ __forceinline__ double2 load_frag(const double2* p) { return __ldg(p); }
+__device__ __forceinline__ double2 load_frag(const float2* p) { const float2 v = __ldg(p); return make_double2((double)v.x, (double)v.y); }
+
+template <typename AT>
 __global__ void pack_Lv3_kernel(Dims d, int KS4, int nvu, const int* __restrict__ vunits, const double2* __restrict__ L,
-                                double2* __restrict__ Lv3) {
+                                AT* __restrict__ Lv3) {
     const size_t total = (size_t)nvu * d.PRT * KS4 * 32;
     for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
         size_t t = idx;
@@ -72,7 +81,7 @@ __global__ void pack_Lv3_kernel(Dims d, int KS4, int nvu, const int* __restrict_
         const int pr = 8 * prt + (lane >> 2), gam = 4 * ks + (lane & 3);
         double2 z = make_double2(0.0, 0.0);
         if (pr < d.m * d.m && gam < d.nchol) z = L[(((size_t)Q * d.Nk + k) * d.nchol + gam) * d.m * d.m + pr];
-        Lv3[idx] = z;
+        store_frag(Lv3 + idx, z);
     }
 }
 
@@ -115,12 +124,14 @@ int afqmc_i_vhs_setup(afqmc_ctx* c, const double2* L, const std::vector<int>& km
     c->nvunits = (int)(vu.size() / 4);
     const int KS4 = (d.nchol + 3) / 4;
     AFQMC_CUDA_TRY(cudaMalloc((void**)&c->vunits, vu.size() * sizeof(int)));
-    AFQMC_CUDA_TRY(cudaMalloc((void**)&c->Lv3, (size_t)c->nvunits * d.PRT * KS4 * 32 * sizeof(double2)));
-    AFQMC_CUDA_TRY(cudaMemcpyAsync(c->vunits, vu.data(), vu.size() * sizeof(int), cudaMemcpyHostToDevice, st));
     const size_t total = (size_t)c->nvunits * d.PRT * KS4 * 32;
+    if (c->prec32) AFQMC_CUDA_TRY(cudaMalloc((void**)&c->Lv3f, total * sizeof(float2)));      // single-precision storage
+    else AFQMC_CUDA_TRY(cudaMalloc((void**)&c->Lv3, total * sizeof(double2)));
+    AFQMC_CUDA_TRY(cudaMemcpyAsync(c->vunits, vu.data(), vu.size() * sizeof(int), cudaMemcpyHostToDevice, st));
     size_t g = (total + 255) / 256;
     if (g > 148 * 64) g = 148 * 64;
-    pack_Lv3_kernel<<<(unsigned)g, 256, 0, st>>>(d, KS4, c->nvunits, c->vunits, L, c->Lv3);
+    if (c->prec32) pack_Lv3_kernel<float2><<<(unsigned)g, 256, 0, st>>>(d, KS4, c->nvunits, c->vunits, L, c->Lv3f);
+    else pack_Lv3_kernel<double2><<<(unsigned)g, 256, 0, st>>>(d, KS4, c->nvunits, c->vunits, L, c->Lv3);
     AFQMC_LAUNCH_CHECK(c);
     AFQMC_CUDA_TRY(cudaStreamSynchronize(st));      // `vu` must outlive the copy
     return AFQMC_OK;
@@ -182,10 +193,10 @@ __global__ void fields3_kernel(Dims d, int nw, int NT, int nwg, int KS4p, const 
 // sets of its row slice (2 NT n-tiles), so the A stream is read once without relying on L1 and every fragment feeds
 // twice as many DMMAs; otherwise warps 0-1 take the block and warps 2-3 its partner.  D = k-steps of A register prefetch
 // (deeper for small batches, where the kernel is bound by the HBM stream of L and needs more bytes in flight).
-template <int NT, bool MERGED, int D>
+template <int NT, bool MERGED, int D, typename AT>
 __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
     Dims d, int KS4, int KS4p, int nw, int nwg, int nsg, const int* __restrict__ vunits, const int* __restrict__ kminus,
-    const double2* __restrict__ Lv3, const double* __restrict__ Bx3, double2* __restrict__ vhs) {
+    const AT* __restrict__ Lv3, const double* __restrict__ Bx3, double2* __restrict__ vhs) {
     extern __shared__ __align__(128) double v3_smem[];
     constexpr int KC = D;                                     // k-steps per stage
     constexpr int SET_DOUBLES = KC * 3 * NT * 32;             // one column set of one stage
@@ -229,9 +240,9 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
 
     // A stream: two m-tiles, contiguous k-steps; rows beyond the block are clamped (their results are not stored)
     const int prt0 = 2 * slice, prt1 = min(prt0 + 1, d.PRT - 1);
-    const double2* pa0 = Lv3 + (((size_t)u * d.PRT + prt0) * KS4) * 32 + lane;
-    const double2* pa1 = Lv3 + (((size_t)u * d.PRT + prt1) * KS4) * 32 + lane;
-    double2 fa0[D], fa1[D];
+    const AT* pa0 = Lv3 + (((size_t)u * d.PRT + prt0) * KS4) * 32 + lane;
+    const AT* pa1 = Lv3 + (((size_t)u * d.PRT + prt1) * KS4) * 32 + lane;
+    AT fa0[D], fa1[D];            // kept in the storage type (half the registers for float2); widened at use
 #pragma unroll
     for (int q = 0; q < D; ++q) {
         const int ks = min(q, KS4 - 1);
@@ -248,8 +259,9 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
 
     int ksg = 0;        // global k-step
     auto kstep = [&](const double* bs, const int qa) {
-        const double a0[3] = {fa0[qa].x + fa0[qa].y, fa0[qa].x, fa0[qa].y};
-        const double a1[3] = {fa1[qa].x + fa1[qa].y, fa1[qa].x, fa1[qa].y};
+        const double x0 = (double)fa0[qa].x, y0 = (double)fa0[qa].y, x1 = (double)fa1[qa].x, y1 = (double)fa1[qa].y;
+        const double a0[3] = {x0 + y0, x0, y0};
+        const double a1[3] = {x1 + y1, x1, y1};
 #pragma unroll
         for (int p = 0; p < 3; ++p) {
             double bf[NTT];
@@ -312,8 +324,8 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
     }
 }
 
-template <int NT, bool MERGED, int D>
-int launch_vhs3(afqmc_ctx* c, int nw, int KS4, int KS4p, double2* vhs, cudaStream_t st) {
+template <int NT, bool MERGED, int D, typename AT>
+int launch_vhs3_t(afqmc_ctx* c, const AT* Lv3, int nw, int KS4, int KS4p, double2* vhs, cudaStream_t st) {
     const Dims& d = c->d;
     const int nwg = (nw + 8 * NT - 1) / (8 * NT);
     const int nslices = (d.PRT + 1) / 2;
@@ -321,11 +333,17 @@ int launch_vhs3(afqmc_ctx* c, int nw, int KS4, int KS4p, double2* vhs, cudaStrea
     const size_t smem = (size_t)V3_STAGES * 2 * D * 3 * NT * 32 * sizeof(double) + 2 * V3_STAGES * sizeof(uint64_t);
     const long long gx = (long long)c->nvunits * nsg;
     if (gx > 0x7fffffffLL || nwg > 65535) return AFQMC_UNSUPPORTED;
-    if (int rc = afqmc_smem_optin(c, (const void*)vhs3_kernel<NT, MERGED, D>, smem)) return rc;
-    vhs3_kernel<NT, MERGED, D><<<dim3((unsigned)gx, nwg), 32 * V3_WARPS, smem, st>>>(d, KS4, KS4p, nw, nwg, nsg, c->vunits, c->kminus, c->Lv3,
-                                                                        reinterpret_cast<const double*>(c->ws_xi), vhs);
+    if (int rc = afqmc_smem_optin(c, (const void*)vhs3_kernel<NT, MERGED, D, AT>, smem)) return rc;
+    vhs3_kernel<NT, MERGED, D, AT><<<dim3((unsigned)gx, nwg), 32 * V3_WARPS, smem, st>>>(d, KS4, KS4p, nw, nwg, nsg, c->vunits, c->kminus, Lv3,
+                                                                            reinterpret_cast<const double*>(c->ws_xi), vhs);
     AFQMC_LAUNCH_CHECK(c);
     return AFQMC_OK;
+}
+
+template <int NT, bool MERGED, int D>
+int launch_vhs3(afqmc_ctx* c, int nw, int KS4, int KS4p, double2* vhs, cudaStream_t st) {
+    if (c->Lv3f) return launch_vhs3_t<NT, MERGED, D, float2>(c, c->Lv3f, nw, KS4, KS4p, vhs, st);      // single-precision storage
+    return launch_vhs3_t<NT, MERGED, D, double2>(c, c->Lv3, nw, KS4, KS4p, vhs, st);
 }
 
 }  // namespace

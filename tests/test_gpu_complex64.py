@@ -92,6 +92,13 @@ def test_complex64_boundary_c5_optional_run():
     _chain(cfg, [0, 5])
 
 
+@pytest.mark.slow
+def test_complex64_boundary_c4_single_precision_storage():
+    """Config 4 (L = 12.6 GB in complex128): with precision = 1 the vHS and force-bias operands are STORED in single
+    precision (half the bytes of the HBM-bound streams) and accumulated in FP64: 1e-4 against the oracle."""
+    _chain(synth.CONFIGS["C4"], [0, 15])
+
+
 def test_complex64_rejects_complex128_tensors():
     from paper_2003_09468_b200 import binding
     cfg = synth.CONFIGS["C1"]
