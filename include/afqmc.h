@@ -26,9 +26,12 @@
  * Precision 1 (optional complex64 path; the paper's production runs are single precision): with
  * afqmc_dims.precision = 1 EVERY complex array of afqmc_create, of the six step calls, of afqmc_step and of
  * afqmc_step_host is complex64 (float re, im) and every real array (x) is float32; shapes and layouts are unchanged.
- * Inside, the small algebra runs in FP64 on widened copies and the exchange contraction on the TF32 tensor cores with a
- * high/low operand split (option "exchange_precision" = 1).  Results agree with the FP64 path to FP32 input/output
- * accuracy (tolerance 1e-4).  The AFQMC-block calls return AFQMC_UNSUPPORTED in this mode.
+ * Inside, the library STORES the two streamed operands that bound the step at small batches in single precision -- the
+ * vHS operand (the largest tensor: L, one block per (Q,-Q) pair) and the force-bias operand (the half-rotated Lh) -- i.e. half
+ * their bytes in HBM and on the bus; fragments are widened in registers and every sum is accumulated in FP64.  The small
+ * algebra runs in FP64 on widened copies and the exchange contraction on the TF32 tensor cores with a high/low operand split
+ * (option "exchange_precision" = 1).  Results agree with the FP64 path to FP32 input/output accuracy (tolerance 1e-4).  The
+ * AFQMC-block calls and open-shell contexts return AFQMC_UNSUPPORTED in this mode.
  *
  * Errors: every call returns an int; 0 = AFQMC_OK.  No exceptions cross the ABI, there is no
  * global state.  A singular overlap cannot be a return code of an asynchronous call: it is
