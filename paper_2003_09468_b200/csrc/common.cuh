@@ -29,7 +29,7 @@ struct Dims {
 
 // Kernel attributes that were set / queried for this context.  A function attribute belongs to the (function, device)
 // pair and a context lives on one device, so the record is per CONTEXT: nothing in the library is process-wide state.
-struct FuncAttr { const void* fn; int smem; int occ; };
+struct FuncAttr { const void* fn; int smem; int occ; int carveout; };
 #define AFQMC_MAX_FATTR 128
 
 // The context.  All pointers are device memory owned by the context.
@@ -222,8 +222,17 @@ static inline FuncAttr* afqmc_fattr(afqmc_ctx* c, const void* fn) {
         if (c->fattr[i].fn == fn) return &c->fattr[i];
     if (c->nfattr == AFQMC_MAX_FATTR) return nullptr;
     FuncAttr* f = &c->fattr[c->nfattr++];
-    f->fn = fn; f->smem = 0; f->occ = -1;
+    f->fn = fn; f->smem = 0; f->occ = -1; f->carveout = 0;
     return f;
+}
+// Asks the driver for the largest shared-memory carveout for `fn` (once per context): kernels whose residency is set by
+// shared memory (many small CTAs) otherwise get a carveout sized for fewer CTAs than the registers allow.
+static inline void afqmc_prefer_smem(afqmc_ctx* c, const void* fn) {
+    FuncAttr* f = afqmc_fattr(c, fn);
+    if (f && f->carveout) return;
+    if (cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared) != cudaSuccess)
+        (void)cudaGetLastError();
+    if (f) { f->carveout = 1; f->occ = -1; }
 }
 static inline int afqmc_smem_optin(afqmc_ctx* c, const void* fn, size_t smem) {
     if (smem <= 48 * 1024) return AFQMC_OK;

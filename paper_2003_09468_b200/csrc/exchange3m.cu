@@ -37,6 +37,7 @@
 #include <type_traits>
 #include "common.cuh"
 
+
 namespace {
 
 struct X3Geom { int KSF, TAIL, KSPT, MSPT; };
@@ -295,7 +296,9 @@ __device__ __forceinline__ void x3_finish_task(double (&acc)[3][2][NP][2], doubl
 #pragma unroll
         for (int e = 0; e < 2; ++e)
             xw[j * 64 + L.sw[e]] = make_double2(acc[0][GIVE][j][e] - acc[2][GIVE][j][e], acc[0][GIVE][j][e] + acc[1][GIVE][j][e]);
-    asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");       // the two warps of the pair
+    // the two warps of the pair (an immediate id where possible: a register id makes ptxas reserve all 16 named barriers)
+    if (bar_id == 1) asm volatile("bar.sync 1, 64;" ::: "memory");
+    else asm volatile("bar.sync 2, 64;" ::: "memory");        // (at most two warp pairs per CTA)
 #pragma unroll
     for (int j = 0; j < NP; ++j)
 #pragma unroll
@@ -744,6 +747,7 @@ int launch_x3(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     const size_t smem = x3_smem_bytes<NP>(g, GRIDPAIRS ? 1 : d.NAG, NPAIR);
     auto kern = exchange3m_kernel<NP, NPAIR, DA, MINB, GRIDPAIRS>;
     if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
+    afqmc_prefer_smem(c, (const void*)kern);
     const int nwg = (nw + 2 * NP - 1) / (2 * NP), npairs = d.NAG * d.NAG;
     int nchunk = 1;
     long long nblocks = (long long)c->nunits * nwg;
@@ -798,6 +802,7 @@ int launch_x3_reg(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     const size_t smem = x3_reg_smem_bytes<NP>(d);
     auto kern = exchange3m_reg_kernel<KSF, TAIL, NP, MAXREG>;
     if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
+    afqmc_prefer_smem(c, (const void*)kern);
     const long long nitems = (long long)c->nunits * ((nw + 2 * NP - 1) / (2 * NP));
     if (nitems > 0x7fffffffLL) return AFQMC_UNSUPPORTED;
     // persistent grid: as many CTAs as are resident (remembered per context)
