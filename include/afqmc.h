@@ -256,6 +256,10 @@ long long afqmc_launch_count(const afqmc_ctx* ctx);
  * walkers, as the kernel executes it (pairs (Q,k,k') ~ (-Q,k'-Q,k-Q) computed once). */
 double afqmc_exchange_flops(const afqmc_ctx* ctx, int nw);
 
+/* Executed real flops of ONE afqmc_force_bias call (a4; Eq. 47) on nw walkers: the kernel uses the 3M complex
+ * product, 6 real flops per complex multiply-add (the plain definition costs 8): 6 Nk^2 n m nchol nw (both channels when open). */
+double afqmc_force_bias_flops(const afqmc_ctx* ctx, int nw);
+
 /* Options: "exchange_warps" (0 = automatic, or 4/5/6/8 warps per CTA of the exchange kernel; tuning aid);
  * "exchange_depth" (0/3 or 2: k-steps of register prefetch in the exchange kernel; tuning aid);
  * "exchange_precision" (0 = default: FP64.  MIXED PRECISION exchange energy on the TF32 tensor cores, the analogue of the

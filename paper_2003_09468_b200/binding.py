@@ -32,7 +32,7 @@ class Dims(ctypes.Structure):
 
 EXPORTS = ["afqmc_strerror", "afqmc_create", "afqmc_destroy", "afqmc_overlap", "afqmc_green", "afqmc_force_bias",
            "afqmc_vhs", "afqmc_propagate", "afqmc_local_energy", "afqmc_step", "afqmc_step_host",
-           "afqmc_launch_count", "afqmc_exchange_flops", "afqmc_set_option", "afqmc_stage_times", "afqmc_probe_fp64",
+           "afqmc_launch_count", "afqmc_exchange_flops", "afqmc_force_bias_flops", "afqmc_set_option", "afqmc_stage_times", "afqmc_probe_fp64",
            "afqmc_set_onebody", "afqmc_apply_onebody", "afqmc_hybrid_weight", "afqmc_orthogonalize",
            "afqmc_mixed_estimator", "afqmc_block"]
 
@@ -64,6 +64,8 @@ def lib():
     L.afqmc_launch_count.restype = ctypes.c_longlong
     L.afqmc_exchange_flops.argtypes = [vp, ci]
     L.afqmc_exchange_flops.restype = cd
+    L.afqmc_force_bias_flops.argtypes = [vp, ci]
+    L.afqmc_force_bias_flops.restype = cd
     L.afqmc_set_option.argtypes = [vp, ctypes.c_char_p, ci]
     L.afqmc_probe_fp64.argtypes = [ci, ci, ctypes.POINTER(cd)]
     L.afqmc_stage_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
@@ -74,7 +76,7 @@ def lib():
     L.afqmc_mixed_estimator.argtypes = [vp, vp, vp, ci, vp, vp]
     L.afqmc_block.argtypes = [vp, vp, vp, vp, cd, ci, ci, ci, vp, vp, vp, vp, vp]
     for name in EXPORTS:
-        if name not in ("afqmc_strerror", "afqmc_destroy", "afqmc_launch_count", "afqmc_exchange_flops"):
+        if name not in ("afqmc_strerror", "afqmc_destroy", "afqmc_launch_count", "afqmc_exchange_flops", "afqmc_force_bias_flops"):
             getattr(L, name).restype = ci
     _lib = L
     return L
@@ -228,6 +230,9 @@ class Afqmc:
 
     def exchange_flops(self, nw) -> float:
         return float(lib().afqmc_exchange_flops(self._h, int(nw)))
+
+    def force_bias_flops(self, nw) -> float:
+        return float(lib().afqmc_force_bias_flops(self._h, int(nw)))
 
     def set_option(self, name: str, value: int):
         _check(lib().afqmc_set_option(self._h, name.encode(), int(value)), "afqmc_set_option")

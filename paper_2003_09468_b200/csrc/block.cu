@@ -139,7 +139,7 @@ int afqmc_i_apply_onebody(afqmc_ctx* c, double2* phi, int nw, cudaStream_t st) {
         // GEMM per k-point, out of place into the Taylor workspace, then copied back
         const size_t per = (size_t)d.M * d.N;
         for (int k = 0; k < d.Nk; ++k) {
-            zg::Args a;
+            zg::Args a = {};
             a.A = c->b1 + (size_t)k * d.m * d.m; a.strideA = 0; a.lda = d.m;
             a.B = phi + (size_t)k * d.m * d.N; a.strideB = (long long)per; a.ldb = d.N;
             a.C = c->ws_T + (size_t)k * d.m * d.N; a.strideC = (long long)per; a.ldc = d.N;
@@ -452,7 +452,7 @@ static int orthogonalize_i(afqmc_ctx* c, double2* phi, int nw, double* logdet_r,
         cholesky_inverse_kernel<<<nw, CH_THREADS, use_smem ? mat : 0, st>>>(d.N, use_smem, c->ws_gram, c->ws_rinv,
                                                                             c->ws_ldr + (size_t)pass * nw, c->ws_info2 + (size_t)pass * nw);
         AFQMC_LAUNCH_CHECK(c);
-        zg::Args a;
+        zg::Args a = {};
         a.A = phi; a.strideA = (long long)per; a.lda = d.N;
         a.B = c->ws_rinv; a.strideB = (long long)d.N * d.N; a.ldb = d.N;
         a.C = c->ws_T; a.strideC = (long long)per; a.ldc = d.N;
@@ -532,6 +532,7 @@ AFQMC_API int afqmc_block(afqmc_ctx* c, void* phi, double* weight, const double*
         AFQMC_LAUNCH_CHECK(c);
         return AFQMC_OK;
     };
+    AfqmcFuseGuard fuse(c);      // Green's epilogue also writes the force-bias B fragments (zgemm.cuh FragOut)
     if ((rc = afqmc_x_green(c, ph, nw, c->ws_theta, ld[0], c->ws_info, st)) != AFQMC_OK) return rc;
     if ((rc = merge(1)) != AFQMC_OK) return rc;
     for (int s = 0; s < nsteps; ++s) {

@@ -7,7 +7,7 @@
 #include "../../include/afqmc.h"
 
 #define AFQMC_MAX_NK 512
-#define AFQMC_FB_MAXKC 16   // max K chunks of the force-bias kernel (sizes its partial-sum workspace)
+#define AFQMC_FB_MAXKC 16   // max pieces a force-bias tile is cut into (sizes the partial-tile workspace)
 #define AFQMC_LX_PAD 1024   // doubles of zero padding after Lx (the exchange kernel prefetches up to 4 k-steps ahead)
 // exported C-ABI entry points (everything else in the library has hidden visibility)
 #define AFQMC_API extern "C" __attribute__((visibility("default")))
@@ -23,13 +23,12 @@ struct Dims {
     int NAG;       // groups of 4 occupied orbitals: ceil(n/4)
     int GP;        // pairs of Cholesky vectors: ceil(nchol/2)   (vHS k-steps)
     int GQ;        // quads of Cholesky vectors: ceil(nchol/4)   (exchange tasks: two M-tiles each)
-    int GT2;       // 16-groups of Cholesky vectors: ceil(nchol/16) (force-bias M-tile pairs)
     int PRT;       // octets of (p,r) pairs: ceil(m*m/8)         (vHS M-tiles)
 };
 
 // Kernel attributes that were set / queried for this context.  A function attribute belongs to the (function, device)
 // pair and a context lives on one device, so the record is per CONTEXT: nothing in the library is process-wide state.
-struct FuncAttr { const void* fn; int smem; int occ; int carveout; };
+struct FuncAttr { const void* fn; int smem; int occ; int carveout; int occ_smem; };
 #define AFQMC_MAX_FATTR 128
 
 // The context.  All pointers are device memory owned by the context.
@@ -54,8 +53,8 @@ struct afqmc_ctx {
                     // (only the default one of Lxc / Lx3t is packed in a0; the other on first use)
     double* Lx;     // exchange, 4M kernel (energy.cu): [Q][k][ag][gq][s][lane][2]; packed on first use (option exchange_3m = 0)
     float* LxT;     // exchange, TF32 fragments [Q][k][gq][ks][lane][4] (exchange_tf32.cu; n <= 4 only); packed on first use
-    double* Lf;     // force-bias fragment layout [Q][gtp][k][a][s][lane][2]
-    float* Lff;     // precision = 1: the force-bias operand in single precision (Lf is then NULL)
+    double* Lf;     // force-bias operand Lf3[Q][m-tile][k-step][lane] complex fragments over the flattened K = (k,a,r) (force_bias.cu)
+    float* Lff;     // precision = 1: the same in single precision (Lf is then NULL)
     float2* Lv3f;   // precision = 1: the vHS operand in single precision (Lv3 is then NULL): half the bytes of the HBM-bound streams
     double2* Lv3;   // vHS operand [unit][prt][ks][lane] complex fragments (vhs.cu); one block per (Q,-Q) pair if vhs_paired
     int* vunits;    // vHS work units, int4-packed (Q, k, kind, 0) [nvunits]; kind 1 = block + its (-Q,k-Q) partner
@@ -71,7 +70,8 @@ struct afqmc_ctx {
     double2* ws_T;      // [2][nw][M][N] Taylor ping-pong (legacy GEMM path)
     double* ws_Tx;      // [2][nw][expanded] Taylor ping-pong in the expanded B-fragment layout of tgemm.cuh
     double2* ws_expart; // [nunits][nw]  exchange partial sums
-    double2* ws_fbpart; // [AFQMC_FB_MAXKC][nw][Nk][nchol] force-bias K-chunk partial sums
+    double2* ws_thetaF; // [Nk(Q)][walker groups][k-steps][NT][32] theta as B fragments of the force-bias GEMM (force_bias.cu)
+    double2* ws_fbpart; // [AFQMC_FB_MAXKC][nw][Nk][nchol] force-bias partial tiles (stream-K pieces)
     double* ws_x;       // [nw][Nk][nchol] (host-entry staging)
     double2* ws_phi;    // [nw][M][N]     (host-entry staging)
     double2* ws_energy; // [nw][3]
@@ -98,10 +98,11 @@ struct afqmc_ctx {
     double* ws_ldr_chan; // [nw] this channel's log det R of the orthogonalisation
     int prec32;         // 1 = complex64 boundary (afqmc_dims.precision = 1, boundary32.cu)
     float* ws_f32;      // precision 1: device staging of afqmc_step_host ([nw][M][N][2] + x + energy + logdet floats)
+    int fuse_frag;      // 1 while a composition (afqmc_step, afqmc_block) runs: Green's epilogue also writes ws_thetaF ...
+    int frag_nw;        // ... for this many walkers (0: ws_thetaF holds no valid fragments) ...
+    const void* frag_src; // ... of the Green's function at this address
     long long launches;
     int opt_exchange_depth; // 0/3 = three k-steps of fragment prefetch, 2 = two
-    int opt_fb_tile;        // tuning aid: warp tile of the force-bias kernel for > 16 walkers (0: 4x4, 1: 4x8, 2: 2x8 m x n tiles)
-    int opt_fb_pf;          // L2 prefetch distance (k-steps) of the Lf stream in the force-bias kernel
     int opt_exchange_minb;  // tuning aid: 1 = ask for more resident CTAs per SM
     int opt_exchange_prec;  // 0 (default) = FP64 exchange kernels; mixed precision on the TF32 tensor cores (n <= 4): 1 = 3xTF32 split, 2 = 1xTF32
     int opt_exchange_3m;    // 1 (default) = 3M exchange kernel when n <= 4, 0 = the 4M kernel of energy.cu
@@ -112,6 +113,7 @@ struct afqmc_ctx {
     int opt_taylor_legacy;  // testing aid: 1 = shared-memory-tiled zgemm for the Taylor chain
     int opt_taylor_wpc;     // tuning aid: 0 = automatic, else 3/4/5 warps per CTA of the Taylor GEMM
     int opt_taylor_groups;  // tuning aid: 0 = automatic, else the number of column groups of the Taylor GEMM
+    int opt_taylor_subbatch; // 0 = all walkers per Taylor pass, else walkers per pass (their V stays in L2 across the orders)
     int opt_green_cs;       // tuning aid: 4 = cluster of four CTAs per walker for 64 < N <= 128 (default two)
     int opt_green_legacy;   // testing aid: 1 = shared/global-memory elimination kernel instead of the register-resident one
     cudaStream_t copy_stream;   // afqmc_step_host: downloads the propagated walkers during the energy evaluation
@@ -222,7 +224,7 @@ static inline FuncAttr* afqmc_fattr(afqmc_ctx* c, const void* fn) {
         if (c->fattr[i].fn == fn) return &c->fattr[i];
     if (c->nfattr == AFQMC_MAX_FATTR) return nullptr;
     FuncAttr* f = &c->fattr[c->nfattr++];
-    f->fn = fn; f->smem = 0; f->occ = -1; f->carveout = 0;
+    f->fn = fn; f->smem = 0; f->occ = -1; f->carveout = 0; f->occ_smem = -1;
     return f;
 }
 // Asks the driver for the largest shared-memory carveout for `fn` (once per context): kernels whose residency is set by
@@ -254,6 +256,18 @@ static inline int afqmc_smem_optin(afqmc_ctx* c, const void* fn, size_t smem) {
 int afqmc_i_green(afqmc_ctx* c, const double2* phi, int nw, double2* theta, double2* logdet,
                   int* info, cudaStream_t st);
 int afqmc_i_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias, cudaStream_t st);
+int afqmc_i_pack_force_bias_operand(afqmc_ctx* c, cudaStream_t st);
+void afqmc_i_fb_frag_layout(const afqmc_ctx* c, int nw, int* NT, int* nwg, int* KSf);   // layout of ws_thetaF for nw walkers
+// switches the Green -> force-bias fragment fusion on / off for a composition (both spin channels)
+static inline void afqmc_set_fuse(afqmc_ctx* c, int on) {
+    c->fuse_frag = on; c->frag_nw = 0; c->frag_src = nullptr;
+    if (c->dn) afqmc_set_fuse(c->dn, on);
+}
+struct AfqmcFuseGuard {      // on for the lifetime of a composition call, off on every return path
+    afqmc_ctx* c;
+    explicit AfqmcFuseGuard(afqmc_ctx* ctx) : c(ctx) { afqmc_set_fuse(c, 1); }
+    ~AfqmcFuseGuard() { afqmc_set_fuse(c, 0); }
+};                     // a0: Lh -> Lf3 (allocates Lf / Lff)
 int afqmc_i_vhs(afqmc_ctx* c, const double* x, const double2* vbias, double dtau, int nw,
                 double2* vhs, cudaStream_t st);
 int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, double2* phi, int nw,

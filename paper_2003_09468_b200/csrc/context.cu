@@ -29,9 +29,8 @@ AFQMC_API const char* afqmc_strerror(int code) {
 //                        per lane (one LDG.128 feeds both); rows (gl = row>>2, al = row&3):
 //                        gamma = 4gq+2i+gl, a = 4ag+al;  K = (r, part) of Lh[Q][k][a][gamma][r]
 //                        (+ AFQMC_LX_PAD zero doubles at the end: the kernel's prefetch may run past the last task)
-//  Lf (force bias, a4): [Q][gtp][k][a][s][lane][i] two M-tiles i = 0,1 per 16 gammas, interleaved per lane;
-//                        rows gamma = 16gtp+8i+row;  K = (r, part), per (k,a); one contiguous K stream per gtp
-//  (the vHS operand Lv3 and the 3M exchange operand Lx3 are described and packed in vhs.cu / exchange3m.cu)
+//  (the force-bias operand Lf3, the vHS operand Lv3 and the 3M exchange operands are described and packed in force_bias.cu,
+//   vhs.cu and exchange3m.cu)
 // Out-of-range rows / K entries are stored as zeros, so kernels never branch on tails.
 // ---------------------------------------------------------------------------------------
 // Lh[Q][k][a][gam][r] = sum_p conj(A_k[p][a]) L[Q][k][gam][p][r], computed once; natural layout
@@ -83,30 +82,6 @@ __global__ void pack_Lx_kernel(Dims d, const double2* __restrict__ Lh, double* _
     }
 }
 
-template <typename T>
-__global__ void pack_Lf_kernel(Dims d, const double2* __restrict__ Lh, T* __restrict__ Lf, size_t total) {
-    for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total;
-         idx += (size_t)gridDim.x * blockDim.x) {
-        size_t t = idx;
-        int i = (int)(t & 1); t >>= 1;
-        int lane = (int)(t & 31); t >>= 5;
-        int s = (int)(t % d.KS); t /= d.KS;
-        int a = (int)(t % d.n); t /= d.n;
-        int k = (int)(t % d.Nk); t /= d.Nk;
-        int gtp = (int)(t % d.GT2);
-        int Q = (int)(t / d.GT2);
-        int row = lane >> 2, kk = lane & 3;
-        int gam = 16 * gtp + 8 * i + row;
-        int j = 4 * s + kk, r = j >> 1, c = j & 1;
-        double v = 0.0;
-        if (gam < d.nchol && r < d.m) {
-            double2 z = lh_elem(Lh, d, Q, k, a, gam, r);
-            v = c ? z.y : z.x;
-        }
-        Lf[idx] = (T)v;
-    }
-}
-
 __global__ void half_rot_h_kernel(Dims d, const double2* __restrict__ h1, const double2* __restrict__ psi_t,
                                   double2* __restrict__ ht) {
     // ht[k][a][q] = sum_p conj(A_k[p][a]) h_k[p][q]     (first line of Eq. 49)
@@ -150,7 +125,7 @@ AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     if (c->is_child) c->b1 = nullptr;        // owned by the spin-up context
     void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lh, c->Lxc, c->Lx3t, c->Lx, c->LxT, c->Lf, c->Lff, c->Lv3, c->Lv3f, c->vunits,
                     c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T, c->ws_Tx,
-                    c->ws_expart, c->ws_fbpart, c->ws_vbtot, c->ws_ld_chan, c->ws_info_chan, c->ws_ldr_chan, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
+                    c->ws_expart, c->ws_fbpart, c->ws_thetaF, c->ws_vbtot, c->ws_ld_chan, c->ws_info_chan, c->ws_ldr_chan, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
                     c->ws_f32, c->b1, c->ws_b1tmp, c->ws_gram, c->ws_rinv, c->ws_logdet2, c->ws_ldr, c->ws_info2};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -179,11 +154,9 @@ static int create_channel(afqmc_ctx** out, const afqmc_dims* dims, int n_chan, i
     d.NAG = (d.n + 3) / 4;
     d.GP = (d.nchol + 1) / 2;
     d.GQ = (d.nchol + 3) / 4;
-    d.GT2 = (d.nchol + 15) / 16;
     d.PRT = (d.m * d.m + 7) / 8;
     c->max_walkers = dims->max_walkers;
     c->prec32 = dims->precision == 1 ? 1 : 0;
-    c->opt_fb_pf = 8;
     c->opt_exchange_3m = 1;
     c->opt_exchange_regb = 1;
     c->spin_factor = open_shell ? 1.0 : 2.0;
@@ -226,7 +199,6 @@ static int create_channel(afqmc_ctx** out, const afqmc_dims* dims, int n_chan, i
     int rc = AFQMC_OK;
     auto A = [&](int r) { if (rc == AFQMC_OK) rc = r; };
     const size_t nLh = (size_t)Nk * Nk * d.n * d.nchol * d.m;
-    const size_t nLf = (size_t)Nk * d.GT2 * Nk * d.n * d.KS * 64;
     const int LD = d.N | 1;
     A(dev_alloc(&c->kminus, (size_t)Nk * Nk));
     A(dev_alloc(&c->kplus, (size_t)Nk * Nk));
@@ -235,8 +207,6 @@ static int create_channel(afqmc_ctx** out, const afqmc_dims* dims, int n_chan, i
     A(dev_alloc(&c->psi_t, (size_t)Nk * d.m * d.n));
     A(dev_alloc(&c->ht, (size_t)Nk * d.n * d.m));
     A(dev_alloc(&c->Lh, nLh));
-    if (c->prec32) A(dev_alloc(&c->Lff, nLf));      // single-precision storage of the force-bias operand
-    else A(dev_alloc(&c->Lf, nLf));
     A(dev_alloc(&c->ws_O, (size_t)nw * d.N * LD));
     A(dev_alloc(&c->ws_oinvT, (size_t)nw * d.N * d.N));
     A(dev_alloc(&c->ws_theta, (size_t)nw * (child ? d.N : Nk * n_total) * d.M));     // spin-up context: both channels, spin-major
@@ -302,10 +272,10 @@ static int create_channel(afqmc_ctx** out, const afqmc_dims* dims, int n_chan, i
         auto grid = [&](size_t total) { return (int)((total + T - 1) / T > 148 * 64 ? 148 * 64 : (total + T - 1) / T); };
         half_rot_h_kernel<<<grid((size_t)Nk * d.n * d.m), T, 0, st>>>(d, (const double2*)h1, c->psi_t, c->ht);
         half_rot_L_kernel<<<grid(nLh), T, 0, st>>>(d, (const double2*)L, c->psi_t, c->Lh, nLh);     // the half rotation, once
-        if (c->prec32) pack_Lf_kernel<float><<<grid(nLf), T, 0, st>>>(d, c->Lh, c->Lff, nLf);
-        else pack_Lf_kernel<double><<<grid(nLf), T, 0, st>>>(d, c->Lh, c->Lf, nLf);
-        c->launches += 3;
+        c->launches += 2;
         if (cudaGetLastError() != cudaSuccess) rc = AFQMC_CUDA_ERROR;
+        // force-bias operand Lf3 (single-precision storage when precision = 1)
+        if (rc == AFQMC_OK) rc = afqmc_i_pack_force_bias_operand(c, st);
         if (rc == AFQMC_OK) rc = afqmc_i_pack_exchange_operand(c, st);
         if (rc == AFQMC_OK && !child) rc = afqmc_i_vhs_setup(c, (const double2*)L, kminus, kneg, st);
     }
@@ -401,16 +371,6 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
         c->opt_exchange_wpc = value;
         return AFQMC_OK;
     }
-    if (strcmp(name, "force_bias_tile") == 0) {
-        if (value < 0 || value > 2) return AFQMC_INVALID_ARGUMENT;
-        c->opt_fb_tile = value;
-        return AFQMC_OK;
-    }
-    if (strcmp(name, "force_bias_prefetch") == 0) {
-        if (value < 0 || value > 256) return AFQMC_INVALID_ARGUMENT;
-        c->opt_fb_pf = value;
-        return AFQMC_OK;
-    }
     if (strcmp(name, "exchange_precision") == 0) {
         if (value < 0 || value > 2) return AFQMC_INVALID_ARGUMENT;
         if (value != 0) {                                           // n > 4: AFQMC_UNSUPPORTED
@@ -460,6 +420,11 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
     if (strcmp(name, "taylor_groups") == 0) {
         if (value < 0 || value > 64) return AFQMC_INVALID_ARGUMENT;
         c->opt_taylor_groups = value;
+        return AFQMC_OK;
+    }
+    if (strcmp(name, "taylor_subbatch") == 0) {
+        if (value < 0) return AFQMC_INVALID_ARGUMENT;
+        c->opt_taylor_subbatch = value;
         return AFQMC_OK;
     }
     if (strcmp(name, "green_cluster") == 0) {

@@ -445,12 +445,18 @@ int afqmc_i_green(afqmc_ctx* c, const double2* phi, int nw, double2* theta, doub
     int rc = run_overlap_inverse(c, phi, nw, theta ? c->ws_oinvT : nullptr, logdet, info, st);
     if (rc != AFQMC_OK || !theta) return rc;
     // Theta[i][q] = sum_j OinvT[i][j] * Phi[q][j]   (B is K-contiguous: element (k=j, col=q) at phi[q*N + j])
-    zg::Args a;
+    zg::Args a = {};
     a.A = c->ws_oinvT; a.strideA = (long long)d.N * d.N; a.lda = d.N;
     a.B = phi; a.strideB = (long long)d.M * d.N; a.ldb = d.N;
     a.C = theta; a.strideC = (long long)d.N * d.M; a.ldc = d.M;
     a.D = nullptr; a.strideD = 0; a.ldd = 0;
     a.M = d.N; a.N = d.M; a.K = d.N; a.alpha = 1.0;
+    c->frag_nw = 0; c->frag_src = nullptr;
+    if (c->fuse_frag) {      // inside afqmc_step / afqmc_block: the epilogue also writes the force-bias B fragments of this Theta
+        a.frag.F = c->ws_thetaF; a.frag.ktab = c->kminus; a.frag.m = d.m; a.frag.n = d.n; a.frag.Nk = d.Nk;
+        afqmc_i_fb_frag_layout(c, nw, &a.frag.NT, &a.frag.nwg, &a.frag.KSf);
+        c->frag_nw = nw; c->frag_src = theta;
+    }
     if (zg::launch<true>(c, a, nw, st) != cudaSuccess) return AFQMC_CUDA_ERROR;
     c->launches++;
     return AFQMC_OK;

@@ -20,7 +20,7 @@ int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, 
         if (cudaMemcpyAsync(T[0], phi, (size_t)nw * per * sizeof(double2), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
             return AFQMC_CUDA_ERROR;
         for (int j = 1; j <= order; ++j) {
-            zg::Args a;
+            zg::Args a = {};
             a.A = vhs; a.strideA = (long long)d.M * d.M; a.lda = d.M;
             a.B = T[(j - 1) & 1]; a.strideB = (long long)per; a.ldb = d.N;
             a.C = T[j & 1]; a.strideC = (long long)per; a.ldc = d.N;
@@ -31,23 +31,30 @@ int afqmc_i_propagate(afqmc_ctx* c, const double2* vhs, double dtau, int order, 
         }
         return AFQMC_OK;
     }
-    const int G = c->opt_taylor_groups > 0 ? c->opt_taylor_groups : tg::pick_groups(c, d.M, d.N, nw);
-    const size_t perx = tg::expanded_doubles(d.M, d.N, G);
-    if (perx > afqmc_i_taylor_ws_doubles(d)) return AFQMC_INVALID_ARGUMENT;   // a forced group count the workspace was not sized for
-    double* Tx[2] = {c->ws_Tx, c->ws_Tx + (size_t)c->max_walkers * afqmc_i_taylor_ws_doubles(d)};
-    if (tg::launch_expand<false>(phi, (long long)per, d.N, Tx[0], d.M, d.N, nw, st, G) != cudaSuccess) return AFQMC_CUDA_ERROR;
-    c->launches++;
-    for (int j = 1; j <= order; ++j) {
-        tg::Args a = {};
-        a.A = vhs; a.strideA = (long long)d.M * d.M; a.lda = d.M;
-        a.Bx = Tx[(j - 1) & 1]; a.strideBx = (long long)perx;
-        a.Cx = j < order ? Tx[j & 1] : nullptr; a.strideCx = (long long)perx;
-        a.D = phi; a.strideD = (long long)per; a.ldd = d.N;
-        a.Ct = nullptr; a.strideCt = 0; a.ldct = 0;
-        a.M = d.M; a.N = d.N; a.K = d.M; a.alpha = s / (double)j;
-        a.wpc = c->opt_taylor_wpc;
-        if (tg::launch(c, a, nw, st, G) != cudaSuccess) return AFQMC_CUDA_ERROR;
+    // Walkers per pass: all of them by default.  Option "taylor_subbatch" = b runs the whole series for b walkers at a time, so
+    // that their V (b * 16 M^2 bytes) can stay in L2 across the orders instead of being streamed from HBM once per order.
+    const int sb = (c->opt_taylor_subbatch > 0 && c->opt_taylor_subbatch < nw) ? c->opt_taylor_subbatch : nw;
+    for (int b0 = 0; b0 < nw; b0 += sb) {
+        const int nb = nw - b0 < sb ? nw - b0 : sb;
+        const int G = c->opt_taylor_groups > 0 ? c->opt_taylor_groups : tg::pick_groups(c, d.M, d.N, nb);
+        const size_t perx = tg::expanded_doubles(d.M, d.N, G);
+        if (perx > afqmc_i_taylor_ws_doubles(d)) return AFQMC_INVALID_ARGUMENT;   // a forced group count the workspace was not sized for
+        double* Tx[2] = {c->ws_Tx, c->ws_Tx + (size_t)c->max_walkers * afqmc_i_taylor_ws_doubles(d)};
+        double2* ph = phi + (size_t)b0 * per;
+        if (tg::launch_expand<false>(ph, (long long)per, d.N, Tx[0], d.M, d.N, nb, st, G) != cudaSuccess) return AFQMC_CUDA_ERROR;
         c->launches++;
+        for (int j = 1; j <= order; ++j) {
+            tg::Args a = {};
+            a.A = vhs + (size_t)b0 * d.M * d.M; a.strideA = (long long)d.M * d.M; a.lda = d.M;
+            a.Bx = Tx[(j - 1) & 1]; a.strideBx = (long long)perx;
+            a.Cx = j < order ? Tx[j & 1] : nullptr; a.strideCx = (long long)perx;
+            a.D = ph; a.strideD = (long long)per; a.ldd = d.N;
+            a.Ct = nullptr; a.strideCt = 0; a.ldct = 0;
+            a.M = d.M; a.N = d.N; a.K = d.M; a.alpha = s / (double)j;
+            a.wpc = c->opt_taylor_wpc;
+            if (tg::launch(c, a, nb, st, G) != cudaSuccess) return AFQMC_CUDA_ERROR;
+            c->launches++;
+        }
     }
     return AFQMC_OK;
 }

@@ -2,8 +2,8 @@
 // PAPER.md:87-107/:142-160 on phi, then the energy evaluation of PAPER.md:306-319 on the new phi.
 #include "common.cuh"
 
-int afqmc_i_step(afqmc_ctx* c, double2* ph, const double* x, double dtau, int order, int nw, double2* energy,
-                 double2* logdet, int* info, cudaStream_t st, cudaEvent_t phi_final) {
+static int step_body(afqmc_ctx* c, double2* ph, const double* x, double dtau, int order, int nw, double2* energy,
+                     double2* logdet, int* info, cudaStream_t st, cudaEvent_t phi_final) {
     int rc;
     afqmc_mark(c, 0, st);
     if ((rc = afqmc_x_green(c, ph, nw, c->ws_theta, nullptr, nullptr, st)) != AFQMC_OK) return rc;
@@ -21,6 +21,14 @@ int afqmc_i_step(afqmc_ctx* c, double2* ph, const double* x, double dtau, int or
     afqmc_mark(c, 8, st);      // marks 6 and 7 are recorded around the exchange kernel inside local_energy
     if (c->opt_timers) c->ev_valid = 1;
     return AFQMC_OK;
+}
+
+// Inside the composition both Green's functions live in the library's workspace, so Green's epilogue also writes them as the
+// force-bias kernel's B fragments (afqmc_set_fuse; zgemm.cuh FragOut) and the force-bias calls skip their re-layout pass.
+int afqmc_i_step(afqmc_ctx* c, double2* ph, const double* x, double dtau, int order, int nw, double2* energy,
+                 double2* logdet, int* info, cudaStream_t st, cudaEvent_t phi_final) {
+    AfqmcFuseGuard fuse(c);
+    return step_body(c, ph, x, dtau, order, nw, energy, logdet, info, st, phi_final);
 }
 
 AFQMC_API int afqmc_step(afqmc_ctx* c, void* phi, const double* x, double dtau, int order, int nw,

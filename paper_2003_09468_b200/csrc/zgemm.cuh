@@ -31,7 +31,16 @@ struct Cfg {
     static constexpr int B_LD = (BK * BN + NTHR - 1) / NTHR;
 };
 
+// Optional second output of the epilogue (a3 -> a4 fusion): C[i][j] of batch entry w is also stored as an element of the
+// force-bias B-fragment operand thetaF (force_bias.cu): row i = (k,a), column j = (k',r), Q = k - k' (table ktab[k*Nk + k']),
+// kappa = i*m + r  ->  thetaF[Q][w / (8 NT)][kappa >> 2][(w >> 3) % NT][lane = (w & 7)*4 + (kappa & 3)].
+struct FragOut {
+    double2* F; const int* ktab;
+    int m, n, Nk, NT, nwg, KSf;
+};
+
 struct Args {
+    FragOut frag;                              // frag.F == nullptr: off
     const double2* A; long long strideA; int lda;
     const double2* B; long long strideB; int ldb;
     double2* C; long long strideC; int ldc;
@@ -141,6 +150,12 @@ __global__ void __launch_bounds__(32 * WGM) zgemm_kernel(Args p) {
             if (j >= p.N) continue;
             double2 v = make_double2(p.alpha * acc[mt][nt][0], p.alpha * acc[mt][nt][1]);
             C[(size_t)i * p.ldc + j] = v;
+            if (p.frag.F) {
+                const FragOut& f = p.frag;
+                const int k2 = j / f.m, r = j - k2 * f.m, kap = i * f.m + r;
+                const int Q = f.ktab[(i / f.n) * f.Nk + k2];
+                f.F[((((size_t)Q * f.nwg + b / (8 * f.NT)) * f.KSf + (kap >> 2)) * f.NT + ((b >> 3) % f.NT)) * 32 + (b & 7) * 4 + (kap & 3)] = v;
+            }
             if (D) {
                 double2 o = D[(size_t)i * p.ldd + j];
                 o.x += v.x; o.y += v.y;
