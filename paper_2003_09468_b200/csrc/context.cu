@@ -391,7 +391,8 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
         return AFQMC_OK;
     }
     if (strcmp(name, "exchange_regb") == 0) {
-        c->opt_exchange_regb = value ? 1 : 0;
+        if (value < 0 || value > 2) return AFQMC_INVALID_ARGUMENT;
+        c->opt_exchange_regb = value;
         return AFQMC_OK;
     }
     if (strcmp(name, "exchange_np") == 0) {

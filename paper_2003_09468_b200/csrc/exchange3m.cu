@@ -316,6 +316,66 @@ __device__ __forceinline__ void x3_finish_task(double (&acc)[3][2][NP][2], doubl
             for (int j = 0; j < NP; ++j) acc[p][i][j][0] = acc[p][i][j][1] = 0.0;
 }
 
+// ---- pieces of the DEFERRED hand-over (exchange3m_reg_kernel, ASYNC): the tile a warp gives to its partner is published with
+// a non-blocking bar.arrive and collected by the partner one task LATER with bar.sync, so neither warp ever waits for the other
+// at a task end (the blocking version lost 6.5 % of its warp-samples there, profiles/r02c).  Named barrier 1 + 2 h + buf: "the
+// tile of role h in hand-over buffer buf is written" (32 arriving + 32 waiting threads); immediates, see x3_finish_task.
+__device__ __forceinline__ void x3_bar_arrive(int h, int buf) {
+    switch (2 * h + buf) {
+        case 0: asm volatile("bar.arrive 1, 64;" ::: "memory"); break;
+        case 1: asm volatile("bar.arrive 2, 64;" ::: "memory"); break;
+        case 2: asm volatile("bar.arrive 3, 64;" ::: "memory"); break;
+        default: asm volatile("bar.arrive 4, 64;" ::: "memory"); break;
+    }
+}
+__device__ __forceinline__ void x3_bar_wait(int h, int buf) {
+    switch (2 * h + buf) {
+        case 0: asm volatile("bar.sync 1, 64;" ::: "memory"); break;
+        case 1: asm volatile("bar.sync 2, 64;" ::: "memory"); break;
+        case 2: asm volatile("bar.sync 3, 64;" ::: "memory"); break;
+        default: asm volatile("bar.sync 4, 64;" ::: "memory"); break;
+    }
+}
+// contracts the kept tile of the PREVIOUS task with the partner's tile of that task (in `xr`, hand-over buffer `buf`)
+template <int NP>
+__device__ __forceinline__ void x3_collect(const double2 (&keep)[NP][2], const double2* __restrict__ xr, int h, int buf, const X3Lane& L,
+                                           double (&er)[NP], double (&ei)[NP]) {
+    x3_bar_wait(h ^ 1, buf);
+#pragma unroll
+    for (int j = 0; j < NP; ++j)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const double2 p = xr[j * 64 + L.sr[e]];
+            er[j] = fma(keep[j][e].x, p.x, er[j]); er[j] = fma(-keep[j][e].y, p.y, er[j]);
+            ei[j] = fma(keep[j][e].x, p.y, ei[j]); ei[j] = fma(keep[j][e].y, p.x, ei[j]);
+        }
+}
+// end of a task: combine the three products, publish m-tile 1-KEEP in `xw` (buffer `buf`), keep m-tile KEEP, clear
+template <int NP, int KEEP>
+__device__ __forceinline__ void x3_publish(double (&acc)[3][2][NP][2], double2 (&keep)[NP][2], double2* __restrict__ xw, int h, int buf,
+                                           const X3Lane& L) {
+    constexpr int GIVE = 1 - KEEP;
+#pragma unroll
+    for (int j = 0; j < NP; ++j)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            xw[j * 64 + L.sw[e]] = make_double2(acc[0][GIVE][j][e] - acc[2][GIVE][j][e], acc[0][GIVE][j][e] + acc[1][GIVE][j][e]);
+            keep[j][e] = make_double2(acc[0][KEEP][j][e] - acc[2][KEEP][j][e], acc[0][KEEP][j][e] + acc[1][KEEP][j][e]);
+        }
+    x3_bar_arrive(h, buf);
+#pragma unroll
+    for (int p = 0; p < 3; ++p)
+#pragma unroll
+        for (int i = 0; i < 2; ++i)
+#pragma unroll
+            for (int j = 0; j < NP; ++j) acc[p][i][j][0] = acc[p][i][j][1] = 0.0;
+}
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;\n" ::"r"(smem_u32(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
 // Sum over the lanes of each walker-in-pair (lane bit 1 = wp), then over the warps in a fixed order (deterministic).
 template <int NP, int NWARP, bool GRIDPAIRS>
 __device__ __forceinline__ void x3_reduce_store(double* red /* shared, [warp][NWC][2] */, const double (&er)[NP], const double (&ei)[NP],
@@ -517,7 +577,7 @@ __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
 //      next item's stream): the inner loop is LDG.128 + DMMA only;
 //   4. at the end of each task the two warps swap one m-tile through shared memory and contract (x3_finish_task).
 // ---------------------------------------------------------------------------------------------------------------------
-template <int KSF, int TAIL, int NP, int MAXREG>
+template <int KSF, int TAIL, int NP, int MAXREG, bool ASYNC>
 __global__ void __launch_bounds__(64) __maxnreg__(MAXREG) exchange3m_reg_kernel(
     Dims d, int nw, int nitems, const int* __restrict__ units, const int* __restrict__ kminus, const int* __restrict__ kplus,
     const int* __restrict__ kneg, const double* __restrict__ Lx3t, const double2* __restrict__ theta,
@@ -534,7 +594,8 @@ __global__ void __launch_bounds__(64) __maxnreg__(MAXREG) exchange3m_reg_kernel(
     double2* raw = reinterpret_cast<double2*>(x3_smem);
     double2* xbuf = raw + 4 * raw_len;
     double2* red = xbuf + 2 * NBUF * NP * 64;
-    uint64_t* mbar = reinterpret_cast<uint64_t*>(red + 2 * NWC);
+    double2* aring = red + 2 * NWC;                  // ASYNC: [role][MST][32] one task of the A stream per warp, lane-private slots
+    uint64_t* mbar = reinterpret_cast<uint64_t*>(aring + (ASYNC ? 2 * MST * 32 : 0));
     if (threadIdx.x == 0) {
         for (int i = 0; i < 4; ++i) mbar_init(&mbar[i], 1);
         mbar_fence_init();
@@ -578,17 +639,33 @@ __global__ void __launch_bounds__(64) __maxnreg__(MAXREG) exchange3m_reg_kernel(
     issue_theta(cur, 0);
     int bufsel = 0, phase = 0;          // phase: bit b = parity to wait for on buffer b
     // A ring: fa[slot][p] = micro-load p of the k-step in that slot; prologue = the first DA k-steps of the first item
-    double2 fa[DA][3];
+    // (ASYNC: the ring is one whole task in shared memory, filled by per-lane cp.async, one commit group per k-step; slot =
+    // micro-load index, so every address is a constant and the lookahead is a full task)
+    double2 fa[ASYNC ? 1 : DA][3];
     const double2* pa = stream_ptr(cur, 0);
+    double2* ar = aring + h * (MST * 32) + lane;
+    if (ASYNC) {
 #pragma unroll
-    for (int q = 0; q < DA; ++q) {
+        for (int ks = 0; ks < KSPT; ++ks) {
+            if (ks < KSF) {
 #pragma unroll
-        for (int p = 0; p < 3; ++p) fa[q][p] = make_double2(0.0, 0.0);
-        if (q < KSF) {
+                for (int p = 0; p < 3; ++p) cp_async16(ar + (3 * ks + p) * 32, pa + (3 * ks + p) * 32);
+            } else {
+                cp_async16(ar + (3 * KSF) * 32, pa + (3 * KSF) * 32);
+            }
+            cp_async_commit();
+        }
+    } else {
 #pragma unroll
-            for (int p = 0; p < 3; ++p) fa[q][p] = __ldg(pa + (3 * q + p) * 32);
-        } else {
-            fa[q][0] = __ldg(pa + (3 * KSF) * 32);
+        for (int q = 0; q < DA; ++q) {
+#pragma unroll
+            for (int p = 0; p < 3; ++p) fa[q][p] = make_double2(0.0, 0.0);
+            if (q < KSF) {
+#pragma unroll
+                for (int p = 0; p < 3; ++p) fa[q][p] = __ldg(pa + (3 * q + p) * 32);
+            } else {
+                fa[q][0] = __ldg(pa + (3 * KSF) * 32);
+            }
         }
     }
     int base = 0;                       // ring slot of the next task's first k-step
@@ -597,6 +674,9 @@ __global__ void __launch_bounds__(64) __maxnreg__(MAXREG) exchange3m_reg_kernel(
 #pragma unroll
     for (int j = 0; j < NP; ++j) er[j] = ei[j] = 0.0;
     int buf = 0, par = 0;
+    double2 keep[NP][2];                // ASYNC: the kept m-tile of the previous task (contracted one task later)
+#pragma unroll
+    for (int j = 0; j < NP; ++j) keep[j][0] = keep[j][1] = make_double2(0.0, 0.0);
     double acc[3][2][NP][2];
 #pragma unroll
     for (int p = 0; p < 3; ++p)
@@ -692,14 +772,55 @@ __global__ void __launch_bounds__(64) __maxnreg__(MAXREG) exchange3m_reg_kernel(
                 else x3_finish_task<NP, 1>(acc, xw, xr, 1, L, er, ei);
                 buf ^= 1;
             };
+            // ASYNC: the same gamma-quad with the A fragments read from the shared-memory ring (slot = micro-load index) and the
+            // slot refilled at once with the same micro-load of the NEXT task (cp.async from `pn`); the partner's tile of the
+            // previous task is collected first, this task's tile is published without waiting
+            auto task_async = [&](const double2* pn, const bool have_prev) {
+                if (have_prev) x3_collect<NP>(keep, xbuf + (((h ^ 1) * NBUF + (buf ^ 1)) * NP) * 64, h, buf ^ 1, L, er, ei);
+#pragma unroll
+                for (int ks = 0; ks < KSPT; ++ks) {
+                    cp_async_wait<KSPT - 1>();                          // the commit group of this k-step has landed
+                    if (ks < KSF) {
+                        double2 f[3];
+#pragma unroll
+                        for (int p = 0; p < 3; ++p) f[p] = ar[(3 * ks + p) * 32];
+#pragma unroll
+                        for (int p = 0; p < 3; ++p)
+#pragma unroll
+                            for (int j = 0; j < NP; ++j) {
+                                dmma884(acc[p][0][j][0], acc[p][0][j][1], f[p].x, B[3 * ks + p][j]);
+                                dmma884(acc[p][1][j][0], acc[p][1][j][1], f[p].y, B[3 * ks + p][j]);
+                            }
+#pragma unroll
+                        for (int p = 0; p < 3; ++p) cp_async16(ar + (3 * ks + p) * 32, pn + (3 * ks + p) * 32);
+                    } else {                                             // tail k-step
+                        const double2 f = ar[(3 * KSF) * 32];
+#pragma unroll
+                        for (int p = 0; p < 2; ++p)
+#pragma unroll
+                            for (int j = 0; j < NP; ++j) {
+                                dmma884(acc[p][0][j][0], acc[p][0][j][1], f.x, B[3 * KSF + (TAIL ? p : 0)][j]);
+                                dmma884(acc[p][1][j][0], acc[p][1][j][1], f.y, B[3 * KSF + (TAIL ? p : 0)][j]);
+                            }
+                        cp_async16(ar + (3 * KSF) * 32, pn + (3 * KSF) * 32);
+                    }
+                    cp_async_commit();
+                }
+                double2* xw = xbuf + ((h * NBUF + buf) * NP) * 64;
+                if (h == 0) x3_publish<NP, 0>(acc, keep, xw, h, buf, L);
+                else x3_publish<NP, 1>(acc, keep, xw, h, buf, L);
+                buf ^= 1;
+            };
             for (int tq = 0; tq < GQ; ++tq) {
                 const double2* pn = tq + 1 < GQ ? pa + TASK : pcont;
-                if (DA == 1 || base == 0) task(std::integral_constant<int, 0>(), pn);
+                if (ASYNC) task_async(pn, ab > 0 || tq > 0);
+                else if (DA == 1 || base == 0) task(std::integral_constant<int, 0>(), pn);
                 else task(std::integral_constant<int, 1 % DA>(), pn);
                 base = (base + KSPT) % DA;
                 pa += TASK;
             }
         }
+        if (ASYNC) x3_collect<NP>(keep, xbuf + (((h ^ 1) * NBUF + (buf ^ 1)) * NP) * 64, h, buf ^ 1, L, er, ei);      // the item's last tile
         // ---- the item's result: lanes of each walker-in-pair (lane bit 1), then the two warps (fixed order) ----
 #pragma unroll
         for (int j = 0; j < NP; ++j) {
@@ -716,7 +837,8 @@ __global__ void __launch_bounds__(64) __maxnreg__(MAXREG) exchange3m_reg_kernel(
 #pragma unroll
             for (int j = 0; j < NP; ++j) red[par * NWC + 2 * j + (lane >> 1)] = make_double2(er[j], ei[j]);
         }
-        asm volatile("bar.sync 1, 64;" ::: "memory");
+        if (ASYNC) asm volatile("bar.sync 5, 64;" ::: "memory");      // (1..4 are the hand-over barriers)
+        else asm volatile("bar.sync 1, 64;" ::: "memory");
         if (h == 0 && (lane == 0 || lane == 2)) {
 #pragma unroll
             for (int j = 0; j < NP; ++j) {
@@ -731,6 +853,7 @@ __global__ void __launch_bounds__(64) __maxnreg__(MAXREG) exchange3m_reg_kernel(
         if (!has_next) break;
         item = nxt; cur = nx; bufsel ^= 1;
     }
+    if (ASYNC) cp_async_wait<0>();      // (the last task refilled the ring once more: loaded, never used)
 }
 
 template <int NP>
@@ -787,20 +910,22 @@ int launch_x3_cfg(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
 }
 
 template <int NP>
-size_t x3_reg_smem_bytes(const Dims& d) {
+size_t x3_reg_smem_bytes(const Dims& d, bool async) {
     const size_t raw = (size_t)4 * 2 * NP * d.n * d.m * sizeof(double2);
-    return raw + (size_t)2 * 2 * NP * 64 * sizeof(double2) + (size_t)2 * 2 * NP * sizeof(double2) + 4 * sizeof(uint64_t);
+    const X3Geom g = x3_geom(d.m);
+    const size_t aring = async ? (size_t)2 * (3 * g.KSF + g.TAIL) * 32 * sizeof(double2) : 0;
+    return raw + (size_t)2 * 2 * NP * 64 * sizeof(double2) + (size_t)2 * 2 * NP * sizeof(double2) + aring + 4 * sizeof(uint64_t);
 }
 
-template <int KSF, int TAIL, int NP>
+template <int KSF, int TAIL, int NP, bool ASYNC>
 int launch_x3_reg(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     // registers: MSPT * NP B fragments + 12 NP accumulators (doubles) + the A ring; 200 registers = five resident CTAs,
     // 168 = six, 128 = eight
     constexpr int MS = 3 * KSF + 2 * TAIL;
     constexpr int MAXREG = NP == 1 ? 168 : 255;
     const Dims& d = c->d;
-    const size_t smem = x3_reg_smem_bytes<NP>(d);
-    auto kern = exchange3m_reg_kernel<KSF, TAIL, NP, MAXREG>;
+    const size_t smem = x3_reg_smem_bytes<NP>(d, ASYNC);
+    auto kern = exchange3m_reg_kernel<KSF, TAIL, NP, MAXREG, ASYNC>;
     if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
     afqmc_prefer_smem(c, (const void*)kern);
     const long long nitems = (long long)c->nunits * ((nw + 2 * NP - 1) / (2 * NP));
@@ -823,8 +948,12 @@ int launch_x3_reg(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
 
 template <int KSF, int TAIL>
 int launch_x3_reg_np(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
-    if (nw <= 2 || c->opt_exchange_np == 1) return launch_x3_reg<KSF, TAIL, 1>(c, theta, nw, st);      // two walkers per CTA
-    return launch_x3_reg<KSF, TAIL, 2>(c, theta, nw, st);
+    // option exchange_regb: 1 = A stream by cp.async through a shared-memory ring + deferred hand-over (default), 2 = A stream
+    // prefetched in registers + blocking hand-over
+    const bool async = c->opt_exchange_regb != 2;
+    if (nw <= 2 || c->opt_exchange_np == 1)      // two walkers per CTA
+        return async ? launch_x3_reg<KSF, TAIL, 1, true>(c, theta, nw, st) : launch_x3_reg<KSF, TAIL, 1, false>(c, theta, nw, st);
+    return async ? launch_x3_reg<KSF, TAIL, 2, true>(c, theta, nw, st) : launch_x3_reg<KSF, TAIL, 2, false>(c, theta, nw, st);
 }
 
 }  // namespace

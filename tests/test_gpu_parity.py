@@ -551,7 +551,9 @@ def test_exchange_3m_and_4m_kernels_against_the_oracle(kw):
                            ("3m_generic_depth2", {"exchange_regb": 0, "exchange_depth": 2}),
                            ("3m_generic_4warps", {"exchange_warps": 4}), ("3m_generic_np4", {"exchange_np": 4}),
                            ("3m_generic_np1_4warps", {"exchange_regb": 0, "exchange_np": 1, "exchange_warps": 4}),
-                           ("3m_two_walkers_per_cta", {"exchange_np": 1})):
+                           ("3m_two_walkers_per_cta", {"exchange_np": 1}),
+                           ("3m_register_prefetch_blocking_handover", {"exchange_regb": 2}),
+                           ("3m_register_prefetch_two_walkers", {"exchange_regb": 2, "exchange_np": 1})):
             for k, v in opts.items():
                 case.ctx.set_option(k, v)
             res[name] = case.ctx.local_energy(theta_d).cpu().numpy()
