@@ -31,9 +31,9 @@ METRIC = "walker-steps/s incl. local energy"
 UNIT = "walker-steps/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE exchange-kernel launch, from the committed
-# `ncu --set full` capture of this same command (profiles/r01g_ncu_full_metrics.txt, the default 3M kernel); bench.py
+# `ncu --set full` capture of the default exchange kernel (profiles/r02c_ncu_exchange.md names the command); bench.py
 # cannot measure DRAM traffic itself.  Only the configuration that was captured has a value.
-EXCHANGE_DRAM_TRAFFIC = {"C3": {"bytes": 722.316e6 + 9.972e6, "source": "profiles/r01g_ncu_full_metrics.txt"}}
+EXCHANGE_DRAM_TRAFFIC = {"C3": {"bytes": 989.908e6 + 9.361e6, "source": "profiles/r02c_ncu_exchange.md"}}
 
 
 def load_measured_peaks():
@@ -329,9 +329,12 @@ def run_ours(args):
         ex_flops = ex_flops_default
         achieved = ex_flops / (ex_ms * 1e-3) / 1e12
         peak_probe = binding.probe_fp64(1, 20000)          # DMMA issue-rate probe, this GPU, now
-        # algorithmic bytes of one exchange launch: the packed operand once (Lx3 of the 3M kernel: Re+Im, Re, Im of
-        # Lh with r padded to a multiple of 4 = 24 bytes per complex element) + theta once
-        ctx_alg_bytes = cfg.nk ** 2 * cfg.n * cfg.nchol * (4 * ((cfg.m + 3) // 4)) * 24 + nw * cfg.N * cfg.M * 16
+        # algorithmic bytes of one exchange launch = the METHOD's bytes: the half-rotated tensor once + Theta once, 16 bytes
+        # per complex number; beside it what the kernel's own packed operand occupies (Lx3t: the three A
+        # variants Re+Im, Re, Im stored = 24 bytes per element, K padded to k-steps)
+        ctx_alg_bytes = cfg.nk ** 2 * cfg.n * cfg.nchol * cfg.m * 16 + nw * cfg.N * cfg.M * 16
+        ksf, tail = ((cfg.m // 4, 1) if cfg.m % 4 in (1, 2) else ((cfg.m + 3) // 4, 0))
+        packed_bytes = cfg.nk ** 2 * ((cfg.n + 3) // 4) * ((cfg.nchol + 3) // 4) * (3 * ksf + tail) * 64 * 8 + nw * cfg.N * cfg.M * 16
         peaks = load_measured_peaks()
         roofline = {
             "kernel": "exchange (a9), afqmc_local_energy", "bound": "tensor", "achieved": achieved,
@@ -340,6 +343,7 @@ def run_ours(args):
             "traffic_unit": "bytes per launch (DRAM read+write)",
             "traffic_source": EXCHANGE_DRAM_TRAFFIC.get(cfg.name, {}).get("source"),
             "algorithmic_bytes": float(ctx_alg_bytes),
+            "packed_operand_bytes": float(packed_bytes),
             "peak_source": "live FP64 DMMA.8x8x4 probe (afqmc_probe_fp64); MEASURED_PEAKS.json has no FP64 entry",
             "flops_per_launch": ex_flops, "ms_per_launch": ex_ms,
             "flops_note": "EXECUTED real flops of the default kernel (3M complex product when n <= 4: 6 per complex "
@@ -351,6 +355,12 @@ def run_ours(args):
         }
         if peaks and "bf16_tflops" in peaks:
             roofline["peak_alt_bf16_ratio"] = peaks["bf16_tflops"] * 45.0 / 2250.0
+        # sanity check of the probe from the record itself: 148 SMs x 128 FP64 flops per clock (one DMMA.8x8x4 = 512 flops per
+        # 16 cycles and SM sub-partition) x the SM clock sampled during the timed region
+        clk = sampler.summary()
+        if clk and clk.get("sm_mhz"):
+            roofline["peak_check"] = {"formula": "num_sms * 128 flop/clk * sm_mhz", "num_sms": 148, "sm_mhz": clk["sm_mhz"],
+                                      "tflops": 148 * 128 * clk["sm_mhz"] * 1e6 / 1e12}
         stages = {k: v / args.steps for k, v in stage_acc.items()}
         # the other kernel the north_star names: force bias (a4).  EXECUTED flops: 3M complex product, 6 Nk^2 n m nchol real
         # flops per walker (the plain definition / a real embedding costs 8); the stage time includes the reduction kernel

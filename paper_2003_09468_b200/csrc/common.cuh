@@ -108,6 +108,7 @@ struct afqmc_ctx {
     int opt_exchange_3m;    // 1 (default) = 3M exchange kernel when n <= 4, 0 = the 4M kernel of energy.cu
     int opt_exchange_wpc;   // 0 = automatic, else warps per CTA of the exchange kernel (4,5,6,8)
     int opt_exchange_np;    // tuning aid (3M kernel): 0 = automatic, else 1/2/4 walker pairs (n-tiles) per warp
+    int opt_exchange_ctas;  // tuning aid: 0 = as many CTAs of the register-B exchange kernel per SM as fit, else at most this many
     int opt_exchange_regb;  // 1 (default) = theta block of a warp in registers when m <= 28 (exchange3m_reg_kernel), 0 = generic kernel
     int opt_timers;     // record stage events in afqmc_step
     int opt_taylor_legacy;  // testing aid: 1 = shared-memory-tiled zgemm for the Taylor chain

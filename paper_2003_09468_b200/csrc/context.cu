@@ -395,6 +395,11 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
         c->opt_exchange_regb = value;
         return AFQMC_OK;
     }
+    if (strcmp(name, "exchange_ctas") == 0) {
+        if (value < 0 || value > 16) return AFQMC_INVALID_ARGUMENT;
+        c->opt_exchange_ctas = value;
+        return AFQMC_OK;
+    }
     if (strcmp(name, "exchange_np") == 0) {
         if (value != 0 && value != 1 && value != 2 && value != 4) return AFQMC_INVALID_ARGUMENT;
         c->opt_exchange_np = value;

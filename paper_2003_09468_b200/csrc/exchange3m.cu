@@ -924,7 +924,12 @@ int launch_x3_reg(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     constexpr int MS = 3 * KSF + 2 * TAIL;
     constexpr int MAXREG = NP == 1 ? 168 : 255;
     const Dims& d = c->d;
-    const size_t smem = x3_reg_smem_bytes<NP>(d, ASYNC);
+    size_t smem = x3_reg_smem_bytes<NP>(d, ASYNC);
+    // tuning aid "exchange_ctas": at most that many CTAs per SM (the shared-memory request is padded so that no more fit)
+    if (c->opt_exchange_ctas > 0) {
+        const size_t pad = ((size_t)c->smem_sm / c->opt_exchange_ctas - 1024) & ~(size_t)127;
+        if (pad > smem && pad <= (size_t)c->smem_optin) smem = pad;
+    }
     auto kern = exchange3m_reg_kernel<KSF, TAIL, NP, MAXREG, ASYNC>;
     if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
     afqmc_prefer_smem(c, (const void*)kern);
@@ -932,11 +937,11 @@ int launch_x3_reg(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     if (nitems > 0x7fffffffLL) return AFQMC_UNSUPPORTED;
     // persistent grid: as many CTAs as are resident (remembered per context)
     FuncAttr* f = afqmc_fattr(c, (const void*)kern);
-    int occ = f ? f->occ : -1;
+    int occ = (f && f->occ_smem == (int)smem) ? f->occ : -1;
     if (occ < 0) {
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 64, smem) != cudaSuccess) { (void)cudaGetLastError(); return AFQMC_CUDA_ERROR; }
         if (occ < 1) return AFQMC_UNSUPPORTED;
-        if (f) f->occ = occ;
+        if (f) { f->occ = occ; f->occ_smem = (int)smem; }
     }
     long long grid = (long long)occ * c->num_sms;
     if (grid > nitems) grid = nitems;

@@ -386,6 +386,45 @@ def test_a0_half_rotation_probed_through_the_abi(kw):
         ctx.close()
 
 
+# walker counts that reach every split of the force-bias kernel (force_bias.cu): one n-tile per warp (nw <= 8), two (16),
+# warp pairs sharing the A ring (17..32), four warps per A ring with idle warps in the last walker super-group (40, 70), and
+# Cholesky counts that give 1..5 m-tiles per warp incl. a ragged last m-group (nchol = 100: 13 tiles = 5 + 5 + 3)
+@pytest.mark.parametrize("kw", [dict(mesh=(2, 2, 1), m=6, n=2, nchol=5, nw=7), dict(mesh=(3, 1, 1), m=7, n=3, nchol=16, nw=16),
+                                dict(mesh=(2, 1, 2), m=9, n=2, nchol=24, nw=21), dict(mesh=(1, 3, 1), m=10, n=3, nchol=29, nw=32),
+                                dict(mesh=(2, 2, 1), m=5, n=2, nchol=100, nw=40), dict(mesh=(1, 1, 2), m=26, n=4, nchol=41, nw=70)],
+                         ids=lambda k: "c%d_w%d" % (k["nchol"], k["nw"]))
+def test_force_bias_tile_and_walker_splits(kw):
+    """afqmc_force_bias on random (not Green-derived) Theta against orc.force_bias on every walker, and the same numbers
+    from afqmc_step's fused path (Green's epilogue writes the B fragments) through the step's Coulomb energy."""
+    from paper_2003_09468_b200 import binding
+    cfg = synth.tiny_config(seed=31, **kw)
+    pb = synth.make_problem(cfg)
+    ctx = binding.from_problem(pb)
+    try:
+        Lh, _ = orc.half_rotate(pb.L, pb.psi_t, pb.h1)
+        rng = np.random.default_rng(5)
+        theta = rng.standard_normal((cfg.nw, cfg.N, cfg.M)) + 1j * rng.standard_normal((cfg.nw, cfg.N, cfg.M))
+        vb = ctx.force_bias(_to_dev(theta)).cpu().numpy()
+        for w in range(cfg.nw):
+            vb_o = orc.force_bias(cfg.mesh, Lh, theta[w])
+            assert relerr(vb[w], vb_o) < 1e-12, (w, relerr(vb[w], vb_o))
+        # fewer walkers than the context was made for: the fragment workspace keeps finite leftovers of the larger batch
+        nsub = max(1, cfg.nw // 3)
+        vb_s = ctx.force_bias(_to_dev(theta[:nsub])).cpu().numpy()
+        assert relerr(vb_s, vb[:nsub]) < 1e-13       # (another walker count cuts the K range elsewhere: not bitwise)
+        # fused path: the Coulomb energy of afqmc_step is 1/2 sum v[Q] v[-Q] of the force bias of the propagated walkers
+        phi_d, x_d = _to_dev(pb.phi), _to_dev(pb.x)
+        e, _, info = ctx.step(phi_d, x_d, cfg.dtau, cfg.order)
+        assert int(info.abs().sum()) == 0
+        th2, _, _ = ctx.green(phi_d)                   # phi_d now holds the propagated walkers
+        vb2 = ctx.force_bias(th2).cpu().numpy()         # unfused: the re-layout kernel
+        _, kneg = orc.k_tables(cfg.mesh)
+        ec = 0.5 * np.einsum("wqg,wqg->w", vb2, vb2[:, kneg, :])
+        assert relerr(e.cpu().numpy()[:, 1], ec) < 1e-11
+    finally:
+        ctx.close()
+
+
 def test_singular_overlap_reports_info(small_case):
     case = small_case
     phi = case.pb.phi[:2].copy()
