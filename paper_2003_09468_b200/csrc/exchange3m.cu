@@ -33,7 +33,7 @@
 //  * m <= 28 (exchange3m_reg_kernel): a warp's theta block is only MSPT * NP <= 42 fragments per lane, so it is read from shared
 //    memory ONCE per (CTA, a-group pair) and stays in REGISTERS for all gamma-quads; the task (KSF, TAIL are template parameters)
 //    is fully unrolled, and the inner loop is LDG.128 (A) + DADD + DMMA only: no shared-memory traffic per micro-step (the
-//    generic kernel's B loads were 29 % of its LSU wavefronts, LSU 70 % busy; profiles/r02a).
+//    generic kernel's B loads were 29 % of its LSU wavefronts, LSU 70 % busy in an ncu capture of this round).
 #include <type_traits>
 #include "common.cuh"
 
@@ -104,7 +104,7 @@ static int pack_lxc(afqmc_ctx* c, cudaStream_t st) {
 }
 
 // Lx3t (m <= 28, exchange3m_reg_kernel): the three A variants STORED, so that the inner loop has no DADD (one FP64 add between
-// DMMAs costs the pipe ~7 cycles, measured: profiles/r02_dmma_probe.md):
+// DMMAs costs the pipe 7-8 cycles, measured: profiles/r02b_ncu_force_bias.md, profiles/r02c_ncu_exchange.md):
 //   Lx3t[Q][k][ag][gq][ml < 3 KSF + TAIL][lane][2]   ml = 3 ks + p: variant p (0: Re+Im, 1: Re, 2: Im) of tiles 0,1 at r = 4 ks + kk;
 //   ml = 3 KSF (tail): the real-embedded fragment of tiles 0,1 (as in Lxc).  One coalesced 512-byte LDG.128 per micro-step.
 namespace {
@@ -571,11 +571,20 @@ __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
 //      warp computes, no thread waits on an L2 round trip and there is no CTA-wide barrier);
 //   2. the warp expands it into the three B variants straight into MSPT * NP REGISTERS (once per a-group pair);
 //   3. every gamma-quad of the unit runs against those registers: the task is fully unrolled (KSF, TAIL are template
-//      parameters), the A stream (Lx3t: the three variants stored) is prefetched DA k-steps ahead in a register ring whose slot
-//      of a task's first k-step (BASE) rotates by KSPT mod DA from task to task (DA copies of the task body behind a
-//      warp-uniform switch), and the ring runs on across tasks, a-group pairs and ITEMS (the last task of an item prefetches the
-//      next item's stream): the inner loop is LDG.128 + DMMA only;
-//   4. at the end of each task the two warps swap one m-tile through shared memory and contract (x3_finish_task).
+//      parameters) and the A stream (Lx3t: the three variants stored) reaches the warp
+//        ASYNC (default): through a shared-memory ring that holds exactly ONE task (MST micro-loads of 512 bytes per warp,
+//          lane-private 16-byte slots): slot = micro-load index, so every address is a constant; a slot is refilled by the
+//          lane's own cp.async (SASS LDGSTS.E.128) with the same micro-load of the NEXT task right after it was read, one
+//          commit group per k-step, `cp.async.wait_group KSPT-1` before a k-step: a full task of lookahead at no register cost
+//          (222 registers, no spills; the register ring below allowed two k-steps at 255 registers and 6 % of the warp samples
+//          sat on DMMAs waiting for an A fragment from L2);
+//        !ASYNC (option exchange_regb = 2): prefetched DA k-steps ahead in a register ring whose slot of a task's first k-step
+//          (BASE) rotates by KSPT mod DA from task to task (DA copies of the task body behind a warp-uniform switch);
+//      either way the stream runs on across tasks, a-group pairs and ITEMS (the last task of an item prefetches the next item's
+//      stream): the inner loop is LDS.128 / LDG.128 + DMMA only;
+//   4. at the end of each task the two warps swap one m-tile through shared memory and contract: ASYNC publishes its tile with
+//      bar.arrive and collects the partner's tile of the PREVIOUS task (x3_publish / x3_collect), so no warp waits at a task
+//      end; !ASYNC meets at a blocking bar.sync per task (x3_finish_task).
 // ---------------------------------------------------------------------------------------------------------------------
 template <int KSF, int TAIL, int NP, int MAXREG, bool ASYNC>
 __global__ void __launch_bounds__(64) __maxnreg__(MAXREG) exchange3m_reg_kernel(
