@@ -912,7 +912,12 @@ int launch_x3_np(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
 
 template <bool GRIDPAIRS>
 int launch_x3_cfg(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
-    const bool two_pairs = GRIDPAIRS || c->opt_exchange_wpc == 4;         // option "exchange_warps" = 4: two warp pairs per CTA
+    // Warp pairs per CTA: one (64 threads) while seven such CTAs fit an SM's shared memory (the register budget of the
+    // two-walker-pair tile); when the staged theta blocks are larger than that (m = 52 at C4: 45 KB per CTA) two pairs share one
+    // staging, which keeps 12 warps resident instead of 10 and halves the theta traffic (C4: 25.5 -> 20.6 ms; round 1's kernel:
+    // 23.0 ms).  Option "exchange_warps" = 4 forces two pairs, = 2 one.
+    const size_t smem1 = x3_smem_bytes<2>(x3_geom(c->d.m), GRIDPAIRS ? 1 : c->d.NAG, 1);
+    const bool two_pairs = GRIDPAIRS || c->opt_exchange_wpc == 4 || (c->opt_exchange_wpc == 0 && smem1 * 7 > (size_t)c->smem_sm);
     const int da = c->opt_exchange_depth == 2 ? 2 : 3;                     // option "exchange_depth": k-steps of A prefetch
     if (two_pairs) return da == 2 ? launch_x3_np<2, 2, GRIDPAIRS>(c, theta, nw, st) : launch_x3_np<2, 3, GRIDPAIRS>(c, theta, nw, st);
     return da == 2 ? launch_x3_np<1, 2, GRIDPAIRS>(c, theta, nw, st) : launch_x3_np<1, 3, GRIDPAIRS>(c, theta, nw, st);
