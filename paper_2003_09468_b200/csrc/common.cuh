@@ -96,6 +96,10 @@ struct afqmc_ctx {
     double2* ws_ld_chan; // [nw] this channel's log det (open shell: combined by openshell.cu)
     int* ws_info_chan;  // [nw] this channel's status
     double* ws_ldr_chan; // [nw] this channel's log det R of the orthogonalisation
+    // real orbitals (the dense Gamma-point supercell representation of PAPER.md:260, :276-284): detected in a0 as exactly zero
+    // imaginary parts of the half-rotated tensor Lh (force bias, exchange) / of L (vHS); the contractions then need two real
+    // products per complex product instead of three.  opt_real = 0 switches the shortcut off (testing aid).
+    int real_lh, real_l, opt_real;
     int prec32;         // 1 = complex64 boundary (afqmc_dims.precision = 1, boundary32.cu)
     float* ws_f32;      // precision 1: device staging of afqmc_step_host ([nw][M][N][2] + x + energy + logdet floats)
     int fuse_frag;      // 1 while a composition (afqmc_step, afqmc_block) runs: Green's epilogue also writes ws_thetaF ...
@@ -175,6 +179,11 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}\n" ::"r"(smem_u32(bar)), "r"(parity)
         : "memory");
 }
+// Orders this thread's earlier generic-proxy accesses to shared memory (LDS) before later async-proxy accesses (the bulk copy
+// that refills a ring stage).  Every consumer executes it before it releases a stage: without it the refill of a stage is not
+// ordered after the reads of its previous contents (PTX memory model: two proxies), and the vHS kernel's two-product variant
+// was seen to read partly refilled stages at 4 resident CTAs per SM (run-to-run differences in whole warp slices).
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
 }
@@ -257,6 +266,7 @@ static inline int afqmc_smem_optin(afqmc_ctx* c, const void* fn, size_t smem) {
 int afqmc_i_green(afqmc_ctx* c, const double2* phi, int nw, double2* theta, double2* logdet,
                   int* info, cudaStream_t st);
 int afqmc_i_force_bias(afqmc_ctx* c, const double2* theta, int nw, double2* vbias, cudaStream_t st);
+int afqmc_i_max_abs_imag(afqmc_ctx* c, const double2* p, size_t n, double* out_host, cudaStream_t st);   // synchronises st
 int afqmc_i_pack_force_bias_operand(afqmc_ctx* c, cudaStream_t st);
 void afqmc_i_fb_frag_layout(const afqmc_ctx* c, int nw, int* NT, int* nwg, int* KSf);   // layout of ws_thetaF for nw walkers
 // switches the Green -> force-bias fragment fusion on / off for a composition (both spin channels)

@@ -82,6 +82,28 @@ __global__ void pack_Lx_kernel(Dims d, const double2* __restrict__ Lh, double* _
     }
 }
 
+// max |Im z| over an array (ordered-int atomic on the bit pattern of a non-negative double: exact, order independent)
+__global__ void max_abs_imag_kernel(const double2* __restrict__ p, size_t n, unsigned long long* __restrict__ out) {
+    double mx = 0.0;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) mx = fmax(mx, fabs(p[i].y));
+    atomicMax(out, (unsigned long long)__double_as_longlong(mx));
+}
+
+int afqmc_i_max_abs_imag(afqmc_ctx* c, const double2* p, size_t n, double* out_host, cudaStream_t st) {
+    unsigned long long* d = nullptr;
+    AFQMC_CUDA_TRY(cudaMalloc((void**)&d, sizeof(unsigned long long)));
+    cudaMemsetAsync(d, 0, sizeof(unsigned long long), st);
+    max_abs_imag_kernel<<<148 * 8, 256, 0, st>>>(p, n, d);
+    c->launches++;
+    unsigned long long h = 0;
+    cudaError_t e = cudaMemcpyAsync(&h, d, sizeof(h), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return AFQMC_CUDA_ERROR; }
+    memcpy(out_host, &h, 8);
+    return AFQMC_OK;
+}
+
 __global__ void half_rot_h_kernel(Dims d, const double2* __restrict__ h1, const double2* __restrict__ psi_t,
                                   double2* __restrict__ ht) {
     // ht[k][a][q] = sum_p conj(A_k[p][a]) h_k[p][q]     (first line of Eq. 49)
@@ -158,6 +180,7 @@ static int create_channel(afqmc_ctx** out, const afqmc_dims* dims, int n_chan, i
     c->max_walkers = dims->max_walkers;
     c->prec32 = dims->precision == 1 ? 1 : 0;
     c->opt_exchange_3m = 1;
+    c->opt_real = 1;
     c->opt_exchange_regb = 1;
     c->spin_factor = open_shell ? 1.0 : 2.0;
     c->is_child = child ? 1 : 0;
@@ -274,6 +297,12 @@ static int create_channel(afqmc_ctx** out, const afqmc_dims* dims, int n_chan, i
         half_rot_L_kernel<<<grid(nLh), T, 0, st>>>(d, (const double2*)L, c->psi_t, c->Lh, nLh);     // the half rotation, once
         c->launches += 2;
         if (cudaGetLastError() != cudaSuccess) rc = AFQMC_CUDA_ERROR;
+        // real orbitals?  (exact zeros: a real L half-rotated with a real trial has no imaginary part at all)
+        if (rc == AFQMC_OK) {
+            double im = 1.0;
+            rc = afqmc_i_max_abs_imag(c, c->Lh, nLh, &im, st);
+            c->real_lh = (rc == AFQMC_OK && im == 0.0) ? 1 : 0;
+        }
         // force-bias operand Lf3 (single-precision storage when precision = 1)
         if (rc == AFQMC_OK) rc = afqmc_i_pack_force_bias_operand(c, st);
         if (rc == AFQMC_OK) rc = afqmc_i_pack_exchange_operand(c, st);
@@ -357,6 +386,9 @@ AFQMC_API double afqmc_exchange_flops(const afqmc_ctx* c, int nw) {
     if (c->opt_exchange_prec != 0 && c->LxT) return (c->opt_exchange_prec == 1 ? 3.0 : 1.0) * per * (double)c->nunits * (double)nw;      // TF32 kernel: the 4M real embedding
     // (counted as pure 3M; the <= 2 tail elements of a row with m mod 4 in {1,2} are really done as 4M: not counted)
     if (c->opt_exchange_3m) per = 12.0 * d.n * d.n * d.m * d.nchol + 6.0 * d.n * d.n * d.nchol + 8.0 * d.n * d.n * d.nchol;
+    // real orbitals (two real products per complex product, one addition per T element), default prefetch depth only
+    if (c->opt_exchange_3m && c->real_lh && c->opt_real && c->opt_exchange_depth != 2)
+        per = 8.0 * d.n * d.n * d.m * d.nchol + 2.0 * d.n * d.n * d.nchol + 8.0 * d.n * d.n * d.nchol;
     return per * (double)c->nunits * (double)nw;
 }
 
@@ -426,6 +458,10 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
     if (strcmp(name, "taylor_groups") == 0) {
         if (value < 0 || value > 64) return AFQMC_INVALID_ARGUMENT;
         c->opt_taylor_groups = value;
+        return AFQMC_OK;
+    }
+    if (strcmp(name, "real_orbitals") == 0) {      // 0 = run the complex kernels even if the inputs were detected as real
+        c->opt_real = value ? 1 : 0;
         return AFQMC_OK;
     }
     if (strcmp(name, "taylor_subbatch") == 0) {

@@ -287,7 +287,8 @@ __device__ __forceinline__ X3Lane x3_lane(int lane) {
 // End of a task (gamma-quad): combine the three products (Re = P0 - P2, Im = P0 + P1), hand m-tile 1-KEEP to the partner warp
 // of the pair through `xw`, take the partner's tile KEEP from `xr` (this is also the (a,b) transpose) and contract it with the
 // own tile KEEP; the accumulators are cleared.
-template <int NP, int KEEP>
+// (REAL: the third product does not exist, Re = P0)
+template <int NP, int KEEP, bool REAL = false>
 __device__ __forceinline__ void x3_finish_task(double (&acc)[3][2][NP][2], double2* __restrict__ xw, const double2* __restrict__ xr,
                                                int bar_id, const X3Lane& L, double (&er)[NP], double (&ei)[NP]) {
     constexpr int GIVE = 1 - KEEP;
@@ -295,7 +296,7 @@ __device__ __forceinline__ void x3_finish_task(double (&acc)[3][2][NP][2], doubl
     for (int j = 0; j < NP; ++j)
 #pragma unroll
         for (int e = 0; e < 2; ++e)
-            xw[j * 64 + L.sw[e]] = make_double2(acc[0][GIVE][j][e] - acc[2][GIVE][j][e], acc[0][GIVE][j][e] + acc[1][GIVE][j][e]);
+            xw[j * 64 + L.sw[e]] = make_double2(REAL ? acc[0][GIVE][j][e] : acc[0][GIVE][j][e] - acc[2][GIVE][j][e], acc[0][GIVE][j][e] + acc[1][GIVE][j][e]);
     // the two warps of the pair (an immediate id where possible: a register id makes ptxas reserve all 16 named barriers)
     if (bar_id == 1) asm volatile("bar.sync 1, 64;" ::: "memory");
     else asm volatile("bar.sync 2, 64;" ::: "memory");        // (at most two warp pairs per CTA)
@@ -303,7 +304,7 @@ __device__ __forceinline__ void x3_finish_task(double (&acc)[3][2][NP][2], doubl
     for (int j = 0; j < NP; ++j)
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-            const double tr = acc[0][KEEP][j][e] - acc[2][KEEP][j][e], ti = acc[0][KEEP][j][e] + acc[1][KEEP][j][e];
+            const double tr = REAL ? acc[0][KEEP][j][e] : acc[0][KEEP][j][e] - acc[2][KEEP][j][e], ti = acc[0][KEEP][j][e] + acc[1][KEEP][j][e];
             const double2 p = xr[j * 64 + L.sr[e]];
             er[j] = fma(tr, p.x, er[j]); er[j] = fma(-ti, p.y, er[j]);
             ei[j] = fma(tr, p.y, ei[j]); ei[j] = fma(ti, p.x, ei[j]);
@@ -415,7 +416,10 @@ __device__ __forceinline__ void x3_reduce_store(double* red /* shared, [warp][NW
 //                      Gamma-point supercell shape); a unit then contributes NAG^2 * nchunk partial sums.
 // DA = k-steps of register prefetch of the Lxc stream (L2 resident); the B fragments (shared memory) run one k-step ahead.
 // ---------------------------------------------------------------------------------------------------------------------
-template <int NP, int NPAIR, int DA, int MINB, bool GRIDPAIRS>
+// REAL = the half-rotated tensor is real (real orbitals, detected in a0): T = Lh theta needs two real products per complex one
+// (P0 = Ar Br = Re, P1 = Ar (Bi - Br), Im = P0 + P1): the third product and the addition Ar + Ai are skipped; the operand keeps
+// its complex fragment layout (its imaginary parts are zeros).
+template <int NP, int NPAIR, int DA, int MINB, bool GRIDPAIRS, bool REAL>
 __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
     Dims d, X3Geom g, int nchunk, int nw, const int* __restrict__ units, const int* __restrict__ kminus,
     const int* __restrict__ kplus, const int* __restrict__ kneg, const double* __restrict__ Lxc,
@@ -484,7 +488,8 @@ __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
                 }
             }
         };
-        load_b(0, 0); load_b(1, 0); load_b(2, 0);
+        load_b(0, 0); load_b(1, 0);
+        if (!REAL) load_b(2, 0);
         double acc[3][2][NP][2];
 #pragma unroll
         for (int p = 0; p < 3; ++p)
@@ -499,7 +504,7 @@ __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
             const double2 x0 = fa[q][0], x1 = fa[q][1];
             const int nxt = (cs + 1 == g.KSPT) ? 0 : 3 * (cs + 1);      // first micro-step of the next k-step (wraps at the task end)
             if (cs < g.KSF) {
-                const double s0 = x0.x + x0.y, s1 = x1.x + x1.y;        // Ar + Ai
+                const double s0 = REAL ? x0.x : x0.x + x0.y, s1 = REAL ? x1.x : x1.x + x1.y;        // Ar + Ai
 #pragma unroll
                 for (int j = 0; j < NP; ++j) {
                     dmma884(acc[0][0][j][0], acc[0][0][j][1], s0, fb[0][j]);
@@ -512,12 +517,14 @@ __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
                     dmma884(acc[1][1][j][0], acc[1][1][j][1], x1.x, fb[1][j]);
                 }
                 load_b(1, nxt);
+                if (!REAL) {
 #pragma unroll
-                for (int j = 0; j < NP; ++j) {
-                    dmma884(acc[2][0][j][0], acc[2][0][j][1], x0.y, fb[2][j]);
-                    dmma884(acc[2][1][j][0], acc[2][1][j][1], x1.y, fb[2][j]);
+                    for (int j = 0; j < NP; ++j) {
+                        dmma884(acc[2][0][j][0], acc[2][0][j][1], x0.y, fb[2][j]);
+                        dmma884(acc[2][1][j][0], acc[2][1][j][1], x1.y, fb[2][j]);
+                    }
+                    load_b(2, nxt);
                 }
-                load_b(2, nxt);
             } else {                                                     // tail k-step: x0 = (tile 0, tile 1) real-embedded
 #pragma unroll
                 for (int j = 0; j < NP; ++j) {
@@ -531,7 +538,7 @@ __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
                     dmma884(acc[1][1][j][0], acc[1][1][j][1], x0.y, fb[1][j]);
                 }
                 load_b(1, nxt);
-                load_b(2, nxt);
+                if (!REAL) load_b(2, nxt);
             }
             // refill this ring slot with the k-step DA ahead (may run past the warp's last task: loaded, never used)
             fa[q][0] = __ldg(pa); fa[q][1] = __ldg(pa + 1);
@@ -541,8 +548,8 @@ __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
                 // two hand-over buffers: the partner may still read one while the next task is written into the other
                 double2* xw = xbuf + (((pair * 2 + h) * NBUF + buf) * NP) * 64;
                 const double2* xr = xbuf + (((pair * 2 + (h ^ 1)) * NBUF + buf) * NP) * 64;
-                if (h == 0) x3_finish_task<NP, 0>(acc, xw, xr, pair + 1, L, er, ei);
-                else x3_finish_task<NP, 1>(acc, xw, xr, pair + 1, L, er, ei);
+                if (h == 0) x3_finish_task<NP, 0, REAL>(acc, xw, xr, pair + 1, L, er, ei);
+                else x3_finish_task<NP, 1, REAL>(acc, xw, xr, pair + 1, L, er, ei);
                 buf ^= 1;
             }
         };
@@ -732,6 +739,7 @@ __global__ void __launch_bounds__(64) __maxnreg__(MAXREG) exchange3m_reg_kernel(
             }
             const bool last_pair = ab == npairs - 1;
             if (last_pair) {          // the raw buffer of the previous item is free: fetch the next item's block into it
+                fence_proxy_async_smem();       // (its reads before the bulk copies that refill it, common.cuh)
                 __syncwarp();
                 if (has_next) issue_theta(nx, bufsel ^ 1);
             }
@@ -872,12 +880,12 @@ size_t x3_smem_bytes(const X3Geom& g, int NGS, int NPAIR) {
     return bs + xb;
 }
 
-template <int NP, int NPAIR, int DA, int MINB, bool GRIDPAIRS>
-int launch_x3(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+template <int NP, int NPAIR, int DA, int MINB, bool GRIDPAIRS, bool REAL>
+int launch_x3_r(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     const Dims& d = c->d;
     const X3Geom g = x3_geom(d.m);
     const size_t smem = x3_smem_bytes<NP>(g, GRIDPAIRS ? 1 : d.NAG, NPAIR);
-    auto kern = exchange3m_kernel<NP, NPAIR, DA, MINB, GRIDPAIRS>;
+    auto kern = exchange3m_kernel<NP, NPAIR, DA, MINB, GRIDPAIRS, REAL>;
     if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
     afqmc_prefer_smem(c, (const void*)kern);
     const int nwg = (nw + 2 * NP - 1) / (2 * NP), npairs = d.NAG * d.NAG;
@@ -899,11 +907,25 @@ int launch_x3(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     return AFQMC_OK;
 }
 
+// real orbitals: the two-product variant (instantiated for the default prefetch depth only)
+template <int NP, int NPAIR, int DA, int MINB, bool GRIDPAIRS>
+int launch_x3(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
+    if (DA == 3 && c->real_lh && c->opt_real) return launch_x3_r<NP, NPAIR, DA, MINB, GRIDPAIRS, (DA == 3)>(c, theta, nw, st);
+    return launch_x3_r<NP, NPAIR, DA, MINB, GRIDPAIRS, false>(c, theta, nw, st);
+}
+
 // n-tiles per warp: 2 (four walkers per CTA) unless there are at most two walkers; 4 (eight walkers per CTA) on request
 template <int NPAIR, int DA, bool GRIDPAIRS>
 int launch_x3_np(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     int np = c->opt_exchange_np;
-    if (np == 0) np = nw <= 2 ? 1 : 2;
+    if (np == 0) {
+        np = nw <= 2 ? 1 : 2;
+        // long rows (the Gamma-point supercell shape, m = 208): the staged theta blocks of four walkers leave room for one CTA
+        // per SM only (160 KB); two walkers per CTA keep two CTAs resident (G1: exchange 1.95 -> 1.59 ms)
+        const X3Geom g = x3_geom(c->d.m);
+        const int ngs = GRIDPAIRS ? 1 : c->d.NAG;
+        if (np == 2 && 2 * x3_smem_bytes<2>(g, ngs, NPAIR) > (size_t)c->smem_sm && 2 * x3_smem_bytes<1>(g, ngs, NPAIR) <= (size_t)c->smem_sm) np = 1;
+    }
     // resident CTAs asked of the compiler: the register budget per thread is 65536 / (MINB * 64 * NPAIR)
     if (np == 1) return launch_x3<1, NPAIR, DA, (NPAIR == 1 ? 8 : 4), GRIDPAIRS>(c, theta, nw, st);
     if (np == 4) return launch_x3<4, NPAIR, (DA > 2 ? 2 : DA), (NPAIR == 1 ? 5 : 2), GRIDPAIRS>(c, theta, nw, st);
@@ -991,7 +1013,8 @@ int afqmc_i_exchange3m(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t 
     c->ex_parts = 1;
     const X3Geom g = x3_geom(c->d.m);
     // m <= 28: the theta block of a warp lives in registers (unless the tuning options ask for the generic kernel)
-    if (c->opt_exchange_regb && x3_prefers_reg(c->d) && c->opt_exchange_np <= 1 && c->opt_exchange_wpc != 4) {
+    // (real orbitals: the generic kernel has the two-product variant)
+    if (c->opt_exchange_regb && x3_prefers_reg(c->d) && c->opt_exchange_np <= 1 && c->opt_exchange_wpc != 4 && !(c->real_lh && c->opt_real)) {
         int rc = ensure_operand(c, true, st);
         if (rc != AFQMC_OK) return rc;
         rc = AFQMC_UNSUPPORTED;

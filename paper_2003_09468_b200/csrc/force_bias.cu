@@ -28,6 +28,7 @@
 //    the shape (the previous kernel lost 19 % to wave quantisation and 11 % to a padded m-tile pair at C3).  A piece that
 //    crosses a tile boundary produces two partial tiles; partial tiles are combined in a fixed order by
 //    force_bias3_reduce_kernel (no atomics: bitwise reproducible).
+#include <type_traits>
 #include "common.cuh"
 
 namespace {
@@ -105,7 +106,9 @@ __global__ void __launch_bounds__(256) theta_frag_kernel(Dims d, int NT, int nwg
 }
 
 // AT = double2: FP64 storage of the operand; float2: single-precision storage (precision = 1), widened at use
-template <int MT, int NT, typename AT>
+// REAL: the operand is real (real orbitals: imaginary parts exactly zero, detected in a0): Re = Ar Br, Im = Ar Bi, two real
+// products per complex product and no addition at all
+template <int MT, int NT, typename AT, bool REAL>
 __global__ void __launch_bounds__(32 * FB_WARPS, AFQMC_FB_MINB) force_bias3_kernel(
     Dims d, FbPlan p, int nw, const AT* __restrict__ Lf3, const double2* __restrict__ thetaF, double2* __restrict__ part) {
     extern __shared__ __align__(128) unsigned char fb_smem[];
@@ -177,9 +180,10 @@ __global__ void __launch_bounds__(32 * FB_WARPS, AFQMC_FB_MINB) force_bias3_kern
 #pragma unroll 1
         for (int c = 0; c < FB_S - 1 && c < nch; ++c) issue(c);
 
-        double acc[3][MT][NT][2];
+        constexpr int NV = REAL ? 2 : 3;
+        double acc[NV][MT][NT][2];
 #pragma unroll
-        for (int v = 0; v < 3; ++v)
+        for (int v = 0; v < NV; ++v)
 #pragma unroll
             for (int i = 0; i < MT; ++i)
 #pragma unroll
@@ -204,29 +208,24 @@ __global__ void __launch_bounds__(32 * FB_WARPS, AFQMC_FB_MINB) force_bias3_kern
                     for (int j = 0; j < NT; ++j) {
                         const double2 v = rb[(kin * NT + j) * 32];
                         b[0][j] = v.x; b[1][j] = v.y;
+                        b[2][j] = REAL ? 0.0 : v.x + v.y;
                     }
 #pragma unroll
                     for (int i = 0; i < MT; ++i) {
                         const AT f = ra[(kin * MT + i) * 32];
-                        a[0][i] = (double)f.x; a[1][i] = (double)f.y;
-                    }
-#pragma unroll
+                        a[0][i] = (double)f.x; a[1][i] = REAL ? a[0][i] : (double)f.y;
 #ifdef FB_NOADD      // timing experiment only (wrong results): what the kernel would cost without the additions
-                    for (int j = 0; j < NT; ++j) b[2][j] = b[1][j];
-#pragma unroll
-                    for (int i = 0; i < MT; ++i) a[2][i] = a[1][i];
+                        a[2][i] = a[1][i];
 #else
-                    for (int j = 0; j < NT; ++j) b[2][j] = b[0][j] + b[1][j];
-#pragma unroll
-                    for (int i = 0; i < MT; ++i) a[2][i] = a[0][i] + a[1][i];
+                        a[2][i] = REAL ? 0.0 : a[0][i] + a[1][i];
 #endif
+                    }
 #pragma unroll
                     for (int i = 0; i < MT; ++i)
 #pragma unroll
                         for (int j = 0; j < NT; ++j) {
-                            dmma884(acc[0][i][j][0], acc[0][i][j][1], a[0][i], b[0][j]);
-                            dmma884(acc[1][i][j][0], acc[1][i][j][1], a[1][i], b[1][j]);
-                            dmma884(acc[2][i][j][0], acc[2][i][j][1], a[2][i], b[2][j]);
+#pragma unroll
+                            for (int v = 0; v < NV; ++v) dmma884(acc[v][i][j][0], acc[v][i][j][1], a[v][i], b[v][j]);
                         }
                 };
                 const int rel0 = c * FB_KPC;
@@ -239,6 +238,7 @@ __global__ void __launch_bounds__(32 * FB_WARPS, AFQMC_FB_MINB) force_bias3_kern
                         if (rel0 + kin < nks) kstep(kin);
                 }
             }
+            fence_proxy_async_smem();                       // this chunk's reads before the refill of its stages (common.cuh)
             __syncwarp();                                   // every lane has read the chunk
             if (lane == 0) mbar_arrive(&emptyA[st]);
         }
@@ -260,7 +260,8 @@ __global__ void __launch_bounds__(32 * FB_WARPS, AFQMC_FB_MINB) force_bias3_kern
                     const int w = w0 + 8 * j + 2 * kk + e;
                     if (w < nw)
                         dst[((size_t)w * d.Nk + Q) * d.nchol + gam] =
-                            make_double2(acc[0][i][j][e] - acc[1][i][j][e], acc[2][i][j][e] - acc[0][i][j][e] - acc[1][i][j][e]);
+                            REAL ? make_double2(acc[0][i][j][e], acc[1][i][j][e])
+                                 : make_double2(acc[0][i][j][e] - acc[1][i][j][e], acc[NV - 1][i][j][e] - acc[0][i][j][e] - acc[1][i][j][e]);
                 }
         }
     }
@@ -321,7 +322,7 @@ void fb_set_pieces(FbPlan& p, long long resident_ctas) {
     p.U = (int)U;
 }
 
-template <int MT, int NT, typename AT>
+template <int MT, int NT, typename AT, bool REAL>
 int launch_fb3(afqmc_ctx* c, FbPlan p, const AT* Lf3, const double2* theta, int nw, double2* vbias, cudaStream_t st) {
     const Dims& d = c->d;
     // theta -> B fragments (workspace sized for max_walkers in a0), unless Green's epilogue has just written them
@@ -335,7 +336,7 @@ int launch_fb3(afqmc_ctx* c, FbPlan p, const AT* Lf3, const double2* theta, int 
     const int nunit = FB_WARPS / p.WG;
     const size_t smem = (size_t)nunit * FB_S * FB_KPC * MT * 32 * sizeof(AT) + (size_t)FB_WARPS * FB_S * FB_KPC * NT * 32 * sizeof(double2) +
                         3 * FB_WARPS * FB_S * sizeof(uint64_t);
-    auto kern = force_bias3_kernel<MT, NT, AT>;
+    auto kern = force_bias3_kernel<MT, NT, AT, REAL>;
     if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
     afqmc_prefer_smem(c, (const void*)kern);
     // resident CTAs (per shared-memory size: it depends on the walker count through WG); remembered in the context
@@ -360,7 +361,11 @@ int launch_fb3(afqmc_ctx* c, FbPlan p, const AT* Lf3, const double2* theta, int 
 
 template <int MT, typename AT>
 int launch_fb3_nt(afqmc_ctx* c, const FbPlan& p, const AT* Lf3, const double2* theta, int nw, double2* vbias, cudaStream_t st) {
-    return p.NT == 1 ? launch_fb3<MT, 1, AT>(c, p, Lf3, theta, nw, vbias, st) : launch_fb3<MT, 2, AT>(c, p, Lf3, theta, nw, vbias, st);
+    // real orbitals: the two-product kernel (FP64 storage only)
+    if (std::is_same<AT, double2>::value && c->real_lh && c->opt_real)
+        return p.NT == 1 ? launch_fb3<MT, 1, double2, true>(c, p, reinterpret_cast<const double2*>(Lf3), theta, nw, vbias, st)
+                         : launch_fb3<MT, 2, double2, true>(c, p, reinterpret_cast<const double2*>(Lf3), theta, nw, vbias, st);
+    return p.NT == 1 ? launch_fb3<MT, 1, AT, false>(c, p, Lf3, theta, nw, vbias, st) : launch_fb3<MT, 2, AT, false>(c, p, Lf3, theta, nw, vbias, st);
 }
 
 template <typename AT>
@@ -415,8 +420,9 @@ void afqmc_i_fb_frag_layout(const afqmc_ctx* c, int nw, int* NT, int* nwg, int* 
 AFQMC_API double afqmc_force_bias_flops(const afqmc_ctx* c, int nw) {
     if (!c) return 0.0;
     const Dims& d = c->d;
-    double f = 6.0 * d.Nk * d.Nk * d.n * (double)d.m * d.nchol * nw;
-    if (c->dn) f += 6.0 * d.Nk * d.Nk * c->dn->d.n * (double)d.m * d.nchol * nw;
+    const double per = (c->real_lh && c->opt_real && !c->prec32) ? 4.0 : 6.0;      // real orbitals: two real products
+    double f = per * d.Nk * d.Nk * d.n * (double)d.m * d.nchol * nw;
+    if (c->dn) f += per * d.Nk * d.Nk * c->dn->d.n * (double)d.m * d.nchol * nw;
     return f;
 }
 

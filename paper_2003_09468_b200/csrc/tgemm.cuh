@@ -190,6 +190,7 @@ __device__ __forceinline__ void body(const Args& p, const double* stage0, uint64
                 }
             }
         }
+        fence_proxy_async_smem();       // the stage's reads before its refill by the bulk copy (see common.cuh)
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[st]);
     }

@@ -39,12 +39,12 @@ constexpr int V3_STAGES = 3;
 constexpr int V3_DMAX = 6;
 constexpr int V3_WARPS = 4;
 
-// max |L[-Q][k-Q][g][r][p] - conj(L[Q][k][g][p][r])| and max |L| (both as ordered-int atomics on the bit patterns of
+// max |L[-Q][k-Q][g][r][p] - conj(L[Q][k][g][p][r])|, max |L| and max |Im L| (as ordered-int atomics on the bit patterns of
 // non-negative doubles, which is exact and order independent)
 __global__ void pair_symmetry_kernel(Dims d, const int* __restrict__ kminus, const int* __restrict__ kneg,
                                      const double2* __restrict__ L, unsigned long long* __restrict__ out) {
     const size_t total = (size_t)d.Nk * d.Nk * d.nchol * d.m * d.m;
-    double dev = 0.0, mx = 0.0;
+    double dev = 0.0, mx = 0.0, im = 0.0;
     for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
         size_t t = idx;
         const int r = (int)(t % d.m); t /= d.m;
@@ -57,9 +57,11 @@ __global__ void pair_symmetry_kernel(Dims d, const int* __restrict__ kminus, con
         const double2 b = L[((((size_t)mQ * d.Nk + kq) * d.nchol + g) * d.m + r) * d.m + p];
         dev = fmax(dev, fmax(fabs(a.x - b.x), fabs(a.y + b.y)));
         mx = fmax(mx, fmax(fabs(a.x), fabs(a.y)));
+        im = fmax(im, fabs(a.y));
     }
     atomicMax(out, (unsigned long long)__double_as_longlong(dev));
     atomicMax(out + 1, (unsigned long long)__double_as_longlong(mx));
+    atomicMax(out + 2, (unsigned long long)__double_as_longlong(im));
 }
 
 __device__ __forceinline__ void store_frag(double2* p, double2 z) { *p = z; }
@@ -94,11 +96,11 @@ int afqmc_i_vhs_setup(afqmc_ctx* c, const double2* L, const std::vector<int>& km
     const Dims& d = c->d;
     const int Nk = d.Nk;
     unsigned long long* dchk = nullptr;
-    AFQMC_CUDA_TRY(cudaMalloc((void**)&dchk, 2 * sizeof(unsigned long long)));
-    cudaMemsetAsync(dchk, 0, 2 * sizeof(unsigned long long), st);
+    AFQMC_CUDA_TRY(cudaMalloc((void**)&dchk, 3 * sizeof(unsigned long long)));
+    cudaMemsetAsync(dchk, 0, 3 * sizeof(unsigned long long), st);
     pair_symmetry_kernel<<<148 * 16, 256, 0, st>>>(d, c->kminus, c->kneg, L, dchk);
     c->launches++;
-    unsigned long long h[2] = {0, 0};
+    unsigned long long h[3] = {0, 0, 0};
     cudaError_t e = cudaMemcpyAsync(h, dchk, sizeof(h), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     cudaFree(dchk);
@@ -107,6 +109,9 @@ int afqmc_i_vhs_setup(afqmc_ctx* c, const double2* L, const std::vector<int>& km
     memcpy(&dev, &h[0], 8);
     memcpy(&mx, &h[1], 8);
     c->vhs_paired = (dev <= 1e-13 * mx) ? 1 : 0;
+    double im;
+    memcpy(&im, &h[2], 8);
+    c->real_l = im == 0.0 ? 1 : 0;                 // real orbitals: two real products per complex product in vhs3_kernel
 
     // units: (Q, k, kind, 0); kind 0 = single block (no pairing, or a self-partner block), 1 = block + partner
     std::vector<int> vu;
@@ -193,7 +198,9 @@ __global__ void fields3_kernel(Dims d, int nw, int NT, int nwg, int KS4p, const 
 // sets of its row slice (2 NT n-tiles), so the A stream is read once without relying on L1 and every fragment feeds
 // twice as many DMMAs; otherwise warps 0-1 take the block and warps 2-3 its partner.  D = k-steps of A register prefetch
 // (deeper for small batches, where the kernel is bound by the HBM stream of L and needs more bytes in flight).
-template <int NT, bool MERGED, int D, typename AT>
+// REAL: L is real (real orbitals, detected in a0): Re = Ar Br, Im = Ar Br + Ar (Bi - Br): the third product and the addition
+// Ar + Ai are skipped (the operand keeps its complex fragment layout).
+template <int NT, bool MERGED, int D, typename AT, bool REAL>
 __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
     Dims d, int KS4, int KS4p, int nw, int nwg, int nsg, const int* __restrict__ vunits, const int* __restrict__ kminus,
     const AT* __restrict__ Lv3, const double* __restrict__ Bx3, double2* __restrict__ vhs) {
@@ -260,10 +267,10 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
     int ksg = 0;        // global k-step
     auto kstep = [&](const double* bs, const int qa) {
         const double x0 = (double)fa0[qa].x, y0 = (double)fa0[qa].y, x1 = (double)fa1[qa].x, y1 = (double)fa1[qa].y;
-        const double a0[3] = {x0 + y0, x0, y0};
-        const double a1[3] = {x1 + y1, x1, y1};
+        const double a0[3] = {REAL ? x0 : x0 + y0, x0, y0};
+        const double a1[3] = {REAL ? x1 : x1 + y1, x1, y1};
 #pragma unroll
-        for (int p = 0; p < 3; ++p) {
+        for (int p = 0; p < (REAL ? 2 : 3); ++p) {
             double bf[NTT];
 #pragma unroll
             for (int j = 0; j < NTT; ++j) bf[j] = bs[(j / NT) * SET_DOUBLES + (p * NT + j % NT) * 32];
@@ -293,6 +300,7 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
                 }
             }
         }
+        fence_proxy_async_smem();       // the stage's reads before its refill by the bulk copy (see common.cuh)
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[s]);
     }
@@ -324,7 +332,7 @@ __global__ void __launch_bounds__(32 * V3_WARPS, 3) vhs3_kernel(
     }
 }
 
-template <int NT, bool MERGED, int D, typename AT>
+template <int NT, bool MERGED, int D, typename AT, bool REAL>
 int launch_vhs3_t(afqmc_ctx* c, const AT* Lv3, int nw, int KS4, int KS4p, double2* vhs, cudaStream_t st) {
     const Dims& d = c->d;
     const int nwg = (nw + 8 * NT - 1) / (8 * NT);
@@ -333,8 +341,8 @@ int launch_vhs3_t(afqmc_ctx* c, const AT* Lv3, int nw, int KS4, int KS4p, double
     const size_t smem = (size_t)V3_STAGES * 2 * D * 3 * NT * 32 * sizeof(double) + 2 * V3_STAGES * sizeof(uint64_t);
     const long long gx = (long long)c->nvunits * nsg;
     if (gx > 0x7fffffffLL || nwg > 65535) return AFQMC_UNSUPPORTED;
-    if (int rc = afqmc_smem_optin(c, (const void*)vhs3_kernel<NT, MERGED, D, AT>, smem)) return rc;
-    vhs3_kernel<NT, MERGED, D, AT><<<dim3((unsigned)gx, nwg), 32 * V3_WARPS, smem, st>>>(d, KS4, KS4p, nw, nwg, nsg, c->vunits, c->kminus, Lv3,
+    if (int rc = afqmc_smem_optin(c, (const void*)vhs3_kernel<NT, MERGED, D, AT, REAL>, smem)) return rc;
+    vhs3_kernel<NT, MERGED, D, AT, REAL><<<dim3((unsigned)gx, nwg), 32 * V3_WARPS, smem, st>>>(d, KS4, KS4p, nw, nwg, nsg, c->vunits, c->kminus, Lv3,
                                                                             reinterpret_cast<const double*>(c->ws_xi), vhs);
     AFQMC_LAUNCH_CHECK(c);
     return AFQMC_OK;
@@ -342,8 +350,9 @@ int launch_vhs3_t(afqmc_ctx* c, const AT* Lv3, int nw, int KS4, int KS4p, double
 
 template <int NT, bool MERGED, int D>
 int launch_vhs3(afqmc_ctx* c, int nw, int KS4, int KS4p, double2* vhs, cudaStream_t st) {
-    if (c->Lv3f) return launch_vhs3_t<NT, MERGED, D, float2>(c, c->Lv3f, nw, KS4, KS4p, vhs, st);      // single-precision storage
-    return launch_vhs3_t<NT, MERGED, D, double2>(c, c->Lv3, nw, KS4, KS4p, vhs, st);
+    if (c->Lv3f) return launch_vhs3_t<NT, MERGED, D, float2, false>(c, c->Lv3f, nw, KS4, KS4p, vhs, st);      // single-precision storage
+    if (c->real_l && c->opt_real) return launch_vhs3_t<NT, MERGED, D, double2, true>(c, c->Lv3, nw, KS4, KS4p, vhs, st);   // real orbitals
+    return launch_vhs3_t<NT, MERGED, D, double2, false>(c, c->Lv3, nw, KS4, KS4p, vhs, st);
 }
 
 }  // namespace

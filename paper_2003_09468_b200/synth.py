@@ -89,6 +89,11 @@ def _cn(rng, shape, var):
     return z.view(np.complex128)[..., 0]
 
 
+def _rn(rng, shape, var):
+    """Real draws of the same variance, stored as complex128 with zero imaginary parts (real orbitals)."""
+    return (rng.standard_normal(shape) * np.sqrt(var)).astype(np.complex128)
+
+
 @dataclass
 class Problem:
     cfg: Config
@@ -100,9 +105,12 @@ class Problem:
     extra: dict = field(default_factory=dict)
 
 
-def make_hamiltonian(cfg: Config, rng):
+def make_hamiltonian(cfg: Config, rng, real_orbitals=False):
+    """`real_orbitals`: h1, psi_t and L are drawn REAL (same shapes, variances and symmetry structure): the dense Gamma-point
+    supercell representation with real orbitals of PAPER.md:260, :276-284.  Walkers stay complex."""
     nk, m, n, nchol = cfg.nk, cfg.m, cfg.n, cfg.nchol
     kminus, neg = kpoint_tables(cfg.mesh)
+    _cn = globals()["_rn"] if real_orbitals else globals()["_cn"]
     g = _cn(rng, (nk, m, m), 1.0)
     h1 = 0.5 * (g + np.conj(np.swapaxes(g, -1, -2)))
     psi_t = np.empty((nk, m, n), dtype=np.complex128)
@@ -138,14 +146,14 @@ def make_walkers(cfg: Config, psi_t, rng, nw=None, noise=0.1):
     return phi
 
 
-def make_problem(cfg: Config, nw=None, l_scale=1.0) -> Problem:
+def make_problem(cfg: Config, nw=None, l_scale=1.0, real_orbitals=False) -> Problem:
     """`l_scale` multiplies L after the draw (same random stream).  1.0 is BASELINE.json's recipe, whose
     sqrt(dtau)*vHS has norm 2-16 (R9): every kernel is tested there, but in a hybrid AFQMC block such
     steps rotate the overlap phase by more than pi/2 and the phaseless projection sets most weights to 0.  The
     block tests and the block bench therefore also use a 'physically scaled' L (l_scale ~ 0.05-0.1, steps of
     norm < 1), as SURVEY.md P9 suggests; shapes and structure are unchanged."""
     rng = np.random.default_rng(cfg.seed)
-    h1, psi_t, L = make_hamiltonian(cfg, rng)
+    h1, psi_t, L = make_hamiltonian(cfg, rng, real_orbitals)
     if l_scale != 1.0:
         L *= l_scale
     phi = make_walkers(cfg, psi_t, rng, nw)

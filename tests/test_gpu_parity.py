@@ -35,10 +35,10 @@ def _to_dev(a):
 
 
 class Case:
-    def __init__(self, cfg, nw=None):
+    def __init__(self, cfg, nw=None, real_orbitals=False):
         from paper_2003_09468_b200 import binding
         self.cfg = cfg
-        self.pb = synth.make_problem(cfg, nw)
+        self.pb = synth.make_problem(cfg, nw, real_orbitals=real_orbitals)
         self.nw = self.pb.phi.shape[0]
         self.ctx = binding.from_problem(self.pb)
         self.Lh, self.ht = orc.half_rotate(self.pb.L, self.pb.psi_t, self.pb.h1)
