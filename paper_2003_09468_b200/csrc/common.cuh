@@ -49,6 +49,7 @@ struct afqmc_ctx {
     double2* Lh;    // half-rotated Cholesky tensor, natural layout [Q][k][a][gamma][r]: computed ONCE in a0; every packed
                     // operand below is a pure re-layout of it
     double* Lxc;    // exchange, generic 3M kernel (exchange3m.cu; default for m > 28): complex fragments [Q][k][ag][gq][ks][lane][4]
+    double* Lxr;    // exchange, generic kernel with a REAL operand (real orbitals): real parts only, [Q][k][ag][gq][ks][lane][2]; first use
     double* Lx3t;   // exchange, register-B 3M kernel (default for m <= 28): the three A variants [Q][k][ag][gq][ml][lane][2]
                     // (only the default one of Lxc / Lx3t is packed in a0; the other on first use)
     double* Lx;     // exchange, 4M kernel (energy.cu): [Q][k][ag][gq][s][lane][2]; packed on first use (option exchange_3m = 0)

@@ -145,7 +145,7 @@ AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     if (!c) return;
     if (c->dn) { afqmc_destroy(c->dn); c->dn = nullptr; }
     if (c->is_child) c->b1 = nullptr;        // owned by the spin-up context
-    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lh, c->Lxc, c->Lx3t, c->Lx, c->LxT, c->Lf, c->Lff, c->Lv3, c->Lv3f, c->vunits,
+    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lh, c->Lxc, c->Lxr, c->Lx3t, c->Lx, c->LxT, c->Lf, c->Lff, c->Lv3, c->Lv3f, c->vunits,
                     c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T, c->ws_Tx,
                     c->ws_expart, c->ws_fbpart, c->ws_thetaF, c->ws_vbtot, c->ws_ld_chan, c->ws_info_chan, c->ws_ldr_chan, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
                     c->ws_f32, c->b1, c->ws_b1tmp, c->ws_gram, c->ws_rinv, c->ws_logdet2, c->ws_ldr, c->ws_info2};
@@ -386,9 +386,9 @@ AFQMC_API double afqmc_exchange_flops(const afqmc_ctx* c, int nw) {
     if (c->opt_exchange_prec != 0 && c->LxT) return (c->opt_exchange_prec == 1 ? 3.0 : 1.0) * per * (double)c->nunits * (double)nw;      // TF32 kernel: the 4M real embedding
     // (counted as pure 3M; the <= 2 tail elements of a row with m mod 4 in {1,2} are really done as 4M: not counted)
     if (c->opt_exchange_3m) per = 12.0 * d.n * d.n * d.m * d.nchol + 6.0 * d.n * d.n * d.nchol + 8.0 * d.n * d.n * d.nchol;
-    // real orbitals (two real products per complex product, one addition per T element), default prefetch depth only
-    if (c->opt_exchange_3m && c->real_lh && c->opt_real && c->opt_exchange_depth != 2)
-        per = 8.0 * d.n * d.n * d.m * d.nchol + 2.0 * d.n * d.n * d.nchol + 8.0 * d.n * d.n * d.nchol;
+    // real orbitals (two real products per complex product, no additions before the contraction), default prefetch depth only
+    if (c->opt_exchange_3m && c->real_lh && c->opt_real && c->opt_exchange_depth != 2)      // (the generic kernel's default depths)
+        per = 8.0 * d.n * d.n * d.m * d.nchol + 8.0 * d.n * d.n * d.nchol;
     return per * (double)c->nunits * (double)nw;
 }
 

@@ -40,7 +40,7 @@
 
 namespace {
 
-struct X3Geom { int KSF, TAIL, KSPT, MSPT; };
+struct X3Geom { int KSF, TAIL, KSPT, MSPT, PV; };      // PV = real products (micro-steps) per full k-step: 3, or 2 for a real operand
 // k-steps of a task: KSF full ones (3 micro-steps = products each) + TAIL (0/1) real-embedded one (2 micro-steps)
 __host__ __device__ inline X3Geom x3_geom(int m) {
     X3Geom g;
@@ -49,6 +49,13 @@ __host__ __device__ inline X3Geom x3_geom(int m) {
     g.KSF = g.TAIL ? m / 4 : (m + 3) / 4;
     g.KSPT = g.KSF + g.TAIL;
     g.MSPT = 3 * g.KSF + 2 * g.TAIL;
+    g.PV = 3;
+    return g;
+}
+// real operand (real orbitals): K = r in k-steps of 4, no tail trick, two products per k-step (Ar Br, Ar Bi)
+__host__ __device__ inline X3Geom x3_geom_real(int m) {
+    X3Geom g;
+    g.TAIL = 0; g.KSF = (m + 3) / 4; g.KSPT = g.KSF; g.MSPT = 2 * g.KSF; g.PV = 2;
     return g;
 }
 
@@ -99,6 +106,40 @@ static int pack_lxc(afqmc_ctx* c, cudaStream_t st) {
     size_t nb = (total_in + 255) / 256;
     if (nb > 148 * 64) nb = 148 * 64;
     pack_Lxc_kernel<<<(unsigned)nb, 256, 0, st>>>(d, g, c->Lh, c->Lxc, total_in, afqmc_i_lxc_doubles(d));
+    AFQMC_LAUNCH_CHECK(c);
+    return AFQMC_OK;
+}
+
+// Lxr (real orbitals, generic kernel): the REAL parts only,  Lxr[Q][k][ag][gq][ks < ceil(m/4)][lane][2] = (tile 0, tile 1) at
+// r = 4 ks + kk: half the bytes of Lxc, one LDG.128 per k-step and lane
+namespace {
+__global__ void pack_Lxr_kernel(Dims d, int KSF, const double2* __restrict__ Lh, double* __restrict__ Lxr, size_t total_in, size_t total_out) {
+    for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total_in; idx += (size_t)gridDim.x * blockDim.x) {
+        size_t t = idx;
+        const int i = (int)(t & 1); t >>= 1;
+        const int lane = (int)(t & 31); t >>= 5;
+        const int ks = (int)(t % KSF); t /= KSF;
+        const int gq = (int)(t % d.GQ); t /= d.GQ;
+        const int ag = (int)(t % d.NAG); t /= d.NAG;
+        const int k = (int)(t % d.Nk);
+        const int Q = (int)(t / d.Nk);
+        const int row = lane >> 2, r = 4 * ks + (lane & 3);
+        const int gam = 4 * gq + 2 * i + (row >> 2), a = 4 * ag + (row & 3);
+        Lxr[idx] = (a < d.n && gam < d.nchol && r < d.m) ? Lh[((((size_t)Q * d.Nk + k) * d.n + a) * d.nchol + gam) * d.m + r].x : 0.0;
+    }
+    for (size_t idx = total_in + blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total_out; idx += (size_t)gridDim.x * blockDim.x) Lxr[idx] = 0.0;
+}
+}  // namespace
+
+static int ensure_lxr(afqmc_ctx* c, cudaStream_t st) {
+    if (c->Lxr) return AFQMC_OK;
+    const Dims& d = c->d;
+    const X3Geom g = x3_geom_real(d.m);
+    const size_t total_in = (size_t)d.Nk * d.Nk * d.NAG * d.GQ * g.KSF * 64, total_out = total_in + AFQMC_LX_PAD;
+    if (cudaMalloc((void**)&c->Lxr, total_out * sizeof(double)) != cudaSuccess) { (void)cudaGetLastError(); c->Lxr = nullptr; return AFQMC_OUT_OF_MEMORY; }
+    size_t nb = (total_in + 255) / 256;
+    if (nb > 148 * 64) nb = 148 * 64;
+    pack_Lxr_kernel<<<(unsigned)nb, 256, 0, st>>>(d, g.KSF, c->Lh, c->Lxr, total_in, total_out);
     AFQMC_LAUNCH_CHECK(c);
     return AFQMC_OK;
 }
@@ -249,7 +290,11 @@ __device__ __forceinline__ void x3_stage_theta(double* __restrict__ Bs, const Di
             v = __ldg(theta + ((size_t)w * d.N + rowblk * d.n + orb) * d.M + (size_t)colblk * d.m + r);
         const int col = w_lo * 4 + b;
         double* base = Bs + which * bs_half + gs * bs_grp + (j / W) * (32 * W) + (j % W);    // + ms * bs_step + lane * W
-        if (r_hi < g.KSF) {
+        if (g.PV == 2) {                        // real operand: the two B sides are Re and Im themselves
+            double* dst = base + 2 * r_hi * bs_step + ((col << 2) | r_lo) * W;
+            dst[0] = v.x;
+            dst[bs_step] = v.y;
+        } else if (r_hi < g.KSF) {
             double* dst = base + 3 * r_hi * bs_step + ((col << 2) | r_lo) * W;
             dst[0] = v.x;                       // Br
             dst[bs_step] = v.y - v.x;           // Bi - Br
@@ -287,7 +332,7 @@ __device__ __forceinline__ X3Lane x3_lane(int lane) {
 // End of a task (gamma-quad): combine the three products (Re = P0 - P2, Im = P0 + P1), hand m-tile 1-KEEP to the partner warp
 // of the pair through `xw`, take the partner's tile KEEP from `xr` (this is also the (a,b) transpose) and contract it with the
 // own tile KEEP; the accumulators are cleared.
-// (REAL: the third product does not exist, Re = P0)
+// (REAL: two products, Re = P0 = Ar Br, Im = P1 = Ar Bi)
 template <int NP, int KEEP, bool REAL = false>
 __device__ __forceinline__ void x3_finish_task(double (&acc)[3][2][NP][2], double2* __restrict__ xw, const double2* __restrict__ xr,
                                                int bar_id, const X3Lane& L, double (&er)[NP], double (&ei)[NP]) {
@@ -296,7 +341,8 @@ __device__ __forceinline__ void x3_finish_task(double (&acc)[3][2][NP][2], doubl
     for (int j = 0; j < NP; ++j)
 #pragma unroll
         for (int e = 0; e < 2; ++e)
-            xw[j * 64 + L.sw[e]] = make_double2(REAL ? acc[0][GIVE][j][e] : acc[0][GIVE][j][e] - acc[2][GIVE][j][e], acc[0][GIVE][j][e] + acc[1][GIVE][j][e]);
+            xw[j * 64 + L.sw[e]] = REAL ? make_double2(acc[0][GIVE][j][e], acc[1][GIVE][j][e])
+                                        : make_double2(acc[0][GIVE][j][e] - acc[2][GIVE][j][e], acc[0][GIVE][j][e] + acc[1][GIVE][j][e]);
     // the two warps of the pair (an immediate id where possible: a register id makes ptxas reserve all 16 named barriers)
     if (bar_id == 1) asm volatile("bar.sync 1, 64;" ::: "memory");
     else asm volatile("bar.sync 2, 64;" ::: "memory");        // (at most two warp pairs per CTA)
@@ -304,7 +350,8 @@ __device__ __forceinline__ void x3_finish_task(double (&acc)[3][2][NP][2], doubl
     for (int j = 0; j < NP; ++j)
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-            const double tr = REAL ? acc[0][KEEP][j][e] : acc[0][KEEP][j][e] - acc[2][KEEP][j][e], ti = acc[0][KEEP][j][e] + acc[1][KEEP][j][e];
+            const double tr = REAL ? acc[0][KEEP][j][e] : acc[0][KEEP][j][e] - acc[2][KEEP][j][e];
+            const double ti = REAL ? acc[1][KEEP][j][e] : acc[0][KEEP][j][e] + acc[1][KEEP][j][e];
             const double2 p = xr[j * 64 + L.sr[e]];
             er[j] = fma(tr, p.x, er[j]); er[j] = fma(-ti, p.y, er[j]);
             ei[j] = fma(tr, p.y, ei[j]); ei[j] = fma(ti, p.x, ei[j]);
@@ -417,8 +464,8 @@ __device__ __forceinline__ void x3_reduce_store(double* red /* shared, [warp][NW
 // DA = k-steps of register prefetch of the Lxc stream (L2 resident); the B fragments (shared memory) run one k-step ahead.
 // ---------------------------------------------------------------------------------------------------------------------
 // REAL = the half-rotated tensor is real (real orbitals, detected in a0): T = Lh theta needs two real products per complex one
-// (P0 = Ar Br = Re, P1 = Ar (Bi - Br), Im = P0 + P1): the third product and the addition Ar + Ai are skipped; the operand keeps
-// its complex fragment layout (its imaginary parts are zeros).
+// (Re = Ar Br, Im = Ar Bi, no addition anywhere); the operand is the real-parts-only layout Lxr (half the bytes, one LDG.128 per
+// k-step), the geometry x3_geom_real (no tail trick) and the staged theta blocks hold two B sides per k-step (2/3 of the bytes).
 template <int NP, int NPAIR, int DA, int MINB, bool GRIDPAIRS, bool REAL>
 __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
     Dims d, X3Geom g, int nchunk, int nw, const int* __restrict__ units, const int* __restrict__ kminus,
@@ -444,8 +491,10 @@ __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
     const int t_end = q_begin + (int)((long long)(pair + 1) * (q_end - q_begin) / NPAIR);
     const int total = (t_end - t_begin) * g.KSPT;                 // k-steps of this warp per (ag,bg) pair
     const size_t blk = h == 0 ? (size_t)t.Q * d.Nk + t.k : (size_t)t.mQ * d.Nk + t.k2;
-    auto stream_ptr = [&](int grp) {            // 2 double2 per lane and k-step; k-step stride 64 double2
-        return reinterpret_cast<const double2*>(Lxc + (((blk * NAG + grp) * GQ + t_begin) * (size_t)g.KSPT) * 128) + lane * 2;
+    constexpr int AST = REAL ? 32 : 64;         // k-step stride of a lane's A stream in double2
+    auto stream_ptr = [&](int grp) {            // 2 double2 per lane and k-step (REAL: one = the real parts of both tiles)
+        return REAL ? reinterpret_cast<const double2*>(Lxc + (((blk * NAG + grp) * GQ + t_begin) * (size_t)g.KSPT) * 64) + lane
+                    : reinterpret_cast<const double2*>(Lxc + (((blk * NAG + grp) * GQ + t_begin) * (size_t)g.KSPT) * 128) + lane * 2;
     };
     double2 fa[DA][2];
     const double2* pa = stream_ptr(h == 0 ? t.ab0 / NAG : t.ab0 % NAG);
@@ -453,7 +502,7 @@ __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
 #pragma unroll
     for (int q = 0; q < DA; ++q) {
         fa[q][0] = fa[q][1] = make_double2(0.0, 0.0);
-        if (total > 0) { fa[q][0] = __ldg(pa + q * 64); fa[q][1] = __ldg(pa + q * 64 + 1); }
+        if (total > 0) { fa[q][0] = __ldg(pa + q * AST); if (!REAL) fa[q][1] = __ldg(pa + q * AST + 1); }
     }
     x3_stage_theta<NP, 64 * NPAIR, GRIDPAIRS>(Bs, d, g, t, nw, theta);
     __syncthreads();   // B fragments staged
@@ -470,9 +519,9 @@ __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
             pa = stream_ptr(h == 0 ? ag : bg);
 #pragma unroll
             for (int q = 0; q < DA; ++q)
-                if (total > 0) { fa[q][0] = __ldg(pa + q * 64); fa[q][1] = __ldg(pa + q * 64 + 1); }
+                if (total > 0) { fa[q][0] = __ldg(pa + q * AST); if (!REAL) fa[q][1] = __ldg(pa + q * AST + 1); }
         }
-        pa += DA * 64;
+        pa += DA * AST;
         // T1 needs theta rows bg of k2 (which 0), T2 theta rows ag of k (which 1)
         const double* pb = Bs + h * bs_half + (GRIDPAIRS ? 0 : (h == 0 ? bg : ag)) * bs_grp + lane * W;
         double fb[3][NP];
@@ -488,6 +537,7 @@ __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
                 }
             }
         };
+        constexpr int PV = REAL ? 2 : 3;
         load_b(0, 0); load_b(1, 0);
         if (!REAL) load_b(2, 0);
         double acc[3][2][NP][2];
@@ -501,9 +551,9 @@ __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
         int cs = 0;   // k-step of the compute state inside its task
         auto kstep = [&](auto Q_) {
             constexpr int q = decltype(Q_)::value;
-            const double2 x0 = fa[q][0], x1 = fa[q][1];
-            const int nxt = (cs + 1 == g.KSPT) ? 0 : 3 * (cs + 1);      // first micro-step of the next k-step (wraps at the task end)
-            if (cs < g.KSF) {
+            const double2 x0 = REAL ? make_double2(fa[q][0].x, 0.0) : fa[q][0], x1 = REAL ? make_double2(fa[q][0].y, 0.0) : fa[q][1];
+            const int nxt = (cs + 1 == g.KSPT) ? 0 : PV * (cs + 1);     // first micro-step of the next k-step (wraps at the task end)
+            if (REAL || cs < g.KSF) {
                 const double s0 = REAL ? x0.x : x0.x + x0.y, s1 = REAL ? x1.x : x1.x + x1.y;        // Ar + Ai
 #pragma unroll
                 for (int j = 0; j < NP; ++j) {
@@ -541,8 +591,9 @@ __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
                 if (!REAL) load_b(2, nxt);
             }
             // refill this ring slot with the k-step DA ahead (may run past the warp's last task: loaded, never used)
-            fa[q][0] = __ldg(pa); fa[q][1] = __ldg(pa + 1);
-            pa += 64;
+            fa[q][0] = __ldg(pa);
+            if (!REAL) fa[q][1] = __ldg(pa + 1);
+            pa += AST;
             if (++cs == g.KSPT) {
                 cs = 0;
                 // two hand-over buffers: the partner may still read one while the next task is written into the other
@@ -559,10 +610,14 @@ __global__ void __launch_bounds__(64 * NPAIR, MINB) exchange3m_kernel(
             if (DA > 1) kstep(std::integral_constant<int, 1 % DA>());
             if (DA > 2) kstep(std::integral_constant<int, 2 % DA>());
             if (DA > 3) kstep(std::integral_constant<int, 3 % DA>());
+            if (DA > 4) kstep(std::integral_constant<int, 4 % DA>());
+            if (DA > 5) kstep(std::integral_constant<int, 5 % DA>());
         }
         if (nfull + 0 < total) kstep(std::integral_constant<int, 0>());
         if (DA > 2 && nfull + 1 < total) kstep(std::integral_constant<int, 1 % DA>());
         if (DA > 3 && nfull + 2 < total) kstep(std::integral_constant<int, 2 % DA>());
+        if (DA > 4 && nfull + 3 < total) kstep(std::integral_constant<int, 3 % DA>());
+        if (DA > 5 && nfull + 4 < total) kstep(std::integral_constant<int, 4 % DA>());
     }
     x3_reduce_store<NP, NWARP, GRIDPAIRS>(x3_smem, er, ei, t, d, nchunk, nw, partial);
 }
@@ -883,7 +938,7 @@ size_t x3_smem_bytes(const X3Geom& g, int NGS, int NPAIR) {
 template <int NP, int NPAIR, int DA, int MINB, bool GRIDPAIRS, bool REAL>
 int launch_x3_r(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     const Dims& d = c->d;
-    const X3Geom g = x3_geom(d.m);
+    const X3Geom g = REAL ? x3_geom_real(d.m) : x3_geom(d.m);
     const size_t smem = x3_smem_bytes<NP>(g, GRIDPAIRS ? 1 : d.NAG, NPAIR);
     auto kern = exchange3m_kernel<NP, NPAIR, DA, MINB, GRIDPAIRS, REAL>;
     if (int rc = afqmc_smem_optin(c, (const void*)kern, smem)) return rc;
@@ -901,7 +956,7 @@ int launch_x3_r(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
         nblocks *= (long long)npairs * nchunk;
     }
     if (nblocks > 0x7fffffffLL) return AFQMC_UNSUPPORTED;
-    kern<<<(unsigned)nblocks, 64 * NPAIR, smem, st>>>(d, g, nchunk, nw, c->units, c->kminus, c->kplus, c->kneg, c->Lxc, theta, c->ws_expart);
+    kern<<<(unsigned)nblocks, 64 * NPAIR, smem, st>>>(d, g, nchunk, nw, c->units, c->kminus, c->kplus, c->kneg, REAL ? c->Lxr : c->Lxc, theta, c->ws_expart);
     AFQMC_LAUNCH_CHECK(c);
     c->ex_parts = GRIDPAIRS ? npairs * nchunk : 1;
     return AFQMC_OK;
@@ -910,7 +965,7 @@ int launch_x3_r(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
 // real orbitals: the two-product variant (instantiated for the default prefetch depth only)
 template <int NP, int NPAIR, int DA, int MINB, bool GRIDPAIRS>
 int launch_x3(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
-    if (DA == 3 && c->real_lh && c->opt_real) return launch_x3_r<NP, NPAIR, DA, MINB, GRIDPAIRS, (DA == 3)>(c, theta, nw, st);
+    if ((DA == 3 || DA == 6) && c->real_lh && c->opt_real) return launch_x3_r<NP, NPAIR, DA, MINB, GRIDPAIRS, (DA == 3 || DA == 6)>(c, theta, nw, st);
     return launch_x3_r<NP, NPAIR, DA, MINB, GRIDPAIRS, false>(c, theta, nw, st);
 }
 
@@ -922,12 +977,14 @@ int launch_x3_np(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
         np = nw <= 2 ? 1 : 2;
         // long rows (the Gamma-point supercell shape, m = 208): the staged theta blocks of four walkers leave room for one CTA
         // per SM only (160 KB); two walkers per CTA keep two CTAs resident (G1: exchange 1.95 -> 1.59 ms)
-        const X3Geom g = x3_geom(c->d.m);
+        const X3Geom g = (c->real_lh && c->opt_real) ? x3_geom_real(c->d.m) : x3_geom(c->d.m);
         const int ngs = GRIDPAIRS ? 1 : c->d.NAG;
         if (np == 2 && 2 * x3_smem_bytes<2>(g, ngs, NPAIR) > (size_t)c->smem_sm && 2 * x3_smem_bytes<1>(g, ngs, NPAIR) <= (size_t)c->smem_sm) np = 1;
     }
     // resident CTAs asked of the compiler: the register budget per thread is 65536 / (MINB * 64 * NPAIR)
-    if (np == 1) return launch_x3<1, NPAIR, DA, (NPAIR == 1 ? 8 : 4), GRIDPAIRS>(c, theta, nw, st);
+    // two walkers per CTA: a k-step is only six DMMAs, so the A stream runs six k-steps ahead in registers (three left 43 % of
+    // the warp samples of the Gamma-point shape G1 waiting for A fragments: DMMA pipe 41 % busy)
+    if (np == 1) return launch_x3<1, NPAIR, (DA == 3 ? 6 : DA), (NPAIR == 1 ? 8 : 4), GRIDPAIRS>(c, theta, nw, st);
     if (np == 4) return launch_x3<4, NPAIR, (DA > 2 ? 2 : DA), (NPAIR == 1 ? 5 : 2), GRIDPAIRS>(c, theta, nw, st);
     return launch_x3<2, NPAIR, DA, (NPAIR == 1 ? 7 : 3), GRIDPAIRS>(c, theta, nw, st);
 }
@@ -938,7 +995,7 @@ int launch_x3_cfg(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st) {
     // two-walker-pair tile); when the staged theta blocks are larger than that (m = 52 at C4: 45 KB per CTA) two pairs share one
     // staging, which keeps 12 warps resident instead of 10 and halves the theta traffic (C4: 25.5 -> 20.6 ms; round 1's kernel:
     // 23.0 ms).  Option "exchange_warps" = 4 forces two pairs, = 2 one.
-    const size_t smem1 = x3_smem_bytes<2>(x3_geom(c->d.m), GRIDPAIRS ? 1 : c->d.NAG, 1);
+    const size_t smem1 = x3_smem_bytes<2>((c->real_lh && c->opt_real) ? x3_geom_real(c->d.m) : x3_geom(c->d.m), GRIDPAIRS ? 1 : c->d.NAG, 1);
     const bool two_pairs = GRIDPAIRS || c->opt_exchange_wpc == 4 || (c->opt_exchange_wpc == 0 && smem1 * 7 > (size_t)c->smem_sm);
     const int da = c->opt_exchange_depth == 2 ? 2 : 3;                     // option "exchange_depth": k-steps of A prefetch
     if (two_pairs) return da == 2 ? launch_x3_np<2, 2, GRIDPAIRS>(c, theta, nw, st) : launch_x3_np<2, 3, GRIDPAIRS>(c, theta, nw, st);
@@ -1027,7 +1084,7 @@ int afqmc_i_exchange3m(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t 
         }
         if (rc != AFQMC_UNSUPPORTED) return rc;      // else: the raw theta blocks of all orbitals exceed shared memory
     }
-    int rc = ensure_operand(c, false, st);
+    int rc = (c->real_lh && c->opt_real && c->opt_exchange_depth != 2) ? ensure_lxr(c, st) : ensure_operand(c, false, st);
     if (rc != AFQMC_OK) return rc;
     rc = launch_x3_cfg<false>(c, theta, nw, st);
     if (rc == AFQMC_UNSUPPORTED && c->d.NAG > 1 && c->ex_parts_max > 1) rc = launch_x3_cfg<true>(c, theta, nw, st);

@@ -53,3 +53,19 @@ def test_product_path_does_not_import_the_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle", src, flags=re.M), f
                 assert "afqmc_oracle" not in src and "oracle/" not in src and '#include "oracle' not in src, f
+
+
+def test_synth_real_orbital_inputs_are_real_and_keep_the_pair_identity():
+    """synth.make_problem(real_orbitals=True): h1, psi_t, L real (zero imaginary parts), the (Q,-Q) identity holds with
+    transposes, walkers stay complex; the default stream is unchanged by the option's existence."""
+    import numpy as np
+    from paper_2003_09468_b200 import synth
+    cfg = synth.tiny_config(mesh=(2, 1, 1), m=4, n=2, nchol=3, nw=2, seed=9)
+    pb = synth.make_problem(cfg, real_orbitals=True)
+    assert np.all(pb.L.imag == 0) and np.all(pb.psi_t.imag == 0) and np.all(pb.h1.imag == 0)
+    assert np.abs(pb.phi.imag).max() > 0
+    kminus, neg = synth.kpoint_tables(cfg.mesh)
+    for Q in range(cfg.nk):
+        for k in range(cfg.nk):
+            assert np.array_equal(pb.L[neg[Q], kminus[k, Q]], np.swapaxes(pb.L[Q, k], -1, -2))
+    assert np.array_equal(synth.make_problem(cfg).L, synth.make_problem(cfg, real_orbitals=False).L)
