@@ -33,6 +33,9 @@ struct FuncAttr { const void* fn; int smem; int occ; int carveout; int occ_smem;
 
 // The context.  All pointers are device memory owned by the context.
 struct afqmc_ctx {
+    alignas(64) unsigned char tmap_lxu[128];   // CUtensorMaps of LxU and ws_thetaU (exchange_tc.cu); valid iff tmap_lxu_ok
+    alignas(64) unsigned char tmap_thu[128];
+    int tmap_lxu_ok;
     Dims d;
     int max_walkers;
     // static tables
@@ -53,6 +56,7 @@ struct afqmc_ctx {
     double* Lx3t;   // exchange, register-B 3M kernel (default for m <= 28): the three A variants [Q][k][ag][gq][ml][lane][2]
                     // (only the default one of Lxc / Lx3t is packed in a0; the other on first use)
     double* Lx;     // exchange, 4M kernel (energy.cu): [Q][k][ag][gq][s][lane][2]; packed on first use (option exchange_3m = 0)
+    float* LxU;     // exchange, tcgen05 TF32 kernel (exchange_tc.cu): shared-memory tile images [Q][k][tile][hi/lo][128 x KP]; first use
     float* LxT;     // exchange, TF32 fragments [Q][k][gq][ks][lane][4] (exchange_tf32.cu; n <= 4 only); packed on first use
     double* Lf;     // force-bias operand Lf3[Q][m-tile][k-step][lane] complex fragments over the flattened K = (k,a,r) (force_bias.cu)
     float* Lff;     // precision = 1: the same in single precision (Lf is then NULL)
@@ -71,6 +75,7 @@ struct afqmc_ctx {
     double2* ws_T;      // [2][nw][M][N] Taylor ping-pong (legacy GEMM path)
     double* ws_Tx;      // [2][nw][expanded] Taylor ping-pong in the expanded B-fragment layout of tgemm.cuh
     double2* ws_expart; // [nunits][nw]  exchange partial sums
+    float* ws_thetaU;   // [Nk][Nk][walker groups of 8][hi/lo][64 x KP] theta blocks as B images of the tcgen05 exchange kernel
     double2* ws_thetaF; // [Nk(Q)][walker groups][k-steps][NT][32] theta as B fragments of the force-bias GEMM (force_bias.cu)
     double2* ws_fbpart; // [AFQMC_FB_MAXKC][nw][Nk][nchol] force-bias partial tiles (stream-K pieces)
     double* ws_x;       // [nw][Nk][nchol] (host-entry staging)
@@ -109,6 +114,7 @@ struct afqmc_ctx {
     long long launches;
     int opt_exchange_depth; // 0/3 = three k-steps of fragment prefetch, 2 = two
     int opt_exchange_minb;  // tuning aid: 1 = ask for more resident CTAs per SM
+    int opt_exchange_tc;    // 1 (default) = the mixed-precision exchange runs on tcgen05.mma / TMEM (exchange_tc.cu), 0 = mma.sync kernel
     int opt_exchange_prec;  // 0 (default) = FP64 exchange kernels; mixed precision on the TF32 tensor cores (n <= 4): 1 = 3xTF32 split, 2 = 1xTF32
     int opt_exchange_3m;    // 1 (default) = 3M exchange kernel when n <= 4, 0 = the 4M kernel of energy.cu
     int opt_exchange_wpc;   // 0 = automatic, else warps per CTA of the exchange kernel (4,5,6,8)
@@ -289,6 +295,7 @@ int afqmc_i_exchange3m(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t 
 int afqmc_i_pack_exchange_operand(afqmc_ctx* c, cudaStream_t st);                       // a0: Lh -> Lx3t (m <= 28) or Lxc
 size_t afqmc_i_lxc_doubles(const Dims& d);
 int afqmc_i_exchange3m_parts_max(const afqmc_ctx* c);
+int afqmc_i_exchange_tc(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st);    // tcgen05 version; AFQMC_UNSUPPORTED if n > 4 / too large
 int afqmc_i_exchange_tf32(afqmc_ctx* c, const double2* theta, int nw, cudaStream_t st);  // AFQMC_UNSUPPORTED if n > 4
 int afqmc_i_ensure_lx(afqmc_ctx* c, cudaStream_t st);     // packs the 4M operand Lx from Lh on first use
 int afqmc_i_ensure_lxt(afqmc_ctx* c, cudaStream_t st);    // packs the TF32 operand LxT from Lh on first use (n <= 4)

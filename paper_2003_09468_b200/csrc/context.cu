@@ -145,9 +145,9 @@ AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     if (!c) return;
     if (c->dn) { afqmc_destroy(c->dn); c->dn = nullptr; }
     if (c->is_child) c->b1 = nullptr;        // owned by the spin-up context
-    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lh, c->Lxc, c->Lxr, c->Lx3t, c->Lx, c->LxT, c->Lf, c->Lff, c->Lv3, c->Lv3f, c->vunits,
+    void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lh, c->Lxc, c->Lxr, c->Lx3t, c->Lx, c->LxT, c->LxU, c->Lf, c->Lff, c->Lv3, c->Lv3f, c->vunits,
                     c->ws_O, c->ws_oinvT, c->ws_theta, c->ws_vbias, c->ws_xi, c->ws_vhs, c->ws_T, c->ws_Tx,
-                    c->ws_expart, c->ws_fbpart, c->ws_thetaF, c->ws_vbtot, c->ws_ld_chan, c->ws_info_chan, c->ws_ldr_chan, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
+                    c->ws_expart, c->ws_fbpart, c->ws_thetaF, c->ws_thetaU, c->ws_vbtot, c->ws_ld_chan, c->ws_info_chan, c->ws_ldr_chan, c->ws_x, c->ws_phi, c->ws_energy, c->ws_logdet, c->ws_info,
                     c->ws_f32, c->b1, c->ws_b1tmp, c->ws_gram, c->ws_rinv, c->ws_logdet2, c->ws_ldr, c->ws_info2};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -181,6 +181,7 @@ static int create_channel(afqmc_ctx** out, const afqmc_dims* dims, int n_chan, i
     c->prec32 = dims->precision == 1 ? 1 : 0;
     c->opt_exchange_3m = 1;
     c->opt_real = 1;
+    c->opt_exchange_tc = 1;
     c->opt_exchange_regb = 1;
     c->spin_factor = open_shell ? 1.0 : 2.0;
     c->is_child = child ? 1 : 0;
@@ -312,12 +313,7 @@ static int create_channel(afqmc_ctx** out, const afqmc_dims* dims, int n_chan, i
     if (cudaStreamSynchronize(st) != cudaSuccess && rc == AFQMC_OK) rc = AFQMC_CUDA_ERROR;
     cudaFree(h1w); cudaFree(Lw); cudaFree(psiw);
     if (rc != AFQMC_OK) { (void)cudaGetLastError(); afqmc_destroy(c); return rc; }
-    if (c->prec32 && d.NAG == 1) {      // complex64 boundary: 3xTF32 exchange by default
-        rc = afqmc_i_ensure_lxt(c, st);
-        if (rc == AFQMC_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = AFQMC_CUDA_ERROR;
-        if (rc != AFQMC_OK) { (void)cudaGetLastError(); afqmc_destroy(c); return rc; }
-        c->opt_exchange_prec = 1;
-    }
+    if (c->prec32 && d.NAG == 1) c->opt_exchange_prec = 1;      // complex64 boundary: 3xTF32 exchange by default (operands packed on first use)
     *out = c;
     return AFQMC_OK;
 }
@@ -383,7 +379,7 @@ AFQMC_API double afqmc_exchange_flops(const afqmc_ctx* c, int nw) {
     // 4M kernel: 8 real flops per complex multiply-add = 2 * 8*n*n*m*nchol.  3M kernel (exchange3m.cu): 6 real
     // flops per complex multiply-add = 2 * 6*n*n*m*nchol, plus 3 additions per element of both T tensors.
     double per = 16.0 * d.n * d.n * d.m * d.nchol + 8.0 * d.n * d.n * d.nchol;
-    if (c->opt_exchange_prec != 0 && c->LxT) return (c->opt_exchange_prec == 1 ? 3.0 : 1.0) * per * (double)c->nunits * (double)nw;      // TF32 kernel: the 4M real embedding
+    if (c->opt_exchange_prec != 0 && c->d.NAG == 1) return (c->opt_exchange_prec == 1 ? 3.0 : 1.0) * per * (double)c->nunits * (double)nw;      // TF32 kernel: the 4M real embedding
     // (counted as pure 3M; the <= 2 tail elements of a row with m mod 4 in {1,2} are really done as 4M: not counted)
     if (c->opt_exchange_3m) per = 12.0 * d.n * d.n * d.m * d.nchol + 6.0 * d.n * d.n * d.nchol + 8.0 * d.n * d.n * d.nchol;
     // real orbitals (two real products per complex product, no additions before the contraction), default prefetch depth only
@@ -405,12 +401,12 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
     }
     if (strcmp(name, "exchange_precision") == 0) {
         if (value < 0 || value > 2) return AFQMC_INVALID_ARGUMENT;
-        if (value != 0) {                                           // n > 4: AFQMC_UNSUPPORTED
-            int rc = afqmc_i_ensure_lxt(c, 0);
-            if (rc == AFQMC_OK && cudaStreamSynchronize(0) != cudaSuccess) rc = AFQMC_CUDA_ERROR;
-            if (rc != AFQMC_OK) return rc;
-        }
+        if (value != 0 && c->d.NAG != 1) return AFQMC_UNSUPPORTED;   // the mixed-precision kernels take n <= 4 (operands: first use)
         c->opt_exchange_prec = value;
+        return AFQMC_OK;
+    }
+    if (strcmp(name, "exchange_tc") == 0) {        // 0 = the mma.sync TF32 kernel instead of the tcgen05 one
+        c->opt_exchange_tc = value ? 1 : 0;
         return AFQMC_OK;
     }
     if (strcmp(name, "exchange_3m") == 0) {

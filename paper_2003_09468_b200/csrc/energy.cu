@@ -337,8 +337,12 @@ static int channel_energy_parts(afqmc_ctx* c, afqmc_ctx* timers, const double2* 
     if (rc != AFQMC_OK) return rc;
     if (timers) afqmc_mark(timers, 6, st);
     c->ex_parts = 1;
-    rc = c->opt_exchange_prec != 0 ? afqmc_i_exchange_tf32(c, theta, nw, st)
-         : c->opt_exchange_3m    ? afqmc_i_exchange3m(c, theta, nw, st) : AFQMC_UNSUPPORTED;
+    if (c->opt_exchange_prec != 0) {       // mixed precision: tcgen05 kernel, else (or if it cannot take the shape) the mma.sync one
+        rc = c->opt_exchange_tc ? afqmc_i_exchange_tc(c, theta, nw, st) : AFQMC_UNSUPPORTED;
+        if (rc == AFQMC_UNSUPPORTED && (rc = afqmc_i_ensure_lxt(c, st)) == AFQMC_OK) rc = afqmc_i_exchange_tf32(c, theta, nw, st);
+    } else {
+        rc = c->opt_exchange_3m ? afqmc_i_exchange3m(c, theta, nw, st) : AFQMC_UNSUPPORTED;
+    }
     if (rc == AFQMC_UNSUPPORTED) {          // the 4M kernel was asked for (or the TF32 option with n > 4)
         if ((rc = afqmc_i_ensure_lx(c, st)) != AFQMC_OK) return rc;
         if (nw >= 3) rc = launch_exchange<4>(c, theta, nw, st);

@@ -612,25 +612,31 @@ def test_exchange_3m_and_4m_kernels_against_the_oracle(kw):
                                 dict(mesh=(1, 2, 2), m=9, n=1, nchol=5, nw=2), dict(mesh=(3, 1, 1), m=26, n=4, nchol=18, nw=7)],
                          ids=["n4", "n3_odd", "n1_two_walkers", "m26_seven_walkers"])
 def test_mixed_precision_exchange_against_the_oracle(kw):
-    """Option exchange_precision (exchange_tf32.cu), the analogue of the paper's single-precision mode and
-    of the north_star's optional complex64 path (tolerance 1e-4): mode 1 (3xTF32 split) is held to 1e-5 relative on EX
-    against the FP64 oracle, mode 2 (operands rounded once to TF32) only to 1e-2 (it is documented as outside the 1e-4
-    tolerance).  E1 and EC must not change at all."""
+    """Option exchange_precision, the analogue of the paper's single-precision mode and of the north_star's
+    optional complex64 path (tolerance 1e-4), on BOTH kernels: the tcgen05 / TMEM one (exchange_tc.cu, default) and the
+    mma.sync one (exchange_tf32.cu, option exchange_tc = 0).  Mode 1 (3xTF32 split) is held to 1e-5 relative on EX against
+    the FP64 oracle, mode 2 (operands rounded once to TF32) only to 1e-2 (it is documented as outside the 1e-4 tolerance).
+    E1 and EC must not change at all."""
     case = Case(synth.tiny_config(seed=19, **kw))
     try:
         theta_d, _, _ = case.ctx.green(_to_dev(case.pb.phi))
         theta = theta_d.cpu().numpy()
         e_o = np.array([orc.local_energy(case.cfg.mesh, case.Lh, case.ht, theta[w]) for w in range(case.nw)])
         e64 = case.ctx.local_energy(theta_d).cpu().numpy()
-        for mode, tol in ((1, 1e-5), (2, 1e-2)):
-            case.ctx.set_option("exchange_precision", mode)
-            try:
-                e = case.ctx.local_energy(theta_d).cpu().numpy()
-            finally:
-                case.ctx.set_option("exchange_precision", 0)
-            assert np.array_equal(e[:, :2], e64[:, :2])
-            for w in range(case.nw):
-                assert abs(e[w, 2] - e_o[w, 2]) / abs(e_o[w, 2]) < tol, (mode, w, e[w, 2], e_o[w, 2])
+        for tc in (1, 0):
+            for mode, tol in ((1, 1e-5), (2, 1e-2)):
+                case.ctx.set_option("exchange_tc", tc)
+                case.ctx.set_option("exchange_precision", mode)
+                try:
+                    e = case.ctx.local_energy(theta_d).cpu().numpy()
+                    e_again = case.ctx.local_energy(theta_d).cpu().numpy()
+                finally:
+                    case.ctx.set_option("exchange_precision", 0)
+                    case.ctx.set_option("exchange_tc", 1)
+                assert np.array_equal(e, e_again)                      # no atomics, fixed summation order
+                assert np.array_equal(e[:, :2], e64[:, :2])
+                for w in range(case.nw):
+                    assert abs(e[w, 2] - e_o[w, 2]) / abs(e_o[w, 2]) < tol, (tc, mode, w, e[w, 2], e_o[w, 2])
     finally:
         case.close()
 
@@ -647,16 +653,21 @@ def test_mixed_precision_exchange_is_unsupported_for_more_than_four_orbitals():
 
 
 def test_mixed_precision_exchange_c3_full_size():
-    """C3 at full size: 3xTF32 against the FP64 kernel on every walker (the FP64 kernel is checked against the oracle in
-    test_config_C3_headline_all_walkers_energy_sampled), and against the oracle on one walker."""
+    """C3 at full size: 3xTF32 (tcgen05 kernel, and the mma.sync kernel) against the FP64 kernel on every walker (the FP64
+    kernel is checked against the oracle in test_config_C3_headline_all_walkers_energy_sampled), and against the oracle on
+    one walker."""
     case = Case(synth.CONFIGS["C3"])
     try:
         theta_d, _, _ = case.ctx.green(_to_dev(case.pb.phi))
         e64 = case.ctx.local_energy(theta_d).cpu().numpy()
         case.ctx.set_option("exchange_precision", 1)
         e = case.ctx.local_energy(theta_d).cpu().numpy()
+        case.ctx.set_option("exchange_tc", 0)
+        e_legacy = case.ctx.local_energy(theta_d).cpu().numpy()
+        case.ctx.set_option("exchange_tc", 1)
         case.ctx.set_option("exchange_precision", 0)
         assert np.max(np.abs(e[:, 2] - e64[:, 2]) / np.abs(e64[:, 2])) < 1e-5
+        assert np.max(np.abs(e_legacy[:, 2] - e64[:, 2]) / np.abs(e64[:, 2])) < 1e-5
         e_o = orc.local_energy(case.cfg.mesh, case.Lh, case.ht, theta_d[5].cpu().numpy())
         assert abs(e[5, 2] - e_o[2]) / abs(e_o[2]) < 1e-5
     finally:
