@@ -29,8 +29,8 @@
  * Inside, the library STORES the two streamed operands that bound the step at small batches in single precision -- the
  * vHS operand (the largest tensor: L, one block per (Q,-Q) pair) and the force-bias operand (the half-rotated Lh) -- i.e. half
  * their bytes in HBM and on the bus; fragments are widened in registers and every sum is accumulated in FP64.  The small
- * algebra runs in FP64 on widened copies and the exchange contraction on the TF32 tensor cores with a high/low operand split
- * (option "exchange_precision" = 1).  Results agree with the FP64 path to FP32 input/output accuracy (tolerance 1e-4).  The
+ * algebra runs in FP64 on widened copies and the exchange contraction on the TF32 tensor cores (tcgen05.mma, accumulators in
+ * tensor memory) with a high/low operand split (option "exchange_precision" = 1).  Results agree with the FP64 path to FP32 input/output accuracy (tolerance 1e-4).  The
  * AFQMC-block calls and open-shell contexts return AFQMC_UNSUPPORTED in this mode.
  *
  * Errors: every call returns an int; 0 = AFQMC_OK.  No exceptions cross the ABI, there is no
@@ -267,7 +267,18 @@ double afqmc_force_bias_flops(const afqmc_ctx* ctx, int nw);
  *   (else AFQMC_UNSUPPORTED):  1 = "3xTF32": operands split into TF32 high + low parts, three MMAs per product, FP32
  *   accumulation per task, FP64 sums: EX agrees with FP64 to ~1e-6 relative (tolerance 1e-4);  2 = "1xTF32": operands
  *   rounded once to TF32, fastest, EX error 2e-5 typical / 2e-3 worst measured: outside the 1e-4 tolerance);
+ * "exchange_tc" (1 = default: the mixed-precision exchange runs on tcgen05.mma.kind::tf32 with TMEM accumulators and tensor-map
+ *   TMA operand copies; 0 = the mma.sync kernel, which is also the fallback for shapes the tcgen05 kernel cannot take);
  * "exchange_3m" (1 = default: three real products per complex product, 0 = the 4M kernel);
+ * "exchange_regb" (1 = default for m <= 28: register-resident Theta block, A stream by cp.async, deferred hand-over; 2 = the
+ *   same kernel with register prefetch and a blocking hand-over; 0 = the generic kernel); "exchange_np", "exchange_ctas",
+ *   "exchange_minblocks" (tuning aids of the exchange kernels);
+ * "real_orbitals" (1 = default: when afqmc_create found h1, L and psi_t real -- exactly zero imaginary parts, the dense
+ *   Gamma-point representation with real orbitals of PAPER.md:260, :276-284 -- force bias, vHS and exchange run two real products
+ *   per complex product instead of three; 0 = the complex kernels on the same inputs.  Results are identical up to rounding);
+ * "taylor_subbatch" (0 = default: every Taylor order over all walkers; b > 0: the whole series for b walkers at a time, whose
+ *   V then stays in L2 -- measured slower, kept as an aid), "taylor_groups", "taylor_warps", "taylor_legacy", "green_cluster",
+ *   "green_legacy" (tuning / testing aids);
  * "timers" (1 = afqmc_step records a CUDA event after each stage, see afqmc_stage_times). */
 int afqmc_set_option(afqmc_ctx* ctx, const char* name, int value);
 
