@@ -34,7 +34,8 @@ struct FuncAttr { const void* fn; int smem; int occ; int carveout; int occ_smem;
 // The context.  All pointers are device memory owned by the context.
 struct afqmc_ctx {
     alignas(64) unsigned char tmap_lxu[128];   // CUtensorMaps of LxU and ws_thetaU (exchange_tc.cu); valid iff tmap_lxu_ok
-    alignas(64) unsigned char tmap_thu[128];
+    alignas(64) unsigned char tmap_thu[128];      // images of 8 walkers
+    alignas(64) unsigned char tmap_thu16[128];    // images of 16 walkers
     int tmap_lxu_ok;
     Dims d;
     int max_walkers;
