@@ -405,8 +405,9 @@ AFQMC_API int afqmc_set_option(afqmc_ctx* c, const char* name, int value) {
         c->opt_exchange_prec = value;
         return AFQMC_OK;
     }
-    if (strcmp(name, "exchange_tc") == 0) {        // 0 = the mma.sync TF32 kernel instead of the tcgen05 one
-        c->opt_exchange_tc = value ? 1 : 0;
+    if (strcmp(name, "exchange_tc") == 0) {        // 0 = the mma.sync TF32 kernel instead of the tcgen05 one; 2..8 = at most that many ring stages
+        if (value < 0 || value > 8) return AFQMC_INVALID_ARGUMENT;
+        c->opt_exchange_tc = value;
         return AFQMC_OK;
     }
     if (strcmp(name, "exchange_3m") == 0) {

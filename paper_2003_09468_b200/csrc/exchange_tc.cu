@@ -11,27 +11,34 @@
 //
 //  * A operand: packed ONCE in a0 as the shared-memory image itself: K-major with the 128-byte swizzle (UMMA layout type
 //    SWIZZLE_128B: K-blocks of 32 floats, rows of 128 bytes, 8-row atoms of 1024 bytes, 16-byte chunk c of row r stored at
-//    c ^ (r & 7)), TF32-rounded high and low planes.  An image (32 KB at m = 26) arrives by ONE tensor-map copy
-//    (cp.async.bulk.tensor.2d, SASS UTMALDG; the operand is viewed as rows of 256 bytes, box = one image, no TMA swizzle: the
-//    bytes are already in place) into a ring of TC_STAGES images.
+//    c ^ (r & 7)), TF32-rounded high and low planes.  A ring stage holds one K-block (32 kappa of the 128 rows, 16 KB) of the
+//    images of BOTH T; it arrives by two tensor-map copies (cp.async.bulk.tensor.2d, SASS UTMALDG; the operand is viewed as rows
+//    of 256 bytes, box = one K-block, no TMA swizzle: the bytes are already in place).  The ring has as many stages as fit beside
+//    the B images (three at 3xTF32, m = 26, 16 walkers; two are nearly as fast: the copies are not the bottleneck).
 //  * B operand: the real-embedded, TF32-split images of EVERY theta block (row block, column block, walker group) are built
 //    once per call by tc_pack_theta_kernel in the same swizzled layout (each block is used by ~2 Nk units) and arrive like A,
-//    four tensor-map copies per work item.
-//  * Warp roles: warp 5 lane 0 is the producer (tensor-map copies of the item's B images and of the A images, as far ahead as the
-//    ring allows); warp 4 lane 0 issues the MMAs (one thread issues for the CTA) and commits them to mbarriers (tcgen05.commit);
-//    warps 0-3 are the epilogue: tcgen05.ld of their 32 TMEM lanes (rows), the (a,b) transpose of the T2 values across the four
-//    adjacent lanes of a gamma (two butterfly stages of shuffles), the complex contraction sum_b T1[(g,a),(w,b)] T2[(g,b),(w,a)]
-//    in FP32 per tile and FP64 across tiles.  TMEM holds two accumulator buffers (2 x (D1, D2) x N columns = all 512 at N = 128),
-//    so the epilogue of tile t overlaps the MMAs of tile t + 1.
-//  * Results: unit partial sums in ws_expart, exactly like the FP64 kernels (energy_finalize_kernel applies multiplicities).
-//  * Measured (C3, exchange stage incl. the theta pack): 3xTF32 3.98 ms, 1xTF32 1.68 ms (mma.sync kernel: 7.19 / 3.66 ms).  What
-//    the versions on the way showed (ablation builds at N = 64, C3; profiles/r02g_ncu_exchange_tc.md): thread-built B images cost
-//    1.2 ms per call; chains of dependent 128x64x8 MMAs into ONE accumulator ran at ~120 cycles per instruction (floor 32),
-//    alternating the T1 / T2 accumulators brought that to ~90, four chains and the swizzle no further; an instruction took the SAME
-//    time at N = 128 as at N = 64 (its cost is the fetch of the A tile), hence 16 walkers per CTA: 6.01 -> 3.98 ms and 2.51 ->
-//    1.68 ms.  The first (a,b) transpose by shuffles picked its registers with lane-dependent compares, which the compiler turned
-//    into divergent branches (11 ms); the butterfly transpose selects by lane bits only.  With 16 walkers the four B planes of
-//    3xTF32 (128 KB at m = 26) leave room for three A stages, so that mode multiplies one image at a time (no T1 / T2 pairs).
+//    K-block by K-block: block kb of the NEXT item is fetched as soon as the last tiles of the current item are through with
+//    block kb (the uses of a tile run K-block by K-block), i.e. behind their remaining MMAs.
+//  * Warp roles (13 warps): warp 12 lane 0 is the producer (all tensor-map copies, as far ahead as the ring allows).
+//    Lane 0 of warps 8-11 issue the MMAs: thread (T, parity) those of T1 or T2 of the even or odd tiles of the item, and commits
+//    them to mbarriers (tcgen05.commit).  One issuing thread was the bottleneck of the first version: clock64 around its
+//    sections showed ~100 cycles per MMA and ~160 per commit, all serial, 2.5 of 3.4 ms, with the tensor pipe idle whenever that
+//    thread committed or waited; with four independent streams (two T x two accumulator buffers) the pipe is shared at ~66 cycles
+//    per 128x128x8 MMA (its nominal rate is 68) and the commits and waits of one stream hide behind the MMAs of the others.
+//    Warps 0-7 are the epilogue (TMEM lane quarter w & 3, walker half w >> 2): tcgen05.ld of both accumulators in the
+//    16-lane x 256-bit shape, which hands a thread the SAME orbital pair (a, b) of T1 of four gammas that it needs, and T2's element
+//    with the pair exchanged sits in the lane with two 2-bit fields swapped: one shuffle per value; then the complex contraction
+//    sum_{ab} T1[(g,a),(w,b)] T2[(g,b),(w,a)] in FP32 per tile and FP64 across tiles.  TMEM holds two accumulator buffers
+//    (2 x (D1, D2) x N columns = all 512 at N = 128), so the epilogue of tile t overlaps the MMAs of tiles t + 1, t + 2.
+//  * Results: unit partial sums in ws_expart, exactly like the FP64 kernels (energy_finalize_kernel applies multiplicities);
+//    the item's sum over rows is a halving butterfly over lanes and a fixed order over warps: bitwise reproducible; only the
+//    epilogue warps synchronise per item (named barrier), the copy and MMA threads run on into the next item.
+//  * Measured (C3, afqmc_local_energy incl. the theta pack, force bias and finalize, ~0.2 ms): 3xTF32 2.57 ms, 1xTF32 1.31 ms
+//    (mma.sync kernel: 7.37 / 3.86 ms).  The way there (profiles/r02g_ncu_exchange_tc.md, r02h): thread-built B images cost 1.2 ms
+//    per call; chains of dependent MMAs into ONE accumulator ran at ~120 cycles per instruction; an instruction took the SAME time
+//    at N = 128 as at N = 64, hence 16 walkers per CTA; a first (a,b) transpose by shuffles picked its registers with
+//    lane-dependent compares, which the compiler turned into divergent branches; a CTA-wide barrier per item drained the pipe;
+//    neither deeper rings nor removing the A copies altogether changed the time, the single issuing thread did (above).
 #include <cuda.h>      // CUtensorMap and the encode function's type only: the entry point is fetched through the runtime, no libcuda link
 #include "common.cuh"
 
@@ -40,12 +47,12 @@ namespace {
 // walkers per CTA: NWC = 16 (N = 128 columns; an MMA instruction costs the same at N = 64, so wider is free) unless the batch
 // has at most 8 walkers (NWC = 8: no padded columns)
 constexpr int TC_M = 128;                 // rows of a tile: 32 gamma x 4 orbitals
-constexpr int TC_THREADS = 192;           // warps 0-3: epilogue, warp 4: MMA issue, warp 5: bulk copies of the A images
-// ring of A images (one image of one plane of one T per stage): what fits beside the B images (3xTF32, 16 walkers: 4 x 32 KB of
-// B at m = 26 leave room for three); with four stages the two T of a plane are multiplied as a PAIR (alternating accumulators)
+constexpr int TC_EPI_WARPS = 8;           // epilogue warps: TMEM lane quarter w & 3, walker half w >> 2
+constexpr int TC_THREADS = 32 * (TC_EPI_WARPS + 5);       // warps 0-7: epilogue, warps 8-11: MMA issue (T, tile parity), warp 12: tensor-map copies
+constexpr int TC_KB = TC_M * 32;          // floats of one K-block of an A image: 32 kappa of the 128 rows = 16 KB (one swizzle atom column)
+constexpr int TC_MAXKB = 4;               // most K-blocks of an image (2m <= 128)
+constexpr int TC_MAXST = 8;               // most ring stages (a stage = the same K-block of the two operand images T1, T2 = 32 KB)
 template <bool SPLIT, int NWC> struct TcCfg {
-    static constexpr int STAGES = (SPLIT && NWC == 16) ? 3 : 4;
-    static constexpr bool PAIRS = STAGES == 4;
     static constexpr int N = 8 * NWC;                 // columns (w, orbital, re/im)
     static constexpr int TMEM_COLS = 4 * N;           // two accumulator buffers x (D1, D2)
     // instruction descriptor: D = F32 (bits 4-5 = 1), A and B = TF32 (bits 7-9, 10-12 = 2), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
@@ -155,11 +162,12 @@ __device__ __forceinline__ void tc_tma_rows(float* dst, const CUtensorMap* tmap,
                  "l"(reinterpret_cast<uint64_t>(tmap)), "r"(0), "r"(row), "r"(smem_u32(bar))
                  : "memory");
 }
-// 16 consecutive 32-bit columns of this thread's TMEM lane
-__device__ __forceinline__ void tc_ld16(uint32_t taddr, float (&v)[16]) {
+// 16 TMEM lanes x 256 bits, four times along the columns (32 columns): this thread gets, of the lanes l0 + lane/4 (h = 0) and
+// l0 + lane/4 + 8 (h = 1), the columns 8 j + 2 (lane % 4) + e:  v[4 j + 2 h + e]
+__device__ __forceinline__ void tc_ld16x256(uint32_t taddr, float (&v)[16]) {
     uint32_t r[16];
     asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];\n"
+        "tcgen05.ld.sync.aligned.16x256b.x4.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];\n"
         : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), "=r"(r[10]),
           "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
         : "r"(taddr)
@@ -167,244 +175,239 @@ __device__ __forceinline__ void tc_ld16(uint32_t taddr, float (&v)[16]) {
 #pragma unroll
     for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
 }
-// 4 x 4 transpose across the four lanes l & ~3 .. (l & ~3) + 3: afterwards v_b on lane a holds what v_a held on lane b
-__device__ __forceinline__ void tc_transpose4(float& v0, float& v1, float& v2, float& v3, int lane) {
-    {
-        const bool hi = lane & 1;
-        const float r0 = __shfl_xor_sync(0xffffffffu, hi ? v0 : v1, 1), r1 = __shfl_xor_sync(0xffffffffu, hi ? v2 : v3, 1);
-        v0 = hi ? r0 : v0; v1 = hi ? v1 : r0; v2 = hi ? r1 : v2; v3 = hi ? v3 : r1;
-    }
-    {
-        const bool hi = lane & 2;
-        const float r0 = __shfl_xor_sync(0xffffffffu, hi ? v0 : v2, 2), r1 = __shfl_xor_sync(0xffffffffu, hi ? v1 : v3, 2);
-        v0 = hi ? r0 : v0; v2 = hi ? v2 : r0; v1 = hi ? r1 : v1; v3 = hi ? v3 : r1;
-    }
-}
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory"); }
 
 
 template <bool SPLIT, int NWC>
 __global__ void __launch_bounds__(TC_THREADS, 1) exchange_tc_kernel(
-    const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapB, Dims d, int KP, int KS, int NTILE, int nw,
+    const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapB, Dims d, int KP, int KS, int NTILE, int nst, int nw,
     int nitems, const int* __restrict__ units, const int* __restrict__ kminus, const int* __restrict__ kplus,
     const int* __restrict__ kneg, double2* __restrict__ partial) {
     extern __shared__ __align__(1024) unsigned char tc_smem[];
     using Cfg = TcCfg<SPLIT, NWC>;
-    constexpr int NPL = SPLIT ? 2 : 1, TC_STAGES = Cfg::STAGES, TC_N = Cfg::N, TC_NWC = NWC;
+    constexpr int NPL = SPLIT ? 2 : 1, TC_N = Cfg::N, TC_NWC = NWC, TC_NH = NWC / 2;      // NH: walkers of an epilogue warp
     constexpr uint32_t TC_IDESC = Cfg::IDESC;
-    constexpr bool PAIRS = Cfg::PAIRS;
     const int IMG_A = TC_M * KP, IMG_B = TC_N * KP;        // floats (KP a multiple of 32: whole swizzle atoms)
-    float* A_s = reinterpret_cast<float*>(tc_smem);        // [TC_STAGES][IMG_A]: ring of A images
-    float* B_s = A_s + TC_STAGES * IMG_A;                  // [T][plane][IMG_B]: the item's B images
+    const int NKB = KP / 32;                               // K-blocks of an image
+    float* A_s = reinterpret_cast<float*>(tc_smem);        // [nst][T1, T2][TC_KB]: ring of K-block pairs
+    float* B_s = A_s + (size_t)nst * 2 * TC_KB;            // [T][plane][IMG_B]: the item's B images
     double* red = reinterpret_cast<double*>(B_s + 2 * NPL * IMG_B);    // [2][4 warps][TC_NWC][2]
     uint64_t* bars = reinterpret_cast<uint64_t*>(red + 2 * 4 * TC_NWC * 2);
-    uint64_t* fullA = bars;                        // [TC_STAGES]: the image of the stage has landed
-    uint64_t* stage_free = bars + TC_STAGES;       // [TC_STAGES]: the MMAs that read the stage are complete (tcgen05.commit)
-    uint64_t* mma_done = bars + 2 * TC_STAGES;     // [2]: the MMAs into accumulator buffer b (both T) are complete
-    uint64_t* tmem_free = bars + 2 * TC_STAGES + 2;    // [2]: the epilogue has read accumulator buffer b
-    uint64_t* fullB = bars + 2 * TC_STAGES + 4;    // the item's B images have landed
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * TC_STAGES + 5);
+    uint64_t* fullA = bars;                            // [2][TC_MAXST]: a K-block pair has landed; one barrier ring per tile parity (below)
+    uint64_t* stage_free = bars + 2 * TC_MAXST;        // [TC_MAXST]: the MMAs that read the stage are complete (tcgen05.commit)
+    uint64_t* mma_done = bars + 3 * TC_MAXST;          // [2]: the MMAs into accumulator buffer b (both T) are complete
+    uint64_t* tmem_free = bars + 3 * TC_MAXST + 2;     // [2]: the epilogue has read accumulator buffer b
+    uint64_t* fullB = bars + 3 * TC_MAXST + 4;         // [TC_MAXKB]: K-block kb of the item's B images (both T, all planes) has landed
+    uint64_t* freeB = bars + 3 * TC_MAXST + 4 + TC_MAXKB;      // [TC_MAXKB]: the item's last MMAs that read K-block kb of B are complete
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 3 * TC_MAXST + 4 + 2 * TC_MAXKB);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) {
-        for (int i = 0; i < TC_STAGES; ++i) { mbar_init(&fullA[i], 1); mbar_init(&stage_free[i], 1); }
-        mbar_init(&mma_done[0], 1); mbar_init(&mma_done[1], 1);
-        mbar_init(&tmem_free[0], 128); mbar_init(&tmem_free[1], 128);
-        mbar_init(fullB, 1);
+        // (completion barriers count 2: the threads of T1 and T2 commit; freeB 4: all four MMA threads)
+        for (int i = 0; i < TC_MAXST; ++i) { mbar_init(&fullA[i], 1); mbar_init(&fullA[TC_MAXST + i], 1); mbar_init(&stage_free[i], 2); }
+        mbar_init(&mma_done[0], 2); mbar_init(&mma_done[1], 2);
+        mbar_init(&tmem_free[0], 32 * TC_EPI_WARPS); mbar_init(&tmem_free[1], 32 * TC_EPI_WARPS);
+        for (int i = 0; i < TC_MAXKB; ++i) { mbar_init(&fullB[i], 1); mbar_init(&freeB[i], 4); }
         mbar_fence_init();
     }
-    if (warp == 4) tc_alloc(tmem_slot, Cfg::TMEM_COLS);
+    if (warp == TC_EPI_WARPS) tc_alloc(tmem_slot, Cfg::TMEM_COLS);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
     const int nwg = (nw + TC_NWC - 1) / TC_NWC;
-    // One USE = one A image (tile t, T, plane) and the MMAs that read it: plane hi -> Ah Bh (+ Ah Bl), plane lo -> Al Bh.
-    // Use g (counted over the CTA's whole life) lives in ring stage g % TC_STAGES; its copy completes phase g / TC_STAGES of
-    // fullA[stage], the MMAs that read it complete that phase of stage_free[stage].  Tiles are counted likewise (tt): accumulator
-    // buffer tt & 1, phases of mma_done / tmem_free; items (it): phase of fullB, parity of the reduction scratch.
-    constexpr int UPT = 2 * NPL;                                         // uses per tile
-    const int nuse = NTILE * UPT;
-    uint32_t tt = 0, ubase = 0, it = 0;
-    for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it) {
+    // One USE = the K-block kb (32 kappa of all 128 rows, 16 KB) of plane pl of BOTH operand images (T1, T2) of tile t, and the MMAs
+    // that read the pair.  Plane hi -> Ah Bh (+ Ah Bl), plane lo -> Al Bh.
+    //  * Tiles of an item alternate between the two accumulator buffers (buffer = t & 1) and between two pairs of issuing
+    //    threads; the uses of tiles 2p and 2p + 1 are interleaved in the ring (position 2 UPT p + 2 u + (t & 1); an unpaired last
+    //    tile follows), so that the two pairs advance side by side on a ring of two or three stages.
+    //  * Use position pos of the item is the CTA's use g = ubase + pos: ring stage g % nst, phase (g / nst) & 1 of stage_free.
+    //    The "landed" barriers are NOT per stage but a ring of nst per tile parity, used in the order of that parity's uses (the
+    //    c-th use of a parity: barrier c % nst, phase (c / nst) & 1): with an odd number of stages a stage alternates between the
+    //    two pairs of threads, a pair would see only every other phase of a per-stage barrier, and a parity wait that is a whole
+    //    phase ahead of its barrier passes at once (copies complete out of order: a wrong energy and a hang once in ~500
+    //    launches at C3).  A barrier of the ring is re-armed only after its previous use was consumed: at most nst uses are in flight.
+    //  * Buffer b is used cnt_b = ceil or floor(NTILE / 2) times per item: its n-th use (n = it cnt_b + t / 2) completes phase n & 1 of
+    //    mma_done[b] and tmem_free[b].  Items (it): phase of fullB / freeB, parity of the reduction scratch.
+    const int UPT = NPL * NKB;                                           // uses per tile
+    const int nuse = NTILE * UPT, npaired = (NTILE / 2) * 2 * UPT;
+    uint32_t ubase = 0, it = 0, cp0 = 0, cp1 = 0;          // cp: uses of the even / odd tiles so far (producer: issued; MMA thread: its own parity)
+    for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it, ubase += (uint32_t)nuse) {
         const int u = item / nwg, wg = item - u * nwg, w0 = wg * TC_NWC;
-        const int Q = units[4 * u], k = units[4 * u + 1], k2 = units[4 * u + 2];
 
-        double xr64[TC_NWC], xi64[TC_NWC];
+        double xr64[TC_NH], xi64[TC_NH];
 #pragma unroll
-        for (int j = 0; j < TC_NWC; ++j) xr64[j] = xi64[j] = 0.0;
+        for (int j = 0; j < TC_NH; ++j) xr64[j] = xi64[j] = 0.0;
 
-        if (warp == 5) {
-            // ===== producer: one thread streams the item's B images and the A images, as far ahead as the rings allow =====
+        if (warp == TC_EPI_WARPS + 4) {
+            // ===== producer: one thread streams the item's B images and the A K-blocks, as far ahead as the ring allows =====
             if (lane == 0) {
+                const int Q = units[4 * u], k = units[4 * u + 1], k2 = units[4 * u + 2];
                 const int mQ = kneg[Q], kq = kminus[k * d.Nk + Q], k2pq = kplus[k2 * d.Nk + Q];
-                // B: T1 from theta[(k2,.),(k-Q,.)], T2 from theta[(k,.),(k2+Q,.)]; B_s is free once the previous item's MMAs are done
-                if (tt > 0) mbar_wait(&mma_done[(tt - 1) & 1], ((tt - 1) >> 1) & 1);
-                const uint32_t bytes_b = (uint32_t)(IMG_B * sizeof(float));
-                mbar_expect_tx(fullB, 2 * NPL * bytes_b);
-                for (int T = 0; T < 2; ++T)
-                    for (int pl = 0; pl < NPL; ++pl) {
-                        const size_t blk = (((size_t)(T == 0 ? k2 : k) * d.Nk + (T == 0 ? kq : k2pq)) * nwg + wg) * 2 + pl;
-                        tc_tma_rows(B_s + (size_t)(T * NPL + pl) * IMG_B, &tmapB, (int)(blk * (size_t)(IMG_B / 64)), fullB);
-                    }
+                // B: T1 from theta[(k2,.),(k-Q,.)], T2 from theta[(k,.),(k2+Q,.)], K-block by K-block (N rows x 32 kappa each): block kb
+                // of B_s is free once the previous item's last MMAs that read it are done, i.e. while its last tiles are still being
+                // multiplied (uses run K-block by K-block), so these copies are hidden behind those tiles
+                for (int kb = 0; kb < NKB; ++kb) {
+                    if (it > 0) mbar_wait(&freeB[kb], (it - 1) & 1);
+                    mbar_expect_tx(&fullB[kb], 2 * NPL * (uint32_t)(TC_N * 32 * sizeof(float)));
+                    for (int T = 0; T < 2; ++T)
+                        for (int pl = 0; pl < NPL; ++pl) {
+                            const size_t blk = (((size_t)(T == 0 ? k2 : k) * d.Nk + (T == 0 ? kq : k2pq)) * nwg + wg) * 2 + pl;
+                            tc_tma_rows(B_s + (size_t)(T * NPL + pl) * IMG_B + (size_t)kb * (TC_N * 32), &tmapB,
+                                        (int)(blk * (size_t)(IMG_B / 64) + (size_t)kb * (TC_N / 2)), &fullB[kb]);
+                        }
+                }
                 const size_t blk1 = ((size_t)Q * d.Nk + k) * NTILE, blk2 = ((size_t)mQ * d.Nk + k2) * NTILE;
-                const uint32_t bytes_a = (uint32_t)(IMG_A * sizeof(float));
-                for (int j = 0; j < nuse; ++j) {
-                    const uint32_t g = ubase + (uint32_t)j;
-                    const int st = (int)(g % TC_STAGES);
-                    if (g >= TC_STAGES) mbar_wait(&stage_free[st], ((g / TC_STAGES) - 1) & 1);
-                    // use order inside a tile: pairs -> (plane, T) with T fastest; else (T1 hi, T1 lo, T2 hi, T2 lo), one image at a time
-                    const int t = j / UPT, T = PAIRS ? (j & 1) : ((j % UPT) >> 1), pl = PAIRS ? ((j % UPT) >> 1) : (j & 1);
-                    mbar_expect_tx(&fullA[st], bytes_a);
-                    tc_tma_rows(A_s + (size_t)st * IMG_A, &tmapA, (int)((((T == 0 ? blk1 : blk2) + t) * 2 + pl) * (size_t)(IMG_A / 64)), &fullA[st]);
+                uint32_t st = ubase % (uint32_t)nst, ph = (ubase / (uint32_t)nst) & 1;
+                for (int pos = 0; pos < nuse; ++pos) {
+                    int t, uu;
+                    if (pos < npaired) { const int r = pos % (2 * UPT); t = 2 * (pos / (2 * UPT)) + (r & 1); uu = r >> 1; }
+                    else { t = NTILE - 1; uu = pos - npaired; }
+                    const int kb = uu / NPL, pl = uu - kb * NPL;          // use order of a tile: K-block, then plane
+                    if (ubase + (uint32_t)pos >= (uint32_t)nst) mbar_wait(&stage_free[st], ph ^ 1);
+                    const uint32_t c = (t & 1) ? cp1++ : cp0++;
+                    uint64_t* full = &fullA[(t & 1) * TC_MAXST + (int)(c % (uint32_t)nst)];
+                    mbar_expect_tx(full, 2 * TC_KB * (uint32_t)sizeof(float));
+                    float* dst = A_s + (size_t)st * 2 * TC_KB;
+                    // rows of 256 bytes: image (block + t, plane) starts at row index * IMG_A / 64, its K-block kb 64 rows further per block
+                    tc_tma_rows(dst, &tmapA, (int)(((blk1 + t) * 2 + pl) * (size_t)(IMG_A / 64) + (size_t)kb * (TC_KB / 64)), full);
+                    tc_tma_rows(dst + TC_KB, &tmapA, (int)(((blk2 + t) * 2 + pl) * (size_t)(IMG_A / 64) + (size_t)kb * (TC_KB / 64)), full);
+                    if (++st == (uint32_t)nst) { st = 0; ph ^= 1; }
                 }
             }
-            ubase += (uint32_t)nuse;
-            tt += (uint32_t)NTILE;
             __syncwarp();
-        } else if (warp == 4) {
-            // ===== MMA issue: one thread for the CTA =====
+        } else if (warp >= TC_EPI_WARPS) {
+            // ===== MMA issue: four threads, lane 0 of warps 8 .. 11: thread (T, par) issues the MMAs of T (0: T1, 1: T2) of the tiles
+            //       t = par, par + 2, ...  An MMA occupies its issuing thread for ~100 cycles and a tcgen05.commit for ~160 (clock64
+            //       around them; with ONE issuing thread, 2.5 of the 3.4 ms of the 3xTF32 kernel were that thread's time, and the
+            //       tensor pipe idled whenever it committed or waited), so independent streams are issued and committed concurrently:
+            //       the two T of a tile, and two tiles with their own accumulator buffers =====
             if (lane == 0) {
-                const uint32_t a_addr = smem_u32(A_s), b_addr = smem_u32(B_s);
-                mbar_wait(fullB, it & 1);
-                uint32_t buf = tt & 1;
-                const uint32_t db_T[2] = {b_addr, b_addr + (uint32_t)(NPL * IMG_B * 4)};                      // hi planes of B1, B2
-                const uint64_t lo_off = (uint64_t)((IMG_B * 4) >> 4);                                     // hi -> lo plane of a B image
-                // a k-step is 8 kappa = 32 bytes of every row: 32-byte slot ks & 3 of K-block ks >> 2 (rows * 128 bytes each), i.e. the
-                // start-address field of a descriptor (16-byte units) grows by 2, or jumps to the next block
-                auto step_a = [](const int ks) { return (ks & 3) == 3 ? (uint64_t)((TC_M * 128 - 96) >> 4) : (uint64_t)2; };
-                auto step_b = [](const int ks) { return (ks & 3) == 3 ? (uint64_t)((Cfg::N * 128 - 96) >> 4) : (uint64_t)2; };
-                if (!PAIRS) {
-                    // 3xTF32 at 16 walkers: one image per use (the ring holds three beside the four B planes); plane hi -> Ah Bh + Ah Bl, lo -> Al Bh
-                    for (int j = 0; j < nuse; ++j) {
-                        const uint32_t g = ubase + (uint32_t)j;
-                        const int st = (int)(g % TC_STAGES), T = (j >> 1) & 1, pl = j & 1;
-                        if ((j & 3) == 0) {                                   // first use of a tile
-                            buf = tt & 1;
-                            if (tt >= 2) mbar_wait(&tmem_free[buf], ((tt >> 1) - 1) & 1);       // the accumulator buffer was read
-                        }
-                        mbar_wait(&fullA[st], (g / TC_STAGES) & 1);
+                const int T = (warp - TC_EPI_WARPS) & 1, par = (warp - TC_EPI_WARPS) >> 1;
+                const uint32_t a_addr = smem_u32(A_s) + (uint32_t)(T * TC_KB * 4), b_addr = smem_u32(B_s) + (uint32_t)(T * NPL * IMG_B * 4);
+                const uint32_t lo_off = (uint32_t)((IMG_B * 4) >> 4);         // hi -> lo plane of a B image (descriptor units of 16 bytes)
+                const uint32_t dT = tmem_base + par * (2 * TC_N) + T * TC_N;
+                const uint32_t cnt = (uint32_t)((NTILE + 1 - par) >> 1);      // tiles of this parity per item
+                for (int t = par; t < NTILE; t += 2) {
+                    const uint32_t n = it * cnt + (uint32_t)(t >> 1);         // how often the buffer was used before
+                    if (n >= 1) mbar_wait(&tmem_free[par], (n - 1) & 1);      // the accumulator buffer was read
+                    const bool paired = (t | 1) < NTILE;                      // tile t ^ 1 exists: their uses alternate in the ring
+                    const int pos0 = paired ? (t >> 1) * 2 * UPT + (t & 1) : npaired, pstep = paired ? 2 : 1;
+                    for (int uu = 0; uu < UPT; ++uu) {
+                        const int kb = uu / NPL, pl = uu - kb * NPL;
+                        const uint32_t st = (ubase + (uint32_t)(pos0 + pstep * uu)) % (uint32_t)nst, c = cp0++;       // (cp0: this thread's own count)
+                        if (t == par && pl == 0) mbar_wait(&fullB[kb], it & 1);   // first tile: K-block kb of the item's B images has landed
+                        mbar_wait(&fullA[par * TC_MAXST + (int)(c % (uint32_t)nst)], (c / (uint32_t)nst) & 1);
                         tc_fence_after();
-                        const uint32_t dT = tmem_base + buf * (2 * TC_N) + T * TC_N;
-                        uint64_t da = tc_desc(a_addr + (uint32_t)(st * IMG_A * 4)), db = tc_desc(db_T[T]);
-                        uint32_t acc = pl == 0 ? 0u : 1u;                     // the first MMA into D_T of a tile overwrites
-                        for (int ks = 0; ks < KS; ++ks) {
+                        // a k-step is 8 kappa = 32 bytes of every row: slot ks of the K-block's 128-byte rows, i.e. the start-address
+                        // field of the descriptor (16-byte units) grows by 2 per k-step
+                        uint64_t da = tc_desc(a_addr + (uint32_t)(st * 2 * TC_KB * 4)), db = tc_desc(b_addr + (uint32_t)(kb * TC_N * 128));
+                        const int nks = KS - 4 * kb < 4 ? KS - 4 * kb : 4;
+                        uint32_t acc = uu == 0 ? 0u : 1u;                     // the first MMA into D_T of a tile overwrites
+                        for (int ks = 0; ks < nks; ++ks) {
                             tc_mma_tf32(dT, da, db, TC_IDESC, acc);
-                            if (pl == 0) tc_mma_tf32(dT, da, db + lo_off, TC_IDESC, 1);
+                            if (SPLIT && pl == 0) tc_mma_tf32(dT, da, db + lo_off, TC_IDESC, 1);       // plane hi: also Ah Bl
                             acc = 1;
-                            da += step_a(ks); db += step_b(ks);
+                            da += 2; db += 2;
                         }
                         tc_commit(&stage_free[st]);                           // the stage may be refilled once these MMAs are done
-                        if ((j & 3) == 3) { tc_commit(&mma_done[buf]); ++tt; }    // ... and the tile's accumulators are complete
+                        if (t + 2 >= NTILE && pl == NPL - 1) tc_commit(&freeB[kb]);   // (last tile of this thread) ... K-block kb of B_s too
                     }
-                } else {
-                    // the two images (T1, T2) of a plane as a PAIR, their MMAs alternating, so that consecutive instructions accumulate
-                    // into different TMEM columns (dependent MMAs into one accumulator serialise: ~120 against ~90 cycles each)
-                    for (int q = 0; q < nuse / 2; ++q) {
-                        const uint32_t g0 = ubase + 2u * (uint32_t)q, g1 = g0 + 1;
-                        const int s0 = (int)(g0 % TC_STAGES), s1 = (int)(g1 % TC_STAGES);
-                        const int pl = q % NPL;
-                        if (pl == 0) {                                        // first pair of a tile
-                            buf = tt & 1;
-                            if (tt >= 2) mbar_wait(&tmem_free[buf], ((tt >> 1) - 1) & 1);       // the accumulator buffer was read
-                        }
-                        mbar_wait(&fullA[s0], (g0 / TC_STAGES) & 1);
-                        mbar_wait(&fullA[s1], (g1 / TC_STAGES) & 1);
-                        tc_fence_after();
-                        const uint32_t d0 = tmem_base + buf * (2 * TC_N), d1 = d0 + TC_N;
-                        uint64_t da0 = tc_desc(a_addr + (uint32_t)(s0 * IMG_A * 4)), da1 = tc_desc(a_addr + (uint32_t)(s1 * IMG_A * 4));
-                        uint64_t db0 = tc_desc(db_T[0]), db1 = tc_desc(db_T[1]);
-                        uint32_t acc = pl == 0 ? 0u : 1u;                     // the first MMA into D_T of a tile overwrites
-                        for (int ks = 0; ks < KS; ++ks) {
-                            tc_mma_tf32(d0, da0, db0, TC_IDESC, acc);
-                            tc_mma_tf32(d1, da1, db1, TC_IDESC, acc);
-                            if (SPLIT && pl == 0) {                           // plane hi: also Ah Bl
-                                tc_mma_tf32(d0, da0, db0 + lo_off, TC_IDESC, 1);
-                                tc_mma_tf32(d1, da1, db1 + lo_off, TC_IDESC, 1);
-                            }
-                            acc = 1;
-                            da0 += step_a(ks); da1 += step_a(ks); db0 += step_b(ks); db1 += step_b(ks);
-                        }
-                        tc_commit(&stage_free[s0]);
-                        tc_commit(&stage_free[s1]);
-                        if (pl == NPL - 1) { tc_commit(&mma_done[buf]); ++tt; }
-                    }
+                    tc_commit(&mma_done[par]);                                // the tile's accumulator D_T is complete
                 }
-            } else {
-                tt += (uint32_t)NTILE;
+                if (par >= NTILE)                                             // no tile of this parity: nothing of B_s is read here
+                    for (int kb = 0; kb < NKB; ++kb) mbar_arrive(&freeB[kb]);
             }
-            ubase += (uint32_t)nuse;
             __syncwarp();
         } else {
-            // ===== epilogue: warps 0-3 own TMEM lanes 32 warp .. 32 warp + 31 = rows (gamma, orbital) =====
-            for (int t = 0; t < NTILE; ++t, ++tt) {
-                const uint32_t buf = tt & 1;
-                mbar_wait(&mma_done[buf], (tt >> 1) & 1);
+            // ===== epilogue: warps 0-7; warp w reads TMEM lanes 32 (w & 3) .. + 31 = rows (gamma, orbital) and the columns of the
+            //       walker half w >> 2 =====
+            // The contraction needs  X_w += sum_{a,b} T1[(g,a),(w,b)] * T2[(g,b),(w,a)].  Both accumulators are read with the
+            // 16-lane x 256-bit shape: a thread gets, of the rows  l0 + lane/4 (+ 8)  (l0 = 0, 16: two loads), the orbital
+            // column  lane % 4  of every walker, i.e. T1[(g, a = (lane/4) % 4), (w, b = lane % 4)] of four gammas, and of T2 the
+            // element with the two orbitals exchanged sits in the lane with those two 2-bit fields swapped: ONE shuffle per value
+            // (a first version transposed 4 x 4 blocks over adjacent lanes from the one-row-per-lane shape: 4 shuffles + 12 selects).
+            const int partner = (lane & 16) | ((lane & 3) << 2) | ((lane >> 2) & 3);
+            for (int t = 0; t < NTILE; ++t) {
+                const uint32_t buf = t & 1, n = it * (uint32_t)((NTILE + 1 - (int)buf) >> 1) + (uint32_t)(t >> 1);
+                mbar_wait(&mma_done[buf], n & 1);
                 tc_fence_after();
-                const uint32_t trow = tmem_base + ((uint32_t)(32 * warp) << 16) + buf * (2 * TC_N);
-                // four walkers (32 columns) of both accumulator rows at a time.  The contraction needs
-                //   X_w += sum_b T1[(g,a),(w,b)] * T2[(g,b),(w,a)]:
-                // T2[(g,b),(w,a)] sits in lane (g,b), one of the four adjacent lanes of this gamma, at the column of the RECEIVER's
-                // orbital a: a 4 x 4 transpose across those lanes (no shared memory)
+                const uint32_t trow = tmem_base + ((uint32_t)(32 * (warp & 3)) << 16) + buf * (2 * TC_N) + (warp >> 2) * (TC_N / 2);
 #pragma unroll
-                for (int q4 = 0; q4 < TC_NWC / 4; ++q4) {
-                    float t1[32], t2[32];
+                for (int q4 = 0; q4 < TC_NH / 4; ++q4) {                // four walkers (32 columns) at a time
+                    float t1[2][16], t2[2][16];                         // [l0][4 walker + 2 (row + 8) + re/im]
 #pragma unroll
-                    for (int q = 0; q < 2; ++q) {
-                        float v[16];
-                        tc_ld16(trow + TC_N + 32 * q4 + 16 * q, v);
-#pragma unroll
-                        for (int i = 0; i < 16; ++i) t2[16 * q + i] = v[i];
-                        tc_ld16(trow + 32 * q4 + 16 * q, v);
-#pragma unroll
-                        for (int i = 0; i < 16; ++i) t1[16 * q + i] = v[i];
+                    for (int l = 0; l < 2; ++l) {
+                        tc_ld16x256(trow + ((uint32_t)(16 * l) << 16) + TC_N + 32 * q4, t2[l]);
+                        tc_ld16x256(trow + ((uint32_t)(16 * l) << 16) + 32 * q4, t1[l]);
                     }
                     tc_wait_ld();
-                    if (q4 == TC_NWC / 4 - 1) {                       // the last columns of the buffer are in registers
+                    if (q4 == TC_NH / 4 - 1) {                          // the last columns of the buffer are in registers
                         tc_fence_before();
                         mbar_arrive(&tmem_free[buf]);
                     }
-                    // the T2 values of every walker: 4 x 4 transpose over the four lanes of this gamma (two butterfly stages of
-                    // shuffles, register choice by the lane's bits only: no lane-dependent register indexing)
+#pragma unroll
+                    for (int l = 0; l < 2; ++l)
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) t2[l][i] = __shfl_sync(0xffffffffu, t2[l][i], partner);
 #pragma unroll
                     for (int wl = 0; wl < 4; ++wl) {
+                        float sr = 0.f, si = 0.f;
 #pragma unroll
-                        for (int c = 0; c < 2; ++c) tc_transpose4(t2[8 * wl + c], t2[8 * wl + 2 + c], t2[8 * wl + 4 + c], t2[8 * wl + 6 + c], lane);
-                        float sr = 0.f, si = 0.f;       // now t2[8 wl + 2 b + c] = T2[(g,b),(w,a)] of this lane's a
+                        for (int l = 0; l < 2; ++l)
 #pragma unroll
-                        for (int b = 0; b < 4; ++b) {
-                            const float ar = t1[8 * wl + 2 * b], ai = t1[8 * wl + 2 * b + 1], pr = t2[8 * wl + 2 * b], pi = t2[8 * wl + 2 * b + 1];
-                            sr = fmaf(ar, pr, sr); sr = fmaf(-ai, pi, sr);
-                            si = fmaf(ar, pi, si); si = fmaf(ai, pr, si);
-                        }
+                            for (int h = 0; h < 2; ++h) {
+                                const float ar = t1[l][4 * wl + 2 * h], ai = t1[l][4 * wl + 2 * h + 1];
+                                const float pr = t2[l][4 * wl + 2 * h], pi = t2[l][4 * wl + 2 * h + 1];
+                                sr = fmaf(ar, pr, sr); sr = fmaf(-ai, pi, sr);
+                                si = fmaf(ar, pi, si); si = fmaf(ai, pr, si);
+                            }
                         xr64[4 * q4 + wl] += (double)sr; xi64[4 * q4 + wl] += (double)si;
                     }
                 }
             }
         }
 
-        // ---- the item's result: sum over the 128 rows (lanes, then warps in a fixed order); scratch alternates per item, so one
-        //      CTA-wide barrier per item suffices ----
-        double* rd = red + (it & 1) * (4 * TC_NWC * 2);
-        if (warp < 4) {
+        // ---- the item's result: sum over the 128 rows.  Only the epilogue warps take part (named barrier 1): the producer and the
+        //      MMA threads run on into the next item.  Lanes: a butterfly that halves the number of values at every stage (lane l
+        //      ends with the total of value l % (2 NH): re of the warp's walker l, im of walker l - NH), then the four warps of a
+        //      walker half in a fixed order; the scratch alternates per item, so one barrier per item suffices ----
+        if (warp < TC_EPI_WARPS) {
+            double* rd = red + (it & 1) * (TC_EPI_WARPS * 2 * TC_NH);
+            double v[2 * TC_NH];
 #pragma unroll
-            for (int wl = 0; wl < TC_NWC; ++wl) {
-                const double r = warp_sum(xr64[wl]), i = warp_sum(xi64[wl]);
-                if (lane == 0) { rd[(warp * TC_NWC + wl) * 2] = r; rd[(warp * TC_NWC + wl) * 2 + 1] = i; }
+            for (int j = 0; j < TC_NH; ++j) { v[j] = xr64[j]; v[TC_NH + j] = xi64[j]; }
+#pragma unroll
+            for (int m = 16; m >= 2 * TC_NH; m >>= 1) {                 // more lanes than values: plain sums first
+#pragma unroll
+                for (int j = 0; j < 2 * TC_NH; ++j) v[j] += __shfl_xor_sync(0xffffffffu, v[j], m);
             }
-        }
-        __syncthreads();
-        if (tid < TC_NWC && w0 + tid < nw) {
-            double r = 0.0, i = 0.0;
-            for (int x = 0; x < 4; ++x) { r += rd[(x * TC_NWC + tid) * 2]; i += rd[(x * TC_NWC + tid) * 2 + 1]; }
-            partial[(size_t)u * nw + w0 + tid] = make_double2(r, i);
+#pragma unroll
+            for (int m = TC_NH; m >= 1; m >>= 1) {
+                const bool hi = lane & m;
+#pragma unroll
+                for (int i = 0; i < m; ++i) {
+                    const double send = hi ? v[i] : v[i + m], keep = hi ? v[i + m] : v[i];
+                    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, m);
+                }
+            }
+            if (lane < 2 * TC_NH) rd[warp * (2 * TC_NH) + lane] = v[0];
+            asm volatile("bar.sync 1, 256;\n" ::: "memory");
+            if (tid < 2 * TC_NWC) {
+                const int wl = tid % TC_NWC, c = tid / TC_NWC, hw = wl / TC_NH, j = wl % TC_NH;
+                if (w0 + wl < nw) {
+                    double r = 0.0;
+                    for (int x = 0; x < 4; ++x) r += rd[(4 * hw + x) * (2 * TC_NH) + c * TC_NH + j];
+                    reinterpret_cast<double*>(partial)[((size_t)u * nw + w0 + wl) * 2 + c] = r;
+                }
+            }
         }
     }
 
     tc_fence_before();
     __syncthreads();
-    if (warp == 4) tc_dealloc(tmem_base, Cfg::TMEM_COLS);
+    if (warp == TC_EPI_WARPS) tc_dealloc(tmem_base, Cfg::TMEM_COLS);
 }
 
 }  // namespace
@@ -452,8 +455,8 @@ int afqmc_i_ensure_lxu(afqmc_ctx* c, cudaStream_t st) {
     if (g > 148 * 64) g = 148 * 64;
     pack_LxU_kernel<<<(unsigned)g, 256, 0, st>>>(d, KP, NTILE, c->Lh, c->LxU, total);
     AFQMC_LAUNCH_CHECK(c);
-    c->tmap_lxu_ok = (tc_make_map(c->tmap_lxu, c->LxU, 2 * total, TC_M * KP / 64) && tc_make_map(c->tmap_thu, c->ws_thetaU, nthu, 64 * KP / 64) &&
-                      tc_make_map(c->tmap_thu16, c->ws_thetaU, nthu, 128 * KP / 64)) ? 1 : 0;
+    c->tmap_lxu_ok = (tc_make_map(c->tmap_lxu, c->LxU, 2 * total, TC_KB / 64) && tc_make_map(c->tmap_thu, c->ws_thetaU, nthu, 64 / 2) &&
+                      tc_make_map(c->tmap_thu16, c->ws_thetaU, nthu, 128 / 2)) ? 1 : 0;
     return AFQMC_OK;
 }
 
@@ -462,9 +465,14 @@ static int tc_launch(afqmc_ctx* c, int KP, int KS, int NTILE, const double2* the
     using Cfg = TcCfg<SPLIT, NWC>;
     const Dims& d = c->d;
     constexpr int npl = SPLIT ? 2 : 1;
-    const size_t smem = (size_t)(Cfg::STAGES * TC_M + 2 * npl * Cfg::N) * KP * sizeof(float) + (size_t)2 * 4 * NWC * 2 * sizeof(double) +
-                        (2 * Cfg::STAGES + 5) * sizeof(uint64_t) + 16;
-    if (smem > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
+    // shared memory: the item's B images, the reduction scratch, the barriers, and as many ring stages as fit beside them
+    const size_t fixed = (size_t)2 * npl * Cfg::N * KP * sizeof(float) + (size_t)2 * 4 * NWC * 2 * sizeof(double) + (3 * TC_MAXST + 4 + 2 * TC_MAXKB) * sizeof(uint64_t) + 16;
+    const size_t stage = (size_t)2 * TC_KB * sizeof(float);
+    if (KP / 32 > TC_MAXKB || fixed + 2 * stage > (size_t)c->smem_optin) return AFQMC_UNSUPPORTED;
+    int nst = (int)(((size_t)c->smem_optin - fixed) / stage);
+    if (nst > TC_MAXST) nst = TC_MAXST;
+    if (c->opt_exchange_tc > 1 && c->opt_exchange_tc < nst) nst = c->opt_exchange_tc;       // (experiments: option exchange_tc = stages)
+    const size_t smem = fixed + (size_t)nst * stage;
     int rc = afqmc_i_ensure_lxu(c, st);
     if (rc != AFQMC_OK) return rc;
     if (!c->tmap_lxu_ok) return AFQMC_UNSUPPORTED;
@@ -484,7 +492,7 @@ static int tc_launch(afqmc_ctx* c, int KP, int KS, int NTILE, const double2* the
     const unsigned grid = (unsigned)(nitems < c->num_sms ? nitems : c->num_sms);
     auto kern = exchange_tc_kernel<SPLIT, NWC>;
     if ((rc = afqmc_smem_optin(c, (const void*)kern, smem)) != AFQMC_OK) return rc;
-    kern<<<grid, TC_THREADS, smem, st>>>(tmapA, tmapB, d, KP, KS, NTILE, nw, (int)nitems, c->units, c->kminus, c->kplus, c->kneg, c->ws_expart);
+    kern<<<grid, TC_THREADS, smem, st>>>(tmapA, tmapB, d, KP, KS, NTILE, nst, nw, (int)nitems, c->units, c->kminus, c->kplus, c->kneg, c->ws_expart);
     AFQMC_LAUNCH_CHECK(c);
     c->ex_parts = 1;
     return AFQMC_OK;
