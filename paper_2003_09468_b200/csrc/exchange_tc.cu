@@ -162,18 +162,16 @@ __device__ __forceinline__ void tc_tma_rows(float* dst, const CUtensorMap* tmap,
                  "l"(reinterpret_cast<uint64_t>(tmap)), "r"(0), "r"(row), "r"(smem_u32(bar))
                  : "memory");
 }
-// 16 TMEM lanes x 256 bits, four times along the columns (32 columns): this thread gets, of the lanes l0 + lane/4 (h = 0) and
-// l0 + lane/4 + 8 (h = 1), the columns 8 j + 2 (lane % 4) + e:  v[4 j + 2 h + e]
-__device__ __forceinline__ void tc_ld16x256(uint32_t taddr, float (&v)[16]) {
-    uint32_t r[16];
-    asm volatile(
-        "tcgen05.ld.sync.aligned.16x256b.x4.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];\n"
-        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), "=r"(r[10]),
-          "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-        : "r"(taddr)
-        : "memory");
+// 16 TMEM lanes x 256 bits, twice along the columns (16 columns = two walkers): this thread gets, of the lanes l0 + lane/4 (h = 0)
+// and l0 + lane/4 + 8 (h = 1), the columns 8 j + 2 (lane % 4) + e:  v[4 j + 2 h + e]
+__device__ __forceinline__ void tc_ld16x256x2(uint32_t taddr, float (&v)[8]) {
+    uint32_t r[8];
+    asm volatile("tcgen05.ld.sync.aligned.16x256b.x2.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];\n"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr)
+                 : "memory");
 #pragma unroll
-    for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+    for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
 }
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory"); }
 
@@ -219,21 +217,23 @@ __global__ void __launch_bounds__(TC_THREADS, 1) exchange_tc_kernel(
     const int nwg = (nw + TC_NWC - 1) / TC_NWC;
     // One USE = the K-block kb (32 kappa of all 128 rows, 16 KB) of plane pl of BOTH operand images (T1, T2) of tile t, and the MMAs
     // that read the pair.  Plane hi -> Ah Bh (+ Ah Bl), plane lo -> Al Bh.
-    //  * Tiles of an item alternate between the two accumulator buffers (buffer = t & 1) and between two pairs of issuing
-    //    threads; the uses of tiles 2p and 2p + 1 are interleaved in the ring (position 2 UPT p + 2 u + (t & 1); an unpaired last
-    //    tile follows), so that the two pairs advance side by side on a ring of two or three stages.
+    //  * Tiles alternate between the two accumulator buffers and between two pairs of issuing threads by the parity of the CTA's
+    //    tile count tbase + t (not of t: with an odd number of tiles per item the last tile of an item and the first of the next
+    //    would share a buffer, and its epilogue would be exposed); the uses of the item's tiles 2p and 2p + 1 are interleaved in
+    //    the ring (position 2 UPT p + 2 u + (t & 1); an unpaired last tile follows), so that the two pairs advance side by side
+    //    on a ring of two or three stages.
     //  * Use position pos of the item is the CTA's use g = ubase + pos: ring stage g % nst, phase (g / nst) & 1 of stage_free.
     //    The "landed" barriers are NOT per stage but a ring of nst per tile parity, used in the order of that parity's uses (the
     //    c-th use of a parity: barrier c % nst, phase (c / nst) & 1): with an odd number of stages a stage alternates between the
     //    two pairs of threads, a pair would see only every other phase of a per-stage barrier, and a parity wait that is a whole
     //    phase ahead of its barrier passes at once (copies complete out of order: a wrong energy and a hang once in ~500
     //    launches at C3).  A barrier of the ring is re-armed only after its previous use was consumed: at most nst uses are in flight.
-    //  * Buffer b is used cnt_b = ceil or floor(NTILE / 2) times per item: its n-th use (n = it cnt_b + t / 2) completes phase n & 1 of
-    //    mma_done[b] and tmem_free[b].  Items (it): phase of fullB / freeB, parity of the reduction scratch.
+    //  * The n-th use of a buffer (n = (tbase + t) / 2) completes phase n & 1 of mma_done[b] and tmem_free[b].  Items (it): phase
+    //    of fullB / freeB, parity of the reduction scratch.
     const int UPT = NPL * NKB;                                           // uses per tile
     const int nuse = NTILE * UPT, npaired = (NTILE / 2) * 2 * UPT;
-    uint32_t ubase = 0, it = 0, cp0 = 0, cp1 = 0;          // cp: uses of the even / odd tiles so far (producer: issued; MMA thread: its own parity)
-    for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it, ubase += (uint32_t)nuse) {
+    uint32_t ubase = 0, tbase = 0, it = 0, cp0 = 0, cp1 = 0;          // cp: uses of the even / odd tiles so far (producer: issued; MMA thread: its own parity)
+    for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it, ubase += (uint32_t)nuse, tbase += (uint32_t)NTILE) {
         const int u = item / nwg, wg = item - u * nwg, w0 = wg * TC_NWC;
 
         double xr64[TC_NH], xi64[TC_NH];
@@ -266,8 +266,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1) exchange_tc_kernel(
                     else { t = NTILE - 1; uu = pos - npaired; }
                     const int kb = uu / NPL, pl = uu - kb * NPL;          // use order of a tile: K-block, then plane
                     if (ubase + (uint32_t)pos >= (uint32_t)nst) mbar_wait(&stage_free[st], ph ^ 1);
-                    const uint32_t c = (t & 1) ? cp1++ : cp0++;
-                    uint64_t* full = &fullA[(t & 1) * TC_MAXST + (int)(c % (uint32_t)nst)];
+                    const int par = (int)((tbase + (uint32_t)t) & 1);
+                    const uint32_t c = par ? cp1++ : cp0++;
+                    uint64_t* full = &fullA[par * TC_MAXST + (int)(c % (uint32_t)nst)];
                     mbar_expect_tx(full, 2 * TC_KB * (uint32_t)sizeof(float));
                     float* dst = A_s + (size_t)st * 2 * TC_KB;
                     // rows of 256 bytes: image (block + t, plane) starts at row index * IMG_A / 64, its K-block kb 64 rows further per block
@@ -284,20 +285,19 @@ __global__ void __launch_bounds__(TC_THREADS, 1) exchange_tc_kernel(
             //       tensor pipe idled whenever it committed or waited), so independent streams are issued and committed concurrently:
             //       the two T of a tile, and two tiles with their own accumulator buffers =====
             if (lane == 0) {
-                const int T = (warp - TC_EPI_WARPS) & 1, par = (warp - TC_EPI_WARPS) >> 1;
+                const int T = (warp - TC_EPI_WARPS) & 1, par = (warp - TC_EPI_WARPS) >> 1, t0 = par ^ (int)(tbase & 1);
                 const uint32_t a_addr = smem_u32(A_s) + (uint32_t)(T * TC_KB * 4), b_addr = smem_u32(B_s) + (uint32_t)(T * NPL * IMG_B * 4);
                 const uint32_t lo_off = (uint32_t)((IMG_B * 4) >> 4);         // hi -> lo plane of a B image (descriptor units of 16 bytes)
                 const uint32_t dT = tmem_base + par * (2 * TC_N) + T * TC_N;
-                const uint32_t cnt = (uint32_t)((NTILE + 1 - par) >> 1);      // tiles of this parity per item
-                for (int t = par; t < NTILE; t += 2) {
-                    const uint32_t n = it * cnt + (uint32_t)(t >> 1);         // how often the buffer was used before
+                for (int t = t0; t < NTILE; t += 2) {
+                    const uint32_t n = (tbase + (uint32_t)t) >> 1;            // how often the buffer was used before
                     if (n >= 1) mbar_wait(&tmem_free[par], (n - 1) & 1);      // the accumulator buffer was read
                     const bool paired = (t | 1) < NTILE;                      // tile t ^ 1 exists: their uses alternate in the ring
                     const int pos0 = paired ? (t >> 1) * 2 * UPT + (t & 1) : npaired, pstep = paired ? 2 : 1;
                     for (int uu = 0; uu < UPT; ++uu) {
                         const int kb = uu / NPL, pl = uu - kb * NPL;
                         const uint32_t st = (ubase + (uint32_t)(pos0 + pstep * uu)) % (uint32_t)nst, c = cp0++;       // (cp0: this thread's own count)
-                        if (t == par && pl == 0) mbar_wait(&fullB[kb], it & 1);   // first tile: K-block kb of the item's B images has landed
+                        if (t == t0 && pl == 0) mbar_wait(&fullB[kb], it & 1);   // first tile: K-block kb of the item's B images has landed
                         mbar_wait(&fullA[par * TC_MAXST + (int)(c % (uint32_t)nst)], (c / (uint32_t)nst) & 1);
                         tc_fence_after();
                         // a k-step is 8 kappa = 32 bytes of every row: slot ks of the K-block's 128-byte rows, i.e. the start-address
@@ -316,7 +316,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) exchange_tc_kernel(
                     }
                     tc_commit(&mma_done[par]);                                // the tile's accumulator D_T is complete
                 }
-                if (par >= NTILE)                                             // no tile of this parity: nothing of B_s is read here
+                if (t0 >= NTILE)                                              // no tile of this parity: nothing of B_s is read here
                     for (int kb = 0; kb < NKB; ++kb) mbar_arrive(&freeB[kb]);
             }
             __syncwarp();
@@ -330,40 +330,47 @@ __global__ void __launch_bounds__(TC_THREADS, 1) exchange_tc_kernel(
             // (a first version transposed 4 x 4 blocks over adjacent lanes from the one-row-per-lane shape: 4 shuffles + 12 selects).
             const int partner = (lane & 16) | ((lane & 3) << 2) | ((lane >> 2) & 3);
             for (int t = 0; t < NTILE; ++t) {
-                const uint32_t buf = t & 1, n = it * (uint32_t)((NTILE + 1 - (int)buf) >> 1) + (uint32_t)(t >> 1);
+                const uint32_t buf = (tbase + (uint32_t)t) & 1, n = (tbase + (uint32_t)t) >> 1;
                 mbar_wait(&mma_done[buf], n & 1);
                 tc_fence_after();
                 const uint32_t trow = tmem_base + ((uint32_t)(32 * (warp & 3)) << 16) + buf * (2 * TC_N) + (warp >> 2) * (TC_N / 2);
+                // two walkers (16 columns) at a time; the loads of the next pair are in flight while this pair is contracted
+                float t1[2][2][8], t2[2][2][8];                         // [parity of the pair][l0][4 walker + 2 (row + 8) + re/im]
 #pragma unroll
-                for (int q4 = 0; q4 < TC_NH / 4; ++q4) {                // four walkers (32 columns) at a time
-                    float t1[2][16], t2[2][16];                         // [l0][4 walker + 2 (row + 8) + re/im]
+                for (int l = 0; l < 2; ++l) {
+                    tc_ld16x256x2(trow + ((uint32_t)(16 * l) << 16) + TC_N, t2[0][l]);
+                    tc_ld16x256x2(trow + ((uint32_t)(16 * l) << 16), t1[0][l]);
+                }
 #pragma unroll
-                    for (int l = 0; l < 2; ++l) {
-                        tc_ld16x256(trow + ((uint32_t)(16 * l) << 16) + TC_N + 32 * q4, t2[l]);
-                        tc_ld16x256(trow + ((uint32_t)(16 * l) << 16) + 32 * q4, t1[l]);
-                    }
+                for (int q2 = 0; q2 < TC_NH / 2; ++q2) {
                     tc_wait_ld();
-                    if (q4 == TC_NH / 4 - 1) {                          // the last columns of the buffer are in registers
+                    if (q2 + 1 < TC_NH / 2) {
+#pragma unroll
+                        for (int l = 0; l < 2; ++l) {
+                            tc_ld16x256x2(trow + ((uint32_t)(16 * l) << 16) + TC_N + 16 * (q2 + 1), t2[(q2 + 1) & 1][l]);
+                            tc_ld16x256x2(trow + ((uint32_t)(16 * l) << 16) + 16 * (q2 + 1), t1[(q2 + 1) & 1][l]);
+                        }
+                    } else {                                            // the last columns of the buffer are in registers
                         tc_fence_before();
                         mbar_arrive(&tmem_free[buf]);
                     }
 #pragma unroll
                     for (int l = 0; l < 2; ++l)
 #pragma unroll
-                        for (int i = 0; i < 16; ++i) t2[l][i] = __shfl_sync(0xffffffffu, t2[l][i], partner);
+                        for (int i = 0; i < 8; ++i) t2[q2 & 1][l][i] = __shfl_sync(0xffffffffu, t2[q2 & 1][l][i], partner);
 #pragma unroll
-                    for (int wl = 0; wl < 4; ++wl) {
+                    for (int wl = 0; wl < 2; ++wl) {
                         float sr = 0.f, si = 0.f;
 #pragma unroll
                         for (int l = 0; l < 2; ++l)
 #pragma unroll
                             for (int h = 0; h < 2; ++h) {
-                                const float ar = t1[l][4 * wl + 2 * h], ai = t1[l][4 * wl + 2 * h + 1];
-                                const float pr = t2[l][4 * wl + 2 * h], pi = t2[l][4 * wl + 2 * h + 1];
+                                const float ar = t1[q2 & 1][l][4 * wl + 2 * h], ai = t1[q2 & 1][l][4 * wl + 2 * h + 1];
+                                const float pr = t2[q2 & 1][l][4 * wl + 2 * h], pi = t2[q2 & 1][l][4 * wl + 2 * h + 1];
                                 sr = fmaf(ar, pr, sr); sr = fmaf(-ai, pi, sr);
                                 si = fmaf(ar, pi, si); si = fmaf(ai, pr, si);
                             }
-                        xr64[4 * q4 + wl] += (double)sr; xi64[4 * q4 + wl] += (double)si;
+                        xr64[2 * q2 + wl] += (double)sr; xi64[2 * q2 + wl] += (double)si;
                     }
                 }
             }
