@@ -609,8 +609,14 @@ def test_exchange_3m_and_4m_kernels_against_the_oracle(kw):
 
 
 @pytest.mark.parametrize("kw", [dict(mesh=(2, 2, 1), m=6, n=4, nchol=10, nw=4), dict(mesh=(2, 3, 1), m=5, n=3, nchol=7, nw=5),
-                                dict(mesh=(1, 2, 2), m=9, n=1, nchol=5, nw=2), dict(mesh=(3, 1, 1), m=26, n=4, nchol=18, nw=7)],
-                         ids=["n4", "n3_odd", "n1_two_walkers", "m26_seven_walkers"])
+                                dict(mesh=(1, 2, 2), m=9, n=1, nchol=5, nw=2), dict(mesh=(3, 1, 1), m=26, n=4, nchol=18, nw=7),
+                                # the tcgen05 kernel's pipeline: two and three row tiles (the tiles alternate between two pairs of
+                                # issuing threads and two accumulator buffers), two walker groups of 16 with one walker in the second,
+                                # K-blocks with one k-step left over, three and four K-blocks, 8-walker images
+                                dict(mesh=(2, 1, 1), m=17, n=4, nchol=40, nw=17), dict(mesh=(1, 2, 1), m=33, n=2, nchol=70, nw=9),
+                                dict(mesh=(1, 1, 2), m=50, n=4, nchol=33, nw=3)],
+                         ids=["n4", "n3_odd", "n1_two_walkers", "m26_seven_walkers", "two_tiles_17_walkers", "three_tiles_three_kblocks",
+                              "four_kblocks"])
 def test_mixed_precision_exchange_against_the_oracle(kw):
     """Option exchange_precision, the analogue of the paper's single-precision mode and of the north_star's
     optional complex64 path (tolerance 1e-4), on BOTH kernels: the tcgen05 / TMEM one (exchange_tc.cu, default) and the
