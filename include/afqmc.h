@@ -67,7 +67,8 @@ enum {
     AFQMC_INVALID_ARGUMENT = 1, /* null pointer, nw < 0 or > max_walkers, bad dims, bad order */
     AFQMC_UNSUPPORTED = 2,      /* precision > 1, open shell or block calls with precision 1 ...   */
     AFQMC_CUDA_ERROR = 3,       /* a CUDA runtime call or launch failed                       */
-    AFQMC_OUT_OF_MEMORY = 4     /* device allocation failed                                   */
+    AFQMC_OUT_OF_MEMORY = 4,    /* device allocation failed                                   */
+    AFQMC_SCRATCH_LIMIT = 5     /* afqmc_overlap_noalloc: the call needs more than the static scratch array holds */
 }/*
  * Open shell (closed_shell = 0; Eq. 36 / Eq. 49 with their explicit spin sums).  Two spin channels
  * with n (spin up) and n_dn (spin down) occupied orbitals per k-point, N_up = Nk*n, N_dn = Nk*n_dn.  Every per-walker array
@@ -297,6 +298,28 @@ int afqmc_stage_times(afqmc_ctx* ctx, float* ms /* host, [AFQMC_NUM_STAGES] */);
  * returns the achieved TFLOP/s in *tflops (host).  Synchronous.
  */
 int afqmc_probe_fp64(int kind, int iters, double* tflops);
+
+/*
+ * a1+a2 WITHOUT any allocation and without a context, for callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it): the same result as afqmc_overlap -- logdet[w] = log det O_w,
+ * O_w = A^dagger Phi_w (PAPER.md:142 Eq. 27-28, :135-146), LU with partial pivoting, arg in (-pi, pi], info[w] as above --
+ * from caller-passed inputs.  Only g, m, n, closed_shell (must be 1) and precision (must be 0) of `dims` are read.
+ *   psi_t [Nk][m][n] device complex128; phi [nw][M][N] device complex128; logdet [nw] device complex128; info [nw] device
+ *   int32 or NULL.  Asynchronous on `stream`.
+ * The matrices O_w (nw * N * (N|1) * 16 bytes, see afqmc_overlap_noalloc_bytes) live in ONE static device array of
+ * afqmc_overlap_noalloc_max_bytes() = 16 MiB inside the library (every GPU that loads the library holds it until exit); the
+ * call runs no cudaMalloc, cudaFree or allocating library routine.  A call that needs more, or N > 1024, returns
+ * AFQMC_SCRATCH_LIMIT and launches nothing (all five configs of the paper's workloads fit: C3 6.0 MB, C5 8.4 MB).
+ * The array is shared by every call and keeps the last call's contents; the kernel writes every element it later reads, so
+ * nothing needs clearing.  Calls that overlap on the GPU (two streams, parallel graph branches) RACE on it: serialise them.
+ * The array's device address is resolved once per device on the first call there (cudaGetSymbolAddress, no allocation);
+ * afqmc_overlap_noalloc_setup() does just that for the current device, e.g. before a graph capture starts.
+ */
+size_t afqmc_overlap_noalloc_max_bytes(void);
+size_t afqmc_overlap_noalloc_bytes(const afqmc_dims* dims, int nw);   /* host arithmetic only; 0 for invalid dims */
+int afqmc_overlap_noalloc_setup(void);
+int afqmc_overlap_noalloc(const afqmc_dims* dims, const void* psi_t, const void* phi, int nw, void* logdet, int* info,
+                          void* stream);
 
 #ifdef __cplusplus
 }

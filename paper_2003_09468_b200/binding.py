@@ -15,7 +15,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libafqmc.so")
 _lib = None
 
-ERRORS = {0: "ok", 1: "invalid argument", 2: "unsupported configuration", 3: "CUDA error", 4: "out of device memory"}
+ERRORS = {0: "ok", 1: "invalid argument", 2: "unsupported configuration", 3: "CUDA error", 4: "out of device memory",
+          5: "request exceeds the static scratch array of the no-allocation entry point"}
 
 
 class AfqmcError(RuntimeError):
@@ -34,7 +35,8 @@ EXPORTS = ["afqmc_strerror", "afqmc_create", "afqmc_destroy", "afqmc_overlap", "
            "afqmc_vhs", "afqmc_propagate", "afqmc_local_energy", "afqmc_step", "afqmc_step_host",
            "afqmc_launch_count", "afqmc_exchange_flops", "afqmc_force_bias_flops", "afqmc_set_option", "afqmc_stage_times", "afqmc_probe_fp64",
            "afqmc_set_onebody", "afqmc_apply_onebody", "afqmc_hybrid_weight", "afqmc_orthogonalize",
-           "afqmc_mixed_estimator", "afqmc_block"]
+           "afqmc_mixed_estimator", "afqmc_block",
+           "afqmc_overlap_noalloc", "afqmc_overlap_noalloc_setup", "afqmc_overlap_noalloc_bytes", "afqmc_overlap_noalloc_max_bytes"]
 
 
 def lib():
@@ -75,8 +77,15 @@ def lib():
     L.afqmc_orthogonalize.argtypes = [vp, vp, ci, vp, vp, vp]
     L.afqmc_mixed_estimator.argtypes = [vp, vp, vp, ci, vp, vp]
     L.afqmc_block.argtypes = [vp, vp, vp, vp, cd, ci, ci, ci, vp, vp, vp, vp, vp]
+    L.afqmc_overlap_noalloc.argtypes = [ctypes.POINTER(Dims), vp, vp, ci, vp, vp, vp]
+    L.afqmc_overlap_noalloc_setup.argtypes = []
+    L.afqmc_overlap_noalloc_bytes.argtypes = [ctypes.POINTER(Dims), ci]
+    L.afqmc_overlap_noalloc_bytes.restype = ctypes.c_size_t
+    L.afqmc_overlap_noalloc_max_bytes.argtypes = []
+    L.afqmc_overlap_noalloc_max_bytes.restype = ctypes.c_size_t
     for name in EXPORTS:
-        if name not in ("afqmc_strerror", "afqmc_destroy", "afqmc_launch_count", "afqmc_exchange_flops", "afqmc_force_bias_flops"):
+        if name not in ("afqmc_strerror", "afqmc_destroy", "afqmc_launch_count", "afqmc_exchange_flops", "afqmc_force_bias_flops",
+                        "afqmc_overlap_noalloc_bytes", "afqmc_overlap_noalloc_max_bytes"):
             getattr(L, name).restype = ci
     _lib = L
     return L
@@ -101,6 +110,37 @@ def _ptr(t, dtype=None, optional=False):
 def _check(code, where):
     if code != 0:
         raise AfqmcError(code, where)
+
+
+def overlap_noalloc_max_bytes() -> int:
+    return int(lib().afqmc_overlap_noalloc_max_bytes())
+
+
+def overlap_noalloc_bytes(mesh, m, n, nw) -> int:
+    d = Dims((ctypes.c_int * 3)(*[int(g) for g in mesh]), int(m), int(n), 0, 1, 0, int(nw), 0)
+    return int(lib().afqmc_overlap_noalloc_bytes(ctypes.byref(d), int(nw)))
+
+
+def overlap_noalloc_setup():
+    """Resolves the static scratch array's device address on the current device (e.g. before a graph capture)."""
+    _check(lib().afqmc_overlap_noalloc_setup(), "afqmc_overlap_noalloc_setup")
+
+
+def overlap_noalloc(mesh, m, n, psi_t, phi, logdet, info=None):
+    """afqmc_overlap_noalloc: log det of the trial-walker overlaps with NO allocation anywhere (no context; the matrices live
+    in the library's static 16 MiB device array).  The caller passes inputs AND outputs: psi_t [Nk][m][n], phi [nw][M][N],
+    logdet [nw] complex128 CUDA tensors, info [nw] int32 or None.  Raises AfqmcError (code 5) beyond the scratch limit."""
+    nk = int(mesh[0]) * int(mesh[1]) * int(mesh[2])
+    nw = int(phi.shape[0])
+    for t, shape, dt, name in ((psi_t, (nk, m, n), torch.complex128, "psi_t"), (phi, (nw, nk * m, nk * n), torch.complex128, "phi"),
+                               (logdet, (nw,), torch.complex128, "logdet")) + (((info, (nw,), torch.int32, "info"),) if info is not None else ()):
+        if not t.is_cuda or t.device != phi.device or tuple(t.shape) != tuple(shape) or t.dtype != dt:
+            raise ValueError("%s: expected a %s CUDA tensor of shape %s on %s" % (name, dt, tuple(shape), phi.device))
+    d = Dims((ctypes.c_int * 3)(*[int(g) for g in mesh]), int(m), int(n), 0, 1, 0, nw, 0)
+    with torch.cuda.device(phi.device):
+        _check(lib().afqmc_overlap_noalloc(ctypes.byref(d), _ptr(psi_t), _ptr(phi), nw, _ptr(logdet), _ptr(info, optional=True), _stream()),
+               "afqmc_overlap_noalloc")
+    return logdet, info
 
 
 def probe_fp64(kind: int, iters: int = 20000) -> float:

@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libafqmc.so")
-SOURCES = ["context.cu", "green.cu", "force_bias.cu", "vhs.cu", "propagate.cu", "energy.cu", "exchange3m.cu", "exchange_tf32.cu", "exchange_tc.cu", "step.cu", "openshell.cu", "block.cu", "boundary32.cu", "probe.cu"]
+SOURCES = ["context.cu", "green.cu", "force_bias.cu", "vhs.cu", "propagate.cu", "energy.cu", "exchange3m.cu", "exchange_tf32.cu", "exchange_tc.cu", "step.cu", "openshell.cu", "block.cu", "boundary32.cu", "probe.cu", "overlap_noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 

@@ -16,6 +16,7 @@ AFQMC_API const char* afqmc_strerror(int code) {
         case AFQMC_UNSUPPORTED: return "unsupported configuration";
         case AFQMC_CUDA_ERROR: return "CUDA error";
         case AFQMC_OUT_OF_MEMORY: return "out of device memory";
+        case AFQMC_SCRATCH_LIMIT: return "request exceeds the static scratch array of the no-allocation entry point";
         default: return "unknown error code";
     }
 }
