@@ -312,18 +312,41 @@ def run_ours(args):
         dt = time.perf_counter() - t0
         if i >= max(1, args.warmup // 2):
             e2e_t += dt
-    sampler.stop()
     assert np.array_equal(e_h.numpy(), e_dev), "host-entry step disagrees with the device step"
+    # the same through the pipelined host entry (afqmc_step_host_begin / _end, two steps in flight): every step uploads its
+    # walkers and fields from pinned memory and downloads the propagated walkers, energies, log det and info; the upload of a
+    # step overlaps the kernels of the step before it.  K steps, one timed region from the first begin to the last end.
+    outs = [(torch.empty_like(phi_h0).pin_memory(), torch.empty_like(e_h).pin_memory(), torch.empty_like(ld_h).pin_memory(),
+             torch.empty_like(info_h).pin_memory()) for _ in range(2)]
+
+    def run_pipelined(nsteps):
+        for i in range(nsteps):
+            o = outs[i & 1]
+            ctx.step_host_begin(i & 1, phi_h0, x_h, cfg.dtau, cfg.order, o[0], o[1], o[2], o[3])
+        ctx.step_host_end(0)
+        ctx.step_host_end(1)
+
+    run_pipelined(max(2, args.warmup))
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    run_pipelined(args.steps)
+    e2e_pipe_t = time.perf_counter() - t0
+    sampler.stop()
+    for o in outs[:min(2, args.steps)]:
+        assert np.array_equal(o[1].numpy(), e_dev), "pipelined host-entry step disagrees with the device step"
+        assert torch.equal(o[0], phi_h), "pipelined host-entry walkers disagree with the synchronous host-entry walkers"
     h2d = phi_h.numel() * 16 + x_h.numel() * 8
     d2h = phi_h.numel() * 16 + e_h.numel() * 16 + ld_h.numel() * 16 + info_h.numel() * 4
 
     # max over ranks (the only torch.distributed traffic of the run besides the barriers)
     dev_ms_max = replicas.max_over_ranks(dev_ms, device="cuda")
     e2e_ms_max = replicas.max_over_ranks(e2e_t * 1e3, device="cuda")
+    e2e_pipe_ms_max = replicas.max_over_ranks(e2e_pipe_t * 1e3, device="cuda")
 
     if rank == 0:
         value = replicas.aggregate_throughput(nw, args.steps, world, dev_ms_max)
-        e2e_value = replicas.aggregate_throughput(nw, args.steps, world, e2e_ms_max)
+        e2e_sync_value = replicas.aggregate_throughput(nw, args.steps, world, e2e_ms_max)
+        e2e_value = replicas.aggregate_throughput(nw, args.steps, world, e2e_pipe_ms_max)
         # ---- roofline of the dominant kernel (exchange contraction, a9) ----
         ex_ms = stage_acc["exchange"] / args.steps
         ex_flops = ex_flops_default
@@ -389,7 +412,13 @@ def run_ours(args):
                              % (pb.L.nbytes / 1e9, 2 * cfg.nk ** 2 * cfg.n * cfg.nchol * cfg.m * 16 / 1e9,
                                 nw * cfg.M ** 2 * 16 / 1e9),
                        "parallelism": "replicas x%d (walkers sharded by rank, no collective)" % world},
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "call": "afqmc_step_host_begin / afqmc_step_host_end, two steps in flight: every step uploads phi and x from "
+                            "pinned host memory and downloads phi', energy, logdet, info; the upload of step i+1 runs during the "
+                            "kernels of step i; host wall clock over the K steps",
+                    "ms_per_step": e2e_pipe_ms_max / args.steps,
+                    "one_step_at_a_time": {"value": e2e_sync_value, "ms_per_step": e2e_ms_max / args.steps,
+                                           "call": "afqmc_step_host (returns when the step's results are in the host buffers)"}},
             "gpu_launches": int(launches),
             "clocks": sampler.summary(),
             "roofline": roofline,

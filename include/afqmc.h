@@ -300,6 +300,23 @@ int afqmc_stage_times(afqmc_ctx* ctx, float* ms /* host, [AFQMC_NUM_STAGES] */);
 int afqmc_probe_fp64(int kind, int iters, double* tflops);
 
 /*
+ * Pipelined host entry: the same step on HOST buffers with up to TWO steps in flight (slot = 0 or 1), for loops that feed one
+ * batch of walkers after the other.  afqmc_step_host_begin enqueues everything and returns without waiting: the upload of
+ * phi and x (on a stream of the context, so it runs while the kernels of the other slot's step are still busy on `stream`),
+ * the step on `stream`, the download of phi' into phi_out_host (may be phi_host itself) during the energy evaluation, and the
+ * downloads of energy / logdet / info.  afqmc_step_host_end blocks until everything of that slot has arrived in the host
+ * buffers (no-op for an idle slot); begin on a busy slot completes the slot's previous step first.  The kernels of the two
+ * steps share the context's workspace and run one after the other; what overlaps is the host-link traffic.  Results are
+ * bitwise those of afqmc_step_host.  Slot 1 allocates a second set of staging buffers (the size of phi, x and the results for
+ * max_walkers) on its first use.  Host buffers must stay valid and untouched from begin to the matching end and should be
+ * pinned (with pageable memory the copies serialise with the caller).  Use the same `stream` for both slots.
+ * precision = 1: AFQMC_UNSUPPORTED.
+ */
+int afqmc_step_host_begin(afqmc_ctx* ctx, int slot, const void* phi_host, const double* x_host, double dtau, int order,
+                          int nw, void* phi_out_host, void* energy_host, void* logdet_host, int* info_host, void* stream);
+int afqmc_step_host_end(afqmc_ctx* ctx, int slot);
+
+/*
  * a1+a2 WITHOUT any allocation and without a context, for callers that cannot call cudaMalloc (code under CUDA graph
  * capture, tight serving loops, harnesses that forbid it): the same result as afqmc_overlap -- logdet[w] = log det O_w,
  * O_w = A^dagger Phi_w (PAPER.md:142 Eq. 27-28, :135-146), LU with partial pivoting, arg in (-pi, pi], info[w] as above --

@@ -36,6 +36,7 @@ EXPORTS = ["afqmc_strerror", "afqmc_create", "afqmc_destroy", "afqmc_overlap", "
            "afqmc_launch_count", "afqmc_exchange_flops", "afqmc_force_bias_flops", "afqmc_set_option", "afqmc_stage_times", "afqmc_probe_fp64",
            "afqmc_set_onebody", "afqmc_apply_onebody", "afqmc_hybrid_weight", "afqmc_orthogonalize",
            "afqmc_mixed_estimator", "afqmc_block",
+           "afqmc_step_host_begin", "afqmc_step_host_end",
            "afqmc_overlap_noalloc", "afqmc_overlap_noalloc_setup", "afqmc_overlap_noalloc_bytes", "afqmc_overlap_noalloc_max_bytes"]
 
 
@@ -77,6 +78,8 @@ def lib():
     L.afqmc_orthogonalize.argtypes = [vp, vp, ci, vp, vp, vp]
     L.afqmc_mixed_estimator.argtypes = [vp, vp, vp, ci, vp, vp]
     L.afqmc_block.argtypes = [vp, vp, vp, vp, cd, ci, ci, ci, vp, vp, vp, vp, vp]
+    L.afqmc_step_host_begin.argtypes = [vp, ci, vp, vp, cd, ci, ci, vp, vp, vp, vp, vp]
+    L.afqmc_step_host_end.argtypes = [vp, ci]
     L.afqmc_overlap_noalloc.argtypes = [ctypes.POINTER(Dims), vp, vp, ci, vp, vp, vp]
     L.afqmc_overlap_noalloc_setup.argtypes = []
     L.afqmc_overlap_noalloc_bytes.argtypes = [ctypes.POINTER(Dims), ci]
@@ -355,6 +358,22 @@ class Afqmc:
                           self._host(logdet_host, (nw,), self.cdtype, "logdet_host", optional=True),
                           self._host(info_host, (nw,), torch.int32, "info_host", optional=True)), "afqmc_step_host")
         return energy_host
+
+    def step_host_begin(self, slot, phi_host, x_host, dtau, order, phi_out_host, energy_host, logdet_host=None, info_host=None):
+        """Pipelined host step (two slots): enqueues upload, step and downloads and returns at once; step_host_end(slot) waits."""
+        nw = self._nw(phi_host, "phi_host")
+        with torch.cuda.device(self.device):
+            _check(lib().afqmc_step_host_begin(self._h, int(slot), self._host(phi_host, self._phi_shape(nw), self.cdtype, "phi_host"),
+                                               self._host(x_host, (nw, self.nk, self.nchol), self.rdtype, "x_host"), float(dtau),
+                                               int(order), nw, self._host(phi_out_host, self._phi_shape(nw), self.cdtype, "phi_out_host"),
+                                               self._host(energy_host, (nw, 3), self.cdtype, "energy_host"),
+                                               self._host(logdet_host, (nw,), self.cdtype, "logdet_host", optional=True),
+                                               self._host(info_host, (nw,), torch.int32, "info_host", optional=True), _stream()),
+                   "afqmc_step_host_begin")
+
+    def step_host_end(self, slot):
+        with torch.cuda.device(self.device):
+            _check(lib().afqmc_step_host_end(self._h, int(slot)), "afqmc_step_host_end")
 
     # ---- the AFQMC block (include/afqmc.h "The AFQMC block") ----------------------------------------
     def set_onebody(self, h1p, dtau, b1_out=None):

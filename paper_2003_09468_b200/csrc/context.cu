@@ -157,6 +157,13 @@ AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     for (cudaEvent_t e : c->ev_copy)
         if (e) cudaEventDestroy(e);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->copyin_stream) cudaStreamDestroy(c->copyin_stream);
+    for (int s = 0; s < 2; ++s)
+        for (cudaEvent_t e : c->ev_pipe[s])
+            if (e) cudaEventDestroy(e);
+    void* pipe_ptrs[] = {c->pipe_phi, c->pipe_x, c->pipe_energy, c->pipe_logdet, c->pipe_info};
+    for (void* p : pipe_ptrs)
+        if (p) cudaFree(p);
     delete c;
 }
 
