@@ -30,10 +30,10 @@ if ROOT not in sys.path:
 METRIC = "walker-steps/s incl. local energy"
 UNIT = "walker-steps/s"
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE exchange-kernel launch, from the committed
-# `ncu --set full` capture of the default exchange kernel (profiles/r02c_ncu_exchange.md names the command); bench.py
-# cannot measure DRAM traffic itself.  Only the configuration that was captured has a value.
-EXCHANGE_DRAM_TRAFFIC = {"C3": {"bytes": 989.908e6 + 9.361e6, "source": "profiles/r02c_ncu_exchange.md"}}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE exchange-kernel launch, from the committed ncu capture of the default
+# exchange kernel (profiles/r02i_summary.md names the command; the `--set full` capture of the same kernel one commit earlier
+# is profiles/r02c_ncu_exchange.md); bench.py cannot measure DRAM traffic itself.  Only the configuration that was captured has a value.
+EXCHANGE_DRAM_TRAFFIC = {"C3": {"bytes": 909.450e6 + 8.798e6, "source": "profiles/r02i_exchange_dram.csv (command: profiles/r02i_summary.md)"}}
 
 
 def load_measured_peaks():

@@ -690,6 +690,10 @@ __global__ void __launch_bounds__(64) __maxnreg__(MAXREG) exchange3m_reg_kernel(
         return reinterpret_cast<const double2*>(Lx3t) + ((it.blk * NAG + grp) * GQ) * (size_t)TASK + lane;
     };
     // bulk copies of this warp's raw theta block of `it` into buffer `b` (rows of padded walkers are not fetched)
+    // Theta (38.8 MB at C3) is re-read in full once per Q pair while the 393 MB operand stream passes through L2 between two
+    // visits; evict_last keeps its lines ahead of the stream's dead blocks (DRAM read per launch at C3: 985 -> 909 MB,
+    // profiles/r02i_exchange_dram.md; no change in time, the kernel is bound by the FP64 pipe)
+    const uint64_t theta_policy = l2_policy_evict_last();
     auto issue_theta = [&](const Item& it, int b) {
         const int nvalid = min(NWC, nw - it.w0) * d.n;
         uint64_t* bar = &mbar[h * 2 + b];
@@ -698,9 +702,9 @@ __global__ void __launch_bounds__(64) __maxnreg__(MAXREG) exchange3m_reg_kernel(
         double2* dst = raw + (h * 2 + b) * raw_len;
         for (int row = lane; row < nvalid; row += 32) {
             const int wl = row / d.n, orb = row - wl * d.n;
-            bulk_g2s(dst + (size_t)row * d.m,
-                     theta + ((size_t)(it.w0 + wl) * d.N + it.rowblk * d.n + orb) * d.M + (size_t)it.colblk * d.m,
-                     (uint32_t)(d.m * 16), bar);
+            bulk_g2s_hint(dst + (size_t)row * d.m,
+                          theta + ((size_t)(it.w0 + wl) * d.N + it.rowblk * d.n + orb) * d.M + (size_t)it.colblk * d.m,
+                          (uint32_t)(d.m * 16), bar, theta_policy);
         }
     };
 

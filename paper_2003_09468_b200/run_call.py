@@ -1,7 +1,7 @@
 """Runs ONE C-ABI call of the step a few times on a synthetic config: the command line that the ncu captures under
 `profiles/` name (a whole `bench.py` run replays every kernel ~40 times under `ncu --set full`; this runs just the call).
 
-  python -m paper_2003_09468_b200.run_call --config C3 --call local_energy --reps 2 [--option exchange_regb=2 ...]
+  python -m paper_2003_09468_b200.run_call --config C3 --call local_energy --reps 2 [--walkers 8] [--option exchange_regb=2 ...]
 
 calls: green, force_bias, vhs, propagate, local_energy, step.  Inputs: `synth.make_problem` of the config (seeded); Theta
 is the Green's function of the config's walkers; nothing here is timed or checked (tests/ and bench.py do that).
@@ -21,6 +21,7 @@ def main():
     ap.add_argument("--call", default="local_energy", choices=["green", "force_bias", "vhs", "propagate", "local_energy", "step"])
     ap.add_argument("--reps", type=int, default=2)
     ap.add_argument("--precision", type=int, default=0)
+    ap.add_argument("--walkers", type=int, default=0, help="use only the first N walkers of the config (0 = all)")
     ap.add_argument("--option", action="append", default=[], help="name=value, passed to afqmc_set_option")
     a = ap.parse_args()
     cfg = synth.CONFIGS[a.config]
@@ -31,8 +32,9 @@ def main():
         ctx.set_option(k, int(v))
     cd = torch.complex64 if a.precision == 1 else torch.complex128
     rd = torch.float32 if a.precision == 1 else torch.float64
-    phi = torch.from_numpy(pb.phi.copy()).cuda().to(cd)
-    x = torch.from_numpy(pb.x).cuda().to(rd)
+    nw = a.walkers if a.walkers > 0 else pb.phi.shape[0]
+    phi = torch.from_numpy(pb.phi[:nw].copy()).cuda().to(cd)
+    x = torch.from_numpy(pb.x[:nw].copy()).cuda().to(rd)
     theta, _, _ = ctx.green(phi)
     vb = ctx.force_bias(theta)
     vhs = ctx.vhs(x, vb, cfg.dtau) if a.call in ("vhs", "propagate") else None
