@@ -6,6 +6,7 @@
 // Gauss-Jordan elimination with partial (row) pivoting -- the same pivot sequence as an LU with
 // partial pivoting, so det O = sign * prod(pivots).  The transposed inverse goes to workspace and
 // Theta = (Phi O^{-1})^T = O^{-T} Phi^T (Eq. 30) is one batched DMMA GEMM.
+#include <type_traits>
 #include <cooperative_groups.h>
 #include <math_constants.h>
 #include "zgemm.cuh"
@@ -224,6 +225,35 @@ __global__ void __launch_bounds__(32 * NWARP, 1) overlap_inverse_reg_kernel(
 
     // ---- a1: O[(k,a)][c] = sum_p conj(A_k[p][a]) Phi[(k,p)][c] for my rows x my columns ----
     double2 a[RT][CT];
+    if (RT * CT <= 8) {
+        // few elements per thread (wide clusters): the RT row slots advance together, so that the loads of one p for all of
+        // them are in flight at once (the phase is latency-bound: one row slot after the other took a quarter of the kernel at C3)
+        const double2* Ab[RT];
+        const double2* Pb[RT];
+        bool ok[RT];
+#pragma unroll
+        for (int t = 0; t < RT; ++t) {
+#pragma unroll
+            for (int cc = 0; cc < CT; ++cc) a[t][cc] = make_double2(0.0, 0.0);
+            const int i = lane + 32 * t;
+            ok[t] = i < N && c0 < N;
+            const int k = ok[t] ? i / d.n : 0, aa = ok[t] ? i - k * d.n : 0;
+            Ab[t] = psi_t + (size_t)k * d.m * d.n + aa;
+            Pb[t] = ph + (size_t)k * d.m * N + (c0 < N ? c0 : 0);
+        }
+#pragma unroll 2
+        for (int p = 0; p < d.m; ++p) {
+#pragma unroll
+            for (int t = 0; t < RT; ++t) {
+                if (!ok[t]) continue;
+                double2 av = __ldg(Ab[t] + (size_t)p * d.n);
+                av.y = -av.y;
+#pragma unroll
+                for (int cc = 0; cc < CT; ++cc)
+                    if (c0 + cc < N) a[t][cc] = cfma(av, __ldg(Pb[t] + (size_t)p * N + cc), a[t][cc]);
+            }
+        }
+    } else {
 #pragma unroll
     for (int t = 0; t < RT; ++t) {
 #pragma unroll
@@ -242,6 +272,7 @@ __global__ void __launch_bounds__(32 * NWARP, 1) overlap_inverse_reg_kernel(
                     if (c0 + cc < N) a[t][cc] = cfma(av, __ldg(Pb + (size_t)p * N + cc), a[t][cc]);
             }
         }
+    }
     }
     if (tid == 0) sh.info = 0;
     unsigned used = 0;                                 // bit t: my row lane+32t has been a pivot row
@@ -271,12 +302,16 @@ __global__ void __launch_bounds__(32 * NWARP, 1) overlap_inverse_reg_kernel(
                     if (mag > bv) { bv = mag; bi = i; }
                 }
             }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                const double ov = __shfl_xor_sync(0xffffffffu, bv, o);
-                const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-                if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-            }
+            // largest modulus over the warp, smallest row index on ties -- the same choice as a butterfly of (value, index)
+            // pairs, in three warp reductions on 32-bit keys: non-negative doubles order like their (high, low) words; a lane
+            // whose rows are all NaN has bv = -1 (class 1, below every number), a lane without candidate rows class 0
+            const unsigned hi = bv >= 0.0 ? (unsigned)__double2hiint(bv) + 2u : (bv == -1.0 ? 1u : 0u);
+            const unsigned mh = __reduce_max_sync(0xffffffffu, hi);
+            const bool c1 = hi == mh;
+            const unsigned lo = (unsigned)__double2loint(bv);
+            const unsigned ml = __reduce_max_sync(0xffffffffu, c1 ? lo : 0u);
+            const bool c2 = c1 && lo == ml;
+            bi = (int)__reduce_min_sync(0xffffffffu, c2 ? (unsigned)bi : 0x7fffffffu);
             const int p = bi, pl = p & 31, pt = p >> 5;
             double2 pvl = col[0];
 #pragma unroll
@@ -286,9 +321,18 @@ __global__ void __launch_bounds__(32 * NWARP, 1) overlap_inverse_reg_kernel(
             pv.y = __shfl_sync(0xffffffffu, pvl.y, pl);
             const double den = pv.x * pv.x + pv.y * pv.y;
             const bool ok = den > 0.0;
-            const double2 ip = ok ? make_double2(pv.x / den, -pv.y / den) : make_double2(0.0, 0.0);
+            const double rden = 1.0 / den;
+            const double2 ip = ok ? make_double2(pv.x * rden, -pv.y * rden) : make_double2(0.0, 0.0);
+            // what the update multiplies the scaled pivot row with: minus the column, and 0 in the pivot row itself (whose new
+            // value is the scaled pivot row: the update below computes 0 * r + r there)
+#pragma unroll
+            for (int t = 0; t < RT; ++t) {
+                const bool isp = (lane == pl) && (t == pt);
+                col[t].x = isp ? 0.0 : -col[t].x;
+                col[t].y = isp ? 0.0 : -col[t].y;
+            }
             // publish to every CTA of the cluster
-#pragma unroll 1
+#pragma unroll(CS <= 4 ? CS : 1)
             for (int q = 0; q < CS; ++q) {
                 GJRegShared<RT, CT>* dst = &sh;
                 if (CS > 1) dst = cg::this_cluster().map_shared_rank(&sh, q);
@@ -307,37 +351,48 @@ __global__ void __launch_bounds__(32 * NWARP, 1) overlap_inverse_reg_kernel(
             if (sh.zero[buf] && sh.info == 0) sh.info = j + 1;
         }
         if (lane == pl) used |= 1u << pt;
-        // scaled pivot row for my columns: r[cc] = a[p][c] / pivot  (column j itself -> 1/pivot)
+        // scaled pivot row for my columns: r[cc] = a[p][c] / pivot  (column j itself -> 1/pivot).  The register slot pt of the
+        // pivot row is the same for every thread, so the slot is picked by a branch (no per-slot selects), and the lane that
+        // owns the pivot row takes r as its new row there (its multiplier was published as 0)
         double2 r[CT];
+        const bool own_col = gw == jw;
+        auto pivot_row = [&](auto tc) {
+            constexpr int t = decltype(tc)::value;
+            if constexpr (t < RT) {
 #pragma unroll
-        for (int cc = 0; cc < CT; ++cc) {
-            double2 v = a[0][cc];
-#pragma unroll
-            for (int t = 1; t < RT; ++t) if (t == pt) v = a[t][cc];
-            v.x = __shfl_sync(0xffffffffu, v.x, pl);
-            v.y = __shfl_sync(0xffffffffu, v.y, pl);
-            r[cc] = cmul(v, ip);
-        }
-        if (gw == jw) {
+                for (int cc = 0; cc < CT; ++cc) {
+                    double2 v;
+                    v.x = __shfl_sync(0xffffffffu, a[t][cc].x, pl);
+                    v.y = __shfl_sync(0xffffffffu, a[t][cc].y, pl);
+                    r[cc] = cmul(v, ip);
+                    if (own_col && cc == tj) r[cc] = ip;
+                    if (lane == pl) a[t][cc] = r[cc];
+                }
+            }
+        };
+        if (own_col) {
 #pragma unroll
             for (int cc = 0; cc < CT; ++cc)
                 if (cc == tj) {
-                    r[cc] = ip;
 #pragma unroll
                     for (int t = 0; t < RT; ++t) a[t][cc] = make_double2(0.0, 0.0);
                 }
         }
+        switch (pt) {
+            case 0: pivot_row(std::integral_constant<int, 0>()); break;
+            case 1: pivot_row(std::integral_constant<int, 1>()); break;
+            case 2: pivot_row(std::integral_constant<int, 2>()); break;
+            case 3: pivot_row(std::integral_constant<int, 3>()); break;
+            case 4: pivot_row(std::integral_constant<int, 4>()); break;
+            case 5: pivot_row(std::integral_constant<int, 5>()); break;
+            case 6: pivot_row(std::integral_constant<int, 6>()); break;
+            default: pivot_row(std::integral_constant<int, 7>()); break;
+        }
 #pragma unroll
         for (int t = 0; t < RT; ++t) {
-            const bool isp = (lane == pl) && (t == pt);
-            double2 f = sh.f[buf][lane + 32 * t];
-            f.x = isp ? 0.0 : -f.x;
-            f.y = isp ? 0.0 : -f.y;
+            const double2 f = sh.f[buf][lane + 32 * t];
 #pragma unroll
-            for (int cc = 0; cc < CT; ++cc) {
-                const double2 u = cfma(f, r[cc], a[t][cc]);
-                a[t][cc] = isp ? r[cc] : u;
-            }
+            for (int cc = 0; cc < CT; ++cc) a[t][cc] = cfma(f, r[cc], a[t][cc]);
         }
     }
     if (CS > 1) cg::this_cluster().sync(); else __syncthreads();
