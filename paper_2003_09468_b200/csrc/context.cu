@@ -144,6 +144,7 @@ static int dev_alloc(T** p, size_t count) {
 
 AFQMC_API void afqmc_destroy(afqmc_ctx* c) {
     if (!c) return;
+    for (int slot = 0; slot < 2; ++slot) (void)afqmc_step_host_end(c, slot);      // pipelined host steps still in flight
     if (c->dn) { afqmc_destroy(c->dn); c->dn = nullptr; }
     if (c->is_child) c->b1 = nullptr;        // owned by the spin-up context
     void* ptrs[] = {c->kminus, c->kplus, c->kneg, c->units, c->psi_t, c->ht, c->Lh, c->Lxc, c->Lxr, c->Lx3t, c->Lx, c->LxT, c->LxU, c->Lf, c->Lff, c->Lv3, c->Lv3f, c->vunits,
