@@ -45,6 +45,13 @@ def test_create_rejects_bad_arguments_before_touching_cuda():
     lib.afqmc_destroy(None)
 
 
+def test_pipelined_host_entry_rejects_bad_arguments_before_touching_cuda():
+    from paper_2003_09468_b200 import binding
+    lib = binding.lib()
+    assert lib.afqmc_step_host_end(None, 0) == 1
+    assert lib.afqmc_step_host_begin(None, 0, None, None, 0.005, 6, 1, None, None, None, None, None) == 1
+
+
 def test_product_path_does_not_import_the_oracle():
     pkg = os.path.join(ROOT, "paper_2003_09468_b200")
     for dirpath, _, files in os.walk(pkg):
