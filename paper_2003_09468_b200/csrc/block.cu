@@ -520,6 +520,10 @@ AFQMC_API int afqmc_block(afqmc_ctx* c, void* phi, double* weight, const double*
         return AFQMC_INVALID_ARGUMENT;
     if (!c->b1_set) return AFQMC_INVALID_ARGUMENT;
     if (nw == 0) return AFQMC_OK;
+    // the block uses the result buffers of pipeline slot 0 (ws_logdet, ws_info): pipelined host steps are completed first
+    for (int slot = 0; slot < 2; ++slot)
+        if (c->pipe_busy[slot])
+            if (int prc = afqmc_step_host_end(c, slot)) return prc;
     const Dims& d = c->d;
     cudaStream_t st = (cudaStream_t)stream;
     double2* ph = (double2*)phi;

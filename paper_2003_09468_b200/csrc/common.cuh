@@ -134,7 +134,7 @@ struct afqmc_ctx {
     // afqmc_step_host_begin / _end: two steps in flight.  Slot 0 stages in ws_phi / ws_x / ws_energy / ws_logdet / ws_info,
     // slot 1 in a second set allocated on its first use; uploads run on copyin_stream, the walker download on copy_stream.
     cudaStream_t copyin_stream;
-    cudaEvent_t ev_pipe[2][4];   // per slot: inputs on the device | propagated walkers final | walkers downloaded | all results downloaded
+    cudaEvent_t ev_pipe[2][4];   // per slot: inputs on the device | propagated walkers final | step complete | all results downloaded
     double2* pipe_phi; double* pipe_x; double2* pipe_energy; double2* pipe_logdet; int* pipe_info;
     int pipe_busy[2];
     cudaEvent_t ev[AFQMC_NUM_STAGES + 1];

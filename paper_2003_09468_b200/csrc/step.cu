@@ -124,8 +124,7 @@ AFQMC_API int afqmc_step_host_end(afqmc_ctx* c, int slot) {
     if (!c || slot < 0 || slot > 1) return AFQMC_INVALID_ARGUMENT;
     if (!c->pipe_busy[slot]) return AFQMC_OK;
     c->pipe_busy[slot] = 0;
-    const cudaError_t e1 = cudaEventSynchronize(c->ev_pipe[slot][2]), e2 = cudaEventSynchronize(c->ev_pipe[slot][3]);
-    if (e1 != cudaSuccess || e2 != cudaSuccess) { (void)cudaGetLastError(); return AFQMC_CUDA_ERROR; }
+    if (cudaEventSynchronize(c->ev_pipe[slot][3]) != cudaSuccess) { (void)cudaGetLastError(); return AFQMC_CUDA_ERROR; }
     return AFQMC_OK;
 }
 
@@ -161,13 +160,16 @@ AFQMC_API int afqmc_step_host_begin(afqmc_ctx* c, int slot, const void* phi_host
         (void)cudaGetLastError();
         return rc;
     }
-    cudaError_t e = cudaStreamWaitEvent(c->copy_stream, ev[1], 0);
+    // every download runs on copy_stream, so that the caller's stream goes straight on to the next step's kernels: the
+    // walkers as soon as they are final (during the energy evaluation), the small results once the step is complete (ev[2])
+    cudaError_t e = cudaEventRecord(ev[2], st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(c->copy_stream, ev[1], 0);
     if (e == cudaSuccess) e = cudaMemcpyAsync(phi_out_host, phi_d, phi_bytes, cudaMemcpyDeviceToHost, c->copy_stream);
-    if (e == cudaSuccess) e = cudaEventRecord(ev[2], c->copy_stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(energy_host, en_d, (size_t)nw * 3 * sizeof(double2), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && logdet_host) e = cudaMemcpyAsync(logdet_host, ld_d, (size_t)nw * sizeof(double2), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && info_host) e = cudaMemcpyAsync(info_host, info_d, (size_t)nw * sizeof(int), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaEventRecord(ev[3], st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(c->copy_stream, ev[2], 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(energy_host, en_d, (size_t)nw * 3 * sizeof(double2), cudaMemcpyDeviceToHost, c->copy_stream);
+    if (e == cudaSuccess && logdet_host) e = cudaMemcpyAsync(logdet_host, ld_d, (size_t)nw * sizeof(double2), cudaMemcpyDeviceToHost, c->copy_stream);
+    if (e == cudaSuccess && info_host) e = cudaMemcpyAsync(info_host, info_d, (size_t)nw * sizeof(int), cudaMemcpyDeviceToHost, c->copy_stream);
+    if (e == cudaSuccess) e = cudaEventRecord(ev[3], c->copy_stream);
     if (e != cudaSuccess) {
         cudaStreamSynchronize(c->copyin_stream); cudaStreamSynchronize(c->copy_stream); cudaStreamSynchronize(st);
         (void)cudaGetLastError();
