@@ -30,10 +30,32 @@ if ROOT not in sys.path:
 METRIC = "walker-steps/s incl. local energy"
 UNIT = "walker-steps/s"
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE exchange-kernel launch, from the committed ncu capture of the default
-# exchange kernel (profiles/r02i_summary.md names the command; the `--set full` capture of the same kernel one commit earlier
-# is profiles/r02c_ncu_exchange.md); bench.py cannot measure DRAM traffic itself.  Only the configuration that was captured has a value.
-EXCHANGE_DRAM_TRAFFIC = {"C3": {"bytes": 909.450e6 + 8.798e6, "source": "profiles/r02i_exchange_dram.csv (command: profiles/r02i_summary.md)"}}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE exchange-kernel launch: bench.py cannot measure DRAM traffic itself, so
+# it reads the committed ncu capture of the default exchange kernel (a text file; profiles/r02i_summary.md names the command;
+# the `--set full` capture of the same kernel one commit earlier is profiles/r02c_ncu_exchange.md).  Only the configuration
+# that was captured has a value.
+EXCHANGE_DRAM_CAPTURES = {"C3": "profiles/r02i_exchange_dram.csv"}
+
+
+def exchange_dram_traffic(config_name):
+    """(bytes per launch, source) from the committed ncu CSV, or (None, None)."""
+    rel = EXCHANGE_DRAM_CAPTURES.get(config_name)
+    if not rel:
+        return None, None
+    try:
+        import csv
+        total, seen = 0.0, set()
+        with open(os.path.join(ROOT, rel), newline="") as f:
+            for row in csv.reader(f):
+                if len(row) >= 15 and row[12] in ("dram__bytes_read.sum", "dram__bytes_write.sum") and row[12] not in seen:
+                    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}[row[13]]
+                    total += float(row[14].replace(",", "")) * scale
+                    seen.add(row[12])
+        if len(seen) != 2:
+            return None, None
+        return total, rel + " (command: profiles/r02i_summary.md)"
+    except (OSError, KeyError, ValueError):
+        return None, None
 
 
 def load_measured_peaks():
@@ -365,9 +387,9 @@ def run_ours(args):
         roofline = {
             "kernel": "exchange (a9), afqmc_local_energy", "bound": "tensor", "achieved": achieved,
             "peak": peak_probe, "unit": "TFLOP/s", "frac": achieved / peak_probe,
-            "traffic": EXCHANGE_DRAM_TRAFFIC.get(cfg.name, {}).get("bytes"),
+            "traffic": exchange_dram_traffic(cfg.name)[0],
             "traffic_unit": "bytes per launch (DRAM read+write)",
-            "traffic_source": EXCHANGE_DRAM_TRAFFIC.get(cfg.name, {}).get("source"),
+            "traffic_source": exchange_dram_traffic(cfg.name)[1],
             "algorithmic_bytes": float(ctx_alg_bytes),
             "packed_operand_bytes": float(packed_bytes),
             "peak_source": "live FP64 DMMA.8x8x4 probe (afqmc_probe_fp64); MEASURED_PEAKS.json has no FP64 entry",
