@@ -399,7 +399,8 @@ __device__ __forceinline__ void x3_collect(const double2 (&keep)[NP][2], const d
         }
 }
 // end of a task: combine the three products, publish m-tile 1-KEEP in `xw` (buffer `buf`), keep m-tile KEEP, clear
-template <int NP, int KEEP>
+// PHASED: acc[0] and acc[1] already hold Re and Im (see task_async: the products were accumulated in two phases), nothing to combine
+template <int NP, int KEEP, bool PHASED = false>
 __device__ __forceinline__ void x3_publish(double (&acc)[3][2][NP][2], double2 (&keep)[NP][2], double2* __restrict__ xw, int h, int buf,
                                            const X3Lane& L) {
     constexpr int GIVE = 1 - KEEP;
@@ -407,8 +408,13 @@ __device__ __forceinline__ void x3_publish(double (&acc)[3][2][NP][2], double2 (
     for (int j = 0; j < NP; ++j)
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-            xw[j * 64 + L.sw[e]] = make_double2(acc[0][GIVE][j][e] - acc[2][GIVE][j][e], acc[0][GIVE][j][e] + acc[1][GIVE][j][e]);
-            keep[j][e] = make_double2(acc[0][KEEP][j][e] - acc[2][KEEP][j][e], acc[0][KEEP][j][e] + acc[1][KEEP][j][e]);
+            if (PHASED) {
+                xw[j * 64 + L.sw[e]] = make_double2(acc[0][GIVE][j][e], acc[1][GIVE][j][e]);
+                keep[j][e] = make_double2(acc[0][KEEP][j][e], acc[1][KEEP][j][e]);
+            } else {
+                xw[j * 64 + L.sw[e]] = make_double2(acc[0][GIVE][j][e] - acc[2][GIVE][j][e], acc[0][GIVE][j][e] + acc[1][GIVE][j][e]);
+                keep[j][e] = make_double2(acc[0][KEEP][j][e] - acc[2][KEEP][j][e], acc[0][KEEP][j][e] + acc[1][KEEP][j][e]);
+            }
         }
     x3_bar_arrive(h, buf);
 #pragma unroll
@@ -719,17 +725,16 @@ __global__ void __launch_bounds__(64) __maxnreg__(MAXREG) exchange3m_reg_kernel(
     double2 fa[ASYNC ? 1 : DA][3];
     const double2* pa = stream_ptr(cur, 0);
     double2* ar = aring + h * (MST * 32) + lane;
-    if (ASYNC) {
+    if (ASYNC) {      // the first task, in the group order of task_async: A_0 .. A_{KSF-1}, B_0 .. B_{KSF-1}, tail
 #pragma unroll
-        for (int ks = 0; ks < KSPT; ++ks) {
-            if (ks < KSF) {
+        for (int ks = 0; ks < KSF; ++ks) { cp_async16(ar + (3 * ks) * 32, pa + (3 * ks) * 32); cp_async_commit(); }
 #pragma unroll
-                for (int p = 0; p < 3; ++p) cp_async16(ar + (3 * ks + p) * 32, pa + (3 * ks + p) * 32);
-            } else {
-                cp_async16(ar + (3 * KSF) * 32, pa + (3 * KSF) * 32);
-            }
+        for (int ks = 0; ks < KSF; ++ks) {
+            cp_async16(ar + (3 * ks + 1) * 32, pa + (3 * ks + 1) * 32);
+            cp_async16(ar + (3 * ks + 2) * 32, pa + (3 * ks + 2) * 32);
             cp_async_commit();
         }
+        if (TAIL) { cp_async16(ar + (3 * KSF) * 32, pa + (3 * KSF) * 32); cp_async_commit(); }
     } else {
 #pragma unroll
         for (int q = 0; q < DA; ++q) {
@@ -785,14 +790,17 @@ __global__ void __launch_bounds__(64) __maxnreg__(MAXREG) exchange3m_reg_kernel(
                         const int r = 4 * ks + kk;
                         double2 v = make_double2(0.0, 0.0);
                         if (ok && r < d.m) v = src[r];
-                        B[3 * ks][j] = v.x; B[3 * ks + 1][j] = v.y - v.x; B[3 * ks + 2][j] = v.x + v.y;
+                        // ASYNC (phased accumulation, see task_async): the third side is negated, so that its product is
+                        // SUBTRACTED from the accumulator that already holds P0: Re = P0 - P2 without an addition
+                        B[3 * ks][j] = v.x; B[3 * ks + 1][j] = v.y - v.x; B[3 * ks + 2][j] = ASYNC ? -(v.x + v.y) : v.x + v.y;
                     }
                     if (TAIL) {       // real embedding: lanes kk = 2t (times Ar) and 2t+1 (times Ai)
                         const int r = 4 * KSF + (kk >> 1);
                         double2 v = make_double2(0.0, 0.0);
                         if (ok && r < d.m) v = src[r];
-                        B[3 * KSF][j] = (kk & 1) ? -v.y : v.x;                               // -> P0:  Ar Br - Ai Bi
-                        B[3 * KSF + (TAIL ? 1 : 0)][j] = (kk & 1) ? v.x + v.y : v.y - v.x;     // -> P1:  Ar (Bi-Br) + Ai (Br+Bi)
+                        B[3 * KSF][j] = (kk & 1) ? -v.y : v.x;                               // -> P0 / Re:  Ar Br - Ai Bi
+                        if (ASYNC) B[3 * KSF + (TAIL ? 1 : 0)][j] = (kk & 1) ? v.x : v.y;      // -> Im:  Ar Bi + Ai Br
+                        else B[3 * KSF + (TAIL ? 1 : 0)][j] = (kk & 1) ? v.x + v.y : v.y - v.x;     // -> P1:  Ar (Bi-Br) + Ai (Br+Bi)
                     }
                 }
             }
@@ -853,38 +861,60 @@ __global__ void __launch_bounds__(64) __maxnreg__(MAXREG) exchange3m_reg_kernel(
             // previous task is collected first, this task's tile is published without waiting
             auto task_async = [&](const double2* pn, const bool have_prev) {
                 if (have_prev) x3_collect<NP>(keep, xbuf + (((h ^ 1) * NBUF + (buf ^ 1)) * NP) * 64, h, buf ^ 1, L, er, ei);
+                // PHASED accumulation: Re = P0 - P2 and Im = P0 + P1 come out of the accumulators themselves.  Phase A runs the
+                // P0 micro-steps of every k-step into acc[0]; acc[1] starts as a copy of it (register moves, not FP64
+                // instructions); phase B subtracts P2 from acc[0] (negated B side) and adds P1 to acc[1], and the real-embedded
+                // tail adds its Re and Im parts directly.  The 16 DADDs per task of the combination are gone (they cost the FP64
+                // pipe 7-8 cycles each among DMMAs, profiles/r02c).  Commit groups follow the order of use: A_ks = the (Re+Im)
+                // micro-load of k-step ks, then B_ks = its Re and Im micro-loads, then the tail: NGRP groups per task.
+                constexpr int NGRP = 2 * KSF + TAIL;
 #pragma unroll
-                for (int ks = 0; ks < KSPT; ++ks) {
-                    cp_async_wait<KSPT - 1>();                          // the commit group of this k-step has landed
-                    if (ks < KSF) {
-                        double2 f[3];
+                for (int ks = 0; ks < KSF; ++ks) {
+                    cp_async_wait<NGRP - 1>();                          // group A_ks of this task has landed
+                    const double2 f = ar[(3 * ks) * 32];
 #pragma unroll
-                        for (int p = 0; p < 3; ++p) f[p] = ar[(3 * ks + p) * 32];
-#pragma unroll
-                        for (int p = 0; p < 3; ++p)
-#pragma unroll
-                            for (int j = 0; j < NP; ++j) {
-                                dmma884(acc[p][0][j][0], acc[p][0][j][1], f[p].x, B[3 * ks + p][j]);
-                                dmma884(acc[p][1][j][0], acc[p][1][j][1], f[p].y, B[3 * ks + p][j]);
-                            }
-#pragma unroll
-                        for (int p = 0; p < 3; ++p) cp_async16(ar + (3 * ks + p) * 32, pn + (3 * ks + p) * 32);
-                    } else {                                             // tail k-step
-                        const double2 f = ar[(3 * KSF) * 32];
-#pragma unroll
-                        for (int p = 0; p < 2; ++p)
-#pragma unroll
-                            for (int j = 0; j < NP; ++j) {
-                                dmma884(acc[p][0][j][0], acc[p][0][j][1], f.x, B[3 * KSF + (TAIL ? p : 0)][j]);
-                                dmma884(acc[p][1][j][0], acc[p][1][j][1], f.y, B[3 * KSF + (TAIL ? p : 0)][j]);
-                            }
-                        cp_async16(ar + (3 * KSF) * 32, pn + (3 * KSF) * 32);
+                    for (int j = 0; j < NP; ++j) {
+                        dmma884(acc[0][0][j][0], acc[0][0][j][1], f.x, B[3 * ks][j]);
+                        dmma884(acc[0][1][j][0], acc[0][1][j][1], f.y, B[3 * ks][j]);
                     }
+                    cp_async16(ar + (3 * ks) * 32, pn + (3 * ks) * 32);
+                    cp_async_commit();
+                }
+#pragma unroll
+                for (int i = 0; i < 2; ++i)
+#pragma unroll
+                    for (int j = 0; j < NP; ++j) { acc[1][i][j][0] = acc[0][i][j][0]; acc[1][i][j][1] = acc[0][i][j][1]; }
+#pragma unroll
+                for (int ks = 0; ks < KSF; ++ks) {
+                    cp_async_wait<NGRP - 1>();                          // group B_ks
+                    const double2 f1 = ar[(3 * ks + 1) * 32], f2 = ar[(3 * ks + 2) * 32];
+#pragma unroll
+                    for (int j = 0; j < NP; ++j) {
+                        dmma884(acc[1][0][j][0], acc[1][0][j][1], f1.x, B[3 * ks + 1][j]);      // Im += Ar (Bi - Br)
+                        dmma884(acc[1][1][j][0], acc[1][1][j][1], f1.y, B[3 * ks + 1][j]);
+                        dmma884(acc[0][0][j][0], acc[0][0][j][1], f2.x, B[3 * ks + 2][j]);      // Re -= Ai (Br + Bi)
+                        dmma884(acc[0][1][j][0], acc[0][1][j][1], f2.y, B[3 * ks + 2][j]);
+                    }
+                    cp_async16(ar + (3 * ks + 1) * 32, pn + (3 * ks + 1) * 32);
+                    cp_async16(ar + (3 * ks + 2) * 32, pn + (3 * ks + 2) * 32);
+                    cp_async_commit();
+                }
+                if (TAIL) {
+                    cp_async_wait<NGRP - 1>();
+                    const double2 f = ar[(3 * KSF) * 32];
+#pragma unroll
+                    for (int p = 0; p < 2; ++p)
+#pragma unroll
+                        for (int j = 0; j < NP; ++j) {
+                            dmma884(acc[p][0][j][0], acc[p][0][j][1], f.x, B[3 * KSF + (TAIL ? p : 0)][j]);
+                            dmma884(acc[p][1][j][0], acc[p][1][j][1], f.y, B[3 * KSF + (TAIL ? p : 0)][j]);
+                        }
+                    cp_async16(ar + (3 * KSF) * 32, pn + (3 * KSF) * 32);
                     cp_async_commit();
                 }
                 double2* xw = xbuf + ((h * NBUF + buf) * NP) * 64;
-                if (h == 0) x3_publish<NP, 0>(acc, keep, xw, h, buf, L);
-                else x3_publish<NP, 1>(acc, keep, xw, h, buf, L);
+                if (h == 0) x3_publish<NP, 0, true>(acc, keep, xw, h, buf, L);
+                else x3_publish<NP, 1, true>(acc, keep, xw, h, buf, L);
                 buf ^= 1;
             };
             for (int tq = 0; tq < GQ; ++tq) {
