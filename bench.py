@@ -31,10 +31,10 @@ METRIC = "walker-steps/s incl. local energy"
 UNIT = "walker-steps/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE exchange-kernel launch: bench.py cannot measure DRAM traffic itself, so
-# it reads the committed ncu capture of the default exchange kernel (a text file; profiles/r02i_summary.md names the command;
+# it reads the committed ncu capture of the default exchange kernel (a text file; profiles/r02l_summary.md names the command;
 # the `--set full` capture of the same kernel one commit earlier is profiles/r02c_ncu_exchange.md).  Only the configuration
 # that was captured has a value.
-EXCHANGE_DRAM_CAPTURES = {"C3": "profiles/r02i_exchange_dram.csv"}
+EXCHANGE_DRAM_CAPTURES = {"C3": "profiles/r02l_exchange_dram.csv"}
 
 
 def exchange_dram_traffic(config_name):
@@ -53,7 +53,7 @@ def exchange_dram_traffic(config_name):
                     seen.add(row[12])
         if len(seen) != 2:
             return None, None
-        return total, rel + " (command: profiles/r02i_summary.md)"
+        return total, rel + " (command: profiles/r02l_summary.md)"
     except (OSError, KeyError, ValueError):
         return None, None
 
